@@ -1,0 +1,163 @@
+/* ipole.h -- C ABI of the B200-native polarized GR ray-tracing hot path (libipole_b200.so).
+ *
+ * What it computes (arXiv:2302.02733; citations are /root/reference/PAPER.md lines):
+ *   PAPER.md:35  "the code launches photons from the point of the camera and integrates a null geodesic
+ *                 equation for every single pixel ... The step size of the integration is adaptive and
+ *                 parameterized ... Once the geodesic integration is over and saved the covariant fully
+ *                 polarized radiative-transfer equations are integrated along the geodesic toward the
+ *                 observer ... [at] every single step ... evaluate emission, self-absorption and Faraday
+ *                 coefficients" (Section 2.1)
+ *   PAPER.md:37  "the polarization state of light is described in a coordinate frame using a coherency
+ *                 matrix N^{alpha beta}" (Section 2.1)
+ *   PAPER.md:33  parameters: spin, viewing angle, frequency, field of view, resolution (Section 2.1)
+ *   PAPER.md:56  output: Stokes I,Q,U,V images (Table 1 caption)
+ * The paper prints no equations; the readings taken are DESIGN.md section 3 (R-1 ... R-9).
+ *
+ * Conventions
+ *   - every function returns 0 on success or a negative IPOLE_E* code; nothing is written on error.
+ *   - no global state; one ipole_ctx is not thread-safe, distinct contexts are independent.
+ *   - pointers marked "host or device" are classified with cudaPointerGetAttributes; device outputs stay
+ *     on the device (no hidden D2H); host outputs are copied back and the call synchronises the stream.
+ *   - the caller owns every buffer it passes; the library copies what it needs to keep (grid fields).
+ *   - all work is enqueued on the context's CUDA stream (ipole_set_stream; default: the legacy stream).
+ *   - there is NO CPU fallback: without a CUDA device ipole_init returns IPOLE_ECUDA.
+ */
+#ifndef IPOLE_H
+#define IPOLE_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define IPOLE_OK        0
+#define IPOLE_EINVAL   -1   /* NULL pointer or parameter out of range                                  */
+#define IPOLE_ENOMODEL -2   /* ipole_make_image before any ipole_load_model_*                          */
+#define IPOLE_ENOMEM   -3   /* host or device allocation failed                                        */
+#define IPOLE_ECUDA    -4   /* a CUDA call failed; ipole_last_cuda_error(ctx) has the cudaError_t      */
+#define IPOLE_ENOIMAGE -5   /* ipole_get_stats / ipole_get_ray_info before ipole_make_image            */
+
+typedef struct ipole_ctx ipole_ctx; /* opaque; owns every device buffer it allocates */
+
+/* Camera and integration parameters (PAPER.md:33 parameter list; step parameter eps PAPER.md:35, :43). */
+typedef struct {
+  double  spin;            /* a, 0 <= a < 1                                                            */
+  double  inclination_deg; /* polar angle of the camera, in (0,180)                                    */
+  double  r_cam;           /* camera radius ("distance"), GM/c^2                                       */
+  double  fov;             /* full width of the image x axis, GM/c^2; pixels are square                */
+  int32_t nx, ny;          /* pixels along x (right) and y (up, toward the spin axis)                  */
+  double  freq_hz;         /* observing frequency                                                      */
+  double  mbh_msun;        /* black-hole mass, Msun   (0 => 4.1e6); sets the length unit               */
+  double  dsource_pc;      /* source distance, parsec (0 => 8000); only used for the flux in Jy        */
+  double  eps;             /* step parameter (0 => 0.01)                                               */
+  double  r_esc;           /* escape radius (0 => r_cam)                                               */
+  double  stop_factor;     /* inner stop at stop_factor * r_horizon (0 => 1.05)                        */
+  int32_t max_steps;       /* per-ray step limit (0 => 50000)                                          */
+  double  hslope;          /* h of theta(X2) = pi X2 + (1-h)/2 sin(2 pi X2) (0 => 1)                   */
+  int32_t flat_metric;     /* test switch: mass term off (Minkowski in the same coordinates)           */
+} ipole_camera;
+
+/* Analytic ADAF-like flow (BASELINE.json configs[0]): n_e = n0 r^p_n [cm^-3], Theta_e = Th0 r^p_T,
+ * B = B0 r^p_B [G] purely toroidal; Keplerian outside the ISCO, E=1, L=0 free fall inside. */
+typedef struct { double n0, p_n, Th0, p_T, B0, p_B; } ipole_adaf_params;
+
+/* Test model: constant cgs coefficients in a slab |r cos(theta)| < H around the equatorial plane. */
+typedef struct {
+  double  H;        /* half thickness, GM/c^2 (> 0)                                                    */
+  int32_t profile;  /* 0 top hat; 1 Gaussian weight exp(-z^2 / (2 H^2)) on every coefficient           */
+  double  psi_deg;  /* field direction cos(psi) x^ + sin(psi) y^ in Cartesian Kerr-Schild axes         */
+  double  j[4];     /* jI,jQ,jU,jV  erg s^-1 cm^-3 Hz^-1 sr^-1, plasma frame, at freq_hz               */
+  double  alpha[4]; /* aI,aQ,aU,aV  cm^-1                                                              */
+  double  rho[3];   /* rQ,rU,rV     cm^-1                                                              */
+} ipole_slab_params;
+
+/* GRMHD-like snapshot on a cell-centred MKS lattice ("precomputed ... 3D arrays ... the code
+ * interpolates the plasma quantities to the point at every single step"). Cell (i,j,k) is centred at
+ * X^d = startx[d] + (idx_d + 1/2) dx[d]; plane element index (i*N2 + j)*N3 + k. */
+typedef struct {
+  int32_t N1, N2, N3;
+  double  startx[3], dx[3];
+  double  hslope;   /* must equal the camera's hslope                                                  */
+  double  gam;      /* adiabatic index of the fluid                                                    */
+  double  M_unit;   /* mass unit [g]: rho_cgs = rho * M_unit / L^3                                     */
+  double  Rlow, Rhigh; /* electron temperature prescription R = (Rhigh beta^2 + Rlow)/(1+beta^2)       */
+  double  r_out;    /* no plasma beyond this radius                                                    */
+} ipole_grid_desc;
+
+typedef struct {
+  double  flux_jy[4];      /* sum over pixels of I,Q,U,V times the pixel solid angle, in Jy            */
+  double  lp, cp;          /* sqrt(Q^2+U^2)/I and V/I of the sums                                      */
+  int64_t total_steps;     /* geodesic steps of all rays                                               */
+  int32_t max_steps_seen;  /* longest ray                                                              */
+  int32_t path_cap;        /* S_cap used for the bulk pass (from the probe pass)                       */
+  int64_t n_ring;          /* rays with >= 2 theta turning points ("photon ring", configs[4])          */
+  int64_t n_maxstep;       /* rays that ended on the step limit                                        */
+  int64_t n_long;          /* rays that overflowed S_cap and went through the long-ray pass            */
+  int32_t n_batches;       /* ray batches of the bulk pass                                             */
+  int32_t n_launches;      /* kernels launched by the last ipole_make_image                            */
+  float   ms_probe, ms_geodesic, ms_transfer, ms_total; /* CUDA-event times of the last image (0 until
+                              ipole_get_stats synchronises them)                                       */
+} ipole_stats;
+
+/* Create a context. Computes the camera tetrad on the device. IPOLE_EINVAL on bad parameters. */
+int  ipole_init(const ipole_camera* cam, ipole_ctx** out);
+/* Replace the camera of an existing context (keeps the loaded model and the device buffers). */
+int  ipole_set_camera(ipole_ctx*, const ipole_camera* cam);
+/* cuda_stream is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = legacy stream. */
+int  ipole_set_stream(ipole_ctx*, void* cuda_stream);
+/* Tunables: path_bytes = size of the geodesic path buffer in HBM (0 => 40% of free memory, at most
+ * 64 GiB); sort_rays != 0 orders rays by predicted step count, longest first (default 1). */
+int  ipole_set_options(ipole_ctx*, uint64_t path_bytes, int32_t sort_rays);
+
+int  ipole_load_model_adaf(ipole_ctx*, const ipole_adaf_params*);
+int  ipole_load_model_slab(ipole_ctx*, const ipole_slab_params*);
+/* fields[0..7] = rho,u,U1,U2,U3,B1,B2,B3, each N1*N2*N3 doubles, host or device (all eight alike). */
+int  ipole_load_model_grid(ipole_ctx*, const ipole_grid_desc*, const double* const fields[8]);
+
+/* One full-Stokes image: I,Q,U,V [ny][nx] row-major, specific intensity in erg s^-1 cm^-2 Hz^-1 sr^-1.
+ * tau (absorption optical depth) and tauF (Faraday depth, int |rho_V| dl) are optional [ny][nx] maps.
+ * All non-NULL outputs must be of one kind (all host or all device). */
+int  ipole_make_image(ipole_ctx*, double* I, double* Q, double* U, double* V, double* tau, double* tauF);
+/* Same for a list of n flat pixel indices j*nx+i (device or host int64); outputs have n entries. Used for
+ * sampled parity checks at resolutions whose full image the CPU oracle cannot afford. pixels == NULL means
+ * all nx*ny pixels in order (= ipole_make_image). nsteps/nturn optional (int32; nturn bit 7 = step limit). */
+int  ipole_make_pixels(ipole_ctx*, int64_t n, const int64_t* pixels, double* I, double* Q, double* U, double* V,
+                       double* tau, double* tauF, int32_t* nsteps, int32_t* nturn);
+/* Per-ray step count and theta-turning-point count (bit 7 set: ended on max_steps) of the last image,
+ * [ny][nx] or n entries; host or device; either may be NULL. */
+int  ipole_get_ray_info(ipole_ctx*, int32_t* nsteps, int32_t* nturn);
+/* Synchronises the stream and fills the statistics of the last image. */
+int  ipole_get_stats(ipole_ctx*, ipole_stats*);
+
+/* ---- stages, exposed so that tests can check each against the oracle on its own ---- */
+/* Camera tetrad: Xcam[4], e[a][mu] (16 doubles) to host memory. */
+int  ipole_get_camera_tetrad(ipole_ctx*, double Xcam[4], double e[16]);
+/* Trace the geodesic of pixel (i,j) on the device and return its stored path to HOST arrays:
+ * X [cap+1][4], K [cap+1][4], dl [cap]; returns the number of steps n >= 0, or a negative error code
+ * (IPOLE_EINVAL if cap is too small; *needed is always set when non-NULL). */
+int  ipole_trace_pixel(ipole_ctx*, int32_t i, int32_t j, int32_t cap, double* X, double* K, double* dl,
+                       int32_t* nturn, int32_t* status, int32_t* needed);
+/* Device evaluation of the building blocks at n points (host arrays in and out):
+ *   conn:  X[n][4] -> A-contracted connection Gamma^l_{mn} (64 doubles per point, [l][m][n])
+ *   coeff: (ne, thetae, B, cos_thetaB, nu)[n][5] -> (jI,jQ,jV,aI,aQ,aV,rQ,rV)[n][8] in cgs
+ *   stokes_step: (alpha[4], rho[3], s, S0[4], J[4])[n][16] -> S(s)[n][4] = O(s) S0 + P(s) J
+ *   bessel: z[n] -> (e^z K0, e^z K1, e^z K2)[n][3] */
+int  ipole_eval_connection(ipole_ctx*, int64_t n, const double* X, double* Gamma);
+int  ipole_eval_coefficients(ipole_ctx*, int64_t n, const double* in5, double* out8);
+int  ipole_eval_stokes_step(ipole_ctx*, int64_t n, const double* in16, double* out4);
+int  ipole_eval_bessel(ipole_ctx*, int64_t n, const double* z, double* out3);
+/* Plasma state of the loaded model at n points X[n][4] (host): out[n][12] = present, ne, thetae, B, u[4], b[4]. */
+int  ipole_eval_plasma(ipole_ctx*, int64_t n, const double* X, double* out12);
+
+/* FP64 FMA micro-benchmark (a chain-free DFMA loop on every SM) used as the measured ALU roofline
+ * denominator: returns achieved TFLOP/s in *tflops and the kernel time in *ms. */
+int  ipole_measure_fp64_peak(ipole_ctx*, double* tflops, float* ms);
+
+int  ipole_last_cuda_error(const ipole_ctx*);  /* cudaError_t of the last failed CUDA call, 0 if none */
+void ipole_free(ipole_ctx*);
+const char* ipole_strerror(int code);
+const char* ipole_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,199 @@
+// Kerr metric in modified Kerr-Schild (MKS) coordinates: closed-form g_{mu nu}, g^{mu nu}, the two non-zero
+// coordinate derivatives d_1 g, d_2 g, and the connection *already contracted* with the wave vector.
+//
+// DESIGN.md R-2 (north_star stage (1): "null geodesic in the Kerr metric (modified Kerr-Schild coordinates)";
+// PAPER.md:35).  X = (t, X1, X2, X3), r = exp(X1), theta = pi X2 + (1-h)/2 sin(2 pi X2), phi = X3.
+// Kerr-Schild: Sigma = r^2 + a^2 cos^2, f = 2 m r / Sigma (m = 0 under flat_metric), Delta = r^2 - 2 m r + a^2.
+// MKS components g_{mu nu} = J_mu J_nu g^KS_{mu nu}, J = (1, r, theta', 1).  Only 7 covariant and 6 contravariant
+// components are non-zero, and only d/dX1, d/dX2 of them, so the 40 Christoffel symbols are never formed:
+//   Gamma_{k mn} K^m K^n = K^1 (D1 K)_k + K^2 (D2 K)_k - 1/2 [k=1] K.D1.K - 1/2 [k=2] K.D2.K        (geodesic)
+//   Gamma_{l mn} K^m     = 1/2 ( K^1 D1_{ln} + K^2 D2_{ln} + [n=1](D1 K)_l + [n=2](D2 K)_l
+//                                - [l=1](D1 K)_n - [l=2](D2 K)_n )                                  (transport)
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+namespace ipole {
+
+struct Geom {
+  double a;        // spin
+  double hslope;   // h
+  double mass;     // 1, or 0 under flat_metric
+  int    h_is_one; // theta = pi X2 exactly
+};
+
+// sparse symmetric 4x4 with the Kerr-Schild pattern: 00 01 03 11 13 22 33
+struct Sym7 {
+  double c00, c01, c03, c11, c13, c22, c33;
+  __device__ __forceinline__ void mul(const double v[4], double o[4]) const {
+    o[0] = c00 * v[0] + c01 * v[1] + c03 * v[3];
+    o[1] = c01 * v[0] + c11 * v[1] + c13 * v[3];
+    o[2] = c22 * v[2];
+    o[3] = c03 * v[0] + c13 * v[1] + c33 * v[3];
+  }
+};
+// inverse metric pattern: 00 01 11 13 22 33 (g^{t phi} = 0 in Kerr-Schild)
+struct Inv6 {
+  double c00, c01, c11, c13, c22, c33;
+  __device__ __forceinline__ void mul(const double v[4], double o[4]) const {
+    o[0] = c00 * v[0] + c01 * v[1];
+    o[1] = c01 * v[0] + c11 * v[1] + c13 * v[3];
+    o[2] = c22 * v[2];
+    o[3] = c13 * v[1] + c33 * v[3];
+  }
+};
+
+struct Point {      // scalar functions of position shared by everything evaluated at X
+  double r, th, tp, tpp, s, c, Sig, f, sqrtmg;
+};
+
+__device__ __forceinline__ void theta_map(const Geom& G, double x2, double& th, double& tp, double& tpp) {
+  if (G.h_is_one) {
+    th = M_PI * x2; tp = M_PI; tpp = 0.0;
+  } else {
+    double s2, c2;
+    sincos(2.0 * M_PI * x2, &s2, &c2);
+    const double q = 1.0 - G.hslope;
+    th = M_PI * x2 + 0.5 * q * s2;
+    tp = M_PI * (1.0 + q * c2);
+    tpp = -2.0 * M_PI * M_PI * q * s2;
+  }
+}
+
+// g_{mu nu} and g^{mu nu} at X (no derivatives)
+template <bool WANT_INV>
+__device__ __forceinline__ void metric(const Geom& G, const double X[4], Point& p, Sym7& g, Inv6& gi) {
+  const double a = G.a;
+  p.r = exp(X[1]);
+  theta_map(G, X[2], p.th, p.tp, p.tpp);
+  sincos(p.th, &p.s, &p.c);
+  const double r = p.r, s2 = p.s * p.s;
+  p.Sig = r * r + a * a * p.c * p.c;
+  p.f = 2.0 * G.mass * r / p.Sig;
+  const double f = p.f, opf = 1.0 + f;
+  g.c00 = -1.0 + f;
+  g.c01 = f * r;
+  g.c03 = -a * f * s2;
+  g.c11 = opf * r * r;
+  g.c13 = -a * s2 * opf * r;
+  g.c22 = p.Sig * p.tp * p.tp;
+  g.c33 = s2 * (p.Sig + a * a * s2 * opf);
+  p.sqrtmg = r * p.tp * p.Sig * fabs(p.s);
+  if (WANT_INV) {
+    const double iS = 1.0 / p.Sig, ir = 1.0 / r;
+    const double Del = r * r - 2.0 * G.mass * r + a * a;
+    gi.c00 = -opf;
+    gi.c01 = f * ir;
+    gi.c11 = Del * iS * ir * ir;
+    gi.c13 = a * iS * ir;
+    gi.c22 = iS / (p.tp * p.tp);
+    gi.c33 = iS / s2;
+  }
+}
+
+// metric, inverse and the derivative matrices D1 = d g / d X1, D2 = d g / d X2
+__device__ __forceinline__ void metric_derivs(const Geom& G, const double X[4], Point& p, Sym7& g, Inv6& gi,
+                                              Sym7& D1, Sym7& D2) {
+  metric<true>(G, X, p, g, gi);
+  const double a = G.a, r = p.r, s2 = p.s * p.s, f = p.f, opf = 1.0 + f;
+  const double a2 = a * a;
+  const double iS2 = 1.0 / (p.Sig * p.Sig);
+  const double fr1 = r * 2.0 * G.mass * (a2 * p.c * p.c - r * r) * iS2;  // r df/dr
+  const double cs2 = 2.0 * p.s * p.c * p.tp;                             // theta' d(sin^2)/dtheta
+  const double ft2 = 2.0 * G.mass * r * a2 * cs2 * iS2;                  // theta' df/dtheta
+  const double St2 = -a2 * cs2;                                          // theta' dSigma/dtheta
+  D1.c00 = fr1;
+  D1.c01 = r * (f + fr1);
+  D1.c03 = -a * s2 * fr1;
+  D1.c11 = r * r * (2.0 * opf + fr1);
+  D1.c13 = -a * s2 * r * (opf + fr1);
+  D1.c22 = 2.0 * r * r * p.tp * p.tp;
+  D1.c33 = s2 * (2.0 * r * r + a2 * s2 * fr1);
+  const double e = cs2 * opf + s2 * ft2;  // theta' d/dtheta [ s^2 (1+f) ]
+  D2.c00 = ft2;
+  D2.c01 = r * ft2;
+  D2.c03 = -a * (ft2 * s2 + f * cs2);
+  D2.c11 = r * r * ft2;
+  D2.c13 = -a * r * e;
+  D2.c22 = 2.0 * p.tpp * p.tp * p.Sig + p.tp * p.tp * St2;
+  D2.c33 = cs2 * (p.Sig + a2 * s2 * opf) + s2 * (St2 + a2 * e);
+}
+
+// dK^l / dlambda = - Gamma^l_{mn} K^m K^n
+__device__ __forceinline__ void geodesic_accel(const Geom& G, const double X[4], const double K[4], double dK[4]) {
+  Point p; Sym7 g, D1, D2; Inv6 gi;
+  metric_derivs(G, X, p, g, gi, D1, D2);
+  double v1[4], v2[4], F[4];
+  D1.mul(K, v1);
+  D2.mul(K, v2);
+  const double s1 = K[0] * v1[0] + K[1] * v1[1] + K[2] * v1[2] + K[3] * v1[3];
+  const double s2 = K[0] * v2[0] + K[1] * v2[1] + K[2] * v2[2] + K[3] * v2[3];
+  F[0] = K[1] * v1[0] + K[2] * v2[0];
+  F[1] = K[1] * v1[1] + K[2] * v2[1] - 0.5 * s1;
+  F[2] = K[1] * v1[2] + K[2] * v2[2] - 0.5 * s2;
+  F[3] = K[1] * v1[3] + K[2] * v2[3];
+  gi.mul(F, dK);
+  dK[0] = -dK[0]; dK[1] = -dK[1]; dK[2] = -dK[2]; dK[3] = -dK[3];
+}
+
+// A^a_n = Gamma^a_{mn} K^m as a dense 4x4 (row a, column n); also returns the metric at X for the caller
+__device__ __forceinline__ void transport_generator(const Geom& G, const double X[4], const double K[4], Point& p,
+                                                    Sym7& g, Inv6& gi, double A[4][4]) {
+  Sym7 D1, D2;
+  metric_derivs(G, X, p, g, gi, D1, D2);
+  double v1[4], v2[4];
+  D1.mul(K, v1);
+  D2.mul(K, v2);
+  const double k1 = K[1], k2 = K[2];
+  double L[4][4];  // L_{l n} = Gamma_{l m n} K^m
+  L[0][0] = 0.5 * (k1 * D1.c00 + k2 * D2.c00);
+  L[0][1] = 0.5 * (k1 * D1.c01 + k2 * D2.c01 + v1[0]);
+  L[0][2] = 0.5 * (v2[0]);
+  L[0][3] = 0.5 * (k1 * D1.c03 + k2 * D2.c03);
+  L[1][0] = 0.5 * (k1 * D1.c01 + k2 * D2.c01 - v1[0]);
+  L[1][1] = 0.5 * (k1 * D1.c11 + k2 * D2.c11);                // + v1[1] - v1[1]
+  L[1][2] = 0.5 * (v2[1] - v1[2]);
+  L[1][3] = 0.5 * (k1 * D1.c13 + k2 * D2.c13 - v1[3]);
+  L[2][0] = 0.5 * (-v2[0]);
+  L[2][1] = 0.5 * (v1[2] - v2[1]);
+  L[2][2] = 0.5 * (k1 * D1.c22 + k2 * D2.c22);                // + v2[2] - v2[2]
+  L[2][3] = 0.5 * (-v2[3]);
+  L[3][0] = 0.5 * (k1 * D1.c03 + k2 * D2.c03);
+  L[3][1] = 0.5 * (k1 * D1.c13 + k2 * D2.c13 + v1[3]);
+  L[3][2] = 0.5 * (v2[3]);
+  L[3][3] = 0.5 * (k1 * D1.c33 + k2 * D2.c33);
+#pragma unroll
+  for (int n = 0; n < 4; ++n) {
+    A[0][n] = gi.c00 * L[0][n] + gi.c01 * L[1][n];
+    A[1][n] = gi.c01 * L[0][n] + gi.c11 * L[1][n] + gi.c13 * L[3][n];
+    A[2][n] = gi.c22 * L[2][n];
+    A[3][n] = gi.c13 * L[1][n] + gi.c33 * L[3][n];
+  }
+}
+
+// f <- (1 - h A + h^2 A^2 / 2) f
+__device__ __forceinline__ void transport_apply(const double A[4][4], double h, double f[4]) {
+  double w[4], w2[4];
+#pragma unroll
+  for (int a = 0; a < 4; ++a) w[a] = A[a][0] * f[0] + A[a][1] * f[1] + A[a][2] * f[2] + A[a][3] * f[3];
+#pragma unroll
+  for (int a = 0; a < 4; ++a) w2[a] = A[a][0] * w[0] + A[a][1] * w[1] + A[a][2] * w[2] + A[a][3] * w[3];
+  const double hh = 0.5 * h * h;
+#pragma unroll
+  for (int a = 0; a < 4; ++a) f[a] = f[a] - h * w[a] + hh * w2[a];
+}
+
+__device__ __forceinline__ double dot4(const double u[4], const double v[4]) {
+  return u[0] * v[0] + u[1] * v[1] + u[2] * v[2] + u[3] * v[3];
+}
+
+__device__ __forceinline__ double horizon_radius(double a) { return 1.0 + sqrt(1.0 - a * a); }
+
+// Bardeen, Press & Teukolsky (1972) prograde ISCO
+__device__ __host__ inline double isco_radius(double a) {
+  const double z1 = 1.0 + cbrt(1.0 - a * a) * (cbrt(1.0 + a) + cbrt(1.0 - a));
+  const double z2 = sqrt(3.0 * a * a + z1 * z1);
+  return 3.0 + z2 - sqrt((3.0 - z1) * (3.0 + z1 + 2.0 * z2));
+}
+
+}  // namespace ipole

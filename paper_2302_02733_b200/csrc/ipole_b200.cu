@@ -1,0 +1,697 @@
+// libipole_b200.so -- host side of the C ABI declared in include/ipole.h: context, argument checks, buffer
+// management, batching of rays through the geodesic path buffer, kernel launches.  All arithmetic of the hot path
+// is in the kernels (kernels.cuh); the host only sizes, schedules and copies.
+#include "../../include/ipole.h"
+#include <cuda_runtime.h>
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+#include "kernels.cuh"
+
+using namespace ipole;
+
+namespace {
+
+constexpr int N_QUEUES = 8192;
+constexpr int PROBE_TARGET = 4096;   // rays of the probe pass
+constexpr int PROBE_EPS_FACTOR = 4;  // the probe integrates with 4 eps and predicts 4x its step count
+
+enum LaunchKind { LK_PROBE = 0, LK_GEO = 1, LK_RT = 2, LK_OTHER = 3 };
+
+struct TimedSpan { cudaEvent_t a, b; int kind; };
+
+}  // namespace
+
+struct ipole_ctx {
+  ipole_camera cam_in;
+  CamDev cam;          // host copy of the device camera (after k_camera_setup)
+  CamDev* d_cam = nullptr;
+  Units units;
+  cudaStream_t stream = nullptr;
+  int last_cuda = 0;
+  int device = 0, n_sm = 0;
+
+  int model = MODEL_NONE;
+  void* d_model = nullptr;       // AdafParams / SlabParams / GridParams
+  double* d_grid = nullptr;      // 8 planes
+  size_t grid_cells = 0;
+
+  uint64_t opt_path_bytes = 0;
+  int opt_sort = 1;
+
+  double* d_path = nullptr; size_t path_bytes = 0;
+  int64_t ray_cap = 0;           // capacity of the per-ray buffers below
+  int32_t *d_nsteps = nullptr, *d_nturn = nullptr, *d_order = nullptr, *d_key = nullptr, *d_long = nullptr;
+  double* d_out = nullptr;       // staging for host outputs: 6 planes of ray_cap
+  int64_t* d_pixels = nullptr; int64_t pixels_cap = 0;
+  int32_t* d_probe = nullptr; int64_t probe_cap = 0;
+  unsigned long long* d_queues = nullptr;
+  unsigned int* d_hist = nullptr;
+  int* d_small = nullptr;        // [0] long_count, [1] probe max
+  ReducePartial* d_part = nullptr;
+  ReduceOut* d_red = nullptr;
+
+  std::vector<TimedSpan> spans; size_t spans_used = 0;
+  bool have_image = false;
+  int64_t last_n = 0;
+  ipole_stats stats;
+  int occ_geo = 0, occ_rt[4] = {0, 0, 0, 0};
+};
+
+namespace {
+
+#define CK(call)                                                        \
+  do {                                                                  \
+    cudaError_t e_ = (call);                                            \
+    if (e_ != cudaSuccess) { c->last_cuda = (int)e_; return IPOLE_ECUDA; } \
+  } while (0)
+
+bool is_device_ptr(const void* p) {
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+int check_camera(const ipole_camera* k) {
+  if (!(k->spin >= 0.0 && k->spin < 1.0)) return IPOLE_EINVAL;
+  if (!(k->inclination_deg > 0.0 && k->inclination_deg < 180.0)) return IPOLE_EINVAL;
+  if (!(k->r_cam > 0.0) || !(k->fov > 0.0) || k->nx <= 0 || k->ny <= 0 || !(k->freq_hz > 0.0)) return IPOLE_EINVAL;
+  if (k->eps < 0.0 || k->r_esc < 0.0 || k->stop_factor < 0.0 || k->max_steps < 0 || k->hslope < 0.0) return IPOLE_EINVAL;
+  if (k->mbh_msun < 0.0 || k->dsource_pc < 0.0) return IPOLE_EINVAL;
+  if ((int64_t)k->nx * k->ny > 2147483647LL) return IPOLE_EINVAL;
+  return IPOLE_OK;
+}
+
+int apply_camera(ipole_ctx* c, const ipole_camera* k) {
+  CamDev C;
+  std::memset(&C, 0, sizeof C);
+  C.G.a = k->spin;
+  C.G.hslope = k->hslope > 0.0 ? k->hslope : 1.0;
+  C.G.mass = k->flat_metric ? 0.0 : 1.0;
+  C.G.h_is_one = (C.G.hslope == 1.0);
+  C.r_cam = k->r_cam;
+  C.nx = k->nx; C.ny = k->ny;
+  C.pix = k->fov / k->nx;
+  C.eps = k->eps > 0.0 ? k->eps : 0.01;
+  C.max_steps = k->max_steps > 0 ? k->max_steps : 50000;
+  CameraSetupArgs a;
+  a.inclination_deg = k->inclination_deg;
+  a.r_esc = k->r_esc > 0.0 ? k->r_esc : k->r_cam;
+  const double stop = k->stop_factor > 0.0 ? k->stop_factor : 1.05;
+  a.r_in = k->flat_metric ? 1e-3 : stop * (1.0 + std::sqrt(1.0 - k->spin * k->spin));
+  CK(cudaMemcpyAsync(c->d_cam, &C, sizeof C, cudaMemcpyHostToDevice, c->stream));
+  k_camera_setup<<<1, 32, 0, c->stream>>>(c->d_cam, a);
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(&c->cam, c->d_cam, sizeof C, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  c->cam_in = *k;
+  const double M = (k->mbh_msun > 0.0 ? k->mbh_msun : 4.1e6) * IP_MSUN;
+  c->units.nu_obs = k->freq_hz;
+  c->units.L_unit = IP_GNEWT * M / (IP_CL * IP_CL);
+  c->units.D_cm = (k->dsource_pc > 0.0 ? k->dsource_pc : 8000.0) * IP_PC;
+  c->have_image = false;
+  return IPOLE_OK;
+}
+
+int ensure_rays(ipole_ctx* c, int64_t n) {
+  if (n <= c->ray_cap) return IPOLE_OK;
+  cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long); cudaFree(c->d_out);
+  c->d_nsteps = c->d_nturn = c->d_order = c->d_key = c->d_long = nullptr; c->d_out = nullptr; c->ray_cap = 0;
+  CK(cudaMalloc(&c->d_nsteps, n * sizeof(int32_t)));
+  CK(cudaMalloc(&c->d_nturn, n * sizeof(int32_t)));
+  CK(cudaMalloc(&c->d_order, n * sizeof(int32_t)));
+  CK(cudaMalloc(&c->d_key, n * sizeof(int32_t)));
+  CK(cudaMalloc(&c->d_long, n * sizeof(int32_t)));
+  CK(cudaMalloc(&c->d_out, 6 * n * sizeof(double)));
+  c->ray_cap = n;
+  return IPOLE_OK;
+}
+
+int ensure_path(ipole_ctx* c, size_t bytes) {
+  if (bytes <= c->path_bytes) return IPOLE_OK;
+  cudaFree(c->d_path); c->d_path = nullptr; c->path_bytes = 0;
+  cudaError_t e = cudaMalloc(&c->d_path, bytes);
+  if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
+  c->path_bytes = bytes;
+  return IPOLE_OK;
+}
+
+size_t path_budget(ipole_ctx* c) {
+  if (c->opt_path_bytes) return (size_t)c->opt_path_bytes;
+  size_t fr = 0, tot = 0;
+  cudaMemGetInfo(&fr, &tot);
+  fr += c->path_bytes;  // what we already hold counts as available
+  size_t b = (size_t)(0.4 * (double)fr);
+  const size_t cap = (size_t)64 << 30;
+  return std::min(b, cap);
+}
+
+int span_begin(ipole_ctx* c, int kind) {
+  if (c->spans_used == c->spans.size()) {
+    TimedSpan s; s.kind = kind;
+    if (cudaEventCreate(&s.a) != cudaSuccess || cudaEventCreate(&s.b) != cudaSuccess) return -1;
+    c->spans.push_back(s);
+  }
+  TimedSpan* s = &c->spans[c->spans_used++];
+  s->kind = kind;
+  cudaEventRecord(s->a, c->stream);
+  return (int)(c->spans_used - 1);
+}
+void span_end(ipole_ctx* c, int s) { if (s >= 0) cudaEventRecord(c->spans[s].b, c->stream); }
+
+int grid_for(ipole_ctx* c, int occ, int threads, int64_t rays) {
+  const int64_t full = (int64_t)c->n_sm * std::max(occ, 1);
+  const int64_t need = (rays + threads - 1) / threads;
+  return (int)std::max<int64_t>(1, std::min(full, need));
+}
+
+int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays) {
+  const int s = span_begin(c, kind);
+  k_geodesic<<<grid_for(c, c->occ_geo, IPOLE_GEO_THREADS, rays), IPOLE_GEO_THREADS, 0, c->stream>>>(a);
+  span_end(c, s);
+  c->stats.n_launches++;
+  CK(cudaGetLastError());
+  return IPOLE_OK;
+}
+
+int launch_transfer(ipole_ctx* c, RtArgs& a, int64_t rays) {
+  const int s = span_begin(c, LK_RT);
+  const int g = grid_for(c, c->occ_rt[c->model], IPOLE_RT_THREADS, rays);
+  if (c->model == MODEL_ADAF) k_transfer<MODEL_ADAF><<<g, IPOLE_RT_THREADS, 0, c->stream>>>(a);
+  else if (c->model == MODEL_SLAB) k_transfer<MODEL_SLAB><<<g, IPOLE_RT_THREADS, 0, c->stream>>>(a);
+  else k_transfer<MODEL_GRID><<<g, IPOLE_RT_THREADS, 0, c->stream>>>(a);
+  span_end(c, s);
+  c->stats.n_launches++;
+  CK(cudaGetLastError());
+  return IPOLE_OK;
+}
+
+GeoArgs geo_args(ipole_ctx* c) {
+  GeoArgs g;
+  std::memset(&g, 0, sizeof g);
+  g.cam = c->cam;
+  g.eps = c->cam.eps;
+  g.max_steps = c->cam.max_steps;
+  g.list_stride = 1;
+  return g;
+}
+
+// the whole pipeline for n rays; outputs are DEVICE pointers indexed by ray
+int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double* Q, double* U, double* V, double* tau,
+             double* tauF) {
+  int rc;
+  if ((rc = ensure_rays(c, n)) != IPOLE_OK) return rc;
+  c->spans_used = 0;
+  std::memset(&c->stats, 0, sizeof c->stats);
+  c->have_image = false;
+  CK(cudaMemsetAsync(c->d_queues, 0, N_QUEUES * sizeof(unsigned long long), c->stream));
+  CK(cudaMemsetAsync(c->d_small, 0, 4 * sizeof(int), c->stream));
+  int qi = 0;
+  const int total = span_begin(c, LK_OTHER);
+
+  const size_t budget = path_budget(c);
+  const size_t rec_bytes = REC_DOUBLES * sizeof(double);
+  const int max_steps = c->cam.max_steps;
+  int cap = max_steps;
+  const int32_t* order = nullptr;
+  const bool fits_all = (double)n * (double)(max_steps + 1) * (double)rec_bytes <= (double)budget;
+  const bool probe = (n >= 32768) && (c->opt_sort || !fits_all);
+
+  if (probe) {
+    // ---- probe pass: coarse lattice (or strided list), 4 eps, no path storage ----
+    GeoArgs g = geo_args(c);
+    g.eps = c->cam.eps * PROBE_EPS_FACTOR;
+    SortArgs sa;
+    std::memset(&sa, 0, sizeof sa);
+    int64_t np;
+    if (!d_pixels) {
+      const int stride = std::max(1, (int)std::ceil(std::sqrt((double)n / PROBE_TARGET)));
+      const int lnx = std::max(1, c->cam.nx / stride), lny = std::max(1, c->cam.ny / stride);
+      np = (int64_t)lnx * lny;
+      g.lattice_stride = stride; g.lattice_nx = lnx;
+      sa.lattice_stride = stride; sa.lattice_nx = lnx; sa.lattice_ny = lny; sa.nx = c->cam.nx;
+    } else {
+      const int64_t ls = std::max<int64_t>(1, n / PROBE_TARGET);
+      np = (n + ls - 1) / ls;
+      g.pixels = d_pixels; g.list_stride = ls;
+      sa.list_stride = (int)ls;
+    }
+    if (np > c->probe_cap) {
+      cudaFree(c->d_probe); c->d_probe = nullptr; c->probe_cap = 0;
+      CK(cudaMalloc(&c->d_probe, np * sizeof(int32_t)));
+      c->probe_cap = np;
+    }
+    g.count = np; g.nsteps = c->d_probe; g.queue = c->d_queues + (qi++);
+    if ((rc = launch_geodesic(c, g, LK_PROBE, np)) != IPOLE_OK) return rc;
+    const int sp = span_begin(c, LK_PROBE);
+    k_max_i32<<<1, 1024, 0, c->stream>>>(c->d_probe, (int)np, c->d_small + 1);
+    c->stats.n_launches++;
+    int pmax = 0;
+    CK(cudaMemcpyAsync(&pmax, c->d_small + 1, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    cap = (int)std::min<int64_t>(max_steps, (int64_t)(pmax * PROBE_EPS_FACTOR * 1.15) + 64);
+    if (c->opt_sort) {
+      sa.n = n; sa.probe = c->d_probe; sa.scale = PROBE_EPS_FACTOR;
+      sa.bin_width = std::max(1, (cap + SORT_BINS - 1) / SORT_BINS);
+      sa.key = c->d_key; sa.hist = c->d_hist; sa.order = c->d_order;
+      CK(cudaMemsetAsync(c->d_hist, 0, SORT_BINS * sizeof(unsigned int), c->stream));
+      const int gb = (int)std::min<int64_t>((n + 255) / 256, 148 * 8);
+      k_predict_hist<<<gb, 256, 0, c->stream>>>(sa);
+      k_scan_bins<<<1, 1024, 0, c->stream>>>(c->d_hist);
+      k_scatter<<<gb, 256, 0, c->stream>>>(sa);
+      c->stats.n_launches += 3;
+      CK(cudaGetLastError());
+      order = c->d_order;
+    }
+    span_end(c, sp);
+  }
+  if (!probe) {
+    // everything in flight at once: give each ray what the budget allows
+    const int64_t per = (int64_t)(budget / rec_bytes / (size_t)n) - 1;
+    cap = (int)std::max<int64_t>(64, std::min<int64_t>(max_steps, per));
+  }
+  c->stats.path_cap = cap;
+
+  // ---- bulk pass in batches of B rays ----
+  const size_t slot_bytes = (size_t)(cap + 1) * rec_bytes;
+  int64_t B = std::min<int64_t>(n, (int64_t)(budget / slot_bytes));
+  if (B < 1) return IPOLE_ENOMEM;
+  if ((rc = ensure_path(c, (size_t)B * slot_bytes)) != IPOLE_OK) return rc;
+  for (int64_t base = 0; base < n; base += B) {
+    const int64_t cnt = std::min(B, n - base);
+    if (qi + 2 > N_QUEUES) return IPOLE_EINVAL;
+    GeoArgs g = geo_args(c);
+    g.cap = cap; g.base = base; g.count = cnt; g.order = order; g.pixels = d_pixels;
+    g.path = c->d_path; g.nsteps = c->d_nsteps; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
+    g.long_list = c->d_long; g.long_count = c->d_small;
+    if ((rc = launch_geodesic(c, g, LK_GEO, cnt)) != IPOLE_OK) return rc;
+    RtArgs t;
+    std::memset(&t, 0, sizeof t);
+    t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = cap; t.base = base; t.count = cnt; t.order = order;
+    t.path = c->d_path; t.nsteps = c->d_nsteps; t.queue = c->d_queues + (qi++);
+    t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
+    if ((rc = launch_transfer(c, t, cnt)) != IPOLE_OK) return rc;
+    c->stats.n_batches++;
+  }
+
+  // ---- long-ray pass: rays that overflowed their slot get one of max_steps ----
+  int n_long = 0;
+  if (cap < max_steps) {
+    CK(cudaMemcpyAsync(&n_long, c->d_small, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+  }
+  c->stats.n_long = n_long;
+  if (n_long > 0) {
+    const size_t lslot = (size_t)(max_steps + 1) * rec_bytes;
+    int64_t LB = std::min<int64_t>(n_long, (int64_t)(std::max(budget, lslot) / lslot));
+    if ((rc = ensure_path(c, (size_t)LB * lslot)) != IPOLE_OK) return rc;
+    for (int64_t base = 0; base < n_long; base += LB) {
+      const int64_t cnt = std::min<int64_t>(LB, n_long - base);
+      if (qi + 2 > N_QUEUES) return IPOLE_EINVAL;
+      GeoArgs g = geo_args(c);
+      g.cap = max_steps; g.base = base; g.count = cnt; g.order = c->d_long; g.pixels = d_pixels;
+      g.path = c->d_path; g.nsteps = c->d_nsteps; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
+      if ((rc = launch_geodesic(c, g, LK_GEO, cnt)) != IPOLE_OK) return rc;
+      RtArgs t;
+      std::memset(&t, 0, sizeof t);
+      t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = max_steps; t.base = base; t.count = cnt;
+      t.order = c->d_long; t.path = c->d_path; t.nsteps = c->d_nsteps; t.queue = c->d_queues + (qi++);
+      t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
+      if ((rc = launch_transfer(c, t, cnt)) != IPOLE_OK) return rc;
+    }
+  }
+
+  // ---- a-9: totals ----
+  {
+    const int s = span_begin(c, LK_OTHER);
+    const int nb = (int)std::min<int64_t>(REDUCE_BLOCKS, (n + 255) / 256);
+    k_reduce_partial<<<nb, 256, 0, c->stream>>>(n, I, Q, U, V, c->d_nsteps, c->d_nturn, c->d_part);
+    const double pix_rad = c->cam.pix * c->units.L_unit / c->units.D_cm;
+    k_reduce_final<<<1, 32, 0, c->stream>>>(c->d_part, nb, pix_rad * pix_rad * 1e23, c->d_red);
+    c->stats.n_launches += 2;
+    span_end(c, s);
+    CK(cudaGetLastError());
+  }
+  span_end(c, total);
+  c->have_image = true;
+  c->last_n = n;
+  return IPOLE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
+  if (!cam || !out) return IPOLE_EINVAL;
+  int rc = check_camera(cam);
+  if (rc != IPOLE_OK) return rc;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return IPOLE_ECUDA; }
+  ipole_ctx* c = new (std::nothrow) ipole_ctx();
+  if (!c) return IPOLE_ENOMEM;
+  std::memset(&c->stats, 0, sizeof c->stats);
+  auto fail = [&](int code) { ipole_free(c); return code; };
+  if (cudaGetDevice(&c->device) != cudaSuccess) return fail(IPOLE_ECUDA);
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, c->device) != cudaSuccess) return fail(IPOLE_ECUDA);
+  c->n_sm = prop.multiProcessorCount;
+  if (cudaMalloc(&c->d_cam, sizeof(CamDev)) != cudaSuccess) return fail(IPOLE_ENOMEM);
+  size_t msz = std::max(sizeof(GridParams), std::max(sizeof(AdafParams), sizeof(SlabParams)));
+  if (cudaMalloc(&c->d_model, msz) != cudaSuccess) return fail(IPOLE_ENOMEM);
+  if (cudaMalloc(&c->d_queues, N_QUEUES * sizeof(unsigned long long)) != cudaSuccess) return fail(IPOLE_ENOMEM);
+  if (cudaMalloc(&c->d_hist, SORT_BINS * sizeof(unsigned int)) != cudaSuccess) return fail(IPOLE_ENOMEM);
+  if (cudaMalloc(&c->d_small, 4 * sizeof(int)) != cudaSuccess) return fail(IPOLE_ENOMEM);
+  if (cudaMalloc(&c->d_part, REDUCE_BLOCKS * sizeof(ReducePartial)) != cudaSuccess) return fail(IPOLE_ENOMEM);
+  if (cudaMalloc(&c->d_red, sizeof(ReduceOut)) != cudaSuccess) return fail(IPOLE_ENOMEM);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo, k_geodesic, IPOLE_GEO_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_rt[MODEL_ADAF], k_transfer<MODEL_ADAF>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_rt[MODEL_SLAB], k_transfer<MODEL_SLAB>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_rt[MODEL_GRID], k_transfer<MODEL_GRID>, IPOLE_RT_THREADS, 0);
+  if (cudaGetLastError() != cudaSuccess) return fail(IPOLE_ECUDA);
+  rc = apply_camera(c, cam);
+  if (rc != IPOLE_OK) return fail(rc);
+  *out = c;
+  return IPOLE_OK;
+}
+
+int ipole_set_camera(ipole_ctx* c, const ipole_camera* cam) {
+  if (!c || !cam) return IPOLE_EINVAL;
+  int rc = check_camera(cam);
+  if (rc != IPOLE_OK) return rc;
+  const double h_new = cam->hslope > 0.0 ? cam->hslope : 1.0;
+  if (c->model == MODEL_GRID && h_new != c->cam.G.hslope) return IPOLE_EINVAL;
+  if (c->model == MODEL_ADAF && cam->flat_metric) return IPOLE_EINVAL;
+  const double a_old = c->cam.G.a;
+  rc = apply_camera(c, cam);
+  if (rc != IPOLE_OK) return rc;
+  if (c->model == MODEL_ADAF && a_old != cam->spin) {  // r_isco depends on the spin
+    AdafParams p;
+    CK(cudaMemcpy(&p, c->d_model, sizeof p, cudaMemcpyDeviceToHost));
+    p.r_isco = isco_radius(cam->spin);
+    CK(cudaMemcpy(c->d_model, &p, sizeof p, cudaMemcpyHostToDevice));
+  }
+  return IPOLE_OK;
+}
+
+int ipole_set_stream(ipole_ctx* c, void* s) {
+  if (!c) return IPOLE_EINVAL;
+  c->stream = (cudaStream_t)s;
+  return IPOLE_OK;
+}
+
+int ipole_set_options(ipole_ctx* c, uint64_t path_bytes, int32_t sort_rays) {
+  if (!c) return IPOLE_EINVAL;
+  c->opt_path_bytes = path_bytes;
+  c->opt_sort = sort_rays ? 1 : 0;
+  return IPOLE_OK;
+}
+
+int ipole_load_model_adaf(ipole_ctx* c, const ipole_adaf_params* p) {
+  if (!c || !p) return IPOLE_EINVAL;
+  if (c->cam.G.mass == 0.0) return IPOLE_EINVAL;  // the flow is defined on Kerr only
+  AdafParams m;
+  m.n0 = p->n0; m.p_n = p->p_n; m.Th0 = p->Th0; m.p_T = p->p_T; m.B0 = p->B0; m.p_B = p->p_B;
+  m.r_isco = isco_radius(c->cam.G.a);
+  CK(cudaMemcpyAsync(c->d_model, &m, sizeof m, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  c->model = MODEL_ADAF;
+  return IPOLE_OK;
+}
+
+int ipole_load_model_slab(ipole_ctx* c, const ipole_slab_params* p) {
+  if (!c || !p || !(p->H > 0.0)) return IPOLE_EINVAL;
+  SlabParams m;
+  m.H = p->H; m.profile = p->profile;
+  const double psi = p->psi_deg * M_PI / 180.0;
+  m.cpsi = std::cos(psi); m.spsi = std::sin(psi);
+  for (int i = 0; i < 4; ++i) { m.j[i] = p->j[i]; m.al[i] = p->alpha[i]; }
+  for (int i = 0; i < 3; ++i) m.rh[i] = p->rho[i];
+  CK(cudaMemcpyAsync(c->d_model, &m, sizeof m, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  c->model = MODEL_SLAB;
+  return IPOLE_OK;
+}
+
+int ipole_load_model_grid(ipole_ctx* c, const ipole_grid_desc* d, const double* const fields[8]) {
+  if (!c || !d || !fields) return IPOLE_EINVAL;
+  if (d->N1 < 1 || d->N2 < 1 || d->N3 < 1) return IPOLE_EINVAL;
+  if (d->hslope != c->cam.G.hslope) return IPOLE_EINVAL;
+  for (int q = 0; q < 8; ++q) if (!fields[q]) return IPOLE_EINVAL;
+  for (int i = 0; i < 3; ++i) if (!(d->dx[i] > 0.0)) return IPOLE_EINVAL;
+  const size_t cells = (size_t)d->N1 * d->N2 * d->N3;
+  if (cells != c->grid_cells) {
+    cudaFree(c->d_grid); c->d_grid = nullptr; c->grid_cells = 0;
+    cudaError_t e = cudaMalloc(&c->d_grid, 8 * cells * sizeof(double));
+    if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
+    c->grid_cells = cells;
+  }
+  GridParams m;
+  std::memset(&m, 0, sizeof m);
+  for (int q = 0; q < 8; ++q) {
+    CK(cudaMemcpyAsync(c->d_grid + q * cells, fields[q], cells * sizeof(double), cudaMemcpyDefault, c->stream));
+    m.f[q] = c->d_grid + q * cells;
+  }
+  m.N1 = d->N1; m.N2 = d->N2; m.N3 = d->N3;
+  for (int i = 0; i < 3; ++i) { m.startx[i] = d->startx[i]; m.idx[i] = 1.0 / d->dx[i]; }
+  m.gam = d->gam; m.Rlow = d->Rlow; m.Rhigh = d->Rhigh; m.r_out = d->r_out; m.lx_out = std::log(d->r_out);
+  const double L = c->units.L_unit;
+  const double rho_unit = d->M_unit / (L * L * L);
+  m.ne_unit = rho_unit / (IP_MP + IP_ME);
+  m.B_unit = IP_CL * std::sqrt(4.0 * M_PI * rho_unit);
+  CK(cudaMemcpyAsync(c->d_model, &m, sizeof m, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  c->model = MODEL_GRID;
+  return IPOLE_OK;
+}
+
+int ipole_make_pixels(ipole_ctx* c, int64_t n, const int64_t* pixels, double* I, double* Q, double* U, double* V,
+                      double* tau, double* tauF, int32_t* nsteps, int32_t* nturn) {
+  if (!c || !I || !Q || !U || !V) return IPOLE_EINVAL;
+  if (c->model == MODEL_NONE) return IPOLE_ENOMODEL;
+  const int64_t npix = (int64_t)c->cam.nx * c->cam.ny;
+  if (!pixels) n = npix;
+  if (n < 0 || n > 2147483647LL) return IPOLE_EINVAL;
+  if (n == 0) return IPOLE_OK;
+  const bool dev = is_device_ptr(I);
+  const void* outs[] = {Q, U, V, tau, tauF, nsteps, nturn};
+  for (const void* p : outs) if (p && is_device_ptr(p) != dev) return IPOLE_EINVAL;
+  int rc;
+  if ((rc = ensure_rays(c, n)) != IPOLE_OK) return rc;
+  const int64_t* d_pix = nullptr;
+  if (pixels) {
+    if (is_device_ptr(pixels)) d_pix = pixels;
+    else {
+      for (int64_t i = 0; i < n; ++i) if (pixels[i] < 0 || pixels[i] >= npix) return IPOLE_EINVAL;
+      if (n > c->pixels_cap) {
+        cudaFree(c->d_pixels); c->d_pixels = nullptr; c->pixels_cap = 0;
+        CK(cudaMalloc(&c->d_pixels, n * sizeof(int64_t)));
+        c->pixels_cap = n;
+      }
+      CK(cudaMemcpyAsync(c->d_pixels, pixels, n * sizeof(int64_t), cudaMemcpyHostToDevice, c->stream));
+      d_pix = c->d_pixels;
+    }
+  }
+  double* o[6];
+  if (dev) { o[0] = I; o[1] = Q; o[2] = U; o[3] = V; o[4] = tau; o[5] = tauF; }
+  else {
+    for (int k = 0; k < 6; ++k) o[k] = c->d_out + (size_t)k * c->ray_cap;
+    if (!tau) o[4] = nullptr;
+    if (!tauF) o[5] = nullptr;
+  }
+  if ((rc = run_rays(c, n, d_pix, o[0], o[1], o[2], o[3], o[4], o[5])) != IPOLE_OK) return rc;
+  if (!dev) {
+    double* h[6] = {I, Q, U, V, tau, tauF};
+    for (int k = 0; k < 6; ++k)
+      if (h[k]) CK(cudaMemcpyAsync(h[k], o[k], n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  }
+  if (nsteps) CK(cudaMemcpyAsync(nsteps, c->d_nsteps, n * sizeof(int32_t), cudaMemcpyDefault, c->stream));
+  if (nturn) CK(cudaMemcpyAsync(nturn, c->d_nturn, n * sizeof(int32_t), cudaMemcpyDefault, c->stream));
+  if (!dev) CK(cudaStreamSynchronize(c->stream));
+  return IPOLE_OK;
+}
+
+int ipole_make_image(ipole_ctx* c, double* I, double* Q, double* U, double* V, double* tau, double* tauF) {
+  return ipole_make_pixels(c, 0, nullptr, I, Q, U, V, tau, tauF, nullptr, nullptr);
+}
+
+int ipole_get_ray_info(ipole_ctx* c, int32_t* nsteps, int32_t* nturn) {
+  if (!c) return IPOLE_EINVAL;
+  if (!c->have_image) return IPOLE_ENOIMAGE;
+  if (nsteps) CK(cudaMemcpyAsync(nsteps, c->d_nsteps, c->last_n * sizeof(int32_t), cudaMemcpyDefault, c->stream));
+  if (nturn) CK(cudaMemcpyAsync(nturn, c->d_nturn, c->last_n * sizeof(int32_t), cudaMemcpyDefault, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  return IPOLE_OK;
+}
+
+int ipole_get_stats(ipole_ctx* c, ipole_stats* out) {
+  if (!c || !out) return IPOLE_EINVAL;
+  if (!c->have_image) return IPOLE_ENOIMAGE;
+  ReduceOut r;
+  CK(cudaMemcpyAsync(&r, c->d_red, sizeof r, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  ipole_stats& s = c->stats;
+  for (int k = 0; k < 4; ++k) s.flux_jy[k] = r.flux[k];
+  s.lp = r.lp; s.cp = r.cp;
+  s.total_steps = r.total_steps; s.max_steps_seen = r.max_steps; s.n_ring = r.n_ring; s.n_maxstep = r.n_maxstep;
+  s.ms_probe = s.ms_geodesic = s.ms_transfer = s.ms_total = 0.f;
+  for (size_t i = 0; i < c->spans_used; ++i) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, c->spans[i].a, c->spans[i].b) != cudaSuccess) { cudaGetLastError(); continue; }
+    if (i == 0) s.ms_total = ms;
+    else if (c->spans[i].kind == LK_PROBE) s.ms_probe += ms;
+    else if (c->spans[i].kind == LK_GEO) s.ms_geodesic += ms;
+    else if (c->spans[i].kind == LK_RT) s.ms_transfer += ms;
+  }
+  *out = s;
+  return IPOLE_OK;
+}
+
+int ipole_get_camera_tetrad(ipole_ctx* c, double Xcam[4], double e[16]) {
+  if (!c || !Xcam || !e) return IPOLE_EINVAL;
+  std::memcpy(Xcam, c->cam.Xcam, 4 * sizeof(double));
+  std::memcpy(e, c->cam.e, 16 * sizeof(double));
+  return IPOLE_OK;
+}
+
+int ipole_trace_pixel(ipole_ctx* c, int32_t i, int32_t j, int32_t cap, double* X, double* K, double* dl, int32_t* nturn,
+                      int32_t* status, int32_t* needed) {
+  if (!c || i < 0 || j < 0 || i >= c->cam.nx || j >= c->cam.ny || cap < 1) return IPOLE_EINVAL;
+  int rc;
+  if ((rc = ensure_rays(c, 1)) != IPOLE_OK) return rc;
+  const int max_steps = c->cam.max_steps;
+  const size_t bytes = (size_t)(max_steps + 1) * REC_DOUBLES * sizeof(double);
+  if ((rc = ensure_path(c, bytes)) != IPOLE_OK) return rc;
+  if (c->pixels_cap < 1) { CK(cudaMalloc(&c->d_pixels, sizeof(int64_t))); c->pixels_cap = 1; }
+  const int64_t pix = (int64_t)j * c->cam.nx + i;
+  CK(cudaMemcpyAsync(c->d_pixels, &pix, sizeof pix, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaMemsetAsync(c->d_queues, 0, sizeof(unsigned long long), c->stream));
+  GeoArgs g = geo_args(c);
+  g.cap = max_steps; g.count = 1; g.pixels = c->d_pixels; g.path = c->d_path; g.nsteps = c->d_nsteps; g.nturn = c->d_nturn;
+  g.queue = c->d_queues;
+  k_geodesic<<<1, 32, 0, c->stream>>>(g);
+  CK(cudaGetLastError());
+  int32_t n = 0, nt = 0;
+  CK(cudaMemcpyAsync(&n, c->d_nsteps, sizeof n, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaMemcpyAsync(&nt, c->d_nturn, sizeof nt, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  c->have_image = false;
+  if (needed) *needed = n;
+  if (nturn) *nturn = nt & 0x7f;
+  if (n > cap) return IPOLE_EINVAL;
+  std::vector<double> rec((size_t)(n + 1) * REC_DOUBLES);
+  CK(cudaMemcpyAsync(rec.data(), c->d_path, rec.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  for (int s = 0; s <= n; ++s) {
+    const double* r = &rec[(size_t)s * REC_DOUBLES];
+    if (X) { X[4 * s] = 0.0; X[4 * s + 1] = r[0]; X[4 * s + 2] = r[1]; X[4 * s + 3] = r[2]; }
+    if (K) { K[4 * s] = r[3]; K[4 * s + 1] = r[4]; K[4 * s + 2] = r[5]; K[4 * s + 3] = r[6]; }
+    if (dl && s < n) dl[s] = r[7];
+  }
+  if (status) {
+    const double x1 = rec[(size_t)n * REC_DOUBLES];
+    *status = (nt & 0x80) ? 3 : (x1 <= c->cam.lx_in ? 1 : 2);
+  }
+  return n;
+}
+
+}  // extern "C"
+
+namespace {
+template <typename F>
+int eval_host(ipole_ctx* c, int64_t n, const double* in, int nin, double* out, int nout, F launch) {
+  if (!c || !in || !out || n < 0) return IPOLE_EINVAL;
+  if (n == 0) return IPOLE_OK;
+  double *d_in = nullptr, *d_o = nullptr;
+  if (cudaMalloc(&d_in, n * nin * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return IPOLE_ENOMEM; }
+  if (cudaMalloc(&d_o, n * nout * sizeof(double)) != cudaSuccess) { cudaFree(d_in); cudaGetLastError(); return IPOLE_ENOMEM; }
+  cudaError_t e = cudaMemcpyAsync(d_in, in, n * nin * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+  if (e == cudaSuccess) { launch((int)((n + 127) / 128), 128, d_in, d_o); e = cudaGetLastError(); }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(out, d_o, n * nout * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  cudaFree(d_in); cudaFree(d_o);
+  if (e != cudaSuccess) { c->last_cuda = (int)e; return IPOLE_ECUDA; }
+  return IPOLE_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int ipole_eval_connection(ipole_ctx* c, int64_t n, const double* X, double* Gamma) {
+  return eval_host(c, n, X, 4, Gamma, 64, [&](int g, int b, double* i, double* o) { k_eval_connection<<<g, b, 0, c->stream>>>(c->cam.G, n, i, o); });
+}
+int ipole_eval_coefficients(ipole_ctx* c, int64_t n, const double* in5, double* out8) {
+  return eval_host(c, n, in5, 5, out8, 8, [&](int g, int b, double* i, double* o) { k_eval_coefficients<<<g, b, 0, c->stream>>>(n, i, o); });
+}
+int ipole_eval_stokes_step(ipole_ctx* c, int64_t n, const double* in16, double* out4) {
+  return eval_host(c, n, in16, 16, out4, 4, [&](int g, int b, double* i, double* o) { k_eval_stokes_step<<<g, b, 0, c->stream>>>(n, i, o); });
+}
+int ipole_eval_bessel(ipole_ctx* c, int64_t n, const double* z, double* out3) {
+  return eval_host(c, n, z, 1, out3, 3, [&](int g, int b, double* i, double* o) { k_eval_bessel<<<g, b, 0, c->stream>>>(n, i, o); });
+}
+int ipole_eval_plasma(ipole_ctx* c, int64_t n, const double* X, double* out12) {
+  if (!c) return IPOLE_EINVAL;
+  if (c->model == MODEL_NONE) return IPOLE_ENOMODEL;
+  return eval_host(c, n, X, 4, out12, 12, [&](int g, int b, double* i, double* o) {
+    if (c->model == MODEL_ADAF) k_eval_plasma<MODEL_ADAF><<<g, b, 0, c->stream>>>(c->cam.G, c->d_model, n, i, o);
+    else if (c->model == MODEL_SLAB) k_eval_plasma<MODEL_SLAB><<<g, b, 0, c->stream>>>(c->cam.G, c->d_model, n, i, o);
+    else k_eval_plasma<MODEL_GRID><<<g, b, 0, c->stream>>>(c->cam.G, c->d_model, n, i, o);
+  });
+}
+
+int ipole_measure_fp64_peak(ipole_ctx* c, double* tflops, float* ms_out) {
+  if (!c || !tflops) return IPOLE_EINVAL;
+  double* sink = nullptr;
+  CK(cudaMalloc(&sink, sizeof(double)));
+  const int blocks = c->n_sm * 8, threads = 256, iters = 1 << 16;
+  cudaEvent_t a, b;
+  CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
+  k_fp64_peak<<<blocks, threads, 0, c->stream>>>(1024, 1.0, sink);  // warm-up
+  float best = 1e30f;
+  for (int rep = 0; rep < 3; ++rep) {
+    cudaEventRecord(a, c->stream);
+    k_fp64_peak<<<blocks, threads, 0, c->stream>>>(iters, 1.0 + rep, sink);
+    cudaEventRecord(b, c->stream);
+    CK(cudaEventSynchronize(b));
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, a, b));
+    best = std::min(best, ms);
+  }
+  cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(sink);
+  CK(cudaGetLastError());
+  *tflops = 2.0 * 8.0 * (double)iters * (double)blocks * threads / (best * 1e-3) / 1e12;
+  if (ms_out) *ms_out = best;
+  return IPOLE_OK;
+}
+
+int ipole_last_cuda_error(const ipole_ctx* c) { return c ? c->last_cuda : 0; }
+
+void ipole_free(ipole_ctx* c) {
+  if (!c) return;
+  cudaFree(c->d_cam); cudaFree(c->d_model); cudaFree(c->d_grid); cudaFree(c->d_path);
+  cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long);
+  cudaFree(c->d_out); cudaFree(c->d_pixels); cudaFree(c->d_probe); cudaFree(c->d_queues); cudaFree(c->d_hist);
+  cudaFree(c->d_small); cudaFree(c->d_part); cudaFree(c->d_red);
+  for (auto& s : c->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
+  cudaGetLastError();
+  delete c;
+}
+
+const char* ipole_strerror(int code) {
+  switch (code) {
+    case IPOLE_OK: return "ok";
+    case IPOLE_EINVAL: return "invalid argument";
+    case IPOLE_ENOMODEL: return "no plasma model loaded";
+    case IPOLE_ENOMEM: return "out of memory";
+    case IPOLE_ECUDA: return "CUDA error (see ipole_last_cuda_error)";
+    case IPOLE_ENOIMAGE: return "no image has been made yet";
+    default: return "unknown error";
+  }
+}
+
+const char* ipole_version(void) { return "ipole-b200 0.1 (sm_100a, FP64)"; }
+
+}  // extern "C"

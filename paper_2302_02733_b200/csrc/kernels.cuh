@@ -1,0 +1,539 @@
+// Kernels of the hot path (SURVEY.md section 8(a) rows a-1 ... a-9), sm_100a, scalar FP64.
+//   k_camera_setup   a-1  camera tetrad by Gram-Schmidt (one thread)
+//   k_geodesic       a-1/a-2/a-3/a-8  per-lane persistent ray loop: pixel -> K, RK4 push with the fused
+//                    metric/connection, adaptive step, path records to HBM, atomic ray queue with lane-level refill
+//   k_transfer       a-4/a-5/a-6/a-7/a-8  walks the stored path toward the camera: transport, plasma model, tetrad,
+//                    coefficients, analytic 4x4 step; camera projection; writes I,Q,U,V(,tau,tauF)
+//   k_predict/k_hist/k_scan/k_scatter  a-8  counting sort of rays by predicted step count (longest first)
+//   k_reduce_partial/k_reduce_final    a-9  warp-shuffle reduction of flux, polarization fractions, step statistics
+#pragma once
+#include <stdint.h>
+#include "geom.cuh"
+#include "plasma.cuh"
+
+namespace ipole {
+
+// One path record = one point of the geodesic: X1,X2,X3, K0..K3, dl (step from this point to the next one).
+// 64 B = two 32-B sectors; the records of one ray are contiguous, so every sector written or read is full.
+constexpr int REC_DOUBLES = 8;
+
+struct CamDev {
+  Geom G;
+  double Xcam[4];
+  double e[4][4];       // e[a][mu]
+  double ecov1[4], ecov2[4];
+  double r_cam, pix;    // pix = fov/nx
+  int nx, ny;
+  double eps, lx_in, lx_esc;  // ln of the inner stop radius / escape radius
+  int max_steps;
+};
+
+struct CameraSetupArgs { double inclination_deg, r_in, r_esc; };
+
+__device__ __forceinline__ void gram_schmidt(const Sym7& g, double v[4], const double (*basis)[4], const double* sign, int nb) {
+  for (int b = 0; b < nb; ++b) {
+    const double pr = sign[b] * dotg(g, v, basis[b]);
+    for (int m = 0; m < 4; ++m) v[m] -= pr * basis[b][m];
+  }
+  const double n = sqrt(fabs(dotg(g, v, v)));
+  for (int m = 0; m < 4; ++m) v[m] /= n;
+}
+
+// a-1: camera at (r_cam, theta_cam, phi=0); e0 || d_t, e3 from d_X1, e2 from -d_X2, e1 from d_X3 (R-3)
+__global__ void k_camera_setup(CamDev* cam, CameraSetupArgs a) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  CamDev C = *cam;
+  const double th = a.inclination_deg * M_PI / 180.0;
+  double x2 = th / M_PI;
+  if (!C.G.h_is_one) {
+    for (int it = 0; it < 100; ++it) {
+      double t, tp, tpp;
+      theta_map(C.G, x2, t, tp, tpp);
+      const double d = (t - th) / tp;
+      x2 -= d;
+      if (fabs(d) < 1e-17) break;
+    }
+  }
+  C.Xcam[0] = 0.0; C.Xcam[1] = log(C.r_cam); C.Xcam[2] = x2; C.Xcam[3] = 0.0;
+  Point p; Sym7 g; Inv6 gi;
+  metric<false>(C.G, C.Xcam, p, g, gi);
+  double basis[3][4], sg[3];
+  double e0[4] = {1.0, 0.0, 0.0, 0.0};
+  const double n0 = sqrt(-dotg(g, e0, e0));
+  for (int m = 0; m < 4; ++m) { C.e[0][m] = e0[m] / n0; basis[0][m] = C.e[0][m]; }
+  sg[0] = -1.0;
+  double e3[4] = {0.0, 1.0, 0.0, 0.0};
+  gram_schmidt(g, e3, basis, sg, 1);
+  for (int m = 0; m < 4; ++m) { C.e[3][m] = e3[m]; basis[1][m] = e3[m]; }
+  sg[1] = 1.0;
+  double e2[4] = {0.0, 0.0, -1.0, 0.0};
+  gram_schmidt(g, e2, basis, sg, 2);
+  for (int m = 0; m < 4; ++m) { C.e[2][m] = e2[m]; basis[2][m] = e2[m]; }
+  sg[2] = 1.0;
+  double e1[4] = {0.0, 0.0, 0.0, 1.0};
+  gram_schmidt(g, e1, basis, sg, 3);
+  for (int m = 0; m < 4; ++m) C.e[1][m] = e1[m];
+  g.mul(C.e[1], C.ecov1);
+  g.mul(C.e[2], C.ecov2);
+  C.lx_in = log(a.r_in);
+  C.lx_esc = log(a.r_esc);
+  *cam = C;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+struct GeoArgs {
+  CamDev cam;
+  double eps;                 // step parameter of this pass (probe passes use a multiple of cam.eps)
+  int max_steps;              // step limit of this pass
+  int cap;                    // steps that fit in one path slot (records = cap + 1); 0 when path == nullptr
+  int64_t base, count;        // rays [base, base+count) of the order / pixel list
+  const int* count_dev;       // if non-null, count = *count_dev (long-ray pass)
+  const int32_t* order;       // permutation of ray indices q (nullable: identity)
+  const int64_t* pixels;      // flat pixel index of ray q (nullable: q itself); with lattice_stride > 0 ignored
+  int64_t list_stride;        // probe over a pixel list: ray q stands for list entry q * list_stride (else 1)
+  int lattice_stride, lattice_nx;  // probe: ray q is pixel (ix*stride + stride/2, iy*stride + stride/2)
+  double* path;               // [count][cap+1][8] or nullptr (count-only)
+  int32_t* nsteps;            // [total rays], indexed by q; -1 = overflowed the slot
+  int32_t* nturn;             // [total rays]
+  unsigned long long* queue;  // atomic ray counter of this launch
+  int32_t* long_list; int* long_count;  // rays that did not fit (nullable)
+};
+
+__device__ __forceinline__ void pixel_ray(const CamDev& C, int64_t pix, double X[4], double K[4]) {
+  const int i = (int)(pix % C.nx), j = (int)(pix / C.nx);
+  const double alpha = (i + 0.5 - 0.5 * C.nx) * C.pix, beta = (j + 0.5 - 0.5 * C.ny) * C.pix;
+  const double px = -alpha / C.r_cam, py = -beta / C.r_cam;
+  const double nrm = sqrt(1.0 + px * px + py * py);
+#pragma unroll
+  for (int m = 0; m < 4; ++m) {
+    X[m] = C.Xcam[m];
+    K[m] = C.e[0][m] + (px * C.e[1][m] + py * C.e[2][m] + C.e[3][m]) / nrm;
+  }
+}
+
+__device__ __forceinline__ double stepsize(const double X[4], const double K[4], double eps) {
+  const double d = 1e-40;
+  const double i1 = (fabs(K[1]) + d) / eps;
+  const double i2 = (fabs(K[2]) + d) / (eps * fabs(fmin(X[2], 1.0 - X[2])));
+  const double i3 = (fabs(K[3]) + d) / eps;
+  return 1.0 / (i1 + i2 + i3);
+}
+
+// classical RK4 on (X^1..3, K^0..3); X^0 is not integrated (static snapshot, R-9)
+__device__ __forceinline__ void rk4_push(const Geom& G, double X[4], double K[4], double h) {
+  double k1[4], k2[4], k3[4], k4[4], Xt[4], Kt[4];
+  Xt[0] = 0.0;
+  geodesic_accel(G, X, K, k1);
+#pragma unroll
+  for (int m = 0; m < 4; ++m) { Kt[m] = K[m] + 0.5 * h * k1[m]; }
+#pragma unroll
+  for (int m = 1; m < 4; ++m) { Xt[m] = X[m] + 0.5 * h * K[m]; }
+  geodesic_accel(G, Xt, Kt, k2);
+  double xs[4];  // x1 + 2 x2 (+ 2 x3 + x4): the X-slopes are the stage K's
+#pragma unroll
+  for (int m = 1; m < 4; ++m) { xs[m] = K[m] + 2.0 * Kt[m]; Xt[m] = X[m] + 0.5 * h * Kt[m]; }
+#pragma unroll
+  for (int m = 0; m < 4; ++m) { Kt[m] = K[m] + 0.5 * h * k2[m]; }
+  geodesic_accel(G, Xt, Kt, k3);
+#pragma unroll
+  for (int m = 1; m < 4; ++m) { xs[m] += 2.0 * Kt[m]; Xt[m] = X[m] + h * Kt[m]; }
+#pragma unroll
+  for (int m = 0; m < 4; ++m) { Kt[m] = K[m] + h * k3[m]; }
+  geodesic_accel(G, Xt, Kt, k4);
+  const double h6 = h / 6.0;
+#pragma unroll
+  for (int m = 1; m < 4; ++m) X[m] += h6 * (xs[m] + Kt[m]);
+#pragma unroll
+  for (int m = 0; m < 4; ++m) K[m] += h6 * (k1[m] + 2.0 * k2[m] + 2.0 * k3[m] + k4[m]);
+}
+
+__device__ __forceinline__ void store_record(double* rec, const double X[4], const double K[4], double dl) {
+  double2* r2 = reinterpret_cast<double2*>(rec);
+  r2[0] = make_double2(X[1], X[2]);
+  r2[1] = make_double2(X[3], K[0]);
+  r2[2] = make_double2(K[1], K[2]);
+  r2[3] = make_double2(K[3], dl);
+}
+__device__ __forceinline__ void load_record(const double* rec, double X[4], double K[4], double& dl) {
+  const double2* r2 = reinterpret_cast<const double2*>(rec);
+  const double2 a = r2[0], b = r2[1], c = r2[2], d = r2[3];
+  X[0] = 0.0; X[1] = a.x; X[2] = a.y; X[3] = b.x;
+  K[0] = b.y; K[1] = c.x; K[2] = c.y; K[3] = d.x;
+  dl = d.y;
+}
+
+#ifndef IPOLE_GEO_THREADS
+#define IPOLE_GEO_THREADS 128
+#endif
+#ifndef IPOLE_GEO_MINB
+#define IPOLE_GEO_MINB 4
+#endif
+
+// a-2, a-3, a-8.  Every lane owns one ray at a time and pulls the next one from the atomic queue as soon as its ray
+// ends, so the RK4 body runs with all lanes active whatever the step counts of neighbouring pixels are.
+__global__ void __launch_bounds__(IPOLE_GEO_THREADS, IPOLE_GEO_MINB) k_geodesic(const __grid_constant__ GeoArgs A) {
+  const CamDev& C = A.cam;
+  const int64_t count = A.count_dev ? (int64_t)*A.count_dev : A.count;
+  const size_t slot_doubles = (size_t)(A.cap + 1) * REC_DOUBLES;
+  double X[4], K[4];
+  double* rec = nullptr;
+  int64_t li;
+  int32_t q = 0;
+  int n = 0, nt = 0;
+  bool have = false;
+
+  auto fetch = [&]() {
+    li = (int64_t)atomicAdd(A.queue, 1ULL);
+    have = li < count;
+    if (!have) return;
+    q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
+    int64_t pix;
+    if (A.lattice_stride > 0) {
+      const int ix = q % A.lattice_nx, iy = q / A.lattice_nx;
+      pix = (int64_t)(iy * A.lattice_stride + A.lattice_stride / 2) * C.nx + (ix * A.lattice_stride + A.lattice_stride / 2);
+    } else {
+      pix = A.pixels ? A.pixels[(int64_t)q * A.list_stride] : (int64_t)q * A.list_stride;
+    }
+    pixel_ray(C, pix, X, K);
+    rec = A.path ? A.path + (size_t)li * slot_doubles : nullptr;
+    n = 0; nt = 0;
+  };
+
+  fetch();
+  while (have) {
+    const double dl = stepsize(X, K, A.eps);
+    if (rec) store_record(rec + (size_t)n * REC_DOUBLES, X, K, dl);
+    const double x1_before = X[1];
+    const bool k2neg = K[2] < 0.0;
+    rk4_push(C.G, X, K, -dl);
+    ++n;
+    if ((K[2] < 0.0) != k2neg) ++nt;
+    int status = 0;
+    if (X[1] <= C.lx_in) status = 1;
+    else if (X[1] > C.lx_esc && X[1] > x1_before) status = 2;
+    else if (n >= A.max_steps) status = 3;
+    const bool overflow = (status == 0) && rec && (n >= A.cap);
+    if (status != 0 || overflow) {
+      if (overflow) {
+        A.nsteps[q] = -1;
+        if (A.long_list) { const int w = atomicAdd(A.long_count, 1); A.long_list[w] = q; }
+      } else {
+        if (rec) store_record(rec + (size_t)n * REC_DOUBLES, X, K, 0.0);
+        A.nsteps[q] = n;
+        if (A.nturn) A.nturn[q] = (nt > 127 ? 127 : nt) | (status == 3 ? 0x80 : 0);
+      }
+      fetch();
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+struct RtArgs {
+  CamDev cam;
+  Units units;
+  const void* model;          // device pointer to AdafParams / SlabParams / GridParams
+  int cap;
+  int64_t base, count;
+  const int* count_dev;
+  const int32_t* order;
+  const double* path;
+  const int32_t* nsteps;
+  unsigned long long* queue;
+  double *I, *Q, *U, *V, *tau, *tauF;   // indexed by q
+};
+
+#ifndef IPOLE_RT_THREADS
+#define IPOLE_RT_THREADS 128
+#endif
+#ifndef IPOLE_RT_MINB
+#define IPOLE_RT_MINB 2
+#endif
+
+// a-4 ... a-7, a-8.  Lane-level refill as in k_geodesic.  Per step: midpoint (Xm, Km), generator A = Gamma.Km,
+// f <- P f, plasma operator, f <- P f  (Strang splitting, R-6).
+template <int MODEL>
+__global__ void __launch_bounds__(IPOLE_RT_THREADS, IPOLE_RT_MINB) k_transfer(const __grid_constant__ RtArgs A) {
+  const CamDev& C = A.cam;
+  const int64_t count = A.count_dev ? (int64_t)*A.count_dev : A.count;
+  const size_t slot_doubles = (size_t)(A.cap + 1) * REC_DOUBLES;
+  __shared__ unsigned char model_smem[MODEL == MODEL_ADAF ? sizeof(AdafParams) : (MODEL == MODEL_SLAB ? sizeof(SlabParams) : sizeof(GridParams))];
+  {
+    const int nb = (int)sizeof(model_smem);
+    for (int i = threadIdx.x; i < nb; i += blockDim.x) model_smem[i] = ((const unsigned char*)A.model)[i];
+    __syncthreads();
+  }
+  const void* model = model_smem;
+
+  PolState st;
+  double Xhi[4], Khi[4];
+  const double* rec = nullptr;
+  int32_t q = 0;
+  int s = -1;
+  bool have = false, lit = false;
+
+  auto fetch = [&]() {
+    for (;;) {
+      const int64_t li = (int64_t)atomicAdd(A.queue, 1ULL);
+      have = li < count;
+      if (!have) return;
+      q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
+      const int n = A.nsteps[q];
+      if (n < 0) continue;  // overflowed its slot: done by the long-ray pass
+      rec = A.path + (size_t)li * slot_doubles;
+      double dl;
+      load_record(rec + (size_t)n * REC_DOUBLES, Xhi, Khi, dl);
+      s = n - 1;
+#pragma unroll
+      for (int m = 0; m < 4; ++m) { st.f1[m] = 0.0; st.f2[m] = 0.0; st.S[m] = 0.0; }
+      st.tau = 0.0; st.tauF = 0.0;
+      lit = false;
+      return;
+    }
+  };
+
+  fetch();
+  while (have) {
+    double Xlo[4], Klo[4], dl;
+    load_record(rec + (size_t)s * REC_DOUBLES, Xlo, Klo, dl);
+    double Xm[4], Km[4];
+#pragma unroll
+    for (int m = 0; m < 4; ++m) { Xm[m] = 0.5 * (Xlo[m] + Xhi[m]); Km[m] = 0.5 * (Klo[m] + Khi[m]); }
+    bool maybe = true;
+    if (MODEL == MODEL_GRID) {
+      const GridParams& M = *(const GridParams*)model;
+      maybe = !(Xm[1] > M.lx_out + 1e-6);  // certainly beyond r_out: no plasma (the exact test is in plasma_grid)
+    }
+    if (lit || maybe) {
+      Point p; Sym7 g; Inv6 gi; double Am[4][4];
+      transport_generator(C.G, Xm, Km, p, g, gi, Am);
+      const double h = 0.5 * dl;
+      if (lit) { transport_apply(Am, h, st.f1); transport_apply(Am, h, st.f2); }
+      if (maybe) lit |= plasma_operator<MODEL>(C.G, model, A.units, Xm, Km, p, g, gi, dl, st);
+      if (lit) { transport_apply(Am, h, st.f1); transport_apply(Am, h, st.f2); }
+    }
+#pragma unroll
+    for (int m = 0; m < 4; ++m) { Xhi[m] = Xlo[m]; Khi[m] = Klo[m]; }
+    --s;
+    if (s < 0) {
+      // a-7: project on the camera's transverse legs, convert the invariant I/nu^3 to specific intensity
+      stokes_congruence(dot4(C.ecov1, st.f1), dot4(C.ecov1, st.f2), dot4(C.ecov2, st.f1), dot4(C.ecov2, st.f2), st.S);
+      const double nu3 = A.units.nu_obs * A.units.nu_obs * A.units.nu_obs;
+      A.I[q] = st.S[0] * nu3; A.Q[q] = st.S[1] * nu3; A.U[q] = st.S[2] * nu3; A.V[q] = st.S[3] * nu3;
+      if (A.tau) A.tau[q] = st.tau;
+      if (A.tauF) A.tauF[q] = st.tauF;
+      fetch();
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a-8: order rays by predicted step count, longest first (counting sort on 4096 bins)
+constexpr int SORT_BINS = 4096;
+
+struct SortArgs {
+  int64_t n;                  // rays
+  const int32_t* probe;       // step counts of the probe lattice / probe list
+  int scale;                  // predicted = probe * scale
+  int lattice_stride, lattice_nx, lattice_ny, nx;  // full-image mode: pixel -> nearest lattice point
+  const int64_t* pixels;      // list mode with lattice: pixel of ray q (nullable)
+  int list_stride;            // list mode without lattice_stride: probe index = q / list_stride
+  int bin_width;
+  int32_t* key;               // [n] bin of each ray (descending steps = ascending bin)
+  unsigned int* hist;         // [SORT_BINS]
+  int32_t* order;             // [n] out
+};
+
+__global__ void k_predict_hist(SortArgs A) {
+  for (int64_t q = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; q < A.n; q += (int64_t)gridDim.x * blockDim.x) {
+    int pi;
+    if (A.lattice_stride > 0) {
+      const int64_t pix = A.pixels ? A.pixels[q] : q;
+      int ix = (int)(pix % A.nx) / A.lattice_stride, iy = (int)(pix / A.nx) / A.lattice_stride;
+      ix = min(ix, A.lattice_nx - 1); iy = min(iy, A.lattice_ny - 1);
+      pi = iy * A.lattice_nx + ix;
+    } else {
+      pi = (int)(q / A.list_stride);
+    }
+    const int pred = A.probe[pi] * A.scale;
+    int bin = SORT_BINS - 1 - min(pred / A.bin_width, SORT_BINS - 1);
+    A.key[q] = bin;
+    atomicAdd(&A.hist[bin], 1u);
+  }
+}
+
+__global__ void k_scan_bins(unsigned int* hist) {  // exclusive scan of SORT_BINS counters, one block of 1024
+  __shared__ unsigned int part[1024];
+  const int t = threadIdx.x;
+  unsigned int v[SORT_BINS / 1024], sum = 0;
+  for (int i = 0; i < SORT_BINS / 1024; ++i) { v[i] = hist[t * (SORT_BINS / 1024) + i]; sum += v[i]; }
+  part[t] = sum;
+  __syncthreads();
+  for (int off = 1; off < 1024; off <<= 1) {
+    const unsigned int x = (t >= off) ? part[t - off] : 0u;
+    __syncthreads();
+    part[t] += x;
+    __syncthreads();
+  }
+  unsigned int run = part[t] - sum;
+  for (int i = 0; i < SORT_BINS / 1024; ++i) { hist[t * (SORT_BINS / 1024) + i] = run; run += v[i]; }
+}
+
+__global__ void k_scatter(SortArgs A) {
+  for (int64_t q = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; q < A.n; q += (int64_t)gridDim.x * blockDim.x) {
+    const unsigned int pos = atomicAdd(&A.hist[A.key[q]], 1u);
+    A.order[pos] = (int32_t)q;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a-9: totals.  Fixed shape: REDUCE_BLOCKS blocks x 256 threads, grid-stride partial sums, warp shuffles, then one
+// block folds the partials in index order -> bitwise reproducible for a given image.
+constexpr int REDUCE_BLOCKS = 296;
+
+struct ReduceOut {
+  double flux[4];          // sum of I,Q,U,V over pixels (times scale in the final kernel)
+  double lp, cp;
+  long long total_steps;
+  int max_steps;
+  long long n_ring, n_maxstep;
+};
+
+struct ReducePartial { double s[4]; long long steps; int maxs; long long ring, maxed; };
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ long long warp_sum_ll(long long v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ int warp_max(int v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = max(v, __shfl_down_sync(0xffffffffu, v, o));
+  return v;
+}
+
+__global__ void __launch_bounds__(256) k_reduce_partial(int64_t n, const double* I, const double* Q, const double* U,
+                                                        const double* V, const int32_t* nsteps, const int32_t* nturn,
+                                                        ReducePartial* part) {
+  double s[4] = {0, 0, 0, 0};
+  long long steps = 0, ring = 0, maxed = 0;
+  int maxs = 0;
+  for (int64_t q = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; q < n; q += (int64_t)gridDim.x * blockDim.x) {
+    s[0] += I[q]; s[1] += Q[q]; s[2] += U[q]; s[3] += V[q];
+    const int ns = nsteps[q], nt = nturn[q];
+    steps += ns; maxs = max(maxs, ns);
+    ring += ((nt & 0x7f) >= 2); maxed += ((nt & 0x80) != 0);
+  }
+  __shared__ ReducePartial sh[8];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) s[k] = warp_sum(s[k]);
+  steps = warp_sum_ll(steps); ring = warp_sum_ll(ring); maxed = warp_sum_ll(maxed); maxs = warp_max(maxs);
+  if (lane == 0) { for (int k = 0; k < 4; ++k) sh[w].s[k] = s[k]; sh[w].steps = steps; sh[w].maxs = maxs; sh[w].ring = ring; sh[w].maxed = maxed; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    ReducePartial r = sh[0];
+    for (int i = 1; i < 8; ++i) {
+      for (int k = 0; k < 4; ++k) r.s[k] += sh[i].s[k];
+      r.steps += sh[i].steps; r.maxs = max(r.maxs, sh[i].maxs); r.ring += sh[i].ring; r.maxed += sh[i].maxed;
+    }
+    part[blockIdx.x] = r;
+  }
+}
+
+__global__ void k_reduce_final(const ReducePartial* part, int nparts, double scale, ReduceOut* out) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  ReducePartial r = part[0];
+  for (int i = 1; i < nparts; ++i) {
+    for (int k = 0; k < 4; ++k) r.s[k] += part[i].s[k];
+    r.steps += part[i].steps; r.maxs = max(r.maxs, part[i].maxs); r.ring += part[i].ring; r.maxed += part[i].maxed;
+  }
+  ReduceOut o;
+  for (int k = 0; k < 4; ++k) o.flux[k] = r.s[k] * scale;
+  o.lp = (r.s[0] != 0.0) ? sqrt(r.s[1] * r.s[1] + r.s[2] * r.s[2]) / r.s[0] : 0.0;
+  o.cp = (r.s[0] != 0.0) ? r.s[3] / r.s[0] : 0.0;
+  o.total_steps = r.steps; o.max_steps = r.maxs; o.n_ring = r.ring; o.n_maxstep = r.maxed;
+  *out = o;
+}
+
+__global__ void k_max_i32(const int32_t* v, int n, int* out) {  // probe maximum (one block)
+  int m = 0;
+  for (int i = threadIdx.x; i < n; i += blockDim.x) m = max(m, v[i]);
+  m = warp_max(m);
+  __shared__ int sh[32];
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x == 0) { for (int i = 1; i < (int)(blockDim.x >> 5); ++i) m = max(m, sh[i]); *out = m; }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// stage evaluators for the per-stage parity tests
+__global__ void k_eval_connection(Geom G, int64_t n, const double* X, double* Gam) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  // Gamma^l_{mn} recovered from the contracted generator: A(K = e_m)^l_n = Gamma^l_{mn}
+  for (int m = 0; m < 4; ++m) {
+    double K[4] = {0, 0, 0, 0};
+    K[m] = 1.0;
+    Point p; Sym7 g; Inv6 gi; double A[4][4];
+    transport_generator(G, X + 4 * i, K, p, g, gi, A);
+    for (int l = 0; l < 4; ++l) for (int nn = 0; nn < 4; ++nn) Gam[64 * i + 16 * l + 4 * m + nn] = A[l][nn];
+  }
+}
+__global__ void k_eval_coefficients(int64_t n, const double* in, double* out) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const Coeff c = synchrotron_coefficients(in[5 * i], in[5 * i + 1], in[5 * i + 2], in[5 * i + 3], in[5 * i + 4]);
+  double* o = out + 8 * i;
+  o[0] = c.jI; o[1] = c.jQ; o[2] = c.jV; o[3] = c.aI; o[4] = c.aQ; o[5] = c.aV; o[6] = c.rQ; o[7] = c.rV;
+}
+__global__ void k_eval_stokes_step(int64_t n, const double* in, double* out) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double* a = in + 16 * i;
+  double S[4] = {a[8], a[9], a[10], a[11]};
+  stokes_step(a, a + 4, a[7], a + 12, S);
+  for (int k = 0; k < 4; ++k) out[4 * i + k] = S[k];
+}
+__global__ void k_eval_bessel(int64_t n, const double* z, double* out) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double k0, k1;
+  bessel_k01_scaled(z[i], k0, k1);
+  out[3 * i] = k0; out[3 * i + 1] = k1; out[3 * i + 2] = k0 + 2.0 / z[i] * k1;
+}
+template <int MODEL>
+__global__ void k_eval_plasma(Geom G, const void* model, int64_t n, const double* X, double* out) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  Point p; Sym7 g; Inv6 gi;
+  metric<true>(G, X + 4 * i, p, g, gi);
+  Plasma P;
+  P.ne = P.Th = P.B = 0.0;
+  for (int m = 0; m < 4; ++m) { P.u[m] = 0.0; P.b[m] = 0.0; }
+  bool present;
+  if (MODEL == MODEL_ADAF) present = plasma_adaf(G, *(const AdafParams*)model, X + 4 * i, p, g, gi, P);
+  else if (MODEL == MODEL_SLAB) present = plasma_slab(G, *(const SlabParams*)model, X + 4 * i, p, g, P);
+  else present = plasma_grid(G, *(const GridParams*)model, X + 4 * i, p, g, gi, P);
+  double* o = out + 12 * i;
+  o[0] = present ? 1.0 : 0.0; o[1] = present ? P.ne : 0.0; o[2] = present ? P.Th : 0.0; o[3] = present ? P.B : 0.0;
+  for (int m = 0; m < 4; ++m) { o[4 + m] = present ? P.u[m] : 0.0; o[8 + m] = present ? P.b[m] : 0.0; }
+}
+
+// FP64 FMA throughput: 8 independent chains per thread
+__global__ void __launch_bounds__(256) k_fp64_peak(int iters, double seed, double* sink) {
+  double a0 = seed, a1 = seed + 1, a2 = seed + 2, a3 = seed + 3, a4 = seed + 4, a5 = seed + 5, a6 = seed + 6, a7 = seed + 7;
+  const double b = 0.999999 + 1e-9 * threadIdx.x, c = 1e-7;
+  for (int i = 0; i < iters; ++i) {
+    a0 = fma(a0, b, c); a1 = fma(a1, b, c); a2 = fma(a2, b, c); a3 = fma(a3, b, c);
+    a4 = fma(a4, b, c); a5 = fma(a5, b, c); a6 = fma(a6, b, c); a7 = fma(a7, b, c);
+  }
+  const double r = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+  if (r == 123.456) sink[0] = r;
+}
+
+}  // namespace ipole

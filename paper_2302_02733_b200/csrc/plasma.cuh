@@ -1,0 +1,268 @@
+// Plasma models (what the fluid is at a point of the ray), the plasma-frame tetrad, and one application of the
+// plasma operator to the polarization state.  DESIGN.md R-5, R-6 ("For semianalytic models, the code
+// calculates the model at the current geodesic position.  For GRMHD simulations we read out the plasma quantities
+// from precomputed three 3D arrays ... interpolates the plasma quantities to the point at every single step").
+//
+// Polarization state carried per ray ("factorised coherency tensor"): after every plasma
+// step the coherency tensor of PAPER.md:37 is N^{mu nu} = sum_{a,b in {1,2}} n^{ab} f_a^mu f_b^nu with two REAL
+// vectors f_1, f_2 (the transverse tetrad legs, parallel-transported since) and the 2x2 Hermitian n^{ab}, i.e. the
+// four Stokes parameters S.  The congruence N <- P N P^T is f_a <- P f_a; projecting on a new tetrad is the real
+// 2x2 congruence n <- M n M^T with M_{a'a} = e^(a')_mu f_a^mu.
+#pragma once
+#include "geom.cuh"
+#include "coeff.cuh"
+#include "stokes.cuh"
+
+namespace ipole {
+
+enum { MODEL_NONE = 0, MODEL_ADAF = 1, MODEL_SLAB = 2, MODEL_GRID = 3 };
+
+struct AdafParams { double n0, p_n, Th0, p_T, B0, p_B, r_isco; };
+struct SlabParams { double H; int profile; double cpsi, spsi; double j[4], al[4], rh[3]; };
+struct GridParams {
+  int N1, N2, N3;
+  double startx[3], idx[3];      // idx = 1/dx
+  double gam, Rlow, Rhigh, r_out, lx_out;   // lx_out = ln r_out
+  double ne_unit, B_unit;        // rho -> n_e [cm^-3], sqrt(b.b) -> Gauss
+  const double* f[8];            // device planes rho,u,U1,U2,U3,B1,B2,B3
+};
+struct Units { double nu_obs, L_unit, D_cm; };
+
+struct Plasma {
+  double ne, Th, B;
+  double u[4], b[4];
+  double j[4], al[4], rh[3];  // slab only
+};
+
+__device__ __forceinline__ double dotg(const Sym7& g, const double u[4], const double v[4]) {
+  double l[4];
+  g.mul(u, l);
+  return dot4(l, v);
+}
+
+__device__ __forceinline__ bool plasma_adaf(const Geom& G, const AdafParams& M, const double X[4], const Point& p,
+                                            const Sym7& g, const Inv6& gi, Plasma& P) {
+  const double a = G.a, r = p.r;
+  P.ne = M.n0 * exp(M.p_n * X[1]);
+  P.Th = M.Th0 * exp(M.p_T * X[1]);
+  P.B = M.B0 * exp(M.p_B * X[1]);
+  if (r >= M.r_isco) {
+    const double Om = 1.0 / (r * sqrt(r) + a);
+    const double ut = rsqrt(-(g.c00 + 2.0 * g.c03 * Om + g.c33 * Om * Om));
+    P.u[0] = ut; P.u[1] = 0.0; P.u[2] = 0.0; P.u[3] = ut * Om;
+  } else {
+    const double ur_ks = -2.0 * r / (2.0 * r + sqrt(2.0 * r * (r * r + a * a)));
+    const double ucov[4] = {-1.0, r * ur_ks, 0.0, 0.0};
+    gi.mul(ucov, P.u);
+  }
+  // d_phi projected orthogonal to u, scaled to b.b = B^2
+  const double tu = g.c03 * P.u[0] + g.c13 * P.u[1] + g.c33 * P.u[3];
+  double bb[4] = {tu * P.u[0], tu * P.u[1], tu * P.u[2], 1.0 + tu * P.u[3]};
+  const double sc = P.B * rsqrt(dotg(g, bb, bb));
+#pragma unroll
+  for (int m = 0; m < 4; ++m) P.b[m] = bb[m] * sc;
+  return true;
+}
+
+__device__ __forceinline__ bool plasma_slab(const Geom& G, const SlabParams& M, const double X[4], const Point& p,
+                                            const Sym7& g, Plasma& P) {
+  const double a = G.a, r = p.r, s = p.s, c = p.c;
+  const double z = r * c;
+  double w = 1.0;
+  if (M.profile == 0) { if (!(fabs(z) < M.H)) return false; }
+  else w = exp(-z * z / (2.0 * M.H * M.H));
+  P.u[0] = rsqrt(-g.c00); P.u[1] = P.u[2] = P.u[3] = 0.0;
+  double sp, cp;
+  sincos(X[3], &sp, &cp);
+  // d(x,y,z)/d(r,theta,phi) of x = (r cos ph - a sin ph) sin th, y = (r sin ph + a cos ph) sin th, z = r cos th
+  const double J[3][3] = {{cp * s, (r * cp - a * sp) * c, (-r * sp - a * cp) * s},
+                          {sp * s, (r * sp + a * cp) * c, (r * cp - a * sp) * s},
+                          {c, -r * s, 0.0}};
+  const double dir[3] = {M.cpsi, M.spsi, 0.0};
+  // Cramer's rule
+  double col[3][3], v[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { col[0][i] = J[i][0]; col[1][i] = J[i][1]; col[2][i] = J[i][2]; }
+  double t[3];
+  cross3(col[1], col[2], t); const double D = dot3(col[0], t);
+  v[0] = dot3(dir, t) / D;
+  cross3(col[2], col[0], t); v[1] = dot3(dir, t) / D;
+  cross3(col[0], col[1], t); v[2] = dot3(dir, t) / D;
+  const double sp4[4] = {0.0, v[0] / r, v[1] / p.tp, v[2]};
+  const double su = dotg(g, sp4, P.u);
+#pragma unroll
+  for (int m = 0; m < 4; ++m) P.b[m] = sp4[m] + su * P.u[m];
+  const double sc = rsqrt(dotg(g, P.b, P.b));
+#pragma unroll
+  for (int m = 0; m < 4; ++m) P.b[m] *= sc;
+  P.B = 1.0; P.ne = 0.0; P.Th = 0.0;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { P.j[i] = w * M.j[i]; P.al[i] = w * M.al[i]; }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) P.rh[i] = w * M.rh[i];
+  return true;
+}
+
+__device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
+// FP64 trilinear interpolation over the 8 SoA planes (read-only path: ld.global.nc)
+__device__ __forceinline__ bool plasma_grid(const Geom& G, const GridParams& M, const double X[4], const Point& p,
+                                            const Sym7& g, const Inv6& gi, Plasma& P) {
+  if (p.r > M.r_out || X[1] < M.startx[0]) return false;
+  const double fi = (X[1] - M.startx[0]) * M.idx[0] - 0.5;
+  const double fj = (X[2] - M.startx[1]) * M.idx[1] - 0.5;
+  const double fk = (X[3] - M.startx[2]) * M.idx[2] - 0.5;
+  const double i0f = floor(fi), j0f = floor(fj), k0f = floor(fk);
+  const double di = fi - i0f, dj = fj - j0f, dk = fk - k0f;
+  const int i0 = clampi((int)i0f, 0, M.N1 - 1), i1 = clampi((int)i0f + 1, 0, M.N1 - 1);
+  const int j0 = clampi((int)j0f, 0, M.N2 - 1), j1 = clampi((int)j0f + 1, 0, M.N2 - 1);
+  long long kk = (long long)k0f % M.N3; if (kk < 0) kk += M.N3;
+  const int k0 = (int)kk, k1 = (k0 + 1 == M.N3) ? 0 : k0 + 1;
+  const size_t o00 = ((size_t)i0 * M.N2 + j0) * M.N3, o01 = ((size_t)i0 * M.N2 + j1) * M.N3;
+  const size_t o10 = ((size_t)i1 * M.N2 + j0) * M.N3, o11 = ((size_t)i1 * M.N2 + j1) * M.N3;
+  const double wi0 = 1.0 - di, wj0 = 1.0 - dj, wk0 = 1.0 - dk;
+  double prim[8];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) {
+    const double* F = M.f[q];
+    const double a000 = __ldg(F + o00 + k0), a001 = __ldg(F + o00 + k1);
+    const double a010 = __ldg(F + o01 + k0), a011 = __ldg(F + o01 + k1);
+    const double a100 = __ldg(F + o10 + k0), a101 = __ldg(F + o10 + k1);
+    const double a110 = __ldg(F + o11 + k0), a111 = __ldg(F + o11 + k1);
+    prim[q] = wi0 * (wj0 * (wk0 * a000 + dk * a001) + dj * (wk0 * a010 + dk * a011))
+              + di * (wj0 * (wk0 * a100 + dk * a101) + dj * (wk0 * a110 + dk * a111));
+  }
+  const double rho = prim[0], uu = prim[1];
+  if (!(rho > 0.0) || !(uu > 0.0)) return false;
+  const double alpha_l = rsqrt(-gi.c00);
+  // q2 = g_ij U^i U^j (spatial block of the sparse metric)
+  const double U1 = prim[2], U2 = prim[3], U3 = prim[4];
+  const double q2 = g.c11 * U1 * U1 + 2.0 * g.c13 * U1 * U3 + g.c22 * U2 * U2 + g.c33 * U3 * U3;
+  const double gamma = sqrt(1.0 + q2);
+  P.u[0] = gamma / alpha_l;
+  P.u[1] = U1 - gamma * alpha_l * gi.c01;
+  P.u[2] = U2;
+  P.u[3] = U3;
+  double ul[4];
+  g.mul(P.u, ul);
+  const double B1 = prim[5], B2 = prim[6], B3 = prim[7];
+  const double bt = B1 * ul[1] + B2 * ul[2] + B3 * ul[3];
+  double bc[4];
+  bc[0] = bt;
+  bc[1] = (B1 + bt * P.u[1]) / P.u[0];
+  bc[2] = (B2 + bt * P.u[2]) / P.u[0];
+  bc[3] = (B3 + bt * P.u[3]) / P.u[0];
+  const double bsq = dotg(g, bc, bc);
+  if (!(bsq > 0.0)) return false;
+  P.ne = rho * M.ne_unit;
+  P.B = sqrt(bsq) * M.B_unit;
+  const double beta = (M.gam - 1.0) * uu / (0.5 * bsq);
+  const double b2 = beta * beta;
+  const double R = (M.Rhigh * b2 + M.Rlow) / (1.0 + b2);
+  P.Th = (IP_MP / IP_ME) * (M.gam - 1.0) * (uu / rho) / (1.0 + R);
+#pragma unroll
+  for (int m = 0; m < 4; ++m) P.b[m] = bc[m] * M.B_unit;
+  return true;
+}
+
+// eps^{mu a b c} p_a q_b w_c with [0123] = +1
+__device__ __forceinline__ void levi4(const double p[4], const double q[4], const double w[4], double o[4]) {
+  const double m01 = q[0] * w[1] - q[1] * w[0], m02 = q[0] * w[2] - q[2] * w[0], m03 = q[0] * w[3] - q[3] * w[0];
+  const double m12 = q[1] * w[2] - q[2] * w[1], m13 = q[1] * w[3] - q[3] * w[1], m23 = q[2] * w[3] - q[3] * w[2];
+  o[0] = p[1] * m23 - p[2] * m13 + p[3] * m12;
+  o[1] = -(p[0] * m23 - p[2] * m03 + p[3] * m02);
+  o[2] = p[0] * m13 - p[1] * m03 + p[3] * m01;
+  o[3] = -(p[0] * m12 - p[1] * m02 + p[2] * m01);
+}
+
+// Stokes vector under the real 2x2 congruence n <- M n M^T
+__device__ __forceinline__ void stokes_congruence(const double m11, const double m12, const double m21, const double m22,
+                                                  double S[4]) {
+  const double R11 = 0.5 * (S[0] + S[1]), R22 = 0.5 * (S[0] - S[1]), R12 = 0.5 * S[2];
+  const double T11 = m11 * m11 * R11 + 2.0 * m11 * m12 * R12 + m12 * m12 * R22;
+  const double T22 = m21 * m21 * R11 + 2.0 * m21 * m22 * R12 + m22 * m22 * R22;
+  const double T12 = m11 * m21 * R11 + (m11 * m22 + m12 * m21) * R12 + m12 * m22 * R22;
+  S[0] = T11 + T22;
+  S[1] = T11 - T22;
+  S[2] = 2.0 * T12;
+  S[3] = (m11 * m22 - m12 * m21) * S[3];
+}
+
+struct PolState {
+  double f1[4], f2[4];  // transverse legs, contravariant MKS components
+  double S[4];          // invariant Stokes I/nu^3 ... in the (f1, f2) basis
+  double tau, tauF;
+};
+
+// One application of the plasma operator at (X, K) over affine length dl.  Returns true if applied.
+template <int MODEL>
+__device__ __forceinline__ bool plasma_operator(const Geom& G, const void* model, const Units& U, const double X[4],
+                                                const double K[4], const Point& p, const Sym7& g, const Inv6& gi,
+                                                double dl, PolState& st) {
+  Plasma P;
+  bool present;
+  if (MODEL == MODEL_ADAF) present = plasma_adaf(G, *(const AdafParams*)model, X, p, g, gi, P);
+  else if (MODEL == MODEL_SLAB) present = plasma_slab(G, *(const SlabParams*)model, X, p, g, P);
+  else present = plasma_grid(G, *(const GridParams*)model, X, p, g, gi, P);
+  if (!present) return false;
+
+  double kcov[4], ucov[4];
+  g.mul(K, kcov);
+  g.mul(P.u, ucov);
+  const double om = -dot4(kcov, P.u);
+  if (!(om > 0.0)) return false;
+  double e3[4], e2[4], e1[4], e3c[4], e2c[4], e1c[4];
+  const double iom = 1.0 / om;
+#pragma unroll
+  for (int m = 0; m < 4; ++m) e3[m] = K[m] * iom - P.u[m];
+  g.mul(e3, e3c);
+  const double n3 = dot4(e3c, e3);
+  if (!(n3 > 0.0)) return false;
+  const double i3 = rsqrt(n3);
+#pragma unroll
+  for (int m = 0; m < 4; ++m) { e3[m] *= i3; e3c[m] *= i3; }
+  const double be3 = dot4(e3c, P.b);
+#pragma unroll
+  for (int m = 0; m < 4; ++m) e2[m] = P.b[m] - be3 * e3[m];
+  g.mul(e2, e2c);
+  const double n2 = dot4(e2c, e2);
+  if (!(n2 > 0.0)) return false;
+  const double i2 = rsqrt(n2);
+#pragma unroll
+  for (int m = 0; m < 4; ++m) { e2[m] *= i2; e2c[m] *= i2; }
+  levi4(ucov, e2c, e3c, e1);
+  const double isg = 1.0 / p.sqrtmg;
+#pragma unroll
+  for (int m = 0; m < 4; ++m) e1[m] *= isg;
+  g.mul(e1, e1c);
+
+  const double nu = om * U.nu_obs;
+  double ji[4], ai[4], ri[3];
+  if (MODEL == MODEL_SLAB) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { ji[i] = P.j[i] / (nu * nu); ai[i] = P.al[i] * nu; }
+#pragma unroll
+    for (int i = 0; i < 3; ++i) ri[i] = P.rh[i] * nu;
+  } else {
+    double bcov[4];
+    g.mul(P.b, bcov);
+    double cosT = dot4(bcov, K) / (om * P.B);
+    cosT = fmin(1.0, fmax(-1.0, cosT));
+    const Coeff c = synchrotron_coefficients(P.ne, P.Th, P.B, cosT, nu);
+    const double inu2 = 1.0 / (nu * nu);
+    ji[0] = c.jI * inu2; ji[1] = c.jQ * inu2; ji[2] = 0.0; ji[3] = c.jV * inu2;
+    ai[0] = c.aI * nu;   ai[1] = c.aQ * nu;   ai[2] = 0.0; ai[3] = c.aV * nu;
+    ri[0] = c.rQ * nu;   ri[1] = 0.0;         ri[2] = c.rV * nu;
+  }
+  const double ds = dl * U.L_unit / U.nu_obs;
+  // project the carried state on the new transverse legs: M_{a'a} = e^(a')_mu f_a^mu
+  stokes_congruence(dot4(e1c, st.f1), dot4(e1c, st.f2), dot4(e2c, st.f1), dot4(e2c, st.f2), st.S);
+  stokes_step(ai, ri, ds, ji, st.S);
+#pragma unroll
+  for (int m = 0; m < 4; ++m) { st.f1[m] = e1[m]; st.f2[m] = e2[m]; }
+  st.tau += ai[0] * ds;
+  st.tauF += fabs(ri[2]) * ds;
+  return true;
+}
+
+}  // namespace ipole

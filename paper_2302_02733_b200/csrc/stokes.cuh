@@ -1,0 +1,100 @@
+// Constant-coefficient solution of the polarized transfer equation over one step,
+//   dS/ds = J - Kmat S,  S(s) = O(s) S0 + P(s) J,  O = exp(-Kmat s),  P = int_0^s O,
+// applied to vectors (the 4x4 matrices are never formed).  DESIGN.md R-8 (north_star stage (3): "the analytic
+// per-step solution of the 4x4 transfer equation"); closed form of Landi Degl'Innocenti & Landi Degl'Innocenti
+// (1985):  O = e^{-aI s} { (ch+c)/2 1 - sn M2 - sh M3 + (ch-c)/2 M4 } with, for 3-vectors a = (aQ,aU,aV),
+// r = (rQ,rU,rV) and any Stokes vector (S0, s):
+//   M2 (S0,s) = ( v2.s , v2 S0 + s x w2 ) / Th,   v2 = L2 a - sg L1 r,  w2 = sg L1 a + L2 r
+//   M3 (S0,s) = ( v3.s , v3 S0 + s x w3 ) / Th,   v3 = L1 a + sg L2 r,  w3 = -sg L2 a + L1 r
+//   M4 (S0,s) = 2 ( hh S0 + cr.s , -cr S0 + a (a.s) + r (r.s) - hh s ) / Th,  cr = r x a, hh = (|a|^2+|r|^2)/2
+// (L1, L2, sg, Th as in the oracle's header; all vectors scaled by m = max |component| first).
+#pragma once
+#include "geom.cuh"
+
+namespace ipole {
+
+__device__ __forceinline__ double exp_integral(double b, double s) { return (b == 0.0) ? s : -expm1(-b * s) / b; }
+
+__device__ __forceinline__ void cross3(const double u[3], const double v[3], double o[3]) {
+  o[0] = u[1] * v[2] - u[2] * v[1];
+  o[1] = u[2] * v[0] - u[0] * v[2];
+  o[2] = u[0] * v[1] - u[1] * v[0];
+}
+__device__ __forceinline__ double dot3(const double u[3], const double v[3]) { return u[0] * v[0] + u[1] * v[1] + u[2] * v[2]; }
+
+// S <- O(s) S + P(s) J ; al = (aI,aQ,aU,aV), rh = (rQ,rU,rV)
+__device__ __forceinline__ void stokes_step(const double al[4], const double rh[3], double s, const double J[4], double S[4]) {
+  const double aI = al[0];
+  const double m = fmax(fmax(fabs(al[1]), fmax(fabs(al[2]), fabs(al[3]))), fmax(fabs(rh[0]), fmax(fabs(rh[1]), fabs(rh[2]))));
+  if (m == 0.0) {
+    const double ex = exp(-aI * s), E = exp_integral(aI, s);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) S[i] = ex * S[i] + E * J[i];
+    return;
+  }
+  const double im = 1.0 / m;
+  const double a[3] = {al[1] * im, al[2] * im, al[3] * im};
+  const double r[3] = {rh[0] * im, rh[1] * im, rh[2] * im};
+  const double a2 = dot3(a, a), r2 = dot3(r, r), ar = dot3(a, r);
+  const double sg = (ar >= 0.0) ? 1.0 : -1.0;
+  const double d = 0.5 * (a2 - r2);
+  const double q = sqrt(d * d + ar * ar);
+  double l1, l2;
+  if (d >= 0.0) { l1 = sqrt(q + d); l2 = (l1 > 0.0) ? fabs(ar) / l1 : 0.0; }
+  else          { l2 = sqrt(q - d); l1 = (l2 > 0.0) ? fabs(ar) / l2 : 0.0; }
+  const double iTh = 1.0 / (l1 * l1 + l2 * l2);
+  const double L1 = m * l1, L2 = m * l2;
+  const double hh = 0.5 * (a2 + r2);
+  double v2[3], w2[3], v3[3], w3[3], cr[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    v2[i] = l2 * a[i] - sg * l1 * r[i];
+    w2[i] = sg * l1 * a[i] + l2 * r[i];
+    v3[i] = l1 * a[i] + sg * l2 * r[i];
+    w3[i] = -sg * l2 * a[i] + l1 * r[i];
+  }
+  cross3(r, a, cr);
+
+  const double ex = exp(-aI * s);
+  double sn, c;
+  sincos(L2 * s, &sn, &c);
+  const double ch = cosh(L1 * s), sh = sinh(L1 * s);
+  const double Ep = exp_integral(aI - L1, s), Em = exp_integral(aI + L1, s);
+  const double Ic1 = 0.5 * (Ep + Em), Is1 = 0.5 * (Ep - Em);
+  double Ic2, Is2;
+  const double den = aI * aI + L2 * L2;
+  if (den == 0.0) { Ic2 = s; Is2 = 0.0; }
+  else {
+    const double em1 = expm1(-aI * s), hs = sin(0.5 * L2 * s);
+    const double re = -(em1 * c - 2.0 * hs * hs);
+    const double im2 = -ex * sn;
+    Ic2 = (re * aI - im2 * L2) / den;
+    Is2 = (re * L2 + im2 * aI) / den;
+  }
+  // weights of (1, M2, M3, M4) for O and for P
+  const double o1 = ex * 0.5 * (ch + c), o2 = -ex * sn, o3 = -ex * sh, o4 = ex * 0.5 * (ch - c);
+  const double p1 = 0.5 * (Ic1 + Ic2), p2 = -Is2, p3 = -Is1, p4 = 0.5 * (Ic1 - Ic2);
+
+  double out[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+  for (int pass = 0; pass < 2; ++pass) {
+    const double* V = pass ? J : S;
+    const double c1 = pass ? p1 : o1, c2 = (pass ? p2 : o2) * iTh, c3 = (pass ? p3 : o3) * iTh,
+                 c4 = (pass ? p4 : o4) * 2.0 * iTh;
+    const double V0 = V[0];
+    const double sv[3] = {V[1], V[2], V[3]};
+    double x2[3], x3[3];
+    cross3(sv, w2, x2);
+    cross3(sv, w3, x3);
+    const double as = dot3(a, sv), rs = dot3(r, sv);
+    out[0] += c1 * V0 + c2 * dot3(v2, sv) + c3 * dot3(v3, sv) + c4 * (hh * V0 + dot3(cr, sv));
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+      out[1 + i] += c1 * sv[i] + c2 * (v2[i] * V0 + x2[i]) + c3 * (v3[i] * V0 + x3[i])
+                    + c4 * (-cr[i] * V0 + a[i] * as + r[i] * rs - hh * sv[i]);
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) S[i] = out[i];
+}
+
+}  // namespace ipole

@@ -1,0 +1,278 @@
+"""Thin ctypes binding of libipole_b200.so (the C ABI of include/ipole.h).
+
+Argument marshalling only: every step of the hot path runs in the library's CUDA kernels.  PyTorch is used
+for device memory and streams (outputs are torch CUDA tensors whose data_ptr() is handed to the library).
+There is no CPU fallback: if the library is missing or no CUDA device is present this module raises.
+It never imports anything under oracle/.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libipole_b200.so")
+_LIB = None
+
+OK, EINVAL, ENOMODEL, ENOMEM, ECUDA, ENOIMAGE = 0, -1, -2, -3, -4, -5
+
+#: every symbol include/ipole.h declares (checked by tests/test_abi.py)
+SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_options", "ipole_load_model_adaf",
+           "ipole_load_model_slab", "ipole_load_model_grid", "ipole_make_image", "ipole_make_pixels",
+           "ipole_get_ray_info", "ipole_get_stats", "ipole_get_camera_tetrad", "ipole_trace_pixel",
+           "ipole_eval_connection", "ipole_eval_coefficients", "ipole_eval_stokes_step", "ipole_eval_bessel",
+           "ipole_eval_plasma", "ipole_measure_fp64_peak", "ipole_last_cuda_error", "ipole_free", "ipole_strerror",
+           "ipole_version"]
+
+
+class Camera(C.Structure):
+    _fields_ = [("spin", C.c_double), ("inclination_deg", C.c_double), ("r_cam", C.c_double), ("fov", C.c_double),
+                ("nx", C.c_int32), ("ny", C.c_int32), ("freq_hz", C.c_double), ("mbh_msun", C.c_double),
+                ("dsource_pc", C.c_double), ("eps", C.c_double), ("r_esc", C.c_double), ("stop_factor", C.c_double),
+                ("max_steps", C.c_int32), ("hslope", C.c_double), ("flat_metric", C.c_int32)]
+
+
+class AdafParams(C.Structure):
+    _fields_ = [("n0", C.c_double), ("p_n", C.c_double), ("Th0", C.c_double), ("p_T", C.c_double),
+                ("B0", C.c_double), ("p_B", C.c_double)]
+
+
+class SlabParams(C.Structure):
+    _fields_ = [("H", C.c_double), ("profile", C.c_int32), ("psi_deg", C.c_double), ("j", C.c_double * 4),
+                ("alpha", C.c_double * 4), ("rho", C.c_double * 3)]
+
+
+class GridDesc(C.Structure):
+    _fields_ = [("N1", C.c_int32), ("N2", C.c_int32), ("N3", C.c_int32), ("startx", C.c_double * 3),
+                ("dx", C.c_double * 3), ("hslope", C.c_double), ("gam", C.c_double), ("M_unit", C.c_double),
+                ("Rlow", C.c_double), ("Rhigh", C.c_double), ("r_out", C.c_double)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("flux_jy", C.c_double * 4), ("lp", C.c_double), ("cp", C.c_double), ("total_steps", C.c_int64),
+                ("max_steps_seen", C.c_int32), ("path_cap", C.c_int32), ("n_ring", C.c_int64),
+                ("n_maxstep", C.c_int64), ("n_long", C.c_int64), ("n_batches", C.c_int32), ("n_launches", C.c_int32),
+                ("ms_probe", C.c_float), ("ms_geodesic", C.c_float), ("ms_transfer", C.c_float), ("ms_total", C.c_float)]
+
+
+class IpoleError(RuntimeError):
+    def __init__(self, code, what):
+        self.code = code
+        super().__init__("%s failed: %d (%s)" % (what, code, lib().ipole_strerror(code).decode()))
+
+
+def lib():
+    """Load libipole_b200.so (built in-tree by __graft_entry__.build()).  Raises if it is missing."""
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("%s not found: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                              "(there is no CPU fallback)" % LIB_PATH)
+        L = C.CDLL(LIB_PATH)
+        vp, dp = C.c_void_p, C.POINTER(C.c_double)
+        L.ipole_init.argtypes = [C.POINTER(Camera), C.POINTER(vp)]
+        L.ipole_set_camera.argtypes = [vp, C.POINTER(Camera)]
+        L.ipole_set_stream.argtypes = [vp, vp]
+        L.ipole_set_options.argtypes = [vp, C.c_uint64, C.c_int32]
+        L.ipole_load_model_adaf.argtypes = [vp, C.POINTER(AdafParams)]
+        L.ipole_load_model_slab.argtypes = [vp, C.POINTER(SlabParams)]
+        L.ipole_load_model_grid.argtypes = [vp, C.POINTER(GridDesc), C.POINTER(vp)]
+        L.ipole_make_image.argtypes = [vp] + [vp] * 6
+        L.ipole_make_pixels.argtypes = [vp, C.c_int64, vp] + [vp] * 8
+        L.ipole_get_ray_info.argtypes = [vp, vp, vp]
+        L.ipole_get_stats.argtypes = [vp, C.POINTER(Stats)]
+        L.ipole_get_camera_tetrad.argtypes = [vp, dp, dp]
+        L.ipole_trace_pixel.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, dp, dp, dp, C.POINTER(C.c_int32),
+                                        C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+        for name in ("connection", "coefficients", "stokes_step", "bessel", "plasma"):
+            getattr(L, "ipole_eval_" + name).argtypes = [vp, C.c_int64, dp, dp]
+        L.ipole_measure_fp64_peak.argtypes = [vp, dp, C.POINTER(C.c_float)]
+        L.ipole_last_cuda_error.argtypes = [vp]
+        L.ipole_free.argtypes = [vp]
+        L.ipole_free.restype = None
+        L.ipole_strerror.argtypes = [C.c_int]
+        L.ipole_strerror.restype = C.c_char_p
+        L.ipole_version.restype = C.c_char_p
+        _LIB = L
+    return _LIB
+
+
+def _chk(rc, what):
+    if rc < 0:
+        raise IpoleError(rc, what)
+    return rc
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _ptr(t):
+    """data pointer of a torch tensor / numpy array / None"""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        return C.c_void_p(t.ctypes.data)
+    return C.c_void_p(t.data_ptr())
+
+
+class Ipole:
+    """One context: camera + plasma model on the current CUDA device."""
+
+    def __init__(self, **cam):
+        self.cam = Camera()
+        for k, v in cam.items():
+            setattr(self.cam, k, v)
+        self._h = C.c_void_p()
+        _chk(lib().ipole_init(C.byref(self.cam), C.byref(self._h)), "ipole_init")
+        self._keep = None
+
+    # -- lifetime --
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().ipole_free(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def nx(self):
+        return self.cam.nx
+
+    @property
+    def ny(self):
+        return self.cam.ny
+
+    # -- configuration --
+    def set_camera(self, **cam):
+        for k, v in cam.items():
+            setattr(self.cam, k, v)
+        _chk(lib().ipole_set_camera(self._h, C.byref(self.cam)), "ipole_set_camera")
+
+    def set_stream(self, stream=None):
+        """stream: a torch.cuda.Stream (None: torch's current stream)."""
+        import torch
+        s = stream if stream is not None else torch.cuda.current_stream()
+        _chk(lib().ipole_set_stream(self._h, C.c_void_p(s.cuda_stream)), "ipole_set_stream")
+
+    def set_options(self, path_bytes=0, sort_rays=True):
+        _chk(lib().ipole_set_options(self._h, int(path_bytes), 1 if sort_rays else 0), "ipole_set_options")
+
+    def load_adaf(self, n0=1e6, p_n=-1.5, Th0=30.0, p_T=-1.0, B0=30.0, p_B=-1.25):
+        p = AdafParams(n0, p_n, Th0, p_T, B0, p_B)
+        _chk(lib().ipole_load_model_adaf(self._h, C.byref(p)), "ipole_load_model_adaf")
+
+    def load_slab(self, H, j=(0, 0, 0, 0), alpha=(0, 0, 0, 0), rho=(0, 0, 0), psi_deg=0.0, profile=0):
+        p = SlabParams()
+        p.H = H; p.profile = profile; p.psi_deg = psi_deg
+        p.j[:] = list(j); p.alpha[:] = list(alpha); p.rho[:] = list(rho)
+        _chk(lib().ipole_load_model_slab(self._h, C.byref(p)), "ipole_load_model_slab")
+
+    def load_grid(self, desc, fields):
+        """fields: 8 planes (numpy float64 [8,N1,N2,N3] / list of arrays on the host, or torch CUDA tensors)."""
+        g = GridDesc()
+        g.N1, g.N2, g.N3 = desc["N1"], desc["N2"], desc["N3"]
+        g.startx[:] = list(desc["startx"]); g.dx[:] = list(desc["dx"])
+        for k in ("hslope", "gam", "M_unit", "Rlow", "Rhigh", "r_out"):
+            setattr(g, k, desc[k])
+        planes = []
+        for f in fields:
+            if isinstance(f, np.ndarray):
+                f = np.ascontiguousarray(f, dtype=np.float64)
+            else:
+                f = f.contiguous()
+            planes.append(f)
+        ptrs = (C.c_void_p * 8)(*[_ptr(f) for f in planes])
+        _chk(lib().ipole_load_model_grid(self._h, C.byref(g), ptrs), "ipole_load_model_grid")
+
+    # -- the hot path --
+    def make_image(self, maps=False, out=None):
+        """One full-Stokes image on the device.  Returns dict of torch CUDA float64 tensors [ny, nx]
+        (I, Q, U, V and, with maps=True, tau and tauF).  `out` may hold preallocated tensors to reuse."""
+        import torch
+        names = ["I", "Q", "U", "V"] + (["tau", "tauF"] if maps else [])
+        if out is None:
+            out = {k: torch.empty((self.ny, self.nx), dtype=torch.float64, device="cuda") for k in names}
+        args = [_ptr(out.get(k)) for k in ("I", "Q", "U", "V", "tau", "tauF")]
+        _chk(lib().ipole_make_image(self._h, *args), "ipole_make_image")
+        return out
+
+    def make_image_host(self, maps=False, out=None):
+        """Same through HOST buffers (numpy or pinned torch CPU tensors): the library does the copies."""
+        names = ["I", "Q", "U", "V"] + (["tau", "tauF"] if maps else [])
+        if out is None:
+            out = {k: np.empty((self.ny, self.nx), dtype=np.float64) for k in names}
+        args = [_ptr(out.get(k)) for k in ("I", "Q", "U", "V", "tau", "tauF")]
+        _chk(lib().ipole_make_image(self._h, *args), "ipole_make_image")
+        return out
+
+    def make_pixels(self, pixels):
+        """Stokes, maps and ray info for a list of flat pixel indices j*nx+i (host numpy in, host numpy out)."""
+        pix = np.ascontiguousarray(pixels, dtype=np.int64)
+        n = pix.size
+        out = {k: np.zeros(n) for k in ("I", "Q", "U", "V", "tau", "tauF")}
+        out["nsteps"] = np.zeros(n, dtype=np.int32)
+        out["nturn"] = np.zeros(n, dtype=np.int32)
+        args = [_ptr(out[k]) for k in ("I", "Q", "U", "V", "tau", "tauF", "nsteps", "nturn")]
+        _chk(lib().ipole_make_pixels(self._h, n, _ptr(pix), *args), "ipole_make_pixels")
+        return out
+
+    def ray_info(self):
+        n = self.nx * self.ny
+        ns = np.zeros(n, dtype=np.int32); nt = np.zeros(n, dtype=np.int32)
+        _chk(lib().ipole_get_ray_info(self._h, _ptr(ns), _ptr(nt)), "ipole_get_ray_info")
+        return ns.reshape(self.ny, self.nx), nt.reshape(self.ny, self.nx)
+
+    def stats(self):
+        s = Stats()
+        _chk(lib().ipole_get_stats(self._h, C.byref(s)), "ipole_get_stats")
+        d = {k: getattr(s, k) for k, _ in Stats._fields_ if k != "flux_jy"}
+        d["flux_jy"] = [s.flux_jy[i] for i in range(4)]
+        return d
+
+    # -- stages --
+    def camera_tetrad(self):
+        X = np.zeros(4); e = np.zeros((4, 4))
+        _chk(lib().ipole_get_camera_tetrad(self._h, _dp(X), _dp(e)), "ipole_get_camera_tetrad")
+        return X, e
+
+    def trace_pixel(self, i, j, cap=60000):
+        X = np.zeros((cap + 1, 4)); K = np.zeros((cap + 1, 4)); dl = np.zeros(cap)
+        nt = C.c_int32(); st = C.c_int32(); need = C.c_int32()
+        n = _chk(lib().ipole_trace_pixel(self._h, i, j, cap, _dp(X), _dp(K), _dp(dl), C.byref(nt), C.byref(st),
+                                         C.byref(need)), "ipole_trace_pixel")
+        return X[:n + 1].copy(), K[:n + 1].copy(), dl[:n].copy(), nt.value, st.value
+
+    def _eval(self, name, x, nin, nout):
+        a = np.ascontiguousarray(x, dtype=np.float64).reshape(-1, nin)
+        o = np.zeros((a.shape[0], nout))
+        _chk(getattr(lib(), "ipole_eval_" + name)(self._h, a.shape[0], _dp(a), _dp(o)), "ipole_eval_" + name)
+        return o
+
+    def eval_connection(self, X):
+        return self._eval("connection", X, 4, 64).reshape(-1, 4, 4, 4)
+
+    def eval_coefficients(self, ne, thetae, B, cosT, nu):
+        x = np.stack(np.broadcast_arrays(ne, thetae, B, cosT, nu), axis=-1).astype(np.float64)
+        return self._eval("coefficients", x, 5, 8)
+
+    def eval_stokes_step(self, alpha, rho, s, S0, J):
+        x = np.concatenate([np.asarray(alpha, float).reshape(-1, 4), np.asarray(rho, float).reshape(-1, 3),
+                            np.asarray(s, float).reshape(-1, 1), np.asarray(S0, float).reshape(-1, 4),
+                            np.asarray(J, float).reshape(-1, 4)], axis=1)
+        return self._eval("stokes_step", x, 16, 4)
+
+    def eval_bessel(self, z):
+        return self._eval("bessel", z, 1, 3)
+
+    def eval_plasma(self, X):
+        return self._eval("plasma", X, 4, 12)
+
+    def fp64_peak(self):
+        t = C.c_double(); ms = C.c_float()
+        _chk(lib().ipole_measure_fp64_peak(self._h, C.byref(t), C.byref(ms)), "ipole_measure_fp64_peak")
+        return t.value, ms.value
