@@ -1,0 +1,303 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the ipole-b200 hot path (BASELINE.json metric: rays/s and full-Stokes FP64
+images/s at 4096^2; FP64 roofline fraction).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload adaf4096|grid4096|...]
+
+One "step" = one full-Stokes FP64 image of the workload (all rows of SURVEY.md 8(a): camera init, geodesics,
+path storage, plasma model, coefficients, transfer, image write, sort, reduction).  N > 1: one process per GPU
+(torchrun), every rank renders the same workload (rays are independent: weak scaling, no data-path collective);
+`value` = rays of all ranks / max-over-ranks device time.
+
+Prints ONE JSON line (rank 0).  See DESIGN.md section 8 for how every field is derived.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+# FP64 operations per geodesic step of each kernel, counted by ncu on this code (DFMA = 2, DADD/DMUL = 1;
+# smsp__sass_thread_inst_executed_op_d{fma,add,mul}_pred_on.sum / total steps), see profiles/ and DESIGN.md 7.
+FLOP_PER_STEP = {"transfer_adaf": None, "geodesic": None, "transfer_grid": None}
+# ALU roofline denominator: 148 SMs x 4 sub-partitions x 16 FP64 lanes x 2 flop x 1.965 GHz
+FP64_PEAK_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
+
+WORKLOADS = {
+    "adaf4096": dict(kind="adaf", n=4096, config=4),
+    "grid4096": dict(kind="grid", n=4096, config=4, grid=(576, 256, 256)),
+    "grid1024": dict(kind="grid", n=1024, config=3, grid=(576, 256, 256), maps=True),
+    "grid256": dict(kind="grid", n=256, config=2, grid=(288, 128, 128)),
+    "adaf256": dict(kind="adaf", n=256, config=1),
+    "adaf32": dict(kind="adaf", n=32, config=0),
+}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons while the timed region runs (B200_PROFILING.md clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.thread.join(timeout=2)
+        sm, mx, reasons, power = [], [], set(), []
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2])); power.append(float(r[3]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(workload, n_rays, nthreads):
+    """The CPU oracle, as it stands, on a strided sample of the workload's image.  Returns (rays, steps, seconds)."""
+    import numpy as np
+    from oracle import ipole_ref
+    from paper_2302_02733_b200 import workloads as W
+    wl = WORKLOADS[workload]
+    cam = W.camera(wl["kind"], wl["n"])
+    r = ipole_ref.Ctx(**cam)
+    if wl["kind"] == "adaf":
+        r.load_adaf(**W.ADAF)
+    else:
+        desc, fields = W.fm_torus_grid(*wl["grid"])
+        r.load_grid(desc, fields)
+    n = wl["n"]
+    stride = max(1, int(round(n / max(1.0, n_rays ** 0.5))))
+    ii, jj = np.meshgrid(np.arange(stride // 2, n, stride), np.arange(stride // 2, n, stride))
+    pix = (jj * n + ii).ravel().astype(np.int64)
+    t0 = time.perf_counter()
+    r.make_pixels(pix, nthreads=nthreads)
+    dt = time.perf_counter() - t0
+    return pix.size, r.total_steps(), dt, stride
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the box's host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import __graft_entry__ as ge
+    ge.build()
+    wl = WORKLOADS[args.workload]
+    cores = os.cpu_count() or 1
+    n_rays = args.ref_rays
+    for _ in range(args.warmup):
+        oracle_sample(args.workload, min(n_rays, 256), cores)
+    rays = steps = 0
+    dt = 0.0
+    stride = 0
+    for _ in range(args.steps):
+        a, b, c, stride = oracle_sample(args.workload, n_rays, cores)
+        rays += a; steps += b; dt += c
+    val = rays / dt
+    line = {"impl": "reference", "metric": "rays_per_s", "value": val, "unit": "rays/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "configs_index": wl["config"], "image": "%dx%d" % (wl["n"], wl["n"]),
+                       "step": "oracle on every %d-th pixel in x and y (%d rays) of the image" % (stride, rays // args.steps)},
+            "cpu_baseline": {"value": val, "unit": "rays/s", "cores": cores, "kind": "oracle",
+                             "sample": "%d rays per step, strided lattice of the %dx%d image" % (rays // args.steps, wl["n"], wl["n"])},
+            "e2e": {"value": val, "unit": "rays/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "steps_per_s": steps / dt, "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="adaf4096", choices=sorted(WORKLOADS))
+    ap.add_argument("--ref-rays", type=int, default=4096, help="rays per step of the --impl reference arm")
+    ap.add_argument("--cpu-baseline-rays", type=int, default=16384)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        import __graft_entry__ as ge
+        ge.build()
+    if world > 1:
+        dist.barrier()
+    from paper_2302_02733_b200 import ipole, workloads as W
+
+    wl = WORKLOADS[args.workload]
+    cam = W.camera(wl["kind"], wl["n"])
+    g = ipole.Ipole(**cam)
+    g.set_stream(torch.cuda.current_stream())
+    grid_bytes = 0
+    if wl["kind"] == "adaf":
+        g.load_adaf(**W.ADAF)
+    else:
+        desc, fields = W.fm_torus_grid(*wl["grid"])
+        g.load_grid(desc, fields)
+        grid_bytes = fields.nbytes
+    maps = bool(wl.get("maps"))
+    names = ["I", "Q", "U", "V"] + (["tau", "tauF"] if maps else [])
+    out = {k: torch.empty((wl["n"], wl["n"]), dtype=torch.float64, device="cuda") for k in names}
+    rays = wl["n"] * wl["n"]
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        g.make_image(maps=maps, out=out)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stats = []
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        g.make_image(maps=maps, out=out)
+        stats.append(None)
+    ev1.record()
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    st = g.stats()  # of the last timed image (event times are per image)
+    clocks = sampler.stop() if rank == 0 else None
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    value = world * rays * args.steps / (ms * 1e-3)
+
+    # ---- e2e: the C-ABI call with HOST buffers (parameters in, image out), copies inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        host = {k: torch.empty((wl["n"], wl["n"]), dtype=torch.float64).pin_memory() for k in names}
+        hnp = {k: v.numpy() for k, v in host.items()}
+        h2d = 0
+        def one_e2e():
+            nonlocal h2d
+            g.set_camera(**cam)                       # parameters travel host -> device every step
+            h2d = ipole.C.sizeof(ipole.Camera)
+            if wl["kind"] == "adaf":
+                g.load_adaf(**W.ADAF); h2d += ipole.C.sizeof(ipole.AdafParams)
+            g.make_image_host(maps=maps, out=hnp)     # synchronises: outputs are host pointers
+        one_e2e()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            one_e2e()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        dt = float(tt.item())
+        e2e = {"value": world * rays * args.steps / dt, "unit": "rays/s", "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": len(names) * rays * 8,
+               "note": "inputs of this workload are parameters only (analytic model)" if wl["kind"] == "adaf" else
+                       "grid planes (%d bytes) are loaded once by ipole_load_model_grid, outside the step" % grid_bytes}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (k_transfer), live CUDA-event time of the last timed image ----
+    key = "transfer_" + wl["kind"]
+    dfma_tf, _ = g.fp64_peak()
+    n_rt = max(1, st["n_batches"] + (1 if st["n_long"] else 0))
+    rt_ms = st["ms_transfer"]
+    roof = {"bound": "alu", "kernel": "k_transfer<%s>" % wl["kind"], "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+            "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz; DFMA micro-benchmark on this GPU: %.1f" % dfma_tf,
+            "launches": n_rt, "avg_launch_ms": rt_ms / n_rt, "kernel_share_of_step": rt_ms / st["ms_total"],
+            "steps_per_launch": st["total_steps"] / n_rt, "traffic": None}
+    if FLOP_PER_STEP.get(key):
+        ach = FLOP_PER_STEP[key] * st["total_steps"] / (rt_ms * 1e-3) / 1e12
+        roof.update(achieved=ach, frac=ach / FP64_PEAK_TFLOPS, flop_per_step=FLOP_PER_STEP[key])
+    else:
+        roof.update(achieved=None, frac=None)
+    roof["hbm_path_gbs"] = 128.0 * st["total_steps"] / ((st["ms_geodesic"] + st["ms_transfer"]) * 1e-3) / 1e9
+
+    line = {"metric": "rays_per_s", "value": value, "unit": "rays/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "configs_index": wl["config"], "image": "%dx%d" % (wl["n"], wl["n"]),
+                       "model": wl["kind"], "freq_ghz": 230, "eps": cam["eps"], "full_stokes": True, "maps": maps,
+                       "l2": "no flush needed: every batch streams a %.1f GB path buffer (>> 126 MB L2)"
+                             % (st["path_cap"] * 64.0 * min(rays, max(1, rays // max(1, st["n_batches"]))) / 1e9),
+                       "parallelism": "rays sharded: one replica per GPU" if world > 1 else "single GPU"},
+            "images_per_s": value / rays, "steps_per_s": world * st["total_steps"] * args.steps / (ms * 1e-3),
+            "mean_steps_per_ray": st["total_steps"] / rays,
+            "stage_ms": {"probe_sort": st["ms_probe"], "geodesic": st["ms_geodesic"], "transfer": st["ms_transfer"],
+                         "total": st["ms_total"], "batches": st["n_batches"], "path_cap": st["path_cap"],
+                         "long_rays": st["n_long"]},
+            "flux_jy": st["flux_jy"], "lp": st["lp"], "cp": st["cp"], "ring_rays": st["n_ring"],
+            "gpu_launches": st["n_launches"] * args.steps, "roofline": roof, "e2e": e2e, "clocks": clocks,
+            "paper_context": {"note": "paper Table 1, other model/hardware (A100): context only",
+                              "a100_semianalytic_4096_rays_per_s": 127583, "a100_grmhd_4096_rays_per_s": 188720}}
+
+    if not args.no_cpu_baseline and world == 1:
+        cores = os.cpu_count() or 1
+        n, steps, dt, stride = oracle_sample(args.workload, args.cpu_baseline_rays, cores)
+        line["cpu_baseline"] = {"value": n / dt, "unit": "rays/s", "cores": cores, "kind": "oracle",
+                                "sample": "%d rays: every %d-th pixel in x and y of the %dx%d image, %.1f s"
+                                          % (n, stride, wl["n"], wl["n"], dt),
+                                "steps_per_s": steps / dt}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

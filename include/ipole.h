@@ -105,7 +105,8 @@ int  ipole_set_camera(ipole_ctx*, const ipole_camera* cam);
 /* cuda_stream is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = legacy stream. */
 int  ipole_set_stream(ipole_ctx*, void* cuda_stream);
 /* Tunables: path_bytes = size of the geodesic path buffer in HBM (0 => 40% of free memory, at most
- * 64 GiB); sort_rays != 0 orders rays by predicted step count, longest first (default 1). */
+ * 64 GiB); sort_rays: 0 = pixel order, 1 = order rays by predicted step count, longest first, when the image
+ * has >= 32768 rays (default), 2 = always run the probe pass and sort (tests). */
 int  ipole_set_options(ipole_ctx*, uint64_t path_bytes, int32_t sort_rays);
 
 int  ipole_load_model_adaf(ipole_ctx*, const ipole_adaf_params*);

@@ -218,7 +218,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   int cap = max_steps;
   const int32_t* order = nullptr;
   const bool fits_all = (double)n * (double)(max_steps + 1) * (double)rec_bytes <= (double)budget;
-  const bool probe = (n >= 32768) && (c->opt_sort || !fits_all);
+  const bool probe = (n >= 32768 || c->opt_sort == 2) && (c->opt_sort || !fits_all);
 
   if (probe) {
     // ---- probe pass: coarse lattice (or strided list), 4 eps, no path storage ----
@@ -406,7 +406,7 @@ int ipole_set_stream(ipole_ctx* c, void* s) {
 int ipole_set_options(ipole_ctx* c, uint64_t path_bytes, int32_t sort_rays) {
   if (!c) return IPOLE_EINVAL;
   c->opt_path_bytes = path_bytes;
-  c->opt_sort = sort_rays ? 1 : 0;
+  c->opt_sort = (sort_rays == 2) ? 2 : (sort_rays ? 1 : 0);
   return IPOLE_OK;
 }
 

@@ -32,9 +32,15 @@ __device__ __forceinline__ void stokes_step(const double al[4], const double rh[
     for (int i = 0; i < 4; ++i) S[i] = ex * S[i] + E * J[i];
     return;
   }
-  const double im = 1.0 / m;
-  const double a[3] = {al[1] * im, al[2] * im, al[3] * im};
-  const double r[3] = {rh[0] * im, rh[1] * im, rh[2] * im};
+  double a[3], r[3];
+  if (m > 1e-290) {
+    const double im = 1.0 / m;
+    a[0] = al[1] * im; a[1] = al[2] * im; a[2] = al[3] * im;
+    r[0] = rh[0] * im; r[1] = rh[1] * im; r[2] = rh[2] * im;
+  } else {  // 1/m would overflow (coefficients in the subnormal range, e.g. far wings of a Gaussian slab)
+    a[0] = al[1] / m; a[1] = al[2] / m; a[2] = al[3] / m;
+    r[0] = rh[0] / m; r[1] = rh[1] / m; r[2] = rh[2] / m;
+  }
   const double a2 = dot3(a, a), r2 = dot3(r, r), ar = dot3(a, r);
   const double sg = (ar >= 0.0) ? 1.0 : -1.0;
   const double d = 0.5 * (a2 - r2);

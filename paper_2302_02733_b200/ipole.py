@@ -160,7 +160,7 @@ class Ipole:
         _chk(lib().ipole_set_stream(self._h, C.c_void_p(s.cuda_stream)), "ipole_set_stream")
 
     def set_options(self, path_bytes=0, sort_rays=True):
-        _chk(lib().ipole_set_options(self._h, int(path_bytes), 1 if sort_rays else 0), "ipole_set_options")
+        _chk(lib().ipole_set_options(self._h, int(path_bytes), int(sort_rays)), "ipole_set_options")
 
     def load_adaf(self, n0=1e6, p_n=-1.5, Th0=30.0, p_T=-1.0, B0=30.0, p_B=-1.25):
         p = AdafParams(n0, p_n, Th0, p_T, B0, p_B)

@@ -1,0 +1,332 @@
+"""GPU image parity (pytest -m gpu): the CUDA path, called through the C ABI, against the CPU oracle on the same
+seeded synthetic inputs (BASELINE.json configs[0..4]; recipe in DESIGN.md section 5).
+
+Tolerances are the ones BASELINE.json north_star states (FP64):
+  total Stokes I flux relative 1e-9; Q/U/V totals absolute 1e-9 of the I total;
+  per-pixel Stokes relative 1e-7 on >= 99.9 % of pixels (Q,U,V measured against the pixel's I: an error of the
+  polarization fraction); at most 1e-4 on rays crossing the photon ring (>= 2 theta turning points).
+Pixels the oracle leaves exactly dark (no plasma on the ray) must be exactly dark on the GPU.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2302_02733_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+NTHREADS = os.cpu_count() or 1
+
+
+@pytest.fixture(scope="module")
+def ipole():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import __graft_entry__ as ge
+    ge.build()
+    from paper_2302_02733_b200 import ipole as m
+    return m
+
+
+def to_np(img):
+    return {k: v.detach().cpu().numpy().ravel() if hasattr(v, "detach") else np.asarray(v).ravel() for k, v in img.items()}
+
+
+def check_parity(gpu, ref, label, min_lit=0.0):
+    """gpu, ref: dicts of flat arrays over the SAME pixels (I,Q,U,V[,tau,tauF,nsteps,nturn])."""
+    I0 = ref["I"]
+    n = I0.size
+    totI = I0.sum()
+    assert abs(gpu["I"].sum() - totI) <= 1e-9 * abs(totI), (label, "total I", gpu["I"].sum(), totI)
+    for k in "QUV":
+        assert abs(gpu[k].sum() - ref[k].sum()) <= 1e-9 * abs(totI), (label, "total " + k)
+    dark = I0 == 0.0
+    for k in "IQUV":
+        assert (gpu[k][dark] == 0.0).all(), (label, "dark pixels", k)
+    lit = ~dark
+    assert lit.mean() >= min_lit, (label, "lit fraction", lit.mean())
+    err = np.zeros(n)
+    for k in "IQUV":
+        err[lit] = np.maximum(err[lit], np.abs(gpu[k][lit] - ref[k][lit]) / np.abs(I0[lit]))
+    ring = (ref["nturn"] & 0x7f) >= 2
+    ok = err <= 1e-7
+    assert ok.mean() >= 0.999, (label, "pixels within 1e-7", ok.mean(), np.sort(err)[-5:])
+    assert err.max() <= 1e-4, (label, "worst pixel", err.max())
+    if ring.any():
+        assert err[ring].max() <= 1e-4, (label, "ring rays", err[ring].max())
+    # invariant that holds at any size: I >= sqrt(Q^2+U^2+V^2)
+    pol = np.sqrt(gpu["Q"] ** 2 + gpu["U"] ** 2 + gpu["V"] ** 2)
+    assert (pol <= gpu["I"] * (1 + 1e-12) + 1e-300).all(), (label, "I >= sqrt(Q^2+U^2+V^2)")
+    assert (gpu["I"] >= 0).all()
+    if "nsteps" in gpu and "nsteps" in ref:
+        same = gpu["nsteps"] == ref["nsteps"]
+        assert same.mean() >= 0.999 and np.abs(gpu["nsteps"] - ref["nsteps"]).max() <= 1, (label, "nsteps")
+        assert (gpu["nturn"] == ref["nturn"]).mean() >= 0.999, (label, "nturn")
+    for k in ("tau", "tauF"):
+        if k in gpu and k in ref:
+            assert np.allclose(gpu[k], ref[k], rtol=1e-7, atol=1e-300), (label, k)
+    return dict(max_err=float(err.max()), ring_frac=float(ring.mean()), lit=float(lit.mean()))
+
+
+def sample_pixels(nx, ny, stride, window=None):
+    """strided lattice of pixel centres plus every pixel of a window (x0, y0, w, h) that straddles the photon ring"""
+    ii, jj = np.meshgrid(np.arange(stride // 2, nx, stride), np.arange(stride // 2, ny, stride))
+    pix = (jj * nx + ii).ravel()
+    if window:
+        x0, y0, w, h = window
+        wi, wj = np.meshgrid(np.arange(x0, x0 + w), np.arange(y0, y0 + h))
+        pix = np.unique(np.concatenate([pix, (wj * nx + wi).ravel()]))
+    return pix.astype(np.int64)
+
+
+def gpu_full_then_sample(g, pix, maps=True):
+    img = g.make_image(maps=maps)
+    ns, nt = g.ray_info()
+    out = {k: v.detach().cpu().numpy().ravel()[pix] for k, v in img.items()}
+    out["nsteps"] = ns.ravel()[pix]
+    out["nturn"] = nt.ravel()[pix]
+    return out, img
+
+
+# ------------------------------------------------------------------ configs[0]: W1, every pixel
+def test_w1_adaf_32_full_image(ipole, ref):
+    cam = W.camera("adaf", 32)
+    g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
+    r = ref.Ctx(**cam); r.load_adaf(**W.ADAF)
+    want = r.make_pixels(nthreads=NTHREADS)
+    got, img = gpu_full_then_sample(g, np.arange(32 * 32))
+    info = check_parity(got, want, "W1", min_lit=0.99)
+    assert info["max_err"] < 1e-9  # what this scheme actually reaches away from discrete events
+    # the same through HOST buffers (the e2e entry): bit-identical to the device-buffer call
+    host = g.make_image_host(maps=True)
+    for k in host:
+        assert np.array_equal(host[k].ravel(), got[k]), k
+    # a-9: totals from the reduction kernel
+    st = g.stats()
+    L = 6.6742e-8 * 4.1e6 * 1.989e33 / 2.99792458e10 ** 2
+    dom = (cam["fov"] / cam["nx"] * L / (8000.0 * 3.085678e18)) ** 2 * 1e23
+    for q, k in enumerate("IQUV"):
+        assert abs(st["flux_jy"][q] - want[k].sum() * dom) <= 1e-9 * abs(want["I"].sum() * dom)
+    assert st["total_steps"] == int(want["nsteps"].sum()) and st["max_steps_seen"] == int(want["nsteps"].max())
+    assert st["n_ring"] == int(((want["nturn"] & 0x7f) >= 2).sum())
+    assert abs(st["lp"] - np.hypot(want["Q"].sum(), want["U"].sum()) / want["I"].sum()) < 1e-9
+    assert abs(st["cp"] - want["V"].sum() / want["I"].sum()) < 1e-9
+
+
+def test_ragged_image_and_other_camera(ipole, ref):
+    """nx != ny, not a multiple of the warp size, other inclination / frequency / spin / hslope."""
+    cam = W.camera("adaf", 8, freq_hz=345e9, inclination_deg=33.0, spin=0.5, hslope=0.7)
+    cam.update(nx=37, ny=23, fov=30.0)
+    g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
+    r = ref.Ctx(**cam); r.load_adaf(**W.ADAF)
+    want = r.make_pixels(nthreads=NTHREADS)
+    got, _ = gpu_full_then_sample(g, np.arange(37 * 23))
+    check_parity(got, want, "ragged", min_lit=0.99)
+
+
+# ------------------------------------------------------------------ configs[1]: W2, sampled
+@pytest.mark.parametrize("freq", [230e9, 345e9])
+def test_w2_adaf_256_sampled(ipole, ref, freq):
+    cam = W.camera("adaf", 256, freq_hz=freq)
+    g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
+    r = ref.Ctx(**cam); r.load_adaf(**W.ADAF)
+    pix = sample_pixels(256, 256, 8, window=(150, 120, 48, 16))  # the window crosses the ring on the +x side
+    want = r.make_pixels(pix, nthreads=NTHREADS)
+    got, img = gpu_full_then_sample(g, pix)
+    info = check_parity(got, want, "W2 %g" % freq, min_lit=0.99)
+    assert info["ring_frac"] > 0.02
+    # the pixel-list entry point gives bit-identical numbers to the full image
+    lst = g.make_pixels(pix)
+    for k in ("I", "Q", "U", "V", "tau", "tauF", "nsteps", "nturn"):
+        assert np.array_equal(lst[k], got[k]), k
+
+
+# ------------------------------------------------------------------ scheduling must not change a single bit
+def test_batching_sorting_and_long_ray_pass_are_bit_neutral(ipole):
+    cam = W.camera("adaf", 48, max_steps=6000)
+    g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
+    base = to_np(g.make_image(maps=True)); st0 = g.stats()
+    assert st0["n_batches"] == 1 and st0["n_long"] == 0
+    # forced probe + sort, default budget
+    g.set_options(0, 2)
+    a = to_np(g.make_image(maps=True)); st1 = g.stats()
+    assert st1["ms_probe"] > 0
+    # tiny path buffer: many batches; S_cap from the probe
+    g.set_options(24 << 20, 2)
+    b = to_np(g.make_image(maps=True)); st2 = g.stats()
+    assert st2["n_batches"] > 3
+    # no probe and a slot far too small for any ray: every ray goes through the long-ray pass
+    g.set_options(40 << 20, 0)
+    c = to_np(g.make_image(maps=True)); st3 = g.stats()
+    assert st3["n_long"] == 48 * 48 and st3["path_cap"] < 300
+    for other in (a, b, c):
+        for k in base:
+            assert np.array_equal(base[k], other[k]), k
+    for st in (st1, st2, st3):
+        assert st["total_steps"] == st0["total_steps"] and st["flux_jy"] == st0["flux_jy"]
+
+
+def test_step_limit_flags_rays(ipole, ref):
+    cam = W.camera("adaf", 16, max_steps=900)
+    g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
+    r = ref.Ctx(**cam); r.load_adaf(**W.ADAF)
+    want = r.make_pixels(nthreads=NTHREADS)
+    got, _ = gpu_full_then_sample(g, np.arange(256))
+    assert ((want["nturn"] & 0x80) != 0).all() and (got["nturn"] == want["nturn"]).all()
+    assert (got["nsteps"] == 900).all()
+    check_parity(got, want, "max_steps")
+    assert g.stats()["n_maxstep"] == 256
+
+
+def test_edge_cases(ipole):
+    import torch
+    cam = W.camera("adaf", 8)
+    g = ipole.Ipole(**cam)
+    with pytest.raises(ipole.IpoleError) as ei:
+        g.make_image()
+    assert ei.value.code == ipole.ENOMODEL
+    g.load_adaf(**W.ADAF)
+    with pytest.raises(ipole.IpoleError) as ei:
+        g.stats()
+    assert ei.value.code == ipole.ENOIMAGE
+    assert g.make_pixels(np.zeros(0, dtype=np.int64))["I"].size == 0          # empty list
+    with pytest.raises(ipole.IpoleError):
+        g.make_pixels(np.array([64], dtype=np.int64))                          # pixel out of range
+    # mixed host/device outputs are rejected
+    I = torch.empty((8, 8), dtype=torch.float64, device="cuda")
+    with pytest.raises(ipole.IpoleError):
+        g.make_image(out=dict(I=I, Q=np.empty((8, 8)), U=I.clone(), V=I.clone()))
+    # 1x1 image, and a camera swap on a live context
+    g.set_camera(nx=1, ny=1)
+    one = to_np(g.make_image())
+    assert one["I"].size == 1 and np.isfinite(one["I"]).all()
+    # a user stream
+    s = torch.cuda.Stream()
+    g.set_camera(nx=8, ny=8)
+    ref_img = to_np(g.make_image())
+    with torch.cuda.stream(s):
+        g.set_stream(s)
+        img = g.make_image()
+    s.synchronize()
+    for k in ref_img:
+        assert np.array_equal(ref_img[k], to_np(img)[k])
+    # flat metric refuses the ADAF flow (defined on Kerr only)
+    with pytest.raises(ipole.IpoleError):
+        g.set_camera(flat_metric=1)
+
+
+# ------------------------------------------------------------------ slab in flat space: closed forms through the whole pipeline
+def _slab_cam(n=16):
+    return W.camera("adaf", n, spin=0.0, flat_metric=1, inclination_deg=40.0, fov=2.0, r_cam=500.0, r_esc=500.0)
+
+
+def test_slab_flat_space_closed_forms(ipole, ref):
+    L = 6.6742e-8 * 4.1e6 * 1.989e33 / 2.99792458e10 ** 2
+    cam = _slab_cam()
+    H = 2.0
+    path = 2 * H / np.cos(np.radians(40.0)) * L  # every ray crosses the slab at the same angle in flat space (to O(fov/r_cam))
+    g = ipole.Ipole(**cam); r = ref.Ctx(**cam)
+    # T3 optically thin emission: I = j * path
+    j = 1e-20
+    for c in (g, r):
+        c.load_slab(H, j=(j, 0, 0, 0))
+    img = to_np(g.make_image()); want = r.make_pixels(nthreads=NTHREADS)
+    assert np.allclose(img["I"], j * path, rtol=5e-3, atol=0)  # closed form (pin-hole camera: angles differ by ~fov/r_cam)
+    assert np.abs(img["I"] - want["I"]).max() <= 1e-9 * want["I"].max()
+    # T4 absorption with emission: I = (j/a)(1 - exp(-a path))
+    a = 3.0 / path
+    for c in (g, r):
+        c.load_slab(H, j=(j, 0, 0, 0), alpha=(a, 0, 0, 0))
+    img = to_np(g.make_image(maps=True)); want = r.make_pixels(nthreads=NTHREADS)
+    assert np.allclose(img["I"], j / a * (1 - np.exp(-a * path)), rtol=5e-3, atol=0)
+    assert np.allclose(img["tau"], 3.0, rtol=5e-3, atol=0)
+    assert np.abs(img["I"] - want["I"]).max() <= 1e-9 * want["I"].max()
+    # T5/T6 Faraday rotation and conversion with polarized emission, all coefficients (incl. the U ones) non-zero
+    kw = dict(H=H, j=(j, 0.3 * j, -0.2 * j, 0.1 * j), alpha=(a, 0.2 * a, 0.1 * a, -0.05 * a), rho=(4 * a, -2 * a, 9 * a),
+              psi_deg=20.0, profile=1)
+    for c in (g, r):
+        c.load_slab(**kw)
+    got, _ = gpu_full_then_sample(g, np.arange(256))
+    want = r.make_pixels(nthreads=NTHREADS)
+    check_parity(got, want, "slab", min_lit=1.0)
+
+
+# ------------------------------------------------------------------ configs[2..4]: grid model
+@pytest.fixture(scope="module")
+def small_grid():
+    return W.fm_torus_grid(72, 32, 32)
+
+
+def test_grid_small_full_image(ipole, ref, small_grid):
+    desc, fields = small_grid
+    cam = W.camera("grid", 32)
+    g = ipole.Ipole(**cam); g.load_grid(desc, fields)
+    r = ref.Ctx(**cam); r.load_grid(desc, fields)
+    want = r.make_pixels(nthreads=NTHREADS)
+    got, _ = gpu_full_then_sample(g, np.arange(1024))
+    info = check_parity(got, want, "grid small", min_lit=0.2)
+    assert info["lit"] < 1.0  # the corners see no plasma: exercises the dark-pixel path
+    # grid planes given as DEVICE pointers (torch tensors) give the same image
+    import torch
+    g2 = ipole.Ipole(**cam)
+    g2.load_grid(desc, [torch.from_numpy(np.ascontiguousarray(f)).cuda() for f in fields])
+    img2 = to_np(g2.make_image(maps=True))
+    for k in img2:
+        assert np.array_equal(img2[k], got[k])
+
+
+def test_w3_grid_256_sampled(ipole, ref):
+    desc, fields = W.fm_torus_grid(288, 128, 128)
+    cam = W.camera("grid", 256)
+    g = ipole.Ipole(**cam); g.load_grid(desc, fields)
+    r = ref.Ctx(**cam); r.load_grid(desc, fields)
+    pix = sample_pixels(256, 256, 8, window=(140, 124, 40, 8))
+    want = r.make_pixels(pix, nthreads=NTHREADS)
+    got, _ = gpu_full_then_sample(g, pix)
+    check_parity(got, want, "W3", min_lit=0.3)
+
+
+# ------------------------------------------------------------------ full sizes, in the configuration bench.py times
+def test_w5_adaf_4096_sampled(ipole, ref):
+    cam = W.camera("adaf", 4096)
+    g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
+    r = ref.Ctx(**cam); r.load_adaf(**W.ADAF)
+    pix = sample_pixels(4096, 4096, 128, window=(2400, 2040, 256, 2))
+    want = r.make_pixels(pix, nthreads=NTHREADS)
+    got, img = gpu_full_then_sample(g, pix, maps=False)
+    info = check_parity(got, want, "W5 adaf", min_lit=0.99)
+    st = g.stats()
+    assert st["n_batches"] >= 1 and st["n_maxstep"] == 0
+    # properties of the whole 4096^2 image
+    import torch
+    pol = torch.sqrt(img["Q"] ** 2 + img["U"] ** 2 + img["V"] ** 2)
+    assert bool((pol <= img["I"] * (1 + 1e-12)).all()) and bool(torch.isfinite(img["I"]).all())
+    assert abs(st["flux_jy"][0] / (float(img["I"].sum()) * (40.0 / 4096 * 6.6742e-8 * 4.1e6 * 1.989e33 / 2.99792458e10 ** 2
+                                                             / (8000.0 * 3.085678e18)) ** 2 * 1e23) - 1) < 1e-12
+
+
+@pytest.fixture(scope="module")
+def big_grid():
+    return W.fm_torus_grid(576, 256, 256)
+
+
+def test_w4_grid_1024_sampled_with_maps(ipole, ref, big_grid):
+    desc, fields = big_grid
+    cam = W.camera("grid", 1024)
+    g = ipole.Ipole(**cam); g.load_grid(desc, fields)
+    r = ref.Ctx(**cam); r.load_grid(desc, fields)
+    pix = sample_pixels(1024, 1024, 32, window=(560, 508, 128, 4))
+    want = r.make_pixels(pix, nthreads=NTHREADS)
+    got, _ = gpu_full_then_sample(g, pix, maps=True)
+    check_parity(got, want, "W4", min_lit=0.3)
+
+
+def test_w5_grid_4096_sampled(ipole, ref, big_grid):
+    desc, fields = big_grid
+    cam = W.camera("grid", 4096)
+    g = ipole.Ipole(**cam); g.load_grid(desc, fields)
+    r = ref.Ctx(**cam); r.load_grid(desc, fields)
+    pix = sample_pixels(4096, 4096, 128, window=(2240, 2040, 256, 2))
+    want = r.make_pixels(pix, nthreads=NTHREADS)
+    got, _ = gpu_full_then_sample(g, pix, maps=False)
+    check_parity(got, want, "W5 grid", min_lit=0.3)
