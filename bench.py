@@ -34,6 +34,7 @@ WORKLOADS = {
     "grid4096": dict(kind="grid", n=4096, config=4, grid=(576, 256, 256)),
     "grid1024": dict(kind="grid", n=1024, config=3, grid=(576, 256, 256), maps=True),
     "grid256": dict(kind="grid", n=256, config=2, grid=(288, 128, 128)),
+    "adaf1024": dict(kind="adaf", n=1024, config=None),   # profiling size (ncu --set full replays each kernel ~40x)
     "adaf256": dict(kind="adaf", n=256, config=1),
     "adaf32": dict(kind="adaf", n=32, config=0),
 }
@@ -172,7 +173,7 @@ def main():
         ge.build()
     if world > 1:
         dist.barrier()
-    from paper_2302_02733_b200 import ipole, workloads as W
+    from paper_2302_02733_b200 import ipole, replicas, workloads as W
 
     wl = WORKLOADS[args.workload]
     cam = W.camera(wl["kind"], wl["n"])
@@ -213,11 +214,8 @@ def main():
     ms = ev0.elapsed_time(ev1)
     st = g.stats()  # of the last timed image (event times are per image)
     clocks = sampler.stop() if rank == 0 else None
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
-    value = world * rays * args.steps / (ms * 1e-3)
+    ms = replicas.max_over_ranks(ms, "cuda")
+    value = replicas.job_throughput(rays * args.steps, ms * 1e-3, world)
 
     # ---- e2e: the C-ABI call with HOST buffers (parameters in, image out), copies inside the timed region ----
     e2e = None
@@ -239,11 +237,8 @@ def main():
             one_e2e()
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        dt = float(tt.item())
-        e2e = {"value": world * rays * args.steps / dt, "unit": "rays/s", "h2d_bytes_per_step": h2d,
+        dt = replicas.max_over_ranks(dt, "cuda")
+        e2e = {"value": replicas.job_throughput(rays * args.steps, dt, world), "unit": "rays/s", "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": len(names) * rays * 8,
                "note": "inputs of this workload are parameters only (analytic model)" if wl["kind"] == "adaf" else
                        "grid planes (%d bytes) are loaded once by ipole_load_model_grid, outside the step" % grid_bytes}
