@@ -67,46 +67,117 @@ __device__ __forceinline__ void bessel_k01_scaled(double z, double& k0, double& 
   }
 }
 
+static_assert(IPOLE_BESSEL_K0_NC == IPOLE_BESSEL_K1_NC, "the two Chebyshev series are evaluated interleaved");
+
 struct Coeff { double jI, jQ, jV, aI, aQ, aV, rQ, rV; };
 
 __device__ __forceinline__ double finite_or_zero(double v) { return isfinite(v) ? v : 0.0; }
 
-// plasma-frame cgs coefficients at frequency nu; cosT = cosine of the angle between wave vector and field
-__device__ __forceinline__ Coeff synchrotron_coefficients(double ne, double Th, double B, double cosT, double nu) {
+// K_0(z)/K_2(z) and K_1(z)/K_2(z): the e^z scaling of bessel_k01_scaled cancels in the ratios, so the series branch
+// skips it here.
+__device__ __forceinline__ void bessel_ratios(double z, double Th, double& r0, double& r1) {
+  double k0, k1;
+  if (z <= 2.0) {
+    const double EUL = 0.57721566490153286061;
+    const double t = 0.25 * z * z;
+    const double lg = log(0.5 * z);
+    double term0 = 1.0, term1 = 1.0, Hk = 0.0;
+    double i0 = 1.0, s0 = 0.0, i1 = 1.0, s1 = 1.0 - 2.0 * EUL;
+#pragma unroll
+    for (int k = 1; k <= 13; ++k) {
+      const double ik = 1.0 / (double)k, ik1 = 1.0 / (double)(k + 1);  // folded at compile time
+      Hk += ik;
+      term0 *= t * (ik * ik);
+      term1 *= t * (ik * ik1);
+      i0 += term0;
+      s0 = fma(term0, Hk, s0);
+      i1 += term1;
+      s1 = fma(term1, 2.0 * Hk + ik1 - 2.0 * EUL, s1);
+    }
+    k0 = s0 - (lg + EUL) * i0;
+    k1 = Th + (0.5 * z) * (lg * i1 - 0.5 * s1);
+  } else {
+    const double xi = 4.0 * Th - 1.0, x2 = 2.0 * xi;
+    double b1 = 0.0, b2 = 0.0, d1 = 0.0, d2 = 0.0;  // Clenshaw, the two series interleaved
+#pragma unroll
+    for (int j = IPOLE_BESSEL_K0_NC - 1; j >= 1; --j) {
+      const double b0 = fma(x2, b1, c_bessel_k0[j] - b2); b2 = b1; b1 = b0;
+      const double d0 = fma(x2, d1, c_bessel_k1[j] - d2); d2 = d1; d1 = d0;
+    }
+    k0 = fma(xi, b1, c_bessel_k0[0] - b2);   // common factor rsqrt(z) cancels in the ratios
+    k1 = fma(xi, d1, c_bessel_k1[0] - d2);
+  }
+  const double ik2 = 1.0 / fma(2.0 * Th, k1, k0);
+  r0 = k0 * ik2;
+  r1 = k1 * ik2;
+}
+
+// constants of the fits, folded at compile time (R-7)
+#define IP_SQRT3 1.7320508075688772935
+#define IP_C_NUC  (3.0 * IP_EE / (4.0 * M_PI * IP_ME * IP_CL))                 /* nu_c = C B sinT Th^2       */
+#define IP_C_PRE  (IP_EE * IP_EE / (2.0 * IP_SQRT3 * IP_CL))                   /* j prefactor / (ne nu/Th^2) */
+#define IP_C_HKT  (IP_HPL / (IP_ME * IP_CL * IP_CL))                           /* h nu / (me c^2 Th)         */
+#define IP_C_IBNU (IP_CL * IP_CL / (2.0 * IP_HPL))                             /* 1/B_nu = C expm1(.)/nu^3   */
+#define IP_C_NUB  (IP_EE / (2.0 * M_PI * IP_ME * IP_CL))
+#define IP_C_RV   (IP_EE * IP_EE * IP_EE / (M_PI * IP_ME * IP_ME * IP_CL * IP_CL))
+#define IP_C_RQ   (IP_EE * IP_EE * IP_EE * IP_EE / (4.0 * M_PI * M_PI * IP_ME * IP_ME * IP_ME * IP_CL * IP_CL * IP_CL))
+
+// INVARIANT: jI,jQ,jV are j/nu^2; aI,aQ,aV are alpha*nu; rQ,rV are rho*nu (R-1), the form the transfer
+// step consumes; otherwise plain plasma-frame cgs coefficients (the form the stage parity test compares).  cosT = cosine of the angle between wave vector and field.  Divisions are replaced by a few
+// shared reciprocals (1/nu, 1/Th, 1/nu_c, cube root reciprocal), pow(X,p) by exp(p ln X).
+template <bool INVARIANT>
+__device__ __forceinline__ Coeff synchrotron(double ne, double Th, double B, double cosT, double nu) {
   Coeff c;
   c.jI = c.jQ = c.jV = c.aI = c.aQ = c.aV = c.rQ = c.rV = 0.0;
   const double sin2 = 1.0 - cosT * cosT;
   if (!(sin2 > 0.0) || !(ne > 0.0) || !(B > 0.0) || !(Th > 0.0)) return c;
-  const double sinT = sqrt(sin2);
-  const double nuc = 3.0 * IP_EE * B * sinT * Th * Th / (4.0 * M_PI * IP_ME * IP_CL);
+  const double isinT = rsqrt(sin2), sinT = sin2 * isinT;
+  const double inu = 1.0 / nu, iTh = 1.0 / Th;
+  const double BsT = B * sinT;
+  const double nuc = IP_C_NUC * BsT * (Th * Th);
   const double x = nu / nuc;
-  const double y = cbrt(x);
-  const double iy = 1.0 / y;
+  const double iy = rcbrt(x), iy2 = iy * iy;
+  const double y = x * iy2;
   const double ex = exp(-1.8899 * y);
-  const double FI = 2.5651 * (1.0 + 1.92 * iy + 0.9977 * iy * iy) * ex;
-  const double FQ = 2.5651 * (1.0 + 0.93193 * iy + 0.499873 * iy * iy) * ex;
-  const double FV = (1.81348 / x + 3.42319 * iy * iy + 0.0292545 * rsqrt(x) + 2.03773 * iy) * ex;
-  const double pre = ne * IP_EE * IP_EE * nu / (2.0 * sqrt(3.0) * IP_CL * Th * Th);
+  const double FI = 2.5651 * fma(fma(0.9977, iy, 1.92), iy, 1.0) * ex;
+  const double FQ = 2.5651 * fma(fma(0.499873, iy, 0.93193), iy, 1.0) * ex;
+  const double FV = (1.81348 * (iy2 * iy) + 3.42319 * iy2 + 0.0292545 * rsqrt(x) + 2.03773 * iy) * ex;
+  // j = C ne nu / Th^2 F
+  const double pre0 = IP_C_PRE * ne * (iTh * iTh);
+  const double pre = pre0 * (INVARIANT ? inu : nu);
+  const double FVc = (4.0 / 3.0) * iTh * (cosT * isinT) * FV;
   c.jI = pre * FI;
   c.jQ = pre * FQ;
-  c.jV = 2.0 * ne * IP_EE * IP_EE * nu * (cosT / sinT) / (3.0 * sqrt(3.0) * IP_CL * Th * Th * Th) * FV;
-  const double iBnu = expm1(IP_HPL * nu / (IP_ME * IP_CL * IP_CL * Th)) / (2.0 * IP_HPL * nu * nu * nu / (IP_CL * IP_CL));
-  c.aI = c.jI * iBnu;
-  c.aQ = c.jQ * iBnu;
-  c.aV = c.jV * iBnu;
-  double k0, k1;
-  bessel_k01_scaled(1.0 / Th, k0, k1);
-  const double k2 = k0 + 2.0 * Th * k1;
-  const double nuB = IP_EE * B / (2.0 * M_PI * IP_ME * IP_CL);
-  const double X = Th * sqrt(sqrt(2.0) * sinT * 1e3 * nuB / nu);
-  const double fX = 2.011 * exp(-pow(X, 1.035) / 4.7) - cos(0.5 * X) * exp(-pow(X, 1.2) / 2.73) - 0.011 * exp(-X / 47.2);
-  c.rV = ne * IP_EE * IP_EE * IP_EE * B * cosT / (M_PI * IP_ME * IP_ME * IP_CL * IP_CL * nu * nu) * (k0 / k2);
-  c.rQ = ne * IP_EE * IP_EE * IP_EE * IP_EE * B * B * sin2
-         / (4.0 * M_PI * M_PI * IP_ME * IP_ME * IP_ME * IP_CL * IP_CL * IP_CL * nu * nu * nu) * fX * (k1 / k2 + 6.0 * Th);
+  c.jV = pre * FVc;
+  // alpha = j / B_nu = j C expm1(h nu / (me c^2 Th)) / nu^3; the prefactors are multiplied first so that alpha
+  // keeps full precision where j/nu^2 itself is subnormal (far Wien tail)
+  const double prea = pre0 * (INVARIANT ? inu : inu * inu) * (IP_C_IBNU * expm1(IP_C_HKT * nu * iTh));
+  // Kirchhoff's law is applied to the emissivity as computed: where the cgs emissivity underflows to zero the
+  // absorptivity is zero too (R-7: alpha_S = j_S / B_nu)
+  const double prec = INVARIANT ? pre0 * nu : pre;
+  c.aI = (prec * FI != 0.0) ? prea * FI : 0.0;
+  c.aQ = (prec * FQ != 0.0) ? prea * FQ : 0.0;
+  c.aV = (prec * FVc != 0.0) ? prea * FVc : 0.0;
+  double r0, r1;
+  bessel_ratios(iTh, Th, r0, r1);
+  const double X = Th * sqrt((1.4142135623730950488e3 * IP_C_NUB) * BsT * inu);
+  const double lX = log(X);
+  const double fX = 2.011 * exp(-(1.0 / 4.7) * exp(1.035 * lX)) - cos(0.5 * X) * exp(-(1.0 / 2.73) * exp(1.2 * lX))
+                    - 0.011 * exp(-(1.0 / 47.2) * X);
+  const double neinu = ne * (INVARIANT ? inu : inu * inu);
+  c.rV = IP_C_RV * neinu * B * cosT * r0;
+  c.rQ = IP_C_RQ * neinu * inu * (BsT * BsT) * fX * (r1 + 6.0 * Th);
   c.jI = finite_or_zero(c.jI); c.jQ = finite_or_zero(c.jQ); c.jV = finite_or_zero(c.jV);
   c.aI = finite_or_zero(c.aI); c.aQ = finite_or_zero(c.aQ); c.aV = finite_or_zero(c.aV);
   c.rQ = finite_or_zero(c.rQ); c.rV = finite_or_zero(c.rV);
   return c;
+}
+
+__device__ __forceinline__ Coeff synchrotron_invariant(double ne, double Th, double B, double cosT, double nu) {
+  return synchrotron<true>(ne, Th, B, cosT, nu);
+}
+__device__ __forceinline__ Coeff synchrotron_coefficients(double ne, double Th, double B, double cosT, double nu) {
+  return synchrotron<false>(ne, Th, B, cosT, nu);
 }
 
 }  // namespace ipole

@@ -44,7 +44,7 @@ struct Inv6 {
 };
 
 struct Point {      // scalar functions of position shared by everything evaluated at X
-  double r, th, tp, tpp, s, c, Sig, f, sqrtmg;
+  double r, th, tp, tpp, s, c, Sig, f, sqrtmg, iSig;
 };
 
 __device__ __forceinline__ void theta_map(const Geom& G, double x2, double& th, double& tp, double& tpp) {
@@ -80,14 +80,19 @@ __device__ __forceinline__ void metric(const Geom& G, const double X[4], Point& 
   g.c33 = s2 * (p.Sig + a * a * s2 * opf);
   p.sqrtmg = r * p.tp * p.Sig * fabs(p.s);
   if (WANT_INV) {
-    const double iS = 1.0 / p.Sig, ir = 1.0 / r;
+    // one reciprocal of the product instead of four: 1/Sigma, 1/r, 1/sin^2, 1/theta'^2
+    const double tp2 = p.tp * p.tp;
+    const double Sr = p.Sig * r, st = s2 * tp2;
+    const double t = 1.0 / (Sr * st);
+    const double iS = t * r * st, ir = t * p.Sig * st, iSst = t * r;   // iSst = 1/(Sigma sin^2 theta'^2)
     const double Del = r * r - 2.0 * G.mass * r + a * a;
     gi.c00 = -opf;
     gi.c01 = f * ir;
     gi.c11 = Del * iS * ir * ir;
     gi.c13 = a * iS * ir;
-    gi.c22 = iS / (p.tp * p.tp);
-    gi.c33 = iS / s2;
+    gi.c22 = iSst * s2;
+    gi.c33 = iSst * tp2;
+    p.iSig = iS;
   }
 }
 
@@ -97,7 +102,7 @@ __device__ __forceinline__ void metric_derivs(const Geom& G, const double X[4], 
   metric<true>(G, X, p, g, gi);
   const double a = G.a, r = p.r, s2 = p.s * p.s, f = p.f, opf = 1.0 + f;
   const double a2 = a * a;
-  const double iS2 = 1.0 / (p.Sig * p.Sig);
+  const double iS2 = p.iSig * p.iSig;
   const double fr1 = r * 2.0 * G.mass * (a2 * p.c * p.c - r * r) * iS2;  // r df/dr
   const double cs2 = 2.0 * p.s * p.c * p.tp;                             // theta' d(sin^2)/dtheta
   const double ft2 = 2.0 * G.mass * r * a2 * cs2 * iS2;                  // theta' df/dtheta

@@ -112,6 +112,7 @@ int apply_camera(ipole_ctx* c, const ipole_camera* k) {
   c->units.nu_obs = k->freq_hz;
   c->units.L_unit = IP_GNEWT * M / (IP_CL * IP_CL);
   c->units.D_cm = (k->dsource_pc > 0.0 ? k->dsource_pc : 8000.0) * IP_PC;
+  c->units.dl_unit = c->units.L_unit / c->units.nu_obs;
   c->have_image = false;
   return IPOLE_OK;
 }

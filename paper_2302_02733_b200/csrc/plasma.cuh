@@ -26,7 +26,7 @@ struct GridParams {
   double ne_unit, B_unit;        // rho -> n_e [cm^-3], sqrt(b.b) -> Gauss
   const double* f[8];            // device planes rho,u,U1,U2,U3,B1,B2,B3
 };
-struct Units { double nu_obs, L_unit, D_cm; };
+struct Units { double nu_obs, L_unit, D_cm, dl_unit; };  // dl_unit = L_unit / nu_obs
 
 struct Plasma {
   double ne, Th, B;
@@ -239,22 +239,22 @@ __device__ __forceinline__ bool plasma_operator(const Geom& G, const void* model
   const double nu = om * U.nu_obs;
   double ji[4], ai[4], ri[3];
   if (MODEL == MODEL_SLAB) {
+    const double inu = 1.0 / nu, inu2 = inu * inu;
 #pragma unroll
-    for (int i = 0; i < 4; ++i) { ji[i] = P.j[i] / (nu * nu); ai[i] = P.al[i] * nu; }
+    for (int i = 0; i < 4; ++i) { ji[i] = P.j[i] * inu2; ai[i] = P.al[i] * nu; }
 #pragma unroll
     for (int i = 0; i < 3; ++i) ri[i] = P.rh[i] * nu;
   } else {
     double bcov[4];
     g.mul(P.b, bcov);
-    double cosT = dot4(bcov, K) / (om * P.B);
+    double cosT = dot4(bcov, K) * iom / P.B;
     cosT = fmin(1.0, fmax(-1.0, cosT));
-    const Coeff c = synchrotron_coefficients(P.ne, P.Th, P.B, cosT, nu);
-    const double inu2 = 1.0 / (nu * nu);
-    ji[0] = c.jI * inu2; ji[1] = c.jQ * inu2; ji[2] = 0.0; ji[3] = c.jV * inu2;
-    ai[0] = c.aI * nu;   ai[1] = c.aQ * nu;   ai[2] = 0.0; ai[3] = c.aV * nu;
-    ri[0] = c.rQ * nu;   ri[1] = 0.0;         ri[2] = c.rV * nu;
+    const Coeff c = synchrotron_invariant(P.ne, P.Th, P.B, cosT, nu);
+    ji[0] = c.jI; ji[1] = c.jQ; ji[2] = 0.0; ji[3] = c.jV;
+    ai[0] = c.aI; ai[1] = c.aQ; ai[2] = 0.0; ai[3] = c.aV;
+    ri[0] = c.rQ; ri[1] = 0.0;  ri[2] = c.rV;
   }
-  const double ds = dl * U.L_unit / U.nu_obs;
+  const double ds = dl * U.dl_unit;
   // project the carried state on the new transverse legs: M_{a'a} = e^(a')_mu f_a^mu
   stokes_congruence(dot4(e1c, st.f1), dot4(e1c, st.f2), dot4(e2c, st.f1), dot4(e2c, st.f2), st.S);
   stokes_step(ai, ri, ds, ji, st.S);

@@ -13,8 +13,6 @@
 
 namespace ipole {
 
-__device__ __forceinline__ double exp_integral(double b, double s) { return (b == 0.0) ? s : -expm1(-b * s) / b; }
-
 __device__ __forceinline__ void cross3(const double u[3], const double v[3], double o[3]) {
   o[0] = u[1] * v[2] - u[2] * v[1];
   o[1] = u[2] * v[0] - u[0] * v[2];
@@ -23,11 +21,17 @@ __device__ __forceinline__ void cross3(const double u[3], const double v[3], dou
 __device__ __forceinline__ double dot3(const double u[3], const double v[3]) { return u[0] * v[0] + u[1] * v[1] + u[2] * v[2]; }
 
 // S <- O(s) S + P(s) J ; al = (aI,aQ,aU,aV), rh = (rQ,rU,rV)
+//
+// Transcendentals per call: three expm1 and one sincos.  With tp = expm1(-(aI-L1)s), tm = expm1(-(aI+L1)s),
+// t0 = expm1(-aI s):  e^{-aI s} cosh(L1 s) = 1 + (tp+tm)/2,  e^{-aI s} sinh(L1 s) = (tp-tm)/2,
+// E(aI -+ L1) = -t{p,m}/(aI -+ L1),  1 - cos x = sin^2 x / (1 + cos x) for cos x > 0.
 __device__ __forceinline__ void stokes_step(const double al[4], const double rh[3], double s, const double J[4], double S[4]) {
   const double aI = al[0];
   const double m = fmax(fmax(fabs(al[1]), fmax(fabs(al[2]), fabs(al[3]))), fmax(fabs(rh[0]), fmax(fabs(rh[1]), fabs(rh[2]))));
+  const double t0 = expm1(-aI * s);
+  const double ex = 1.0 + t0;
   if (m == 0.0) {
-    const double ex = exp(-aI * s), E = exp_integral(aI, s);
+    const double E = (aI == 0.0) ? s : -t0 / aI;
 #pragma unroll
     for (int i = 0; i < 4; ++i) S[i] = ex * S[i] + E * J[i];
     return;
@@ -44,41 +48,47 @@ __device__ __forceinline__ void stokes_step(const double al[4], const double rh[
   const double a2 = dot3(a, a), r2 = dot3(r, r), ar = dot3(a, r);
   const double sg = (ar >= 0.0) ? 1.0 : -1.0;
   const double d = 0.5 * (a2 - r2);
-  const double q = sqrt(d * d + ar * ar);
-  double l1, l2;
-  if (d >= 0.0) { l1 = sqrt(q + d); l2 = (l1 > 0.0) ? fabs(ar) / l1 : 0.0; }
-  else          { l2 = sqrt(q - d); l1 = (l2 > 0.0) ? fabs(ar) / l2 : 0.0; }
-  const double iTh = 1.0 / (l1 * l1 + l2 * l2);
+  const double q = sqrt(d * d + ar * ar);          // >= max scaled component^2 / 2 > 0
+  // the larger of l1, l2 from the root (>= 1/sqrt 2 after scaling), the other from l1 l2 = |a.r|
+  const double big2 = q + fabs(d);
+  const double ibig = rsqrt(big2);
+  const double big = big2 * ibig, small = fabs(ar) * ibig;
+  const double l1 = (d >= 0.0) ? big : small, l2 = (d >= 0.0) ? small : big;
+  const double iTh = 0.5 / q;                      // Theta = l1^2 + l2^2 = 2 q
   const double L1 = m * l1, L2 = m * l2;
   const double hh = 0.5 * (a2 + r2);
+  const double sl1 = sg * l1, sl2 = sg * l2;
   double v2[3], w2[3], v3[3], w3[3], cr[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    v2[i] = l2 * a[i] - sg * l1 * r[i];
-    w2[i] = sg * l1 * a[i] + l2 * r[i];
-    v3[i] = l1 * a[i] + sg * l2 * r[i];
-    w3[i] = -sg * l2 * a[i] + l1 * r[i];
+    v2[i] = l2 * a[i] - sl1 * r[i];
+    w2[i] = sl1 * a[i] + l2 * r[i];
+    v3[i] = l1 * a[i] + sl2 * r[i];
+    w3[i] = l1 * r[i] - sl2 * a[i];
   }
   cross3(r, a, cr);
 
-  const double ex = exp(-aI * s);
   double sn, c;
   sincos(L2 * s, &sn, &c);
-  const double ch = cosh(L1 * s), sh = sinh(L1 * s);
-  const double Ep = exp_integral(aI - L1, s), Em = exp_integral(aI + L1, s);
+  const double bp = aI - L1, bm = aI + L1;
+  const double tp = expm1(-bp * s), tm = expm1(-bm * s);
+  const double exch = 1.0 + 0.5 * (tp + tm), exsh = 0.5 * (tp - tm);
+  const double Ep = (bp == 0.0) ? s : -tp / bp, Em = (bm == 0.0) ? s : -tm / bm;
   const double Ic1 = 0.5 * (Ep + Em), Is1 = 0.5 * (Ep - Em);
   double Ic2, Is2;
   const double den = aI * aI + L2 * L2;
   if (den == 0.0) { Ic2 = s; Is2 = 0.0; }
   else {
-    const double em1 = expm1(-aI * s), hs = sin(0.5 * L2 * s);
-    const double re = -(em1 * c - 2.0 * hs * hs);
+    const double omc = (c > 0.0) ? sn * sn / (1.0 + c) : 1.0 - c;   // 1 - cos(L2 s)
+    const double re = omc - t0 * c;                                  // Re(1 - e^{-aI s} e^{i L2 s})
     const double im2 = -ex * sn;
-    Ic2 = (re * aI - im2 * L2) / den;
-    Is2 = (re * L2 + im2 * aI) / den;
+    const double nc = re * aI - im2 * L2, ns = re * L2 + im2 * aI;
+    if (den > 1e-280) { const double iden = 1.0 / den; Ic2 = nc * iden; Is2 = ns * iden; }
+    else { Ic2 = nc / den; Is2 = ns / den; }   // 1/den would overflow (coefficients near the subnormal range)
   }
   // weights of (1, M2, M3, M4) for O and for P
-  const double o1 = ex * 0.5 * (ch + c), o2 = -ex * sn, o3 = -ex * sh, o4 = ex * 0.5 * (ch - c);
+  const double exc = ex * c;
+  const double o1 = 0.5 * (exch + exc), o2 = -ex * sn, o3 = -exsh, o4 = 0.5 * (exch - exc);
   const double p1 = 0.5 * (Ic1 + Ic2), p2 = -Is2, p3 = -Is1, p4 = 0.5 * (Ic1 - Ic2);
 
   double out[4] = {0.0, 0.0, 0.0, 0.0};
