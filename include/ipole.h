@@ -146,6 +146,9 @@ int  ipole_eval_connection(ipole_ctx*, int64_t n, const double* X, double* Gamma
 int  ipole_eval_coefficients(ipole_ctx*, int64_t n, const double* in5, double* out8);
 int  ipole_eval_stokes_step(ipole_ctx*, int64_t n, const double* in16, double* out4);
 int  ipole_eval_bessel(ipole_ctx*, int64_t n, const double* z, double* out3);
+/* The branch-free elementary functions of the hot loops (csrc/fpmath.cuh) at n points x (host):
+ * out[n][8] = exp(x), expm1(x), ln|x|, sin(x), cos(x), 1/x, 1/sqrt|x|, sqrt|x|.  Domains: see fpmath.cuh. */
+int  ipole_eval_math(ipole_ctx*, int64_t n, const double* x, double* out8);
 /* Plasma state of the loaded model at n points X[n][4] (host): out[n][12] = present, ne, thetae, B, u[4], b[4]. */
 int  ipole_eval_plasma(ipole_ctx*, int64_t n, const double* X, double* out12);
 

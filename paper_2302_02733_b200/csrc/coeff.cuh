@@ -30,7 +30,7 @@ __device__ __forceinline__ void bessel_k01_scaled(double z, double& k0, double& 
     // K1 = 1/z + ln(z/2) I1 - (z/4) sum_{k>=0} (psi(k+1)+psi(k+2)) t^k/(k!(k+1)!)
     const double EUL = 0.57721566490153286061;
     const double t = 0.25 * z * z;
-    const double lg = log(0.5 * z);
+    const double lg = ip_log(0.5 * z);
     double term0 = 1.0;   // t^k/(k!)^2
     double term1 = 1.0;   // t^k/(k!(k+1)!)
     double Hk = 0.0;      // harmonic number H_k
@@ -47,7 +47,7 @@ __device__ __forceinline__ void bessel_k01_scaled(double z, double& k0, double& 
       i1 += term1;
       s1 += term1 * (2.0 * Hk + 1.0 / (double)(k + 1) - 2.0 * EUL);  // psi(k+1)+psi(k+2)
     }
-    const double ez = exp(z);
+    const double ez = ip_exp(z);
     k0 = ez * (-(lg + EUL) * i0 + s0);
     k1 = ez * (1.0 / z + lg * (0.5 * z) * i1 - 0.25 * z * s1);
   } else {
@@ -80,7 +80,7 @@ __device__ __forceinline__ void bessel_ratios(double z, double Th, double& r0, d
   if (z <= 2.0) {
     const double EUL = 0.57721566490153286061;
     const double t = 0.25 * z * z;
-    const double lg = log(0.5 * z);
+    const double lg = ip_log(0.5 * z);
     double term0 = 1.0, term1 = 1.0, Hk = 0.0;
     double i0 = 1.0, s0 = 0.0, i1 = 1.0, s1 = 1.0 - 2.0 * EUL;
 #pragma unroll
@@ -117,7 +117,7 @@ __device__ __forceinline__ void bessel_ratios(double z, double Th, double& r0, d
 #define IP_C_NUC  (3.0 * IP_EE / (4.0 * M_PI * IP_ME * IP_CL))                 /* nu_c = C B sinT Th^2       */
 #define IP_C_PRE  (IP_EE * IP_EE / (2.0 * IP_SQRT3 * IP_CL))                   /* j prefactor / (ne nu/Th^2) */
 #define IP_C_HKT  (IP_HPL / (IP_ME * IP_CL * IP_CL))                           /* h nu / (me c^2 Th)         */
-#define IP_C_IBNU (IP_CL * IP_CL / (2.0 * IP_HPL))                             /* 1/B_nu = C expm1(.)/nu^3   */
+#define IP_C_IBNU (IP_CL * IP_CL / (2.0 * IP_HPL))                             /* 1/B_nu = C ip_expm1(.)/nu^3   */
 #define IP_C_NUB  (IP_EE / (2.0 * M_PI * IP_ME * IP_CL))
 #define IP_C_RV   (IP_EE * IP_EE * IP_EE / (M_PI * IP_ME * IP_ME * IP_CL * IP_CL))
 #define IP_C_RQ   (IP_EE * IP_EE * IP_EE * IP_EE / (4.0 * M_PI * M_PI * IP_ME * IP_ME * IP_ME * IP_CL * IP_CL * IP_CL))
@@ -138,7 +138,7 @@ __device__ __forceinline__ Coeff synchrotron(double ne, double Th, double B, dou
   const double x = nu / nuc;
   const double iy = rcbrt(x), iy2 = iy * iy;
   const double y = x * iy2;
-  const double ex = exp(-1.8899 * y);
+  const double ex = ip_exp(-1.8899 * y);
   const double FI = 2.5651 * fma(fma(0.9977, iy, 1.92), iy, 1.0) * ex;
   const double FQ = 2.5651 * fma(fma(0.499873, iy, 0.93193), iy, 1.0) * ex;
   const double FV = (1.81348 * (iy2 * iy) + 3.42319 * iy2 + 0.0292545 * rsqrt(x) + 2.03773 * iy) * ex;
@@ -151,7 +151,7 @@ __device__ __forceinline__ Coeff synchrotron(double ne, double Th, double B, dou
   c.jV = pre * FVc;
   // alpha = j / B_nu = j C expm1(h nu / (me c^2 Th)) / nu^3; the prefactors are multiplied first so that alpha
   // keeps full precision where j/nu^2 itself is subnormal (far Wien tail)
-  const double prea = pre0 * (INVARIANT ? inu : inu * inu) * (IP_C_IBNU * expm1(IP_C_HKT * nu * iTh));
+  const double prea = pre0 * (INVARIANT ? inu : inu * inu) * (IP_C_IBNU * ip_expm1(IP_C_HKT * nu * iTh));
   // Kirchhoff's law is applied to the emissivity as computed: where the cgs emissivity underflows to zero the
   // absorptivity is zero too (R-7: alpha_S = j_S / B_nu)
   const double prec = INVARIANT ? pre0 * nu : pre;
@@ -161,9 +161,9 @@ __device__ __forceinline__ Coeff synchrotron(double ne, double Th, double B, dou
   double r0, r1;
   bessel_ratios(iTh, Th, r0, r1);
   const double X = Th * sqrt((1.4142135623730950488e3 * IP_C_NUB) * BsT * inu);
-  const double lX = log(X);
-  const double fX = 2.011 * exp(-(1.0 / 4.7) * exp(1.035 * lX)) - cos(0.5 * X) * exp(-(1.0 / 2.73) * exp(1.2 * lX))
-                    - 0.011 * exp(-(1.0 / 47.2) * X);
+  const double lX = ip_log(X);
+  const double fX = 2.011 * ip_exp(-(1.0 / 4.7) * ip_exp(1.035 * lX)) - ip_cos_any(0.5 * X) * ip_exp(-(1.0 / 2.73) * ip_exp(1.2 * lX))
+                    - 0.011 * ip_exp(-(1.0 / 47.2) * X);
   const double neinu = ne * (INVARIANT ? inu : inu * inu);
   c.rV = IP_C_RV * neinu * B * cosT * r0;
   c.rQ = IP_C_RQ * neinu * inu * (BsT * BsT) * fX * (r1 + 6.0 * Th);

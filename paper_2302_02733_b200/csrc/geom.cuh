@@ -12,6 +12,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <math.h>
+#include "fpmath.cuh"
 
 namespace ipole {
 
@@ -52,7 +53,7 @@ __device__ __forceinline__ void theta_map(const Geom& G, double x2, double& th, 
     th = M_PI * x2; tp = M_PI; tpp = 0.0;
   } else {
     double s2, c2;
-    sincos(2.0 * M_PI * x2, &s2, &c2);
+    ip_sincos(2.0 * M_PI * x2, &s2, &c2);
     const double q = 1.0 - G.hslope;
     th = M_PI * x2 + 0.5 * q * s2;
     tp = M_PI * (1.0 + q * c2);
@@ -64,9 +65,9 @@ __device__ __forceinline__ void theta_map(const Geom& G, double x2, double& th, 
 template <bool WANT_INV>
 __device__ __forceinline__ void metric(const Geom& G, const double X[4], Point& p, Sym7& g, Inv6& gi) {
   const double a = G.a;
-  p.r = exp(X[1]);
+  p.r = ip_exp(X[1]);
   theta_map(G, X[2], p.th, p.tp, p.tpp);
-  sincos(p.th, &p.s, &p.c);
+  ip_sincos(p.th, &p.s, &p.c);
   const double r = p.r, s2 = p.s * p.s;
   p.Sig = r * r + a * a * p.c * p.c;
   p.f = 2.0 * G.mass * r / p.Sig;

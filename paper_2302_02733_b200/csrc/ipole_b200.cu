@@ -633,6 +633,9 @@ int ipole_eval_stokes_step(ipole_ctx* c, int64_t n, const double* in16, double* 
 int ipole_eval_bessel(ipole_ctx* c, int64_t n, const double* z, double* out3) {
   return eval_host(c, n, z, 1, out3, 3, [&](int g, int b, double* i, double* o) { k_eval_bessel<<<g, b, 0, c->stream>>>(n, i, o); });
 }
+int ipole_eval_math(ipole_ctx* c, int64_t n, const double* x, double* out8) {
+  return eval_host(c, n, x, 1, out8, 8, [&](int g, int b, double* i, double* o) { k_eval_math<<<g, b, 0, c->stream>>>(n, i, o); });
+}
 int ipole_eval_plasma(ipole_ctx* c, int64_t n, const double* X, double* out12) {
   if (!c) return IPOLE_EINVAL;
   if (c->model == MODEL_NONE) return IPOLE_ENOMODEL;

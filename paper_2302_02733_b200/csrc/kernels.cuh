@@ -248,6 +248,12 @@ struct RtArgs {
 #ifndef IPOLE_RT_MINB
 #define IPOLE_RT_MINB 2
 #endif
+#ifndef IPOLE_RT_SYNC
+#define IPOLE_RT_SYNC 0
+#endif
+#ifndef IPOLE_RT_PREFETCH
+#define IPOLE_RT_PREFETCH 0
+#endif
 
 // a-4 ... a-7, a-8.  Lane-level refill as in k_geodesic.  Per step: midpoint (Xm, Km), generator A = Gamma.Km,
 // f <- P f, plasma operator, f <- P f  (Strang splitting, R-6).
@@ -292,9 +298,19 @@ __global__ void __launch_bounds__(IPOLE_RT_THREADS, IPOLE_RT_MINB) k_transfer(co
   };
 
   fetch();
+#if IPOLE_RT_SYNC
+  // one barrier per step keeps the warps of a block within one iteration of each other, so that they share the
+  // instruction-cache lines of the (large) loop body
+  while (__syncthreads_or(have)) {
+    if (!have) continue;
+#else
   while (have) {
+#endif
     double Xlo[4], Klo[4], dl;
     load_record(rec + (size_t)s * REC_DOUBLES, Xlo, Klo, dl);
+#if IPOLE_RT_PREFETCH
+    if (s > 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(rec + (size_t)(s - 1) * REC_DOUBLES));
+#endif
     double Xm[4], Km[4];
 #pragma unroll
     for (int m = 0; m < 4; ++m) { Xm[m] = 0.5 * (Xlo[m] + Xhi[m]); Km[m] = 0.5 * (Klo[m] + Khi[m]); }
@@ -505,6 +521,15 @@ __global__ void k_eval_bessel(int64_t n, const double* z, double* out) {
   double k0, k1;
   bessel_k01_scaled(z[i], k0, k1);
   out[3 * i] = k0; out[3 * i + 1] = k1; out[3 * i + 2] = k0 + 2.0 / z[i] * k1;
+}
+__global__ void k_eval_math(int64_t n, const double* x, double* out) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double v = x[i];
+  double* o = out + 8 * i;
+  o[0] = ip_exp(v); o[1] = ip_expm1(v); o[2] = ip_log(fabs(v));
+  ip_sincos_any(v, &o[3], &o[4]);
+  o[5] = ip_rcp(v); o[6] = ip_rsqrt(fabs(v)); o[7] = ip_sqrt(fabs(v));
 }
 template <int MODEL>
 __global__ void k_eval_plasma(Geom G, const void* model, int64_t n, const double* X, double* out) {

@@ -43,9 +43,9 @@ __device__ __forceinline__ double dotg(const Sym7& g, const double u[4], const d
 __device__ __forceinline__ bool plasma_adaf(const Geom& G, const AdafParams& M, const double X[4], const Point& p,
                                             const Sym7& g, const Inv6& gi, Plasma& P) {
   const double a = G.a, r = p.r;
-  P.ne = M.n0 * exp(M.p_n * X[1]);
-  P.Th = M.Th0 * exp(M.p_T * X[1]);
-  P.B = M.B0 * exp(M.p_B * X[1]);
+  P.ne = M.n0 * ip_exp(M.p_n * X[1]);
+  P.Th = M.Th0 * ip_exp(M.p_T * X[1]);
+  P.B = M.B0 * ip_exp(M.p_B * X[1]);
   if (r >= M.r_isco) {
     const double Om = 1.0 / (r * sqrt(r) + a);
     const double ut = rsqrt(-(g.c00 + 2.0 * g.c03 * Om + g.c33 * Om * Om));
@@ -70,10 +70,10 @@ __device__ __forceinline__ bool plasma_slab(const Geom& G, const SlabParams& M, 
   const double z = r * c;
   double w = 1.0;
   if (M.profile == 0) { if (!(fabs(z) < M.H)) return false; }
-  else w = exp(-z * z / (2.0 * M.H * M.H));
+  else w = ip_exp(-z * z / (2.0 * M.H * M.H));
   P.u[0] = rsqrt(-g.c00); P.u[1] = P.u[2] = P.u[3] = 0.0;
   double sp, cp;
-  sincos(X[3], &sp, &cp);
+  ip_sincos_any(X[3], &sp, &cp);
   // d(x,y,z)/d(r,theta,phi) of x = (r cos ph - a sin ph) sin th, y = (r sin ph + a cos ph) sin th, z = r cos th
   const double J[3][3] = {{cp * s, (r * cp - a * sp) * c, (-r * sp - a * cp) * s},
                           {sp * s, (r * sp + a * cp) * c, (r * cp - a * sp) * s},

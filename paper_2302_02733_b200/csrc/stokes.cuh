@@ -28,7 +28,7 @@ __device__ __forceinline__ double dot3(const double u[3], const double v[3]) { r
 __device__ __forceinline__ void stokes_step(const double al[4], const double rh[3], double s, const double J[4], double S[4]) {
   const double aI = al[0];
   const double m = fmax(fmax(fabs(al[1]), fmax(fabs(al[2]), fabs(al[3]))), fmax(fabs(rh[0]), fmax(fabs(rh[1]), fabs(rh[2]))));
-  const double t0 = expm1(-aI * s);
+  const double t0 = ip_expm1(-aI * s);
   const double ex = 1.0 + t0;
   if (m == 0.0) {
     const double E = (aI == 0.0) ? s : -t0 / aI;
@@ -69,9 +69,9 @@ __device__ __forceinline__ void stokes_step(const double al[4], const double rh[
   cross3(r, a, cr);
 
   double sn, c;
-  sincos(L2 * s, &sn, &c);
+  ip_sincos_any(L2 * s, &sn, &c);
   const double bp = aI - L1, bm = aI + L1;
-  const double tp = expm1(-bp * s), tm = expm1(-bm * s);
+  const double tp = ip_expm1(-bp * s), tm = ip_expm1(-bm * s);
   const double exch = 1.0 + 0.5 * (tp + tm), exsh = 0.5 * (tp - tm);
   const double Ep = (bp == 0.0) ? s : -tp / bp, Em = (bm == 0.0) ? s : -tm / bm;
   const double Ic1 = 0.5 * (Ep + Em), Is1 = 0.5 * (Ep - Em);

@@ -21,7 +21,7 @@ SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_opti
            "ipole_load_model_slab", "ipole_load_model_grid", "ipole_make_image", "ipole_make_pixels",
            "ipole_get_ray_info", "ipole_get_stats", "ipole_get_camera_tetrad", "ipole_trace_pixel",
            "ipole_eval_connection", "ipole_eval_coefficients", "ipole_eval_stokes_step", "ipole_eval_bessel",
-           "ipole_eval_plasma", "ipole_measure_fp64_peak", "ipole_last_cuda_error", "ipole_free", "ipole_strerror",
+           "ipole_eval_plasma", "ipole_eval_math", "ipole_measure_fp64_peak", "ipole_last_cuda_error", "ipole_free", "ipole_strerror",
            "ipole_version"]
 
 
@@ -84,7 +84,7 @@ def lib():
         L.ipole_get_camera_tetrad.argtypes = [vp, dp, dp]
         L.ipole_trace_pixel.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, dp, dp, dp, C.POINTER(C.c_int32),
                                         C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
-        for name in ("connection", "coefficients", "stokes_step", "bessel", "plasma"):
+        for name in ("connection", "coefficients", "stokes_step", "bessel", "plasma", "math"):
             getattr(L, "ipole_eval_" + name).argtypes = [vp, C.c_int64, dp, dp]
         L.ipole_measure_fp64_peak.argtypes = [vp, dp, C.POINTER(C.c_float)]
         L.ipole_last_cuda_error.argtypes = [vp]
@@ -268,6 +268,10 @@ class Ipole:
 
     def eval_bessel(self, z):
         return self._eval("bessel", z, 1, 3)
+
+    def eval_math(self, x):
+        """exp, expm1, ln|x|, sin, cos, 1/x, 1/sqrt|x|, sqrt|x| of csrc/fpmath.cuh"""
+        return self._eval("math", x, 1, 8)
 
     def eval_plasma(self, X):
         return self._eval("plasma", X, 4, 12)

@@ -157,3 +157,37 @@ def test_fp64_peak_microbenchmark(ipole):
     g = ipole.Ipole(**W.camera("adaf", 8))
     tf, ms = g.fp64_peak()
     assert 10.0 < tf < 60.0 and ms > 0
+
+
+def test_fpmath_against_mpmath(ipole):
+    """The branch-free elementary functions of csrc/fpmath.cuh (exp, expm1, log, sincos, rcp, rsqrt, sqrt) against
+    40-digit mpmath values: <= 2 ulp on the domains stated there, exact limits at the ends."""
+    import mpmath as mp
+    mp.mp.dps = 40
+    g = ipole.Ipole(**W.camera("adaf", 8))
+    rng = np.random.default_rng(17)
+    x = np.concatenate([rng.uniform(-745, 709, 600), rng.uniform(-2, 2, 600), 10 ** rng.uniform(-300, -1, 300),
+                        -10 ** rng.uniform(-300, -1, 300), rng.uniform(-1e5, 1e5, 600), 10 ** rng.uniform(-280, 280, 600),
+                        [0.5, 1.0, 2.0, np.sqrt(2.0), 1.0 / np.sqrt(2.0), 1e-300, -1e-300, 709.0, -745.0, -708.4, 1e5]])
+    out = g.eval_math(x)
+    ulp = lambda got, want: np.abs(got - want) / np.spacing(np.abs(want))
+    f = lambda fn, v: np.array([float(fn(mp.mpf(float(t)))) for t in v])
+    m = x <= 709
+    assert ulp(out[m, 0], f(mp.exp, x[m])).max() <= 2.0                       # includes the subnormal range below -708
+    assert ulp(out[m, 1], f(mp.expm1, x[m])).max() <= 2.0
+    nz = np.abs(x) > 1e-290
+    assert ulp(out[nz, 2], f(mp.log, np.abs(x[nz]))).max() <= 2.0
+    m = np.abs(x) <= 1e5
+    # sin/cos: absolute error <= 1 ulp of 1 near the zeros of the function, <= 2 ulp elsewhere
+    for col, fn in ((3, mp.sin), (4, mp.cos)):
+        want = f(fn, x[m])
+        assert (np.abs(out[m, col] - want) <= 2.0 * np.maximum(np.spacing(np.abs(want)), 1e-22)).all()
+    big = np.array([1e6, 1e9, 3e15])
+    ob = g.eval_math(big)
+    assert np.abs(ob[:, 3] - np.sin(big)).max() < 1e-15 and np.abs(ob[:, 4] - np.cos(big)).max() < 1e-15  # library fallback
+    m = (np.abs(x) > 1e-290) & (np.abs(x) < 1e290)
+    assert ulp(out[m, 5], 1.0 / x[m]).max() <= 1.0
+    assert ulp(out[m, 6], f(lambda t: 1 / mp.sqrt(t), np.abs(x[m]))).max() <= 2.0
+    assert ulp(out[m, 7], np.sqrt(np.abs(x[m]))).max() <= 1.0
+    edge = g.eval_math(np.array([-np.inf, -1e4, -800.0]))
+    assert (edge[:, 0] == 0).all() and (edge[:, 1] == -1).all()
