@@ -107,7 +107,7 @@ __device__ __forceinline__ void bessel_ratios(double z, double Th, double& r0, d
     k0 = fma(xi, b1, c_bessel_k0[0] - b2);   // common factor rsqrt(z) cancels in the ratios
     k1 = fma(xi, d1, c_bessel_k1[0] - d2);
   }
-  const double ik2 = 1.0 / fma(2.0 * Th, k1, k0);
+  const double ik2 = ip_rcp(fma(2.0 * Th, k1, k0));
   r0 = k0 * ik2;
   r1 = k1 * ik2;
 }
@@ -131,17 +131,17 @@ __device__ __forceinline__ Coeff synchrotron(double ne, double Th, double B, dou
   c.jI = c.jQ = c.jV = c.aI = c.aQ = c.aV = c.rQ = c.rV = 0.0;
   const double sin2 = 1.0 - cosT * cosT;
   if (!(sin2 > 0.0) || !(ne > 0.0) || !(B > 0.0) || !(Th > 0.0)) return c;
-  const double isinT = rsqrt(sin2), sinT = sin2 * isinT;
-  const double inu = 1.0 / nu, iTh = 1.0 / Th;
+  const double isinT = ip_rsqrt(sin2), sinT = sin2 * isinT;
+  const double inu = ip_rcp(nu), iTh = ip_rcp(Th);
   const double BsT = B * sinT;
   const double nuc = IP_C_NUC * BsT * (Th * Th);
-  const double x = nu / nuc;
+  const double x = ip_div(nu, nuc);
   const double iy = rcbrt(x), iy2 = iy * iy;
   const double y = x * iy2;
   const double ex = ip_exp(-1.8899 * y);
   const double FI = 2.5651 * fma(fma(0.9977, iy, 1.92), iy, 1.0) * ex;
   const double FQ = 2.5651 * fma(fma(0.499873, iy, 0.93193), iy, 1.0) * ex;
-  const double FV = (1.81348 * (iy2 * iy) + 3.42319 * iy2 + 0.0292545 * rsqrt(x) + 2.03773 * iy) * ex;
+  const double FV = (1.81348 * (iy2 * iy) + 3.42319 * iy2 + 0.0292545 * ip_rsqrt(x) + 2.03773 * iy) * ex;
   // j = C ne nu / Th^2 F
   const double pre0 = IP_C_PRE * ne * (iTh * iTh);
   const double pre = pre0 * (INVARIANT ? inu : nu);
@@ -160,7 +160,7 @@ __device__ __forceinline__ Coeff synchrotron(double ne, double Th, double B, dou
   c.aV = (prec * FVc != 0.0) ? prea * FVc : 0.0;
   double r0, r1;
   bessel_ratios(iTh, Th, r0, r1);
-  const double X = Th * sqrt((1.4142135623730950488e3 * IP_C_NUB) * BsT * inu);
+  const double X = Th * ip_sqrt((1.4142135623730950488e3 * IP_C_NUB) * BsT * inu);
   const double lX = ip_log(X);
   const double fX = 2.011 * ip_exp(-(1.0 / 4.7) * ip_exp(1.035 * lX)) - ip_cos_any(0.5 * X) * ip_exp(-(1.0 / 2.73) * ip_exp(1.2 * lX))
                     - 0.011 * ip_exp(-(1.0 / 47.2) * X);

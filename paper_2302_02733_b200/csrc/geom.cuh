@@ -84,7 +84,7 @@ __device__ __forceinline__ void metric(const Geom& G, const double X[4], Point& 
     // one reciprocal of the product instead of four: 1/Sigma, 1/r, 1/sin^2, 1/theta'^2
     const double tp2 = p.tp * p.tp;
     const double Sr = p.Sig * r, st = s2 * tp2;
-    const double t = 1.0 / (Sr * st);
+    const double t = ip_rcp(Sr * st);
     const double iS = t * r * st, ir = t * p.Sig * st, iSst = t * r;   // iSst = 1/(Sigma sin^2 theta'^2)
     const double Del = r * r - 2.0 * G.mass * r + a * a;
     gi.c00 = -opf;

@@ -111,12 +111,12 @@ __device__ __forceinline__ void pixel_ray(const CamDev& C, int64_t pix, double X
   }
 }
 
-__device__ __forceinline__ double stepsize(const double X[4], const double K[4], double eps) {
+// 1/dl = (|K1|+d)/eps + (|K2|+d)/(eps min(X2,1-X2)) + (|K3|+d)/eps ; ieps = 1/eps
+__device__ __forceinline__ double stepsize(const double X[4], const double K[4], double ieps) {
   const double d = 1e-40;
-  const double i1 = (fabs(K[1]) + d) / eps;
-  const double i2 = (fabs(K[2]) + d) / (eps * fabs(fmin(X[2], 1.0 - X[2])));
-  const double i3 = (fabs(K[3]) + d) / eps;
-  return 1.0 / (i1 + i2 + i3);
+  const double i13 = (fabs(K[1]) + d) + (fabs(K[3]) + d);
+  const double i2 = (fabs(K[2]) + d) * ip_rcp(fabs(fmin(X[2], 1.0 - X[2])));
+  return ip_rcp((i13 + i2) * ieps);
 }
 
 // classical RK4 on (X^1..3, K^0..3); X^0 is not integrated (static snapshot, R-9)
@@ -140,7 +140,7 @@ __device__ __forceinline__ void rk4_push(const Geom& G, double X[4], double K[4]
 #pragma unroll
   for (int m = 0; m < 4; ++m) { Kt[m] = K[m] + h * k3[m]; }
   geodesic_accel(G, Xt, Kt, k4);
-  const double h6 = h / 6.0;
+  const double h6 = h * (1.0 / 6.0);
 #pragma unroll
   for (int m = 1; m < 4; ++m) X[m] += h6 * (xs[m] + Kt[m]);
 #pragma unroll
@@ -199,9 +199,10 @@ __global__ void __launch_bounds__(IPOLE_GEO_THREADS, IPOLE_GEO_MINB) k_geodesic(
     n = 0; nt = 0;
   };
 
+  const double ieps = 1.0 / A.eps;
   fetch();
   while (have) {
-    const double dl = stepsize(X, K, A.eps);
+    const double dl = stepsize(X, K, ieps);
     if (rec) store_record(rec + (size_t)n * REC_DOUBLES, X, K, dl);
     const double x1_before = X[1];
     const bool k2neg = K[2] < 0.0;

@@ -47,18 +47,18 @@ __device__ __forceinline__ bool plasma_adaf(const Geom& G, const AdafParams& M, 
   P.Th = M.Th0 * ip_exp(M.p_T * X[1]);
   P.B = M.B0 * ip_exp(M.p_B * X[1]);
   if (r >= M.r_isco) {
-    const double Om = 1.0 / (r * sqrt(r) + a);
-    const double ut = rsqrt(-(g.c00 + 2.0 * g.c03 * Om + g.c33 * Om * Om));
+    const double Om = ip_rcp(r * ip_sqrt(r) + a);
+    const double ut = ip_rsqrt(-(g.c00 + 2.0 * g.c03 * Om + g.c33 * Om * Om));
     P.u[0] = ut; P.u[1] = 0.0; P.u[2] = 0.0; P.u[3] = ut * Om;
   } else {
-    const double ur_ks = -2.0 * r / (2.0 * r + sqrt(2.0 * r * (r * r + a * a)));
+    const double ur_ks = -2.0 * r * ip_rcp(2.0 * r + ip_sqrt(2.0 * r * (r * r + a * a)));
     const double ucov[4] = {-1.0, r * ur_ks, 0.0, 0.0};
     gi.mul(ucov, P.u);
   }
   // d_phi projected orthogonal to u, scaled to b.b = B^2
   const double tu = g.c03 * P.u[0] + g.c13 * P.u[1] + g.c33 * P.u[3];
   double bb[4] = {tu * P.u[0], tu * P.u[1], tu * P.u[2], 1.0 + tu * P.u[3]};
-  const double sc = P.B * rsqrt(dotg(g, bb, bb));
+  const double sc = P.B * ip_rsqrt(dotg(g, bb, bb));
 #pragma unroll
   for (int m = 0; m < 4; ++m) P.b[m] = bb[m] * sc;
   return true;
@@ -134,12 +134,12 @@ __device__ __forceinline__ bool plasma_grid(const Geom& G, const GridParams& M, 
   }
   const double rho = prim[0], uu = prim[1];
   if (!(rho > 0.0) || !(uu > 0.0)) return false;
-  const double alpha_l = rsqrt(-gi.c00);
+  const double alpha_l = ip_rsqrt(-gi.c00);
   // q2 = g_ij U^i U^j (spatial block of the sparse metric)
   const double U1 = prim[2], U2 = prim[3], U3 = prim[4];
   const double q2 = g.c11 * U1 * U1 + 2.0 * g.c13 * U1 * U3 + g.c22 * U2 * U2 + g.c33 * U3 * U3;
-  const double gamma = sqrt(1.0 + q2);
-  P.u[0] = gamma / alpha_l;
+  const double gamma = ip_sqrt(1.0 + q2);
+  P.u[0] = gamma * ip_sqrt(-gi.c00);
   P.u[1] = U1 - gamma * alpha_l * gi.c01;
   P.u[2] = U2;
   P.u[3] = U3;
@@ -149,17 +149,18 @@ __device__ __forceinline__ bool plasma_grid(const Geom& G, const GridParams& M, 
   const double bt = B1 * ul[1] + B2 * ul[2] + B3 * ul[3];
   double bc[4];
   bc[0] = bt;
-  bc[1] = (B1 + bt * P.u[1]) / P.u[0];
-  bc[2] = (B2 + bt * P.u[2]) / P.u[0];
-  bc[3] = (B3 + bt * P.u[3]) / P.u[0];
+  const double iu0 = ip_rcp(P.u[0]);
+  bc[1] = (B1 + bt * P.u[1]) * iu0;
+  bc[2] = (B2 + bt * P.u[2]) * iu0;
+  bc[3] = (B3 + bt * P.u[3]) * iu0;
   const double bsq = dotg(g, bc, bc);
   if (!(bsq > 0.0)) return false;
   P.ne = rho * M.ne_unit;
-  P.B = sqrt(bsq) * M.B_unit;
-  const double beta = (M.gam - 1.0) * uu / (0.5 * bsq);
+  P.B = ip_sqrt(bsq) * M.B_unit;
+  const double beta = 2.0 * (M.gam - 1.0) * uu * ip_rcp(bsq);
   const double b2 = beta * beta;
-  const double R = (M.Rhigh * b2 + M.Rlow) / (1.0 + b2);
-  P.Th = (IP_MP / IP_ME) * (M.gam - 1.0) * (uu / rho) / (1.0 + R);
+  const double R = (M.Rhigh * b2 + M.Rlow) * ip_rcp(1.0 + b2);
+  P.Th = (IP_MP / IP_ME) * (M.gam - 1.0) * uu * ip_rcp(rho * (1.0 + R));
 #pragma unroll
   for (int m = 0; m < 4; ++m) P.b[m] = bc[m] * M.B_unit;
   return true;
@@ -212,13 +213,13 @@ __device__ __forceinline__ bool plasma_operator(const Geom& G, const void* model
   const double om = -dot4(kcov, P.u);
   if (!(om > 0.0)) return false;
   double e3[4], e2[4], e1[4], e3c[4], e2c[4], e1c[4];
-  const double iom = 1.0 / om;
+  const double iom = ip_rcp(om);
 #pragma unroll
   for (int m = 0; m < 4; ++m) e3[m] = K[m] * iom - P.u[m];
   g.mul(e3, e3c);
   const double n3 = dot4(e3c, e3);
-  if (!(n3 > 0.0)) return false;
-  const double i3 = rsqrt(n3);
+  if (!(n3 > 1e-280)) return false;
+  const double i3 = ip_rsqrt(n3);
 #pragma unroll
   for (int m = 0; m < 4; ++m) { e3[m] *= i3; e3c[m] *= i3; }
   const double be3 = dot4(e3c, P.b);
@@ -226,12 +227,12 @@ __device__ __forceinline__ bool plasma_operator(const Geom& G, const void* model
   for (int m = 0; m < 4; ++m) e2[m] = P.b[m] - be3 * e3[m];
   g.mul(e2, e2c);
   const double n2 = dot4(e2c, e2);
-  if (!(n2 > 0.0)) return false;
-  const double i2 = rsqrt(n2);
+  if (!(n2 > 1e-280)) return false;
+  const double i2 = ip_rsqrt(n2);
 #pragma unroll
   for (int m = 0; m < 4; ++m) { e2[m] *= i2; e2c[m] *= i2; }
   levi4(ucov, e2c, e3c, e1);
-  const double isg = 1.0 / p.sqrtmg;
+  const double isg = ip_rcp(p.sqrtmg);
 #pragma unroll
   for (int m = 0; m < 4; ++m) e1[m] *= isg;
   g.mul(e1, e1c);
@@ -239,7 +240,7 @@ __device__ __forceinline__ bool plasma_operator(const Geom& G, const void* model
   const double nu = om * U.nu_obs;
   double ji[4], ai[4], ri[3];
   if (MODEL == MODEL_SLAB) {
-    const double inu = 1.0 / nu, inu2 = inu * inu;
+    const double inu = ip_rcp(nu), inu2 = inu * inu;
 #pragma unroll
     for (int i = 0; i < 4; ++i) { ji[i] = P.j[i] * inu2; ai[i] = P.al[i] * nu; }
 #pragma unroll
@@ -247,7 +248,7 @@ __device__ __forceinline__ bool plasma_operator(const Geom& G, const void* model
   } else {
     double bcov[4];
     g.mul(P.b, bcov);
-    double cosT = dot4(bcov, K) * iom / P.B;
+    double cosT = dot4(bcov, K) * iom * ip_rcp(P.B);
     cosT = fmin(1.0, fmax(-1.0, cosT));
     const Coeff c = synchrotron_invariant(P.ne, P.Th, P.B, cosT, nu);
     ji[0] = c.jI; ji[1] = c.jQ; ji[2] = 0.0; ji[3] = c.jV;

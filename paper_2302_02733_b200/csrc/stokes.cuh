@@ -20,6 +20,12 @@ __device__ __forceinline__ void cross3(const double u[3], const double v[3], dou
 }
 __device__ __forceinline__ double dot3(const double u[3], const double v[3]) { return u[0] * v[0] + u[1] * v[1] + u[2] * v[2]; }
 
+// a/b: the fast quotient where b is safely normal, the IEEE division otherwise (coefficients near the subnormal range)
+__device__ __forceinline__ double guarded_div(double a, double b) {
+  const double ab = fabs(b);
+  return (ab > 1e-290 && ab < 1e290) ? ip_div(a, b) : a / b;
+}
+
 // S <- O(s) S + P(s) J ; al = (aI,aQ,aU,aV), rh = (rQ,rU,rV)
 //
 // Transcendentals per call: three expm1 and one sincos.  With tp = expm1(-(aI-L1)s), tm = expm1(-(aI+L1)s),
@@ -31,14 +37,14 @@ __device__ __forceinline__ void stokes_step(const double al[4], const double rh[
   const double t0 = ip_expm1(-aI * s);
   const double ex = 1.0 + t0;
   if (m == 0.0) {
-    const double E = (aI == 0.0) ? s : -t0 / aI;
+    const double E = (aI == 0.0) ? s : -guarded_div(t0, aI);
 #pragma unroll
     for (int i = 0; i < 4; ++i) S[i] = ex * S[i] + E * J[i];
     return;
   }
   double a[3], r[3];
   if (m > 1e-290) {
-    const double im = 1.0 / m;
+    const double im = ip_rcp(m);
     a[0] = al[1] * im; a[1] = al[2] * im; a[2] = al[3] * im;
     r[0] = rh[0] * im; r[1] = rh[1] * im; r[2] = rh[2] * im;
   } else {  // 1/m would overflow (coefficients in the subnormal range, e.g. far wings of a Gaussian slab)
@@ -48,13 +54,13 @@ __device__ __forceinline__ void stokes_step(const double al[4], const double rh[
   const double a2 = dot3(a, a), r2 = dot3(r, r), ar = dot3(a, r);
   const double sg = (ar >= 0.0) ? 1.0 : -1.0;
   const double d = 0.5 * (a2 - r2);
-  const double q = sqrt(d * d + ar * ar);          // >= max scaled component^2 / 2 > 0
+  const double q = ip_sqrt(d * d + ar * ar);          // >= max scaled component^2 / 2 > 0
   // the larger of l1, l2 from the root (>= 1/sqrt 2 after scaling), the other from l1 l2 = |a.r|
   const double big2 = q + fabs(d);
-  const double ibig = rsqrt(big2);
+  const double ibig = ip_rsqrt(big2);
   const double big = big2 * ibig, small = fabs(ar) * ibig;
   const double l1 = (d >= 0.0) ? big : small, l2 = (d >= 0.0) ? small : big;
-  const double iTh = 0.5 / q;                      // Theta = l1^2 + l2^2 = 2 q
+  const double iTh = 0.5 * ip_rcp(q);                     // Theta = l1^2 + l2^2 = 2 q
   const double L1 = m * l1, L2 = m * l2;
   const double hh = 0.5 * (a2 + r2);
   const double sl1 = sg * l1, sl2 = sg * l2;
@@ -73,17 +79,17 @@ __device__ __forceinline__ void stokes_step(const double al[4], const double rh[
   const double bp = aI - L1, bm = aI + L1;
   const double tp = ip_expm1(-bp * s), tm = ip_expm1(-bm * s);
   const double exch = 1.0 + 0.5 * (tp + tm), exsh = 0.5 * (tp - tm);
-  const double Ep = (bp == 0.0) ? s : -tp / bp, Em = (bm == 0.0) ? s : -tm / bm;
+  const double Ep = (bp == 0.0) ? s : -guarded_div(tp, bp), Em = (bm == 0.0) ? s : -guarded_div(tm, bm);
   const double Ic1 = 0.5 * (Ep + Em), Is1 = 0.5 * (Ep - Em);
   double Ic2, Is2;
   const double den = aI * aI + L2 * L2;
   if (den == 0.0) { Ic2 = s; Is2 = 0.0; }
   else {
-    const double omc = (c > 0.0) ? sn * sn / (1.0 + c) : 1.0 - c;   // 1 - cos(L2 s)
+    const double omc = (c > 0.0) ? sn * sn * ip_rcp(1.0 + c) : 1.0 - c;   // 1 - cos(L2 s)
     const double re = omc - t0 * c;                                  // Re(1 - e^{-aI s} e^{i L2 s})
     const double im2 = -ex * sn;
     const double nc = re * aI - im2 * L2, ns = re * L2 + im2 * aI;
-    if (den > 1e-280) { const double iden = 1.0 / den; Ic2 = nc * iden; Is2 = ns * iden; }
+    if (den > 1e-280) { const double iden = ip_rcp(den); Ic2 = nc * iden; Is2 = ns * iden; }
     else { Ic2 = nc / den; Is2 = ns / den; }   // 1/den would overflow (coefficients near the subnormal range)
   }
   // weights of (1, M2, M3, M4) for O and for P
