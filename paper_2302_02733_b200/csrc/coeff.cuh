@@ -8,6 +8,7 @@
 #pragma once
 #include "geom.cuh"
 #include "bessel_tables.inc"
+#include "pw_tables.inc"
 
 namespace ipole {
 
@@ -67,6 +68,62 @@ __device__ __forceinline__ void bessel_k01_scaled(double z, double& k0, double& 
   }
 }
 
+// Piecewise polynomial tables (pw_tables.inc, written by gen_pw_tables.py): every binary octave of x is cut into
+// IPOLE_PW_NP = 8 pieces; on piece q the function is a polynomial in v = 16 m - (17 + 2 q), m = x 2^-e in [1, 2).
+// Returns false when x is outside [2^e0, 2^e1) (or not a positive normal number): the caller evaluates the
+// defining formula instead.
+__device__ __forceinline__ bool pw_locate(double x, int e0, int e1, int& piece, double& v) {
+  const int hi = __double2hiint(x);
+  const int e = (hi >> 20) - 1023;
+  const int q = (hi >> 17) & 7;
+  piece = (e - e0) * IPOLE_PW_NP + q;
+  const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(x));
+  v = fma(m, 2.0 * IPOLE_PW_NP, -(double)(2 * IPOLE_PW_NP + 1 + 2 * q));
+  return e >= e0 && e < e1;
+}
+
+__device__ __forceinline__ void bessel_ratios_series(double z, double Th, double& r0, double& r1);
+
+// K_0/K_2 and K_1/K_2 at z = 1/Th
+__device__ __forceinline__ void bessel_ratios(double z, double Th, double& r0, double& r1) {
+  int piece; double v;
+  if (pw_locate(Th, IPOLE_PW_BESSEL_E0, IPOLE_PW_BESSEL_E1, piece, v)) {
+    const double2* t = reinterpret_cast<const double2*>(&g_pw_bessel[piece][0][0]);
+    double2 c = __ldg(t + IPOLE_PW_NC - 1);
+    double a = c.x, b = c.y;
+#pragma unroll
+    for (int j = IPOLE_PW_NC - 2; j >= 0; --j) {
+      c = __ldg(t + j);
+      a = fma(a, v, c.x);
+      b = fma(b, v, c.y);
+    }
+    r0 = a; r1 = b;
+  } else {
+    bessel_ratios_series(z, Th, r0, r1);
+  }
+}
+
+// f(X) of the Faraday-conversion fit (R-7)
+__device__ __forceinline__ double faraday_fX(double X) {
+  int piece; double v;
+  if (pw_locate(X, IPOLE_PW_FX_E0, IPOLE_PW_FX_E1, piece, v)) {
+    const double2* t = reinterpret_cast<const double2*>(&g_pw_fx[piece][0][0]);
+    double p = 0.0;
+#pragma unroll
+    for (int j = IPOLE_PW_NC / 2 - 1; j >= 0; --j) {
+      const double2 c = __ldg(t + j);
+      p = fma(p, v, c.y);
+      p = fma(p, v, c.x);
+    }
+    return p;
+  }
+  const double lX = ip_log(X);
+  return 2.011 * ip_exp(-(1.0 / 4.7) * ip_exp(1.035 * lX)) - ip_cos_any(0.5 * X) * ip_exp(-(1.0 / 2.73) * ip_exp(1.2 * lX))
+         - 0.011 * ip_exp(-(1.0 / 47.2) * X);
+}
+
+static_assert(IPOLE_PW_NC % 2 == 0, "faraday_fX reads its coefficients two at a time");
+
 static_assert(IPOLE_BESSEL_K0_NC == IPOLE_BESSEL_K1_NC, "the two Chebyshev series are evaluated interleaved");
 
 struct Coeff { double jI, jQ, jV, aI, aQ, aV, rQ, rV; };
@@ -75,7 +132,7 @@ __device__ __forceinline__ double finite_or_zero(double v) { return isfinite(v) 
 
 // K_0(z)/K_2(z) and K_1(z)/K_2(z): the e^z scaling of bessel_k01_scaled cancels in the ratios, so the series branch
 // skips it here.
-__device__ __forceinline__ void bessel_ratios(double z, double Th, double& r0, double& r1) {
+__device__ __forceinline__ void bessel_ratios_series(double z, double Th, double& r0, double& r1) {
   double k0, k1;
   if (z <= 2.0) {
     const double EUL = 0.57721566490153286061;
@@ -161,9 +218,7 @@ __device__ __forceinline__ Coeff synchrotron(double ne, double Th, double B, dou
   double r0, r1;
   bessel_ratios(iTh, Th, r0, r1);
   const double X = Th * ip_sqrt((1.4142135623730950488e3 * IP_C_NUB) * BsT * inu);
-  const double lX = ip_log(X);
-  const double fX = 2.011 * ip_exp(-(1.0 / 4.7) * ip_exp(1.035 * lX)) - ip_cos_any(0.5 * X) * ip_exp(-(1.0 / 2.73) * ip_exp(1.2 * lX))
-                    - 0.011 * ip_exp(-(1.0 / 47.2) * X);
+  const double fX = faraday_fX(X);
   const double neinu = ne * (INVARIANT ? inu : inu * inu);
   c.rV = IP_C_RV * neinu * B * cosT * r0;
   c.rQ = IP_C_RQ * neinu * inu * (BsT * BsT) * fX * (r1 + 6.0 * Th);

@@ -452,9 +452,21 @@ int ipole_load_model_grid(ipole_ctx* c, const ipole_grid_desc* d, const double* 
   }
   GridParams m;
   std::memset(&m, 0, sizeof m);
-  for (int q = 0; q < 8; ++q) {
-    CK(cudaMemcpyAsync(c->d_grid + q * cells, fields[q], cells * sizeof(double), cudaMemcpyDefault, c->stream));
-    m.f[q] = c->d_grid + q * cells;
+  {  // SoA planes (caller) -> cell-major records (library copy); one staging plane on the device
+    double* stage = nullptr;
+    cudaError_t e = cudaMalloc(&stage, cells * sizeof(double));
+    if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
+    for (int q = 0; q < 8 && e == cudaSuccess; ++q) {
+      e = cudaMemcpyAsync(stage, fields[q], cells * sizeof(double), cudaMemcpyDefault, c->stream);
+      if (e == cudaSuccess) {
+        k_pack_field<<<c->n_sm * 8, 256, 0, c->stream>>>(cells, q, stage, c->d_grid);
+        e = cudaGetLastError();
+      }
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cudaFree(stage);
+    if (e != cudaSuccess) { c->last_cuda = (int)e; return IPOLE_ECUDA; }
+    m.cells = c->d_grid;
   }
   m.N1 = d->N1; m.N2 = d->N2; m.N3 = d->N3;
   for (int i = 0; i < 3; ++i) { m.startx[i] = d->startx[i]; m.idx[i] = 1.0 / d->dx[i]; }

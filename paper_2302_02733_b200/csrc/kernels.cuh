@@ -523,6 +523,11 @@ __global__ void k_eval_bessel(int64_t n, const double* z, double* out) {
   bessel_k01_scaled(z[i], k0, k1);
   out[3 * i] = k0; out[3 * i + 1] = k1; out[3 * i + 2] = k0 + 2.0 / z[i] * k1;
 }
+// re-tile one SoA plane into the cell-major records of GridParams::cells (load time, not on the hot path)
+__global__ void k_pack_field(size_t cells, int field, const double* __restrict__ plane, double* __restrict__ out) {
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < cells; i += (size_t)gridDim.x * blockDim.x)
+    out[i * 8 + field] = plane[i];
+}
 __global__ void k_eval_math(int64_t n, const double* x, double* out) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;

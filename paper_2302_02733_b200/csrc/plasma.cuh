@@ -24,7 +24,7 @@ struct GridParams {
   double startx[3], idx[3];      // idx = 1/dx
   double gam, Rlow, Rhigh, r_out, lx_out;   // lx_out = ln r_out
   double ne_unit, B_unit;        // rho -> n_e [cm^-3], sqrt(b.b) -> Gauss
-  const double* f[8];            // device planes rho,u,U1,U2,U3,B1,B2,B3
+  const double* cells;           // device, cell-major: cells[((i*N2 + j)*N3 + k)*8 + field], fields rho,u,U1,U2,U3,B1,B2,B3
 };
 struct Units { double nu_obs, L_unit, D_cm, dl_unit; };  // dl_unit = L_unit / nu_obs
 
@@ -105,7 +105,10 @@ __device__ __forceinline__ bool plasma_slab(const Geom& G, const SlabParams& M, 
 
 __device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
 
-// FP64 trilinear interpolation over the 8 SoA planes (read-only path: ld.global.nc)
+// FP64 trilinear interpolation of the 8 fields.  The caller's SoA planes are re-tiled at load time into cell-major
+// records of 8 doubles (64 B = two full sectors, 16-B aligned), so one corner of the stencil is four 128-bit
+// read-only loads (ld.global.nc.v2.f64) instead of eight scattered 8-byte ones, and the two k-neighbours share a
+// 128-B line: 8 lines per evaluation instead of up to 32 sectors in 32 different lines.
 __device__ __forceinline__ bool plasma_grid(const Geom& G, const GridParams& M, const double X[4], const Point& p,
                                             const Sym7& g, const Inv6& gi, Plasma& P) {
   if (p.r > M.r_out || X[1] < M.startx[0]) return false;
@@ -121,16 +124,19 @@ __device__ __forceinline__ bool plasma_grid(const Geom& G, const GridParams& M, 
   const size_t o00 = ((size_t)i0 * M.N2 + j0) * M.N3, o01 = ((size_t)i0 * M.N2 + j1) * M.N3;
   const size_t o10 = ((size_t)i1 * M.N2 + j0) * M.N3, o11 = ((size_t)i1 * M.N2 + j1) * M.N3;
   const double wi0 = 1.0 - di, wj0 = 1.0 - dj, wk0 = 1.0 - dk;
-  double prim[8];
+  const double w[8] = {wi0 * wj0 * wk0, wi0 * wj0 * dk, wi0 * dj * wk0, wi0 * dj * dk,
+                       di * wj0 * wk0,  di * wj0 * dk,  di * dj * wk0,  di * dj * dk};
+  const size_t off[8] = {o00 + k0, o00 + k1, o01 + k0, o01 + k1, o10 + k0, o10 + k1, o11 + k0, o11 + k1};
+  double prim[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+  const double2* C2 = reinterpret_cast<const double2*>(M.cells);
 #pragma unroll
-  for (int q = 0; q < 8; ++q) {
-    const double* F = M.f[q];
-    const double a000 = __ldg(F + o00 + k0), a001 = __ldg(F + o00 + k1);
-    const double a010 = __ldg(F + o01 + k0), a011 = __ldg(F + o01 + k1);
-    const double a100 = __ldg(F + o10 + k0), a101 = __ldg(F + o10 + k1);
-    const double a110 = __ldg(F + o11 + k0), a111 = __ldg(F + o11 + k1);
-    prim[q] = wi0 * (wj0 * (wk0 * a000 + dk * a001) + dj * (wk0 * a010 + dk * a011))
-              + di * (wj0 * (wk0 * a100 + dk * a101) + dj * (wk0 * a110 + dk * a111));
+  for (int c = 0; c < 8; ++c) {
+    const double2* rec = C2 + off[c] * 4;
+    const double2 a = __ldg(rec), b = __ldg(rec + 1), cc = __ldg(rec + 2), d = __ldg(rec + 3);
+    prim[0] = fma(w[c], a.x, prim[0]);  prim[1] = fma(w[c], a.y, prim[1]);
+    prim[2] = fma(w[c], b.x, prim[2]);  prim[3] = fma(w[c], b.y, prim[3]);
+    prim[4] = fma(w[c], cc.x, prim[4]); prim[5] = fma(w[c], cc.y, prim[5]);
+    prim[6] = fma(w[c], d.x, prim[6]);  prim[7] = fma(w[c], d.y, prim[7]);
   }
   const double rho = prim[0], uu = prim[1];
   if (!(rho > 0.0) || !(uu > 0.0)) return false;
