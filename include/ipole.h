@@ -96,6 +96,8 @@ typedef struct {
   int32_t n_launches;      /* kernels launched by the last ipole_make_image                            */
   float   ms_probe, ms_geodesic, ms_transfer, ms_total; /* CUDA-event times of the last image (0 until
                               ipole_get_stats synchronises them)                                       */
+  float   ms_long;         /* long-ray passes (geodesic + transfer) on the side stream; they overlap the
+                              bulk batches, so this is not part of a sum that gives ms_total            */
 } ipole_stats;
 
 /* Create a context. Computes the camera tetrad on the device. IPOLE_EINVAL on bad parameters. */

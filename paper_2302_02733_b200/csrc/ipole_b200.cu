@@ -19,7 +19,7 @@ constexpr int N_QUEUES = 8192;
 constexpr int PROBE_TARGET = 4096;   // rays of the probe pass
 constexpr int PROBE_EPS_FACTOR = 4;  // the probe integrates with 4 eps and predicts 4x its step count
 
-enum LaunchKind { LK_PROBE = 0, LK_GEO = 1, LK_RT = 2, LK_OTHER = 3 };
+enum LaunchKind { LK_PROBE = 0, LK_GEO = 1, LK_RT = 2, LK_OTHER = 3, LK_LONG = 4 };  // LK_LONG: on the side stream
 
 struct TimedSpan { cudaEvent_t a, b; int kind; };
 
@@ -43,6 +43,11 @@ struct ipole_ctx {
   int opt_sort = 1;
 
   double* d_path = nullptr; size_t path_bytes = 0;
+  double* d_path_long = nullptr; size_t path_long_bytes = 0;   // slots of max_steps for the long-ray passes
+  int32_t* d_nsteps_long = nullptr;                             // step counts written by the long-ray passes
+  cudaStream_t side = nullptr;                                  // long-ray passes overlap the bulk batches here
+  cudaStream_t qstream = nullptr;                               // 4-byte read-backs that must not wait for `side`
+  cudaEvent_t ev_geo = nullptr, ev_side = nullptr;
   int64_t ray_cap = 0;           // capacity of the per-ray buffers below
   int32_t *d_nsteps = nullptr, *d_nturn = nullptr, *d_order = nullptr, *d_key = nullptr, *d_long = nullptr;
   double* d_out = nullptr;       // staging for host outputs: 6 planes of ray_cap
@@ -120,12 +125,14 @@ int apply_camera(ipole_ctx* c, const ipole_camera* k) {
 int ensure_rays(ipole_ctx* c, int64_t n) {
   if (n <= c->ray_cap) return IPOLE_OK;
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long); cudaFree(c->d_out);
-  c->d_nsteps = c->d_nturn = c->d_order = c->d_key = c->d_long = nullptr; c->d_out = nullptr; c->ray_cap = 0;
+  cudaFree(c->d_nsteps_long);
+  c->d_nsteps = c->d_nturn = c->d_order = c->d_key = c->d_long = c->d_nsteps_long = nullptr; c->d_out = nullptr; c->ray_cap = 0;
   CK(cudaMalloc(&c->d_nsteps, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_nturn, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_order, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_key, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_long, n * sizeof(int32_t)));
+  CK(cudaMalloc(&c->d_nsteps_long, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_out, 6 * n * sizeof(double)));
   c->ray_cap = n;
   return IPOLE_OK;
@@ -140,17 +147,26 @@ int ensure_path(ipole_ctx* c, size_t bytes) {
   return IPOLE_OK;
 }
 
+int ensure_path_long(ipole_ctx* c, size_t bytes) {
+  if (bytes <= c->path_long_bytes) return IPOLE_OK;
+  cudaFree(c->d_path_long); c->d_path_long = nullptr; c->path_long_bytes = 0;
+  cudaError_t e = cudaMalloc(&c->d_path_long, bytes);
+  if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
+  c->path_long_bytes = bytes;
+  return IPOLE_OK;
+}
+
 size_t path_budget(ipole_ctx* c) {
   if (c->opt_path_bytes) return (size_t)c->opt_path_bytes;
   size_t fr = 0, tot = 0;
   cudaMemGetInfo(&fr, &tot);
-  fr += c->path_bytes;  // what we already hold counts as available
+  fr += c->path_bytes + c->path_long_bytes;  // what we already hold counts as available
   size_t b = (size_t)(0.4 * (double)fr);
   const size_t cap = (size_t)64 << 30;
   return std::min(b, cap);
 }
 
-int span_begin(ipole_ctx* c, int kind) {
+int span_begin(ipole_ctx* c, int kind, cudaStream_t st = nullptr, bool on_side = false) {
   if (c->spans_used == c->spans.size()) {
     TimedSpan s; s.kind = kind;
     if (cudaEventCreate(&s.a) != cudaSuccess || cudaEventCreate(&s.b) != cudaSuccess) return -1;
@@ -158,10 +174,12 @@ int span_begin(ipole_ctx* c, int kind) {
   }
   TimedSpan* s = &c->spans[c->spans_used++];
   s->kind = kind;
-  cudaEventRecord(s->a, c->stream);
+  cudaEventRecord(s->a, on_side ? st : c->stream);
   return (int)(c->spans_used - 1);
 }
-void span_end(ipole_ctx* c, int s) { if (s >= 0) cudaEventRecord(c->spans[s].b, c->stream); }
+void span_end(ipole_ctx* c, int s, cudaStream_t st = nullptr, bool on_side = false) {
+  if (s >= 0) cudaEventRecord(c->spans[s].b, on_side ? st : c->stream);
+}
 
 int grid_for(ipole_ctx* c, int occ, int threads, int64_t rays) {
   const int64_t full = (int64_t)c->n_sm * std::max(occ, 1);
@@ -169,22 +187,24 @@ int grid_for(ipole_ctx* c, int occ, int threads, int64_t rays) {
   return (int)std::max<int64_t>(1, std::min(full, need));
 }
 
-int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays) {
-  const int s = span_begin(c, kind);
-  k_geodesic<<<grid_for(c, c->occ_geo, IPOLE_GEO_THREADS, rays), IPOLE_GEO_THREADS, 0, c->stream>>>(a);
-  span_end(c, s);
+int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays, bool on_side = false) {
+  cudaStream_t st = on_side ? c->side : c->stream;
+  const int s = span_begin(c, kind, st, on_side);
+  k_geodesic<<<grid_for(c, c->occ_geo, IPOLE_GEO_THREADS, rays), IPOLE_GEO_THREADS, 0, st>>>(a);
+  span_end(c, s, st, on_side);
   c->stats.n_launches++;
   CK(cudaGetLastError());
   return IPOLE_OK;
 }
 
-int launch_transfer(ipole_ctx* c, RtArgs& a, int64_t rays) {
-  const int s = span_begin(c, LK_RT);
+int launch_transfer(ipole_ctx* c, RtArgs& a, int64_t rays, bool on_side = false) {
+  cudaStream_t st = on_side ? c->side : c->stream;
+  const int s = span_begin(c, on_side ? LK_LONG : LK_RT, st, on_side);
   const int g = grid_for(c, c->occ_rt[c->model], IPOLE_RT_THREADS, rays);
-  if (c->model == MODEL_ADAF) k_transfer<MODEL_ADAF><<<g, IPOLE_RT_THREADS, 0, c->stream>>>(a);
-  else if (c->model == MODEL_SLAB) k_transfer<MODEL_SLAB><<<g, IPOLE_RT_THREADS, 0, c->stream>>>(a);
-  else k_transfer<MODEL_GRID><<<g, IPOLE_RT_THREADS, 0, c->stream>>>(a);
-  span_end(c, s);
+  if (c->model == MODEL_ADAF) k_transfer<MODEL_ADAF><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
+  else if (c->model == MODEL_SLAB) k_transfer<MODEL_SLAB><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
+  else k_transfer<MODEL_GRID><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
+  span_end(c, s, st, on_side);
   c->stats.n_launches++;
   CK(cudaGetLastError());
   return IPOLE_OK;
@@ -276,11 +296,53 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   }
   c->stats.path_cap = cap;
 
+  // ---- long-ray passes: rays that overflowed their slot get one of max_steps.  They run on the side stream, as
+  // soon as the geodesic kernel of a batch has listed them, concurrently with the remaining bulk batches (one such
+  // ray is up to 50 000 sequential steps: its latency is hidden behind the bulk work instead of trailing it). ----
+  const size_t lslot = (size_t)(max_steps + 1) * rec_bytes;
+  int long_done = 0;          // entries of d_long already handed to the side stream
+  int64_t LBcap = 0;          // rays that fit the long path buffer
+  auto long_pass = [&](int upto) -> int {
+    if (upto <= long_done) return IPOLE_OK;
+    if (LBcap == 0) {
+      const size_t lbudget = std::max(lslot, std::min<size_t>(budget / 4, (size_t)16 << 30));
+      LBcap = std::max<int64_t>(1, std::min<int64_t>(std::max(upto - long_done, 256), (int64_t)(lbudget / lslot)));
+      if (c->path_long_bytes >= lslot) LBcap = std::max<int64_t>(LBcap, (int64_t)(c->path_long_bytes / lslot));
+      int rcl = ensure_path_long(c, (size_t)LBcap * lslot);
+      if (rcl != IPOLE_OK) return rcl;
+    }
+    for (int64_t base = long_done; base < upto; base += LBcap) {
+      const int64_t cnt = std::min<int64_t>(LBcap, upto - base);
+      if (qi + 2 > N_QUEUES) return IPOLE_EINVAL;
+      GeoArgs g = geo_args(c);
+      g.cap = max_steps; g.base = base; g.count = cnt; g.order = c->d_long; g.pixels = d_pixels;
+      g.path = c->d_path_long; g.nsteps = c->d_nsteps_long; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
+      int rcl = launch_geodesic(c, g, LK_LONG, cnt, true);
+      if (rcl != IPOLE_OK) return rcl;
+      RtArgs t;
+      std::memset(&t, 0, sizeof t);
+      t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = max_steps; t.base = base; t.count = cnt;
+      t.order = c->d_long; t.path = c->d_path_long; t.nsteps = c->d_nsteps_long; t.queue = c->d_queues + (qi++);
+      t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
+      if ((rcl = launch_transfer(c, t, cnt, true)) != IPOLE_OK) return rcl;
+    }
+    long_done = upto;
+    return IPOLE_OK;
+  };
+  // number of rays listed so far, read once the geodesic kernel of the current batch has finished
+  auto listed = [&](int& out) -> int {
+    CK(cudaEventSynchronize(c->ev_geo));
+    CK(cudaMemcpyAsync(&out, c->d_small, sizeof(int), cudaMemcpyDeviceToHost, c->qstream));
+    CK(cudaStreamSynchronize(c->qstream));
+    return IPOLE_OK;
+  };
+
   // ---- bulk pass in batches of B rays ----
   const size_t slot_bytes = (size_t)(cap + 1) * rec_bytes;
   int64_t B = std::min<int64_t>(n, (int64_t)(budget / slot_bytes));
   if (B < 1) return IPOLE_ENOMEM;
   if ((rc = ensure_path(c, (size_t)B * slot_bytes)) != IPOLE_OK) return rc;
+  int n_long = 0;
   for (int64_t base = 0; base < n; base += B) {
     const int64_t cnt = std::min(B, n - base);
     if (qi + 2 > N_QUEUES) return IPOLE_EINVAL;
@@ -289,6 +351,10 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     g.path = c->d_path; g.nsteps = c->d_nsteps; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
     g.long_list = c->d_long; g.long_count = c->d_small;
     if ((rc = launch_geodesic(c, g, LK_GEO, cnt)) != IPOLE_OK) return rc;
+    if (cap < max_steps) {
+      CK(cudaEventRecord(c->ev_geo, c->stream));
+      CK(cudaStreamWaitEvent(c->side, c->ev_geo, 0));
+    }
     RtArgs t;
     std::memset(&t, 0, sizeof t);
     t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = cap; t.base = base; t.count = cnt; t.order = order;
@@ -296,33 +362,20 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
     if ((rc = launch_transfer(c, t, cnt)) != IPOLE_OK) return rc;
     c->stats.n_batches++;
-  }
-
-  // ---- long-ray pass: rays that overflowed their slot get one of max_steps ----
-  int n_long = 0;
-  if (cap < max_steps) {
-    CK(cudaMemcpyAsync(&n_long, c->d_small, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-    CK(cudaStreamSynchronize(c->stream));
+    if (cap < max_steps) {   // the transfer kernel just queued keeps the GPU busy while the host waits here
+      if ((rc = listed(n_long)) != IPOLE_OK) return rc;
+      if ((rc = long_pass(n_long)) != IPOLE_OK) return rc;
+    }
   }
   c->stats.n_long = n_long;
   if (n_long > 0) {
-    const size_t lslot = (size_t)(max_steps + 1) * rec_bytes;
-    int64_t LB = std::min<int64_t>(n_long, (int64_t)(std::max(budget, lslot) / lslot));
-    if ((rc = ensure_path(c, (size_t)LB * lslot)) != IPOLE_OK) return rc;
-    for (int64_t base = 0; base < n_long; base += LB) {
-      const int64_t cnt = std::min<int64_t>(LB, n_long - base);
-      if (qi + 2 > N_QUEUES) return IPOLE_EINVAL;
-      GeoArgs g = geo_args(c);
-      g.cap = max_steps; g.base = base; g.count = cnt; g.order = c->d_long; g.pixels = d_pixels;
-      g.path = c->d_path; g.nsteps = c->d_nsteps; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
-      if ((rc = launch_geodesic(c, g, LK_GEO, cnt)) != IPOLE_OK) return rc;
-      RtArgs t;
-      std::memset(&t, 0, sizeof t);
-      t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = max_steps; t.base = base; t.count = cnt;
-      t.order = c->d_long; t.path = c->d_path; t.nsteps = c->d_nsteps; t.queue = c->d_queues + (qi++);
-      t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
-      if ((rc = launch_transfer(c, t, cnt)) != IPOLE_OK) return rc;
-    }
+    // join the side stream, then publish the step counts of the long rays (the bulk transfer kernels read
+    // nsteps[q] = -1 for them, so the long passes keep theirs apart until every bulk kernel is done)
+    CK(cudaEventRecord(c->ev_side, c->side));
+    CK(cudaStreamWaitEvent(c->stream, c->ev_side, 0));
+    k_merge_long<<<(n_long + 255) / 256, 256, 0, c->stream>>>(n_long, c->d_long, c->d_nsteps_long, c->d_nsteps);
+    c->stats.n_launches++;
+    CK(cudaGetLastError());
   }
 
   // ---- a-9: totals ----
@@ -368,6 +421,14 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   if (cudaMalloc(&c->d_small, 4 * sizeof(int)) != cudaSuccess) return fail(IPOLE_ENOMEM);
   if (cudaMalloc(&c->d_part, REDUCE_BLOCKS * sizeof(ReducePartial)) != cudaSuccess) return fail(IPOLE_ENOMEM);
   if (cudaMalloc(&c->d_red, sizeof(ReduceOut)) != cudaSuccess) return fail(IPOLE_ENOMEM);
+  {
+    int lo = 0, hi = 0;
+    cudaDeviceGetStreamPriorityRange(&lo, &hi);   // hi = greatest priority: the few long-ray blocks go first
+    if (cudaStreamCreateWithPriority(&c->side, cudaStreamNonBlocking, hi) != cudaSuccess) return fail(IPOLE_ECUDA);
+    if (cudaStreamCreateWithFlags(&c->qstream, cudaStreamNonBlocking) != cudaSuccess) return fail(IPOLE_ECUDA);
+    if (cudaEventCreateWithFlags(&c->ev_geo, cudaEventDisableTiming) != cudaSuccess) return fail(IPOLE_ECUDA);
+    if (cudaEventCreateWithFlags(&c->ev_side, cudaEventDisableTiming) != cudaSuccess) return fail(IPOLE_ECUDA);
+  }
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo, k_geodesic, IPOLE_GEO_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_rt[MODEL_ADAF], k_transfer<MODEL_ADAF>, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_rt[MODEL_SLAB], k_transfer<MODEL_SLAB>, IPOLE_RT_THREADS, 0);
@@ -550,7 +611,7 @@ int ipole_get_stats(ipole_ctx* c, ipole_stats* out) {
   for (int k = 0; k < 4; ++k) s.flux_jy[k] = r.flux[k];
   s.lp = r.lp; s.cp = r.cp;
   s.total_steps = r.total_steps; s.max_steps_seen = r.max_steps; s.n_ring = r.n_ring; s.n_maxstep = r.n_maxstep;
-  s.ms_probe = s.ms_geodesic = s.ms_transfer = s.ms_total = 0.f;
+  s.ms_probe = s.ms_geodesic = s.ms_transfer = s.ms_total = s.ms_long = 0.f;
   for (size_t i = 0; i < c->spans_used; ++i) {
     float ms = 0.f;
     if (cudaEventElapsedTime(&ms, c->spans[i].a, c->spans[i].b) != cudaSuccess) { cudaGetLastError(); continue; }
@@ -558,6 +619,7 @@ int ipole_get_stats(ipole_ctx* c, ipole_stats* out) {
     else if (c->spans[i].kind == LK_PROBE) s.ms_probe += ms;
     else if (c->spans[i].kind == LK_GEO) s.ms_geodesic += ms;
     else if (c->spans[i].kind == LK_RT) s.ms_transfer += ms;
+    else if (c->spans[i].kind == LK_LONG) s.ms_long += ms;
   }
   *out = s;
   return IPOLE_OK;
@@ -687,6 +749,11 @@ int ipole_last_cuda_error(const ipole_ctx* c) { return c ? c->last_cuda : 0; }
 
 void ipole_free(ipole_ctx* c) {
   if (!c) return;
+  if (c->side) { cudaStreamSynchronize(c->side); cudaStreamDestroy(c->side); }
+  if (c->qstream) cudaStreamDestroy(c->qstream);
+  if (c->ev_geo) cudaEventDestroy(c->ev_geo);
+  if (c->ev_side) cudaEventDestroy(c->ev_side);
+  cudaFree(c->d_path_long); cudaFree(c->d_nsteps_long);
   cudaFree(c->d_cam); cudaFree(c->d_model); cudaFree(c->d_grid); cudaFree(c->d_path);
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long);
   cudaFree(c->d_out); cudaFree(c->d_pixels); cudaFree(c->d_probe); cudaFree(c->d_queues); cudaFree(c->d_hist);

@@ -477,6 +477,12 @@ __global__ void k_reduce_final(const ReducePartial* part, int nparts, double sca
   *out = o;
 }
 
+// step counts of the long-ray passes -> nsteps (after every bulk kernel has finished)
+__global__ void k_merge_long(int n_long, const int32_t* long_list, const int32_t* nsteps_long, int32_t* nsteps) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n_long) { const int32_t q = long_list[i]; nsteps[q] = nsteps_long[q]; }
+}
+
 __global__ void k_max_i32(const int32_t* v, int n, int* out) {  // probe maximum (one block)
   int m = 0;
   for (int i = threadIdx.x; i < n; i += blockDim.x) m = max(m, v[i]);

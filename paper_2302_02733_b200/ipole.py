@@ -52,7 +52,8 @@ class Stats(C.Structure):
     _fields_ = [("flux_jy", C.c_double * 4), ("lp", C.c_double), ("cp", C.c_double), ("total_steps", C.c_int64),
                 ("max_steps_seen", C.c_int32), ("path_cap", C.c_int32), ("n_ring", C.c_int64),
                 ("n_maxstep", C.c_int64), ("n_long", C.c_int64), ("n_batches", C.c_int32), ("n_launches", C.c_int32),
-                ("ms_probe", C.c_float), ("ms_geodesic", C.c_float), ("ms_transfer", C.c_float), ("ms_total", C.c_float)]
+                ("ms_probe", C.c_float), ("ms_geodesic", C.c_float), ("ms_transfer", C.c_float), ("ms_total", C.c_float),
+                ("ms_long", C.c_float)]
 
 
 class IpoleError(RuntimeError):
