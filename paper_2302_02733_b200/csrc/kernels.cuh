@@ -249,6 +249,9 @@ struct RtArgs {
 #ifndef IPOLE_RT_MINB
 #define IPOLE_RT_MINB 2
 #endif
+#ifndef IPOLE_RT_MINB_ANALYTIC
+#define IPOLE_RT_MINB_ANALYTIC 3
+#endif
 #ifndef IPOLE_RT_SYNC
 #define IPOLE_RT_SYNC 0
 #endif
@@ -258,8 +261,11 @@ struct RtArgs {
 
 // a-4 ... a-7, a-8.  Lane-level refill as in k_geodesic.  Per step: midpoint (Xm, Km), generator A = Gamma.Km,
 // f <- P f, plasma operator, f <- P f  (Strang splitting, R-6).
+// Resident blocks per SM: 3 (168 registers, a few spilled doubles) for the analytic models, which ncu shows limited
+// by dependent-issue latency; 2 (255 registers) for the grid model, whose 64 gathered values per step want registers.
 template <int MODEL>
-__global__ void __launch_bounds__(IPOLE_RT_THREADS, IPOLE_RT_MINB) k_transfer(const __grid_constant__ RtArgs A) {
+__global__ void __launch_bounds__(IPOLE_RT_THREADS, (MODEL == MODEL_GRID) ? IPOLE_RT_MINB : IPOLE_RT_MINB_ANALYTIC)
+k_transfer(const __grid_constant__ RtArgs A) {
   const CamDev& C = A.cam;
   const int64_t count = A.count_dev ? (int64_t)*A.count_dev : A.count;
   const size_t slot_doubles = (size_t)(A.cap + 1) * REC_DOUBLES;
@@ -325,8 +331,14 @@ __global__ void __launch_bounds__(IPOLE_RT_THREADS, IPOLE_RT_MINB) k_transfer(co
       transport_generator(C.G, Xm, Km, p, g, gi, Am);
       const double h = 0.5 * dl;
       if (lit) { transport_apply(Am, h, st.f1); transport_apply(Am, h, st.f2); }
-      if (maybe) lit |= plasma_operator<MODEL>(C.G, model, A.units, Xm, Km, p, g, gi, dl, st);
+      // the tetrad first, then the second half of the transport (applied to the NEW legs), and only then the
+      // coefficients and the 4x4 step, which touch the Stokes numbers alone: same result, but the generator and
+      // the tetrad are dead while the register-hungry part runs
+      PlasmaFrame F;
+      const bool applied = maybe && plasma_frame<MODEL>(C.G, model, A.units, Xm, Km, p, g, gi, st, F);
+      lit |= applied;
       if (lit) { transport_apply(Am, h, st.f1); transport_apply(Am, h, st.f2); }
+      if (applied) plasma_apply<MODEL>(A.units, F, dl, st);
     }
 #pragma unroll
     for (int m = 0; m < 4; ++m) { Xhi[m] = Xlo[m]; Khi[m] = Klo[m]; }
@@ -519,7 +531,10 @@ __global__ void k_eval_stokes_step(int64_t n, const double* in, double* out) {
   if (i >= n) return;
   const double* a = in + 16 * i;
   double S[4] = {a[8], a[9], a[10], a[11]};
-  stokes_step(a, a + 4, a[7], a + 12, S);
+  if (a[2] == 0.0 && a[5] == 0.0 && a[14] == 0.0)   // aU = rU = jU = 0: the specialised form the transfer kernel uses
+    stokes_step_qv(a[0], a[1], a[3], a[4], a[6], a[7], a[12], a[13], a[15], S);
+  else
+    stokes_step(a, a + 4, a[7], a + 12, S);
   for (int k = 0; k < 4; ++k) out[4 * i + k] = S[k];
 }
 __global__ void k_eval_bessel(int64_t n, const double* z, double* out) {

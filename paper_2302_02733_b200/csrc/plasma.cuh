@@ -201,11 +201,21 @@ struct PolState {
   double tau, tauF;
 };
 
-// One application of the plasma operator at (X, K) over affine length dl.  Returns true if applied.
+// What the plasma operator needs once the tetrad has been dealt with: the fluid scalars, the frequency, the angle,
+// and the 2x2 projection of the carried legs on the new ones.  Splitting the operator here lets the kernel finish
+// the parallel transport of the new legs before the (register-hungry) coefficient and 4x4 step run.
+struct PlasmaFrame {
+  double ne, Th, B, cosT, nu;
+  double m11, m12, m21, m22;     // M_{a'a} = e^(a')_mu f_a^mu
+  double j[4], al[4], rh[3];     // slab only (cgs)
+};
+
+// Plasma state and tetrad at (X, K); on success the carried legs st.f1, st.f2 are REPLACED by the new transverse
+// legs e_(1), e_(2) and F holds what plasma_apply needs.  Returns false where there is no plasma (nothing changed).
 template <int MODEL>
-__device__ __forceinline__ bool plasma_operator(const Geom& G, const void* model, const Units& U, const double X[4],
-                                                const double K[4], const Point& p, const Sym7& g, const Inv6& gi,
-                                                double dl, PolState& st) {
+__device__ __forceinline__ bool plasma_frame(const Geom& G, const void* model, const Units& U, const double X[4],
+                                             const double K[4], const Point& p, const Sym7& g, const Inv6& gi,
+                                             PolState& st, PlasmaFrame& F) {
   Plasma P;
   bool present;
   if (MODEL == MODEL_ADAF) present = plasma_adaf(G, *(const AdafParams*)model, X, p, g, gi, P);
@@ -243,33 +253,47 @@ __device__ __forceinline__ bool plasma_operator(const Geom& G, const void* model
   for (int m = 0; m < 4; ++m) e1[m] *= isg;
   g.mul(e1, e1c);
 
-  const double nu = om * U.nu_obs;
-  double ji[4], ai[4], ri[3];
+  F.nu = om * U.nu_obs;
+  F.ne = P.ne; F.Th = P.Th; F.B = P.B;
   if (MODEL == MODEL_SLAB) {
-    const double inu = ip_rcp(nu), inu2 = inu * inu;
 #pragma unroll
-    for (int i = 0; i < 4; ++i) { ji[i] = P.j[i] * inu2; ai[i] = P.al[i] * nu; }
+    for (int i = 0; i < 4; ++i) { F.j[i] = P.j[i]; F.al[i] = P.al[i]; }
 #pragma unroll
-    for (int i = 0; i < 3; ++i) ri[i] = P.rh[i] * nu;
+    for (int i = 0; i < 3; ++i) F.rh[i] = P.rh[i];
+    F.cosT = 0.0;
   } else {
     double bcov[4];
     g.mul(P.b, bcov);
-    double cosT = dot4(bcov, K) * iom * ip_rcp(P.B);
-    cosT = fmin(1.0, fmax(-1.0, cosT));
-    const Coeff c = synchrotron_invariant(P.ne, P.Th, P.B, cosT, nu);
-    ji[0] = c.jI; ji[1] = c.jQ; ji[2] = 0.0; ji[3] = c.jV;
-    ai[0] = c.aI; ai[1] = c.aQ; ai[2] = 0.0; ai[3] = c.aV;
-    ri[0] = c.rQ; ri[1] = 0.0;  ri[2] = c.rV;
+    F.cosT = fmin(1.0, fmax(-1.0, dot4(bcov, K) * iom * ip_rcp(P.B)));
   }
-  const double ds = dl * U.dl_unit;
-  // project the carried state on the new transverse legs: M_{a'a} = e^(a')_mu f_a^mu
-  stokes_congruence(dot4(e1c, st.f1), dot4(e1c, st.f2), dot4(e2c, st.f1), dot4(e2c, st.f2), st.S);
-  stokes_step(ai, ri, ds, ji, st.S);
+  F.m11 = dot4(e1c, st.f1); F.m12 = dot4(e1c, st.f2); F.m21 = dot4(e2c, st.f1); F.m22 = dot4(e2c, st.f2);
 #pragma unroll
   for (int m = 0; m < 4; ++m) { st.f1[m] = e1[m]; st.f2[m] = e2[m]; }
-  st.tau += ai[0] * ds;
-  st.tauF += fabs(ri[2]) * ds;
   return true;
+}
+
+// Projection of the Stokes vector on the new legs, coefficients, analytic 4x4 step over affine length dl.
+template <int MODEL>
+__device__ __forceinline__ void plasma_apply(const Units& U, const PlasmaFrame& F, double dl, PolState& st) {
+  const double ds = dl * U.dl_unit;
+  stokes_congruence(F.m11, F.m12, F.m21, F.m22, st.S);
+  double aI, rV;
+  if (MODEL == MODEL_SLAB) {
+    double ji[4], ai[4], ri[3];
+    const double inu = ip_rcp(F.nu), inu2 = inu * inu;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { ji[i] = F.j[i] * inu2; ai[i] = F.al[i] * F.nu; }
+#pragma unroll
+    for (int i = 0; i < 3; ++i) ri[i] = F.rh[i] * F.nu;
+    stokes_step(ai, ri, ds, ji, st.S);
+    aI = ai[0]; rV = ri[2];
+  } else {
+    const Coeff c = synchrotron_invariant(F.ne, F.Th, F.B, F.cosT, F.nu);
+    stokes_step_qv(c.aI, c.aQ, c.aV, c.rQ, c.rV, ds, c.jI, c.jQ, c.jV, st.S);
+    aI = c.aI; rV = c.rV;
+  }
+  st.tau += aI * ds;
+  st.tauF += fabs(rV) * ds;
 }
 
 }  // namespace ipole

@@ -119,4 +119,96 @@ __device__ __forceinline__ void stokes_step(const double al[4], const double rh[
   for (int i = 0; i < 4; ++i) S[i] = out[i];
 }
 
+// The same step for aU = rU = jU = 0, which is what the synchrotron coefficients are in the tetrad whose e_(2) lies
+// along the projected field (R-6/R-7): a = (aQ, 0, aV), r = (rQ, 0, rV), r x a = (0, rV aQ - rQ aV, 0).
+// The operator applied to (V0, x, y, z) = (I, Q, U, V) collapses to ten numbers per weight set (c1..c4):
+//   out0 = P0 V0 + Ax x + G y + Az z          P0,1 = c1 +- c4 hh,  A = c2 v2 + c3 v3,  B = c2 w2 + c3 w3,
+//   outx = Ax V0 + (P1 + Dxx) x + B2 y + Dxz z          G = c4 (r x a)_U,  D = c4 (a a^T + r r^T)
+//   outy = -G V0 - B2 x + P1 y + B0 z
+//   outz = Az V0 + Dxz x - B0 y + (P1 + Dzz) z
+__device__ __forceinline__ void stokes_step_qv(double aI, double aQ, double aV, double rQ, double rV, double s,
+                                               double jI, double jQ, double jV, double S[4]) {
+  const double m = fmax(fmax(fabs(aQ), fabs(aV)), fmax(fabs(rQ), fabs(rV)));
+  const double t0 = ip_expm1(-aI * s);
+  const double ex = 1.0 + t0;
+  if (m == 0.0) {
+    const double E = (aI == 0.0) ? s : -guarded_div(t0, aI);
+    S[0] = ex * S[0] + E * jI; S[1] = ex * S[1] + E * jQ; S[2] = ex * S[2]; S[3] = ex * S[3] + E * jV;
+    return;
+  }
+  double a0, a2, r0, r2;
+  if (m > 1e-290) {
+    const double im = ip_rcp(m);
+    a0 = aQ * im; a2 = aV * im; r0 = rQ * im; r2 = rV * im;
+  } else {
+    a0 = aQ / m; a2 = aV / m; r0 = rQ / m; r2 = rV / m;
+  }
+  const double qa = a0 * a0 + r0 * r0, qz = a2 * a2 + r2 * r2, qxz = a0 * a2 + r0 * r2;
+  const double asq = a0 * a0 + a2 * a2, rsq = r0 * r0 + r2 * r2, ar = a0 * r0 + a2 * r2;
+  const double sg = (ar >= 0.0) ? 1.0 : -1.0;
+  const double d = 0.5 * (asq - rsq);
+  const double q = ip_sqrt(d * d + ar * ar);
+  const double big2 = q + fabs(d);
+  const double ibig = ip_rsqrt(big2);
+  const double big = big2 * ibig, small = fabs(ar) * ibig;
+  const double l1 = (d >= 0.0) ? big : small, l2 = (d >= 0.0) ? small : big;
+  const double iTh = 0.5 * ip_rcp(q);
+  const double L1 = m * l1, L2 = m * l2;
+  const double hh = 0.5 * (asq + rsq);
+  const double sl1 = sg * l1, sl2 = sg * l2;
+  const double v2x = l2 * a0 - sl1 * r0, v2z = l2 * a2 - sl1 * r2;
+  const double w2x = sl1 * a0 + l2 * r0, w2z = sl1 * a2 + l2 * r2;
+  const double v3x = l1 * a0 + sl2 * r0, v3z = l1 * a2 + sl2 * r2;
+  const double w3x = l1 * r0 - sl2 * a0, w3z = l1 * r2 - sl2 * a2;
+  const double cru = r2 * a0 - r0 * a2;
+
+  double sn, c;
+  ip_sincos_any(L2 * s, &sn, &c);
+  const double bp = aI - L1, bm = aI + L1;
+  const double tp = ip_expm1(-bp * s), tm = ip_expm1(-bm * s);
+  const double exch = 1.0 + 0.5 * (tp + tm), exsh = 0.5 * (tp - tm);
+  const double Ep = (bp == 0.0) ? s : -guarded_div(tp, bp), Em = (bm == 0.0) ? s : -guarded_div(tm, bm);
+  const double Ic1 = 0.5 * (Ep + Em), Is1 = 0.5 * (Ep - Em);
+  double Ic2, Is2;
+  const double den = aI * aI + L2 * L2;
+  if (den == 0.0) { Ic2 = s; Is2 = 0.0; }
+  else {
+    const double omc = (c > 0.0) ? sn * sn * ip_rcp(1.0 + c) : 1.0 - c;
+    const double re = omc - t0 * c;
+    const double im2 = -ex * sn;
+    const double nc = re * aI - im2 * L2, ns = re * L2 + im2 * aI;
+    if (den > 1e-280) { const double iden = ip_rcp(den); Ic2 = nc * iden; Is2 = ns * iden; }
+    else { Ic2 = nc / den; Is2 = ns / den; }
+  }
+  const double exc = ex * c;
+  const double i2Th = 2.0 * iTh;
+  // O acting on S
+  double o0, ox, oy, oz;
+  {
+    const double c1 = 0.5 * (exch + exc), c2 = -ex * sn * iTh, c3 = -exsh * iTh, c4 = 0.5 * (exch - exc) * i2Th;
+    const double P0 = fma(c4, hh, c1), P1 = fma(-c4, hh, c1);
+    const double Ax = c2 * v2x + c3 * v3x, Az = c2 * v2z + c3 * v3z;
+    const double B0 = c2 * w2x + c3 * w3x, B2 = c2 * w2z + c3 * w3z;
+    const double G = c4 * cru, Dxx = c4 * qa, Dzz = c4 * qz, Dxz = c4 * qxz;
+    const double V0 = S[0], x = S[1], y = S[2], z = S[3];
+    o0 = P0 * V0 + Ax * x + G * y + Az * z;
+    ox = Ax * V0 + (P1 + Dxx) * x + B2 * y + Dxz * z;
+    oy = -G * V0 - B2 * x + P1 * y + B0 * z;
+    oz = Az * V0 + Dxz * x - B0 * y + (P1 + Dzz) * z;
+  }
+  // P acting on J = (jI, jQ, 0, jV)
+  {
+    const double c1 = 0.5 * (Ic1 + Ic2), c2 = -Is2 * iTh, c3 = -Is1 * iTh, c4 = 0.5 * (Ic1 - Ic2) * i2Th;
+    const double P0 = fma(c4, hh, c1), P1 = fma(-c4, hh, c1);
+    const double Ax = c2 * v2x + c3 * v3x, Az = c2 * v2z + c3 * v3z;
+    const double B0 = c2 * w2x + c3 * w3x, B2 = c2 * w2z + c3 * w3z;
+    const double G = c4 * cru, Dxx = c4 * qa, Dzz = c4 * qz, Dxz = c4 * qxz;
+    o0 += P0 * jI + Ax * jQ + Az * jV;
+    ox += Ax * jI + (P1 + Dxx) * jQ + Dxz * jV;
+    oy += -G * jI - B2 * jQ + B0 * jV;
+    oz += Az * jI + Dxz * jQ + (P1 + Dzz) * jV;
+  }
+  S[0] = o0; S[1] = ox; S[2] = oy; S[3] = oz;
+}
+
 }  // namespace ipole

@@ -90,6 +90,7 @@ def test_stokes_step(ipole, ref):
     J = rng.normal(size=(n, 4)) * scale
     # degenerate cases: no Faraday, no polarized absorption, nothing at all, aU = rU = 0
     rh[:50] = 0; al[50:100, 1:] = 0; al[100:120] = 0; rh[100:120] = 0; al[120:400, 2] = 0; rh[120:400, 1] = 0
+    J[120:300, 2] = 0; J[:10, 2] = 0; J[50:60, 2] = 0; J[100:110, 2] = 0  # aU = rU = jU = 0: the specialised step of the transfer kernel
     out = g.eval_stokes_step(al, rh, s, S0, J)
     want = np.zeros((n, 4))
     for i in range(n):
