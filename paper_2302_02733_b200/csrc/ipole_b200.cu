@@ -166,7 +166,7 @@ size_t path_budget(ipole_ctx* c) {
   return std::min(b, cap);
 }
 
-int span_begin(ipole_ctx* c, int kind, cudaStream_t st = nullptr, bool on_side = false) {
+int span_begin(ipole_ctx* c, int kind, cudaStream_t st) {
   if (c->spans_used == c->spans.size()) {
     TimedSpan s; s.kind = kind;
     if (cudaEventCreate(&s.a) != cudaSuccess || cudaEventCreate(&s.b) != cudaSuccess) return -1;
@@ -174,11 +174,11 @@ int span_begin(ipole_ctx* c, int kind, cudaStream_t st = nullptr, bool on_side =
   }
   TimedSpan* s = &c->spans[c->spans_used++];
   s->kind = kind;
-  cudaEventRecord(s->a, on_side ? st : c->stream);
+  cudaEventRecord(s->a, st);
   return (int)(c->spans_used - 1);
 }
-void span_end(ipole_ctx* c, int s, cudaStream_t st = nullptr, bool on_side = false) {
-  if (s >= 0) cudaEventRecord(c->spans[s].b, on_side ? st : c->stream);
+void span_end(ipole_ctx* c, int s, cudaStream_t st) {
+  if (s >= 0) cudaEventRecord(c->spans[s].b, st);
 }
 
 int grid_for(ipole_ctx* c, int occ, int threads, int64_t rays) {
@@ -187,24 +187,22 @@ int grid_for(ipole_ctx* c, int occ, int threads, int64_t rays) {
   return (int)std::max<int64_t>(1, std::min(full, need));
 }
 
-int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays, bool on_side = false) {
-  cudaStream_t st = on_side ? c->side : c->stream;
-  const int s = span_begin(c, kind, st, on_side);
+int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays, cudaStream_t st) {
+  const int s = span_begin(c, kind, st);
   k_geodesic<<<grid_for(c, c->occ_geo, IPOLE_GEO_THREADS, rays), IPOLE_GEO_THREADS, 0, st>>>(a);
-  span_end(c, s, st, on_side);
+  span_end(c, s, st);
   c->stats.n_launches++;
   CK(cudaGetLastError());
   return IPOLE_OK;
 }
 
-int launch_transfer(ipole_ctx* c, RtArgs& a, int64_t rays, bool on_side = false) {
-  cudaStream_t st = on_side ? c->side : c->stream;
-  const int s = span_begin(c, on_side ? LK_LONG : LK_RT, st, on_side);
+int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_t st) {
+  const int s = span_begin(c, kind, st);
   const int g = grid_for(c, c->occ_rt[c->model], IPOLE_RT_THREADS, rays);
   if (c->model == MODEL_ADAF) k_transfer<MODEL_ADAF><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
   else if (c->model == MODEL_SLAB) k_transfer<MODEL_SLAB><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
   else k_transfer<MODEL_GRID><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
-  span_end(c, s, st, on_side);
+  span_end(c, s, st);
   c->stats.n_launches++;
   CK(cudaGetLastError());
   return IPOLE_OK;
@@ -231,7 +229,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   CK(cudaMemsetAsync(c->d_queues, 0, N_QUEUES * sizeof(unsigned long long), c->stream));
   CK(cudaMemsetAsync(c->d_small, 0, 4 * sizeof(int), c->stream));
   int qi = 0;
-  const int total = span_begin(c, LK_OTHER);
+  const int total = span_begin(c, LK_OTHER, c->stream);
 
   const size_t budget = path_budget(c);
   const size_t rec_bytes = REC_DOUBLES * sizeof(double);
@@ -266,8 +264,8 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
       c->probe_cap = np;
     }
     g.count = np; g.nsteps = c->d_probe; g.queue = c->d_queues + (qi++);
-    if ((rc = launch_geodesic(c, g, LK_PROBE, np)) != IPOLE_OK) return rc;
-    const int sp = span_begin(c, LK_PROBE);
+    if ((rc = launch_geodesic(c, g, LK_PROBE, np, c->stream)) != IPOLE_OK) return rc;
+    const int sp = span_begin(c, LK_PROBE, c->stream);
     k_max_i32<<<1, 1024, 0, c->stream>>>(c->d_probe, (int)np, c->d_small + 1);
     c->stats.n_launches++;
     int pmax = 0;
@@ -287,7 +285,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
       CK(cudaGetLastError());
       order = c->d_order;
     }
-    span_end(c, sp);
+    span_end(c, sp, c->stream);
   }
   if (!probe) {
     // everything in flight at once: give each ray what the budget allows
@@ -317,27 +315,29 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
       GeoArgs g = geo_args(c);
       g.cap = max_steps; g.base = base; g.count = cnt; g.order = c->d_long; g.pixels = d_pixels;
       g.path = c->d_path_long; g.nsteps = c->d_nsteps_long; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
-      int rcl = launch_geodesic(c, g, LK_LONG, cnt, true);
+      int rcl = launch_geodesic(c, g, LK_LONG, cnt, c->side);
       if (rcl != IPOLE_OK) return rcl;
       RtArgs t;
       std::memset(&t, 0, sizeof t);
       t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = max_steps; t.base = base; t.count = cnt;
       t.order = c->d_long; t.path = c->d_path_long; t.nsteps = c->d_nsteps_long; t.queue = c->d_queues + (qi++);
       t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
-      if ((rcl = launch_transfer(c, t, cnt, true)) != IPOLE_OK) return rcl;
+      if ((rcl = launch_transfer(c, t, LK_LONG, cnt, c->side)) != IPOLE_OK) return rcl;
     }
     long_done = upto;
     return IPOLE_OK;
   };
   // number of rays listed so far, read once the geodesic kernel of the current batch has finished
-  auto listed = [&](int& out) -> int {
-    CK(cudaEventSynchronize(c->ev_geo));
+  auto listed = [&](cudaEvent_t geo_done, int& out) -> int {
+    CK(cudaEventSynchronize(geo_done));
     CK(cudaMemcpyAsync(&out, c->d_small, sizeof(int), cudaMemcpyDeviceToHost, c->qstream));
     CK(cudaStreamSynchronize(c->qstream));
     return IPOLE_OK;
   };
 
   // ---- bulk pass in batches of B rays ----
+  // (Running k_geodesic of batch k+1 on a second stream beside k_transfer of batch k was tried and dropped: the
+  // transfer blocks leave no room for useful geodesic occupancy, profiles/r1_notes.md.)
   const size_t slot_bytes = (size_t)(cap + 1) * rec_bytes;
   int64_t B = std::min<int64_t>(n, (int64_t)(budget / slot_bytes));
   if (B < 1) return IPOLE_ENOMEM;
@@ -350,7 +350,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     g.cap = cap; g.base = base; g.count = cnt; g.order = order; g.pixels = d_pixels;
     g.path = c->d_path; g.nsteps = c->d_nsteps; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
     g.long_list = c->d_long; g.long_count = c->d_small;
-    if ((rc = launch_geodesic(c, g, LK_GEO, cnt)) != IPOLE_OK) return rc;
+    if ((rc = launch_geodesic(c, g, LK_GEO, cnt, c->stream)) != IPOLE_OK) return rc;
     if (cap < max_steps) {
       CK(cudaEventRecord(c->ev_geo, c->stream));
       CK(cudaStreamWaitEvent(c->side, c->ev_geo, 0));
@@ -360,10 +360,10 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = cap; t.base = base; t.count = cnt; t.order = order;
     t.path = c->d_path; t.nsteps = c->d_nsteps; t.queue = c->d_queues + (qi++);
     t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
-    if ((rc = launch_transfer(c, t, cnt)) != IPOLE_OK) return rc;
+    if ((rc = launch_transfer(c, t, LK_RT, cnt, c->stream)) != IPOLE_OK) return rc;
     c->stats.n_batches++;
     if (cap < max_steps) {   // the transfer kernel just queued keeps the GPU busy while the host waits here
-      if ((rc = listed(n_long)) != IPOLE_OK) return rc;
+      if ((rc = listed(c->ev_geo, n_long)) != IPOLE_OK) return rc;
       if ((rc = long_pass(n_long)) != IPOLE_OK) return rc;
     }
   }
@@ -380,16 +380,16 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
 
   // ---- a-9: totals ----
   {
-    const int s = span_begin(c, LK_OTHER);
+    const int s = span_begin(c, LK_OTHER, c->stream);
     const int nb = (int)std::min<int64_t>(REDUCE_BLOCKS, (n + 255) / 256);
     k_reduce_partial<<<nb, 256, 0, c->stream>>>(n, I, Q, U, V, c->d_nsteps, c->d_nturn, c->d_part);
     const double pix_rad = c->cam.pix * c->units.L_unit / c->units.D_cm;
     k_reduce_final<<<1, 32, 0, c->stream>>>(c->d_part, nb, pix_rad * pix_rad * 1e23, c->d_red);
     c->stats.n_launches += 2;
-    span_end(c, s);
+    span_end(c, s, c->stream);
     CK(cudaGetLastError());
   }
-  span_end(c, total);
+  span_end(c, total, c->stream);
   c->have_image = true;
   c->last_n = n;
   return IPOLE_OK;
