@@ -181,24 +181,26 @@ void span_end(ipole_ctx* c, int s, cudaStream_t st) {
   if (s >= 0) cudaEventRecord(c->spans[s].b, st);
 }
 
-int grid_for(ipole_ctx* c, int occ, int threads, int64_t rays) {
-  const int64_t full = (int64_t)c->n_sm * std::max(occ, 1);
+// `reserve` blocks are left out of a full grid so that the few blocks of a long-ray pass on the side stream find a
+// free slot at once instead of waiting for a (persistent) bulk block to exit
+int grid_for(ipole_ctx* c, int occ, int threads, int64_t rays, int reserve = 0) {
+  const int64_t full = std::max<int64_t>(1, (int64_t)c->n_sm * std::max(occ, 1) - reserve);
   const int64_t need = (rays + threads - 1) / threads;
   return (int)std::max<int64_t>(1, std::min(full, need));
 }
 
-int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays, cudaStream_t st) {
+int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays, cudaStream_t st, int reserve = 0) {
   const int s = span_begin(c, kind, st);
-  k_geodesic<<<grid_for(c, c->occ_geo, IPOLE_GEO_THREADS, rays), IPOLE_GEO_THREADS, 0, st>>>(a);
+  k_geodesic<<<grid_for(c, c->occ_geo, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
   span_end(c, s, st);
   c->stats.n_launches++;
   CK(cudaGetLastError());
   return IPOLE_OK;
 }
 
-int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_t st) {
+int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_t st, int reserve = 0) {
   const int s = span_begin(c, kind, st);
-  const int g = grid_for(c, c->occ_rt[c->model], IPOLE_RT_THREADS, rays);
+  const int g = grid_for(c, c->occ_rt[c->model], IPOLE_RT_THREADS, rays, reserve);
   if (c->model == MODEL_ADAF) k_transfer<MODEL_ADAF><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
   else if (c->model == MODEL_SLAB) k_transfer<MODEL_SLAB><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
   else k_transfer<MODEL_GRID><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
@@ -343,6 +345,8 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   if (B < 1) return IPOLE_ENOMEM;
   if ((rc = ensure_path(c, (size_t)B * slot_bytes)) != IPOLE_OK) return rc;
   int n_long = 0;
+  // with few batches the long-ray passes cannot wait for kernel boundaries: keep 8 block slots free for them
+  const int reserve = (cap < max_steps && (n + B - 1) / B <= 16) ? 8 : 0;
   for (int64_t base = 0; base < n; base += B) {
     const int64_t cnt = std::min(B, n - base);
     if (qi + 2 > N_QUEUES) return IPOLE_EINVAL;
@@ -350,7 +354,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     g.cap = cap; g.base = base; g.count = cnt; g.order = order; g.pixels = d_pixels;
     g.path = c->d_path; g.nsteps = c->d_nsteps; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
     g.long_list = c->d_long; g.long_count = c->d_small;
-    if ((rc = launch_geodesic(c, g, LK_GEO, cnt, c->stream)) != IPOLE_OK) return rc;
+    if ((rc = launch_geodesic(c, g, LK_GEO, cnt, c->stream, reserve)) != IPOLE_OK) return rc;
     if (cap < max_steps) {
       CK(cudaEventRecord(c->ev_geo, c->stream));
       CK(cudaStreamWaitEvent(c->side, c->ev_geo, 0));
@@ -360,7 +364,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = cap; t.base = base; t.count = cnt; t.order = order;
     t.path = c->d_path; t.nsteps = c->d_nsteps; t.queue = c->d_queues + (qi++);
     t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
-    if ((rc = launch_transfer(c, t, LK_RT, cnt, c->stream)) != IPOLE_OK) return rc;
+    if ((rc = launch_transfer(c, t, LK_RT, cnt, c->stream, reserve)) != IPOLE_OK) return rc;
     c->stats.n_batches++;
     if (cap < max_steps) {   // the transfer kernel just queued keeps the GPU busy while the host waits here
       if ((rc = listed(c->ev_geo, n_long)) != IPOLE_OK) return rc;
