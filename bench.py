@@ -23,9 +23,12 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# FP64 operations per geodesic step of each kernel, counted by ncu on this code (DFMA = 2, DADD/DMUL = 1;
-# smsp__sass_thread_inst_executed_op_d{fma,add,mul}_pred_on.sum / total steps), see profiles/ and DESIGN.md 7.
-FLOP_PER_STEP = {"transfer_adaf": None, "geodesic": None, "transfer_grid": None}
+# FP64 operations per geodesic step of each kernel as shipped, counted by ncu (DFMA = 2, DADD/DMUL = 1;
+# smsp__sass_thread_inst_executed_op_d{fma,add,mul}_pred_on.sum / thread-steps of the launch): profiles/r1_k_*.txt,
+# DESIGN.md section 7.  The grid figure is the average over all steps of a ray, most of which cross no plasma.
+FLOP_PER_STEP = {"transfer_adaf": 1917.0, "transfer_grid": 596.0, "geodesic_adaf": 1121.0, "geodesic_grid": 1325.0}
+# DRAM bytes per step of k_transfer (dram__bytes_read + write of one launch / its thread-steps, same captures)
+DRAM_BYTES_PER_STEP = {"transfer_adaf": 64.2, "transfer_grid": 74.6}
 # ALU roofline denominator: 148 SMs x 4 sub-partitions x 16 FP64 lanes x 2 flop x 1.965 GHz
 FP64_PEAK_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
 
@@ -251,17 +254,23 @@ def main():
     # ---- roofline of the dominant kernel (k_transfer), live CUDA-event time of the last timed image ----
     key = "transfer_" + wl["kind"]
     dfma_tf, _ = g.fp64_peak()
-    n_rt = max(1, st["n_batches"] + (1 if st["n_long"] else 0))
+    n_rt = max(1, st["n_batches"])          # bulk launches; the long-ray passes run beside them on a side stream
     rt_ms = st["ms_transfer"]
     roof = {"bound": "alu", "kernel": "k_transfer<%s>" % wl["kind"], "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
             "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz; DFMA micro-benchmark on this GPU: %.1f" % dfma_tf,
             "launches": n_rt, "avg_launch_ms": rt_ms / n_rt, "kernel_share_of_step": rt_ms / st["ms_total"],
-            "steps_per_launch": st["total_steps"] / n_rt, "traffic": None}
-    if FLOP_PER_STEP.get(key):
-        ach = FLOP_PER_STEP[key] * st["total_steps"] / (rt_ms * 1e-3) / 1e12
-        roof.update(achieved=ach, frac=ach / FP64_PEAK_TFLOPS, flop_per_step=FLOP_PER_STEP[key])
-    else:
-        roof.update(achieved=None, frac=None)
+            "steps_per_launch": st["total_steps"] / n_rt,
+            "traffic": DRAM_BYTES_PER_STEP[key] * st["total_steps"] / n_rt,
+            "traffic_note": "ncu dram__bytes_read+write per launch (profiles/r1_k_transfer_*.txt), scaled by steps; "
+                            "algorithmic: 64 B per step (one path record read)"}
+    ach = FLOP_PER_STEP[key] * st["total_steps"] / (rt_ms * 1e-3) / 1e12
+    roof.update(achieved=ach, frac=ach / FP64_PEAK_TFLOPS, flop_per_step=FLOP_PER_STEP[key])
+    # the whole step against the same roofline: every FP64 operation of both hot kernels over the image time
+    fl_step = (FLOP_PER_STEP[key] + FLOP_PER_STEP["geodesic_" + wl["kind"]]) * st["total_steps"]
+    roof["whole_step"] = {"achieved": fl_step / (st["ms_total"] * 1e-3) / 1e12,
+                          "frac": fl_step / (st["ms_total"] * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+                          "geodesic_tflops": FLOP_PER_STEP["geodesic_" + wl["kind"]] * st["total_steps"]
+                                             / (st["ms_geodesic"] * 1e-3) / 1e12}
     roof["hbm_path_gbs"] = 128.0 * st["total_steps"] / ((st["ms_geodesic"] + st["ms_transfer"]) * 1e-3) / 1e9
 
     line = {"metric": "rays_per_s", "value": value, "unit": "rays/s", "n_gpus": world, "steps": args.steps,
@@ -275,7 +284,7 @@ def main():
             "images_per_s": value / rays, "steps_per_s": world * st["total_steps"] * args.steps / (ms * 1e-3),
             "mean_steps_per_ray": st["total_steps"] / rays,
             "stage_ms": {"probe_sort": st["ms_probe"], "geodesic": st["ms_geodesic"], "transfer": st["ms_transfer"],
-                         "total": st["ms_total"], "batches": st["n_batches"], "path_cap": st["path_cap"],
+                         "long_rays_side_stream": st["ms_long"], "total": st["ms_total"], "batches": st["n_batches"], "path_cap": st["path_cap"],
                          "long_rays": st["n_long"]},
             "flux_jy": st["flux_jy"], "lp": st["lp"], "cp": st["cp"], "ring_rays": st["n_ring"],
             "gpu_launches": st["n_launches"] * args.steps, "roofline": roof, "e2e": e2e, "clocks": clocks,

@@ -252,6 +252,9 @@ struct RtArgs {
 #ifndef IPOLE_RT_MINB_ANALYTIC
 #define IPOLE_RT_MINB_ANALYTIC 3
 #endif
+#ifndef IPOLE_GRID_PREFETCH
+#define IPOLE_GRID_PREFETCH 0
+#endif
 #ifndef IPOLE_RT_SYNC
 #define IPOLE_RT_SYNC 0
 #endif
@@ -325,6 +328,9 @@ k_transfer(const __grid_constant__ RtArgs A) {
     if (MODEL == MODEL_GRID) {
       const GridParams& M = *(const GridParams*)model;
       maybe = !(Xm[1] > M.lx_out + 1e-6);  // certainly beyond r_out: no plasma (the exact test is in plasma_grid)
+#if IPOLE_GRID_PREFETCH
+      if (maybe) grid_prefetch(M, Xm);
+#endif
     }
     if (lit || maybe) {
       Point p; Sym7 g; Inv6 gi; double Am[4][4];

@@ -172,6 +172,25 @@ __device__ __forceinline__ bool plasma_grid(const Geom& G, const GridParams& M, 
   return true;
 }
 
+// Touch the 8 cell records of the stencil at X (same index arithmetic as plasma_grid) so that they are on their way
+// to L1 while the metric and the transport generator are being computed.
+__device__ __forceinline__ void grid_prefetch(const GridParams& M, const double X[4]) {
+  if (X[1] > M.lx_out || X[1] < M.startx[0]) return;
+  const double i0f = floor((X[1] - M.startx[0]) * M.idx[0] - 0.5), j0f = floor((X[2] - M.startx[1]) * M.idx[1] - 0.5);
+  const double k0f = floor((X[3] - M.startx[2]) * M.idx[2] - 0.5);
+  const int i0 = clampi((int)i0f, 0, M.N1 - 1), i1 = clampi((int)i0f + 1, 0, M.N1 - 1);
+  const int j0 = clampi((int)j0f, 0, M.N2 - 1), j1 = clampi((int)j0f + 1, 0, M.N2 - 1);
+  long long kk = (long long)k0f % M.N3; if (kk < 0) kk += M.N3;
+  const int k0 = (int)kk, k1 = (k0 + 1 == M.N3) ? 0 : k0 + 1;
+  const size_t row[4] = {((size_t)i0 * M.N2 + j0) * M.N3, ((size_t)i0 * M.N2 + j1) * M.N3,
+                         ((size_t)i1 * M.N2 + j0) * M.N3, ((size_t)i1 * M.N2 + j1) * M.N3};
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(M.cells + (row[c] + k0) * 8));
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(M.cells + (row[c] + k1) * 8));
+  }
+}
+
 // eps^{mu a b c} p_a q_b w_c with [0123] = +1
 __device__ __forceinline__ void levi4(const double p[4], const double q[4], const double w[4], double o[4]) {
   const double m01 = q[0] * w[1] - q[1] * w[0], m02 = q[0] * w[2] - q[2] * w[0], m03 = q[0] * w[3] - q[3] * w[0];
