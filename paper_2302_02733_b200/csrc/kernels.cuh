@@ -252,14 +252,11 @@ struct RtArgs {
 #ifndef IPOLE_RT_MINB_ANALYTIC
 #define IPOLE_RT_MINB_ANALYTIC 3
 #endif
-#ifndef IPOLE_GRID_PREFETCH
-#define IPOLE_GRID_PREFETCH 0
-#endif
 #ifndef IPOLE_RT_SYNC
 #define IPOLE_RT_SYNC 0
 #endif
 #ifndef IPOLE_RT_PREFETCH
-#define IPOLE_RT_PREFETCH 0
+#define IPOLE_RT_PREFETCH 1   // prefetch.global.L1 of the next path record: 2-3 % (profiles/r1_notes.md)
 #endif
 
 // a-4 ... a-7, a-8.  Lane-level refill as in k_geodesic.  Per step: midpoint (Xm, Km), generator A = Gamma.Km,
@@ -324,14 +321,11 @@ k_transfer(const __grid_constant__ RtArgs A) {
     double Xm[4], Km[4];
 #pragma unroll
     for (int m = 0; m < 4; ++m) { Xm[m] = 0.5 * (Xlo[m] + Xhi[m]); Km[m] = 0.5 * (Klo[m] + Khi[m]); }
+    // `maybe`: this step may cross plasma.  For the grid model the gather comes first (it needs no metric), so a step
+    // that is dark so far and crosses no plasma costs eight record loads and nothing else.
     bool maybe = true;
-    if (MODEL == MODEL_GRID) {
-      const GridParams& M = *(const GridParams*)model;
-      maybe = !(Xm[1] > M.lx_out + 1e-6);  // certainly beyond r_out: no plasma (the exact test is in plasma_grid)
-#if IPOLE_GRID_PREFETCH
-      if (maybe) grid_prefetch(M, Xm);
-#endif
-    }
+    double prim[8];
+    if (MODEL == MODEL_GRID) maybe = grid_gather(*(const GridParams*)model, Xm, prim);
     if (lit || maybe) {
       Point p; Sym7 g; Inv6 gi; double Am[4][4];
       transport_generator(C.G, Xm, Km, p, g, gi, Am);
@@ -341,7 +335,7 @@ k_transfer(const __grid_constant__ RtArgs A) {
       // coefficients and the 4x4 step, which touch the Stokes numbers alone: same result, but the generator and
       // the tetrad are dead while the register-hungry part runs
       PlasmaFrame F;
-      const bool applied = maybe && plasma_frame<MODEL>(C.G, model, A.units, Xm, Km, p, g, gi, st, F);
+      const bool applied = maybe && plasma_frame<MODEL>(C.G, model, A.units, Xm, Km, p, g, gi, prim, st, F);
       lit |= applied;
       if (lit) { transport_apply(Am, h, st.f1); transport_apply(Am, h, st.f2); }
       if (applied) plasma_apply<MODEL>(A.units, F, dl, st);

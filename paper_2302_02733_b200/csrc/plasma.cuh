@@ -109,9 +109,10 @@ __device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? l
 // records of 8 doubles (64 B = two full sectors, 16-B aligned), so one corner of the stencil is four 128-bit
 // read-only loads (ld.global.nc.v2.f64) instead of eight scattered 8-byte ones, and the two k-neighbours share a
 // 128-B line: 8 lines per evaluation instead of up to 32 sectors in 32 different lines.
-__device__ __forceinline__ bool plasma_grid(const Geom& G, const GridParams& M, const double X[4], const Point& p,
-                                            const Sym7& g, const Inv6& gi, Plasma& P) {
-  if (p.r > M.r_out || X[1] < M.startx[0]) return false;
+// Step 1 (needs no metric): the eight interpolated primitives at X.  Returns false where there is certainly no
+// plasma (outside the lattice in X1, or rho <= 0 or u <= 0 after interpolation).
+__device__ __forceinline__ bool grid_gather(const GridParams& M, const double X[4], double prim[8]) {
+  if (X[1] > M.lx_out + 1e-9 || X[1] < M.startx[0]) return false;   // r_out itself is tested exactly in grid_state
   const double fi = (X[1] - M.startx[0]) * M.idx[0] - 0.5;
   const double fj = (X[2] - M.startx[1]) * M.idx[1] - 0.5;
   const double fk = (X[3] - M.startx[2]) * M.idx[2] - 0.5;
@@ -127,7 +128,8 @@ __device__ __forceinline__ bool plasma_grid(const Geom& G, const GridParams& M, 
   const double w[8] = {wi0 * wj0 * wk0, wi0 * wj0 * dk, wi0 * dj * wk0, wi0 * dj * dk,
                        di * wj0 * wk0,  di * wj0 * dk,  di * dj * wk0,  di * dj * dk};
   const size_t off[8] = {o00 + k0, o00 + k1, o01 + k0, o01 + k1, o10 + k0, o10 + k1, o11 + k0, o11 + k1};
-  double prim[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+  for (int q = 0; q < 8; ++q) prim[q] = 0.0;
   const double2* C2 = reinterpret_cast<const double2*>(M.cells);
 #pragma unroll
   for (int c = 0; c < 8; ++c) {
@@ -138,8 +140,14 @@ __device__ __forceinline__ bool plasma_grid(const Geom& G, const GridParams& M, 
     prim[4] = fma(w[c], cc.x, prim[4]); prim[5] = fma(w[c], cc.y, prim[5]);
     prim[6] = fma(w[c], d.x, prim[6]);  prim[7] = fma(w[c], d.y, prim[7]);
   }
+  return prim[0] > 0.0 && prim[1] > 0.0;
+}
+
+// Step 2: fluid four-velocity, field four-vector, n_e, Theta_e, B from the primitives and the metric at X.
+__device__ __forceinline__ bool grid_state(const Geom& G, const GridParams& M, const double prim[8], const Point& p,
+                                           const Sym7& g, const Inv6& gi, Plasma& P) {
+  if (p.r > M.r_out) return false;
   const double rho = prim[0], uu = prim[1];
-  if (!(rho > 0.0) || !(uu > 0.0)) return false;
   const double alpha_l = ip_rsqrt(-gi.c00);
   // q2 = g_ij U^i U^j (spatial block of the sparse metric)
   const double U1 = prim[2], U2 = prim[3], U3 = prim[4];
@@ -172,23 +180,10 @@ __device__ __forceinline__ bool plasma_grid(const Geom& G, const GridParams& M, 
   return true;
 }
 
-// Touch the 8 cell records of the stencil at X (same index arithmetic as plasma_grid) so that they are on their way
-// to L1 while the metric and the transport generator are being computed.
-__device__ __forceinline__ void grid_prefetch(const GridParams& M, const double X[4]) {
-  if (X[1] > M.lx_out || X[1] < M.startx[0]) return;
-  const double i0f = floor((X[1] - M.startx[0]) * M.idx[0] - 0.5), j0f = floor((X[2] - M.startx[1]) * M.idx[1] - 0.5);
-  const double k0f = floor((X[3] - M.startx[2]) * M.idx[2] - 0.5);
-  const int i0 = clampi((int)i0f, 0, M.N1 - 1), i1 = clampi((int)i0f + 1, 0, M.N1 - 1);
-  const int j0 = clampi((int)j0f, 0, M.N2 - 1), j1 = clampi((int)j0f + 1, 0, M.N2 - 1);
-  long long kk = (long long)k0f % M.N3; if (kk < 0) kk += M.N3;
-  const int k0 = (int)kk, k1 = (k0 + 1 == M.N3) ? 0 : k0 + 1;
-  const size_t row[4] = {((size_t)i0 * M.N2 + j0) * M.N3, ((size_t)i0 * M.N2 + j1) * M.N3,
-                         ((size_t)i1 * M.N2 + j0) * M.N3, ((size_t)i1 * M.N2 + j1) * M.N3};
-#pragma unroll
-  for (int c = 0; c < 4; ++c) {
-    asm volatile("prefetch.global.L1 [%0];" ::"l"(M.cells + (row[c] + k0) * 8));
-    asm volatile("prefetch.global.L1 [%0];" ::"l"(M.cells + (row[c] + k1) * 8));
-  }
+__device__ __forceinline__ bool plasma_grid(const Geom& G, const GridParams& M, const double X[4], const Point& p,
+                                            const Sym7& g, const Inv6& gi, Plasma& P) {
+  double prim[8];
+  return grid_gather(M, X, prim) && grid_state(G, M, prim, p, g, gi, P);
 }
 
 // eps^{mu a b c} p_a q_b w_c with [0123] = +1
@@ -234,12 +229,13 @@ struct PlasmaFrame {
 template <int MODEL>
 __device__ __forceinline__ bool plasma_frame(const Geom& G, const void* model, const Units& U, const double X[4],
                                              const double K[4], const Point& p, const Sym7& g, const Inv6& gi,
-                                             PolState& st, PlasmaFrame& F) {
+                                             const double* prim /* grid model: from grid_gather */, PolState& st,
+                                             PlasmaFrame& F) {
   Plasma P;
   bool present;
   if (MODEL == MODEL_ADAF) present = plasma_adaf(G, *(const AdafParams*)model, X, p, g, gi, P);
   else if (MODEL == MODEL_SLAB) present = plasma_slab(G, *(const SlabParams*)model, X, p, g, P);
-  else present = plasma_grid(G, *(const GridParams*)model, X, p, g, gi, P);
+  else present = grid_state(G, *(const GridParams*)model, prim, p, g, gi, P);
   if (!present) return false;
 
   double kcov[4], ucov[4];
