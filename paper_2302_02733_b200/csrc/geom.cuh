@@ -46,7 +46,125 @@ struct Inv6 {
 
 struct Point {      // scalar functions of position shared by everything evaluated at X
   double r, th, tp, tpp, s, c, Sig, f, sqrtmg, iSig;
+  double s2x, c2x;  // sin, cos of 2 pi X2 (only when hslope != 1)
 };
+
+// r, theta(X2) and its derivatives, sin/cos theta: one exp and one (two when hslope != 1) sincos
+__device__ __forceinline__ void point_full(const Geom& G, const double X[4], Point& p) {
+  p.r = ip_exp(X[1]);
+  if (G.h_is_one) {
+    p.th = M_PI * X[2]; p.tp = M_PI; p.tpp = 0.0;
+    p.s2x = 0.0; p.c2x = 1.0;
+  } else {
+    ip_sincos(2.0 * M_PI * X[2], &p.s2x, &p.c2x);
+    const double q = 1.0 - G.hslope;
+    p.th = M_PI * X[2] + 0.5 * q * p.s2x;
+    p.tp = M_PI * (1.0 + q * p.c2x);
+    p.tpp = -2.0 * M_PI * M_PI * q * p.s2x;
+  }
+  ip_sincos(p.th, &p.s, &p.c);
+}
+
+// sin d and cos d - 1 for |d| <= 0.2 (Taylor to d^13 / d^12: truncation < 1e-19 relative)
+__device__ __forceinline__ void sincosm1_small(double d, double& sd, double& cm1) {
+  const double w = d * d;
+  double ps = 1.6059043836821613e-10;              // 1/13!
+  ps = fma(ps, w, -2.5052108385441720e-08);        // -1/11!
+  ps = fma(ps, w, 2.7557319223985893e-06);         // 1/9!
+  ps = fma(ps, w, -1.9841269841269841e-04);        // -1/7!
+  ps = fma(ps, w, 8.3333333333333332e-03);         // 1/5!
+  ps = fma(ps, w, -1.6666666666666666e-01);        // -1/3!
+  sd = fma(d * w, ps, d);
+  double pc = 2.0876756987868100e-09;              // 1/12!
+  pc = fma(pc, w, -2.7557319223985888e-07);        // -1/10!
+  pc = fma(pc, w, 2.4801587301587302e-05);         // 1/8!
+  pc = fma(pc, w, -1.3888888888888889e-03);        // -1/6!
+  pc = fma(pc, w, 4.1666666666666664e-02);         // 1/4!
+  pc = fma(pc, w, -0.5);
+  cm1 = w * pc;
+}
+
+// The same scalars at X0 + (0, d1, d2, .) from those at X0, for the small displacements of the RK4 stages
+// (|d1| <= 0.06, |2 pi d2| <= 0.2: guaranteed by the step rule for eps <= 0.04, R-4):
+//   r = r0 + r0 expm1(d1),   sin(t0 + dt) = s0 + (s0 (cos dt - 1) + c0 sin dt),   cos likewise,
+// with short Taylor polynomials in place of one exp and one or two full sincos.  The increments are added to the
+// base values, so the relative accuracy of sin(theta) near the axis is that of the base value.
+__device__ __forceinline__ void point_shift(const Geom& G, const Point& b, double d1, double d2, Point& p) {
+  double e = 2.7557319223985893e-06;               // expm1(d) = d + d^2/2 + ... + d^9/9!
+  e = fma(e, d1, 2.4801587301587302e-05);
+  e = fma(e, d1, 1.9841269841269841e-04);
+  e = fma(e, d1, 1.3888888888888889e-03);
+  e = fma(e, d1, 8.3333333333333332e-03);
+  e = fma(e, d1, 4.1666666666666664e-02);
+  e = fma(e, d1, 1.6666666666666666e-01);
+  e = fma(e, d1, 0.5);
+  e = fma(d1 * d1, e, d1);
+  p.r = fma(b.r, e, b.r);
+  double dth;
+  if (G.h_is_one) {
+    dth = M_PI * d2;
+    p.tp = M_PI; p.tpp = 0.0; p.s2x = 0.0; p.c2x = 1.0;
+  } else {
+    double sa, cam1;
+    sincosm1_small(2.0 * M_PI * d2, sa, cam1);
+    const double ds2 = fma(b.s2x, cam1, b.c2x * sa), dc2 = fma(b.c2x, cam1, -b.s2x * sa);
+    p.s2x = b.s2x + ds2; p.c2x = b.c2x + dc2;
+    const double q = 1.0 - G.hslope;
+    dth = fma(0.5 * q, ds2, M_PI * d2);
+    p.tp = M_PI * (1.0 + q * p.c2x);
+    p.tpp = -2.0 * M_PI * M_PI * q * p.s2x;
+  }
+  p.th = b.th + dth;
+  double sd, cm1;
+  sincosm1_small(dth, sd, cm1);
+  p.s = b.s + fma(b.s, cm1, b.c * sd);
+  p.c = b.c + fma(b.c, cm1, -b.s * sd);
+}
+
+// g_{mu nu} and g^{mu nu} from the scalars of a filled Point (no derivatives)
+template <bool WANT_INV>
+__device__ __forceinline__ void metric_assemble(const Geom& G, Point& p, Sym7& g, Inv6& gi) {
+  const double a = G.a;
+  const double r = p.r, s2 = p.s * p.s;
+  p.Sig = r * r + a * a * p.c * p.c;
+  const double tp2 = p.tp * p.tp;
+  double iS = 0.0, ir = 0.0, iSst = 0.0;
+  if (WANT_INV) {
+    // one reciprocal of the product instead of four: 1/Sigma, 1/r, 1/sin^2, 1/theta'^2
+    const double Sr = p.Sig * r, st = s2 * tp2;
+    const double t = ip_rcp(Sr * st);
+    iS = t * r * st; ir = t * p.Sig * st; iSst = t * r;   // iSst = 1/(Sigma sin^2 theta'^2)
+    p.f = 2.0 * G.mass * r * iS;
+    p.iSig = iS;
+  } else {
+    p.f = 2.0 * G.mass * r / p.Sig;
+  }
+  const double f = p.f, opf = 1.0 + f;
+  g.c00 = -1.0 + f;
+  g.c01 = f * r;
+  g.c03 = -a * f * s2;
+  g.c11 = opf * r * r;
+  g.c13 = -a * s2 * opf * r;
+  g.c22 = p.Sig * tp2;
+  g.c33 = s2 * (p.Sig + a * a * s2 * opf);
+  p.sqrtmg = r * p.tp * p.Sig * fabs(p.s);
+  if (WANT_INV) {
+    const double Del = r * r - 2.0 * G.mass * r + a * a;
+    gi.c00 = -opf;
+    gi.c01 = f * ir;
+    gi.c11 = Del * iS * ir * ir;
+    gi.c13 = a * iS * ir;
+    gi.c22 = iSst * s2;
+    gi.c33 = iSst * tp2;
+  }
+}
+
+// g_{mu nu} and g^{mu nu} at X (no derivatives)
+template <bool WANT_INV>
+__device__ __forceinline__ void metric(const Geom& G, const double X[4], Point& p, Sym7& g, Inv6& gi) {
+  point_full(G, X, p);
+  metric_assemble<WANT_INV>(G, p, g, gi);
+}
 
 __device__ __forceinline__ void theta_map(const Geom& G, double x2, double& th, double& tp, double& tpp) {
   if (G.h_is_one) {
@@ -61,46 +179,16 @@ __device__ __forceinline__ void theta_map(const Geom& G, double x2, double& th, 
   }
 }
 
-// g_{mu nu} and g^{mu nu} at X (no derivatives)
-template <bool WANT_INV>
-__device__ __forceinline__ void metric(const Geom& G, const double X[4], Point& p, Sym7& g, Inv6& gi) {
-  const double a = G.a;
-  p.r = ip_exp(X[1]);
-  theta_map(G, X[2], p.th, p.tp, p.tpp);
-  ip_sincos(p.th, &p.s, &p.c);
-  const double r = p.r, s2 = p.s * p.s;
-  p.Sig = r * r + a * a * p.c * p.c;
-  p.f = 2.0 * G.mass * r / p.Sig;
-  const double f = p.f, opf = 1.0 + f;
-  g.c00 = -1.0 + f;
-  g.c01 = f * r;
-  g.c03 = -a * f * s2;
-  g.c11 = opf * r * r;
-  g.c13 = -a * s2 * opf * r;
-  g.c22 = p.Sig * p.tp * p.tp;
-  g.c33 = s2 * (p.Sig + a * a * s2 * opf);
-  p.sqrtmg = r * p.tp * p.Sig * fabs(p.s);
-  if (WANT_INV) {
-    // one reciprocal of the product instead of four: 1/Sigma, 1/r, 1/sin^2, 1/theta'^2
-    const double tp2 = p.tp * p.tp;
-    const double Sr = p.Sig * r, st = s2 * tp2;
-    const double t = ip_rcp(Sr * st);
-    const double iS = t * r * st, ir = t * p.Sig * st, iSst = t * r;   // iSst = 1/(Sigma sin^2 theta'^2)
-    const double Del = r * r - 2.0 * G.mass * r + a * a;
-    gi.c00 = -opf;
-    gi.c01 = f * ir;
-    gi.c11 = Del * iS * ir * ir;
-    gi.c13 = a * iS * ir;
-    gi.c22 = iSst * s2;
-    gi.c33 = iSst * tp2;
-    p.iSig = iS;
-  }
-}
-
 // metric, inverse and the derivative matrices D1 = d g / d X1, D2 = d g / d X2
+__device__ __forceinline__ void metric_derivs_at(const Geom& G, Point& p, Sym7& g, Inv6& gi, Sym7& D1, Sym7& D2);
 __device__ __forceinline__ void metric_derivs(const Geom& G, const double X[4], Point& p, Sym7& g, Inv6& gi,
                                               Sym7& D1, Sym7& D2) {
-  metric<true>(G, X, p, g, gi);
+  point_full(G, X, p);
+  metric_derivs_at(G, p, g, gi, D1, D2);
+}
+// the same from a Point whose scalars (r, theta', theta'', sin, cos) are already filled
+__device__ __forceinline__ void metric_derivs_at(const Geom& G, Point& p, Sym7& g, Inv6& gi, Sym7& D1, Sym7& D2) {
+  metric_assemble<true>(G, p, g, gi);
   const double a = G.a, r = p.r, s2 = p.s * p.s, f = p.f, opf = 1.0 + f;
   const double a2 = a * a;
   const double iS2 = p.iSig * p.iSig;
@@ -126,9 +214,9 @@ __device__ __forceinline__ void metric_derivs(const Geom& G, const double X[4], 
 }
 
 // dK^l / dlambda = - Gamma^l_{mn} K^m K^n
-__device__ __forceinline__ void geodesic_accel(const Geom& G, const double X[4], const double K[4], double dK[4]) {
-  Point p; Sym7 g, D1, D2; Inv6 gi;
-  metric_derivs(G, X, p, g, gi, D1, D2);
+__device__ __forceinline__ void geodesic_accel_at(const Geom& G, Point& p, const double K[4], double dK[4]) {
+  Sym7 g, D1, D2; Inv6 gi;
+  metric_derivs_at(G, p, g, gi, D1, D2);
   double v1[4], v2[4], F[4];
   D1.mul(K, v1);
   D2.mul(K, v2);
@@ -140,6 +228,11 @@ __device__ __forceinline__ void geodesic_accel(const Geom& G, const double X[4],
   F[3] = K[1] * v1[3] + K[2] * v2[3];
   gi.mul(F, dK);
   dK[0] = -dK[0]; dK[1] = -dK[1]; dK[2] = -dK[2]; dK[3] = -dK[3];
+}
+__device__ __forceinline__ void geodesic_accel(const Geom& G, const double X[4], const double K[4], double dK[4]) {
+  Point p;
+  point_full(G, X, p);
+  geodesic_accel_at(G, p, K, dK);
 }
 
 // A^a_n = Gamma^a_{mn} K^m as a dense 4x4 (row a, column n); also returns the metric at X for the caller

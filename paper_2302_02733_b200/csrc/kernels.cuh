@@ -119,27 +119,50 @@ __device__ __forceinline__ double stepsize(const double X[4], const double K[4],
   return ip_rcp((i13 + i2) * ieps);
 }
 
-// classical RK4 on (X^1..3, K^0..3); X^0 is not integrated (static snapshot, R-9)
+// classical RK4 on (X^1..3, K^0..3); X^0 is not integrated (static snapshot, R-9).
+// SMALL (eps <= 0.04): r, sin/cos theta at the three displaced stage points come from the values at the start of
+// the step by short Taylor polynomials in the displacement (point_shift) -- one exp and one or two sincos per step
+// instead of four of each; otherwise every stage is evaluated from scratch.
+template <bool SMALL>
 __device__ __forceinline__ void rk4_push(const Geom& G, double X[4], double K[4], double h) {
   double k1[4], k2[4], k3[4], k4[4], Xt[4], Kt[4];
   Xt[0] = 0.0;
-  geodesic_accel(G, X, K, k1);
+  Point p0, pt;
+  point_full(G, X, p0);
+  pt = p0;
+  geodesic_accel_at(G, pt, K, k1);
 #pragma unroll
   for (int m = 0; m < 4; ++m) { Kt[m] = K[m] + 0.5 * h * k1[m]; }
+  if (SMALL) point_shift(G, p0, 0.5 * h * K[1], 0.5 * h * K[2], pt);
+  else {
 #pragma unroll
-  for (int m = 1; m < 4; ++m) { Xt[m] = X[m] + 0.5 * h * K[m]; }
-  geodesic_accel(G, Xt, Kt, k2);
+    for (int m = 1; m < 4; ++m) Xt[m] = X[m] + 0.5 * h * K[m];
+    point_full(G, Xt, pt);
+  }
+  geodesic_accel_at(G, pt, Kt, k2);
   double xs[4];  // x1 + 2 x2 (+ 2 x3 + x4): the X-slopes are the stage K's
 #pragma unroll
-  for (int m = 1; m < 4; ++m) { xs[m] = K[m] + 2.0 * Kt[m]; Xt[m] = X[m] + 0.5 * h * Kt[m]; }
+  for (int m = 1; m < 4; ++m) xs[m] = K[m] + 2.0 * Kt[m];
+  if (SMALL) point_shift(G, p0, 0.5 * h * Kt[1], 0.5 * h * Kt[2], pt);
+  else {
+#pragma unroll
+    for (int m = 1; m < 4; ++m) Xt[m] = X[m] + 0.5 * h * Kt[m];
+    point_full(G, Xt, pt);
+  }
 #pragma unroll
   for (int m = 0; m < 4; ++m) { Kt[m] = K[m] + 0.5 * h * k2[m]; }
-  geodesic_accel(G, Xt, Kt, k3);
+  geodesic_accel_at(G, pt, Kt, k3);
 #pragma unroll
-  for (int m = 1; m < 4; ++m) { xs[m] += 2.0 * Kt[m]; Xt[m] = X[m] + h * Kt[m]; }
+  for (int m = 1; m < 4; ++m) xs[m] += 2.0 * Kt[m];
+  if (SMALL) point_shift(G, p0, h * Kt[1], h * Kt[2], pt);
+  else {
+#pragma unroll
+    for (int m = 1; m < 4; ++m) Xt[m] = X[m] + h * Kt[m];
+    point_full(G, Xt, pt);
+  }
 #pragma unroll
   for (int m = 0; m < 4; ++m) { Kt[m] = K[m] + h * k3[m]; }
-  geodesic_accel(G, Xt, Kt, k4);
+  geodesic_accel_at(G, pt, Kt, k4);
   const double h6 = h * (1.0 / 6.0);
 #pragma unroll
   for (int m = 1; m < 4; ++m) X[m] += h6 * (xs[m] + Kt[m]);
@@ -200,13 +223,15 @@ __global__ void __launch_bounds__(IPOLE_GEO_THREADS, IPOLE_GEO_MINB) k_geodesic(
   };
 
   const double ieps = 1.0 / A.eps;
+  const bool small_steps = A.eps <= 0.04;   // displacements of the RK4 stages within point_shift's range
   fetch();
   while (have) {
     const double dl = stepsize(X, K, ieps);
     if (rec) store_record(rec + (size_t)n * REC_DOUBLES, X, K, dl);
     const double x1_before = X[1];
     const bool k2neg = K[2] < 0.0;
-    rk4_push(C.G, X, K, -dl);
+    if (small_steps) rk4_push<true>(C.G, X, K, -dl);
+    else rk4_push<false>(C.G, X, K, -dl);
     ++n;
     if ((K[2] < 0.0) != k2neg) ++nt;
     int status = 0;
