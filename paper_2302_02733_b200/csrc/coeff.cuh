@@ -87,7 +87,7 @@ __device__ __forceinline__ void bessel_ratios_series(double z, double Th, double
 // K_0/K_2 and K_1/K_2 at z = 1/Th
 __device__ __forceinline__ void bessel_ratios(double z, double Th, double& r0, double& r1) {
   int piece; double v;
-  if (pw_locate(Th, IPOLE_PW_BESSEL_E0, IPOLE_PW_BESSEL_E1, piece, v)) {
+  if (IP_LIKELY(pw_locate(Th, IPOLE_PW_BESSEL_E0, IPOLE_PW_BESSEL_E1, piece, v))) {
     const double2* t = reinterpret_cast<const double2*>(&g_pw_bessel[piece][0][0]);
     double2 c = __ldg(t + IPOLE_PW_NC - 1);
     double a = c.x, b = c.y;
@@ -106,7 +106,7 @@ __device__ __forceinline__ void bessel_ratios(double z, double Th, double& r0, d
 // f(X) of the Faraday-conversion fit (R-7)
 __device__ __forceinline__ double faraday_fX(double X) {
   int piece; double v;
-  if (pw_locate(X, IPOLE_PW_FX_E0, IPOLE_PW_FX_E1, piece, v)) {
+  if (IP_LIKELY(pw_locate(X, IPOLE_PW_FX_E0, IPOLE_PW_FX_E1, piece, v))) {
     const double2* t = reinterpret_cast<const double2*>(&g_pw_fx[piece][0][0]);
     double p = 0.0;
 #pragma unroll

@@ -17,6 +17,10 @@
 
 namespace ipole {
 
+// branch hints: the fallbacks for operands outside the fast paths are placed out of the hot instruction stream
+#define IP_LIKELY(x) __builtin_expect(!!(x), 1)
+#define IP_UNLIKELY(x) __builtin_expect(!!(x), 0)
+
 __device__ __forceinline__ double mk_double(int hi, int lo) { return __hiloint2double(hi, lo); }
 
 // 1/x for normal x (1e-290 < |x| < 1e290): MUFU.RCP64H seed (>= 20 bits), one cubic and one quadratic Newton step
@@ -136,7 +140,7 @@ __device__ __forceinline__ void ip_sincos(double x, double* sp, double* cp) {
 // any finite x: the library routine (Payne-Hanek) beyond the Cody-Waite range; the branch is never taken on the
 // workloads of DESIGN.md section 5 (rotation angles per step are small)
 __device__ __forceinline__ void ip_sincos_any(double x, double* sp, double* cp) {
-  if (fabs(x) <= 1e5) ip_sincos(x, sp, cp);
+  if (IP_LIKELY(fabs(x) <= 1e5)) ip_sincos(x, sp, cp);
   else sincos(x, sp, cp);
 }
 __device__ __forceinline__ double ip_cos_any(double x) {

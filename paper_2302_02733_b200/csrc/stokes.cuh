@@ -23,7 +23,8 @@ __device__ __forceinline__ double dot3(const double u[3], const double v[3]) { r
 // a/b: the fast quotient where b is safely normal, the IEEE division otherwise (coefficients near the subnormal range)
 __device__ __forceinline__ double guarded_div(double a, double b) {
   const double ab = fabs(b);
-  return (ab > 1e-290 && ab < 1e290) ? ip_div(a, b) : a / b;
+  if (IP_LIKELY(ab > 1e-290 && ab < 1e290)) return ip_div(a, b);
+  return a / b;
 }
 
 // S <- O(s) S + P(s) J ; al = (aI,aQ,aU,aV), rh = (rQ,rU,rV)
@@ -36,14 +37,14 @@ __device__ __forceinline__ void stokes_step(const double al[4], const double rh[
   const double m = fmax(fmax(fabs(al[1]), fmax(fabs(al[2]), fabs(al[3]))), fmax(fabs(rh[0]), fmax(fabs(rh[1]), fabs(rh[2]))));
   const double t0 = ip_expm1(-aI * s);
   const double ex = 1.0 + t0;
-  if (m == 0.0) {
+  if (IP_UNLIKELY(m == 0.0)) {
     const double E = (aI == 0.0) ? s : -guarded_div(t0, aI);
 #pragma unroll
     for (int i = 0; i < 4; ++i) S[i] = ex * S[i] + E * J[i];
     return;
   }
   double a[3], r[3];
-  if (m > 1e-290) {
+  if (IP_LIKELY(m > 1e-290)) {
     const double im = ip_rcp(m);
     a[0] = al[1] * im; a[1] = al[2] * im; a[2] = al[3] * im;
     r[0] = rh[0] * im; r[1] = rh[1] * im; r[2] = rh[2] * im;
@@ -83,13 +84,13 @@ __device__ __forceinline__ void stokes_step(const double al[4], const double rh[
   const double Ic1 = 0.5 * (Ep + Em), Is1 = 0.5 * (Ep - Em);
   double Ic2, Is2;
   const double den = aI * aI + L2 * L2;
-  if (den == 0.0) { Ic2 = s; Is2 = 0.0; }
+  if (IP_UNLIKELY(den == 0.0)) { Ic2 = s; Is2 = 0.0; }
   else {
     const double omc = (c > 0.0) ? sn * sn * ip_rcp(1.0 + c) : 1.0 - c;   // 1 - cos(L2 s)
     const double re = omc - t0 * c;                                  // Re(1 - e^{-aI s} e^{i L2 s})
     const double im2 = -ex * sn;
     const double nc = re * aI - im2 * L2, ns = re * L2 + im2 * aI;
-    if (den > 1e-280) { const double iden = ip_rcp(den); Ic2 = nc * iden; Is2 = ns * iden; }
+    if (IP_LIKELY(den > 1e-280)) { const double iden = ip_rcp(den); Ic2 = nc * iden; Is2 = ns * iden; }
     else { Ic2 = nc / den; Is2 = ns / den; }   // 1/den would overflow (coefficients near the subnormal range)
   }
   // weights of (1, M2, M3, M4) for O and for P
@@ -131,13 +132,13 @@ __device__ __forceinline__ void stokes_step_qv(double aI, double aQ, double aV, 
   const double m = fmax(fmax(fabs(aQ), fabs(aV)), fmax(fabs(rQ), fabs(rV)));
   const double t0 = ip_expm1(-aI * s);
   const double ex = 1.0 + t0;
-  if (m == 0.0) {
+  if (IP_UNLIKELY(m == 0.0)) {
     const double E = (aI == 0.0) ? s : -guarded_div(t0, aI);
     S[0] = ex * S[0] + E * jI; S[1] = ex * S[1] + E * jQ; S[2] = ex * S[2]; S[3] = ex * S[3] + E * jV;
     return;
   }
   double a0, a2, r0, r2;
-  if (m > 1e-290) {
+  if (IP_LIKELY(m > 1e-290)) {
     const double im = ip_rcp(m);
     a0 = aQ * im; a2 = aV * im; r0 = rQ * im; r2 = rV * im;
   } else {
@@ -171,13 +172,13 @@ __device__ __forceinline__ void stokes_step_qv(double aI, double aQ, double aV, 
   const double Ic1 = 0.5 * (Ep + Em), Is1 = 0.5 * (Ep - Em);
   double Ic2, Is2;
   const double den = aI * aI + L2 * L2;
-  if (den == 0.0) { Ic2 = s; Is2 = 0.0; }
+  if (IP_UNLIKELY(den == 0.0)) { Ic2 = s; Is2 = 0.0; }
   else {
     const double omc = (c > 0.0) ? sn * sn * ip_rcp(1.0 + c) : 1.0 - c;
     const double re = omc - t0 * c;
     const double im2 = -ex * sn;
     const double nc = re * aI - im2 * L2, ns = re * L2 + im2 * aI;
-    if (den > 1e-280) { const double iden = ip_rcp(den); Ic2 = nc * iden; Is2 = ns * iden; }
+    if (IP_LIKELY(den > 1e-280)) { const double iden = ip_rcp(den); Ic2 = nc * iden; Is2 = ns * iden; }
     else { Ic2 = nc / den; Is2 = ns / den; }
   }
   const double exc = ex * c;
