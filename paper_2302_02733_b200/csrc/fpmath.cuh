@@ -23,6 +23,17 @@ namespace ipole {
 
 __device__ __forceinline__ double mk_double(int hi, int lo) { return __hiloint2double(hi, lo); }
 
+// 256-bit global accesses (sm_100: LDG/STG.E.ENL2.256), 32-byte aligned addresses
+__device__ __forceinline__ void ld_global_v4(const double* p, double& a, double& b, double& c, double& d) {
+  asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p) : "memory");
+}
+__device__ __forceinline__ void ld_global_nc_v4(const double* p, double& a, double& b, double& c, double& d) {
+  asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
+}
+__device__ __forceinline__ void st_global_v4(double* p, double a, double b, double c, double d) {
+  asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+
 // 1/x for normal x (1e-290 < |x| < 1e290): MUFU.RCP64H seed (>= 20 bits), one cubic and one quadratic Newton step
 __device__ __forceinline__ double ip_rcp(double x) {
   double y;

@@ -14,7 +14,8 @@
 namespace ipole {
 
 // One path record = one point of the geodesic: X1,X2,X3, K0..K3, dl (step from this point to the next one).
-// 64 B = two 32-B sectors; the records of one ray are contiguous, so every sector written or read is full.
+// 64 B = two 32-B sectors, moved as two 256-bit accesses; the records of one ray are contiguous, so every sector
+// written or read is full.
 constexpr int REC_DOUBLES = 8;
 
 struct CamDev {
@@ -171,18 +172,13 @@ __device__ __forceinline__ void rk4_push(const Geom& G, double X[4], double K[4]
 }
 
 __device__ __forceinline__ void store_record(double* rec, const double X[4], const double K[4], double dl) {
-  double2* r2 = reinterpret_cast<double2*>(rec);
-  r2[0] = make_double2(X[1], X[2]);
-  r2[1] = make_double2(X[3], K[0]);
-  r2[2] = make_double2(K[1], K[2]);
-  r2[3] = make_double2(K[3], dl);
+  st_global_v4(rec, X[1], X[2], X[3], K[0]);
+  st_global_v4(rec + 4, K[1], K[2], K[3], dl);
 }
 __device__ __forceinline__ void load_record(const double* rec, double X[4], double K[4], double& dl) {
-  const double2* r2 = reinterpret_cast<const double2*>(rec);
-  const double2 a = r2[0], b = r2[1], c = r2[2], d = r2[3];
-  X[0] = 0.0; X[1] = a.x; X[2] = a.y; X[3] = b.x;
-  K[0] = b.y; K[1] = c.x; K[2] = c.y; K[3] = d.x;
-  dl = d.y;
+  X[0] = 0.0;
+  ld_global_v4(rec, X[1], X[2], X[3], K[0]);
+  ld_global_v4(rec + 4, K[1], K[2], K[3], dl);
 }
 
 #ifndef IPOLE_GEO_THREADS

@@ -106,8 +106,8 @@ __device__ __forceinline__ bool plasma_slab(const Geom& G, const SlabParams& M, 
 __device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
 
 // FP64 trilinear interpolation of the 8 fields.  The caller's SoA planes are re-tiled at load time into cell-major
-// records of 8 doubles (64 B = two full sectors, 16-B aligned), so one corner of the stencil is four 128-bit
-// read-only loads (ld.global.nc.v2.f64) instead of eight scattered 8-byte ones, and the two k-neighbours share a
+// records of 8 doubles (64 B = two full sectors, 16-B aligned), so one corner of the stencil is two 256-bit
+// read-only loads (ld.global.nc.v4.f64) instead of eight scattered 8-byte ones, and the two k-neighbours share a
 // 128-B line: 8 lines per evaluation instead of up to 32 sectors in 32 different lines.
 // Step 1 (needs no metric): the eight interpolated primitives at X.  Returns false where there is certainly no
 // plasma (outside the lattice in X1, or rho <= 0 or u <= 0 after interpolation).
@@ -130,15 +130,14 @@ __device__ __forceinline__ bool grid_gather(const GridParams& M, const double X[
   const size_t off[8] = {o00 + k0, o00 + k1, o01 + k0, o01 + k1, o10 + k0, o10 + k1, o11 + k0, o11 + k1};
 #pragma unroll
   for (int q = 0; q < 8; ++q) prim[q] = 0.0;
-  const double2* C2 = reinterpret_cast<const double2*>(M.cells);
 #pragma unroll
   for (int c = 0; c < 8; ++c) {
-    const double2* rec = C2 + off[c] * 4;
-    const double2 a = __ldg(rec), b = __ldg(rec + 1), cc = __ldg(rec + 2), d = __ldg(rec + 3);
-    prim[0] = fma(w[c], a.x, prim[0]);  prim[1] = fma(w[c], a.y, prim[1]);
-    prim[2] = fma(w[c], b.x, prim[2]);  prim[3] = fma(w[c], b.y, prim[3]);
-    prim[4] = fma(w[c], cc.x, prim[4]); prim[5] = fma(w[c], cc.y, prim[5]);
-    prim[6] = fma(w[c], d.x, prim[6]);  prim[7] = fma(w[c], d.y, prim[7]);
+    const double* rec = M.cells + off[c] * 8;
+    double v[8];
+    ld_global_nc_v4(rec, v[0], v[1], v[2], v[3]);
+    ld_global_nc_v4(rec + 4, v[4], v[5], v[6], v[7]);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) prim[q] = fma(w[c], v[q], prim[q]);
   }
   return prim[0] > 0.0 && prim[1] > 0.0;
 }
