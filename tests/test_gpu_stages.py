@@ -154,6 +154,23 @@ def test_geodesic_path(ipole, ref, kind, pix):
     assert np.allclose(dg, do, rtol=tol)
 
 
+@pytest.mark.parametrize("kind,eps", [("adaf", 0.04), ("grid", 0.04), ("adaf", 0.08), ("grid", 0.08), ("grid", 0.0025)])
+def test_geodesic_path_other_step_parameters(ipole, ref, kind, eps):
+    """The RK4 push has two forms (kernels.cuh rk4_push<SMALL>): stage points by short Taylor shifts from the start
+    point for eps <= 0.04 (the 4-eps probe pass runs at that edge), from scratch above.  Both against the oracle."""
+    cam = W.camera(kind, 32, eps=eps)
+    g = ipole.Ipole(**cam); r = ref.Ctx(**cam)
+    for pix in ((5, 7), (16, 16), (20, 14)):
+        Xg, Kg, dg, ntg, stg = g.trace_pixel(*pix)
+        X0, K0 = r.camera_ray(*pix)
+        Xo, Ko, do, nto, sto = r.trace(X0, K0)
+        assert len(dg) == len(do) and ntg == nto and stg == sto
+        tol = 1e-9 if nto >= 2 else 1e-11
+        assert np.abs(Xg[:, 1:] - Xo[:, 1:]).max() < tol
+        assert (np.abs(Kg - Ko) / np.abs(Ko).max(axis=1, keepdims=True)).max() < tol
+        assert np.allclose(dg, do, rtol=tol)
+
+
 def test_fp64_peak_microbenchmark(ipole):
     g = ipole.Ipole(**W.camera("adaf", 8))
     tf, ms = g.fp64_peak()
