@@ -553,7 +553,7 @@ __global__ void k_eval_stokes_step(int64_t n, const double* in, double* out) {
   const double* a = in + 16 * i;
   double S[4] = {a[8], a[9], a[10], a[11]};
   if (a[2] == 0.0 && a[5] == 0.0 && a[14] == 0.0)   // aU = rU = jU = 0: the specialised form the transfer kernel uses
-    stokes_step_qv(a[0], a[1], a[3], a[4], a[6], a[7], a[12], a[13], a[15], S);
+    stokes_step_qv<true>(a[0], a[1], a[3], a[4], a[6], a[7], a[12], a[13], a[15], S);
   else
     stokes_step(a, a + 4, a[7], a + 12, S);
   for (int k = 0; k < 4; ++k) out[4 * i + k] = S[k];

@@ -303,7 +303,7 @@ __device__ __forceinline__ void plasma_apply(const Units& U, const PlasmaFrame& 
     aI = ai[0]; rV = ri[2];
   } else {
     const Coeff c = synchrotron_invariant(F.ne, F.Th, F.B, F.cosT, F.nu);
-    stokes_step_qv(c.aI, c.aQ, c.aV, c.rQ, c.rV, ds, c.jI, c.jQ, c.jV, st.S);
+    stokes_step_qv<MODEL != MODEL_GRID>(c.aI, c.aQ, c.aV, c.rQ, c.rV, ds, c.jI, c.jQ, c.jV, st.S);
     aI = c.aI; rV = c.rV;
   }
   st.tau += aI * ds;
