@@ -36,7 +36,8 @@ struct ipole_ctx {
 
   int model = MODEL_NONE;
   void* d_model = nullptr;       // AdafParams / SlabParams / GridParams
-  double* d_grid = nullptr;      // 8 planes
+  unsigned int* d_occ = nullptr; // stencil occupancy bitmap of the grid
+  double* d_grid = nullptr;      // cell-major records
   size_t grid_cells = 0;
 
   uint64_t opt_path_bytes = 0;
@@ -511,6 +512,7 @@ int ipole_load_model_grid(ipole_ctx* c, const ipole_grid_desc* d, const double* 
   const size_t cells = (size_t)d->N1 * d->N2 * d->N3;
   if (cells != c->grid_cells) {
     cudaFree(c->d_grid); c->d_grid = nullptr; c->grid_cells = 0;
+    cudaFree(c->d_occ); c->d_occ = nullptr;
     cudaError_t e = cudaMalloc(&c->d_grid, 8 * cells * sizeof(double));
     if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
     c->grid_cells = cells;
@@ -532,6 +534,17 @@ int ipole_load_model_grid(ipole_ctx* c, const ipole_grid_desc* d, const double* 
     cudaFree(stage);
     if (e != cudaSuccess) { c->last_cuda = (int)e; return IPOLE_ECUDA; }
     m.cells = c->d_grid;
+  }
+  m.N1 = d->N1; m.N2 = d->N2; m.N3 = d->N3;
+  {  // stencil occupancy bitmap
+    const size_t bits = (size_t)(d->N1 + 1) * (d->N2 + 1) * d->N3, words = (bits + 31) / 32;
+    cudaFree(c->d_occ); c->d_occ = nullptr;
+    cudaError_t e = cudaMalloc(&c->d_occ, words * sizeof(unsigned int));
+    if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
+    CK(cudaMemsetAsync(c->d_occ, 0, words * sizeof(unsigned int), c->stream));
+    m.occ = c->d_occ;
+    k_build_occupancy<<<c->n_sm * 8, 256, 0, c->stream>>>(m, c->d_occ);
+    CK(cudaGetLastError());
   }
   m.N1 = d->N1; m.N2 = d->N2; m.N3 = d->N3;
   for (int i = 0; i < 3; ++i) { m.startx[i] = d->startx[i]; m.idx[i] = 1.0 / d->dx[i]; }
@@ -757,7 +770,7 @@ void ipole_free(ipole_ctx* c) {
   if (c->qstream) cudaStreamDestroy(c->qstream);
   if (c->ev_geo) cudaEventDestroy(c->ev_geo);
   if (c->ev_side) cudaEventDestroy(c->ev_side);
-  cudaFree(c->d_path_long); cudaFree(c->d_nsteps_long);
+  cudaFree(c->d_path_long); cudaFree(c->d_nsteps_long); cudaFree(c->d_occ);
   cudaFree(c->d_cam); cudaFree(c->d_model); cudaFree(c->d_grid); cudaFree(c->d_path);
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long);
   cudaFree(c->d_out); cudaFree(c->d_pixels); cudaFree(c->d_probe); cudaFree(c->d_queues); cudaFree(c->d_hist);

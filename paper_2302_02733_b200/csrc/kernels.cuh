@@ -570,6 +570,25 @@ __global__ void k_pack_field(size_t cells, int field, const double* __restrict__
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < cells; i += (size_t)gridDim.x * blockDim.x)
     out[i * 8 + field] = plane[i];
 }
+// stencil occupancy bitmap of the grid model: bit (ib, jb, k) covers the trilinear stencil whose base cell is
+// (ib-1, jb-1, k) before clamping, i.e. exactly the eight cells grid_gather reads there
+__global__ void k_build_occupancy(GridParams M, unsigned int* occ) {
+  const size_t total = (size_t)(M.N1 + 1) * (M.N2 + 1) * M.N3;
+  for (size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x; t < total; t += (size_t)gridDim.x * blockDim.x) {
+    const int k0 = (int)(t % M.N3);
+    const int jb = (int)((t / M.N3) % (M.N2 + 1)), ib = (int)(t / ((size_t)M.N3 * (M.N2 + 1)));
+    const int i0 = clampi(ib - 1, 0, M.N1 - 1), i1 = clampi(ib, 0, M.N1 - 1);
+    const int j0 = clampi(jb - 1, 0, M.N2 - 1), j1 = clampi(jb, 0, M.N2 - 1);
+    const int k1 = (k0 + 1 == M.N3) ? 0 : k0 + 1;
+    const int ii[2] = {i0, i1}, jj[2] = {j0, j1}, kk[2] = {k0, k1};
+    bool rho = false, u = false;
+    for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) for (int c = 0; c < 2; ++c) {
+      const double* rec = M.cells + (((size_t)ii[a] * M.N2 + jj[b]) * M.N3 + kk[c]) * 8;
+      rho |= rec[0] > 0.0; u |= rec[1] > 0.0;
+    }
+    if (rho && u) atomicOr(occ + (t >> 5), 1u << (t & 31));
+  }
+}
 __global__ void k_eval_math(int64_t n, const double* x, double* out) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
