@@ -535,7 +535,7 @@ int ipole_load_model_grid(ipole_ctx* c, const ipole_grid_desc* d, const double* 
     if (e != cudaSuccess) { c->last_cuda = (int)e; return IPOLE_ECUDA; }
     m.cells = c->d_grid;
   }
-  m.N1 = d->N1; m.N2 = d->N2; m.N3 = d->N3;
+  m.N1 = d->N1; m.N2 = d->N2; m.N3 = d->N3; m.iN3 = 1.0 / d->N3;
   {  // stencil occupancy bitmap
     const size_t bits = (size_t)(d->N1 + 1) * (d->N2 + 1) * d->N3, words = (bits + 31) / 32;
     cudaFree(c->d_occ); c->d_occ = nullptr;

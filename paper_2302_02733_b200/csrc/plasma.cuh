@@ -22,6 +22,7 @@ struct SlabParams { double H; int profile; double cpsi, spsi; double j[4], al[4]
 struct GridParams {
   int N1, N2, N3;
   double startx[3], idx[3];      // idx = 1/dx
+  double iN3;                    // 1/N3
   double gam, Rlow, Rhigh, r_out, lx_out;   // lx_out = ln r_out
   double ne_unit, B_unit;        // rho -> n_e [cm^-3], sqrt(b.b) -> Gauss
   const unsigned int* occ;       // device bitmap over stencil base cells (N1+1)(N2+1)N3: 1 = some corner has plasma
@@ -121,8 +122,12 @@ __device__ __forceinline__ bool grid_gather(const GridParams& M, const double X[
   const double di = fi - i0f, dj = fj - j0f, dk = fk - k0f;
   const int i0 = clampi((int)i0f, 0, M.N1 - 1), i1 = clampi((int)i0f + 1, 0, M.N1 - 1);
   const int j0 = clampi((int)j0f, 0, M.N2 - 1), j1 = clampi((int)j0f + 1, 0, M.N2 - 1);
-  long long kk = (long long)k0f % M.N3; if (kk < 0) kk += M.N3;
-  const int k0 = (int)kk, k1 = (k0 + 1 == M.N3) ? 0 : k0 + 1;
+  // k0f mod N3 in double arithmetic (a 64-bit integer remainder is ~100 emulated instructions); k0f is an exact
+  // integer, so the only possible slip is the quotient being one off, which the two wrap tests repair
+  int k0 = (int)(k0f - (double)M.N3 * floor(k0f * M.iN3));
+  if (k0 >= M.N3) k0 -= M.N3;
+  if (k0 < 0) k0 += M.N3;
+  const int k1 = (k0 + 1 == M.N3) ? 0 : k0 + 1;
   // one bit says whether any of the eight corners holds plasma (built at load time by k_build_occupancy with the
   // same index rules): most steps inside r_out cross none, and then cost one 4-byte load instead of 512 bytes
   {
