@@ -26,9 +26,9 @@ if ROOT not in sys.path:
 # FP64 operations per geodesic step of each kernel as shipped, counted by ncu (DFMA = 2, DADD/DMUL = 1;
 # smsp__sass_thread_inst_executed_op_d{fma,add,mul}_pred_on.sum / thread-steps of the launch): profiles/r1_k_*.txt,
 # DESIGN.md section 7.  The grid figure is the average over all steps of a ray, most of which cross no plasma.
-FLOP_PER_STEP = {"transfer_adaf": 1663.0, "transfer_grid": 470.0, "geodesic_adaf": 994.0, "geodesic_grid": 1169.0}
+FLOP_PER_STEP = {"transfer_adaf": 1663.0, "transfer_grid": 404.0, "geodesic_adaf": 994.0, "geodesic_grid": 1169.0}
 # DRAM bytes per step of k_transfer (dram__bytes_read + write of one launch / its thread-steps, same captures)
-DRAM_BYTES_PER_STEP = {"transfer_adaf": 64.2, "transfer_grid": 79.4}
+DRAM_BYTES_PER_STEP = {"transfer_adaf": 64.2, "transfer_grid": 69.6}
 # ALU roofline denominator: 148 SMs x 4 sub-partitions x 16 FP64 lanes x 2 flop x 1.965 GHz
 FP64_PEAK_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
 
