@@ -11,6 +11,7 @@
 #include "ref_stokes_op.hpp"
 #include "ref_plasma.hpp"
 #include "ref_transfer.hpp"
+#include "ref_pathfree.hpp"
 
 using namespace iref;
 
@@ -19,6 +20,7 @@ struct ipole_ref_ctx {
   Units units;
   Model model;
   std::atomic<int64_t> total_steps{0};
+  int path_free = 0;   // 1: PAPER.md:43 bidirectional variant (ref_pathfree.hpp)
 };
 
 static Geom mkgeom(double a, double h, int flat) { Geom G; G.a = a; G.hslope = h; G.flat = flat; return G; }
@@ -95,8 +97,15 @@ static void one_pixel(ipole_ref_ctx* x, int64_t pix, double out[6], int32_t* nst
   cplx N[4][4];
   for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) N[a][b] = 0.0;
   double tau = 0.0, tauF = 0.0, S[4];
-  transfer_along_path(C.geom, x->model, x->units, path, N, &tau, &tauF);
-  camera_stokes(C.geom, C, N, S);
+  if (x->path_free) {
+    const int n = (int)path.dl.size();
+    double Xend[4];
+    transfer_path_free(C, x->model, x->units, path.X[n].data(), path.K[n].data(), N, &tau, &tauF, Xend);
+    end_point_stokes(C, Xend, N, S);
+  } else {
+    transfer_along_path(C.geom, x->model, x->units, path, N, &tau, &tauF);
+    camera_stokes(C.geom, C, N, S);
+  }
   const double nu3 = x->units.nu_obs * x->units.nu_obs * x->units.nu_obs;
   for (int q = 0; q < 4; ++q) out[q] = S[q] * nu3;
   out[4] = tau; out[5] = tauF;
@@ -140,6 +149,31 @@ int ipole_ref_make_pixels(ipole_ref_ctx* x, int64_t n, const int64_t* pixels, in
 }
 
 void ipole_ref_free(ipole_ref_ctx* x) { delete x; }
+
+int ipole_ref_set_path_free(ipole_ref_ctx* x, int on) {
+  if (!x) return -1;
+  x->path_free = on ? 1 : 0;
+  return 0;
+}
+
+int ipole_ref_retrace(ipole_ref_ctx* x, const double Xn[4], const double Kn[4], int cap, double* X, double* K, double* dl) {
+  if (!x || !Xn || !Kn || cap < 0 || !X || !K || !dl) return -1;
+  Retrace r;
+  double Xend[4];
+  const int n = transfer_path_free(x->cam, x->model, x->units, Xn, Kn, nullptr, nullptr, nullptr, Xend, &r);
+  if (n > cap) return -n;
+  for (int s = 0; s <= n; ++s) for (int m = 0; m < 4; ++m) { X[4 * s + m] = r.X[s][m]; K[4 * s + m] = r.K[s][m]; }
+  for (int s = 0; s < n; ++s) dl[s] = r.dl[s];
+  return n;
+}
+
+int ipole_ref_observer_tetrad(ipole_ref_ctx* x, const double X[4], double e[16]) {
+  if (!x || !X || !e) return -1;
+  double t[4][4];
+  observer_tetrad(x->cam.geom, X, t);
+  for (int a = 0; a < 4; ++a) for (int m = 0; m < 4; ++m) e[4 * a + m] = t[a][m];
+  return 0;
+}
 
 int64_t ipole_ref_total_steps(ipole_ref_ctx* x) { return x ? x->total_steps.load() : 0; }
 

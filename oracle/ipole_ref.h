@@ -61,38 +61,17 @@ int  ipole_ref_make_pixels(ipole_ref_ctx*, int64_t n, const int64_t* pixels, int
                            double* I, double* Q, double* U, double* V, double* tau, double* tauF,
                            int32_t* nsteps, int32_t* nturn);
 void ipole_ref_free(ipole_ref_ctx*);
-
-/* ---- pieces, exposed so that each can be pinned on its own ---- */
-void ipole_ref_gcov(double a, double hslope, int flat, const double X[4], double g[16]);
-void ipole_ref_gcon(double a, double hslope, int flat, const double X[4], double g[16]);
-void ipole_ref_dgcov(double a, double hslope, int flat, const double X[4], double dg[64]); /* [k][m][n] */
-void ipole_ref_conn(double a, double hslope, int flat, const double X[4], double G[64]);   /* [l][m][n] */
-double ipole_ref_x2_of_theta(double hslope, double theta);
-double ipole_ref_theta_of_x2(double hslope, double x2);
-double ipole_ref_isco(double a);
-int  ipole_ref_camera_tetrad(ipole_ref_ctx*, double Xcam[4], double e[16]);   /* e[a][mu] */
-int  ipole_ref_camera_ray(ipole_ref_ctx*, int i, int j, double X[4], double K[4]);
-int  ipole_ref_camera_ray_ab(ipole_ref_ctx*, double alpha, double beta, double X[4], double K[4]);
-/* trace one ray; arrays sized cap+1 points / cap steps; returns number of steps n (points 0..n),
- * or -(needed) if cap is too small.  status: 1 horizon, 2 escaped, 3 max_steps. */
-int  ipole_ref_trace(ipole_ref_ctx*, const double X0[4], const double K0[4], int cap,
-                     double* X /*[cap+1][4]*/, double* K /*[cap+1][4]*/, double* dl /*[cap]*/,
-                     int32_t* nturn, int32_t* status);
-/* thermal synchrotron coefficients in cgs (not invariant): out = jI,jQ,jV,aI,aQ,aV,rQ,rV */
-void ipole_ref_coefficients(double ne, double thetae, double B, double cos_thetaB, double nu, double out[8]);
-void ipole_ref_bessel_kscaled(double z, double out[3]);  /* e^z K_0, e^z K_1, e^z K_2 */
-/* O(s) and P(s)=int_0^s O for constant coefficients; alpha=(aI,aQ,aU,aV), rho=(rQ,rU,rV) */
-void ipole_ref_stokes_operator(const double alpha[4], const double rho[3], double s, double O[16], double P[16]);
-/* plasma state of the loaded model at X: out = present, ne, thetae, B, u[4], b[4] (12 doubles) */
-int  ipole_ref_plasma(ipole_ref_ctx*, const double X[4], double out[12]);
-/* plasma tetrad at X for wavevector K, fluid velocity u and field b (all MKS contravariant):
- * econ[a][mu] = e_(a)^mu, ecov[a][mu] = e^(a)_mu; returns -4 if it cannot be built */
-int  ipole_ref_plasma_tetrad(ipole_ref_ctx*, const double X[4], const double K[4], const double u[4],
-                             const double b[4], double econ[16], double ecov[16]);
-/* parallel-transport a complex tensor given as 32 doubles (re,im interleaved, [mu][nu]) along a traced
- * path from point n to point 0 with no plasma (pin T1) */
-int  ipole_ref_transport_vacuum(ipole_ref_ctx*, int n, const double* X, const double* K, const double* dl, double N[32]);
-int64_t ipole_ref_total_steps(ipole_ref_ctx*);   /* steps taken by the last make_pixels call */
+/* Path-free bidirectional variant (reading R-10 in ref_pathfree.hpp): when on, make_pixels keeps only
+ * the end point of the backward pass and re-integrates forward to r >= r_cam, one transfer step per forward step;
+ * Stokes are read in the observer tetrad at the forward end point.  nsteps/nturn stay those of the backward pass.
+ * Pins PF1-PF5 (tests/test_oracle_pathfree.py). */
+int  ipole_ref_set_path_free(ipole_ref_ctx*, int on);
+/* The forward pass alone, from (Xn, Kn): returns its step count n, points 0..n (0 = far end) and the n step sizes;
+ * -(needed) if cap is too small. */
+int  ipole_ref_retrace(ipole_ref_ctx*, const double Xn[4], const double Kn[4], int cap,
+                       double* X /*[cap+1][4]*/, double* K /*[cap+1][4]*/, double* dl /*[cap]*/);
+/* camera-type tetrad e[a][mu] at an arbitrary point (static observer, e3 from d_X1, e2 from -d_X2, e1 from d_X3) */
+int  ipole_ref_observer_tetrad(ipole_ref_ctx*, const double X[4], double e[16]);
 
 #ifdef __cplusplus
 }

@@ -76,6 +76,9 @@ def lib():
         L.ipole_ref_plasma.argtypes = [C.c_void_p, dp, dp]
         L.ipole_ref_plasma_tetrad.argtypes = [C.c_void_p, dp, dp, dp, dp, dp, dp]
         L.ipole_ref_transport_vacuum.argtypes = [C.c_void_p, C.c_int, dp, dp, dp, dp]
+        L.ipole_ref_set_path_free.argtypes = [C.c_void_p, C.c_int]
+        L.ipole_ref_retrace.argtypes = [C.c_void_p, dp, dp, C.c_int, dp, dp, dp]
+        L.ipole_ref_observer_tetrad.argtypes = [C.c_void_p, dp, dp]
         L.ipole_ref_total_steps.argtypes = [C.c_void_p]
         L.ipole_ref_total_steps.restype = C.c_int64
         _LIB = L
@@ -217,6 +220,25 @@ class Ctx:
         if n < 0:
             raise RuntimeError("trace: cap too small, need %d" % -n)
         return X[:n + 1].copy(), K[:n + 1].copy(), dl[:n].copy(), nt.value, st.value
+
+    def set_path_free(self, on=True):
+        """PAPER.md:43 bidirectional variant: make_pixels re-integrates the geodesic forward instead of using a stored path."""
+        rc = lib().ipole_ref_set_path_free(self._h, 1 if on else 0)
+        if rc != 0:
+            raise RuntimeError("set_path_free failed: %d" % rc)
+
+    def retrace(self, Xn, Kn, cap=60000):
+        """Forward pass of the path-free variant from the far end (Xn, Kn): points 0..n (0 = far end), n step sizes."""
+        X = np.zeros((cap + 1, 4)); K = np.zeros((cap + 1, 4)); dl = np.zeros(cap)
+        n = lib().ipole_ref_retrace(self._h, _dp(_vec(Xn)), _dp(_vec(Kn)), cap, _dp(X), _dp(K), _dp(dl))
+        if n < 0:
+            raise RuntimeError("retrace failed: %d" % n)
+        return X[:n + 1].copy(), K[:n + 1].copy(), dl[:n].copy()
+
+    def observer_tetrad(self, X):
+        e = np.zeros((4, 4))
+        lib().ipole_ref_observer_tetrad(self._h, _dp(_vec(X)), _dp(e))
+        return e
 
     def plasma(self, X):
         out = np.zeros(12)
