@@ -29,6 +29,9 @@ if ROOT not in sys.path:
 FLOP_PER_STEP = {"transfer_adaf": 1663.0, "transfer_grid": 404.0, "geodesic_adaf": 994.0, "geodesic_grid": 1169.0}
 # DRAM bytes per step of k_transfer (dram__bytes_read + write of one launch / its thread-steps, same captures)
 DRAM_BYTES_PER_STEP = {"transfer_adaf": 64.2, "transfer_grid": 69.6}
+# --path-free (PAPER.md:43 variant): per FORWARD step of k_transfer<model, 1> (RK4 push + transfer step in one kernel)
+FLOP_PER_STEP_PF = {"transfer_adaf": 2657.0, "transfer_grid": 1573.0}
+DRAM_BYTES_PER_STEP_PF = {"transfer_adaf": 0.1, "transfer_grid": 6.0}
 # ALU roofline denominator: 148 SMs x 4 sub-partitions x 16 FP64 lanes x 2 flop x 1.965 GHz
 FP64_PEAK_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
 
@@ -91,7 +94,7 @@ class ClockSampler:
                 "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_sample(workload, n_rays, nthreads):
+def oracle_sample(workload, n_rays, nthreads, path_free=False):
     """The CPU oracle, as it stands, on a strided sample of the workload's image.  Returns (rays, steps, seconds)."""
     import numpy as np
     from oracle import ipole_ref
@@ -104,6 +107,8 @@ def oracle_sample(workload, n_rays, nthreads):
     else:
         desc, fields = W.fm_torus_grid(*wl["grid"])
         r.load_grid(desc, fields)
+    if path_free:
+        r.set_path_free(True)
     n = wl["n"]
     stride = max(1, int(round(n / max(1.0, n_rays ** 0.5))))
     ii, jj = np.meshgrid(np.arange(stride // 2, n, stride), np.arange(stride // 2, n, stride))
@@ -156,6 +161,8 @@ def main():
     ap.add_argument("--cpu-baseline-rays", type=int, default=16384)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--path-free", action="store_true",
+                    help="the paper's own GPU design (PAPER.md:43): no stored path, forward re-integration")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -182,6 +189,8 @@ def main():
     cam = W.camera(wl["kind"], wl["n"])
     g = ipole.Ipole(**cam)
     g.set_stream(torch.cuda.current_stream())
+    if args.path_free:
+        g.set_path_free(True)
     grid_bytes = 0
     if wl["kind"] == "adaf":
         g.load_adaf(**W.ADAF)
@@ -253,36 +262,44 @@ def main():
 
     # ---- roofline of the dominant kernel (k_transfer), live CUDA-event time of the last timed image ----
     key = "transfer_" + wl["kind"]
+    pf = args.path_free
+    fl_rt = FLOP_PER_STEP_PF[key] if pf else FLOP_PER_STEP[key]
+    rt_steps = st["total_steps_forward"] if pf else st["total_steps"]   # steps the transfer kernel walks
+    dram_rt = DRAM_BYTES_PER_STEP_PF[key] if pf else DRAM_BYTES_PER_STEP[key]
     dfma_tf, _ = g.fp64_peak()
     n_rt = max(1, st["n_batches"])          # bulk launches; the long-ray passes run beside them on a side stream
     rt_ms = st["ms_transfer"]
-    roof = {"bound": "alu", "kernel": "k_transfer<%s>" % wl["kind"], "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+    roof = {"bound": "alu", "kernel": "k_transfer<%s%s>" % (wl["kind"], ", path-free" if pf else ""), "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
             "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz; DFMA micro-benchmark on this GPU: %.1f" % dfma_tf,
             "launches": n_rt, "avg_launch_ms": rt_ms / n_rt, "kernel_share_of_step": rt_ms / st["ms_total"],
-            "steps_per_launch": st["total_steps"] / n_rt,
-            "traffic": DRAM_BYTES_PER_STEP[key] * st["total_steps"] / n_rt,
+            "steps_per_launch": rt_steps / n_rt,
+            "traffic": dram_rt * rt_steps / n_rt,
             "traffic_note": "ncu dram__bytes_read+write per launch (profiles/r1_k_transfer_*.txt), scaled by steps; "
-                            "algorithmic: 64 B per step (one path record read)"}
-    ach = FLOP_PER_STEP[key] * st["total_steps"] / (rt_ms * 1e-3) / 1e12
-    roof.update(achieved=ach, frac=ach / FP64_PEAK_TFLOPS, flop_per_step=FLOP_PER_STEP[key])
+                            + ("algorithmic: 64 B read and 32-48 B written per RAY, nothing per step" if pf else
+                               "algorithmic: 64 B per step (one path record read)")}
+    ach = fl_rt * rt_steps / (rt_ms * 1e-3) / 1e12
+    roof.update(achieved=ach, frac=ach / FP64_PEAK_TFLOPS, flop_per_step=fl_rt)
     # the whole step against the same roofline: every FP64 operation of both hot kernels over the image time
-    fl_step = (FLOP_PER_STEP[key] + FLOP_PER_STEP["geodesic_" + wl["kind"]]) * st["total_steps"]
+    fl_step = fl_rt * rt_steps + FLOP_PER_STEP["geodesic_" + wl["kind"]] * st["total_steps"]
     roof["whole_step"] = {"achieved": fl_step / (st["ms_total"] * 1e-3) / 1e12,
                           "frac": fl_step / (st["ms_total"] * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
                           "geodesic_tflops": FLOP_PER_STEP["geodesic_" + wl["kind"]] * st["total_steps"]
                                              / (st["ms_geodesic"] * 1e-3) / 1e12}
-    roof["hbm_path_gbs"] = 128.0 * st["total_steps"] / ((st["ms_geodesic"] + st["ms_transfer"]) * 1e-3) / 1e9
+    roof["hbm_path_gbs"] = (0.0 if pf else 128.0) * st["total_steps"] / ((st["ms_geodesic"] + st["ms_transfer"]) * 1e-3) / 1e9
 
     line = {"metric": "rays_per_s", "value": value, "unit": "rays/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.workload, "configs_index": wl["config"], "image": "%dx%d" % (wl["n"], wl["n"]),
                        "model": wl["kind"], "freq_ghz": 230, "eps": cam["eps"], "full_stokes": True, "maps": maps,
-                       "l2": "no flush needed: every batch streams a %.1f GB path buffer (>> 126 MB L2)"
+                       "variant": "path-free bidirectional (PAPER.md:43)" if pf else "stored path",
+                       "l2": ("no flush needed: nothing is re-read; per image %.2f GB of end points and outputs stream once"
+                              % (rays * (64.0 + 8.0 * len(names)) / 1e9)) if pf else
+                             "no flush needed: every batch streams a %.1f GB path buffer (>> 126 MB L2)"
                              % (st["path_cap"] * 64.0 * min(rays, max(1, rays // max(1, st["n_batches"]))) / 1e9),
                        "parallelism": "rays sharded: one replica per GPU" if world > 1 else "single GPU"},
             "images_per_s": value / rays, "steps_per_s": world * st["total_steps"] * args.steps / (ms * 1e-3),
-            "mean_steps_per_ray": st["total_steps"] / rays,
+            "mean_steps_per_ray": st["total_steps"] / rays, "forward_steps": st["total_steps_forward"],
             "stage_ms": {"probe_sort": st["ms_probe"], "geodesic": st["ms_geodesic"], "transfer": st["ms_transfer"],
                          "long_rays_side_stream": st["ms_long"], "total": st["ms_total"], "batches": st["n_batches"], "path_cap": st["path_cap"],
                          "long_rays": st["n_long"]},
@@ -293,7 +310,7 @@ def main():
 
     if not args.no_cpu_baseline and world == 1:
         cores = os.cpu_count() or 1
-        n, steps, dt, stride = oracle_sample(args.workload, args.cpu_baseline_rays, cores)
+        n, steps, dt, stride = oracle_sample(args.workload, args.cpu_baseline_rays, cores, path_free=pf)
         line["cpu_baseline"] = {"value": n / dt, "unit": "rays/s", "cores": cores, "kind": "oracle",
                                 "sample": "%d rays: every %d-th pixel in x and y of the %dx%d image, %.1f s"
                                           % (n, stride, wl["n"], wl["n"], dt),

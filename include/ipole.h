@@ -98,6 +98,7 @@ typedef struct {
                               ipole_get_stats synchronises them)                                       */
   float   ms_long;         /* long-ray passes (geodesic + transfer) on the side stream; they overlap the
                               bulk batches, so this is not part of a sum that gives ms_total            */
+  int64_t total_steps_forward; /* path-free variant: steps of the forward passes of all rays (else 0)     */
 } ipole_stats;
 
 /* Create a context. Computes the camera tetrad on the device. IPOLE_EINVAL on bad parameters. */
@@ -110,6 +111,17 @@ int  ipole_set_stream(ipole_ctx*, void* cuda_stream);
  * 64 GiB); sort_rays: 0 = pixel order, 1 = order rays by predicted step count, longest first, when the image
  * has >= 32768 rays (default), 2 = always run the probe pass and sort (tests). */
 int  ipole_set_options(ipole_ctx*, uint64_t path_bytes, int32_t sort_rays);
+/* Path-free bidirectional variant, the paper's own GPU design (section 2.2: "The GPU code does this
+ * integration in both directions, away from the observer ... and toward the observer ..., without saving the path in
+ * both cases"; reading R-10 in DESIGN.md).  on != 0: ipole_make_image / ipole_make_pixels keep only
+ * the end point of each backward pass (64 B per ray), then re-integrate every ray forward with one RK4 push per
+ * step (step rule evaluated at the point the step starts from), each push followed by the transfer step over its
+ * two end points, until r >= r_cam moving outward; Stokes are read in the observer tetrad built at that end point.
+ * No path buffer is allocated and the whole image is one geodesic launch and one transfer launch.  nsteps / nturn
+ * remain those of the backward pass; ipole_stats.total_steps_forward counts the forward steps.  The image differs
+ * from the stored-path one at the level the integrator is not time-reversible (paper: "negligible").
+ * on == 0 (default): stored path.  Returns IPOLE_EINVAL for a NULL context. */
+int  ipole_set_path_free(ipole_ctx*, int32_t on);
 
 int  ipole_load_model_adaf(ipole_ctx*, const ipole_adaf_params*);
 int  ipole_load_model_slab(ipole_ctx*, const ipole_slab_params*);

@@ -42,6 +42,10 @@ struct ipole_ctx {
 
   uint64_t opt_path_bytes = 0;
   int opt_sort = 1;
+  int opt_path_free = 0;         // PAPER.md:43 bidirectional variant
+  int last_pf = 0;               // the last image was made path-free
+  double* d_endp = nullptr; int64_t endp_cap = 0;   // end points of the backward passes, [rays][8]
+  long long* d_sum = nullptr;    // forward-step total of the path-free variant
 
   double* d_path = nullptr; size_t path_bytes = 0;
   double* d_path_long = nullptr; size_t path_long_bytes = 0;   // slots of max_steps for the long-ray passes
@@ -64,7 +68,7 @@ struct ipole_ctx {
   bool have_image = false;
   int64_t last_n = 0;
   ipole_stats stats;
-  int occ_geo = 0, occ_rt[4] = {0, 0, 0, 0};
+  int occ_geo = 0, occ_rt[4] = {0, 0, 0, 0}, occ_pf[4][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
 };
 
 namespace {
@@ -199,12 +203,20 @@ int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays, cudaStream
   return IPOLE_OK;
 }
 
-int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_t st, int reserve = 0) {
+template <int PF>
+void launch_transfer_model(int model, int g, cudaStream_t st, const RtArgs& a) {
+  if (model == MODEL_ADAF) k_transfer<MODEL_ADAF, PF><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
+  else if (model == MODEL_SLAB) k_transfer<MODEL_SLAB, PF><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
+  else k_transfer<MODEL_GRID, PF><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
+}
+
+// pf: 0 stored path, 1 path-free with eps <= 0.04, 2 path-free with any eps
+int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_t st, int reserve = 0, int pf = 0) {
   const int s = span_begin(c, kind, st);
-  const int g = grid_for(c, c->occ_rt[c->model], IPOLE_RT_THREADS, rays, reserve);
-  if (c->model == MODEL_ADAF) k_transfer<MODEL_ADAF><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
-  else if (c->model == MODEL_SLAB) k_transfer<MODEL_SLAB><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
-  else k_transfer<MODEL_GRID><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
+  const int g = grid_for(c, pf ? c->occ_pf[c->model][pf] : c->occ_rt[c->model], IPOLE_RT_THREADS, rays, reserve);
+  if (pf == 0) launch_transfer_model<0>(c->model, g, st, a);
+  else if (pf == 1) launch_transfer_model<1>(c->model, g, st, a);
+  else launch_transfer_model<2>(c->model, g, st, a);
   span_end(c, s, st);
   c->stats.n_launches++;
   CK(cudaGetLastError());
@@ -221,6 +233,25 @@ GeoArgs geo_args(ipole_ctx* c) {
   return g;
 }
 
+// a-9 and the bookkeeping that closes an image
+int finish_image(ipole_ctx* c, int64_t n, double* I, double* Q, double* U, double* V, int total) {
+  {
+    const int s = span_begin(c, LK_OTHER, c->stream);
+    const int nb = (int)std::min<int64_t>(REDUCE_BLOCKS, (n + 255) / 256);
+    k_reduce_partial<<<nb, 256, 0, c->stream>>>(n, I, Q, U, V, c->d_nsteps, c->d_nturn, c->d_part);
+    const double pix_rad = c->cam.pix * c->units.L_unit / c->units.D_cm;
+    k_reduce_final<<<1, 32, 0, c->stream>>>(c->d_part, nb, pix_rad * pix_rad * 1e23, c->d_red);
+    c->stats.n_launches += 2;
+    span_end(c, s, c->stream);
+    CK(cudaGetLastError());
+  }
+  span_end(c, total, c->stream);
+  c->have_image = true;
+  c->last_n = n;
+  return IPOLE_OK;
+}
+
+
 // the whole pipeline for n rays; outputs are DEVICE pointers indexed by ray
 int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double* Q, double* U, double* V, double* tau,
              double* tauF) {
@@ -229,6 +260,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   c->spans_used = 0;
   std::memset(&c->stats, 0, sizeof c->stats);
   c->have_image = false;
+  c->last_pf = 0;
   CK(cudaMemsetAsync(c->d_queues, 0, N_QUEUES * sizeof(unsigned long long), c->stream));
   CK(cudaMemsetAsync(c->d_small, 0, 4 * sizeof(int), c->stream));
   int qi = 0;
@@ -294,6 +326,37 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     // everything in flight at once: give each ray what the budget allows
     const int64_t per = (int64_t)(budget / rec_bytes / (size_t)n) - 1;
     cap = (int)std::max<int64_t>(64, std::min<int64_t>(max_steps, per));
+  }
+  if (c->opt_path_free) {
+    // ---- path-free bidirectional variant: one geodesic launch that keeps the end points, one
+    // transfer launch that re-integrates forward.  Rays are ordered longest first, so the few very long rays start
+    // at once and run beside the bulk. ----
+    if (n > c->endp_cap) {
+      cudaFree(c->d_endp); c->d_endp = nullptr; c->endp_cap = 0;
+      cudaError_t e = cudaMalloc(&c->d_endp, (size_t)n * rec_bytes);
+      if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
+      c->endp_cap = n;
+    }
+    GeoArgs g = geo_args(c);
+    g.cap = 0; g.base = 0; g.count = n; g.order = order; g.pixels = d_pixels;
+    g.path = nullptr; g.nsteps = c->d_nsteps; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
+    g.endp = c->d_endp;
+    if ((rc = launch_geodesic(c, g, LK_GEO, n, c->stream)) != IPOLE_OK) return rc;
+    RtArgs t;
+    std::memset(&t, 0, sizeof t);
+    t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.base = 0; t.count = n; t.order = order;
+    t.nsteps = c->d_nsteps; t.queue = c->d_queues + (qi++);
+    t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
+    t.endp = c->d_endp; t.nfwd = c->d_nsteps_long; t.eps = c->cam.eps; t.max_steps = max_steps;
+    if ((rc = launch_transfer(c, t, LK_RT, n, c->stream, 0, c->cam.eps <= 0.04 ? 1 : 2)) != IPOLE_OK) return rc;
+    c->stats.n_batches = 1;
+    c->stats.path_cap = 0;
+    c->last_pf = 1;
+    CK(cudaMemsetAsync(c->d_sum, 0, sizeof(long long), c->stream));
+    k_sum_i32<<<(int)std::min<int64_t>((n + 255) / 256, 592), 256, 0, c->stream>>>(c->d_nsteps_long, n, c->d_sum);
+    c->stats.n_launches++;
+    CK(cudaGetLastError());
+    return finish_image(c, n, I, Q, U, V, total);
   }
   c->stats.path_cap = cap;
 
@@ -383,21 +446,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     CK(cudaGetLastError());
   }
 
-  // ---- a-9: totals ----
-  {
-    const int s = span_begin(c, LK_OTHER, c->stream);
-    const int nb = (int)std::min<int64_t>(REDUCE_BLOCKS, (n + 255) / 256);
-    k_reduce_partial<<<nb, 256, 0, c->stream>>>(n, I, Q, U, V, c->d_nsteps, c->d_nturn, c->d_part);
-    const double pix_rad = c->cam.pix * c->units.L_unit / c->units.D_cm;
-    k_reduce_final<<<1, 32, 0, c->stream>>>(c->d_part, nb, pix_rad * pix_rad * 1e23, c->d_red);
-    c->stats.n_launches += 2;
-    span_end(c, s, c->stream);
-    CK(cudaGetLastError());
-  }
-  span_end(c, total, c->stream);
-  c->have_image = true;
-  c->last_n = n;
-  return IPOLE_OK;
+  return finish_image(c, n, I, Q, U, V, total);
 }
 
 }  // namespace
@@ -435,10 +484,17 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
     if (cudaEventCreateWithFlags(&c->ev_side, cudaEventDisableTiming) != cudaSuccess) return fail(IPOLE_ECUDA);
   }
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo, k_geodesic, IPOLE_GEO_THREADS, 0);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_rt[MODEL_ADAF], k_transfer<MODEL_ADAF>, IPOLE_RT_THREADS, 0);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_rt[MODEL_SLAB], k_transfer<MODEL_SLAB>, IPOLE_RT_THREADS, 0);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_rt[MODEL_GRID], k_transfer<MODEL_GRID>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_rt[MODEL_ADAF], k_transfer<MODEL_ADAF, 0>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_rt[MODEL_SLAB], k_transfer<MODEL_SLAB, 0>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_rt[MODEL_GRID], k_transfer<MODEL_GRID, 0>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_pf[MODEL_ADAF][1], k_transfer<MODEL_ADAF, 1>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_pf[MODEL_SLAB][1], k_transfer<MODEL_SLAB, 1>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_pf[MODEL_GRID][1], k_transfer<MODEL_GRID, 1>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_pf[MODEL_ADAF][2], k_transfer<MODEL_ADAF, 2>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_pf[MODEL_SLAB][2], k_transfer<MODEL_SLAB, 2>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_pf[MODEL_GRID][2], k_transfer<MODEL_GRID, 2>, IPOLE_RT_THREADS, 0);
   if (cudaGetLastError() != cudaSuccess) return fail(IPOLE_ECUDA);
+  if (cudaMalloc(&c->d_sum, sizeof(long long)) != cudaSuccess) return fail(IPOLE_ENOMEM);
   rc = apply_camera(c, cam);
   if (rc != IPOLE_OK) return fail(rc);
   *out = c;
@@ -474,6 +530,12 @@ int ipole_set_options(ipole_ctx* c, uint64_t path_bytes, int32_t sort_rays) {
   if (!c) return IPOLE_EINVAL;
   c->opt_path_bytes = path_bytes;
   c->opt_sort = (sort_rays == 2) ? 2 : (sort_rays ? 1 : 0);
+  return IPOLE_OK;
+}
+
+int ipole_set_path_free(ipole_ctx* c, int32_t on) {
+  if (!c) return IPOLE_EINVAL;
+  c->opt_path_free = on ? 1 : 0;
   return IPOLE_OK;
 }
 
@@ -628,6 +690,12 @@ int ipole_get_stats(ipole_ctx* c, ipole_stats* out) {
   for (int k = 0; k < 4; ++k) s.flux_jy[k] = r.flux[k];
   s.lp = r.lp; s.cp = r.cp;
   s.total_steps = r.total_steps; s.max_steps_seen = r.max_steps; s.n_ring = r.n_ring; s.n_maxstep = r.n_maxstep;
+  s.total_steps_forward = 0;
+  if (c->last_pf) {
+    long long f = 0;
+    CK(cudaMemcpy(&f, c->d_sum, sizeof f, cudaMemcpyDeviceToHost));
+    s.total_steps_forward = f;
+  }
   s.ms_probe = s.ms_geodesic = s.ms_transfer = s.ms_total = s.ms_long = 0.f;
   for (size_t i = 0; i < c->spans_used; ++i) {
     float ms = 0.f;
@@ -774,7 +842,7 @@ void ipole_free(ipole_ctx* c) {
   cudaFree(c->d_cam); cudaFree(c->d_model); cudaFree(c->d_grid); cudaFree(c->d_path);
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long);
   cudaFree(c->d_out); cudaFree(c->d_pixels); cudaFree(c->d_probe); cudaFree(c->d_queues); cudaFree(c->d_hist);
-  cudaFree(c->d_small); cudaFree(c->d_part); cudaFree(c->d_red);
+  cudaFree(c->d_small); cudaFree(c->d_part); cudaFree(c->d_red); cudaFree(c->d_endp); cudaFree(c->d_sum);
   for (auto& s : c->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
   cudaGetLastError();
   delete c;

@@ -40,7 +40,32 @@ __device__ __forceinline__ void gram_schmidt(const Sym7& g, double v[4], const d
   for (int m = 0; m < 4; ++m) v[m] /= n;
 }
 
-// a-1: camera at (r_cam, theta_cam, phi=0); e0 || d_t, e3 from d_X1, e2 from -d_X2, e1 from d_X3 (R-3)
+// camera-type tetrad at X: e0 || d_t, e3 from d_X1, e2 from -d_X2, e1 from d_X3 (R-3), and the covariant
+// components of the two transverse legs
+__device__ __forceinline__ void observer_tetrad(const Geom& G, const double X[4], double e[4][4], double ecov1[4], double ecov2[4]) {
+  Point p; Sym7 g; Inv6 gi;
+  metric<false>(G, X, p, g, gi);
+  double basis[3][4], sg[3];
+  double e0[4] = {1.0, 0.0, 0.0, 0.0};
+  const double n0 = sqrt(-dotg(g, e0, e0));
+  for (int m = 0; m < 4; ++m) { e[0][m] = e0[m] / n0; basis[0][m] = e[0][m]; }
+  sg[0] = -1.0;
+  double e3[4] = {0.0, 1.0, 0.0, 0.0};
+  gram_schmidt(g, e3, basis, sg, 1);
+  for (int m = 0; m < 4; ++m) { e[3][m] = e3[m]; basis[1][m] = e3[m]; }
+  sg[1] = 1.0;
+  double e2[4] = {0.0, 0.0, -1.0, 0.0};
+  gram_schmidt(g, e2, basis, sg, 2);
+  for (int m = 0; m < 4; ++m) { e[2][m] = e2[m]; basis[2][m] = e2[m]; }
+  sg[2] = 1.0;
+  double e1[4] = {0.0, 0.0, 0.0, 1.0};
+  gram_schmidt(g, e1, basis, sg, 3);
+  for (int m = 0; m < 4; ++m) e[1][m] = e1[m];
+  g.mul(e[1], ecov1);
+  g.mul(e[2], ecov2);
+}
+
+// a-1: camera at (r_cam, theta_cam, phi=0)
 __global__ void k_camera_setup(CamDev* cam, CameraSetupArgs a) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   CamDev C = *cam;
@@ -56,26 +81,7 @@ __global__ void k_camera_setup(CamDev* cam, CameraSetupArgs a) {
     }
   }
   C.Xcam[0] = 0.0; C.Xcam[1] = log(C.r_cam); C.Xcam[2] = x2; C.Xcam[3] = 0.0;
-  Point p; Sym7 g; Inv6 gi;
-  metric<false>(C.G, C.Xcam, p, g, gi);
-  double basis[3][4], sg[3];
-  double e0[4] = {1.0, 0.0, 0.0, 0.0};
-  const double n0 = sqrt(-dotg(g, e0, e0));
-  for (int m = 0; m < 4; ++m) { C.e[0][m] = e0[m] / n0; basis[0][m] = C.e[0][m]; }
-  sg[0] = -1.0;
-  double e3[4] = {0.0, 1.0, 0.0, 0.0};
-  gram_schmidt(g, e3, basis, sg, 1);
-  for (int m = 0; m < 4; ++m) { C.e[3][m] = e3[m]; basis[1][m] = e3[m]; }
-  sg[1] = 1.0;
-  double e2[4] = {0.0, 0.0, -1.0, 0.0};
-  gram_schmidt(g, e2, basis, sg, 2);
-  for (int m = 0; m < 4; ++m) { C.e[2][m] = e2[m]; basis[2][m] = e2[m]; }
-  sg[2] = 1.0;
-  double e1[4] = {0.0, 0.0, 0.0, 1.0};
-  gram_schmidt(g, e1, basis, sg, 3);
-  for (int m = 0; m < 4; ++m) C.e[1][m] = e1[m];
-  g.mul(C.e[1], C.ecov1);
-  g.mul(C.e[2], C.ecov2);
+  observer_tetrad(C.G, C.Xcam, C.e, C.ecov1, C.ecov2);
   C.lx_in = log(a.r_in);
   C.lx_esc = log(a.r_esc);
   *cam = C;
@@ -98,6 +104,8 @@ struct GeoArgs {
   int32_t* nturn;             // [total rays]
   unsigned long long* queue;  // atomic ray counter of this launch
   int32_t* long_list; int* long_count;  // rays that did not fit (nullable)
+  double* endp;               // [total rays][8], indexed by q: last point (X1..3, K0..3, 0) of the ray (nullable);
+                              // all the path-free variant keeps of the backward pass
 };
 
 __device__ __forceinline__ void pixel_ray(const CamDev& C, int64_t pix, double X[4], double K[4]) {
@@ -241,6 +249,7 @@ __global__ void __launch_bounds__(IPOLE_GEO_THREADS, IPOLE_GEO_MINB) k_geodesic(
         if (A.long_list) { const int w = atomicAdd(A.long_count, 1); A.long_list[w] = q; }
       } else {
         if (rec) store_record(rec + (size_t)n * REC_DOUBLES, X, K, 0.0);
+        if (A.endp) store_record(A.endp + (size_t)q * REC_DOUBLES, X, K, 0.0);
         A.nsteps[q] = n;
         if (A.nturn) A.nturn[q] = (nt > 127 ? 127 : nt) | (status == 3 ? 0x80 : 0);
       }
@@ -262,6 +271,10 @@ struct RtArgs {
   const int32_t* nsteps;
   unsigned long long* queue;
   double *I, *Q, *U, *V, *tau, *tauF;   // indexed by q
+  // path-free variant (PF != 0): no path; the ray restarts from the end point of its backward pass
+  const double* endp;         // [total rays][8], indexed by q
+  int32_t* nfwd;              // [total rays] steps of the forward pass (nullable)
+  double eps; int max_steps;
 };
 
 #ifndef IPOLE_RT_THREADS
@@ -284,7 +297,14 @@ struct RtArgs {
 // f <- P f, plasma operator, f <- P f  (Strang splitting, R-6).
 // Resident blocks per SM: 3 (168 registers, a few spilled doubles) for the analytic models, which ncu shows limited
 // by dependent-issue latency; 2 (255 registers) for the grid model, whose 64 gathered values per step want registers.
-template <int MODEL>
+//
+// PF = 0: the stored path is walked from its far end to the camera.
+// PF = 1, 2: path-free bidirectional variant (R-10; 1: eps <= 0.04, RK4 stage points by Taylor
+// shifts, 2: any eps).  The ray restarts at the end point of its backward pass and is re-integrated forward, one RK4
+// push of +dl per step (dl = the step rule at the point the step starts from), each push followed by the same
+// transfer step over its two end points; it stops at r >= r_cam moving outward (or r <= r_in moving inward, or after
+// max_steps steps), and the tensor is read in the observer tetrad built at that end point.
+template <int MODEL, int PF>
 __global__ void __launch_bounds__(IPOLE_RT_THREADS, (MODEL == MODEL_GRID) ? IPOLE_RT_MINB : IPOLE_RT_MINB_ANALYTIC)
 k_transfer(const __grid_constant__ RtArgs A) {
   const CamDev& C = A.cam;
@@ -311,12 +331,17 @@ k_transfer(const __grid_constant__ RtArgs A) {
       have = li < count;
       if (!have) return;
       q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
-      const int n = A.nsteps[q];
-      if (n < 0) continue;  // overflowed its slot: done by the long-ray pass
-      rec = A.path + (size_t)li * slot_doubles;
       double dl;
-      load_record(rec + (size_t)n * REC_DOUBLES, Xhi, Khi, dl);
-      s = n - 1;
+      if (PF) {
+        load_record(A.endp + (size_t)q * REC_DOUBLES, Xhi, Khi, dl);
+        s = 0;   // forward steps taken
+      } else {
+        const int n = A.nsteps[q];
+        if (n < 0) continue;  // overflowed its slot: done by the long-ray pass
+        rec = A.path + (size_t)li * slot_doubles;
+        load_record(rec + (size_t)n * REC_DOUBLES, Xhi, Khi, dl);
+        s = n - 1;
+      }
 #pragma unroll
       for (int m = 0; m < 4; ++m) { st.f1[m] = 0.0; st.f2[m] = 0.0; st.S[m] = 0.0; }
       st.tau = 0.0; st.tauF = 0.0;
@@ -325,6 +350,7 @@ k_transfer(const __grid_constant__ RtArgs A) {
     }
   };
 
+  const double ieps = PF ? 1.0 / A.eps : 0.0;
   fetch();
 #if IPOLE_RT_SYNC
   // one barrier per step keeps the warps of a block within one iteration of each other, so that they share the
@@ -335,10 +361,17 @@ k_transfer(const __grid_constant__ RtArgs A) {
   while (have) {
 #endif
     double Xlo[4], Klo[4], dl;
-    load_record(rec + (size_t)s * REC_DOUBLES, Xlo, Klo, dl);
+    if (PF) {
+      dl = stepsize(Xhi, Khi, ieps);
+#pragma unroll
+      for (int m = 0; m < 4; ++m) { Xlo[m] = Xhi[m]; Klo[m] = Khi[m]; }
+      rk4_push<PF == 1>(C.G, Xlo, Klo, dl);
+    } else {
+      load_record(rec + (size_t)s * REC_DOUBLES, Xlo, Klo, dl);
 #if IPOLE_RT_PREFETCH
-    if (s > 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(rec + (size_t)(s - 1) * REC_DOUBLES));
+      if (s > 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(rec + (size_t)(s - 1) * REC_DOUBLES));
 #endif
+    }
     double Xm[4], Km[4];
 #pragma unroll
     for (int m = 0; m < 4; ++m) { Xm[m] = 0.5 * (Xlo[m] + Xhi[m]); Km[m] = 0.5 * (Klo[m] + Khi[m]); }
@@ -361,11 +394,24 @@ k_transfer(const __grid_constant__ RtArgs A) {
       if (lit) { transport_apply(Am, h, st.f1); transport_apply(Am, h, st.f2); }
       if (applied) plasma_apply<MODEL>(A.units, F, dl, st);
     }
+    bool done;
+    if (PF) {
+      ++s;
+      done = (Xlo[1] >= C.Xcam[1] && Xlo[1] > Xhi[1]) || (Xlo[1] <= C.lx_in && Xlo[1] < Xhi[1]) || s >= A.max_steps;
+    } else {
+      --s;
+      done = s < 0;
+    }
 #pragma unroll
     for (int m = 0; m < 4; ++m) { Xhi[m] = Xlo[m]; Khi[m] = Klo[m]; }
-    --s;
-    if (s < 0) {
+    if (done) {
       // a-7: project on the camera's transverse legs, convert the invariant I/nu^3 to specific intensity
+      if (PF) {
+        double e[4][4], c1[4], c2[4];
+        observer_tetrad(C.G, Xhi, e, c1, c2);
+        stokes_congruence(dot4(c1, st.f1), dot4(c1, st.f2), dot4(c2, st.f1), dot4(c2, st.f2), st.S);
+        if (A.nfwd) A.nfwd[q] = s;
+      } else
       stokes_congruence(dot4(C.ecov1, st.f1), dot4(C.ecov1, st.f2), dot4(C.ecov2, st.f1), dot4(C.ecov2, st.f2), st.S);
       const double nu3 = A.units.nu_obs * A.units.nu_obs * A.units.nu_obs;
       A.I[q] = st.S[0] * nu3; A.Q[q] = st.S[1] * nu3; A.U[q] = st.S[2] * nu3; A.V[q] = st.S[3] * nu3;
@@ -514,6 +560,14 @@ __global__ void k_reduce_final(const ReducePartial* part, int nparts, double sca
 __global__ void k_merge_long(int n_long, const int32_t* long_list, const int32_t* nsteps_long, int32_t* nsteps) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n_long) { const int32_t q = long_list[i]; nsteps[q] = nsteps_long[q]; }
+}
+
+// sum of the forward-step counts of the path-free variant (integer: order-independent)
+__global__ void k_sum_i32(const int32_t* v, int64_t n, long long* out) {
+  long long s = 0;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) s += v[i];
+  s = warp_sum_ll(s);
+  if ((threadIdx.x & 31) == 0 && s != 0) atomicAdd((unsigned long long*)out, (unsigned long long)s);
 }
 
 __global__ void k_max_i32(const int32_t* v, int n, int* out) {  // probe maximum (one block)
