@@ -30,8 +30,8 @@ FLOP_PER_STEP = {"transfer_adaf": 1663.0, "transfer_grid": 404.0, "geodesic_adaf
 # DRAM bytes per step of k_transfer (dram__bytes_read + write of one launch / its thread-steps, same captures)
 DRAM_BYTES_PER_STEP = {"transfer_adaf": 64.2, "transfer_grid": 69.6}
 # --path-free (PAPER.md:43 variant): per FORWARD step of k_transfer<model, 1> (RK4 push + transfer step in one kernel)
-FLOP_PER_STEP_PF = {"transfer_adaf": 2657.0, "transfer_grid": 1573.0}
-DRAM_BYTES_PER_STEP_PF = {"transfer_adaf": 0.1, "transfer_grid": 6.0}
+FLOP_PER_STEP_PF = {"transfer_adaf": 2656.0, "transfer_grid": 1589.0}
+DRAM_BYTES_PER_STEP_PF = {"transfer_adaf": 0.1, "transfer_grid": 0.9}
 # ALU roofline denominator: 148 SMs x 4 sub-partitions x 16 FP64 lanes x 2 flop x 1.965 GHz
 FP64_PEAK_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
 

@@ -286,6 +286,12 @@ struct RtArgs {
 #ifndef IPOLE_RT_MINB_ANALYTIC
 #define IPOLE_RT_MINB_ANALYTIC 3
 #endif
+#ifndef IPOLE_PF_MINB_ANALYTIC
+#define IPOLE_PF_MINB_ANALYTIC 2   // path-free variant: resident blocks per SM, analytic models / grid model
+#endif
+#ifndef IPOLE_PF_MINB_GRID
+#define IPOLE_PF_MINB_GRID 3         // (measured: profiles/r1_pathfree.md)
+#endif
 #ifndef IPOLE_RT_SYNC
 #define IPOLE_RT_SYNC 0
 #endif
@@ -305,7 +311,8 @@ struct RtArgs {
 // transfer step over its two end points; it stops at r >= r_cam moving outward (or r <= r_in moving inward, or after
 // max_steps steps), and the tensor is read in the observer tetrad built at that end point.
 template <int MODEL, int PF>
-__global__ void __launch_bounds__(IPOLE_RT_THREADS, (MODEL == MODEL_GRID) ? IPOLE_RT_MINB : IPOLE_RT_MINB_ANALYTIC)
+__global__ void __launch_bounds__(IPOLE_RT_THREADS, (MODEL == MODEL_GRID) ? (PF ? IPOLE_PF_MINB_GRID : IPOLE_RT_MINB)
+                                                                           : (PF ? IPOLE_PF_MINB_ANALYTIC : IPOLE_RT_MINB_ANALYTIC))
 k_transfer(const __grid_constant__ RtArgs A) {
   const CamDev& C = A.cam;
   const int64_t count = A.count_dev ? (int64_t)*A.count_dev : A.count;

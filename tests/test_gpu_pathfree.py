@@ -142,3 +142,31 @@ def test_pf_w5_adaf_4096_sampled(ipole, ref):
     import torch
     pol = torch.sqrt(img["Q"] ** 2 + img["U"] ** 2 + img["V"] ** 2)
     assert bool((pol <= img["I"] * (1 + 1e-12)).all()) and bool(torch.isfinite(img["I"]).all())
+
+
+def test_pf_difference_from_stored_path_vs_eps(ipole, capsys):
+    """"for a typically adopted value of epsilon the differences in all Stokes parameter images produced
+    by CPU and GPU codes are negligible" -- measured here on the GPU for both variants (W2 geometry, 256^2, 230 GHz).
+    `pytest tests/test_gpu_pathfree.py -m gpu -k vs_eps -s` prints the table kept in profiles/r1_pathfree.md."""
+    rows = []
+    for eps in (0.04, 0.02, 0.01, 0.005):
+        cam = W.camera("adaf", 256, eps=eps)
+        g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
+        a = to_np(g.make_image())
+        ns, nt = g.ray_info()
+        g.set_path_free(True)
+        b = to_np(g.make_image())
+        tot = a["I"].sum()
+        dtot = [abs(b[k].sum() - a[k].sum()) / tot for k in "IQUV"]
+        lit = a["I"] > 1e-6 * a["I"].max()
+        rel = np.abs(b["I"] - a["I"])[lit] / a["I"][lit]
+        pol = np.maximum.reduce([np.abs(b[k] - a[k])[lit] / a["I"][lit] for k in "QUV"])
+        rows.append((eps, dtot, np.median(rel), np.percentile(rel, 99), rel.max(), np.median(pol), np.percentile(pol, 99)))
+    with capsys.disabled():
+        print("\neps    |dI|/I    |dQ|/I    |dU|/I    |dV|/I   pixel I: median   p99      max     pixel Q,U,V/I: median  p99")
+        for eps, dtot, med, p99, mx, pmed, pp99 in rows:
+            print("%.3f  %.2e  %.2e  %.2e  %.2e   %.2e  %.2e  %.2e   %.2e  %.2e" % ((eps,) + tuple(dtot) + (med, p99, mx, pmed, pp99)))
+    for eps, dtot, med, p99, mx, pmed, pp99 in rows:
+        if eps <= 0.02:
+            assert max(dtot) < 1e-3 and med < 1e-4 and pmed < 1e-4
+    assert rows[-1][2] < rows[0][2]   # the typical pixel difference shrinks with eps
