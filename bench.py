@@ -43,7 +43,110 @@ WORKLOADS = {
     "adaf1024": dict(kind="adaf", n=1024, config=None),   # profiling size (ncu --set full replays each kernel ~40x)
     "adaf256": dict(kind="adaf", n=256, config=1),
     "adaf32": dict(kind="adaf", n=32, config=0),
+    # many-small-images mode (128x128 images for model fitting): 64 parameter sets per call
+    "sweep128": dict(kind="adaf", n=128, config=None, sweep=64),
 }
+
+
+def sweep_models(M):
+    """Parameter sets of the model-fitting sweep: density, temperature and field scales on a seeded log-uniform draw."""
+    import numpy as np
+    rng = np.random.default_rng(230202733)
+    return [dict(n0=1e6 * 10 ** rng.uniform(-0.5, 0.5), Th0=30.0 * 10 ** rng.uniform(-0.3, 0.3),
+                 B0=30.0 * 10 ** rng.uniform(-0.3, 0.3)) for _ in range(M)]
+
+
+def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier):
+    """One step = one ipole_make_images_adaf call: M full-Stokes images of one camera (geodesics shared)."""
+    import torch
+    M, n = wl["sweep"], wl["n"]
+    models = sweep_models(M)
+    names = ["I", "Q", "U", "V"]
+    out = {k: torch.empty((M, n, n), dtype=torch.float64, device="cuda") for k in names}
+    for _ in range(args.warmup):
+        g.make_images_adaf(models, out=out)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        g.make_images_adaf(models, out=out)
+    ev1.record()
+    barrier()
+    ms = replicas.max_over_ranks(ev0.elapsed_time(ev1), "cuda")
+    st = g.stats()
+    # the same images by M separate calls (what a fitting loop does without the batch entry)
+    single = {k: torch.empty((n, n), dtype=torch.float64, device="cuda") for k in names}
+    def separate():
+        for mod in models:
+            g.load_adaf(**mod)
+            g.make_image(out=single)
+    separate()
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        separate()
+    ev1.record()
+    barrier()
+    ms_sep = replicas.max_over_ranks(ev0.elapsed_time(ev1), "cuda")
+    clocks = sampler.stop() if rank == 0 else None
+    # e2e: host buffers out (M images), parameters in
+    host = {k: torch.empty((M, n, n), dtype=torch.float64).pin_memory().numpy() for k in names}
+    g.make_images_adaf(models, out=host)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        g.set_camera(**cam)
+        g.make_images_adaf(models, out=host)
+    torch.cuda.synchronize()
+    dt = replicas.max_over_ranks(time.perf_counter() - t0, "cuda")
+    if rank != 0:
+        return
+    rays = M * n * n
+    value = replicas.job_throughput(rays * args.steps, ms * 1e-3, world)
+    rt_ms, steps_rt = st["ms_transfer"], st["total_steps"] * M
+    dfma_tf, _ = g.fp64_peak()
+    ach = FLOP_PER_STEP["transfer_adaf"] * steps_rt / (rt_ms * 1e-3) / 1e12
+    line = {"metric": "rays_per_s", "value": value, "unit": "rays/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "image": "%dx%d" % (n, n), "models_per_call": M, "model": "adaf",
+                       "freq_ghz": 230, "eps": cam["eps"], "full_stokes": True,
+                       "note": "a ray here is one (pixel, parameter set) pair; the %d geodesics are integrated once per call" % (n * n),
+                       "l2": "each call streams %.2f GB of path records once per warp (>> 126 MB L2)" % (st["total_steps"] * 64 / 1e9),
+                       "parallelism": "single GPU" if world == 1 else "one replica per GPU"},
+            "images_per_s": world * M * args.steps / (ms * 1e-3),
+            "separate_calls": {"images_per_s": world * M * args.steps / (ms_sep * 1e-3), "ms_per_%d_images" % M: ms_sep / args.steps,
+                               "speedup_of_the_batch_entry": ms_sep / ms},
+            "stage_ms": {"probe_sort": st["ms_probe"], "geodesic": st["ms_geodesic"], "transfer": rt_ms, "total": st["ms_total"]},
+            "gpu_launches": st["n_launches"] * args.steps,
+            "roofline": {"bound": "alu", "kernel": "k_transfer<adaf, sweep>", "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                         "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz; DFMA micro-benchmark on this GPU: %.1f" % dfma_tf,
+                         "achieved": ach, "frac": ach / FP64_PEAK_TFLOPS, "flop_per_step": FLOP_PER_STEP["transfer_adaf"],
+                         "avg_launch_ms": rt_ms, "kernel_share_of_step": rt_ms / st["ms_total"], "traffic": None},
+            "e2e": {"value": replicas.job_throughput(rays * args.steps, dt, world), "unit": "rays/s",
+                    "h2d_bytes_per_step": ipole.C.sizeof(ipole.Camera) + M * (ipole.C.sizeof(ipole.AdafParams) + 32),
+                    "d2h_bytes_per_step": 4 * rays * 8 + M * 32},
+            "clocks": clocks}
+    if not args.no_cpu_baseline and world == 1:
+        import numpy as np
+        from oracle import ipole_ref
+        cores = os.cpu_count() or 1
+        r = ipole_ref.Ctx(**cam); r.load_adaf(**models[0])
+        pix = (np.arange(8, n, 16)[:, None] * n + np.arange(8, n, 16)[None, :]).ravel().astype(np.int64)
+        t0 = time.perf_counter()
+        nm = 0
+        while time.perf_counter() - t0 < 10.0 and nm < M:
+            r.load_adaf(**models[nm]); r.make_pixels(pix, nthreads=cores); nm += 1
+        dtc = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": nm * pix.size / dtc, "unit": "rays/s", "cores": cores, "kind": "oracle",
+                                "sample": "%d parameter sets x %d rays (every 16th pixel of the %dx%d image), %.1f s; the oracle "
+                                          "re-integrates the geodesics for every parameter set" % (nm, pix.size, n, n, dtc)}
+    print(json.dumps(line), flush=True)
+
 
 
 class ClockSampler:
@@ -198,15 +301,20 @@ def main():
         desc, fields = W.fm_torus_grid(*wl["grid"])
         g.load_grid(desc, fields)
         grid_bytes = fields.nbytes
-    maps = bool(wl.get("maps"))
-    names = ["I", "Q", "U", "V"] + (["tau", "tauF"] if maps else [])
-    out = {k: torch.empty((wl["n"], wl["n"]), dtype=torch.float64, device="cuda") for k in names}
-    rays = wl["n"] * wl["n"]
-
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
+
+    if wl.get("sweep"):
+        run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier)
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    maps = bool(wl.get("maps"))
+    names = ["I", "Q", "U", "V"] + (["tau", "tauF"] if maps else [])
+    out = {k: torch.empty((wl["n"], wl["n"]), dtype=torch.float64, device="cuda") for k in names}
+    rays = wl["n"] * wl["n"]
 
     for _ in range(args.warmup):
         g.make_image(maps=maps, out=out)

@@ -137,6 +137,20 @@ int  ipole_make_image(ipole_ctx*, double* I, double* Q, double* U, double* V, do
  * all nx*ny pixels in order (= ipole_make_image). nsteps/nturn optional (int32; nturn bit 7 = step limit). */
 int  ipole_make_pixels(ipole_ctx*, int64_t n, const int64_t* pixels, double* I, double* Q, double* U, double* V,
                        double* tau, double* tauF, int32_t* nsteps, int32_t* nturn);
+/* Many small images for model fitting ("we run the ipole code up to 10,000,000 times ... images of
+ * moderate (to low) resolution of 128 x 128"): n_models analytic-flow parameter sets, optionally each
+ * at its own observing frequency freq_hz[m] (NULL: the camera's), seen by the context's camera.  The geodesics
+ * depend on the camera and the spin only, so they are integrated and stored ONCE and the stored paths are walked once
+ * per parameter set: work item (ray, model), the lanes of a warp share a ray.  Every image is what
+ * ipole_load_model_adaf(models[m]) + ipole_make_image would give at freq_hz[m].
+ * Outputs: I,Q,U,V (and optional tau, tauF) are [n_models][ny][nx], all host or all device, caller-owned;
+ * flux_jy (nullable, host or device) is [n_models][4] = sums of I,Q,U,V times the pixel solid angle in Jy.
+ * The model loaded in the context, if any, is left as it was; ipole_get_stats afterwards describes the shared
+ * geodesic pass and the image of models[0].  The stored-path design is used whatever ipole_set_path_free says.
+ * IPOLE_EINVAL: NULL arguments, n_models < 1, a non-positive frequency, a flat-metric camera, mixed host/device
+ * outputs, nx*ny*n_models > 2^31-1. */
+int  ipole_make_images_adaf(ipole_ctx*, int32_t n_models, const ipole_adaf_params* models, const double* freq_hz,
+                            double* I, double* Q, double* U, double* V, double* tau, double* tauF, double* flux_jy);
 /* Per-ray step count and theta-turning-point count (bit 7 set: ended on max_steps) of the last image,
  * [ny][nx] or n entries; host or device; either may be NULL. */
 int  ipole_get_ray_info(ipole_ctx*, int32_t* nsteps, int32_t* nturn);

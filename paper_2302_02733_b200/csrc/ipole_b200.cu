@@ -46,6 +46,9 @@ struct ipole_ctx {
   int last_pf = 0;               // the last image was made path-free
   double* d_endp = nullptr; int64_t endp_cap = 0;   // end points of the backward passes, [rays][8]
   long long* d_sum = nullptr;    // forward-step total of the path-free variant
+  AdafParams* d_sweep_models = nullptr; Units* d_sweep_units = nullptr;   // model sweep: SWEEP_MAX_MODELS entries each
+  double* d_sweep_out = nullptr; size_t sweep_out_doubles = 0;            // staging for host outputs of a sweep
+  int occ_sweep = 0;
 
   double* d_path = nullptr; size_t path_bytes = 0;
   double* d_path_long = nullptr; size_t path_long_bytes = 0;   // slots of max_steps for the long-ray passes
@@ -203,6 +206,14 @@ int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays, cudaStream
   return IPOLE_OK;
 }
 
+// model sweep (ipole_make_images_adaf): n_models parameter sets walked over the same stored paths
+struct Sweep {
+  int n_models;                 // all of them
+  const AdafParams* models;     // host
+  const Units* units;           // host
+  size_t out_stride;            // doubles between the planes of consecutive models
+};
+
 template <int PF>
 void launch_transfer_model(int model, int g, cudaStream_t st, const RtArgs& a) {
   if (model == MODEL_ADAF) k_transfer<MODEL_ADAF, PF><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
@@ -211,7 +222,32 @@ void launch_transfer_model(int model, int g, cudaStream_t st, const RtArgs& a) {
 }
 
 // pf: 0 stored path, 1 path-free with eps <= 0.04, 2 path-free with any eps
-int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_t st, int reserve = 0, int pf = 0) {
+int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_t st, int reserve = 0, int pf = 0,
+                    const Sweep* sw = nullptr) {
+  if (sw) {
+    // chunks of SWEEP_MAX_MODELS parameter sets; the parameter tables are re-sent per chunk on the launching stream
+    // (stream order keeps a table alive until the kernel that reads it has finished)
+    RtArgs t = a;
+    double* planes[6] = {a.I, a.Q, a.U, a.V, a.tau, a.tauF};
+    for (int m0 = 0; m0 < sw->n_models; m0 += SWEEP_MAX_MODELS) {
+      const int mc = std::min(SWEEP_MAX_MODELS, sw->n_models - m0);
+      const int s = span_begin(c, kind, st);
+      CK(cudaMemcpyAsync(c->d_sweep_models, sw->models + m0, mc * sizeof(AdafParams), cudaMemcpyHostToDevice, st));
+      CK(cudaMemcpyAsync(c->d_sweep_units, sw->units + m0, mc * sizeof(Units), cudaMemcpyHostToDevice, st));
+      t.model = c->d_sweep_models; t.units_arr = c->d_sweep_units; t.n_models = mc; t.out_stride = sw->out_stride;
+      t.I = planes[0] + (size_t)m0 * sw->out_stride; t.Q = planes[1] + (size_t)m0 * sw->out_stride;
+      t.U = planes[2] + (size_t)m0 * sw->out_stride; t.V = planes[3] + (size_t)m0 * sw->out_stride;
+      t.tau = planes[4] ? planes[4] + (size_t)m0 * sw->out_stride : nullptr;
+      t.tauF = planes[5] ? planes[5] + (size_t)m0 * sw->out_stride : nullptr;
+      CK(cudaMemsetAsync(t.queue, 0, sizeof(unsigned long long), st));
+      const int g = grid_for(c, c->occ_sweep, IPOLE_RT_THREADS, rays * mc, reserve);
+      k_transfer<MODEL_ADAF, 0, true><<<g, IPOLE_RT_THREADS, 0, st>>>(t);
+      span_end(c, s, st);
+      c->stats.n_launches++;
+      CK(cudaGetLastError());
+    }
+    return IPOLE_OK;
+  }
   const int s = span_begin(c, kind, st);
   const int g = grid_for(c, pf ? c->occ_pf[c->model][pf] : c->occ_rt[c->model], IPOLE_RT_THREADS, rays, reserve);
   if (pf == 0) launch_transfer_model<0>(c->model, g, st, a);
@@ -254,7 +290,7 @@ int finish_image(ipole_ctx* c, int64_t n, double* I, double* Q, double* U, doubl
 
 // the whole pipeline for n rays; outputs are DEVICE pointers indexed by ray
 int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double* Q, double* U, double* V, double* tau,
-             double* tauF) {
+             double* tauF, const Sweep* sw = nullptr) {
   int rc;
   if ((rc = ensure_rays(c, n)) != IPOLE_OK) return rc;
   c->spans_used = 0;
@@ -327,7 +363,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     const int64_t per = (int64_t)(budget / rec_bytes / (size_t)n) - 1;
     cap = (int)std::max<int64_t>(64, std::min<int64_t>(max_steps, per));
   }
-  if (c->opt_path_free) {
+  if (c->opt_path_free && !sw) {
     // ---- path-free bidirectional variant: one geodesic launch that keeps the end points, one
     // transfer launch that re-integrates forward.  Rays are ordered longest first, so the few very long rays start
     // at once and run beside the bulk. ----
@@ -388,7 +424,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
       t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = max_steps; t.base = base; t.count = cnt;
       t.order = c->d_long; t.path = c->d_path_long; t.nsteps = c->d_nsteps_long; t.queue = c->d_queues + (qi++);
       t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
-      if ((rcl = launch_transfer(c, t, LK_LONG, cnt, c->side)) != IPOLE_OK) return rcl;
+      if ((rcl = launch_transfer(c, t, LK_LONG, cnt, c->side, 0, 0, sw)) != IPOLE_OK) return rcl;
     }
     long_done = upto;
     return IPOLE_OK;
@@ -428,7 +464,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = cap; t.base = base; t.count = cnt; t.order = order;
     t.path = c->d_path; t.nsteps = c->d_nsteps; t.queue = c->d_queues + (qi++);
     t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
-    if ((rc = launch_transfer(c, t, LK_RT, cnt, c->stream, reserve)) != IPOLE_OK) return rc;
+    if ((rc = launch_transfer(c, t, LK_RT, cnt, c->stream, reserve, 0, sw)) != IPOLE_OK) return rc;
     c->stats.n_batches++;
     if (cap < max_steps) {   // the transfer kernel just queued keeps the GPU busy while the host waits here
       if ((rc = listed(c->ev_geo, n_long)) != IPOLE_OK) return rc;
@@ -495,6 +531,9 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_pf[MODEL_GRID][2], k_transfer<MODEL_GRID, 2>, IPOLE_RT_THREADS, 0);
   if (cudaGetLastError() != cudaSuccess) return fail(IPOLE_ECUDA);
   if (cudaMalloc(&c->d_sum, sizeof(long long)) != cudaSuccess) return fail(IPOLE_ENOMEM);
+  if (cudaMalloc(&c->d_sweep_models, SWEEP_MAX_MODELS * sizeof(AdafParams)) != cudaSuccess) return fail(IPOLE_ENOMEM);
+  if (cudaMalloc(&c->d_sweep_units, SWEEP_MAX_MODELS * sizeof(Units)) != cudaSuccess) return fail(IPOLE_ENOMEM);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_sweep, k_transfer<MODEL_ADAF, 0, true>, IPOLE_RT_THREADS, 0);
   rc = apply_camera(c, cam);
   if (rc != IPOLE_OK) return fail(rc);
   *out = c;
@@ -664,6 +703,66 @@ int ipole_make_pixels(ipole_ctx* c, int64_t n, const int64_t* pixels, double* I,
   if (nsteps) CK(cudaMemcpyAsync(nsteps, c->d_nsteps, n * sizeof(int32_t), cudaMemcpyDefault, c->stream));
   if (nturn) CK(cudaMemcpyAsync(nturn, c->d_nturn, n * sizeof(int32_t), cudaMemcpyDefault, c->stream));
   if (!dev) CK(cudaStreamSynchronize(c->stream));
+  return IPOLE_OK;
+}
+
+int ipole_make_images_adaf(ipole_ctx* c, int32_t n_models, const ipole_adaf_params* models, const double* freq_hz,
+                           double* I, double* Q, double* U, double* V, double* tau, double* tauF, double* flux_jy) {
+  if (!c || !models || n_models < 1 || !I || !Q || !U || !V) return IPOLE_EINVAL;
+  if (c->cam.G.mass == 0.0) return IPOLE_EINVAL;   // the flow is defined on Kerr only
+  const int64_t n = (int64_t)c->cam.nx * c->cam.ny;
+  if ((double)n * n_models > 2147483647.0) return IPOLE_EINVAL;
+  const bool dev = is_device_ptr(I);
+  const void* outs[] = {Q, U, V, tau, tauF};
+  for (const void* p : outs) if (p && is_device_ptr(p) != dev) return IPOLE_EINVAL;
+  if (freq_hz) for (int m = 0; m < n_models; ++m) if (!(freq_hz[m] > 0.0)) return IPOLE_EINVAL;
+  std::vector<AdafParams> pm(n_models);
+  std::vector<Units> um(n_models);
+  for (int m = 0; m < n_models; ++m) {
+    AdafParams& a = pm[m];
+    a.n0 = models[m].n0; a.p_n = models[m].p_n; a.Th0 = models[m].Th0; a.p_T = models[m].p_T; a.B0 = models[m].B0;
+    a.p_B = models[m].p_B; a.r_isco = isco_radius(c->cam.G.a);
+    um[m] = c->units;
+    if (freq_hz) { um[m].nu_obs = freq_hz[m]; um[m].dl_unit = um[m].L_unit / um[m].nu_obs; }
+  }
+  int rc;
+  if ((rc = ensure_rays(c, n)) != IPOLE_OK) return rc;
+  const size_t plane = (size_t)n * n_models;
+  double* o[6] = {I, Q, U, V, tau, tauF};
+  // the fluxes live at the start of the staging buffer; host outputs are staged behind them
+  const size_t need = (size_t)n_models * 4 + (dev ? 0 : plane * 6);
+  if (need > c->sweep_out_doubles) {
+    cudaFree(c->d_sweep_out); c->d_sweep_out = nullptr; c->sweep_out_doubles = 0;
+    cudaError_t e = cudaMalloc(&c->d_sweep_out, need * sizeof(double));
+    if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
+    c->sweep_out_doubles = need;
+  }
+  double* d_flux = c->d_sweep_out;
+  if (!dev) {
+    for (int k = 0; k < 6; ++k) o[k] = c->d_sweep_out + (size_t)n_models * 4 + (size_t)k * plane;
+    if (!tau) o[4] = nullptr;
+    if (!tauF) o[5] = nullptr;
+  }
+  Sweep sw;
+  sw.n_models = n_models; sw.models = pm.data(); sw.units = um.data(); sw.out_stride = (size_t)n;
+  const int model_before = c->model;
+  c->model = MODEL_ADAF;
+  rc = run_rays(c, n, nullptr, o[0], o[1], o[2], o[3], o[4], o[5], &sw);
+  c->model = model_before;
+  if (rc != IPOLE_OK) return rc;
+  if (flux_jy) {
+    const double pix_rad = c->cam.pix * c->units.L_unit / c->units.D_cm;
+    k_reduce_models<<<n_models, 256, 0, c->stream>>>(n, (size_t)n, o[0], o[1], o[2], o[3], pix_rad * pix_rad * 1e23, d_flux);
+    c->stats.n_launches++;
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(flux_jy, d_flux, (size_t)n_models * 4 * sizeof(double), cudaMemcpyDefault, c->stream));
+  }
+  if (!dev) {
+    double* h[6] = {I, Q, U, V, tau, tauF};
+    for (int k = 0; k < 6; ++k)
+      if (h[k]) CK(cudaMemcpyAsync(h[k], o[k], plane * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  }
+  if (!dev || (flux_jy && !is_device_ptr(flux_jy))) CK(cudaStreamSynchronize(c->stream));
   return IPOLE_OK;
 }
 
@@ -842,7 +941,7 @@ void ipole_free(ipole_ctx* c) {
   cudaFree(c->d_cam); cudaFree(c->d_model); cudaFree(c->d_grid); cudaFree(c->d_path);
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long);
   cudaFree(c->d_out); cudaFree(c->d_pixels); cudaFree(c->d_probe); cudaFree(c->d_queues); cudaFree(c->d_hist);
-  cudaFree(c->d_small); cudaFree(c->d_part); cudaFree(c->d_red); cudaFree(c->d_endp); cudaFree(c->d_sum);
+  cudaFree(c->d_small); cudaFree(c->d_part); cudaFree(c->d_red); cudaFree(c->d_endp); cudaFree(c->d_sum); cudaFree(c->d_sweep_models); cudaFree(c->d_sweep_units); cudaFree(c->d_sweep_out);
   for (auto& s : c->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
   cudaGetLastError();
   delete c;

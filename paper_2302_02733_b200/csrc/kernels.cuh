@@ -275,7 +275,12 @@ struct RtArgs {
   const double* endp;         // [total rays][8], indexed by q
   int32_t* nfwd;              // [total rays] steps of the forward pass (nullable)
   double eps; int max_steps;
+  // model sweep (SWEEP): work item w = ray * n_models + m; `model` points at n_models AdafParams, `units_arr` at
+  // n_models Units; outputs of model m start at plane + m * out_stride
+  int n_models; const Units* units_arr; size_t out_stride;
 };
+
+constexpr int SWEEP_MAX_MODELS = 64;   // parameter sets per transfer launch (shared memory: 88 B each)
 
 #ifndef IPOLE_RT_THREADS
 #define IPOLE_RT_THREADS 128
@@ -310,20 +315,29 @@ struct RtArgs {
 // push of +dl per step (dl = the step rule at the point the step starts from), each push followed by the same
 // transfer step over its two end points; it stops at r >= r_cam moving outward (or r <= r_in moving inward, or after
 // max_steps steps), and the tensor is read in the observer tetrad built at that end point.
-template <int MODEL, int PF>
+//
+// SWEEP: many small images for model fitting: the same stored paths are walked once
+// per parameter set.  Work item w -> (ray w / n_models, model w % n_models): the lanes of a warp share a ray, so one
+// 64-B record load serves up to 32 models and all of them finish the ray on the same step.
+template <int MODEL, int PF, bool SWEEP = false>
 __global__ void __launch_bounds__(IPOLE_RT_THREADS, (MODEL == MODEL_GRID) ? (PF ? IPOLE_PF_MINB_GRID : IPOLE_RT_MINB)
                                                                            : (PF ? IPOLE_PF_MINB_ANALYTIC : IPOLE_RT_MINB_ANALYTIC))
 k_transfer(const __grid_constant__ RtArgs A) {
+  static_assert(!SWEEP || (MODEL == MODEL_ADAF && PF == 0), "the sweep is built for the analytic model on stored paths");
   const CamDev& C = A.cam;
-  const int64_t count = A.count_dev ? (int64_t)*A.count_dev : A.count;
+  const int64_t count = (A.count_dev ? (int64_t)*A.count_dev : A.count) * (SWEEP ? A.n_models : 1);
   const size_t slot_doubles = (size_t)(A.cap + 1) * REC_DOUBLES;
-  __shared__ unsigned char model_smem[MODEL == MODEL_ADAF ? sizeof(AdafParams) : (MODEL == MODEL_SLAB ? sizeof(SlabParams) : sizeof(GridParams))];
+  constexpr int MODEL_BYTES = MODEL == MODEL_ADAF ? sizeof(AdafParams) : (MODEL == MODEL_SLAB ? sizeof(SlabParams) : sizeof(GridParams));
+  __shared__ __align__(8) unsigned char model_smem[MODEL_BYTES * (SWEEP ? SWEEP_MAX_MODELS : 1)];
+  __shared__ Units units_smem[SWEEP ? SWEEP_MAX_MODELS : 1];
   {
-    const int nb = (int)sizeof(model_smem);
+    const int nb = MODEL_BYTES * (SWEEP ? A.n_models : 1);
     for (int i = threadIdx.x; i < nb; i += blockDim.x) model_smem[i] = ((const unsigned char*)A.model)[i];
+    if (SWEEP) for (int i = threadIdx.x; i < A.n_models; i += blockDim.x) units_smem[i] = A.units_arr[i];
     __syncthreads();
   }
   const void* model = model_smem;
+  int mi = 0;             // SWEEP: parameter set of the lane's current work item
 
   PolState st;
   double Xhi[4], Khi[4];
@@ -334,9 +348,14 @@ k_transfer(const __grid_constant__ RtArgs A) {
 
   auto fetch = [&]() {
     for (;;) {
-      const int64_t li = (int64_t)atomicAdd(A.queue, 1ULL);
+      int64_t li = (int64_t)atomicAdd(A.queue, 1ULL);
       have = li < count;
       if (!have) return;
+      if (SWEEP) {
+        mi = (int)(li % A.n_models);
+        li /= A.n_models;
+        model = model_smem + (size_t)mi * MODEL_BYTES;
+      }
       q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
       double dl;
       if (PF) {
@@ -396,10 +415,10 @@ k_transfer(const __grid_constant__ RtArgs A) {
       // coefficients and the 4x4 step, which touch the Stokes numbers alone: same result, but the generator and
       // the tetrad are dead while the register-hungry part runs
       PlasmaFrame F;
-      const bool applied = maybe && plasma_frame<MODEL>(C.G, model, A.units, Xm, Km, p, g, gi, prim, st, F);
+      const bool applied = maybe && plasma_frame<MODEL>(C.G, model, SWEEP ? units_smem[mi] : A.units, Xm, Km, p, g, gi, prim, st, F);
       lit |= applied;
       if (lit) { transport_apply(Am, h, st.f1); transport_apply(Am, h, st.f2); }
-      if (applied) plasma_apply<MODEL>(A.units, F, dl, st);
+      if (applied) plasma_apply<MODEL>(SWEEP ? units_smem[mi] : A.units, F, dl, st);
     }
     bool done;
     if (PF) {
@@ -420,10 +439,12 @@ k_transfer(const __grid_constant__ RtArgs A) {
         if (A.nfwd) A.nfwd[q] = s;
       } else
       stokes_congruence(dot4(C.ecov1, st.f1), dot4(C.ecov1, st.f2), dot4(C.ecov2, st.f1), dot4(C.ecov2, st.f2), st.S);
-      const double nu3 = A.units.nu_obs * A.units.nu_obs * A.units.nu_obs;
-      A.I[q] = st.S[0] * nu3; A.Q[q] = st.S[1] * nu3; A.U[q] = st.S[2] * nu3; A.V[q] = st.S[3] * nu3;
-      if (A.tau) A.tau[q] = st.tau;
-      if (A.tauF) A.tauF[q] = st.tauF;
+      const double nu_o = SWEEP ? units_smem[mi].nu_obs : A.units.nu_obs;
+      const double nu3 = nu_o * nu_o * nu_o;
+      const size_t o = SWEEP ? (size_t)mi * A.out_stride + q : (size_t)q;
+      A.I[o] = st.S[0] * nu3; A.Q[o] = st.S[1] * nu3; A.U[o] = st.S[2] * nu3; A.V[o] = st.S[3] * nu3;
+      if (A.tau) A.tau[o] = st.tau;
+      if (A.tauF) A.tauF[o] = st.tauF;
       fetch();
     }
   }
@@ -561,6 +582,24 @@ __global__ void k_reduce_final(const ReducePartial* part, int nparts, double sca
   o.cp = (r.s[0] != 0.0) ? r.s[3] / r.s[0] : 0.0;
   o.total_steps = r.steps; o.max_steps = r.maxs; o.n_ring = r.ring; o.n_maxstep = r.maxed;
   *out = o;
+}
+
+// model sweep: flux of every image of the batch, one block per model (fixed shape => reproducible)
+__global__ void __launch_bounds__(256) k_reduce_models(int64_t n, size_t stride, const double* I, const double* Q,
+                                                       const double* U, const double* V, double scale, double* flux) {
+  const size_t o = (size_t)blockIdx.x * stride;
+  double s[4] = {0, 0, 0, 0};
+  for (int64_t q = threadIdx.x; q < n; q += blockDim.x) { s[0] += I[o + q]; s[1] += Q[o + q]; s[2] += U[o + q]; s[3] += V[o + q]; }
+  __shared__ double sh[8][4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) s[k] = warp_sum(s[k]);
+  if ((threadIdx.x & 31) == 0) for (int k = 0; k < 4; ++k) sh[threadIdx.x >> 5][k] = s[k];
+  __syncthreads();
+  if (threadIdx.x < 4) {
+    double t = sh[0][threadIdx.x];
+    for (int w = 1; w < 8; ++w) t += sh[w][threadIdx.x];
+    flux[4 * blockIdx.x + threadIdx.x] = t * scale;
+  }
 }
 
 // step counts of the long-ray passes -> nsteps (after every bulk kernel has finished)

@@ -18,7 +18,7 @@ OK, EINVAL, ENOMODEL, ENOMEM, ECUDA, ENOIMAGE = 0, -1, -2, -3, -4, -5
 
 #: every symbol include/ipole.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_options", "ipole_set_path_free", "ipole_load_model_adaf",
-           "ipole_load_model_slab", "ipole_load_model_grid", "ipole_make_image", "ipole_make_pixels",
+           "ipole_load_model_slab", "ipole_load_model_grid", "ipole_make_image", "ipole_make_pixels", "ipole_make_images_adaf",
            "ipole_get_ray_info", "ipole_get_stats", "ipole_get_camera_tetrad", "ipole_trace_pixel",
            "ipole_eval_connection", "ipole_eval_coefficients", "ipole_eval_stokes_step", "ipole_eval_bessel",
            "ipole_eval_plasma", "ipole_eval_math", "ipole_measure_fp64_peak", "ipole_last_cuda_error", "ipole_free", "ipole_strerror",
@@ -81,6 +81,7 @@ def lib():
         L.ipole_load_model_grid.argtypes = [vp, C.POINTER(GridDesc), C.POINTER(vp)]
         L.ipole_make_image.argtypes = [vp] + [vp] * 6
         L.ipole_make_pixels.argtypes = [vp, C.c_int64, vp] + [vp] * 8
+        L.ipole_make_images_adaf.argtypes = [vp, C.c_int32, C.POINTER(AdafParams), vp] + [vp] * 7
         L.ipole_get_ray_info.argtypes = [vp, vp, vp]
         L.ipole_get_stats.argtypes = [vp, C.POINTER(Stats)]
         L.ipole_get_camera_tetrad.argtypes = [vp, dp, dp]
@@ -214,6 +215,32 @@ class Ipole:
             out = {k: np.empty((self.ny, self.nx), dtype=np.float64) for k in names}
         args = [_ptr(out.get(k)) for k in ("I", "Q", "U", "V", "tau", "tauF")]
         _chk(lib().ipole_make_image(self._h, *args), "ipole_make_image")
+        return out
+
+    def make_images_adaf(self, models, freqs=None, maps=False, out=None, host=False):
+        """Many small images for model fitting (include/ipole.h ipole_make_images_adaf): `models` is a
+        list of dicts with the keys of load_adaf; `freqs` an optional list of observing frequencies in Hz.  The
+        geodesics are integrated once; returns dict of [n_models, ny, nx] arrays (torch CUDA tensors, or numpy with
+        host=True) plus "flux_jy" [n_models, 4] (numpy)."""
+        M = len(models)
+        arr = (AdafParams * M)()
+        for m, kw in enumerate(models):
+            d = dict(n0=1e6, p_n=-1.5, Th0=30.0, p_T=-1.0, B0=30.0, p_B=-1.25); d.update(kw)
+            arr[m] = AdafParams(d["n0"], d["p_n"], d["Th0"], d["p_T"], d["B0"], d["p_B"])
+        fr = None if freqs is None else np.ascontiguousarray(freqs, dtype=np.float64)
+        assert fr is None or fr.size == M
+        names = ["I", "Q", "U", "V"] + (["tau", "tauF"] if maps else [])
+        if out is None:
+            if host:
+                out = {k: np.empty((M, self.ny, self.nx), dtype=np.float64) for k in names}
+            else:
+                import torch
+                out = {k: torch.empty((M, self.ny, self.nx), dtype=torch.float64, device="cuda") for k in names}
+        flux = np.zeros((M, 4))
+        args = [_ptr(out.get(k)) for k in ("I", "Q", "U", "V", "tau", "tauF")]
+        _chk(lib().ipole_make_images_adaf(self._h, M, arr, _ptr(fr), *args, _ptr(flux)), "ipole_make_images_adaf")
+        out = dict(out)
+        out["flux_jy"] = flux
         return out
 
     def make_pixels(self, pixels):

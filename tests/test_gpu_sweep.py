@@ -1,0 +1,101 @@
+"""Many-small-images mode, pytest -m gpu: ipole_make_images_adaf walks the stored
+paths of one geodesic pass once per parameter set.  Every image of the batch must be the image ipole_make_image gives
+for that parameter set and frequency, and must match the oracle to the north-star tolerances."""
+import numpy as np
+import pytest
+
+from paper_2302_02733_b200 import workloads as W
+from test_gpu_parity import check_parity, to_np, ipole, NTHREADS  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+MODELS = [dict(n0=1e6, Th0=30.0, B0=30.0), dict(n0=3e5, Th0=45.0, B0=20.0, p_n=-1.3), dict(n0=2e6, Th0=12.0, B0=55.0, p_T=-0.8),
+          dict(n0=5e6, Th0=8.0, B0=80.0, p_B=-1.1), dict(n0=1e5, Th0=60.0, B0=10.0)]
+FREQS = [230e9, 345e9, 86e9, 230e9, 690e9]
+
+
+def single(ipole, cam, model, freq, maps=True):
+    g = ipole.Ipole(**dict(cam, freq_hz=freq)); g.load_adaf(**model)
+    img = to_np(g.make_image(maps=maps))
+    return img, g.stats()
+
+
+def close(a, b, scale):
+    return np.abs(a - b).max() <= 1e-12 * scale
+
+
+def test_sweep_equals_single_images_and_oracle(ipole, ref):
+    cam = W.camera("adaf", 32)
+    g = ipole.Ipole(**cam)
+    out = g.make_images_adaf(MODELS, FREQS, maps=True)
+    st = g.stats()
+    assert st["n_batches"] == 1
+    for m, (mod, fr) in enumerate(zip(MODELS, FREQS)):
+        img, st1 = single(ipole, cam, mod, fr)
+        sc = img["I"].max()
+        for k in ("I", "Q", "U", "V"):
+            assert close(out[k][m].cpu().numpy().ravel(), img[k], sc), (m, k)
+        for k in ("tau", "tauF"):
+            assert np.allclose(out[k][m].cpu().numpy().ravel(), img[k], rtol=1e-12, atol=0), (m, k)
+        assert np.allclose(out["flux_jy"][m], st1["flux_jy"], rtol=1e-12, atol=1e-12 * abs(st1["flux_jy"][0]))
+        # against the oracle, north-star tolerances
+        r = ref.Ctx(**dict(cam, freq_hz=fr)); r.load_adaf(**mod)
+        want = r.make_pixels(nthreads=NTHREADS)
+        got = {k: out[k][m].cpu().numpy().ravel() for k in ("I", "Q", "U", "V", "tau", "tauF")}
+        check_parity(got, want, "sweep model %d" % m, min_lit=0.99)
+    # the shared geodesic pass is the ordinary one
+    assert st["total_steps"] == int(want["nsteps"].sum())
+
+
+def test_sweep_chunks_batches_long_rays_and_host_buffers(ipole):
+    cam = W.camera("adaf", 24, max_steps=6000)
+    g = ipole.Ipole(**cam)
+    g.load_adaf(n0=7e5)                          # a loaded model must survive the sweep untouched
+    before = to_np(g.make_image())
+    models = [dict(n0=1e6 * (1 + 0.03 * (m % 64)), Th0=30.0 - 0.2 * (m % 64)) for m in range(70)]   # > 64: two chunks
+    a = g.make_images_adaf(models, maps=True)
+    A = {k: a[k].cpu().numpy() for k in ("I", "Q", "U", "V", "tau", "tauF")}
+    for k in A:
+        assert np.array_equal(A[k][0:6], A[k][64:70]), k      # same parameters in both chunks: same bits
+    assert not np.array_equal(A["I"][0], A["I"][1])
+    after = to_np(g.make_image())
+    for k in before:
+        assert np.array_equal(before[k], after[k])
+    # spot-check two images of the batch against single calls
+    for m in (3, 69):
+        img, _ = single(ipole, cam, models[m], cam["freq_hz"])
+        for k in ("I", "Q", "U", "V"):
+            assert close(A[k][m].ravel(), img[k], img["I"].max()), (m, k)
+    # host buffers: the same bits as device buffers
+    h = g.make_images_adaf(models, maps=True, host=True)
+    for k in A:
+        assert np.array_equal(h[k], A[k]), k
+    assert np.array_equal(h["flux_jy"], a["flux_jy"])
+    # tiny path buffer: several ray batches, S_cap from the probe; then a slot too small for any ray (long-ray pass)
+    for opts in ((8 << 20, 2), (12 << 20, 0)):
+        g.set_options(*opts)
+        b = g.make_images_adaf(models[:9], maps=True)
+        st = g.stats()
+        assert st["n_batches"] > 1 or st["n_long"] > 0
+        for k in A:
+            assert np.array_equal(b[k].cpu().numpy(), A[k][:9]), (opts, k)
+    # the path-free switch does not apply to the sweep (the shared stored path is its point)
+    g.set_options(0, 1); g.set_path_free(True)
+    c = g.make_images_adaf(models[:3])
+    for k in ("I", "Q", "U", "V"):
+        assert np.array_equal(c[k].cpu().numpy(), A[k][:3])
+
+
+def test_sweep_errors(ipole):
+    g = ipole.Ipole(**W.camera("adaf", 8))
+    with pytest.raises(ipole.IpoleError):
+        g.make_images_adaf([])
+    with pytest.raises(ipole.IpoleError):
+        g.make_images_adaf([dict()], freqs=[0.0])
+    flat = ipole.Ipole(**W.camera("adaf", 8, spin=0.0, flat_metric=1))
+    with pytest.raises(ipole.IpoleError):
+        flat.make_images_adaf([dict()])
+    out = g.make_images_adaf([dict()])        # one model, default parameters = W1's flow
+    g.load_adaf(**W.ADAF)
+    img = to_np(g.make_image())
+    assert close(out["I"][0].cpu().numpy().ravel(), img["I"], img["I"].max())
