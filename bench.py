@@ -45,6 +45,7 @@ WORKLOADS = {
     "adaf32": dict(kind="adaf", n=32, config=0),
     # many-small-images mode (128x128 images for model fitting): 64 parameter sets per call
     "sweep128": dict(kind="adaf", n=128, config=None, sweep=64),
+    "gridsweep128": dict(kind="grid", n=128, config=None, sweep=64, grid=(288, 128, 128)),
 }
 
 
@@ -56,11 +57,25 @@ def sweep_models(M):
                  B0=30.0 * 10 ** rng.uniform(-0.3, 0.3)) for _ in range(M)]
 
 
-def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier):
-    """One step = one ipole_make_images_adaf call: M full-Stokes images of one camera (geodesics shared)."""
+def sweep_sets(M, desc):
+    import numpy as np
+    rng = np.random.default_rng(230202733)
+    return [dict(M_unit=desc["M_unit"] * 10 ** rng.uniform(-0.5, 0.5), Rlow=1.0, Rhigh=10 ** rng.uniform(0.0, 2.0)) for _ in range(M)]
+
+
+def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier, grid=None):
+    """One step = one ipole_make_images_{adaf,grid} call: M full-Stokes images of one camera (geodesics shared)."""
     import torch
     M, n = wl["sweep"], wl["n"]
-    models = sweep_models(M)
+    is_grid = wl["kind"] == "grid"
+    models = sweep_sets(M, grid[0]) if is_grid else sweep_models(M)
+    if is_grid:
+        g.make_images_adaf = g.make_images_grid     # same call shape below
+        def load_one(mod):
+            d = dict(grid[0]); d.update(mod); g.load_grid(d, grid[1])
+    else:
+        def load_one(mod):
+            g.load_adaf(**mod)
     names = ["I", "Q", "U", "V"]
     out = {k: torch.empty((M, n, n), dtype=torch.float64, device="cuda") for k in names}
     for _ in range(args.warmup):
@@ -82,7 +97,7 @@ def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier)
     single = {k: torch.empty((n, n), dtype=torch.float64, device="cuda") for k in names}
     def separate():
         for mod in models:
-            g.load_adaf(**mod)
+            load_one(mod)
             g.make_image(out=single)
     separate()
     barrier()
@@ -109,11 +124,12 @@ def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier)
     value = replicas.job_throughput(rays * args.steps, ms * 1e-3, world)
     rt_ms, steps_rt = st["ms_transfer"], st["total_steps"] * M
     dfma_tf, _ = g.fp64_peak()
-    ach = FLOP_PER_STEP["transfer_adaf"] * steps_rt / (rt_ms * 1e-3) / 1e12
+    fkey = "transfer_" + wl["kind"]
+    ach = FLOP_PER_STEP[fkey] * steps_rt / (rt_ms * 1e-3) / 1e12
     line = {"metric": "rays_per_s", "value": value, "unit": "rays/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "image": "%dx%d" % (n, n), "models_per_call": M, "model": "adaf",
+            "config": {"workload": args.workload, "image": "%dx%d" % (n, n), "models_per_call": M, "model": wl["kind"],
                        "freq_ghz": 230, "eps": cam["eps"], "full_stokes": True,
                        "note": "a ray here is one (pixel, parameter set) pair; the %d geodesics are integrated once per call" % (n * n),
                        "l2": "each call streams %.2f GB of path records once per warp (>> 126 MB L2)" % (st["total_steps"] * 64 / 1e9),
@@ -123,9 +139,10 @@ def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier)
                                "speedup_of_the_batch_entry": ms_sep / ms},
             "stage_ms": {"probe_sort": st["ms_probe"], "geodesic": st["ms_geodesic"], "transfer": rt_ms, "total": st["ms_total"]},
             "gpu_launches": st["n_launches"] * args.steps,
-            "roofline": {"bound": "alu", "kernel": "k_transfer<adaf, sweep>", "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+            "roofline": {"bound": "alu", "kernel": "k_transfer<%s, sweep>" % wl["kind"], "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                          "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz; DFMA micro-benchmark on this GPU: %.1f" % dfma_tf,
-                         "achieved": ach, "frac": ach / FP64_PEAK_TFLOPS, "flop_per_step": FLOP_PER_STEP["transfer_adaf"],
+                         "achieved": ach, "frac": ach / FP64_PEAK_TFLOPS, "flop_per_step": FLOP_PER_STEP[fkey],
+                         "flop_note": "flop per step of the single-image kernel (the sweep runs the same arithmetic per pair)",
                          "avg_launch_ms": rt_ms, "kernel_share_of_step": rt_ms / st["ms_total"], "traffic": None},
             "e2e": {"value": replicas.job_throughput(rays * args.steps, dt, world), "unit": "rays/s",
                     "h2d_bytes_per_step": ipole.C.sizeof(ipole.Camera) + M * (ipole.C.sizeof(ipole.AdafParams) + 32),
@@ -135,12 +152,17 @@ def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier)
         import numpy as np
         from oracle import ipole_ref
         cores = os.cpu_count() or 1
-        r = ipole_ref.Ctx(**cam); r.load_adaf(**models[0])
+        r = ipole_ref.Ctx(**cam)
+        def ref_load(mod):
+            if is_grid:
+                d = dict(grid[0]); d.update(mod); r.load_grid(d, grid[1])
+            else:
+                r.load_adaf(**mod)
         pix = (np.arange(8, n, 16)[:, None] * n + np.arange(8, n, 16)[None, :]).ravel().astype(np.int64)
         t0 = time.perf_counter()
         nm = 0
         while time.perf_counter() - t0 < 10.0 and nm < M:
-            r.load_adaf(**models[nm]); r.make_pixels(pix, nthreads=cores); nm += 1
+            ref_load(models[nm]); r.make_pixels(pix, nthreads=cores); nm += 1
         dtc = time.perf_counter() - t0
         line["cpu_baseline"] = {"value": nm * pix.size / dtc, "unit": "rays/s", "cores": cores, "kind": "oracle",
                                 "sample": "%d parameter sets x %d rays (every 16th pixel of the %dx%d image), %.1f s; the oracle "
@@ -307,7 +329,8 @@ def main():
         torch.cuda.synchronize()
 
     if wl.get("sweep"):
-        run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier)
+        run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier,
+                  grid=(desc, fields) if wl["kind"] == "grid" else None)
         if world > 1:
             dist.destroy_process_group()
         return

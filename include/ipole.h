@@ -151,6 +151,14 @@ int  ipole_make_pixels(ipole_ctx*, int64_t n, const int64_t* pixels, double* I, 
  * outputs, nx*ny*n_models > 2^31-1. */
 int  ipole_make_images_adaf(ipole_ctx*, int32_t n_models, const ipole_adaf_params* models, const double* freq_hz,
                             double* I, double* Q, double* U, double* V, double* tau, double* tauF, double* flux_jy);
+/* The same for the grid model loaded in the context (IPOLE_ENOMODEL otherwise): each set replaces the mass unit and
+ * the electron-temperature parameters of ipole_grid_desc, optionally at its own frequency -- the parameters a GRMHD
+ * fit varies at fixed snapshot and viewing angle.  Every image is what ipole_load_model_grid with those three numbers
+ * + ipole_make_image would give.  The lanes of a warp share a ray, so the eight-cell gather of a step is one
+ * broadcast load for up to 32 sets.  IPOLE_EINVAL also for M_unit <= 0. */
+typedef struct { double M_unit, Rlow, Rhigh; } ipole_grid_scales;
+int  ipole_make_images_grid(ipole_ctx*, int32_t n_models, const ipole_grid_scales* sets, const double* freq_hz,
+                            double* I, double* Q, double* U, double* V, double* tau, double* tauF, double* flux_jy);
 /* Per-ray step count and theta-turning-point count (bit 7 set: ended on max_steps) of the last image,
  * [ny][nx] or n entries; host or device; either may be NULL. */
 int  ipole_get_ray_info(ipole_ctx*, int32_t* nsteps, int32_t* nturn);

@@ -46,9 +46,9 @@ struct ipole_ctx {
   int last_pf = 0;               // the last image was made path-free
   double* d_endp = nullptr; int64_t endp_cap = 0;   // end points of the backward passes, [rays][8]
   long long* d_sum = nullptr;    // forward-step total of the path-free variant
-  AdafParams* d_sweep_models = nullptr; Units* d_sweep_units = nullptr;   // model sweep: SWEEP_MAX_MODELS entries each
+  void* d_sweep_models = nullptr; Units* d_sweep_units = nullptr;   // model sweep: SWEEP_MAX_MODELS entries each
   double* d_sweep_out = nullptr; size_t sweep_out_doubles = 0;            // staging for host outputs of a sweep
-  int occ_sweep = 0;
+  int occ_sweep[4] = {0, 0, 0, 0};
 
   double* d_path = nullptr; size_t path_bytes = 0;
   double* d_path_long = nullptr; size_t path_long_bytes = 0;   // slots of max_steps for the long-ray passes
@@ -209,7 +209,8 @@ int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays, cudaStream
 // model sweep (ipole_make_images_adaf): n_models parameter sets walked over the same stored paths
 struct Sweep {
   int n_models;                 // all of them
-  const AdafParams* models;     // host
+  const void* lane_tab;         // host: AdafParams[n_models] or GridScales[n_models]
+  size_t lane_bytes;
   const Units* units;           // host
   size_t out_stride;            // doubles between the planes of consecutive models
 };
@@ -232,16 +233,18 @@ int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_
     for (int m0 = 0; m0 < sw->n_models; m0 += SWEEP_MAX_MODELS) {
       const int mc = std::min(SWEEP_MAX_MODELS, sw->n_models - m0);
       const int s = span_begin(c, kind, st);
-      CK(cudaMemcpyAsync(c->d_sweep_models, sw->models + m0, mc * sizeof(AdafParams), cudaMemcpyHostToDevice, st));
+      CK(cudaMemcpyAsync(c->d_sweep_models, (const char*)sw->lane_tab + (size_t)m0 * sw->lane_bytes, mc * sw->lane_bytes,
+                         cudaMemcpyHostToDevice, st));
       CK(cudaMemcpyAsync(c->d_sweep_units, sw->units + m0, mc * sizeof(Units), cudaMemcpyHostToDevice, st));
-      t.model = c->d_sweep_models; t.units_arr = c->d_sweep_units; t.n_models = mc; t.out_stride = sw->out_stride;
+      t.lane_tab = c->d_sweep_models; t.units_arr = c->d_sweep_units; t.n_models = mc; t.out_stride = sw->out_stride;
       t.I = planes[0] + (size_t)m0 * sw->out_stride; t.Q = planes[1] + (size_t)m0 * sw->out_stride;
       t.U = planes[2] + (size_t)m0 * sw->out_stride; t.V = planes[3] + (size_t)m0 * sw->out_stride;
       t.tau = planes[4] ? planes[4] + (size_t)m0 * sw->out_stride : nullptr;
       t.tauF = planes[5] ? planes[5] + (size_t)m0 * sw->out_stride : nullptr;
       CK(cudaMemsetAsync(t.queue, 0, sizeof(unsigned long long), st));
-      const int g = grid_for(c, c->occ_sweep, IPOLE_RT_THREADS, rays * mc, reserve);
-      k_transfer<MODEL_ADAF, 0, true><<<g, IPOLE_RT_THREADS, 0, st>>>(t);
+      const int g = grid_for(c, c->occ_sweep[c->model], IPOLE_RT_THREADS, rays * mc, reserve);
+      if (c->model == MODEL_ADAF) k_transfer<MODEL_ADAF, 0, true><<<g, IPOLE_RT_THREADS, 0, st>>>(t);
+      else k_transfer<MODEL_GRID, 0, true><<<g, IPOLE_RT_THREADS, 0, st>>>(t);
       span_end(c, s, st);
       c->stats.n_launches++;
       CK(cudaGetLastError());
@@ -531,9 +534,10 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_pf[MODEL_GRID][2], k_transfer<MODEL_GRID, 2>, IPOLE_RT_THREADS, 0);
   if (cudaGetLastError() != cudaSuccess) return fail(IPOLE_ECUDA);
   if (cudaMalloc(&c->d_sum, sizeof(long long)) != cudaSuccess) return fail(IPOLE_ENOMEM);
-  if (cudaMalloc(&c->d_sweep_models, SWEEP_MAX_MODELS * sizeof(AdafParams)) != cudaSuccess) return fail(IPOLE_ENOMEM);
+  if (cudaMalloc(&c->d_sweep_models, SWEEP_MAX_MODELS * std::max(sizeof(AdafParams), sizeof(GridScales))) != cudaSuccess) return fail(IPOLE_ENOMEM);
   if (cudaMalloc(&c->d_sweep_units, SWEEP_MAX_MODELS * sizeof(Units)) != cudaSuccess) return fail(IPOLE_ENOMEM);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_sweep, k_transfer<MODEL_ADAF, 0, true>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_sweep[MODEL_ADAF], k_transfer<MODEL_ADAF, 0, true>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_sweep[MODEL_GRID], k_transfer<MODEL_GRID, 0, true>, IPOLE_RT_THREADS, 0);
   rc = apply_camera(c, cam);
   if (rc != IPOLE_OK) return fail(rc);
   *out = c;
@@ -706,25 +710,17 @@ int ipole_make_pixels(ipole_ctx* c, int64_t n, const int64_t* pixels, double* I,
   return IPOLE_OK;
 }
 
-int ipole_make_images_adaf(ipole_ctx* c, int32_t n_models, const ipole_adaf_params* models, const double* freq_hz,
-                           double* I, double* Q, double* U, double* V, double* tau, double* tauF, double* flux_jy) {
-  if (!c || !models || n_models < 1 || !I || !Q || !U || !V) return IPOLE_EINVAL;
-  if (c->cam.G.mass == 0.0) return IPOLE_EINVAL;   // the flow is defined on Kerr only
+}  // extern "C"
+
+namespace {
+// common part of the two sweep entries; `model` is the model the transfer kernel runs (the context's own stays loaded)
+int make_images(ipole_ctx* c, int model, int32_t n_models, const void* lane_tab, size_t lane_bytes, const Units* um,
+                double* I, double* Q, double* U, double* V, double* tau, double* tauF, double* flux_jy) {
   const int64_t n = (int64_t)c->cam.nx * c->cam.ny;
   if ((double)n * n_models > 2147483647.0) return IPOLE_EINVAL;
   const bool dev = is_device_ptr(I);
   const void* outs[] = {Q, U, V, tau, tauF};
   for (const void* p : outs) if (p && is_device_ptr(p) != dev) return IPOLE_EINVAL;
-  if (freq_hz) for (int m = 0; m < n_models; ++m) if (!(freq_hz[m] > 0.0)) return IPOLE_EINVAL;
-  std::vector<AdafParams> pm(n_models);
-  std::vector<Units> um(n_models);
-  for (int m = 0; m < n_models; ++m) {
-    AdafParams& a = pm[m];
-    a.n0 = models[m].n0; a.p_n = models[m].p_n; a.Th0 = models[m].Th0; a.p_T = models[m].p_T; a.B0 = models[m].B0;
-    a.p_B = models[m].p_B; a.r_isco = isco_radius(c->cam.G.a);
-    um[m] = c->units;
-    if (freq_hz) { um[m].nu_obs = freq_hz[m]; um[m].dl_unit = um[m].L_unit / um[m].nu_obs; }
-  }
   int rc;
   if ((rc = ensure_rays(c, n)) != IPOLE_OK) return rc;
   const size_t plane = (size_t)n * n_models;
@@ -744,9 +740,9 @@ int ipole_make_images_adaf(ipole_ctx* c, int32_t n_models, const ipole_adaf_para
     if (!tauF) o[5] = nullptr;
   }
   Sweep sw;
-  sw.n_models = n_models; sw.models = pm.data(); sw.units = um.data(); sw.out_stride = (size_t)n;
+  sw.n_models = n_models; sw.lane_tab = lane_tab; sw.lane_bytes = lane_bytes; sw.units = um; sw.out_stride = (size_t)n;
   const int model_before = c->model;
-  c->model = MODEL_ADAF;
+  c->model = model;
   rc = run_rays(c, n, nullptr, o[0], o[1], o[2], o[3], o[4], o[5], &sw);
   c->model = model_before;
   if (rc != IPOLE_OK) return rc;
@@ -764,6 +760,50 @@ int ipole_make_images_adaf(ipole_ctx* c, int32_t n_models, const ipole_adaf_para
   }
   if (!dev || (flux_jy && !is_device_ptr(flux_jy))) CK(cudaStreamSynchronize(c->stream));
   return IPOLE_OK;
+}
+
+void sweep_units(const ipole_ctx* c, int32_t n_models, const double* freq_hz, std::vector<Units>& um) {
+  um.assign(n_models, c->units);
+  if (freq_hz) for (int m = 0; m < n_models; ++m) { um[m].nu_obs = freq_hz[m]; um[m].dl_unit = um[m].L_unit / um[m].nu_obs; }
+}
+}  // namespace
+
+extern "C" {
+
+int ipole_make_images_adaf(ipole_ctx* c, int32_t n_models, const ipole_adaf_params* models, const double* freq_hz,
+                           double* I, double* Q, double* U, double* V, double* tau, double* tauF, double* flux_jy) {
+  if (!c || !models || n_models < 1 || !I || !Q || !U || !V) return IPOLE_EINVAL;
+  if (c->cam.G.mass == 0.0) return IPOLE_EINVAL;   // the flow is defined on Kerr only
+  if (freq_hz) for (int m = 0; m < n_models; ++m) if (!(freq_hz[m] > 0.0)) return IPOLE_EINVAL;
+  std::vector<AdafParams> pm(n_models);
+  std::vector<Units> um;
+  sweep_units(c, n_models, freq_hz, um);
+  for (int m = 0; m < n_models; ++m) {
+    AdafParams& a = pm[m];
+    a.n0 = models[m].n0; a.p_n = models[m].p_n; a.Th0 = models[m].Th0; a.p_T = models[m].p_T; a.B0 = models[m].B0;
+    a.p_B = models[m].p_B; a.r_isco = isco_radius(c->cam.G.a);
+  }
+  // the kernel reads the uniform model block too (unused by the analytic sweep): any valid device block will do
+  return make_images(c, MODEL_ADAF, n_models, pm.data(), sizeof(AdafParams), um.data(), I, Q, U, V, tau, tauF, flux_jy);
+}
+
+int ipole_make_images_grid(ipole_ctx* c, int32_t n_models, const ipole_grid_scales* sets, const double* freq_hz,
+                           double* I, double* Q, double* U, double* V, double* tau, double* tauF, double* flux_jy) {
+  if (!c || !sets || n_models < 1 || !I || !Q || !U || !V) return IPOLE_EINVAL;
+  if (c->model != MODEL_GRID) return IPOLE_ENOMODEL;
+  if (freq_hz) for (int m = 0; m < n_models; ++m) if (!(freq_hz[m] > 0.0)) return IPOLE_EINVAL;
+  std::vector<GridScales> gs(n_models);
+  std::vector<Units> um;
+  sweep_units(c, n_models, freq_hz, um);
+  const double L = c->units.L_unit;
+  for (int m = 0; m < n_models; ++m) {
+    if (!(sets[m].M_unit > 0.0)) return IPOLE_EINVAL;
+    const double rho_unit = sets[m].M_unit / (L * L * L);    // as in ipole_load_model_grid
+    gs[m].ne_unit = rho_unit / (IP_MP + IP_ME);
+    gs[m].B_unit = IP_CL * std::sqrt(4.0 * M_PI * rho_unit);
+    gs[m].Rlow = sets[m].Rlow; gs[m].Rhigh = sets[m].Rhigh;
+  }
+  return make_images(c, MODEL_GRID, n_models, gs.data(), sizeof(GridScales), um.data(), I, Q, U, V, tau, tauF, flux_jy);
 }
 
 int ipole_make_image(ipole_ctx* c, double* I, double* Q, double* U, double* V, double* tau, double* tauF) {

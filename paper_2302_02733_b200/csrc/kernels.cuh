@@ -275,12 +275,13 @@ struct RtArgs {
   const double* endp;         // [total rays][8], indexed by q
   int32_t* nfwd;              // [total rays] steps of the forward pass (nullable)
   double eps; int max_steps;
-  // model sweep (SWEEP): work item w = ray * n_models + m; `model` points at n_models AdafParams, `units_arr` at
-  // n_models Units; outputs of model m start at plane + m * out_stride
-  int n_models; const Units* units_arr; size_t out_stride;
+  // model sweep (SWEEP): work item w = ray * n_models + m; `lane_tab` points at n_models AdafParams (analytic model)
+  // or GridScales (grid model; `model` is the shared GridParams), `units_arr` at n_models Units; outputs of model m
+  // start at plane + m * out_stride
+  int n_models; const void* lane_tab; const Units* units_arr; size_t out_stride;
 };
 
-constexpr int SWEEP_MAX_MODELS = 64;   // parameter sets per transfer launch (shared memory: 88 B each)
+constexpr int SWEEP_MAX_MODELS = 64;   // parameter sets per transfer launch (shared memory: <= 88 B each)
 
 #ifndef IPOLE_RT_THREADS
 #define IPOLE_RT_THREADS 128
@@ -317,27 +318,33 @@ constexpr int SWEEP_MAX_MODELS = 64;   // parameter sets per transfer launch (sh
 // max_steps steps), and the tensor is read in the observer tetrad built at that end point.
 //
 // SWEEP: many small images for model fitting: the same stored paths are walked once
-// per parameter set.  Work item w -> (ray w / n_models, model w % n_models): the lanes of a warp share a ray, so one
+// per parameter set (analytic model: AdafParams per set; grid model: the four scale numbers GridScales per set over
+// the shared grid).  Work item w -> (ray w / n_models, model w % n_models): the lanes of a warp share a ray, so one
 // 64-B record load serves up to 32 models and all of them finish the ray on the same step.
 template <int MODEL, int PF, bool SWEEP = false>
 __global__ void __launch_bounds__(IPOLE_RT_THREADS, (MODEL == MODEL_GRID) ? (PF ? IPOLE_PF_MINB_GRID : IPOLE_RT_MINB)
                                                                            : (PF ? IPOLE_PF_MINB_ANALYTIC : IPOLE_RT_MINB_ANALYTIC))
 k_transfer(const __grid_constant__ RtArgs A) {
-  static_assert(!SWEEP || (MODEL == MODEL_ADAF && PF == 0), "the sweep is built for the analytic model on stored paths");
+  static_assert(!SWEEP || (MODEL != MODEL_SLAB && PF == 0), "the sweep is built for the ADAF and grid models on stored paths");
   const CamDev& C = A.cam;
   const int64_t count = (A.count_dev ? (int64_t)*A.count_dev : A.count) * (SWEEP ? A.n_models : 1);
   const size_t slot_doubles = (size_t)(A.cap + 1) * REC_DOUBLES;
   constexpr int MODEL_BYTES = MODEL == MODEL_ADAF ? sizeof(AdafParams) : (MODEL == MODEL_SLAB ? sizeof(SlabParams) : sizeof(GridParams));
-  __shared__ __align__(8) unsigned char model_smem[MODEL_BYTES * (SWEEP ? SWEEP_MAX_MODELS : 1)];
+  constexpr int LANE_BYTES = MODEL == MODEL_ADAF ? sizeof(AdafParams) : sizeof(GridScales);
+  __shared__ __align__(8) unsigned char model_smem[MODEL_BYTES];
+  __shared__ __align__(8) unsigned char lane_smem[SWEEP ? LANE_BYTES * SWEEP_MAX_MODELS : 8];
   __shared__ Units units_smem[SWEEP ? SWEEP_MAX_MODELS : 1];
   {
-    const int nb = MODEL_BYTES * (SWEEP ? A.n_models : 1);
-    for (int i = threadIdx.x; i < nb; i += blockDim.x) model_smem[i] = ((const unsigned char*)A.model)[i];
-    if (SWEEP) for (int i = threadIdx.x; i < A.n_models; i += blockDim.x) units_smem[i] = A.units_arr[i];
+    for (int i = threadIdx.x; i < MODEL_BYTES; i += blockDim.x) model_smem[i] = ((const unsigned char*)A.model)[i];
+    if (SWEEP) {
+      for (int i = threadIdx.x; i < LANE_BYTES * A.n_models; i += blockDim.x) lane_smem[i] = ((const unsigned char*)A.lane_tab)[i];
+      for (int i = threadIdx.x; i < A.n_models; i += blockDim.x) units_smem[i] = A.units_arr[i];
+    }
     __syncthreads();
   }
   const void* model = model_smem;
-  int mi = 0;             // SWEEP: parameter set of the lane's current work item
+  const void* lane = nullptr;   // SWEEP: the lane's own parameter set
+  int mi = 0;                   // SWEEP: its index
 
   PolState st;
   double Xhi[4], Khi[4];
@@ -354,7 +361,7 @@ k_transfer(const __grid_constant__ RtArgs A) {
       if (SWEEP) {
         mi = (int)(li % A.n_models);
         li /= A.n_models;
-        model = model_smem + (size_t)mi * MODEL_BYTES;
+        lane = lane_smem + (size_t)mi * LANE_BYTES;
       }
       q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
       double dl;
@@ -415,7 +422,7 @@ k_transfer(const __grid_constant__ RtArgs A) {
       // coefficients and the 4x4 step, which touch the Stokes numbers alone: same result, but the generator and
       // the tetrad are dead while the register-hungry part runs
       PlasmaFrame F;
-      const bool applied = maybe && plasma_frame<MODEL>(C.G, model, SWEEP ? units_smem[mi] : A.units, Xm, Km, p, g, gi, prim, st, F);
+      const bool applied = maybe && plasma_frame<MODEL>(C.G, model, SWEEP ? lane : nullptr, SWEEP ? units_smem[mi] : A.units, Xm, Km, p, g, gi, prim, st, F);
       lit |= applied;
       if (lit) { transport_apply(Am, h, st.f1); transport_apply(Am, h, st.f2); }
       if (applied) plasma_apply<MODEL>(SWEEP ? units_smem[mi] : A.units, F, dl, st);

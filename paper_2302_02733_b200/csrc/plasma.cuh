@@ -28,7 +28,9 @@ struct GridParams {
   const unsigned int* occ;       // device bitmap over stencil base cells (N1+1)(N2+1)N3: 1 = some corner has plasma
   const double* cells;           // device, cell-major: cells[((i*N2 + j)*N3 + k)*8 + field], fields rho,u,U1,U2,U3,B1,B2,B3
 };
-struct Units { double nu_obs, L_unit, D_cm, dl_unit; };  // dl_unit = L_unit / nu_obs
+struct Units { double nu_obs, L_unit, D_cm, dl_unit; };
+// the four numbers of GridParams a model-fitting sweep varies (ipole_make_images_grid)
+struct GridScales { double ne_unit, B_unit, Rlow, Rhigh; };  // dl_unit = L_unit / nu_obs
 
 struct Plasma {
   double ne, Th, B;
@@ -156,8 +158,8 @@ __device__ __forceinline__ bool grid_gather(const GridParams& M, const double X[
 }
 
 // Step 2: fluid four-velocity, field four-vector, n_e, Theta_e, B from the primitives and the metric at X.
-__device__ __forceinline__ bool grid_state(const Geom& G, const GridParams& M, const double prim[8], const Point& p,
-                                           const Sym7& g, const Inv6& gi, Plasma& P) {
+__device__ __forceinline__ bool grid_state(const Geom& G, const GridParams& M, const GridScales& S, const double prim[8],
+                                           const Point& p, const Sym7& g, const Inv6& gi, Plasma& P) {
   if (p.r > M.r_out) return false;
   const double rho = prim[0], uu = prim[1];
   const double alpha_l = ip_rsqrt(-gi.c00);
@@ -181,21 +183,22 @@ __device__ __forceinline__ bool grid_state(const Geom& G, const GridParams& M, c
   bc[3] = (B3 + bt * P.u[3]) * iu0;
   const double bsq = dotg(g, bc, bc);
   if (!(bsq > 0.0)) return false;
-  P.ne = rho * M.ne_unit;
-  P.B = ip_sqrt(bsq) * M.B_unit;
+  P.ne = rho * S.ne_unit;
+  P.B = ip_sqrt(bsq) * S.B_unit;
   const double beta = 2.0 * (M.gam - 1.0) * uu * ip_rcp(bsq);
   const double b2 = beta * beta;
-  const double R = (M.Rhigh * b2 + M.Rlow) * ip_rcp(1.0 + b2);
+  const double R = (S.Rhigh * b2 + S.Rlow) * ip_rcp(1.0 + b2);
   P.Th = (IP_MP / IP_ME) * (M.gam - 1.0) * uu * ip_rcp(rho * (1.0 + R));
 #pragma unroll
-  for (int m = 0; m < 4; ++m) P.b[m] = bc[m] * M.B_unit;
+  for (int m = 0; m < 4; ++m) P.b[m] = bc[m] * S.B_unit;
   return true;
 }
 
 __device__ __forceinline__ bool plasma_grid(const Geom& G, const GridParams& M, const double X[4], const Point& p,
                                             const Sym7& g, const Inv6& gi, Plasma& P) {
   double prim[8];
-  return grid_gather(M, X, prim) && grid_state(G, M, prim, p, g, gi, P);
+  const GridScales S = {M.ne_unit, M.B_unit, M.Rlow, M.Rhigh};
+  return grid_gather(M, X, prim) && grid_state(G, M, S, prim, p, g, gi, P);
 }
 
 // eps^{mu a b c} p_a q_b w_c with [0123] = +1
@@ -238,16 +241,22 @@ struct PlasmaFrame {
 
 // Plasma state and tetrad at (X, K); on success the carried legs st.f1, st.f2 are REPLACED by the new transverse
 // legs e_(1), e_(2) and F holds what plasma_apply needs.  Returns false where there is no plasma (nothing changed).
+// `lane` (model sweep only, else nullptr): the lane's own parameter set -- AdafParams, or GridScales overriding the four
+// scale numbers of the shared GridParams.
 template <int MODEL>
-__device__ __forceinline__ bool plasma_frame(const Geom& G, const void* model, const Units& U, const double X[4],
+__device__ __forceinline__ bool plasma_frame(const Geom& G, const void* model, const void* lane, const Units& U, const double X[4],
                                              const double K[4], const Point& p, const Sym7& g, const Inv6& gi,
                                              const double* prim /* grid model: from grid_gather */, PolState& st,
                                              PlasmaFrame& F) {
   Plasma P;
   bool present;
-  if (MODEL == MODEL_ADAF) present = plasma_adaf(G, *(const AdafParams*)model, X, p, g, gi, P);
+  if (MODEL == MODEL_ADAF) present = plasma_adaf(G, *(const AdafParams*)(lane ? lane : model), X, p, g, gi, P);
   else if (MODEL == MODEL_SLAB) present = plasma_slab(G, *(const SlabParams*)model, X, p, g, P);
-  else present = grid_state(G, *(const GridParams*)model, prim, p, g, gi, P);
+  else {
+    const GridParams& M = *(const GridParams*)model;
+    if (lane) present = grid_state(G, M, *(const GridScales*)lane, prim, p, g, gi, P);
+    else { const GridScales S = {M.ne_unit, M.B_unit, M.Rlow, M.Rhigh}; present = grid_state(G, M, S, prim, p, g, gi, P); }
+  }
   if (!present) return false;
 
   double kcov[4], ucov[4];

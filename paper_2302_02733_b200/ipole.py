@@ -18,7 +18,7 @@ OK, EINVAL, ENOMODEL, ENOMEM, ECUDA, ENOIMAGE = 0, -1, -2, -3, -4, -5
 
 #: every symbol include/ipole.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_options", "ipole_set_path_free", "ipole_load_model_adaf",
-           "ipole_load_model_slab", "ipole_load_model_grid", "ipole_make_image", "ipole_make_pixels", "ipole_make_images_adaf",
+           "ipole_load_model_slab", "ipole_load_model_grid", "ipole_make_image", "ipole_make_pixels", "ipole_make_images_adaf", "ipole_make_images_grid",
            "ipole_get_ray_info", "ipole_get_stats", "ipole_get_camera_tetrad", "ipole_trace_pixel",
            "ipole_eval_connection", "ipole_eval_coefficients", "ipole_eval_stokes_step", "ipole_eval_bessel",
            "ipole_eval_plasma", "ipole_eval_math", "ipole_measure_fp64_peak", "ipole_last_cuda_error", "ipole_free", "ipole_strerror",
@@ -56,6 +56,10 @@ class Stats(C.Structure):
                 ("ms_long", C.c_float), ("total_steps_forward", C.c_int64)]
 
 
+class GridScales(C.Structure):
+    _fields_ = [("M_unit", C.c_double), ("Rlow", C.c_double), ("Rhigh", C.c_double)]
+
+
 class IpoleError(RuntimeError):
     def __init__(self, code, what):
         self.code = code
@@ -82,6 +86,7 @@ def lib():
         L.ipole_make_image.argtypes = [vp] + [vp] * 6
         L.ipole_make_pixels.argtypes = [vp, C.c_int64, vp] + [vp] * 8
         L.ipole_make_images_adaf.argtypes = [vp, C.c_int32, C.POINTER(AdafParams), vp] + [vp] * 7
+        L.ipole_make_images_grid.argtypes = [vp, C.c_int32, C.POINTER(GridScales), vp] + [vp] * 7
         L.ipole_get_ray_info.argtypes = [vp, vp, vp]
         L.ipole_get_stats.argtypes = [vp, C.POINTER(Stats)]
         L.ipole_get_camera_tetrad.argtypes = [vp, dp, dp]
@@ -227,6 +232,18 @@ class Ipole:
         for m, kw in enumerate(models):
             d = dict(n0=1e6, p_n=-1.5, Th0=30.0, p_T=-1.0, B0=30.0, p_B=-1.25); d.update(kw)
             arr[m] = AdafParams(d["n0"], d["p_n"], d["Th0"], d["p_T"], d["B0"], d["p_B"])
+        return self._make_images(lib().ipole_make_images_adaf, "ipole_make_images_adaf", M, arr, freqs, maps, out, host)
+
+    def make_images_grid(self, sets, freqs=None, maps=False, out=None, host=False):
+        """The same for the loaded grid model: `sets` is a list of dicts M_unit, Rlow, Rhigh (include/ipole.h
+        ipole_make_images_grid)."""
+        M = len(sets)
+        arr = (GridScales * M)()
+        for m, kw in enumerate(sets):
+            arr[m] = GridScales(kw["M_unit"], kw["Rlow"], kw["Rhigh"])
+        return self._make_images(lib().ipole_make_images_grid, "ipole_make_images_grid", M, arr, freqs, maps, out, host)
+
+    def _make_images(self, fn, what, M, arr, freqs, maps, out, host):
         fr = None if freqs is None else np.ascontiguousarray(freqs, dtype=np.float64)
         assert fr is None or fr.size == M
         names = ["I", "Q", "U", "V"] + (["tau", "tauF"] if maps else [])
@@ -238,7 +255,7 @@ class Ipole:
                 out = {k: torch.empty((M, self.ny, self.nx), dtype=torch.float64, device="cuda") for k in names}
         flux = np.zeros((M, 4))
         args = [_ptr(out.get(k)) for k in ("I", "Q", "U", "V", "tau", "tauF")]
-        _chk(lib().ipole_make_images_adaf(self._h, M, arr, _ptr(fr), *args, _ptr(flux)), "ipole_make_images_adaf")
+        _chk(fn(self._h, M, arr, _ptr(fr), *args, _ptr(flux)), what)
         out = dict(out)
         out["flux_jy"] = flux
         return out

@@ -99,3 +99,47 @@ def test_sweep_errors(ipole):
     g.load_adaf(**W.ADAF)
     img = to_np(g.make_image())
     assert close(out["I"][0].cpu().numpy().ravel(), img["I"], img["I"].max())
+
+
+def test_grid_sweep_equals_single_images_and_oracle(ipole, ref):
+    desc, fields = W.fm_torus_grid(72, 32, 32)
+    cam = W.camera("grid", 32)
+    sets = [dict(M_unit=desc["M_unit"], Rlow=desc["Rlow"], Rhigh=desc["Rhigh"]),
+            dict(M_unit=3.0 * desc["M_unit"], Rlow=1.0, Rhigh=10.0), dict(M_unit=0.2 * desc["M_unit"], Rlow=2.0, Rhigh=80.0),
+            dict(M_unit=desc["M_unit"], Rlow=1.0, Rhigh=1.0)]
+    freqs = [230e9, 230e9, 86e9, 345e9]
+    g = ipole.Ipole(**cam); g.load_grid(desc, fields)
+    before = to_np(g.make_image(maps=True))
+    out = g.make_images_grid(sets, freqs, maps=True)
+    after = to_np(g.make_image(maps=True))
+    for k in before:
+        assert np.array_equal(before[k], after[k]), k      # the loaded model is untouched
+    for m, (st_, fr) in enumerate(zip(sets, freqs)):
+        d = dict(desc); d.update(st_)
+        g1 = ipole.Ipole(**dict(cam, freq_hz=fr)); g1.load_grid(d, fields)
+        img = to_np(g1.make_image(maps=True)); s1 = g1.stats()
+        sc = img["I"].max()
+        for k in ("I", "Q", "U", "V"):
+            assert close(out[k][m].cpu().numpy().ravel(), img[k], sc), (m, k)
+        for k in ("tau", "tauF"):
+            assert np.allclose(out[k][m].cpu().numpy().ravel(), img[k], rtol=1e-12, atol=0), (m, k)
+        assert np.allclose(out["flux_jy"][m], s1["flux_jy"], rtol=1e-12, atol=1e-12 * abs(s1["flux_jy"][0]))
+        r = ref.Ctx(**dict(cam, freq_hz=fr)); r.load_grid(d, fields)
+        want = r.make_pixels(nthreads=NTHREADS)
+        got = {k: out[k][m].cpu().numpy().ravel() for k in ("I", "Q", "U", "V", "tau", "tauF")}
+        check_parity(got, want, "grid sweep set %d" % m, min_lit=0.2)
+    assert np.array_equal(out["I"][0].cpu().numpy().ravel(), before["I"]) or close(out["I"][0].cpu().numpy().ravel(), before["I"], before["I"].max())
+    # 70 sets: two chunks; host buffers
+    many = [dict(M_unit=desc["M_unit"] * (1 + 0.05 * (m % 64)), Rlow=1.0, Rhigh=40.0) for m in range(70)]
+    a = g.make_images_grid(many)
+    h = g.make_images_grid(many, host=True)
+    for k in ("I", "Q", "U", "V"):
+        A = a[k].cpu().numpy()
+        assert np.array_equal(A[0:6], A[64:70]) and np.array_equal(h[k], A), k
+    # errors
+    with pytest.raises(ipole.IpoleError):
+        g.make_images_grid([dict(M_unit=0.0, Rlow=1.0, Rhigh=1.0)])
+    g0 = ipole.Ipole(**cam)
+    with pytest.raises(ipole.IpoleError) as ei:
+        g0.make_images_grid(sets)
+    assert ei.value.code == ipole.ENOMODEL
