@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <new>
 #include <vector>
 #include "kernels.cuh"
@@ -43,6 +44,7 @@ struct ipole_ctx {
   uint64_t opt_path_bytes = 0;
   int opt_sort = 1;
   int opt_path_free = 0;         // PAPER.md:43 bidirectional variant
+  int opt_occ = 1;               // grid model: plasma-contact range per ray (IPOLE_NO_OCC=1 in the environment turns it off)
   int last_pf = 0;               // the last image was made path-free
   double* d_endp = nullptr; int64_t endp_cap = 0;   // end points of the backward passes, [rays][8]
   long long* d_sum = nullptr;    // forward-step total of the path-free variant
@@ -58,6 +60,7 @@ struct ipole_ctx {
   cudaEvent_t ev_geo = nullptr, ev_side = nullptr;
   int64_t ray_cap = 0;           // capacity of the per-ray buffers below
   int32_t *d_nsteps = nullptr, *d_nturn = nullptr, *d_order = nullptr, *d_key = nullptr, *d_long = nullptr;
+  int2* d_srange = nullptr;      // grid model: per ray, the steps that may cross plasma (k_geodesic<true>)
   double* d_out = nullptr;       // staging for host outputs: 6 planes of ray_cap
   int64_t* d_pixels = nullptr; int64_t pixels_cap = 0;
   int32_t* d_probe = nullptr; int64_t probe_cap = 0;
@@ -71,7 +74,7 @@ struct ipole_ctx {
   bool have_image = false;
   int64_t last_n = 0;
   ipole_stats stats;
-  int occ_geo = 0, occ_rt[4] = {0, 0, 0, 0}, occ_pf[4][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+  int occ_geo = 0, occ_geo_occ = 0, occ_rt[4] = {0, 0, 0, 0}, occ_pf[4][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
 };
 
 namespace {
@@ -133,7 +136,7 @@ int apply_camera(ipole_ctx* c, const ipole_camera* k) {
 int ensure_rays(ipole_ctx* c, int64_t n) {
   if (n <= c->ray_cap) return IPOLE_OK;
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long); cudaFree(c->d_out);
-  cudaFree(c->d_nsteps_long);
+  cudaFree(c->d_nsteps_long); cudaFree(c->d_srange); c->d_srange = nullptr;
   c->d_nsteps = c->d_nturn = c->d_order = c->d_key = c->d_long = c->d_nsteps_long = nullptr; c->d_out = nullptr; c->ray_cap = 0;
   CK(cudaMalloc(&c->d_nsteps, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_nturn, n * sizeof(int32_t)));
@@ -141,6 +144,7 @@ int ensure_rays(ipole_ctx* c, int64_t n) {
   CK(cudaMalloc(&c->d_key, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_long, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_nsteps_long, n * sizeof(int32_t)));
+  CK(cudaMalloc(&c->d_srange, n * sizeof(int2)));
   CK(cudaMalloc(&c->d_out, 6 * n * sizeof(double)));
   c->ray_cap = n;
   return IPOLE_OK;
@@ -199,7 +203,8 @@ int grid_for(ipole_ctx* c, int occ, int threads, int64_t rays, int reserve = 0) 
 
 int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays, cudaStream_t st, int reserve = 0) {
   const int s = span_begin(c, kind, st);
-  k_geodesic<<<grid_for(c, c->occ_geo, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
+  if (a.grid) k_geodesic<true><<<grid_for(c, c->occ_geo_occ, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
+  else k_geodesic<false><<<grid_for(c, c->occ_geo, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
   span_end(c, s, st);
   c->stats.n_launches++;
   CK(cudaGetLastError());
@@ -402,6 +407,8 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   // ---- long-ray passes: rays that overflowed their slot get one of max_steps.  They run on the side stream, as
   // soon as the geodesic kernel of a batch has listed them, concurrently with the remaining bulk batches (one such
   // ray is up to 50 000 sequential steps: its latency is hidden behind the bulk work instead of trailing it). ----
+  // grid model: k_geodesic marks the steps that may cross plasma, k_transfer walks only from the first of them
+  const bool use_occ = (c->model == MODEL_GRID) && c->opt_occ;
   const size_t lslot = (size_t)(max_steps + 1) * rec_bytes;
   int long_done = 0;          // entries of d_long already handed to the side stream
   int64_t LBcap = 0;          // rays that fit the long path buffer
@@ -420,12 +427,14 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
       GeoArgs g = geo_args(c);
       g.cap = max_steps; g.base = base; g.count = cnt; g.order = c->d_long; g.pixels = d_pixels;
       g.path = c->d_path_long; g.nsteps = c->d_nsteps_long; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
+      if (use_occ) { g.grid = (const GridParams*)c->d_model; g.srange = c->d_srange; }
       int rcl = launch_geodesic(c, g, LK_LONG, cnt, c->side);
       if (rcl != IPOLE_OK) return rcl;
       RtArgs t;
       std::memset(&t, 0, sizeof t);
       t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = max_steps; t.base = base; t.count = cnt;
       t.order = c->d_long; t.path = c->d_path_long; t.nsteps = c->d_nsteps_long; t.queue = c->d_queues + (qi++);
+      if (use_occ) t.srange = c->d_srange;
       t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
       if ((rcl = launch_transfer(c, t, LK_LONG, cnt, c->side, 0, 0, sw)) != IPOLE_OK) return rcl;
     }
@@ -457,6 +466,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     g.cap = cap; g.base = base; g.count = cnt; g.order = order; g.pixels = d_pixels;
     g.path = c->d_path; g.nsteps = c->d_nsteps; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
     g.long_list = c->d_long; g.long_count = c->d_small;
+    if (use_occ) { g.grid = (const GridParams*)c->d_model; g.srange = c->d_srange; }
     if ((rc = launch_geodesic(c, g, LK_GEO, cnt, c->stream, reserve)) != IPOLE_OK) return rc;
     if (cap < max_steps) {
       CK(cudaEventRecord(c->ev_geo, c->stream));
@@ -466,6 +476,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     std::memset(&t, 0, sizeof t);
     t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = cap; t.base = base; t.count = cnt; t.order = order;
     t.path = c->d_path; t.nsteps = c->d_nsteps; t.queue = c->d_queues + (qi++);
+    if (use_occ) t.srange = c->d_srange;
     t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
     if ((rc = launch_transfer(c, t, LK_RT, cnt, c->stream, reserve, 0, sw)) != IPOLE_OK) return rc;
     c->stats.n_batches++;
@@ -501,6 +512,7 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   ipole_ctx* c = new (std::nothrow) ipole_ctx();
   if (!c) return IPOLE_ENOMEM;
   std::memset(&c->stats, 0, sizeof c->stats);
+  { const char* e = std::getenv("IPOLE_NO_OCC"); if (e && e[0] == '1') c->opt_occ = 0; }
   auto fail = [&](int code) { ipole_free(c); return code; };
   if (cudaGetDevice(&c->device) != cudaSuccess) return fail(IPOLE_ECUDA);
   cudaDeviceProp prop;
@@ -522,7 +534,8 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
     if (cudaEventCreateWithFlags(&c->ev_geo, cudaEventDisableTiming) != cudaSuccess) return fail(IPOLE_ECUDA);
     if (cudaEventCreateWithFlags(&c->ev_side, cudaEventDisableTiming) != cudaSuccess) return fail(IPOLE_ECUDA);
   }
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo, k_geodesic, IPOLE_GEO_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo, k_geodesic<false>, IPOLE_GEO_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo_occ, k_geodesic<true>, IPOLE_GEO_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_rt[MODEL_ADAF], k_transfer<MODEL_ADAF, 0>, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_rt[MODEL_SLAB], k_transfer<MODEL_SLAB, 0>, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_rt[MODEL_GRID], k_transfer<MODEL_GRID, 0>, IPOLE_RT_THREADS, 0);
@@ -871,7 +884,7 @@ int ipole_trace_pixel(ipole_ctx* c, int32_t i, int32_t j, int32_t cap, double* X
   GeoArgs g = geo_args(c);
   g.cap = max_steps; g.count = 1; g.pixels = c->d_pixels; g.path = c->d_path; g.nsteps = c->d_nsteps; g.nturn = c->d_nturn;
   g.queue = c->d_queues;
-  k_geodesic<<<1, 32, 0, c->stream>>>(g);
+  k_geodesic<false><<<1, 32, 0, c->stream>>>(g);
   CK(cudaGetLastError());
   int32_t n = 0, nt = 0;
   CK(cudaMemcpyAsync(&n, c->d_nsteps, sizeof n, cudaMemcpyDeviceToHost, c->stream));

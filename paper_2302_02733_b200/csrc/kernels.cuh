@@ -106,6 +106,9 @@ struct GeoArgs {
   int32_t* long_list; int* long_count;  // rays that did not fit (nullable)
   double* endp;               // [total rays][8], indexed by q: last point (X1..3, K0..3, 0) of the ray (nullable);
                               // all the path-free variant keeps of the backward pass
+  // grid model (k_geodesic<true>): the steps of the ray whose midpoint stencil holds plasma
+  const GridParams* grid;     // device
+  int2* srange;               // [total rays], indexed by q: (largest, smallest) such step index; (-1, 0) if none
 };
 
 __device__ __forceinline__ void pixel_ray(const CamDev& C, int64_t pix, double X[4], double K[4]) {
@@ -198,8 +201,21 @@ __device__ __forceinline__ void load_record(const double* rec, double X[4], doub
 
 // a-2, a-3, a-8.  Every lane owns one ray at a time and pulls the next one from the atomic queue as soon as its ray
 // ends, so the RK4 body runs with all lanes active whatever the step counts of neighbouring pixels are.
+//
+// OCC (grid model): every step's midpoint -- the point k_transfer evaluates the plasma at -- is tested against the
+// grid's stencil-occupancy bitmap, and the first and last step that may cross plasma are kept per ray.  k_transfer
+// then starts a ray at its first contact with plasma instead of its far end (everything before is dark vacuum and
+// changes nothing), skips the bitmap test after the last contact, and a ray that meets no plasma is not walked at all.
+template <bool OCC>
 __global__ void __launch_bounds__(IPOLE_GEO_THREADS, IPOLE_GEO_MINB) k_geodesic(const __grid_constant__ GeoArgs A) {
   const CamDev& C = A.cam;
+  __shared__ __align__(8) unsigned char grid_smem[OCC ? sizeof(GridParams) : 8];
+  if (OCC) {
+    for (int i = threadIdx.x; i < (int)sizeof(GridParams); i += blockDim.x) grid_smem[i] = ((const unsigned char*)A.grid)[i];
+    __syncthreads();
+  }
+  const GridParams& GP = *(const GridParams*)grid_smem;
+  int s_hi = -1, s_lo = 0;
   const int64_t count = A.count_dev ? (int64_t)*A.count_dev : A.count;
   const size_t slot_doubles = (size_t)(A.cap + 1) * REC_DOUBLES;
   double X[4], K[4];
@@ -224,6 +240,7 @@ __global__ void __launch_bounds__(IPOLE_GEO_THREADS, IPOLE_GEO_MINB) k_geodesic(
     pixel_ray(C, pix, X, K);
     rec = A.path ? A.path + (size_t)li * slot_doubles : nullptr;
     n = 0; nt = 0;
+    s_hi = -1; s_lo = 0;
   };
 
   const double ieps = 1.0 / A.eps;
@@ -234,8 +251,17 @@ __global__ void __launch_bounds__(IPOLE_GEO_THREADS, IPOLE_GEO_MINB) k_geodesic(
     if (rec) store_record(rec + (size_t)n * REC_DOUBLES, X, K, dl);
     const double x1_before = X[1];
     const bool k2neg = K[2] < 0.0;
+    double Xa[4];
+    if (OCC) { Xa[0] = X[0]; Xa[1] = X[1]; Xa[2] = X[2]; Xa[3] = X[3]; }
     if (small_steps) rk4_push<true>(C.G, X, K, -dl);
     else rk4_push<false>(C.G, X, K, -dl);
+    if (OCC) {
+      // the midpoint exactly as k_transfer forms it: 0.5 * (X_lo + X_hi) with lo = point n, hi = point n + 1
+      double Xm[4];
+#pragma unroll
+      for (int m = 0; m < 4; ++m) Xm[m] = 0.5 * (Xa[m] + X[m]);
+      if (grid_occupied(GP, Xm)) { if (s_hi < 0) s_lo = n; s_hi = n; }
+    }
     ++n;
     if ((K[2] < 0.0) != k2neg) ++nt;
     int status = 0;
@@ -250,6 +276,7 @@ __global__ void __launch_bounds__(IPOLE_GEO_THREADS, IPOLE_GEO_MINB) k_geodesic(
       } else {
         if (rec) store_record(rec + (size_t)n * REC_DOUBLES, X, K, 0.0);
         if (A.endp) store_record(A.endp + (size_t)q * REC_DOUBLES, X, K, 0.0);
+        if (OCC && A.srange) A.srange[q] = make_int2(s_hi, s_lo);
         A.nsteps[q] = n;
         if (A.nturn) A.nturn[q] = (nt > 127 ? 127 : nt) | (status == 3 ? 0x80 : 0);
       }
@@ -271,6 +298,7 @@ struct RtArgs {
   const int32_t* nsteps;
   unsigned long long* queue;
   double *I, *Q, *U, *V, *tau, *tauF;   // indexed by q
+  const int2* srange;         // grid model, stored path: steps that may cross plasma (from k_geodesic<true>; nullable)
   // path-free variant (PF != 0): no path; the ray restarts from the end point of its backward pass
   const double* endp;         // [total rays][8], indexed by q
   int32_t* nfwd;              // [total rays] steps of the forward pass (nullable)
@@ -350,7 +378,7 @@ k_transfer(const __grid_constant__ RtArgs A) {
   double Xhi[4], Khi[4];
   const double* rec = nullptr;
   int32_t q = 0;
-  int s = -1;
+  int s = -1, s_lo = 0;
   bool have = false, lit = false;
 
   auto fetch = [&]() {
@@ -369,8 +397,20 @@ k_transfer(const __grid_constant__ RtArgs A) {
         load_record(A.endp + (size_t)q * REC_DOUBLES, Xhi, Khi, dl);
         s = 0;   // forward steps taken
       } else {
-        const int n = A.nsteps[q];
+        int n = A.nsteps[q];
         if (n < 0) continue;  // overflowed its slot: done by the long-ray pass
+        if (MODEL == MODEL_GRID && A.srange) {
+          const int2 r = A.srange[q];
+          s_lo = r.y;
+          if (r.x < 0) {      // the ray meets no plasma: dark
+            const size_t o = SWEEP ? (size_t)mi * A.out_stride + q : (size_t)q;
+            A.I[o] = 0.0; A.Q[o] = 0.0; A.U[o] = 0.0; A.V[o] = 0.0;
+            if (A.tau) A.tau[o] = 0.0;
+            if (A.tauF) A.tauF[o] = 0.0;
+            continue;
+          }
+          n = r.x + 1;        // start at the first contact with plasma: the steps before it are dark vacuum
+        }
         rec = A.path + (size_t)li * slot_doubles;
         load_record(rec + (size_t)n * REC_DOUBLES, Xhi, Khi, dl);
         s = n - 1;
@@ -412,7 +452,7 @@ k_transfer(const __grid_constant__ RtArgs A) {
     // that is dark so far and crosses no plasma costs eight record loads and nothing else.
     bool maybe = true;
     double prim[8];
-    if (MODEL == MODEL_GRID) maybe = grid_gather(*(const GridParams*)model, Xm, prim);
+    if (MODEL == MODEL_GRID) maybe = (PF != 0 || s >= s_lo) && grid_gather(*(const GridParams*)model, Xm, prim);
     if (lit || maybe) {
       Point p; Sym7 g; Inv6 gi; double Am[4][4];
       transport_generator(C.G, Xm, Km, p, g, gi, Am);

@@ -109,6 +109,23 @@ __device__ __forceinline__ bool plasma_slab(const Geom& G, const SlabParams& M, 
 
 __device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
 
+// The first two tests of grid_gather alone (same arithmetic, so it is false only where grid_gather is false): X inside
+// the lattice in X1 and the stencil-occupancy bit set.  k_geodesic<true> marks with it the steps of a ray that may
+// cross plasma.
+__device__ __forceinline__ bool grid_occupied(const GridParams& M, const double X[4]) {
+  if (X[1] > M.lx_out + 1e-9 || X[1] < M.startx[0]) return false;
+  const double fi = (X[1] - M.startx[0]) * M.idx[0] - 0.5;
+  const double fj = (X[2] - M.startx[1]) * M.idx[1] - 0.5;
+  const double fk = (X[3] - M.startx[2]) * M.idx[2] - 0.5;
+  const double i0f = floor(fi), j0f = floor(fj), k0f = floor(fk);
+  int k0 = (int)(k0f - (double)M.N3 * floor(k0f * M.iN3));
+  if (k0 >= M.N3) k0 -= M.N3;
+  if (k0 < 0) k0 += M.N3;
+  const int ib = clampi((int)i0f + 1, 0, M.N1), jb = clampi((int)j0f + 1, 0, M.N2);
+  const size_t bit = ((size_t)ib * (M.N2 + 1) + jb) * M.N3 + k0;
+  return ((__ldg(M.occ + (bit >> 5)) >> (bit & 31)) & 1u) != 0u;
+}
+
 // FP64 trilinear interpolation of the 8 fields.  The caller's SoA planes are re-tiled at load time into cell-major
 // records of 8 doubles (64 B = two full sectors, 16-B aligned), so one corner of the stencil is two 256-bit
 // read-only loads (ld.global.nc.v4.f64) instead of eight scattered 8-byte ones, and the two k-neighbours share a

@@ -275,6 +275,26 @@ def test_grid_small_full_image(ipole, ref, small_grid):
         assert np.array_equal(img2[k], got[k])
 
 
+def test_grid_plasma_contact_range_is_bit_neutral(ipole, small_grid, monkeypatch):
+    """k_geodesic<true> marks the steps that may cross plasma and k_transfer starts at the first of them: same bits as
+    walking every step (IPOLE_NO_OCC=1), through batches and the long-ray pass too."""
+    desc, fields = small_grid
+    cam = W.camera("grid", 48, max_steps=6000)
+    monkeypatch.setenv("IPOLE_NO_OCC", "1")
+    g0 = ipole.Ipole(**cam); g0.load_grid(desc, fields)
+    monkeypatch.delenv("IPOLE_NO_OCC")
+    base = to_np(g0.make_image(maps=True)); st0 = g0.stats()
+    g = ipole.Ipole(**cam); g.load_grid(desc, fields)
+    for opts in ((0, 1), (0, 2), (24 << 20, 2), (40 << 20, 0)):
+        g.set_options(*opts)
+        img = to_np(g.make_image(maps=True)); st = g.stats()
+        for k in base:
+            assert np.array_equal(base[k], img[k]), (opts, k)
+        assert st["total_steps"] == st0["total_steps"] and st["flux_jy"] == st0["flux_jy"]
+    assert st["n_long"] == 48 * 48
+    assert (base["I"] == 0).any() and (base["I"] > 0).any()   # dark rays (never walked) and lit ones
+
+
 def test_w3_grid_256_sampled(ipole, ref):
     desc, fields = W.fm_torus_grid(288, 128, 128)
     cam = W.camera("grid", 256)
