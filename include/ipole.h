@@ -159,6 +159,25 @@ int  ipole_make_images_adaf(ipole_ctx*, int32_t n_models, const ipole_adaf_param
 typedef struct { double M_unit, Rlow, Rhigh; } ipole_grid_scales;
 int  ipole_make_images_grid(ipole_ctx*, int32_t n_models, const ipole_grid_scales* sets, const double* freq_hz,
                             double* I, double* Q, double* U, double* V, double* tau, double* tauF, double* flux_jy);
+/* Adaptive ray tracing ("another factor of 10 with adaptive ray tracing which reduces the number of light
+ * rays to follow"; the paper gives no algorithm: reading R-11 in DESIGN.md).  Dyadic lattice levels
+ * l = 0..levels of stride 2^(levels-l) (plus the last row and column): level 0 and 1 are traced everywhere; from then
+ * on a new lattice point is traced only if it lies in a cell whose already traced points differ from the bilinear
+ * interpolation of the cell's corners by more than rel_tol*|I| + abs_tol in some Stokes parameter, and is bilinearly
+ * interpolated otherwise.  The per-ray kernels are those of ipole_make_image (stored path or path-free as set).
+ * I,Q,U,V: [ny][nx], all host or all device.  state (nullable, host or device): [ny][nx] bytes, 1 = traced,
+ * 2 = interpolated.  info (nullable) is filled on return.  The call synchronises the stream once per level.
+ * IPOLE_EINVAL: NULL outputs, levels outside 1..12, negative tolerances, mixed host/device outputs. */
+typedef struct {
+  int64_t n_traced;            /* rays followed, all levels                                  */
+  int64_t n_traced_level[16];  /* per level 0..levels                                        */
+  int64_t total_steps;         /* geodesic steps of those rays                               */
+  double  flux_jy[4];          /* sums of I,Q,U,V of the finished image times the pixel solid angle, Jy */
+  float   ms_total;            /* CUDA-event time of the whole call (without the final copies to host buffers) */
+  int32_t n_launches;          /* kernels launched                                           */
+} ipole_adaptive_info;
+int  ipole_make_image_adaptive(ipole_ctx*, int32_t levels, double rel_tol, double abs_tol, double* I, double* Q, double* U,
+                               double* V, uint8_t* state, ipole_adaptive_info* info);
 /* Per-ray step count and theta-turning-point count (bit 7 set: ended on max_steps) of the last image,
  * [ny][nx] or n entries; host or device; either may be NULL. */
 int  ipole_get_ray_info(ipole_ctx*, int32_t* nsteps, int32_t* nturn);

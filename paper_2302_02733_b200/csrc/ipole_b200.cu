@@ -11,6 +11,7 @@
 #include <new>
 #include <vector>
 #include "kernels.cuh"
+#include "adaptive.cuh"
 
 using namespace ipole;
 
@@ -51,6 +52,8 @@ struct ipole_ctx {
   void* d_sweep_models = nullptr; Units* d_sweep_units = nullptr;   // model sweep: SWEEP_MAX_MODELS entries each
   double* d_sweep_out = nullptr; size_t sweep_out_doubles = 0;            // staging for host outputs of a sweep
   int occ_sweep[4] = {0, 0, 0, 0};
+  unsigned char* d_ada = nullptr; size_t ada_bytes = 0;   // adaptive ray tracing: staging planes, list, state, flags
+  cudaEvent_t ev_ada0 = nullptr, ev_ada1 = nullptr;
 
   double* d_path = nullptr; size_t path_bytes = 0;
   double* d_path_long = nullptr; size_t path_long_bytes = 0;   // slots of max_steps for the long-ray passes
@@ -741,7 +744,9 @@ int make_images(ipole_ctx* c, int model, int32_t n_models, const void* lane_tab,
   // the fluxes live at the start of the staging buffer; host outputs are staged behind them
   const size_t need = (size_t)n_models * 4 + (dev ? 0 : plane * 6);
   if (need > c->sweep_out_doubles) {
-    cudaFree(c->d_sweep_out); c->d_sweep_out = nullptr; c->sweep_out_doubles = 0;
+    cudaFree(c->d_sweep_out); cudaFree(c->d_ada);
+  if (c->ev_ada0) cudaEventDestroy(c->ev_ada0);
+  if (c->ev_ada1) cudaEventDestroy(c->ev_ada1); c->d_sweep_out = nullptr; c->sweep_out_doubles = 0;
     cudaError_t e = cudaMalloc(&c->d_sweep_out, need * sizeof(double));
     if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
     c->sweep_out_doubles = need;
@@ -817,6 +822,97 @@ int ipole_make_images_grid(ipole_ctx* c, int32_t n_models, const ipole_grid_scal
     gs[m].Rlow = sets[m].Rlow; gs[m].Rhigh = sets[m].Rhigh;
   }
   return make_images(c, MODEL_GRID, n_models, gs.data(), sizeof(GridScales), um.data(), I, Q, U, V, tau, tauF, flux_jy);
+}
+
+int ipole_make_image_adaptive(ipole_ctx* c, int32_t levels, double rel_tol, double abs_tol, double* I, double* Q, double* U,
+                              double* V, uint8_t* state, ipole_adaptive_info* info) {
+  if (!c || !I || !Q || !U || !V) return IPOLE_EINVAL;
+  if (levels < 1 || levels > 12 || !(rel_tol >= 0.0) || !(abs_tol >= 0.0)) return IPOLE_EINVAL;
+  if (c->model == MODEL_NONE) return IPOLE_ENOMODEL;
+  const int nx = c->cam.nx, ny = c->cam.ny;
+  const int64_t n = (int64_t)nx * ny;
+  const bool dev = is_device_ptr(I);
+  const void* outs[] = {Q, U, V};
+  for (const void* p : outs) if (is_device_ptr(p) != dev) return IPOLE_EINVAL;
+  int rc;
+  if ((rc = ensure_rays(c, n)) != IPOLE_OK) return rc;
+  const size_t need = (size_t)n * (4 * sizeof(double) + sizeof(int64_t) + 3);
+  if (need > c->ada_bytes) {
+    cudaFree(c->d_ada); c->d_ada = nullptr; c->ada_bytes = 0;
+    cudaError_t e = cudaMalloc(&c->d_ada, need);
+    if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
+    c->ada_bytes = need;
+  }
+  if (!c->ev_ada0) { CK(cudaEventCreate(&c->ev_ada0)); CK(cudaEventCreate(&c->ev_ada1)); }
+  double* stage = (double*)c->d_ada;
+  int64_t* list = (int64_t*)(stage + 4 * n);
+  uint8_t* st8 = (uint8_t*)(list + n);
+  uint8_t* flag_a = st8 + n;
+  uint8_t* flag_b = flag_a + n;
+  AdaArgs A;
+  std::memset(&A, 0, sizeof A);
+  A.nx = nx; A.ny = ny; A.rel_tol = rel_tol; A.abs_tol = abs_tol;
+  double* host_out[4] = {I, Q, U, V};
+  for (int k = 0; k < 4; ++k) A.img[k] = dev ? host_out[k] : stage + (size_t)k * n;
+  A.state = st8; A.list = list; A.count = c->d_small + 2;
+  // values of the traced list entries: the ordinary staging planes of the context (ray-indexed)
+  double* val[4];
+  for (int k = 0; k < 4; ++k) { val[k] = c->d_out + (size_t)k * c->ray_cap; A.val[k] = val[k]; }
+  const int gb = (int)std::min<int64_t>((n + 255) / 256, (int64_t)c->n_sm * 8);
+  ipole_adaptive_info inf;
+  std::memset(&inf, 0, sizeof inf);
+  CK(cudaEventRecord(c->ev_ada0, c->stream));
+  int launches = 0;
+  for (int l = 0; l <= levels; ++l) {
+    A.s = 1 << (levels - l);
+    uint8_t* fprev = (l & 1) ? flag_a : flag_b;   // written at level l-1
+    uint8_t* fcur = (l & 1) ? flag_b : flag_a;
+    A.flag_prev = fprev; A.flag_cur = fcur;
+    CK(cudaMemsetAsync(A.count, 0, sizeof(int), c->stream));
+    if (l == 0) k_ada_level0<<<gb, 256, 0, c->stream>>>(A, fcur);
+    else k_ada_select<<<gb, 256, 0, c->stream>>>(A);
+    ++launches;
+    CK(cudaGetLastError());
+    int cnt = 0;
+    CK(cudaMemcpyAsync(&cnt, A.count, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    if (cnt > 0) {
+      // the per-ray kernels, unchanged, on the listed pixels (run_rays resets the queues; its own d_small[0..1] only)
+      if ((rc = run_rays(c, cnt, list, val[0], val[1], val[2], val[3], nullptr, nullptr)) != IPOLE_OK) return rc;
+      launches += c->stats.n_launches;
+      ReduceOut r;
+      CK(cudaMemcpyAsync(&r, c->d_red, sizeof r, cudaMemcpyDeviceToHost, c->stream));
+      k_ada_scatter<<<(int)std::min<int64_t>((cnt + 255) / 256, (int64_t)c->n_sm * 8), 256, 0, c->stream>>>(A, cnt);
+      ++launches;
+      CK(cudaGetLastError());
+      CK(cudaStreamSynchronize(c->stream));
+      inf.total_steps += r.total_steps;
+    }
+    inf.n_traced_level[l] = cnt;
+    inf.n_traced += cnt;
+    if (l >= 1 && l < levels) {
+      CK(cudaMemsetAsync(fcur, 0, (size_t)n, c->stream));
+      k_ada_flag<<<gb, 256, 0, c->stream>>>(A);
+      ++launches;
+      CK(cudaGetLastError());
+    }
+  }
+  const double pix_rad = c->cam.pix * c->units.L_unit / c->units.D_cm;
+  k_reduce_models<<<1, 256, 0, c->stream>>>(n, (size_t)n, A.img[0], A.img[1], A.img[2], A.img[3], pix_rad * pix_rad * 1e23,
+                                            (double*)c->d_part);
+  ++launches;
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(inf.flux_jy, c->d_part, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaEventRecord(c->ev_ada1, c->stream));
+  if (!dev)
+    for (int k = 0; k < 4; ++k) CK(cudaMemcpyAsync(host_out[k], A.img[k], (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  if (state) CK(cudaMemcpyAsync(state, st8, (size_t)n, cudaMemcpyDefault, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  CK(cudaEventElapsedTime(&inf.ms_total, c->ev_ada0, c->ev_ada1));
+  inf.n_launches = launches;
+  c->have_image = false;   // ipole_get_stats / ipole_get_ray_info describe whole-image calls only
+  if (info) *info = inf;
+  return IPOLE_OK;
 }
 
 int ipole_make_image(ipole_ctx* c, double* I, double* Q, double* U, double* V, double* tau, double* tauF) {
@@ -994,7 +1090,9 @@ void ipole_free(ipole_ctx* c) {
   cudaFree(c->d_cam); cudaFree(c->d_model); cudaFree(c->d_grid); cudaFree(c->d_path);
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long);
   cudaFree(c->d_out); cudaFree(c->d_pixels); cudaFree(c->d_probe); cudaFree(c->d_queues); cudaFree(c->d_hist);
-  cudaFree(c->d_small); cudaFree(c->d_part); cudaFree(c->d_red); cudaFree(c->d_endp); cudaFree(c->d_sum); cudaFree(c->d_sweep_models); cudaFree(c->d_sweep_units); cudaFree(c->d_sweep_out);
+  cudaFree(c->d_small); cudaFree(c->d_part); cudaFree(c->d_red); cudaFree(c->d_endp); cudaFree(c->d_sum); cudaFree(c->d_sweep_models); cudaFree(c->d_sweep_units); cudaFree(c->d_sweep_out); cudaFree(c->d_ada);
+  if (c->ev_ada0) cudaEventDestroy(c->ev_ada0);
+  if (c->ev_ada1) cudaEventDestroy(c->ev_ada1);
   for (auto& s : c->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
   cudaGetLastError();
   delete c;

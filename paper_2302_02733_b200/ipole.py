@@ -18,7 +18,7 @@ OK, EINVAL, ENOMODEL, ENOMEM, ECUDA, ENOIMAGE = 0, -1, -2, -3, -4, -5
 
 #: every symbol include/ipole.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_options", "ipole_set_path_free", "ipole_load_model_adaf",
-           "ipole_load_model_slab", "ipole_load_model_grid", "ipole_make_image", "ipole_make_pixels", "ipole_make_images_adaf", "ipole_make_images_grid",
+           "ipole_load_model_slab", "ipole_load_model_grid", "ipole_make_image", "ipole_make_pixels", "ipole_make_images_adaf", "ipole_make_images_grid", "ipole_make_image_adaptive",
            "ipole_get_ray_info", "ipole_get_stats", "ipole_get_camera_tetrad", "ipole_trace_pixel",
            "ipole_eval_connection", "ipole_eval_coefficients", "ipole_eval_stokes_step", "ipole_eval_bessel",
            "ipole_eval_plasma", "ipole_eval_math", "ipole_measure_fp64_peak", "ipole_last_cuda_error", "ipole_free", "ipole_strerror",
@@ -60,6 +60,11 @@ class GridScales(C.Structure):
     _fields_ = [("M_unit", C.c_double), ("Rlow", C.c_double), ("Rhigh", C.c_double)]
 
 
+class AdaptiveInfo(C.Structure):
+    _fields_ = [("n_traced", C.c_int64), ("n_traced_level", C.c_int64 * 16), ("total_steps", C.c_int64),
+                ("flux_jy", C.c_double * 4), ("ms_total", C.c_float), ("n_launches", C.c_int32)]
+
+
 class IpoleError(RuntimeError):
     def __init__(self, code, what):
         self.code = code
@@ -86,6 +91,7 @@ def lib():
         L.ipole_make_image.argtypes = [vp] + [vp] * 6
         L.ipole_make_pixels.argtypes = [vp, C.c_int64, vp] + [vp] * 8
         L.ipole_make_images_adaf.argtypes = [vp, C.c_int32, C.POINTER(AdafParams), vp] + [vp] * 7
+        L.ipole_make_image_adaptive.argtypes = [vp, C.c_int32, C.c_double, C.c_double, vp, vp, vp, vp, vp, C.POINTER(AdaptiveInfo)]
         L.ipole_make_images_grid.argtypes = [vp, C.c_int32, C.POINTER(GridScales), vp] + [vp] * 7
         L.ipole_get_ray_info.argtypes = [vp, vp, vp]
         L.ipole_get_stats.argtypes = [vp, C.POINTER(Stats)]
@@ -259,6 +265,27 @@ class Ipole:
         out = dict(out)
         out["flux_jy"] = flux
         return out
+
+    def make_image_adaptive(self, levels=3, rel_tol=1e-2, abs_tol=0.0, out=None, host=False):
+        """Adaptive ray tracing (include/ipole.h ipole_make_image_adaptive).  Returns (dict of I,Q,U,V
+        [ny, nx] and "state" uint8 [ny, nx]: 1 traced, 2 interpolated; info dict)."""
+        names = ["I", "Q", "U", "V"]
+        if out is None:
+            if host:
+                out = {k: np.empty((self.ny, self.nx), dtype=np.float64) for k in names}
+            else:
+                import torch
+                out = {k: torch.empty((self.ny, self.nx), dtype=torch.float64, device="cuda") for k in names}
+        state = np.zeros((self.ny, self.nx), dtype=np.uint8)
+        info = AdaptiveInfo()
+        _chk(lib().ipole_make_image_adaptive(self._h, int(levels), float(rel_tol), float(abs_tol), *[_ptr(out[k]) for k in names],
+                                             _ptr(state), C.byref(info)), "ipole_make_image_adaptive")
+        out = dict(out)
+        out["state"] = state
+        d = dict(n_traced=info.n_traced, n_traced_level=[info.n_traced_level[i] for i in range(levels + 1)],
+                 total_steps=info.total_steps, flux_jy=[info.flux_jy[i] for i in range(4)], ms_total=info.ms_total,
+                 n_launches=info.n_launches)
+        return out, d
 
     def make_pixels(self, pixels):
         """Stokes, maps and ray info for a list of flat pixel indices j*nx+i (host numpy in, host numpy out)."""
