@@ -244,6 +244,71 @@ def oracle_sample(workload, n_rays, nthreads, path_free=False):
     return pix.size, r.total_steps(), dt, stride
 
 
+def run_adaptive(args, g, replicas, wl, cam, world, rank, local, barrier):
+    """One step = one ipole_make_image_adaptive call; the full image of the same workload is made once for the error."""
+    import torch
+    n = wl["n"]
+    names = ["I", "Q", "U", "V"]
+    full = g.make_image()
+    st_full = g.stats()
+    peak = float(full["I"].max())
+    rel, ab = 0.02, 1e-3 * peak
+    out = {k: torch.empty((n, n), dtype=torch.float64, device="cuda") for k in names}
+    for _ in range(args.warmup):
+        g.make_image_adaptive(args.adaptive, rel, ab, out=out)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        res, info = g.make_image_adaptive(args.adaptive, rel, ab, out=out)
+    ev1.record()
+    barrier()
+    ms = replicas.max_over_ranks(ev0.elapsed_time(ev1), "cuda")
+    clocks = sampler.stop() if rank == 0 else None
+    host = {k: torch.empty((n, n), dtype=torch.float64).pin_memory().numpy() for k in names}
+    g.make_image_adaptive(args.adaptive, rel, ab, out=host)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        g.set_camera(**cam)
+        g.make_image_adaptive(args.adaptive, rel, ab, out=host)
+    torch.cuda.synchronize()
+    dt = replicas.max_over_ranks(time.perf_counter() - t0, "cuda")
+    if rank != 0:
+        return
+    err = (out["I"] - full["I"]).abs() / peak
+    pol = torch.maximum(torch.maximum((out["Q"] - full["Q"]).abs(), (out["U"] - full["U"]).abs()), (out["V"] - full["V"]).abs()) / peak
+    pix = n * n
+    line = {"metric": "rays_per_s", "value": replicas.job_throughput(pix * args.steps, ms * 1e-3, world), "unit": "rays/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "image": "%dx%d" % (n, n), "model": wl["kind"], "freq_ghz": 230, "eps": cam["eps"],
+                       "full_stokes": True, "variant": "adaptive ray tracing (PAPER.md:70): %d lattice levels, rel_tol %.3g, "
+                                                        "abs_tol 1e-3 of the brightest pixel" % (args.adaptive, rel),
+                       "note": "value counts image PIXELS delivered per second; the rays actually followed are in `adaptive`",
+                       "l2": "no flush needed: every level streams its own path buffer", "parallelism": "single GPU"},
+            "images_per_s": world * args.steps / (ms * 1e-3),
+            "adaptive": {"rays_followed": info["n_traced"], "fraction_of_pixels": info["n_traced"] / pix,
+                         "per_level": info["n_traced_level"], "rays_followed_per_s": info["n_traced"] * args.steps / (ms * 1e-3),
+                         "geodesic_steps": info["total_steps"], "speedup_vs_full_image": st_full["ms_total"] / (ms / args.steps),
+                         "full_image_ms": st_full["ms_total"],
+                         "error_vs_full_image": {"I_max_over_peak": float(err.max()), "I_p99_over_peak": float(torch.quantile(err.flatten()[:: max(1, pix // 1000000)], 0.99)),
+                                                 "QUV_max_over_peak": float(pol.max()),
+                                                 "total_flux_rel": abs(float(out["I"].sum()) / float(full["I"].sum()) - 1)}},
+            "gpu_launches": info["n_launches"] * args.steps,
+            "roofline": {"bound": "alu", "kernel": "k_transfer<%s>" % wl["kind"], "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                         "achieved": None, "frac": None, "traffic": None,
+                         "note": "the per-ray kernels are those of the full image (see the default bench line); this line measures the ray saving"},
+            "e2e": {"value": replicas.job_throughput(pix * args.steps, dt, world), "unit": "rays/s",
+                    "h2d_bytes_per_step": 160, "d2h_bytes_per_step": 4 * pix * 8 + pix},
+            "clocks": clocks}
+    print(json.dumps(line), flush=True)
+
+
 def run_reference(args):
     """--impl reference: the oracle on the box's host cores (rank 0 only)."""
     rank = int(os.environ.get("RANK", "0"))
@@ -286,6 +351,8 @@ def main():
     ap.add_argument("--cpu-baseline-rays", type=int, default=16384)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--adaptive", type=int, default=0, metavar="LEVELS",
+                    help="adaptive ray tracing (PAPER.md:70) with this many lattice levels, rel_tol 0.02, abs_tol 1e-3 of the peak")
     ap.add_argument("--path-free", action="store_true",
                     help="the paper's own GPU design (PAPER.md:43): no stored path, forward re-integration")
     args = ap.parse_args()
@@ -331,6 +398,11 @@ def main():
     if wl.get("sweep"):
         run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier,
                   grid=(desc, fields) if wl["kind"] == "grid" else None)
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    if args.adaptive:
+        run_adaptive(args, g, replicas, wl, cam, world, rank, local, barrier)
         if world > 1:
             dist.destroy_process_group()
         return
