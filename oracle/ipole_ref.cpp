@@ -12,6 +12,7 @@
 #include "ref_plasma.hpp"
 #include "ref_transfer.hpp"
 #include "ref_pathfree.hpp"
+#include "ref_unpol.hpp"
 
 using namespace iref;
 
@@ -21,6 +22,7 @@ struct ipole_ref_ctx {
   Model model;
   std::atomic<int64_t> total_steps{0};
   int path_free = 0;   // 1: PAPER.md:43 bidirectional variant (ref_pathfree.hpp)
+  int unpolarized = 0; // 1: scalar transfer of I alone (ref_unpol.hpp); takes precedence over path_free
 };
 
 static Geom mkgeom(double a, double h, int flat) { Geom G; G.a = a; G.hslope = h; G.flat = flat; return G; }
@@ -97,7 +99,10 @@ static void one_pixel(ipole_ref_ctx* x, int64_t pix, double out[6], int32_t* nst
   cplx N[4][4];
   for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) N[a][b] = 0.0;
   double tau = 0.0, tauF = 0.0, S[4];
-  if (x->path_free) {
+  if (x->unpolarized) {
+    S[0] = transfer_unpolarized(C.geom, x->model, x->units, path, &tau);
+    S[1] = S[2] = S[3] = 0.0;
+  } else if (x->path_free) {
     const int n = (int)path.dl.size();
     double Xend[4];
     transfer_path_free(C, x->model, x->units, path.X[n].data(), path.K[n].data(), N, &tau, &tauF, Xend);
@@ -149,6 +154,12 @@ int ipole_ref_make_pixels(ipole_ref_ctx* x, int64_t n, const int64_t* pixels, in
 }
 
 void ipole_ref_free(ipole_ref_ctx* x) { delete x; }
+
+int ipole_ref_set_unpolarized(ipole_ref_ctx* x, int on) {
+  if (!x) return -1;
+  x->unpolarized = on ? 1 : 0;
+  return 0;
+}
 
 int ipole_ref_set_path_free(ipole_ref_ctx* x, int on) {
   if (!x) return -1;

@@ -66,6 +66,9 @@ void ipole_ref_free(ipole_ref_ctx*);
  * Stokes are read in the observer tetrad at the forward end point.  nsteps/nturn stay those of the backward pass.
  * Pins PF1-PF5 (tests/test_oracle_pathfree.py). */
 int  ipole_ref_set_path_free(ipole_ref_ctx*, int on);
+/* Unpolarized transfer ("nonpolarized images"; reading R-12 in ref_unpol.hpp): make_pixels solves the
+ * scalar equation for I alone on the stored path; Q = U = V = 0, tauF = 0.  Pins U1-U3 (tests/test_oracle_unpol.py). */
+int  ipole_ref_set_unpolarized(ipole_ref_ctx*, int on);
 /* The forward pass alone, from (Xn, Kn): returns its step count n, points 0..n (0 = far end) and the n step sizes;
  * -(needed) if cap is too small. */
 int  ipole_ref_retrace(ipole_ref_ctx*, const double Xn[4], const double Kn[4], int cap,

@@ -77,6 +77,7 @@ def lib():
         L.ipole_ref_plasma_tetrad.argtypes = [C.c_void_p, dp, dp, dp, dp, dp, dp]
         L.ipole_ref_transport_vacuum.argtypes = [C.c_void_p, C.c_int, dp, dp, dp, dp]
         L.ipole_ref_set_path_free.argtypes = [C.c_void_p, C.c_int]
+        L.ipole_ref_set_unpolarized.argtypes = [C.c_void_p, C.c_int]
         L.ipole_ref_retrace.argtypes = [C.c_void_p, dp, dp, C.c_int, dp, dp, dp]
         L.ipole_ref_observer_tetrad.argtypes = [C.c_void_p, dp, dp]
         L.ipole_ref_total_steps.argtypes = [C.c_void_p]
@@ -226,6 +227,12 @@ class Ctx:
         rc = lib().ipole_ref_set_path_free(self._h, 1 if on else 0)
         if rc != 0:
             raise RuntimeError("set_path_free failed: %d" % rc)
+
+    def set_unpolarized(self, on=True):
+        """Scalar transfer of I alone (oracle/ref_unpol.hpp)."""
+        rc = lib().ipole_ref_set_unpolarized(self._h, 1 if on else 0)
+        if rc != 0:
+            raise RuntimeError("set_unpolarized failed: %d" % rc)
 
     def retrace(self, Xn, Kn, cap=60000):
         """Forward pass of the path-free variant from the far end (Xn, Kn): points 0..n (0 = far end), n step sizes."""
