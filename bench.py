@@ -29,6 +29,8 @@ if ROOT not in sys.path:
 FLOP_PER_STEP = {"transfer_adaf": 1663.0, "transfer_grid": 404.0, "geodesic_adaf": 994.0, "geodesic_grid": 1169.0}
 # DRAM bytes per step of k_transfer (dram__bytes_read + write of one launch / its thread-steps, same captures)
 DRAM_BYTES_PER_STEP = {"transfer_adaf": 64.2, "transfer_grid": 69.6}
+# --unpolarized: per step of k_transfer_unpol<model> (ncu, profiles/r1_unpolarized.md)
+FLOP_PER_STEP_UNPOL = {"transfer_adaf": None, "transfer_grid": None}
 # --path-free (PAPER.md:43 variant): per FORWARD step of k_transfer<model, 1> (RK4 push + transfer step in one kernel)
 FLOP_PER_STEP_PF = {"transfer_adaf": 2656.0, "transfer_grid": 1589.0}
 DRAM_BYTES_PER_STEP_PF = {"transfer_adaf": 0.1, "transfer_grid": 0.9}
@@ -125,12 +127,14 @@ def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier,
     rt_ms, steps_rt = st["ms_transfer"], st["total_steps"] * M
     dfma_tf, _ = g.fp64_peak()
     fkey = "transfer_" + wl["kind"]
-    ach = FLOP_PER_STEP[fkey] * steps_rt / (rt_ms * 1e-3) / 1e12
+    fl_step = (FLOP_PER_STEP_UNPOL[fkey] or 0.0) if args.unpolarized else FLOP_PER_STEP[fkey]
+    ach = fl_step * steps_rt / (rt_ms * 1e-3) / 1e12
     line = {"metric": "rays_per_s", "value": value, "unit": "rays/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.workload, "image": "%dx%d" % (n, n), "models_per_call": M, "model": wl["kind"],
-                       "freq_ghz": 230, "eps": cam["eps"], "full_stokes": True,
+                       "freq_ghz": 230, "eps": cam["eps"], "full_stokes": not args.unpolarized,
+                       "variant": "unpolarized, I alone (PAPER.md:74)" if args.unpolarized else "full Stokes",
                        "note": "a ray here is one (pixel, parameter set) pair; the %d geodesics are integrated once per call" % (n * n),
                        "l2": "each call streams %.2f GB of path records once per warp (>> 126 MB L2)" % (st["total_steps"] * 64 / 1e9),
                        "parallelism": "single GPU" if world == 1 else "one replica per GPU"},
@@ -141,7 +145,7 @@ def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier,
             "gpu_launches": st["n_launches"] * args.steps,
             "roofline": {"bound": "alu", "kernel": "k_transfer<%s, sweep>" % wl["kind"], "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                          "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz; DFMA micro-benchmark on this GPU: %.1f" % dfma_tf,
-                         "achieved": ach, "frac": ach / FP64_PEAK_TFLOPS, "flop_per_step": FLOP_PER_STEP[fkey],
+                         "achieved": ach, "frac": ach / FP64_PEAK_TFLOPS, "flop_per_step": fl_step,
                          "flop_note": "flop per step of the single-image kernel (the sweep runs the same arithmetic per pair)",
                          "avg_launch_ms": rt_ms, "kernel_share_of_step": rt_ms / st["ms_total"], "traffic": None},
             "e2e": {"value": replicas.job_throughput(rays * args.steps, dt, world), "unit": "rays/s",
@@ -153,6 +157,8 @@ def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier,
         from oracle import ipole_ref
         cores = os.cpu_count() or 1
         r = ipole_ref.Ctx(**cam)
+        if args.unpolarized:
+            r.set_unpolarized(True)
         def ref_load(mod):
             if is_grid:
                 d = dict(grid[0]); d.update(mod); r.load_grid(d, grid[1])
@@ -219,7 +225,7 @@ class ClockSampler:
                 "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_sample(workload, n_rays, nthreads, path_free=False):
+def oracle_sample(workload, n_rays, nthreads, path_free=False, unpolarized=False):
     """The CPU oracle, as it stands, on a strided sample of the workload's image.  Returns (rays, steps, seconds)."""
     import numpy as np
     from oracle import ipole_ref
@@ -234,6 +240,8 @@ def oracle_sample(workload, n_rays, nthreads, path_free=False):
         r.load_grid(desc, fields)
     if path_free:
         r.set_path_free(True)
+    if unpolarized:
+        r.set_unpolarized(True)
     n = wl["n"]
     stride = max(1, int(round(n / max(1.0, n_rays ** 0.5))))
     ii, jj = np.meshgrid(np.arange(stride // 2, n, stride), np.arange(stride // 2, n, stride))
@@ -353,6 +361,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--adaptive", type=int, default=0, metavar="LEVELS",
                     help="adaptive ray tracing (PAPER.md:70) with this many lattice levels, rel_tol 0.02, abs_tol 1e-3 of the peak")
+    ap.add_argument("--unpolarized", action="store_true", help="I alone (PAPER.md:74 'nonpolarized images')")
     ap.add_argument("--path-free", action="store_true",
                     help="the paper's own GPU design (PAPER.md:43): no stored path, forward re-integration")
     args = ap.parse_args()
@@ -383,6 +392,8 @@ def main():
     g.set_stream(torch.cuda.current_stream())
     if args.path_free:
         g.set_path_free(True)
+    if args.unpolarized:
+        g.set_unpolarized(True)
     grid_bytes = 0
     if wl["kind"] == "adaf":
         g.load_adaf(**W.ADAF)
@@ -467,12 +478,15 @@ def main():
     key = "transfer_" + wl["kind"]
     pf = args.path_free
     fl_rt = FLOP_PER_STEP_PF[key] if pf else FLOP_PER_STEP[key]
+    if args.unpolarized:
+        fl_rt = FLOP_PER_STEP_UNPOL[key] or 0.0
     rt_steps = st["total_steps_forward"] if pf else st["total_steps"]   # steps the transfer kernel walks
     dram_rt = DRAM_BYTES_PER_STEP_PF[key] if pf else DRAM_BYTES_PER_STEP[key]
     dfma_tf, _ = g.fp64_peak()
     n_rt = max(1, st["n_batches"])          # bulk launches; the long-ray passes run beside them on a side stream
     rt_ms = st["ms_transfer"]
-    roof = {"bound": "alu", "kernel": "k_transfer<%s%s>" % (wl["kind"], ", path-free" if pf else ""), "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+    roof = {"bound": "alu", "kernel": ("k_transfer_unpol<%s>" % wl["kind"]) if args.unpolarized else
+            "k_transfer<%s%s>" % (wl["kind"], ", path-free" if pf else ""), "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
             "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz; DFMA micro-benchmark on this GPU: %.1f" % dfma_tf,
             "launches": n_rt, "avg_launch_ms": rt_ms / n_rt, "kernel_share_of_step": rt_ms / st["ms_total"],
             "steps_per_launch": rt_steps / n_rt,
@@ -494,8 +508,10 @@ def main():
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.workload, "configs_index": wl["config"], "image": "%dx%d" % (wl["n"], wl["n"]),
-                       "model": wl["kind"], "freq_ghz": 230, "eps": cam["eps"], "full_stokes": True, "maps": maps,
-                       "variant": "path-free bidirectional (PAPER.md:43)" if pf else "stored path",
+                       "model": wl["kind"], "freq_ghz": 230, "eps": cam["eps"], "maps": maps,
+                       "variant": "unpolarized, I alone (PAPER.md:74), stored path" if args.unpolarized else
+                                  "path-free bidirectional (PAPER.md:43)" if pf else "stored path",
+                       "full_stokes": not args.unpolarized,
                        "l2": ("no flush needed: nothing is re-read; per image %.2f GB of end points and outputs stream once"
                               % (rays * (64.0 + 8.0 * len(names)) / 1e9)) if pf else
                              "no flush needed: every batch streams a %.1f GB path buffer (>> 126 MB L2)"
@@ -513,7 +529,7 @@ def main():
 
     if not args.no_cpu_baseline and world == 1:
         cores = os.cpu_count() or 1
-        n, steps, dt, stride = oracle_sample(args.workload, args.cpu_baseline_rays, cores, path_free=pf)
+        n, steps, dt, stride = oracle_sample(args.workload, args.cpu_baseline_rays, cores, path_free=pf, unpolarized=args.unpolarized)
         line["cpu_baseline"] = {"value": n / dt, "unit": "rays/s", "cores": cores, "kind": "oracle",
                                 "sample": "%d rays: every %d-th pixel in x and y of the %dx%d image, %.1f s"
                                           % (n, stride, wl["n"], wl["n"], dt),

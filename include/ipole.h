@@ -122,6 +122,15 @@ int  ipole_set_options(ipole_ctx*, uint64_t path_bytes, int32_t sort_rays);
  * from the stored-path one at the level the integrator is not time-reversible (paper: "negligible").
  * on == 0 (default): stored path.  Returns IPOLE_EINVAL for a NULL context. */
 int  ipole_set_path_free(ipole_ctx*, int32_t on);
+/* Unpolarized transfer (the model-fitting loop makes "nonpolarized images"; polarized
+ * transfer is "far more complex and computationally demanding"; reading R-12 in DESIGN.md).  on != 0: every image
+ * entry (ipole_make_image, _pixels, _images_adaf, _images_grid, _image_adaptive) solves the scalar equation
+ * d(I/nu^3)/dlambda = j_I/nu^2 - alpha_I nu (I/nu^3) exactly per step on the stored path, with the same midpoints,
+ * plasma state, frequency, pitch angle and thermal synchrotron j_I, alpha_I as the polarized path; no tetrad, no
+ * parallel transport, no Faraday coefficients.  I is written, Q = U = V = 0, tau as usual, tauF = 0.  This is not
+ * Stokes I of the polarized solution (alpha_Q, alpha_V couple I to Q and V there).  Takes precedence over
+ * ipole_set_path_free.  Returns IPOLE_EINVAL for a NULL context. */
+int  ipole_set_unpolarized(ipole_ctx*, int32_t on);
 
 int  ipole_load_model_adaf(ipole_ctx*, const ipole_adaf_params*);
 int  ipole_load_model_slab(ipole_ctx*, const ipole_slab_params*);

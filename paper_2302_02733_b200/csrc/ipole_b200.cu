@@ -47,6 +47,8 @@ struct ipole_ctx {
   int opt_path_free = 0;         // PAPER.md:43 bidirectional variant
   int opt_occ = 1;               // grid model: plasma-contact range per ray (IPOLE_NO_OCC=1 in the environment turns it off)
   int last_pf = 0;               // the last image was made path-free
+  int opt_unpol = 0;             // unpolarized transfer of I alone
+  int occ_unpol[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};
   double* d_endp = nullptr; int64_t endp_cap = 0;   // end points of the backward passes, [rays][8]
   long long* d_sum = nullptr;    // forward-step total of the path-free variant
   void* d_sweep_models = nullptr; Units* d_sweep_units = nullptr;   // model sweep: SWEEP_MAX_MODELS entries each
@@ -233,6 +235,17 @@ void launch_transfer_model(int model, int g, cudaStream_t st, const RtArgs& a) {
 // pf: 0 stored path, 1 path-free with eps <= 0.04, 2 path-free with any eps
 int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_t st, int reserve = 0, int pf = 0,
                     const Sweep* sw = nullptr) {
+  if (c->opt_unpol && !sw) {
+    const int s = span_begin(c, kind, st);
+    const int g = grid_for(c, c->occ_unpol[c->model][0], IPOLE_RT_THREADS, rays, reserve);
+    if (c->model == MODEL_ADAF) k_transfer_unpol<MODEL_ADAF, false><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
+    else if (c->model == MODEL_SLAB) k_transfer_unpol<MODEL_SLAB, false><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
+    else k_transfer_unpol<MODEL_GRID, false><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
+    span_end(c, s, st);
+    c->stats.n_launches++;
+    CK(cudaGetLastError());
+    return IPOLE_OK;
+  }
   if (sw) {
     // chunks of SWEEP_MAX_MODELS parameter sets; the parameter tables are re-sent per chunk on the launching stream
     // (stream order keeps a table alive until the kernel that reads it has finished)
@@ -250,8 +263,11 @@ int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_
       t.tau = planes[4] ? planes[4] + (size_t)m0 * sw->out_stride : nullptr;
       t.tauF = planes[5] ? planes[5] + (size_t)m0 * sw->out_stride : nullptr;
       CK(cudaMemsetAsync(t.queue, 0, sizeof(unsigned long long), st));
-      const int g = grid_for(c, c->occ_sweep[c->model], IPOLE_RT_THREADS, rays * mc, reserve);
-      if (c->model == MODEL_ADAF) k_transfer<MODEL_ADAF, 0, true><<<g, IPOLE_RT_THREADS, 0, st>>>(t);
+      const int g = grid_for(c, c->opt_unpol ? c->occ_unpol[c->model][1] : c->occ_sweep[c->model], IPOLE_RT_THREADS, rays * mc, reserve);
+      if (c->opt_unpol) {
+        if (c->model == MODEL_ADAF) k_transfer_unpol<MODEL_ADAF, true><<<g, IPOLE_RT_THREADS, 0, st>>>(t);
+        else k_transfer_unpol<MODEL_GRID, true><<<g, IPOLE_RT_THREADS, 0, st>>>(t);
+      } else if (c->model == MODEL_ADAF) k_transfer<MODEL_ADAF, 0, true><<<g, IPOLE_RT_THREADS, 0, st>>>(t);
       else k_transfer<MODEL_GRID, 0, true><<<g, IPOLE_RT_THREADS, 0, st>>>(t);
       span_end(c, s, st);
       c->stats.n_launches++;
@@ -374,7 +390,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     const int64_t per = (int64_t)(budget / rec_bytes / (size_t)n) - 1;
     cap = (int)std::max<int64_t>(64, std::min<int64_t>(max_steps, per));
   }
-  if (c->opt_path_free && !sw) {
+  if (c->opt_path_free && !sw && !c->opt_unpol) {
     // ---- path-free bidirectional variant: one geodesic launch that keeps the end points, one
     // transfer launch that re-integrates forward.  Rays are ordered longest first, so the few very long rays start
     // at once and run beside the bulk. ----
@@ -553,6 +569,11 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   if (cudaMalloc(&c->d_sweep_models, SWEEP_MAX_MODELS * std::max(sizeof(AdafParams), sizeof(GridScales))) != cudaSuccess) return fail(IPOLE_ENOMEM);
   if (cudaMalloc(&c->d_sweep_units, SWEEP_MAX_MODELS * sizeof(Units)) != cudaSuccess) return fail(IPOLE_ENOMEM);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_sweep[MODEL_ADAF], k_transfer<MODEL_ADAF, 0, true>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_unpol[MODEL_ADAF][0], k_transfer_unpol<MODEL_ADAF, false>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_unpol[MODEL_SLAB][0], k_transfer_unpol<MODEL_SLAB, false>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_unpol[MODEL_GRID][0], k_transfer_unpol<MODEL_GRID, false>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_unpol[MODEL_ADAF][1], k_transfer_unpol<MODEL_ADAF, true>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_unpol[MODEL_GRID][1], k_transfer_unpol<MODEL_GRID, true>, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_sweep[MODEL_GRID], k_transfer<MODEL_GRID, 0, true>, IPOLE_RT_THREADS, 0);
   rc = apply_camera(c, cam);
   if (rc != IPOLE_OK) return fail(rc);
@@ -589,6 +610,12 @@ int ipole_set_options(ipole_ctx* c, uint64_t path_bytes, int32_t sort_rays) {
   if (!c) return IPOLE_EINVAL;
   c->opt_path_bytes = path_bytes;
   c->opt_sort = (sort_rays == 2) ? 2 : (sort_rays ? 1 : 0);
+  return IPOLE_OK;
+}
+
+int ipole_set_unpolarized(ipole_ctx* c, int32_t on) {
+  if (!c) return IPOLE_EINVAL;
+  c->opt_unpol = on ? 1 : 0;
   return IPOLE_OK;
 }
 

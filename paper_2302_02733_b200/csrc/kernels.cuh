@@ -498,6 +498,129 @@ k_transfer(const __grid_constant__ RtArgs A) {
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// Unpolarized transfer ("nonpolarized images" of the model-fitting loop; R-12): I alone on the
+// stored path.  Per step: midpoint, metric (no derivatives, no transport), plasma state, nu = -k.u nu_obs, pitch
+// angle, thermal synchrotron j_I and alpha_I, exact scalar step  I <- I e^{-x} + j ds (1 - e^{-x})/x,  x = alpha ds.
+// Work items and refill as in k_transfer (SWEEP: (ray, parameter set) pairs, the lanes of a warp share a ray).
+template <int MODEL, bool SWEEP>
+__global__ void __launch_bounds__(IPOLE_RT_THREADS, (MODEL == MODEL_GRID) ? 3 : 4) k_transfer_unpol(const __grid_constant__ RtArgs A) {
+  static_assert(!SWEEP || MODEL != MODEL_SLAB, "the sweep is built for the ADAF and grid models");
+  const CamDev& C = A.cam;
+  const int64_t count = (A.count_dev ? (int64_t)*A.count_dev : A.count) * (SWEEP ? A.n_models : 1);
+  const size_t slot_doubles = (size_t)(A.cap + 1) * REC_DOUBLES;
+  constexpr int MODEL_BYTES = MODEL == MODEL_ADAF ? sizeof(AdafParams) : (MODEL == MODEL_SLAB ? sizeof(SlabParams) : sizeof(GridParams));
+  constexpr int LANE_BYTES = MODEL == MODEL_ADAF ? sizeof(AdafParams) : sizeof(GridScales);
+  __shared__ __align__(8) unsigned char model_smem[MODEL_BYTES];
+  __shared__ __align__(8) unsigned char lane_smem[SWEEP ? LANE_BYTES * SWEEP_MAX_MODELS : 8];
+  __shared__ Units units_smem[SWEEP ? SWEEP_MAX_MODELS : 1];
+  {
+    for (int i = threadIdx.x; i < MODEL_BYTES; i += blockDim.x) model_smem[i] = ((const unsigned char*)A.model)[i];
+    if (SWEEP) {
+      for (int i = threadIdx.x; i < LANE_BYTES * A.n_models; i += blockDim.x) lane_smem[i] = ((const unsigned char*)A.lane_tab)[i];
+      for (int i = threadIdx.x; i < A.n_models; i += blockDim.x) units_smem[i] = A.units_arr[i];
+    }
+    __syncthreads();
+  }
+  const void* model = model_smem;
+  const void* lane = nullptr;
+  int mi = 0;
+  double I = 0.0, tau = 0.0;
+  double Xhi[4], Khi[4];
+  const double* rec = nullptr;
+  int32_t q = 0;
+  int s = -1, s_lo = 0;
+  bool have = false;
+
+  auto finish = [&]() {
+    const double nu_o = SWEEP ? units_smem[mi].nu_obs : A.units.nu_obs;
+    const size_t o = SWEEP ? (size_t)mi * A.out_stride + q : (size_t)q;
+    A.I[o] = I * (nu_o * nu_o * nu_o); A.Q[o] = 0.0; A.U[o] = 0.0; A.V[o] = 0.0;
+    if (A.tau) A.tau[o] = tau;
+    if (A.tauF) A.tauF[o] = 0.0;
+  };
+  auto fetch = [&]() {
+    for (;;) {
+      int64_t li = (int64_t)atomicAdd(A.queue, 1ULL);
+      have = li < count;
+      if (!have) return;
+      if (SWEEP) { mi = (int)(li % A.n_models); li /= A.n_models; lane = lane_smem + (size_t)mi * LANE_BYTES; }
+      q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
+      int n = A.nsteps[q];
+      if (n < 0) continue;   // overflowed its slot: done by the long-ray pass
+      I = 0.0; tau = 0.0; s_lo = 0;
+      if (MODEL == MODEL_GRID && A.srange) {
+        const int2 r = A.srange[q];
+        if (r.x < 0) { finish(); continue; }   // the ray meets no plasma
+        n = r.x + 1; s_lo = r.y;
+      }
+      rec = A.path + (size_t)li * slot_doubles;
+      double dl;
+      load_record(rec + (size_t)n * REC_DOUBLES, Xhi, Khi, dl);
+      s = n - 1;
+      return;
+    }
+  };
+
+  fetch();
+  while (have) {
+    double Xlo[4], Klo[4], dl;
+    load_record(rec + (size_t)s * REC_DOUBLES, Xlo, Klo, dl);
+    double Xm[4], Km[4];
+#pragma unroll
+    for (int m = 0; m < 4; ++m) { Xm[m] = 0.5 * (Xlo[m] + Xhi[m]); Km[m] = 0.5 * (Klo[m] + Khi[m]); }
+    bool maybe = true;
+    double prim[8];
+    if (MODEL == MODEL_GRID) maybe = grid_gather(*(const GridParams*)model, Xm, prim);
+    if (maybe) {
+      Point p; Sym7 g; Inv6 gi;
+      metric<true>(C.G, Xm, p, g, gi);
+      Plasma P;
+      bool present;
+      if (MODEL == MODEL_ADAF) present = plasma_adaf(C.G, *(const AdafParams*)(SWEEP ? lane : model), Xm, p, g, gi, P);
+      else if (MODEL == MODEL_SLAB) present = plasma_slab(C.G, *(const SlabParams*)model, Xm, p, g, P);
+      else {
+        const GridParams& M = *(const GridParams*)model;
+        if (SWEEP) present = grid_state(C.G, M, *(const GridScales*)lane, prim, p, g, gi, P);
+        else { const GridScales S = {M.ne_unit, M.B_unit, M.Rlow, M.Rhigh}; present = grid_state(C.G, M, S, prim, p, g, gi, P); }
+      }
+      if (present) {
+        const Units& U = SWEEP ? units_smem[mi] : A.units;
+        double kcov[4];
+        g.mul(Km, kcov);
+        const double om = -dot4(kcov, P.u);
+        if (om > 0.0) {
+          const double nu = om * U.nu_obs;
+          double ji, ai;
+          if (MODEL == MODEL_SLAB) {
+            const double inu = ip_rcp(nu);
+            ji = P.j[0] * inu * inu; ai = P.al[0] * nu;
+          } else {
+            double bcov[4];
+            g.mul(P.b, bcov);
+            const double cosT = fmin(1.0, fmax(-1.0, dot4(bcov, Km) * ip_rcp(om) * ip_rcp(P.B)));
+            const Coeff c = synchrotron_invariant(P.ne, P.Th, P.B, cosT, nu);
+            ji = c.jI; ai = c.aI;
+          }
+          const double ds = dl * U.dl_unit;
+          const double x = ai * ds;
+          const double em = ip_expm1(-x);
+          const double E = (x > 0.0) ? -em * ip_rcp(x) : 1.0;
+          I = I + I * em + ji * ds * E;
+          tau += x;
+        }
+      }
+    }
+#pragma unroll
+    for (int m = 0; m < 4; ++m) { Xhi[m] = Xlo[m]; Khi[m] = Klo[m]; }
+    --s;
+    if (s < s_lo) {   // below the last step that may cross plasma nothing changes any more (s_lo = 0 without the range)
+      finish();
+      fetch();
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // a-8: order rays by predicted step count, longest first (counting sort on 4096 bins)
 constexpr int SORT_BINS = 4096;
 
