@@ -172,11 +172,12 @@ int  ipole_make_images_grid(ipole_ctx*, int32_t n_models, const ipole_grid_scale
  * rays to follow"; the paper gives no algorithm: reading R-11 in DESIGN.md).  Dyadic lattice levels
  * l = 0..levels of stride 2^(levels-l) (plus the last row and column): level 0 and 1 are traced everywhere; from then
  * on a new lattice point is traced only if it lies in a cell whose already traced points differ from the bilinear
- * interpolation of the cell's corners by more than rel_tol*|I| + abs_tol in some Stokes parameter, and is bilinearly
- * interpolated otherwise.  The per-ray kernels are those of ipole_make_image (stored path or path-free as set).
+ * interpolation of the cell's corners by more than rel_tol*|I| + abs_tol in some Stokes parameter (a cell narrower
+ * than the stride, which gained no point at a level, keeps its flag), and is bilinearly interpolated otherwise.  The per-ray kernels are those of ipole_make_image (stored path or path-free as set).
  * I,Q,U,V: [ny][nx], all host or all device.  state (nullable, host or device): [ny][nx] bytes, 1 = traced,
  * 2 = interpolated.  info (nullable) is filled on return.  The call synchronises the stream once per level.
- * IPOLE_EINVAL: NULL outputs, levels outside 1..12, negative tolerances, mixed host/device outputs. */
+ * IPOLE_EINVAL: NULL outputs, levels outside 1..12, negative tolerances, an image with fewer than 2 pixels in x or y,
+ * mixed host/device outputs. */
 typedef struct {
   int64_t n_traced;            /* rays followed, all levels                                  */
   int64_t n_traced_level[16];  /* per level 0..levels                                        */

@@ -14,8 +14,9 @@ here in full and followed literally by the CUDA path (reading R-11 in DESIGN.md;
     point on an edge shared by two cells, the one to its right / above it, the other one at the image border).
     Then every flagged level-(l-1) cell P is examined: it needs refinement if, for some new point p in its closed
     rectangle and some Stokes parameter k, |S_k(p) - B_P,k(p)| > rel_tol * |I(p)| + abs_tol, with B_P the bilinear
-    interpolant of P's four corners.  The level-l cells inside P are flagged iff P needs refinement; the cells inside
-    an unflagged P are unflagged.
+    interpolant of P's four corners; a flagged cell that gains no new point at this level (it is narrower than the
+    stride both ways) also counts as needing refinement, i.e. its flag is carried down.  The level-l cells inside P
+    are flagged iff P needs refinement; the cells inside an unflagged P are unflagged.
   After level L (stride 1) every pixel has a value.  Bilinear weights use the actual corner coordinates.
 
 `trace(pixels) -> array [n, 4]` is any per-pixel function (the CPU oracle's make_pixels in the parity tests, closed
@@ -41,6 +42,7 @@ def bilinear(img, i0, i1, j0, j1, i, j):
 
 def adaptive_image(trace, nx, ny, L, rel_tol, abs_tol=0.0):
     """Returns img [4, ny, nx], state [ny, nx] (1 traced, 2 interpolated), and the number of traced pixels per level."""
+    assert nx >= 2 and ny >= 2 and L >= 1
     img = np.zeros((4, ny, nx))
     state = np.zeros((ny, nx), dtype=np.uint8)
     S = 1 << L
@@ -91,7 +93,7 @@ def adaptive_image(trace, nx, ny, L, rel_tol, abs_tol=0.0):
                 continue
             xs = [i for i in range(i0, i1 + 1) if i in lxs]
             ys = [j for j in range(j0, j1 + 1) if j in lys]
-            refine = False
+            refine = len(xs) == 2 and len(ys) == 2   # no new point in P: the flag is carried down
             for j in ys:
                 for i in xs:
                     if i in pxs and j in pys:

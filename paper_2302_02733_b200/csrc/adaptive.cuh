@@ -6,7 +6,8 @@
 //   rectangle between consecutive lines.  Level 0: all lattice points traced, all cells flagged.  Level l >= 1: a new
 //   lattice point is traced if a level-(l-1) cell containing it is flagged, else it takes the bilinear interpolation
 //   of that cell's corners; a flagged level-(l-1) cell P needs refinement if |S_k(p) - B_P,k(p)| > rel_tol |I(p)| +
-//   abs_tol for some new point p in it and some Stokes parameter k; its level-l cells are flagged iff it does.
+//   abs_tol for some new point p in it and some Stokes parameter k, or if it has no new point at this level (narrower
+//   than the stride both ways: the flag is carried down); its level-l cells are flagged iff it does.
 //
 // Arrays are indexed by flat pixel j*nx+i; a cell's flag lives at its lower-left corner pixel.
 #pragma once
@@ -101,7 +102,7 @@ __global__ void k_ada_flag(AdaArgs A) {
     int xs[3], ys[3], nxs = 0, nys = 0;
     xs[nxs++] = i0; if (i0 + s < i1) xs[nxs++] = i0 + s; xs[nxs++] = i1;
     ys[nys++] = j0; if (j0 + s < j1) ys[nys++] = j0 + s; ys[nys++] = j1;
-    bool refine = false;
+    bool refine = (nxs == 2 && nys == 2);   // no new point in this cell: its flag is carried down
     for (int b = 0; b < nys; ++b)
       for (int a = 0; a < nxs; ++a) {
         const int i = xs[a], j = ys[b];

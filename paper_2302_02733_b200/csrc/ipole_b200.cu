@@ -855,6 +855,7 @@ int ipole_make_image_adaptive(ipole_ctx* c, int32_t levels, double rel_tol, doub
                               double* V, uint8_t* state, ipole_adaptive_info* info) {
   if (!c || !I || !Q || !U || !V) return IPOLE_EINVAL;
   if (levels < 1 || levels > 12 || !(rel_tol >= 0.0) || !(abs_tol >= 0.0)) return IPOLE_EINVAL;
+  if (c->cam.nx < 2 || c->cam.ny < 2) return IPOLE_EINVAL;   // a lattice cell needs two lines each way
   if (c->model == MODEL_NONE) return IPOLE_ENOMODEL;
   const int nx = c->cam.nx, ny = c->cam.ny;
   const int64_t n = (int64_t)nx * ny;
