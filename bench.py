@@ -72,8 +72,8 @@ def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier,
     M, n = wl["sweep"], wl["n"]
     is_grid = wl["kind"] == "grid"
     models = sweep_sets(M, grid[0]) if is_grid else sweep_models(M)
+    make_images = g.make_images_grid if is_grid else g.make_images_adaf
     if is_grid:
-        g.make_images_adaf = g.make_images_grid     # same call shape below
         def load_one(mod):
             d = dict(grid[0]); d.update(mod); g.load_grid(d, grid[1])
     else:
@@ -82,7 +82,7 @@ def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier,
     names = ["I", "Q", "U", "V"]
     out = {k: torch.empty((M, n, n), dtype=torch.float64, device="cuda") for k in names}
     for _ in range(args.warmup):
-        g.make_images_adaf(models, out=out)
+        make_images(models, out=out)
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
@@ -91,7 +91,7 @@ def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier,
     barrier()
     ev0.record()
     for _ in range(args.steps):
-        g.make_images_adaf(models, out=out)
+        make_images(models, out=out)
     ev1.record()
     barrier()
     ms = replicas.max_over_ranks(ev0.elapsed_time(ev1), "cuda")
@@ -113,12 +113,12 @@ def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier,
     clocks = sampler.stop() if rank == 0 else None
     # e2e: host buffers out (M images), parameters in
     host = {k: torch.empty((M, n, n), dtype=torch.float64).pin_memory().numpy() for k in names}
-    g.make_images_adaf(models, out=host)
+    make_images(models, out=host)
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
         g.set_camera(**cam)
-        g.make_images_adaf(models, out=host)
+        make_images(models, out=host)
     torch.cuda.synchronize()
     dt = replicas.max_over_ranks(time.perf_counter() - t0, "cuda")
     if rank != 0:
