@@ -42,15 +42,15 @@ __device__ __forceinline__ double ada_bilinear(const double* p, int nx, int i0, 
   return __dadd_rn(__dadd_rn(__dadd_rn(__dmul_rn(w00, a), __dmul_rn(w10, b)), __dmul_rn(w01, c)), __dmul_rn(w11, d));
 }
 
-// level 0: list every lattice point, flag every cell
-__global__ void k_ada_level0(AdaArgs A, uint8_t* flag0) {
+// levels 0 and 1 in one go (both are traced everywhere, so one launch of the per-ray kernels serves them): list every
+// level-1 lattice point (stride A.s), flag every level-0 cell (stride s0 = 2 A.s)
+__global__ void k_ada_level01(AdaArgs A, uint8_t* flag0, int s0) {
   const int64_t n = (int64_t)A.nx * A.ny;
   for (int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
     const int i = (int)(p % A.nx), j = (int)(p / A.nx);
-    const bool on = ada_on_line(i, A.nx, A.s) && ada_on_line(j, A.ny, A.s);
     A.state[p] = 0;
-    flag0[p] = (on && i < A.nx - 1 && j < A.ny - 1) ? 1 : 0;
-    if (on) A.list[atomicAdd(A.count, 1)] = p;
+    flag0[p] = ((i % s0) == 0 && (j % s0) == 0 && i < A.nx - 1 && j < A.ny - 1) ? 1 : 0;
+    if (ada_on_line(i, A.nx, A.s) && ada_on_line(j, A.ny, A.s)) A.list[atomicAdd(A.count, 1)] = p;
   }
 }
 

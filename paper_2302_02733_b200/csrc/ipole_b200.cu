@@ -891,13 +891,15 @@ int ipole_make_image_adaptive(ipole_ctx* c, int32_t levels, double rel_tol, doub
   std::memset(&inf, 0, sizeof inf);
   CK(cudaEventRecord(c->ev_ada0, c->stream));
   int launches = 0;
+  auto n_lines = [](int n_, int s_) { return (n_ + s_ - 1) / s_ + (((n_ - 1) % s_) ? 1 : 0); };
   for (int l = 0; l <= levels; ++l) {
-    A.s = 1 << (levels - l);
-    uint8_t* fprev = (l & 1) ? flag_a : flag_b;   // written at level l-1
+    if (l == 1) continue;                          // traced together with level 0
+    A.s = 1 << (levels - std::max(l, 1));          // level 0 lists the level-1 lattice
+    uint8_t* fprev = (l & 1) ? flag_a : flag_b;    // written at level l-1
     uint8_t* fcur = (l & 1) ? flag_b : flag_a;
     A.flag_prev = fprev; A.flag_cur = fcur;
     CK(cudaMemsetAsync(A.count, 0, sizeof(int), c->stream));
-    if (l == 0) k_ada_level0<<<gb, 256, 0, c->stream>>>(A, fcur);
+    if (l == 0) k_ada_level01<<<gb, 256, 0, c->stream>>>(A, fcur, 1 << levels);
     else k_ada_select<<<gb, 256, 0, c->stream>>>(A);
     ++launches;
     CK(cudaGetLastError());
@@ -916,10 +918,21 @@ int ipole_make_image_adaptive(ipole_ctx* c, int32_t levels, double rel_tol, doub
       CK(cudaStreamSynchronize(c->stream));
       inf.total_steps += r.total_steps;
     }
-    inf.n_traced_level[l] = cnt;
+    if (l == 0) {
+      const int64_t n0 = (int64_t)n_lines(nx, 1 << levels) * n_lines(ny, 1 << levels);
+      inf.n_traced_level[0] = n0;
+      inf.n_traced_level[1] = cnt - n0;
+    } else {
+      inf.n_traced_level[l] = cnt;
+    }
     inf.n_traced += cnt;
-    if (l >= 1 && l < levels) {
-      CK(cudaMemsetAsync(fcur, 0, (size_t)n, c->stream));
+    // cells of level max(l,1)-1 are examined with the points of level max(l,1); after level 0+1 that is level 1
+    const int lf = std::max(l, 1);
+    if (lf < levels) {
+      uint8_t* fp = (lf & 1) ? flag_a : flag_b;
+      uint8_t* fc = (lf & 1) ? flag_b : flag_a;
+      A.flag_prev = fp; A.flag_cur = fc;
+      CK(cudaMemsetAsync(fc, 0, (size_t)n, c->stream));
       k_ada_flag<<<gb, 256, 0, c->stream>>>(A);
       ++launches;
       CK(cudaGetLastError());
