@@ -26,10 +26,10 @@ if ROOT not in sys.path:
 # FP64 operations per geodesic step of each kernel as shipped, counted by ncu (DFMA = 2, DADD/DMUL = 1;
 # smsp__sass_thread_inst_executed_op_d{fma,add,mul}_pred_on.sum / thread-steps of the launch): profiles/r1_k_*.txt,
 # DESIGN.md section 7.  The grid figures are averages over ALL steps of a ray (stats.total_steps): k_transfer<grid> walks
-# only half of them (785 flop and 66.9 B per walked step; rays start at their first contact with plasma).
+# only half of them (786 flop and 68.2 B per walked step; rays start at their first contact with plasma).
 FLOP_PER_STEP = {"transfer_adaf": 1663.0, "transfer_grid": 390.0, "geodesic_adaf": 994.0, "geodesic_grid": 1183.0}
 # DRAM bytes per step of k_transfer (dram__bytes_read + write of one launch / its thread-steps, same captures)
-DRAM_BYTES_PER_STEP = {"transfer_adaf": 64.2, "transfer_grid": 33.2}
+DRAM_BYTES_PER_STEP = {"transfer_adaf": 64.2, "transfer_grid": 33.8}
 # --unpolarized: per step of k_transfer_unpol<model> (ncu, profiles/r1_unpolarized.md)
 FLOP_PER_STEP_UNPOL = {"transfer_adaf": 652.0, "transfer_grid": 76.4}   # grid: 601 per walked step, 12.7 % of the steps walked
 # --path-free (PAPER.md:43 variant): per FORWARD step of k_transfer<model, 1> (RK4 push + transfer step in one kernel)

@@ -315,7 +315,7 @@ constexpr int SWEEP_MAX_MODELS = 64;   // parameter sets per transfer launch (sh
 #define IPOLE_RT_THREADS 128
 #endif
 #ifndef IPOLE_RT_MINB
-#define IPOLE_RT_MINB 2
+#define IPOLE_RT_MINB 3   // grid model; 2 (254 registers) was better until rays started at their first plasma contact
 #endif
 #ifndef IPOLE_RT_MINB_ANALYTIC
 #define IPOLE_RT_MINB_ANALYTIC 3
@@ -336,7 +336,8 @@ constexpr int SWEEP_MAX_MODELS = 64;   // parameter sets per transfer launch (sh
 // a-4 ... a-7, a-8.  Lane-level refill as in k_geodesic.  Per step: midpoint (Xm, Km), generator A = Gamma.Km,
 // f <- P f, plasma operator, f <- P f  (Strang splitting, R-6).
 // Resident blocks per SM: 3 (168 registers, a few spilled doubles) for the analytic models, which ncu shows limited
-// by dependent-issue latency; 2 (255 registers) for the grid model, whose 64 gathered values per step want registers.
+// by dependent-issue latency, and for the grid model too since k_geodesic<true> marks the plasma-contact range (a
+// walked step is now mostly transport and plasma arithmetic, not a dark gather test): 117 -> 102 ms at 1024^2.
 //
 // PF = 0: the stored path is walked from its far end to the camera.
 // PF = 1, 2: path-free bidirectional variant (R-10; 1: eps <= 0.04, RK4 stage points by Taylor
