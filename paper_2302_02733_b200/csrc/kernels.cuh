@@ -503,8 +503,14 @@ k_transfer(const __grid_constant__ RtArgs A) {
 // stored path.  Per step: midpoint, metric (no derivatives, no transport), plasma state, nu = -k.u nu_obs, pitch
 // angle, thermal synchrotron j_I and alpha_I, exact scalar step  I <- I e^{-x} + j ds (1 - e^{-x})/x,  x = alpha ds.
 // Work items and refill as in k_transfer (SWEEP: (ray, parameter set) pairs, the lanes of a warp share a ray).
+#ifndef IPOLE_UNPOL_MINB_ANALYTIC
+#define IPOLE_UNPOL_MINB_ANALYTIC 5   // measured: 3..6 blocks, profiles/r1_unpolarized.md
+#endif
+#ifndef IPOLE_UNPOL_MINB_GRID
+#define IPOLE_UNPOL_MINB_GRID 4
+#endif
 template <int MODEL, bool SWEEP>
-__global__ void __launch_bounds__(IPOLE_RT_THREADS, (MODEL == MODEL_GRID) ? 3 : 4) k_transfer_unpol(const __grid_constant__ RtArgs A) {
+__global__ void __launch_bounds__(IPOLE_RT_THREADS, (MODEL == MODEL_GRID) ? IPOLE_UNPOL_MINB_GRID : IPOLE_UNPOL_MINB_ANALYTIC) k_transfer_unpol(const __grid_constant__ RtArgs A) {
   static_assert(!SWEEP || MODEL != MODEL_SLAB, "the sweep is built for the ADAF and grid models");
   const CamDev& C = A.cam;
   const int64_t count = (A.count_dev ? (int64_t)*A.count_dev : A.count) * (SWEEP ? A.n_models : 1);
