@@ -49,6 +49,8 @@ WORKLOADS = {
     # many-small-images mode (128x128 images for model fitting): 64 parameter sets per call
     "sweep128": dict(kind="adaf", n=128, config=None, sweep=64),
     "gridsweep128": dict(kind="grid", n=128, config=None, sweep=64, grid=(288, 128, 128)),
+    # small images whose GEOMETRY differs (inclination): nothing to share, so independent contexts run side by side
+    "cams128": dict(kind="adaf", n=128, config=None, cams=8),
 }
 
 
@@ -253,6 +255,69 @@ def oracle_sample(workload, n_rays, nthreads, path_free=False, unpolarized=False
     return pix.size, r.total_steps(), dt, stride
 
 
+def run_cams(args, ipole, replicas, W, wl, world, rank, local, barrier):
+    """One step = one 128x128 image for each of `cams` cameras (different inclinations).  Contexts are independent
+    (include/ipole.h), so each camera gets its own context, CUDA stream and host thread; compared with the same images
+    made one after the other on a single context."""
+    import threading as th
+    import torch
+    n, nc = wl["n"], wl["cams"]
+    incl = [20.0 + 60.0 * k / max(1, nc - 1) for k in range(nc)]
+    cams = [W.camera("adaf", n, inclination_deg=a) for a in incl]
+    names = ["I", "Q", "U", "V"]
+    ctxs, streams, outs = [], [], []
+    for cam in cams:
+        g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
+        g.set_options(4 << 30, 1)                  # 4 GiB of path buffer per context instead of 40 % of the free memory
+        s = torch.cuda.Stream(); g.set_stream(s)
+        ctxs.append(g); streams.append(s)
+        outs.append({k: torch.empty((n, n), dtype=torch.float64, device="cuda") for k in names})
+
+    def side_by_side():
+        def work(k):
+            torch.cuda.set_device(local)
+            ctxs[k].make_image(out=outs[k])
+        ts = [th.Thread(target=work, args=(k,)) for k in range(nc)]
+        for t in ts: t.start()
+        for t in ts: t.join()
+        for s in streams: s.synchronize()
+
+    def one_by_one():
+        for k in range(nc):
+            ctxs[k].make_image(out=outs[k])
+            streams[k].synchronize()
+
+    res = {}
+    for name, fn in (("side_by_side", side_by_side), ("one_by_one", one_by_one)):
+        for _ in range(args.warmup):
+            fn()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            fn()
+        torch.cuda.synchronize()
+        res[name] = replicas.max_over_ranks(time.perf_counter() - t0, "cuda") / args.steps
+    if rank != 0:
+        return
+    rays = nc * n * n
+    line = {"metric": "rays_per_s", "value": world * rays / res["side_by_side"], "unit": "rays/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": res["side_by_side"] * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "image": "%dx%d" % (n, n), "cameras": nc, "inclinations_deg": incl,
+                       "model": "adaf", "freq_ghz": 230, "full_stokes": True, "timing": "host wall clock around %d threads, "
+                       "one context and stream each, all streams synchronised inside" % nc,
+                       "l2": "not flushed: 8 independent images per step, each streaming its own path buffer", "parallelism": "single GPU"},
+            "images_per_s": world * nc / res["side_by_side"],
+            "one_by_one": {"images_per_s": world * nc / res["one_by_one"], "ms_per_%d_images" % nc: res["one_by_one"] * 1e3,
+                           "speedup_side_by_side": res["one_by_one"] / res["side_by_side"]},
+            "gpu_launches": sum(g.stats()["n_launches"] for g in ctxs) * args.steps,
+            "roofline": {"bound": "alu", "kernel": "k_transfer<adaf>", "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "achieved": None,
+                         "frac": None, "traffic": None, "note": "latency study of small images; see the default bench line for the kernels"},
+            "e2e": {"value": world * rays / res["side_by_side"], "unit": "rays/s", "h2d_bytes_per_step": 0,
+                    "d2h_bytes_per_step": 0, "note": "device outputs; the timing is host wall clock already"}}
+    print(json.dumps(line), flush=True)
+
+
 def run_adaptive(args, g, replicas, wl, cam, world, rank, local, barrier):
     """One step = one ipole_make_image_adaptive call; the full image of the same workload is made once for the error."""
     import torch
@@ -388,6 +453,15 @@ def main():
     from paper_2302_02733_b200 import ipole, replicas, workloads as W
 
     wl = WORKLOADS[args.workload]
+    if wl.get("cams"):
+        def barrier0():
+            if world > 1:
+                dist.barrier()
+            torch.cuda.synchronize()
+        run_cams(args, ipole, replicas, W, wl, world, rank, local, barrier0)
+        if world > 1:
+            dist.destroy_process_group()
+        return
     cam = W.camera(wl["kind"], wl["n"])
     g = ipole.Ipole(**cam)
     g.set_stream(torch.cuda.current_stream())

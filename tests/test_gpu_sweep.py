@@ -143,3 +143,33 @@ def test_grid_sweep_equals_single_images_and_oracle(ipole, ref):
     with pytest.raises(ipole.IpoleError) as ei:
         g0.make_images_grid(sets)
     assert ei.value.code == ipole.ENOMODEL
+
+
+def test_independent_contexts_side_by_side(ipole):
+    """include/ipole.h: distinct contexts are independent.  Four cameras on four contexts, streams and host threads
+    give the same bits as one after the other (bench.py --workload cams128 measures the gain)."""
+    import threading
+    import torch
+    incl = [25.0, 45.0, 60.0, 75.0]
+    cams = [W.camera("adaf", 40, inclination_deg=a) for a in incl]
+    want = []
+    for cam in cams:
+        g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
+        want.append(to_np(g.make_image(maps=True)))
+    ctxs, streams, outs = [], [], [None] * 4
+    for cam in cams:
+        g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF); g.set_options(1 << 30, 1)
+        s = torch.cuda.Stream(); g.set_stream(s)
+        ctxs.append(g); streams.append(s)
+
+    def work(k):
+        outs[k] = ctxs[k].make_image(maps=True)
+    for _ in range(3):
+        ts = [threading.Thread(target=work, args=(k,)) for k in range(4)]
+        for t in ts: t.start()
+        for t in ts: t.join()
+        for s in streams: s.synchronize()
+        for k in range(4):
+            got = to_np(outs[k])
+            for name in want[k]:
+                assert np.array_equal(got[name], want[k][name]), (k, name)
