@@ -27,13 +27,13 @@ if ROOT not in sys.path:
 # smsp__sass_thread_inst_executed_op_d{fma,add,mul}_pred_on.sum / thread-steps of the launch): profiles/r1_k_*.txt,
 # DESIGN.md section 7.  The grid figures are averages over ALL steps of a ray (stats.total_steps): k_transfer<grid> walks
 # only half of them (786 flop and 68.2 B per walked step; rays start at their first contact with plasma).
-FLOP_PER_STEP = {"transfer_adaf": 1663.0, "transfer_grid": 390.0, "geodesic_adaf": 994.0, "geodesic_grid": 1183.0}
+FLOP_PER_STEP = {"transfer_adaf": 1576.0, "transfer_grid": 390.0, "geodesic_adaf": 994.0, "geodesic_grid": 1183.0}
 # DRAM bytes per step of k_transfer (dram__bytes_read + write of one launch / its thread-steps, same captures)
 DRAM_BYTES_PER_STEP = {"transfer_adaf": 64.2, "transfer_grid": 33.8}
 # --unpolarized: per step of k_transfer_unpol<model> (ncu, profiles/r1_unpolarized.md)
 FLOP_PER_STEP_UNPOL = {"transfer_adaf": 652.0, "transfer_grid": 76.4}   # grid: 601 per walked step, 12.7 % of the steps walked
 # --path-free (PAPER.md:43 variant): per FORWARD step of k_transfer<model, 1> (RK4 push + transfer step in one kernel)
-FLOP_PER_STEP_PF = {"transfer_adaf": 2646.0, "transfer_grid": 1587.0}
+FLOP_PER_STEP_PF = {"transfer_adaf": 2559.0, "transfer_grid": 1587.0}
 DRAM_BYTES_PER_STEP_PF = {"transfer_adaf": 0.1, "transfer_grid": 1.0}
 # ALU roofline denominator: 148 SMs x 4 sub-partitions x 16 FP64 lanes x 2 flop x 1.965 GHz
 FP64_PEAK_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
