@@ -99,6 +99,10 @@ typedef struct {
   float   ms_long;         /* long-ray passes (geodesic + transfer) on the side stream; they overlap the
                               bulk batches, so this is not part of a sum that gives ms_total            */
   int64_t total_steps_forward; /* path-free variant: steps of the forward passes of all rays (else 0)     */
+  float   ms_stepop, ms_apply; /* split transfer (ipole_set_transfer_split): the step-parallel operator pass and
+                              the per-ray apply pass; both are part of ms_transfer                      */
+  int64_t n_retry;         /* rays that outgrew the path slots of their batch (sized from the predicted step count of the
+                              batch's longest ray) and were traced again with S_cap slots                  */
 } ipole_stats;
 
 /* Create a context. Computes the camera tetrad on the device. IPOLE_EINVAL on bad parameters. */
@@ -122,6 +126,16 @@ int  ipole_set_options(ipole_ctx*, uint64_t path_bytes, int32_t sort_rays);
  * from the stored-path one at the level the integrator is not time-reversible (paper: "negligible").
  * on == 0 (default): stored path.  Returns IPOLE_EINVAL for a NULL context. */
 int  ipole_set_path_free(ipole_ctx*, int32_t on);
+/* Transfer as two kernels (default on; "at every single step ... evaluate emission, self-absorption and
+ * Faraday coefficients at a given point": everything of a step except the update of the four Stokes numbers depends
+ * on the stored path alone).  on != 0: on the stored path, for the analytic flow, a step-parallel kernel turns every
+ * path step into a 96-byte operator record (projection of the carried polarization basis on the step's plasma tetrad,
+ * and the eight coefficients times the step length), and a per-ray kernel applies the records from the far end to
+ * the camera.  on == 0: the single per-ray transfer kernel does both (also used, whatever this switch says, for the
+ * slab and grid models, the sweeps, the path-free and unpolarized variants, long rays, and rays with a step that
+ * crosses no plasma).  The two give the same image up to rounding.  on == 2 is a test mode: as 1, but every seventh
+ * ray of a batch is handed to the single kernel as if it had such a step.  Returns IPOLE_EINVAL for a NULL context. */
+int  ipole_set_transfer_split(ipole_ctx*, int32_t on);
 /* Unpolarized transfer (the model-fitting loop makes "nonpolarized images"; polarized
  * transfer is "far more complex and computationally demanding"; reading R-12 in DESIGN.md).  on != 0: every image
  * entry (ipole_make_image, _pixels, _images_adaf, _images_grid, _image_adaptive) solves the scalar equation

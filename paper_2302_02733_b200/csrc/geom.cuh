@@ -236,10 +236,22 @@ __device__ __forceinline__ void geodesic_accel(const Geom& G, const double X[4],
 }
 
 // A^a_n = Gamma^a_{mn} K^m as a dense 4x4 (row a, column n); also returns the metric at X for the caller
+__device__ __forceinline__ void transport_generator_from(const Sym7& D1, const Sym7& D2, const Inv6& gi, const double K[4],
+                                                         double A[4][4]);
 __device__ __forceinline__ void transport_generator(const Geom& G, const double X[4], const double K[4], Point& p,
                                                     Sym7& g, Inv6& gi, double A[4][4]) {
   Sym7 D1, D2;
   metric_derivs(G, X, p, g, gi, D1, D2);
+  transport_generator_from(D1, D2, gi, K, A);
+}
+// the same from a Point whose scalars are already filled (metric and derivatives are rebuilt from it)
+__device__ __forceinline__ void transport_generator_at(const Geom& G, const double K[4], Point& p, double A[4][4]) {
+  Sym7 g, D1, D2; Inv6 gi;
+  metric_derivs_at(G, p, g, gi, D1, D2);
+  transport_generator_from(D1, D2, gi, K, A);
+}
+__device__ __forceinline__ void transport_generator_from(const Sym7& D1, const Sym7& D2, const Inv6& gi, const double K[4],
+                                                         double A[4][4]) {
   double v1[4], v2[4];
   D1.mul(K, v1);
   D2.mul(K, v2);
@@ -280,6 +292,18 @@ __device__ __forceinline__ void transport_apply(const double A[4][4], double h, 
   const double hh = 0.5 * h * h;
 #pragma unroll
   for (int a = 0; a < 4; ++a) f[a] = f[a] - h * w[a] + hh * w2[a];
+}
+
+// c <- (1 - h A + h^2 A^2 / 2)^T c : the pull-back of a covector through the same half step
+__device__ __forceinline__ void transport_apply_transposed(const double A[4][4], double h, double c[4]) {
+  double w[4], w2[4];
+#pragma unroll
+  for (int n = 0; n < 4; ++n) w[n] = A[0][n] * c[0] + A[1][n] * c[1] + A[2][n] * c[2] + A[3][n] * c[3];
+#pragma unroll
+  for (int n = 0; n < 4; ++n) w2[n] = A[0][n] * w[0] + A[1][n] * w[1] + A[2][n] * w[2] + A[3][n] * w[3];
+  const double hh = 0.5 * h * h;
+#pragma unroll
+  for (int n = 0; n < 4; ++n) c[n] = c[n] - h * w[n] + hh * w2[n];
 }
 
 __device__ __forceinline__ double dot4(const double u[4], const double v[4]) {

@@ -11,6 +11,7 @@
 #include <new>
 #include <vector>
 #include "kernels.cuh"
+#include "stepop.cuh"
 #include "adaptive.cuh"
 
 using namespace ipole;
@@ -21,7 +22,8 @@ constexpr int N_QUEUES = 8192;
 constexpr int PROBE_TARGET = 4096;   // rays of the probe pass
 constexpr int PROBE_EPS_FACTOR = 4;  // the probe integrates with 4 eps and predicts 4x its step count
 
-enum LaunchKind { LK_PROBE = 0, LK_GEO = 1, LK_RT = 2, LK_OTHER = 3, LK_LONG = 4 };  // LK_LONG: on the side stream
+enum LaunchKind { LK_PROBE = 0, LK_GEO = 1, LK_RT = 2, LK_OTHER = 3, LK_LONG = 4,   // LK_LONG: on the side stream
+                  LK_OPS = 5, LK_APPLY = 6 };                                          // split transfer: k_stepop, k_apply
 
 struct TimedSpan { cudaEvent_t a, b; int kind; };
 
@@ -48,6 +50,13 @@ struct ipole_ctx {
   int opt_occ = 1;               // grid model: plasma-contact range per ray (IPOLE_NO_OCC=1 in the environment turns it off)
   int last_pf = 0;               // the last image was made path-free
   int opt_unpol = 0;             // unpolarized transfer of I alone
+  AdafParams adaf_host;          // host copy of the loaded analytic model (k_apply takes it by value)
+  int opt_tight = 1;             // sorted rays: path slots sized batch by batch from the predicted step counts
+  int32_t* d_retry = nullptr;    // rays that outgrew their batch's slots (retried with the global S_cap)
+  int opt_split = 1;             // stored path, analytic flow: transfer as k_stepop + k_apply (stepop.cuh)
+  double* d_ops = nullptr; size_t ops_bytes = 0;   // operator records of one batch
+  int32_t* d_irr = nullptr;      // slots of the rays k_stepop leaves to k_transfer
+  int occ_op = 0, occ_ap = 0;
   int occ_unpol[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};
   double* d_endp = nullptr; int64_t endp_cap = 0;   // end points of the backward passes, [rays][8]
   long long* d_sum = nullptr;    // forward-step total of the path-free variant
@@ -71,7 +80,7 @@ struct ipole_ctx {
   int32_t* d_probe = nullptr; int64_t probe_cap = 0;
   unsigned long long* d_queues = nullptr;
   unsigned int* d_hist = nullptr;
-  int* d_small = nullptr;        // [0] long_count, [1] probe max
+  int* d_small = nullptr;        // [0] long_count, [1] probe max, [2] adaptive list length, [4] irregular rays of a batch
   ReducePartial* d_part = nullptr;
   ReduceOut* d_red = nullptr;
 
@@ -141,8 +150,8 @@ int apply_camera(ipole_ctx* c, const ipole_camera* k) {
 int ensure_rays(ipole_ctx* c, int64_t n) {
   if (n <= c->ray_cap) return IPOLE_OK;
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long); cudaFree(c->d_out);
-  cudaFree(c->d_nsteps_long); cudaFree(c->d_srange); c->d_srange = nullptr;
-  c->d_nsteps = c->d_nturn = c->d_order = c->d_key = c->d_long = c->d_nsteps_long = nullptr; c->d_out = nullptr; c->ray_cap = 0;
+  cudaFree(c->d_nsteps_long); cudaFree(c->d_srange); c->d_srange = nullptr; cudaFree(c->d_irr); cudaFree(c->d_retry); c->d_retry = nullptr;
+  c->d_nsteps = c->d_nturn = c->d_order = c->d_key = c->d_long = c->d_nsteps_long = c->d_irr = nullptr; c->d_out = nullptr; c->ray_cap = 0;
   CK(cudaMalloc(&c->d_nsteps, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_nturn, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_order, n * sizeof(int32_t)));
@@ -150,6 +159,8 @@ int ensure_rays(ipole_ctx* c, int64_t n) {
   CK(cudaMalloc(&c->d_long, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_nsteps_long, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_srange, n * sizeof(int2)));
+  CK(cudaMalloc(&c->d_irr, n * sizeof(int32_t)));
+  CK(cudaMalloc(&c->d_retry, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_out, 6 * n * sizeof(double)));
   c->ray_cap = n;
   return IPOLE_OK;
@@ -161,6 +172,15 @@ int ensure_path(ipole_ctx* c, size_t bytes) {
   cudaError_t e = cudaMalloc(&c->d_path, bytes);
   if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
   c->path_bytes = bytes;
+  return IPOLE_OK;
+}
+
+int ensure_ops(ipole_ctx* c, size_t bytes) {
+  if (bytes <= c->ops_bytes) return IPOLE_OK;
+  cudaFree(c->d_ops); c->d_ops = nullptr; c->ops_bytes = 0;
+  cudaError_t e = cudaMalloc(&c->d_ops, bytes);
+  if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
+  c->ops_bytes = bytes;
   return IPOLE_OK;
 }
 
@@ -177,9 +197,9 @@ size_t path_budget(ipole_ctx* c) {
   if (c->opt_path_bytes) return (size_t)c->opt_path_bytes;
   size_t fr = 0, tot = 0;
   cudaMemGetInfo(&fr, &tot);
-  fr += c->path_bytes + c->path_long_bytes;  // what we already hold counts as available
-  size_t b = (size_t)(0.4 * (double)fr);
-  const size_t cap = (size_t)64 << 30;
+  fr += c->path_bytes + c->path_long_bytes + c->ops_bytes;  // what we already hold counts as available
+  size_t b = (size_t)(0.5 * (double)fr);
+  const size_t cap = (size_t)96 << 30;
   return std::min(b, cap);
 }
 
@@ -286,6 +306,51 @@ int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_
   return IPOLE_OK;
 }
 
+// split transfer of one batch (stepop.cuh): k_stepop over the steps, k_apply over the rays, then k_transfer for the
+// rays k_stepop could not express (listed on the device; usually none)
+int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStream_t st, int reserve) {
+  int* irr_count = c->d_small + 4;
+  CK(cudaMemsetAsync(irr_count, 0, sizeof(int), st));
+  OpArgs o;
+  std::memset(&o, 0, sizeof o);
+  o.cam = a.cam; o.units = a.units; o.model = a.model; o.cap = a.cap; o.base = a.base; o.count = a.count; o.order = a.order;
+  o.path = a.path; o.nsteps = a.nsteps; o.queue = a.queue; o.ops = c->d_ops; o.irr_slots = c->d_irr; o.irr_count = irr_count; o.test_irregular = (c->opt_split == 2);
+  {
+    const int s = span_begin(c, LK_OPS, st);
+    // one warp per ray at a time
+    const int g = grid_for(c, c->occ_op, IPOLE_OP_THREADS / 32, rays, reserve);
+    k_stepop<MODEL_ADAF><<<g, IPOLE_OP_THREADS, 0, st>>>(o);
+    span_end(c, s, st);
+    c->stats.n_launches++;
+    CK(cudaGetLastError());
+  }
+  ApArgs p;
+  std::memset(&p, 0, sizeof p);
+  p.nu3 = a.units.nu_obs * a.units.nu_obs * a.units.nu_obs;
+  p.model = c->adaf_host;
+  p.cap = a.cap; p.base = a.base; p.count = a.count; p.order = a.order; p.ops = c->d_ops; p.nsteps = a.nsteps;
+  p.queue = a.queue + 1;
+  p.I = a.I; p.Q = a.Q; p.U = a.U; p.V = a.V; p.tau = a.tau; p.tauF = a.tauF;
+  {
+    const int s = span_begin(c, LK_APPLY, st);
+    const int g = grid_for(c, c->occ_ap, IPOLE_AP_THREADS / 32, (rays + 31) / 32, reserve);   // one warp per 32 rays
+    k_apply<<<g, IPOLE_AP_THREADS, 0, st>>>(p);
+    span_end(c, s, st);
+    c->stats.n_launches++;
+    CK(cudaGetLastError());
+  }
+  RtArgs t = a;
+  t.queue = a.queue + 2; t.count_dev = irr_count; t.slots = c->d_irr;
+  {
+    const int s = span_begin(c, LK_RT, st);
+    k_transfer<MODEL_ADAF, 0><<<std::max(1, c->n_sm / 8), IPOLE_RT_THREADS, 0, st>>>(t);
+    span_end(c, s, st);
+    c->stats.n_launches++;
+    CK(cudaGetLastError());
+  }
+  return IPOLE_OK;
+}
+
 GeoArgs geo_args(ipole_ctx* c) {
   GeoArgs g;
   std::memset(&g, 0, sizeof g);
@@ -325,7 +390,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   c->have_image = false;
   c->last_pf = 0;
   CK(cudaMemsetAsync(c->d_queues, 0, N_QUEUES * sizeof(unsigned long long), c->stream));
-  CK(cudaMemsetAsync(c->d_small, 0, 4 * sizeof(int), c->stream));
+  CK(cudaMemsetAsync(c->d_small, 0, 2 * sizeof(int), c->stream));
   int qi = 0;
   const int total = span_begin(c, LK_OTHER, c->stream);
 
@@ -334,6 +399,8 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   const int max_steps = c->cam.max_steps;
   int cap = max_steps;
   const int32_t* order = nullptr;
+  std::vector<unsigned int> bin_prefix;   // sorted rays: number of rays in the bins before each bin (longer rays)
+  int bin_width = 1;
   const bool fits_all = (double)n * (double)(max_steps + 1) * (double)rec_bytes <= (double)budget;
   const bool probe = (n >= 32768 || c->opt_sort == 2) && (c->opt_sort || !fits_all);
 
@@ -378,9 +445,14 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
       const int gb = (int)std::min<int64_t>((n + 255) / 256, 148 * 8);
       k_predict_hist<<<gb, 256, 0, c->stream>>>(sa);
       k_scan_bins<<<1, 1024, 0, c->stream>>>(c->d_hist);
+      // rays before each bin in the sorted order: sizes the path slots batch by batch (below)
+      bin_prefix.resize(SORT_BINS);
+      CK(cudaMemcpyAsync(bin_prefix.data(), c->d_hist, SORT_BINS * sizeof(unsigned int), cudaMemcpyDeviceToHost, c->stream));
       k_scatter<<<gb, 256, 0, c->stream>>>(sa);
       c->stats.n_launches += 3;
       CK(cudaGetLastError());
+      CK(cudaStreamSynchronize(c->stream));
+      bin_width = sa.bin_width;
       order = c->d_order;
     }
     span_end(c, sp, c->stream);
@@ -468,40 +540,107 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     return IPOLE_OK;
   };
 
-  // ---- bulk pass in batches of B rays ----
+  // ---- bulk pass in batches ----
   // (Running k_geodesic of batch k+1 on a second stream beside k_transfer of batch k was tried and dropped: the
   // transfer blocks leave no room for useful geodesic occupancy, profiles/r1_notes.md.)
-  const size_t slot_bytes = (size_t)(cap + 1) * rec_bytes;
-  int64_t B = std::min<int64_t>(n, (int64_t)(budget / slot_bytes));
-  if (B < 1) return IPOLE_ENOMEM;
-  if ((rc = ensure_path(c, (size_t)B * slot_bytes)) != IPOLE_OK) return rc;
+  // split transfer (stepop.cuh): the batch also holds one 96-B operator record per step.
+  //
+  // Slots per batch: the rays are in order of predicted step count, longest first, so a batch needs slots only as
+  // long as the prediction of its FIRST ray (times the same 1.15 margin as the global S_cap).  The longest rays fill
+  // the first batch or two; every later batch holds two to three times as many rays in the same memory, and the
+  // persistent kernels have that many fewer tails.  A ray that outgrows its batch's slot is listed and retried at
+  // the end with the global S_cap (second level); one that outgrows S_cap goes to the long-ray pass as before.
+  const bool split = c->opt_split && !sw && !c->opt_unpol && c->model == MODEL_ADAF;
+  const size_t step_bytes = rec_bytes + (split ? OP_DOUBLES * sizeof(double) : 0);
+  const bool tight = order != nullptr && !bin_prefix.empty() && c->opt_tight;
+  struct Batch { int64_t base, cnt; int cap; };
+  std::vector<Batch> plan;
+  auto make_plan = [&](int64_t total_rays, bool use_bins) {
+    plan.clear();
+    for (int64_t base = 0; base < total_rays;) {
+      int cb = cap;
+      if (use_bins) {
+        const int bin = (int)(std::upper_bound(bin_prefix.begin(), bin_prefix.end(), (unsigned int)base) - bin_prefix.begin()) - 1;
+        const int64_t pred_hi = (int64_t)(SORT_BINS - std::max(bin, 0)) * bin_width;
+        cb = (int)std::min<int64_t>(cap, (int64_t)(pred_hi * 1.15) + 64);
+      }
+      int64_t B = (int64_t)(budget / ((size_t)(cb + 1) * step_bytes));
+      if (B >= 64) B &= ~(int64_t)31;           // whole groups of 32 slots (operator records, stepop.cuh)
+      B = std::max<int64_t>(1, std::min(B, total_rays - base));
+      plan.push_back({base, B, cb});
+      base += B;
+    }
+  };
+  make_plan(n, tight);
+  size_t need_path = 0, need_ops = 0;
+  for (const Batch& b : plan) {
+    need_path = std::max(need_path, (size_t)b.cnt * (size_t)(b.cap + 1) * rec_bytes);
+    need_ops = std::max(need_ops, (size_t)((b.cnt + 31) / 32 * 32) * (size_t)(b.cap + 1) * OP_DOUBLES * sizeof(double));
+  }
+  if (tight) {   // the retry level runs with the global S_cap
+    const int64_t Br = std::max<int64_t>(1, (int64_t)(budget / ((size_t)(cap + 1) * step_bytes)));
+    const int64_t rr = std::min<int64_t>(Br, std::max<int64_t>(n / 8, 1));   // more than n/8 retries never happen; the buffer grows if they do
+    need_path = std::max(need_path, (size_t)rr * (size_t)(cap + 1) * rec_bytes);
+    need_ops = std::max(need_ops, (size_t)((rr + 31) / 32 * 32) * (size_t)(cap + 1) * OP_DOUBLES * sizeof(double));
+  }
+  if ((rc = ensure_path(c, need_path)) != IPOLE_OK) return rc;
+  if (split && (rc = ensure_ops(c, need_ops)) != IPOLE_OK) return rc;
   int n_long = 0;
+  int* retry_count = c->d_small + 5;
   // with few batches the long-ray passes cannot wait for kernel boundaries: keep 8 block slots free for them
-  const int reserve = (cap < max_steps && (n + B - 1) / B <= 16) ? 8 : 0;
-  for (int64_t base = 0; base < n; base += B) {
-    const int64_t cnt = std::min(B, n - base);
-    if (qi + 2 > N_QUEUES) return IPOLE_EINVAL;
+  const int reserve = (cap < max_steps && plan.size() <= 16) ? 8 : 0;
+  auto run_batch = [&](const Batch& b, const int32_t* ord) -> int {
+    if (qi + 4 > N_QUEUES) return IPOLE_EINVAL;
+    const bool top = b.cap >= cap;             // overflow means "longer than S_cap": the long-ray pass
     GeoArgs g = geo_args(c);
-    g.cap = cap; g.base = base; g.count = cnt; g.order = order; g.pixels = d_pixels;
+    g.cap = b.cap; g.base = b.base; g.count = b.cnt; g.order = ord; g.pixels = d_pixels;
     g.path = c->d_path; g.nsteps = c->d_nsteps; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
-    g.long_list = c->d_long; g.long_count = c->d_small;
+    if (top) { g.long_list = c->d_long; g.long_count = c->d_small; }
+    else { g.long_list = c->d_retry; g.long_count = retry_count; }
     if (use_occ) { g.grid = (const GridParams*)c->d_model; g.srange = c->d_srange; }
-    if ((rc = launch_geodesic(c, g, LK_GEO, cnt, c->stream, reserve)) != IPOLE_OK) return rc;
-    if (cap < max_steps) {
+    int rcb;
+    if ((rcb = launch_geodesic(c, g, LK_GEO, b.cnt, c->stream, reserve)) != IPOLE_OK) return rcb;
+    if (top && cap < max_steps) {
       CK(cudaEventRecord(c->ev_geo, c->stream));
       CK(cudaStreamWaitEvent(c->side, c->ev_geo, 0));
     }
     RtArgs t;
     std::memset(&t, 0, sizeof t);
-    t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = cap; t.base = base; t.count = cnt; t.order = order;
-    t.path = c->d_path; t.nsteps = c->d_nsteps; t.queue = c->d_queues + (qi++);
+    t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = b.cap; t.base = b.base; t.count = b.cnt; t.order = ord;
+    t.path = c->d_path; t.nsteps = c->d_nsteps; t.queue = c->d_queues + qi;
+    qi += split ? 3 : 1;
     if (use_occ) t.srange = c->d_srange;
     t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
-    if ((rc = launch_transfer(c, t, LK_RT, cnt, c->stream, reserve, 0, sw)) != IPOLE_OK) return rc;
+    if (split) rcb = launch_transfer_split(c, t, b.cnt, c->stream, reserve);
+    else rcb = launch_transfer(c, t, LK_RT, b.cnt, c->stream, reserve, 0, sw);
+    if (rcb != IPOLE_OK) return rcb;
     c->stats.n_batches++;
-    if (cap < max_steps) {   // the transfer kernel just queued keeps the GPU busy while the host waits here
-      if ((rc = listed(c->ev_geo, n_long)) != IPOLE_OK) return rc;
-      if ((rc = long_pass(n_long)) != IPOLE_OK) return rc;
+    if (top && cap < max_steps) {   // the transfer kernel just queued keeps the GPU busy while the host waits here
+      if ((rcb = listed(c->ev_geo, n_long)) != IPOLE_OK) return rcb;
+      if ((rcb = long_pass(n_long)) != IPOLE_OK) return rcb;
+    }
+    return IPOLE_OK;
+  };
+  CK(cudaMemsetAsync(retry_count, 0, sizeof(int), c->stream));
+  for (const Batch& b : plan)
+    if ((rc = run_batch(b, order)) != IPOLE_OK) return rc;
+  if (tight) {
+    // second level: the rays that outgrew their batch's slots, with the global S_cap
+    int n_retry = 0;
+    CK(cudaMemcpyAsync(&n_retry, retry_count, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    c->stats.n_retry = n_retry;
+    if (n_retry > 0) {
+      make_plan(n_retry, false);
+      size_t np2 = 0, no2 = 0;
+      for (const Batch& b : plan) {
+        np2 = std::max(np2, (size_t)b.cnt * (size_t)(b.cap + 1) * rec_bytes);
+        no2 = std::max(no2, (size_t)((b.cnt + 31) / 32 * 32) * (size_t)(b.cap + 1) * OP_DOUBLES * sizeof(double));
+      }
+      if ((rc = ensure_path(c, np2)) != IPOLE_OK) return rc;
+      if (split && (rc = ensure_ops(c, no2)) != IPOLE_OK) return rc;
+      for (const Batch& b : plan)
+        if ((rc = run_batch(b, c->d_retry)) != IPOLE_OK) return rc;
     }
   }
   c->stats.n_long = n_long;
@@ -542,7 +681,7 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   if (cudaMalloc(&c->d_model, msz) != cudaSuccess) return fail(IPOLE_ENOMEM);
   if (cudaMalloc(&c->d_queues, N_QUEUES * sizeof(unsigned long long)) != cudaSuccess) return fail(IPOLE_ENOMEM);
   if (cudaMalloc(&c->d_hist, SORT_BINS * sizeof(unsigned int)) != cudaSuccess) return fail(IPOLE_ENOMEM);
-  if (cudaMalloc(&c->d_small, 4 * sizeof(int)) != cudaSuccess) return fail(IPOLE_ENOMEM);
+  if (cudaMalloc(&c->d_small, 8 * sizeof(int)) != cudaSuccess) return fail(IPOLE_ENOMEM);
   if (cudaMalloc(&c->d_part, REDUCE_BLOCKS * sizeof(ReducePartial)) != cudaSuccess) return fail(IPOLE_ENOMEM);
   if (cudaMalloc(&c->d_red, sizeof(ReduceOut)) != cudaSuccess) return fail(IPOLE_ENOMEM);
   {
@@ -575,6 +714,10 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_unpol[MODEL_ADAF][1], k_transfer_unpol<MODEL_ADAF, true>, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_unpol[MODEL_GRID][1], k_transfer_unpol<MODEL_GRID, true>, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_sweep[MODEL_GRID], k_transfer<MODEL_GRID, 0, true>, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_op, k_stepop<MODEL_ADAF>, IPOLE_OP_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap, k_apply, IPOLE_AP_THREADS, 0);
+  { const char* e = std::getenv("IPOLE_NO_SPLIT"); if (e && e[0] == '1') c->opt_split = 0; }
+  { const char* e = std::getenv("IPOLE_NO_TIGHT"); if (e && e[0] == '1') c->opt_tight = 0; }
   rc = apply_camera(c, cam);
   if (rc != IPOLE_OK) return fail(rc);
   *out = c;
@@ -592,10 +735,9 @@ int ipole_set_camera(ipole_ctx* c, const ipole_camera* cam) {
   rc = apply_camera(c, cam);
   if (rc != IPOLE_OK) return rc;
   if (c->model == MODEL_ADAF && a_old != cam->spin) {  // r_isco depends on the spin
-    AdafParams p;
-    CK(cudaMemcpy(&p, c->d_model, sizeof p, cudaMemcpyDeviceToHost));
-    p.r_isco = isco_radius(cam->spin);
-    CK(cudaMemcpy(c->d_model, &p, sizeof p, cudaMemcpyHostToDevice));
+    c->adaf_host.r_isco = isco_radius(cam->spin);
+    CK(cudaMemcpyAsync(c->d_model, &c->adaf_host, sizeof(AdafParams), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
   }
   return IPOLE_OK;
 }
@@ -619,6 +761,12 @@ int ipole_set_unpolarized(ipole_ctx* c, int32_t on) {
   return IPOLE_OK;
 }
 
+int ipole_set_transfer_split(ipole_ctx* c, int32_t on) {
+  if (!c) return IPOLE_EINVAL;
+  c->opt_split = (on == 2) ? 2 : (on ? 1 : 0);
+  return IPOLE_OK;
+}
+
 int ipole_set_path_free(ipole_ctx* c, int32_t on) {
   if (!c) return IPOLE_EINVAL;
   c->opt_path_free = on ? 1 : 0;
@@ -631,7 +779,8 @@ int ipole_load_model_adaf(ipole_ctx* c, const ipole_adaf_params* p) {
   AdafParams m;
   m.n0 = p->n0; m.p_n = p->p_n; m.Th0 = p->Th0; m.p_T = p->p_T; m.B0 = p->B0; m.p_B = p->p_B;
   m.r_isco = isco_radius(c->cam.G.a);
-  CK(cudaMemcpyAsync(c->d_model, &m, sizeof m, cudaMemcpyHostToDevice, c->stream));
+  c->adaf_host = m;
+  CK(cudaMemcpyAsync(c->d_model, &c->adaf_host, sizeof m, cudaMemcpyHostToDevice, c->stream));
   CK(cudaStreamSynchronize(c->stream));
   c->model = MODEL_ADAF;
   return IPOLE_OK;
@@ -771,9 +920,7 @@ int make_images(ipole_ctx* c, int model, int32_t n_models, const void* lane_tab,
   // the fluxes live at the start of the staging buffer; host outputs are staged behind them
   const size_t need = (size_t)n_models * 4 + (dev ? 0 : plane * 6);
   if (need > c->sweep_out_doubles) {
-    cudaFree(c->d_sweep_out); cudaFree(c->d_ada);
-  if (c->ev_ada0) cudaEventDestroy(c->ev_ada0);
-  if (c->ev_ada1) cudaEventDestroy(c->ev_ada1); c->d_sweep_out = nullptr; c->sweep_out_doubles = 0;
+    cudaFree(c->d_sweep_out); c->d_sweep_out = nullptr; c->sweep_out_doubles = 0;
     cudaError_t e = cudaMalloc(&c->d_sweep_out, need * sizeof(double));
     if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
     c->sweep_out_doubles = need;
@@ -985,7 +1132,7 @@ int ipole_get_stats(ipole_ctx* c, ipole_stats* out) {
     CK(cudaMemcpy(&f, c->d_sum, sizeof f, cudaMemcpyDeviceToHost));
     s.total_steps_forward = f;
   }
-  s.ms_probe = s.ms_geodesic = s.ms_transfer = s.ms_total = s.ms_long = 0.f;
+  s.ms_probe = s.ms_geodesic = s.ms_transfer = s.ms_total = s.ms_long = s.ms_stepop = s.ms_apply = 0.f;
   for (size_t i = 0; i < c->spans_used; ++i) {
     float ms = 0.f;
     if (cudaEventElapsedTime(&ms, c->spans[i].a, c->spans[i].b) != cudaSuccess) { cudaGetLastError(); continue; }
@@ -994,6 +1141,8 @@ int ipole_get_stats(ipole_ctx* c, ipole_stats* out) {
     else if (c->spans[i].kind == LK_GEO) s.ms_geodesic += ms;
     else if (c->spans[i].kind == LK_RT) s.ms_transfer += ms;
     else if (c->spans[i].kind == LK_LONG) s.ms_long += ms;
+    else if (c->spans[i].kind == LK_OPS) { s.ms_stepop += ms; s.ms_transfer += ms; }
+    else if (c->spans[i].kind == LK_APPLY) { s.ms_apply += ms; s.ms_transfer += ms; }
   }
   *out = s;
   return IPOLE_OK;
@@ -1132,6 +1281,7 @@ void ipole_free(ipole_ctx* c) {
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long);
   cudaFree(c->d_out); cudaFree(c->d_pixels); cudaFree(c->d_probe); cudaFree(c->d_queues); cudaFree(c->d_hist);
   cudaFree(c->d_small); cudaFree(c->d_part); cudaFree(c->d_red); cudaFree(c->d_endp); cudaFree(c->d_sum); cudaFree(c->d_sweep_models); cudaFree(c->d_sweep_units); cudaFree(c->d_sweep_out); cudaFree(c->d_ada);
+  cudaFree(c->d_ops); cudaFree(c->d_irr); cudaFree(c->d_retry);
   if (c->ev_ada0) cudaEventDestroy(c->ev_ada0);
   if (c->ev_ada1) cudaEventDestroy(c->ev_ada1);
   for (auto& s : c->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }

@@ -307,6 +307,8 @@ struct RtArgs {
   // or GridScales (grid model; `model` is the shared GridParams), `units_arr` at n_models Units; outputs of model m
   // start at plane + m * out_stride
   int n_models; const void* lane_tab; const Units* units_arr; size_t out_stride;
+  // work item -> slot of the batch (nullable: identity): the rays k_stepop left to this kernel (stepop.cuh)
+  const int32_t* slots;
 };
 
 constexpr int SWEEP_MAX_MODELS = 64;   // parameter sets per transfer launch (shared memory: <= 88 B each)
@@ -392,6 +394,7 @@ k_transfer(const __grid_constant__ RtArgs A) {
         li /= A.n_models;
         lane = lane_smem + (size_t)mi * LANE_BYTES;
       }
+      if (A.slots) li = A.slots[li];
       q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
       double dl;
       if (PF) {
@@ -646,16 +649,21 @@ struct SortArgs {
 
 __global__ void k_predict_hist(SortArgs A) {
   for (int64_t q = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; q < A.n; q += (int64_t)gridDim.x * blockDim.x) {
-    int pi;
+    int pr;
     if (A.lattice_stride > 0) {
+      // the longest of the four probe rays around the pixel (lattice point (ix, iy) is pixel (ix + 1/2) * stride):
+      // next to the photon ring the step count jumps by a factor of two to three within one lattice cell, and the
+      // per-batch path slots (run_rays) are sized from this prediction
       const int64_t pix = A.pixels ? A.pixels[q] : q;
-      int ix = (int)(pix % A.nx) / A.lattice_stride, iy = (int)(pix / A.nx) / A.lattice_stride;
-      ix = min(ix, A.lattice_nx - 1); iy = min(iy, A.lattice_ny - 1);
-      pi = iy * A.lattice_nx + ix;
+      const int px = (int)(pix % A.nx) - A.lattice_stride / 2, py = (int)(pix / A.nx) - A.lattice_stride / 2;
+      const int ix0 = min(max(px, 0) / A.lattice_stride, A.lattice_nx - 1), iy0 = min(max(py, 0) / A.lattice_stride, A.lattice_ny - 1);
+      const int ix1 = min(ix0 + 1, A.lattice_nx - 1), iy1 = min(iy0 + 1, A.lattice_ny - 1);
+      pr = max(max(A.probe[iy0 * A.lattice_nx + ix0], A.probe[iy0 * A.lattice_nx + ix1]),
+               max(A.probe[iy1 * A.lattice_nx + ix0], A.probe[iy1 * A.lattice_nx + ix1]));
     } else {
-      pi = (int)(q / A.list_stride);
+      pr = A.probe[(int)(q / A.list_stride)];
     }
-    const int pred = A.probe[pi] * A.scale;
+    const int pred = pr * A.scale;
     int bin = SORT_BINS - 1 - min(pred / A.bin_width, SORT_BINS - 1);
     A.key[q] = bin;
     atomicAdd(&A.hist[bin], 1u);

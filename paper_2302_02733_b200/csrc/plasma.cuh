@@ -44,12 +44,21 @@ __device__ __forceinline__ double dotg(const Sym7& g, const double u[4], const d
   return dot4(l, v);
 }
 
+// the three power laws of the analytic flow at X1 = ln r
+__device__ __forceinline__ void adaf_scalars(const AdafParams& M, double x1, double& ne, double& Th, double& B) {
+  ne = M.n0 * ip_exp(M.p_n * x1);
+  Th = M.Th0 * ip_exp(M.p_T * x1);
+  B = M.B0 * ip_exp(M.p_B * x1);
+}
+
+// SCALARS = false: flow velocity and field DIRECTION only (b is a unit vector, P.B = 1; n_e, Theta_e are not set):
+// what the tetrad and the pitch angle need (k_stepop; the scalars are evaluated where the coefficients are, k_apply)
+template <bool SCALARS = true>
 __device__ __forceinline__ bool plasma_adaf(const Geom& G, const AdafParams& M, const double X[4], const Point& p,
                                             const Sym7& g, const Inv6& gi, Plasma& P) {
   const double a = G.a, r = p.r;
-  P.ne = M.n0 * ip_exp(M.p_n * X[1]);
-  P.Th = M.Th0 * ip_exp(M.p_T * X[1]);
-  P.B = M.B0 * ip_exp(M.p_B * X[1]);
+  if (SCALARS) adaf_scalars(M, X[1], P.ne, P.Th, P.B);
+  else { P.ne = 0.0; P.Th = 0.0; P.B = 1.0; }
   if (r >= M.r_isco) {
     const double Om = ip_rcp(r * ip_sqrt(r) + a);
     const double ut = ip_rsqrt(-(g.c00 + 2.0 * g.c03 * Om + g.c33 * Om * Om));
@@ -256,18 +265,19 @@ struct PlasmaFrame {
   double j[4], al[4], rh[3];     // slab only (cgs)
 };
 
-// Plasma state and tetrad at (X, K); on success the carried legs st.f1, st.f2 are REPLACED by the new transverse
-// legs e_(1), e_(2) and F holds what plasma_apply needs.  Returns false where there is no plasma (nothing changed).
+// Plasma state and plasma-frame tetrad at (X, K): what one step's plasma operator needs and what does NOT depend on
+// the polarization state carried along the ray -- the two transverse legs e_(1), e_(2) (contravariant and covariant
+// MKS components) and the fluid scalars, local frequency and pitch angle in F.  Returns false where there is no plasma.
 // `lane` (model sweep only, else nullptr): the lane's own parameter set -- AdafParams, or GridScales overriding the four
 // scale numbers of the shared GridParams.
-template <int MODEL>
-__device__ __forceinline__ bool plasma_frame(const Geom& G, const void* model, const void* lane, const Units& U, const double X[4],
-                                             const double K[4], const Point& p, const Sym7& g, const Inv6& gi,
-                                             const double* prim /* grid model: from grid_gather */, PolState& st,
-                                             PlasmaFrame& F) {
+template <int MODEL, bool SCALARS = true>
+__device__ __forceinline__ bool plasma_tetrad(const Geom& G, const void* model, const void* lane, const Units& U, const double X[4],
+                                              const double K[4], const Point& p, const Sym7& g, const Inv6& gi,
+                                              const double* prim /* grid model: from grid_gather */, double e1[4], double e2[4],
+                                              double e1c[4], double e2c[4], PlasmaFrame& F) {
   Plasma P;
   bool present;
-  if (MODEL == MODEL_ADAF) present = plasma_adaf(G, *(const AdafParams*)(lane ? lane : model), X, p, g, gi, P);
+  if (MODEL == MODEL_ADAF) present = plasma_adaf<SCALARS>(G, *(const AdafParams*)(lane ? lane : model), X, p, g, gi, P);
   else if (MODEL == MODEL_SLAB) present = plasma_slab(G, *(const SlabParams*)model, X, p, g, P);
   else {
     const GridParams& M = *(const GridParams*)model;
@@ -281,7 +291,7 @@ __device__ __forceinline__ bool plasma_frame(const Geom& G, const void* model, c
   g.mul(P.u, ucov);
   const double om = -dot4(kcov, P.u);
   if (!(om > 0.0)) return false;
-  double e3[4], e2[4], e1[4], e3c[4], e2c[4], e1c[4];
+  double e3[4], e3c[4];
   const double iom = ip_rcp(om);
 #pragma unroll
   for (int m = 0; m < 4; ++m) e3[m] = K[m] * iom - P.u[m];
@@ -319,6 +329,19 @@ __device__ __forceinline__ bool plasma_frame(const Geom& G, const void* model, c
     g.mul(P.b, bcov);
     F.cosT = fmin(1.0, fmax(-1.0, dot4(bcov, K) * iom * ip_rcp(P.B)));
   }
+  return true;
+}
+
+// The same for the sequential kernels: on success the carried legs st.f1, st.f2 are REPLACED by the new transverse
+// legs and F also holds the 2x2 projection of the old legs on the new ones.  Returns false where there is no plasma
+// (nothing changed).
+template <int MODEL>
+__device__ __forceinline__ bool plasma_frame(const Geom& G, const void* model, const void* lane, const Units& U, const double X[4],
+                                             const double K[4], const Point& p, const Sym7& g, const Inv6& gi,
+                                             const double* prim /* grid model: from grid_gather */, PolState& st,
+                                             PlasmaFrame& F) {
+  double e1[4], e2[4], e1c[4], e2c[4];
+  if (!plasma_tetrad<MODEL>(G, model, lane, U, X, K, p, g, gi, prim, e1, e2, e1c, e2c, F)) return false;
   F.m11 = dot4(e1c, st.f1); F.m12 = dot4(e1c, st.f2); F.m21 = dot4(e2c, st.f1); F.m22 = dot4(e2c, st.f2);
 #pragma unroll
   for (int m = 0; m < 4; ++m) { st.f1[m] = e1[m]; st.f2[m] = e2[m]; }

@@ -1,0 +1,256 @@
+// Transfer split in two kernels (SURVEY.md section 8(a) rows a-4 ... a-7; "at every single step ...
+// evaluate emission, self-absorption and Faraday coefficients at a given point").
+//
+// Along a stored path everything a transfer step needs -- the midpoint metric and transport generator, the plasma
+// state, the plasma-frame tetrad, the eight coefficients -- depends on the two end points of that step alone, not on
+// the polarization state carried by the ray.  Even the 2x2 projection M of the carried legs on a step's new tetrad is
+// state-free as long as the previous (farther) step also crossed plasma: the carried legs are then that step's own
+// tetrad legs, transported by its P and by this step's P ("factorised coherency tensor").  What
+// is sequential is only   S <- C(M) S,   S <- O S + P J   on four Stokes numbers.  So:
+//
+//   k_stepop  one thread per STEP (a warp takes 31 consecutive steps of one ray plus one halo step, lanes <-> steps):
+//             metric, generator, flow, tetrad, leg transport; writes one 64-B operator record per step:
+//             M (4), and what the coefficients need: ln r, cos(pitch angle), local frequency, ds.  No loop-carried state.
+//   k_apply   one warp per 32 RAYS, lane <-> ray, in lockstep from the far end to the camera: plasma scalars, the eight
+//             coefficients, congruence + the analytic 4x4 step, then the camera projection.  Its record stream (64 B per
+//             step, coalesced) runs at HBM speed; the coefficient arithmetic lives here because this kernel has the
+//             registers to spare for 5 warps per scheduler, which the geometry kernel has not.
+//
+// A ray with a step that is NOT applied (no plasma there, or a degenerate tetrad) breaks the state-free chain of the
+// legs; k_stepop lists such rays (`irregular`) and the single-kernel k_transfer renders them from the same path
+// buffer.  With the analytic ADAF flow every step crosses plasma, so the list is empty in practice.
+#pragma once
+#include "kernels.cuh"
+
+namespace ipole {
+
+constexpr int OP_PARTS = 2;        // operator record: two 32-B parts, {M11, M12, M21, M22} and {ln r, cos theta_B, nu, ds}
+constexpr int OP_DOUBLES = 4 * OP_PARTS;
+
+// Layout of the operator records of a batch: rays are taken in groups of 32 consecutive slots (one k_apply warp walks
+// a group in lockstep, lane <-> ray), and the record of (slot li, step s) is cut in OP_PARTS 32-byte parts j:
+//   ops[ (((li/32) * (cap+1) + s) * OP_PARTS + j) * 32 + li%32 ][4 doubles]
+// so that for one step the 32 lanes of k_apply read OP_PARTS x 1 KB of contiguous memory (8 full lines per 256-bit load
+// instead of 32 partial ones), while k_stepop -- lanes <-> consecutive steps of one ray -- writes full 32-B sectors.
+__device__ __forceinline__ size_t op_addr(int64_t li, int cap, int s, int j) {
+  return ((((size_t)(li >> 5) * (size_t)(cap + 1) + (size_t)s) * OP_PARTS + j) * 32 + (size_t)(li & 31)) * 4;
+}
+
+struct OpArgs {
+  CamDev cam;
+  Units units;
+  const void* model;          // device pointer to AdafParams
+  int cap;                    // steps per slot (records = cap + 1) of both the path and the operator buffer
+  int64_t base, count;        // rays [base, base+count) of the order
+  const int32_t* order;
+  const double* path;         // [count][cap+1][8]
+  const int32_t* nsteps;      // indexed by q; -1 = overflowed its slot (long-ray pass)
+  unsigned long long* queue;
+  double* ops;                // operator records of the batch, layout op_addr(); record n of a ray: camera projection (4), irregular flag (1)
+  int32_t* irr_slots; int* irr_count;   // slots (positions in the batch) of the rays left to k_transfer
+  int test_irregular;         // tests: declare every 7th slot irregular, so that the hand-over to k_transfer is exercised
+};
+
+#ifndef IPOLE_OP_THREADS
+#define IPOLE_OP_THREADS 128
+#endif
+#ifndef IPOLE_OP_MINB
+#define IPOLE_OP_MINB 3
+#endif
+
+__device__ __forceinline__ void shfl_down4(const double v[4], double o[4]) {
+#pragma unroll
+  for (int m = 0; m < 4; ++m) o[m] = __shfl_down_sync(0xffffffffu, v[m], 1);
+}
+
+template <int MODEL>
+__global__ void __launch_bounds__(IPOLE_OP_THREADS, IPOLE_OP_MINB) k_stepop(const __grid_constant__ OpArgs A) {
+  static_assert(MODEL == MODEL_ADAF, "the step-parallel pass is built for the analytic flow");
+  const CamDev& C = A.cam;
+  __shared__ __align__(8) unsigned char model_smem[sizeof(AdafParams)];
+  for (int i = threadIdx.x; i < (int)sizeof(AdafParams); i += blockDim.x) model_smem[i] = ((const unsigned char*)A.model)[i];
+  __syncthreads();
+  const void* model = model_smem;
+  const int lane = threadIdx.x & 31;
+  const size_t slot_rec = (size_t)(A.cap + 1) * REC_DOUBLES;
+
+  for (;;) {
+    // lane 0 leaves the previous iteration later than the others (it writes the ray's last record): without this
+    // the warp stays split in 1 + 31 threads and issues every instruction of the body twice
+    __syncwarp();
+    long long li = 0;
+    if (lane == 0) li = (long long)atomicAdd(A.queue, 1ULL);
+    li = __shfl_sync(0xffffffffu, li, 0);
+    if (li >= A.count) break;
+    const int32_t q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
+    const int n = A.nsteps[q];
+    if (n < 0) continue;                     // overflowed its slot: done by the long-ray pass
+    const double* rec = A.path + (size_t)li * slot_rec;
+    bool regular = true;
+    double mc[4] = {0.0, 0.0, 0.0, 0.0};     // lane 0, first chunk: projection of step 0's legs on the camera tetrad
+
+    for (int s0 = 0; s0 < n; s0 += 31) {
+      const int s = s0 + lane;               // step s: from point s+1 to point s (point 0 = camera)
+      const bool act = s < n;
+      // the next chunk's records (lane l: points s0+31+l and, for the halo lane, one more) into L1 while this one computes
+      if (s + 31 <= n) asm volatile("prefetch.global.L1 [%0];" ::"l"(rec + (size_t)(s + 31) * REC_DOUBLES));
+      if (lane == 31 && s + 32 <= n) asm volatile("prefetch.global.L1 [%0];" ::"l"(rec + (size_t)(s + 32) * REC_DOUBLES));
+      // fo: this step's new legs after its second half transport, P e_(a): what the next step towards the camera receives
+      double fo1[4] = {0, 0, 0, 0}, fo2[4] = {0, 0, 0, 0};
+      double e1c[4], e2c[4], Am[4][4];
+      double h = 0.0, dl = 0.0, x1m = 0.0;
+      PlasmaFrame F;
+      bool applied = false;
+      if (act) {
+        double Xm[4], Km[4];
+        {
+          double Xlo[4], Klo[4], Xhi[4], Khi[4], dlh;
+          load_record(rec + (size_t)s * REC_DOUBLES, Xlo, Klo, dl);
+          load_record(rec + (size_t)(s + 1) * REC_DOUBLES, Xhi, Khi, dlh);
+#pragma unroll
+          for (int m = 0; m < 4; ++m) { Xm[m] = 0.5 * (Xlo[m] + Xhi[m]); Km[m] = 0.5 * (Klo[m] + Khi[m]); }
+        }
+        x1m = Xm[1];
+        Point p; Sym7 g; Inv6 gi;
+        transport_generator(C.G, Xm, Km, p, g, gi, Am);
+        h = 0.5 * dl;
+        double e1[4], e2[4];
+        applied = plasma_tetrad<MODEL, false>(C.G, model, nullptr, A.units, Xm, Km, p, g, gi, nullptr, e1, e2, e1c, e2c, F);
+        if (applied) {
+#pragma unroll
+          for (int m = 0; m < 4; ++m) { fo1[m] = e1[m]; fo2[m] = e2[m]; }
+          transport_apply(Am, h, fo1);
+          transport_apply(Am, h, fo2);
+        }
+      }
+      regular &= (applied || !act);
+      // legs arriving at step s = legs leaving step s+1 (the neighbouring lane)
+      double fi1[4], fi2[4];
+      shfl_down4(fo1, fi1);
+      shfl_down4(fo2, fi2);
+      if (act && lane < 31) {
+        double m11 = 0.0, m12 = 0.0, m21 = 0.0, m22 = 0.0;
+        if (s < n - 1 && applied) {          // the far end starts dark: nothing arrives there
+          transport_apply(Am, h, fi1);
+          transport_apply(Am, h, fi2);
+          m11 = dot4(e1c, fi1); m12 = dot4(e1c, fi2); m21 = dot4(e2c, fi1); m22 = dot4(e2c, fi2);
+        }
+        double* o = A.ops + op_addr(li, A.cap, s, 0);   // part 1 at o + 128
+        st_global_v4(o, m11, m12, m21, m22);
+        st_global_v4(o + 128, x1m, applied ? F.cosT : 0.0, applied ? F.nu : 0.0, dl * A.units.dl_unit);
+        if (s == 0) {
+          mc[0] = dot4(C.ecov1, fo1); mc[1] = dot4(C.ecov1, fo2); mc[2] = dot4(C.ecov2, fo1); mc[3] = dot4(C.ecov2, fo2);
+        }
+      }
+    }
+    regular = __all_sync(0xffffffffu, regular) && !(A.test_irregular && (li % 7) == 3);
+    if (lane == 0) {
+      double* o = A.ops + op_addr(li, A.cap, n, 0);
+      st_global_v4(o, mc[0], mc[1], mc[2], mc[3]);
+      st_global_v4(o + 128, regular ? 0.0 : 1.0, 0.0, 0.0, 0.0);
+      if (!regular) { const int w = atomicAdd(A.irr_count, 1); A.irr_slots[w] = (int32_t)li; }
+    }
+  }
+}
+
+struct ApArgs {
+  AdafParams model;           // the three power laws (by value: 56 B)
+  double nu3;                 // nu_obs^3: invariant I/nu^3 -> specific intensity at the camera
+  int cap;
+  int64_t base, count;
+  const int32_t* order;
+  const double* ops;
+  const int32_t* nsteps;
+  unsigned long long* queue;
+  double *I, *Q, *U, *V, *tau, *tauF;   // indexed by q
+};
+
+#ifndef IPOLE_AP_THREADS
+#define IPOLE_AP_THREADS 128
+#endif
+#ifndef IPOLE_AP_MINB
+#define IPOLE_AP_MINB 4
+#endif
+
+// a step that is not thin (never on the analytic workloads): the closed form, kept out of the slim loop.  Stokes in
+// and out by value, so that the caller's S stays in registers.
+struct Stokes4 { double I, Q, U, V; };
+__device__ __noinline__ Stokes4 stokes_step_qv_closed(double aI, double aQ, double aV, double rQ, double rV, double jI, double jQ,
+                                                      double jV, Stokes4 in) {
+  double S[4] = {in.I, in.Q, in.U, in.V};
+  stokes_step_qv<false>(aI, aQ, aV, rQ, rV, 1.0, jI, jQ, jV, S);
+  Stokes4 o = {S[0], S[1], S[2], S[3]};
+  return o;
+}
+
+// One warp walks a group of 32 consecutive slots of the batch in lockstep, lane <-> ray, from the longest ray's far end
+// to the camera; a lane joins when the walk reaches its own far end.  Rays are ordered by predicted step count, so
+// the 32 rays of a group have similar lengths.  The record of the next step is loaded (three coalesced 256-bit loads)
+// while the current one is applied.
+__global__ void __launch_bounds__(IPOLE_AP_THREADS, IPOLE_AP_MINB) k_apply(const __grid_constant__ ApArgs A) {
+  const int lane = threadIdx.x & 31;
+  const int64_t n_groups = (A.count + 31) >> 5;
+  for (;;) {
+    __syncwarp();
+    long long g = 0;
+    if (lane == 0) g = (long long)atomicAdd(A.queue, 1ULL);
+    g = __shfl_sync(0xffffffffu, g, 0);
+    if (g >= n_groups) break;
+    const int64_t li = (g << 5) + lane;
+    int32_t q = 0;
+    int n = 0;                                   // steps of this lane's ray; 0: nothing to do
+    double mc[4] = {0, 0, 0, 0};
+    if (li < A.count) {
+      q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
+      n = A.nsteps[q];
+      if (n < 0) n = 0;                          // overflowed its slot: long-ray pass
+      else {
+        double flag, z0, z1, z2;
+        ld_global_v4(A.ops + op_addr(li, A.cap, n, 0), mc[0], mc[1], mc[2], mc[3]);
+        ld_global_v4(A.ops + op_addr(li, A.cap, n, 1), flag, z0, z1, z2);
+        if (flag != 0.0) n = 0;                  // irregular: rendered by k_transfer
+      }
+    }
+    int smax = n;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) smax = max(smax, __shfl_xor_sync(0xffffffffu, smax, o));
+    double S[4] = {0, 0, 0, 0}, tau = 0.0, tauF = 0.0;
+    double R[OP_DOUBLES] = {0, 0, 0, 0, 0, 0, 0, 0};
+    const double* base = A.ops + op_addr(li, A.cap, 0, 0);   // step s, part j at base + (s*OP_PARTS + j) * 128
+    auto load = [&](int s) {
+      const double* p = base + (size_t)s * (OP_PARTS * 128);
+      ld_global_v4(p, R[0], R[1], R[2], R[3]);
+      ld_global_v4(p + 128, R[4], R[5], R[6], R[7]);
+    };
+    if (smax - 1 < n) load(smax - 1);
+    for (int s = smax - 1; s >= 0; --s) {
+      const bool on = s < n;
+      const double m11 = R[0], m12 = R[1], m21 = R[2], m22 = R[3];
+      const double x1 = R[4], cosT = R[5], nu = R[6], ds = R[7];
+      if (s > 0 && s - 1 < n) load(s - 1);
+      if (on) {
+        stokes_congruence(m11, m12, m21, m22, S);
+        double ne, Th, B;
+        adaf_scalars(A.model, x1, ne, Th, B);
+        const Coeff c = synchrotron_invariant(ne, Th, B, cosT, nu);
+        const double xI = c.aI * ds, xQ = c.aQ * ds, xV = c.aV * ds, yQ = c.rQ * ds, yV = c.rV * ds;
+        const double eI = c.jI * ds, eQ = c.jQ * ds, eV = c.jV * ds;
+        if (IP_UNLIKELY(!stokes_step_qv_series(xI, xQ, xV, yQ, yV, 1.0, eI, eQ, eV, S))) {
+          const Stokes4 in = {S[0], S[1], S[2], S[3]};
+          const Stokes4 o = stokes_step_qv_closed(xI, xQ, xV, yQ, yV, eI, eQ, eV, in);
+          S[0] = o.I; S[1] = o.Q; S[2] = o.U; S[3] = o.V;
+        }
+        tau += xI;
+        tauF += fabs(yV);
+      }
+    }
+    if (n > 0) {
+      stokes_congruence(mc[0], mc[1], mc[2], mc[3], S);
+      A.I[q] = S[0] * A.nu3; A.Q[q] = S[1] * A.nu3; A.U[q] = S[2] * A.nu3; A.V[q] = S[3] * A.nu3;
+      if (A.tau) A.tau[q] = tau;
+      if (A.tauF) A.tauF[q] = tauF;
+    }
+  }
+}
+
+}  // namespace ipole

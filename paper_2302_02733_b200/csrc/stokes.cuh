@@ -128,46 +128,49 @@ __device__ __forceinline__ void stokes_step(const double al[4], const double rh[
 //   outx = Ax V0 + (P1 + Dxx) x + B2 y + Dxz z          G = c4 (r x a)_U,  D = c4 (a a^T + r r^T)
 //   outy = -G V0 - B2 x + P1 y + B0 z
 //   outz = Az V0 + Dxz x - B0 y + (P1 + Dzz) z
+// Thin step: || Kmat s ||_inf <= nb < 2^-7.  S(s) solves S' = J - Kmat S with constant coefficients, so
+//   S(s) = S0 + sum_{n>=1} w_n,   w_1 = s (J - Kmat S0),   w_{n+1} = -(s/(n+1)) Kmat w_n,
+// one chain of sparse 4x4 products for O S0 and P J together, no transcendentals and no divisions.  At most seven
+// terms: the first dropped one is below nb^7/8! < 5e-20 of w_1.  This is the same matrix exponential the closed form
+// evaluates (R-8).  Every step of the analytic ADAF workloads is thin (per-step optical and Faraday
+// depths <= 1e-3).  Returns false (S untouched) when the step is not thin: the caller uses the closed form.
+__device__ __forceinline__ bool stokes_step_qv_series(double aI, double aQ, double aV, double rQ, double rV, double s,
+                                                      double jI, double jQ, double jV, double S[4]) {
+  const double nb = fabs(s) * (fabs(aI) + fabs(aQ) + fabs(aV) + fabs(rQ) + fabs(rV));
+  if (IP_UNLIKELY(!(nb < 0.0078125))) return false;
+  double w0 = s * (jI - (aI * S[0] + aQ * S[1] + aV * S[3]));
+  double w1 = s * (jQ - (aQ * S[0] + aI * S[1] + rV * S[2]));
+  double w2 = s * (rV * S[1] - aI * S[2] - rQ * S[3]);
+  double w3 = s * (jV - (aV * S[0] - rQ * S[2] + aI * S[3]));
+  double o0 = w0, o1 = w1, o2 = w2, o3 = w3;
+  // The chain is cut where the first dropped term is below 2e-17 of w_1: three terms for nb < 2^-17, five for
+  // nb < 2^-10, seven otherwise.  Most steps of the ADAF workloads are in the lowest tier, and a warp whose lanes
+  // all are skips the rest of the chain.
+  auto term = [&](int n) {
+    const double c = -s * (1.0 / (double)n);
+    const double t0 = aI * w0 + aQ * w1 + aV * w3;
+    const double t1 = aQ * w0 + aI * w1 + rV * w2;
+    const double t2 = aI * w2 - rV * w1 + rQ * w3;
+    const double t3 = aV * w0 - rQ * w2 + aI * w3;
+    w0 = c * t0; w1 = c * t1; w2 = c * t2; w3 = c * t3;
+    o0 += w0; o1 += w1; o2 += w2; o3 += w3;
+  };
+  term(2); term(3);
+  if (nb >= 7.62939453125e-06) {          // 2^-17: (2^-17)^3 / 4! = 1.8e-17
+    term(4); term(5);
+    if (nb >= 9.765625e-4) { term(6); term(7); }   // 2^-10: (2^-10)^5 / 6! = 1.2e-18
+  }
+  S[0] += o0; S[1] += o1; S[2] += o2; S[3] += o3;
+  return true;
+}
+
+// THIN_SERIES: try the series first.  The grid model keeps the closed form alone: its plasma steps are 1 in 8 and
+// reach depths of order one, and the extra code cost more than it saved there (profiles/r1_notes.md).
 template <bool THIN_SERIES>
 __device__ __forceinline__ void stokes_step_qv(double aI, double aQ, double aV, double rQ, double rV, double s,
                                                double jI, double jQ, double jV, double S[4]) {
-  // Thin step (THIN_SERIES): || Kmat s ||_inf <= nb < 2^-7.  S(s) solves S' = J - Kmat S with constant
-  // coefficients, so
-  //   S(s) = S0 + sum_{n>=1} w_n,   w_1 = s (J - Kmat S0),   w_{n+1} = -(s/(n+1)) Kmat w_n,
-  // one chain of sparse 4x4 products for O S0 and P J together, no transcendentals and no divisions.  At most seven
-  // terms: the first dropped one is below nb^7/8! < 5e-20 of w_1.  This is the same matrix exponential the closed form
-  // evaluates (R-8).  Every step of the analytic ADAF workloads is thin (per-step optical and Faraday
-  // depths <= 1e-3); the closed form below serves the rest.  The grid model keeps the closed form alone: its
-  // plasma steps are 1 in 8 and reach depths of order one, and the extra code cost more than it saved there
-  // (profiles/r1_notes.md).
   if (THIN_SERIES) {
-    const double nb = fabs(s) * (fabs(aI) + fabs(aQ) + fabs(aV) + fabs(rQ) + fabs(rV));
-    if (IP_LIKELY(nb < 0.0078125)) {
-      double w0 = s * (jI - (aI * S[0] + aQ * S[1] + aV * S[3]));
-      double w1 = s * (jQ - (aQ * S[0] + aI * S[1] + rV * S[2]));
-      double w2 = s * (rV * S[1] - aI * S[2] - rQ * S[3]);
-      double w3 = s * (jV - (aV * S[0] - rQ * S[2] + aI * S[3]));
-      double o0 = w0, o1 = w1, o2 = w2, o3 = w3;
-      // The chain is cut where the first dropped term is below 2e-17 of w_1: three terms for nb < 2^-17, five for
-      // nb < 2^-10, seven otherwise.  Most steps of the ADAF workloads are in the lowest tier, and a warp whose lanes
-      // all are skips the rest of the chain.
-      auto term = [&](int n) {
-        const double c = -s * (1.0 / (double)n);
-        const double t0 = aI * w0 + aQ * w1 + aV * w3;
-        const double t1 = aQ * w0 + aI * w1 + rV * w2;
-        const double t2 = aI * w2 - rV * w1 + rQ * w3;
-        const double t3 = aV * w0 - rQ * w2 + aI * w3;
-        w0 = c * t0; w1 = c * t1; w2 = c * t2; w3 = c * t3;
-        o0 += w0; o1 += w1; o2 += w2; o3 += w3;
-      };
-      term(2); term(3);
-      if (nb >= 7.62939453125e-06) {          // 2^-17: (2^-17)^3 / 4! = 1.8e-17
-        term(4); term(5);
-        if (nb >= 9.765625e-4) { term(6); term(7); }   // 2^-10: (2^-10)^5 / 6! = 1.2e-18
-      }
-      S[0] += o0; S[1] += o1; S[2] += o2; S[3] += o3;
-      return;
-    }
+    if (stokes_step_qv_series(aI, aQ, aV, rQ, rV, s, jI, jQ, jV, S)) return;
   }
   const double m = fmax(fmax(fabs(aQ), fabs(aV)), fmax(fabs(rQ), fabs(rV)));
   const double t0 = ip_expm1(-aI * s);

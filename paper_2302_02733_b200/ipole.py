@@ -17,7 +17,7 @@ _LIB = None
 OK, EINVAL, ENOMODEL, ENOMEM, ECUDA, ENOIMAGE = 0, -1, -2, -3, -4, -5
 
 #: every symbol include/ipole.h declares (checked by tests/test_abi.py)
-SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_options", "ipole_set_path_free", "ipole_set_unpolarized", "ipole_load_model_adaf",
+SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_options", "ipole_set_path_free", "ipole_set_transfer_split", "ipole_set_unpolarized", "ipole_load_model_adaf",
            "ipole_load_model_slab", "ipole_load_model_grid", "ipole_make_image", "ipole_make_pixels", "ipole_make_images_adaf", "ipole_make_images_grid", "ipole_make_image_adaptive",
            "ipole_get_ray_info", "ipole_get_stats", "ipole_get_camera_tetrad", "ipole_trace_pixel",
            "ipole_eval_connection", "ipole_eval_coefficients", "ipole_eval_stokes_step", "ipole_eval_bessel",
@@ -53,7 +53,7 @@ class Stats(C.Structure):
                 ("max_steps_seen", C.c_int32), ("path_cap", C.c_int32), ("n_ring", C.c_int64),
                 ("n_maxstep", C.c_int64), ("n_long", C.c_int64), ("n_batches", C.c_int32), ("n_launches", C.c_int32),
                 ("ms_probe", C.c_float), ("ms_geodesic", C.c_float), ("ms_transfer", C.c_float), ("ms_total", C.c_float),
-                ("ms_long", C.c_float), ("total_steps_forward", C.c_int64)]
+                ("ms_long", C.c_float), ("total_steps_forward", C.c_int64), ("ms_stepop", C.c_float), ("ms_apply", C.c_float), ("n_retry", C.c_int64)]
 
 
 class GridScales(C.Structure):
@@ -86,6 +86,7 @@ def lib():
         L.ipole_set_options.argtypes = [vp, C.c_uint64, C.c_int32]
         L.ipole_set_path_free.argtypes = [vp, C.c_int32]
         L.ipole_set_unpolarized.argtypes = [vp, C.c_int32]
+        L.ipole_set_transfer_split.argtypes = [vp, C.c_int32]
         L.ipole_load_model_adaf.argtypes = [vp, C.POINTER(AdafParams)]
         L.ipole_load_model_slab.argtypes = [vp, C.POINTER(SlabParams)]
         L.ipole_load_model_grid.argtypes = [vp, C.POINTER(GridDesc), C.POINTER(vp)]
@@ -180,6 +181,10 @@ class Ipole:
     def set_path_free(self, on=True):
         """Path-free bidirectional variant: no stored path, forward re-integration (include/ipole.h)."""
         _chk(lib().ipole_set_path_free(self._h, 1 if on else 0), "ipole_set_path_free")
+
+    def set_transfer_split(self, on=True):
+        """Transfer as a step-parallel operator pass + a per-ray apply pass (include/ipole.h ipole_set_transfer_split)."""
+        _chk(lib().ipole_set_transfer_split(self._h, int(on)), "ipole_set_transfer_split")
 
     def set_unpolarized(self, on=True):
         """Unpolarized transfer of I alone (include/ipole.h ipole_set_unpolarized)."""

@@ -145,6 +145,7 @@ def test_w2_adaf_256_sampled(ipole, ref, freq):
 def test_batching_sorting_and_long_ray_pass_are_bit_neutral(ipole):
     cam = W.camera("adaf", 48, max_steps=6000)
     g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
+    g.set_transfer_split(False)   # the long-ray pass is always the single kernel: compare like with like
     base = to_np(g.make_image(maps=True)); st0 = g.stats()
     assert st0["n_batches"] == 1 and st0["n_long"] == 0
     # forced probe + sort, default budget
@@ -164,6 +165,36 @@ def test_batching_sorting_and_long_ray_pass_are_bit_neutral(ipole):
             assert np.array_equal(base[k], other[k]), k
     for st in (st1, st2, st3):
         assert st["total_steps"] == st0["total_steps"] and st["flux_jy"] == st0["flux_jy"]
+
+
+def test_split_transfer_matches_the_single_kernel(ipole):
+    """k_stepop + k_apply against k_transfer on the same stored paths: rounding-level agreement per pixel, the same
+    under batching with per-batch slots and the retry level, and with every seventh ray handed over to k_transfer."""
+    cam = W.camera("adaf", 64)
+    g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
+    g.set_transfer_split(False)
+    one = to_np(g.make_image(maps=True))
+    g.set_transfer_split(True)
+    two = to_np(g.make_image(maps=True)); st = g.stats()
+    assert st["ms_stepop"] > 0 and st["ms_apply"] > 0
+    scale = np.abs(one["I"]) + 1e-300
+    for k in ("I", "Q", "U", "V"):
+        assert np.max(np.abs(one[k] - two[k]) / scale) < 1e-11, k
+    assert np.allclose(one["tau"], two["tau"], rtol=1e-12, atol=0) and np.allclose(one["tauF"], two["tauF"], rtol=1e-12, atol=0)
+    # many batches with slots sized from the predicted step counts; some rays outgrow them and are retried
+    g.set_options(48 << 20, 2)
+    three = to_np(g.make_image(maps=True)); st3 = g.stats()
+    assert st3["n_batches"] > 3
+    for k in two:
+        assert np.array_equal(two[k], three[k]), k
+    g.set_options(0, 1)
+    g.set_transfer_split(2)
+    four = to_np(g.make_image(maps=True))
+    changed = 0
+    for k in ("I", "Q", "U", "V"):
+        assert np.max(np.abs(four[k] - two[k]) / scale) < 1e-11, k
+        changed += int((four[k] != two[k]).sum())
+    assert changed > 0   # the handed-over rays really went through the other kernel
 
 
 def test_step_limit_flags_rays(ipole, ref):
