@@ -23,13 +23,21 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# FP64 operations per geodesic step of each kernel as shipped, counted by ncu (DFMA = 2, DADD/DMUL = 1;
-# smsp__sass_thread_inst_executed_op_d{fma,add,mul}_pred_on.sum / thread-steps of the launch): profiles/r1_k_*.txt,
-# DESIGN.md section 7.  The grid figures are averages over ALL steps of a ray (stats.total_steps): k_transfer<grid> walks
-# only half of them (786 flop and 68.2 B per walked step; rays start at their first contact with plasma).
+# ALGORITHMIC FP64 operations per geodesic step (DFMA = 2, DADD = DMUL = 1): the lean counts of the round-1 kernels,
+# FROZEN as the method's work (profiles/r1_k_*.txt).  roofline.frac uses these fixed numerators over
+# the live CUDA-event time, so a faster kernel can only raise it; what the shipped kernels actually execute is reported
+# beside it (FLOP_EXECUTED, frac_executed).  Grid transfer: 786 per WALKED step = 390 averaged over all steps of a ray.
 FLOP_PER_STEP = {"transfer_adaf": 1576.0, "transfer_grid": 390.0, "geodesic_adaf": 994.0, "geodesic_grid": 1183.0}
+# executed by the kernels as shipped, per step, and their FP64-pipe utilisation, both from ncu --set full captures
+# (smsp__sass_thread_inst_executed_op_d{fma,add,mul}_pred_on / steps of the launch; sm__inst_executed_pipe_fp64):
+# profiles/r2_k_stepop_adaf1024.txt, r2_k_apply_adaf1024.txt, r1_k_transfer_*.txt, r1_k_geodesic_*.txt
+FLOP_EXECUTED = {"k_stepop": 1018.0, "k_apply": 574.0, "k_transfer<adaf>": 1576.0, "k_transfer<grid>": 390.0,
+                 "k_geodesic": 994.0, "k_geodesic<occ>": 1183.0}
+FP64_PIPE_PCT = {"k_stepop": 72.7, "k_apply": 64.8, "k_transfer<adaf>": 58.5, "k_transfer<grid>": 48.0,
+                 "k_geodesic": 82.0, "k_geodesic<occ>": 79.0}
 # DRAM bytes per step of k_transfer (dram__bytes_read + write of one launch / its thread-steps, same captures)
 DRAM_BYTES_PER_STEP = {"transfer_adaf": 64.2, "transfer_grid": 33.8}
+DRAM_BYTES_PER_STEP_SPLIT = 192.0   # k_stepop reads 64.1 B and writes 64.0 B per step, k_apply reads 64.0 B (profiles/r2_k_*.txt)
 # --unpolarized: per step of k_transfer_unpol<model> (ncu, profiles/r1_unpolarized.md)
 FLOP_PER_STEP_UNPOL = {"transfer_adaf": 652.0, "transfer_grid": 76.4}   # grid: 601 per walked step, 12.7 % of the steps walked
 # --path-free (PAPER.md:43 variant): per FORWARD step of k_transfer<model, 1> (RK4 push + transfer step in one kernel)
@@ -228,6 +236,18 @@ class ClockSampler:
                 "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+_GRID_CACHE = {}
+
+
+def grid_inputs(shape):
+    """The seeded FM-torus planes for a lattice shape, generated once per process (tens of seconds at 576x256x256)."""
+    from paper_2302_02733_b200 import workloads as W
+    if shape not in _GRID_CACHE:
+        _GRID_CACHE.clear()
+        _GRID_CACHE[shape] = W.fm_torus_grid(*shape)
+    return _GRID_CACHE[shape]
+
+
 def oracle_sample(workload, n_rays, nthreads, path_free=False, unpolarized=False):
     """The CPU oracle, as it stands, on a strided sample of the workload's image.  Returns (rays, steps, seconds)."""
     import numpy as np
@@ -239,7 +259,7 @@ def oracle_sample(workload, n_rays, nthreads, path_free=False, unpolarized=False
     if wl["kind"] == "adaf":
         r.load_adaf(**W.ADAF)
     else:
-        desc, fields = W.fm_torus_grid(*wl["grid"])
+        desc, fields = grid_inputs(tuple(wl["grid"]))
         r.load_grid(desc, fields)
     if path_free:
         r.set_path_free(True)
@@ -383,85 +403,12 @@ def run_adaptive(args, g, replicas, wl, cam, world, rank, local, barrier):
     print(json.dumps(line), flush=True)
 
 
-def run_reference(args):
-    """--impl reference: the oracle on the box's host cores (rank 0 only)."""
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
-        return
-    import __graft_entry__ as ge
-    ge.build()
-    wl = WORKLOADS[args.workload]
-    cores = os.cpu_count() or 1
-    n_rays = args.ref_rays
-    for _ in range(args.warmup):
-        oracle_sample(args.workload, min(n_rays, 256), cores)
-    rays = steps = 0
-    dt = 0.0
-    stride = 0
-    for _ in range(args.steps):
-        a, b, c, stride = oracle_sample(args.workload, n_rays, cores)
-        rays += a; steps += b; dt += c
-    val = rays / dt
-    line = {"impl": "reference", "metric": "rays_per_s", "value": val, "unit": "rays/s", "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "configs_index": wl["config"], "image": "%dx%d" % (wl["n"], wl["n"]),
-                       "step": "oracle on every %d-th pixel in x and y (%d rays) of the image" % (stride, rays // args.steps)},
-            "cpu_baseline": {"value": val, "unit": "rays/s", "cores": cores, "kind": "oracle",
-                             "sample": "%d rays per step, strided lattice of the %dx%d image" % (rays // args.steps, wl["n"], wl["n"])},
-            "e2e": {"value": val, "unit": "rays/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "steps_per_s": steps / dt, "gpu_launches": 0}
-    print(json.dumps(line), flush=True)
-
-
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=2)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="adaf4096", choices=sorted(WORKLOADS))
-    ap.add_argument("--ref-rays", type=int, default=4096, help="rays per step of the --impl reference arm")
-    ap.add_argument("--cpu-baseline-rays", type=int, default=16384)
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--adaptive", type=int, default=0, metavar="LEVELS",
-                    help="adaptive ray tracing (PAPER.md:70) with this many lattice levels, rel_tol 0.02, abs_tol 1e-3 of the peak")
-    ap.add_argument("--unpolarized", action="store_true", help="I alone (PAPER.md:74 'nonpolarized images')")
-    ap.add_argument("--path-free", action="store_true",
-                    help="the paper's own GPU design (PAPER.md:43): no stored path, forward re-integration")
-    args = ap.parse_args()
-    if args.impl == "reference":
-        return run_reference(args)
-
-    import numpy as np
+def measure_image(args, name, ipole, replicas, W, world, rank, local, barrier):
+    """Time `args.steps` full-Stokes images of workload `name` through ipole_make_image (device outputs), then the same
+    through host buffers (e2e), the roofline of the transfer stage, and the oracle on a strided sample.  Returns the
+    JSON line as a dict (rank 0; None elsewhere)."""
     import torch
-    import torch.distributed as dist
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    if rank == 0:
-        import __graft_entry__ as ge
-        ge.build()
-    if world > 1:
-        dist.barrier()
-    from paper_2302_02733_b200 import ipole, replicas, workloads as W
-
-    wl = WORKLOADS[args.workload]
-    if wl.get("cams"):
-        def barrier0():
-            if world > 1:
-                dist.barrier()
-            torch.cuda.synchronize()
-        run_cams(args, ipole, replicas, W, wl, world, rank, local, barrier0)
-        if world > 1:
-            dist.destroy_process_group()
-        return
+    wl = WORKLOADS[name]
     cam = W.camera(wl["kind"], wl["n"])
     g = ipole.Ipole(**cam)
     g.set_stream(torch.cuda.current_stream())
@@ -469,29 +416,16 @@ def main():
         g.set_path_free(True)
     if args.unpolarized:
         g.set_unpolarized(True)
+    if args.single_kernel:
+        g.set_transfer_split(False)
     grid_bytes = 0
     if wl["kind"] == "adaf":
         g.load_adaf(**W.ADAF)
     else:
-        desc, fields = W.fm_torus_grid(*wl["grid"])
+        desc, fields = grid_inputs(tuple(wl["grid"]))
         g.load_grid(desc, fields)
         grid_bytes = fields.nbytes
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    if wl.get("sweep"):
-        run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier,
-                  grid=(desc, fields) if wl["kind"] == "grid" else None)
-        if world > 1:
-            dist.destroy_process_group()
-        return
-    if args.adaptive:
-        run_adaptive(args, g, replicas, wl, cam, world, rank, local, barrier)
-        if world > 1:
-            dist.destroy_process_group()
-        return
+        del fields
     maps = bool(wl.get("maps"))
     names = ["I", "Q", "U", "V"] + (["tau", "tauF"] if maps else [])
     out = {k: torch.empty((wl["n"], wl["n"]), dtype=torch.float64, device="cuda") for k in names}
@@ -504,12 +438,10 @@ def main():
     if rank == 0:
         sampler.start()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    stats = []
     barrier()
     ev0.record()
     for _ in range(args.steps):
         g.make_image(maps=maps, out=out)
-        stats.append(None)
     ev1.record()
     barrier()
     ms = ev0.elapsed_time(ev1)
@@ -543,75 +475,238 @@ def main():
                "d2h_bytes_per_step": len(names) * rays * 8,
                "note": "inputs of this workload are parameters only (analytic model)" if wl["kind"] == "adaf" else
                        "grid planes (%d bytes) are loaded once by ipole_load_model_grid, outside the step" % grid_bytes}
-
+        del host, hnp
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
+        g.close()
+        return None
 
-    # ---- roofline of the dominant kernel (k_transfer), live CUDA-event time of the last timed image ----
+    # ---- roofline of the transfer stage (67 % of the image), live CUDA-event time of the last timed image ----
     key = "transfer_" + wl["kind"]
     pf = args.path_free
+    split = st["ms_stepop"] > 0.0
     fl_rt = FLOP_PER_STEP_PF[key] if pf else FLOP_PER_STEP[key]
     if args.unpolarized:
         fl_rt = FLOP_PER_STEP_UNPOL[key] or 0.0
-    rt_steps = st["total_steps_forward"] if pf else st["total_steps"]   # steps the transfer kernel walks
-    dram_rt = DRAM_BYTES_PER_STEP_PF[key] if pf else DRAM_BYTES_PER_STEP[key]
+    # steps the bulk transfer kernels walk: the long rays (>= path_cap steps each) run on the side stream, outside rt_ms
+    rt_steps = st["total_steps_forward"] if pf else st["total_steps"] - st["n_long"] * st["path_cap"]
+    dram_rt = DRAM_BYTES_PER_STEP_PF[key] if pf else (DRAM_BYTES_PER_STEP_SPLIT if split else DRAM_BYTES_PER_STEP[key])
     dfma_tf, _ = g.fp64_peak()
     n_rt = max(1, st["n_batches"])          # bulk launches; the long-ray passes run beside them on a side stream
     rt_ms = st["ms_transfer"]
-    roof = {"bound": "alu", "kernel": ("k_transfer_unpol<%s>" % wl["kind"]) if args.unpolarized else
-            "k_transfer<%s%s>" % (wl["kind"], ", path-free" if pf else ""), "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+    if args.unpolarized:
+        kname = "k_transfer_unpol<%s>" % wl["kind"]
+    elif split:
+        kname = "k_stepop<%s> + k_apply (split transfer)" % wl["kind"]
+    else:
+        kname = "k_transfer<%s%s>" % (wl["kind"], ", path-free" if pf else "")
+    roof = {"bound": "alu", "kernel": kname, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
             "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz; DFMA micro-benchmark on this GPU: %.1f" % dfma_tf,
-            "launches": n_rt, "avg_launch_ms": rt_ms / n_rt, "kernel_share_of_step": rt_ms / st["ms_total"],
+            "launches": n_rt * (2 if split else 1), "avg_launch_ms": rt_ms / n_rt, "kernel_share_of_step": rt_ms / st["ms_total"],
             "steps_per_launch": rt_steps / n_rt,
             "traffic": dram_rt * rt_steps / n_rt,
-            "traffic_note": "ncu dram__bytes_read+write per launch (profiles/r1_k_transfer_*.txt), scaled by steps; "
+            "traffic_note": "ncu dram__bytes_read+write per step of the stage (profiles/), scaled by the steps of a batch; "
                             + ("algorithmic: 64 B read and 32-48 B written per RAY, nothing per step" if pf else
+                               "algorithmic: 64 B path record read + 64 B operator record written and read per step" if split else
                                "algorithmic: 64 B per step (one path record read)")}
     ach = fl_rt * rt_steps / (rt_ms * 1e-3) / 1e12
-    roof.update(achieved=ach, frac=ach / FP64_PEAK_TFLOPS, flop_per_step=fl_rt)
-    # the whole step against the same roofline: every FP64 operation of both hot kernels over the image time
-    fl_step = fl_rt * rt_steps + FLOP_PER_STEP["geodesic_" + wl["kind"]] * st["total_steps"]
+    roof.update(achieved=ach, frac=ach / FP64_PEAK_TFLOPS, flop_per_step_algorithmic=fl_rt,
+                flop_note="frac = frozen algorithmic flop per step (round-1 lean count, DESIGN.md section 7) x steps / live "
+                          "CUDA-event time / peak; frac_executed uses what the shipped kernels execute (ncu); "
+                          "fp64_pipe_pct is sm__inst_executed_pipe_fp64 of the ncu captures under profiles/, not live")
+    if not (pf or args.unpolarized):
+        if split:
+            parts = {"k_stepop": st["ms_stepop"], "k_apply": st["ms_apply"]}
+        else:
+            parts = {"k_transfer<%s>" % wl["kind"]: rt_ms}
+        roof["kernels"] = {k: {"ms": v, "flop_per_step_executed": FLOP_EXECUTED[k], "fp64_pipe_pct": FP64_PIPE_PCT[k],
+                               "tflops_executed": FLOP_EXECUTED[k] * rt_steps / (v * 1e-3) / 1e12,
+                               "frac_executed": FLOP_EXECUTED[k] * rt_steps / (v * 1e-3) / 1e12 / FP64_PEAK_TFLOPS}
+                           for k, v in parts.items() if v > 0}
+        fx = sum(FLOP_EXECUTED[k] for k in parts)
+        roof["flop_per_step_executed"] = fx
+        roof["frac_executed"] = fx * rt_steps / (rt_ms * 1e-3) / 1e12 / FP64_PEAK_TFLOPS
+        roof["fp64_pipe_pct"] = sum(FP64_PIPE_PCT[k] * v for k, v in parts.items()) / max(1e-9, sum(parts.values()))
+    # the whole step against the same roofline: the algorithmic FP64 operations of both stages over the image time
+    gkey = "geodesic_" + wl["kind"]
+    fl_step = fl_rt * rt_steps + FLOP_PER_STEP[gkey] * st["total_steps"]
+    gk = "k_geodesic<occ>" if wl["kind"] == "grid" else "k_geodesic"
     roof["whole_step"] = {"achieved": fl_step / (st["ms_total"] * 1e-3) / 1e12,
                           "frac": fl_step / (st["ms_total"] * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
-                          "geodesic_tflops": FLOP_PER_STEP["geodesic_" + wl["kind"]] * st["total_steps"]
-                                             / (st["ms_geodesic"] * 1e-3) / 1e12}
-    roof["hbm_path_gbs"] = (0.0 if pf else 128.0) * st["total_steps"] / ((st["ms_geodesic"] + st["ms_transfer"]) * 1e-3) / 1e9
+                          "geodesic_tflops": FLOP_PER_STEP[gkey] * st["total_steps"] / (st["ms_geodesic"] * 1e-3) / 1e12,
+                          "geodesic_frac": FLOP_PER_STEP[gkey] * st["total_steps"] / (st["ms_geodesic"] * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+                          "geodesic_fp64_pipe_pct": FP64_PIPE_PCT[gk]}
+    path_bytes = 0.0 if pf else (256.0 if split else 128.0)
+    roof["hbm_path_gbs"] = path_bytes * st["total_steps"] / ((st["ms_geodesic"] + st["ms_transfer"]) * 1e-3) / 1e9
 
     line = {"metric": "rays_per_s", "value": value, "unit": "rays/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "configs_index": wl["config"], "image": "%dx%d" % (wl["n"], wl["n"]),
+            "config": {"workload": name, "configs_index": wl["config"], "image": "%dx%d" % (wl["n"], wl["n"]),
                        "model": wl["kind"], "freq_ghz": 230, "eps": cam["eps"], "maps": maps,
                        "variant": "unpolarized, I alone (PAPER.md:74), stored path" if args.unpolarized else
-                                  "path-free bidirectional (PAPER.md:43)" if pf else "stored path",
+                                  "path-free bidirectional (PAPER.md:43)" if pf else
+                                  "stored path, split transfer (k_stepop + k_apply)" if split else "stored path, single transfer kernel",
                        "full_stokes": not args.unpolarized,
                        "l2": ("no flush needed: nothing is re-read; per image %.2f GB of end points and outputs stream once"
                               % (rays * (64.0 + 8.0 * len(names)) / 1e9)) if pf else
-                             "no flush needed: every batch streams a %.1f GB path buffer (>> 126 MB L2)"
-                             % (st["path_cap"] * 64.0 * min(rays, max(1, rays // max(1, st["n_batches"]))) / 1e9),
+                             "no flush needed: every batch streams %.1f GB of path and operator records (>> 126 MB L2)"
+                             % (path_bytes / 2 * st["total_steps"] / max(1, st["n_batches"]) / 1e9),
                        "parallelism": "rays sharded: one replica per GPU" if world > 1 else "single GPU"},
             "images_per_s": value / rays, "steps_per_s": world * st["total_steps"] * args.steps / (ms * 1e-3),
             "mean_steps_per_ray": st["total_steps"] / rays, "forward_steps": st["total_steps_forward"],
             "stage_ms": {"probe_sort": st["ms_probe"], "geodesic": st["ms_geodesic"], "transfer": st["ms_transfer"],
+                         "stepop": st["ms_stepop"], "apply": st["ms_apply"],
                          "long_rays_side_stream": st["ms_long"], "total": st["ms_total"], "batches": st["n_batches"], "path_cap": st["path_cap"],
-                         "long_rays": st["n_long"]},
+                         "long_rays": st["n_long"], "retried_rays": st["n_retry"]},
             "flux_jy": st["flux_jy"], "lp": st["lp"], "cp": st["cp"], "ring_rays": st["n_ring"],
             "gpu_launches": st["n_launches"] * args.steps, "roofline": roof, "e2e": e2e, "clocks": clocks,
             "paper_context": {"note": "paper Table 1, other model/hardware (A100): context only",
                               "a100_semianalytic_4096_rays_per_s": 127583, "a100_grmhd_4096_rays_per_s": 188720}}
+    g.close()
+    del out
+    torch.cuda.empty_cache()
 
     if not args.no_cpu_baseline and world == 1:
         cores = os.cpu_count() or 1
-        n, steps, dt, stride = oracle_sample(args.workload, args.cpu_baseline_rays, cores, path_free=pf, unpolarized=args.unpolarized)
+        n, steps, dt, stride = oracle_sample(name, args.cpu_baseline_rays, cores, path_free=pf, unpolarized=args.unpolarized)
         line["cpu_baseline"] = {"value": n / dt, "unit": "rays/s", "cores": cores, "kind": "oracle",
                                 "sample": "%d rays: every %d-th pixel in x and y of the %dx%d image, %.1f s"
                                           % (n, stride, wl["n"], wl["n"], dt),
                                 "steps_per_s": steps / dt}
+    return line
+
+def reference_line(args, name, cores):
+    """The oracle, as it stands, on a strided lattice of workload `name`: `args.steps` timed steps of `args.ref_rays` rays."""
+    wl = WORKLOADS[name]
+    n_rays = args.ref_rays
+    for _ in range(args.warmup):
+        oracle_sample(name, min(n_rays, 256), cores)
+    rays = steps = 0
+    dt = 0.0
+    stride = 0
+    for _ in range(args.steps):
+        a, b, c, stride = oracle_sample(name, n_rays, cores)
+        rays += a; steps += b; dt += c
+    val = rays / dt
+    return {"impl": "reference", "metric": "rays_per_s", "value": val, "unit": "rays/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": name, "configs_index": wl["config"], "image": "%dx%d" % (wl["n"], wl["n"]),
+                       "model": wl["kind"], "freq_ghz": 230, "eps": 0.01, "maps": bool(wl.get("maps")), "full_stokes": True,
+                       "variant": "CPU oracle (oracle/), one ray per work item, %d host threads" % cores,
+                       "step": "oracle on every %d-th pixel in x and y (%d rays) of the image" % (stride, rays // args.steps)},
+            "cpu_baseline": {"value": val, "unit": "rays/s", "cores": cores, "kind": "oracle",
+                             "sample": "%d rays per step, strided lattice of the %dx%d image" % (rays // args.steps, wl["n"], wl["n"])},
+            "e2e": {"value": val, "unit": "rays/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "steps_per_s": steps / dt, "gpu_launches": 0}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the box's host cores (rank 0 only).  Builds and loads the oracle alone: the
+    product library is neither compiled nor opened in this arm."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import __graft_entry__ as ge
+    ge.build_oracle()
+    cores = os.cpu_count() or 1
+    line = reference_line(args, args.workload, cores)
+    if args.workload == "adaf4096" and not args.no_second_workload:   # the other half of configs[4], as in our arm
+        other = reference_line(args, "grid4096", cores)
+        for k in ("impl", "metric", "unit", "n_gpus", "steps", "warmup", "higher_is_better", "scaling", "vs_baseline", "dtype", "data"):
+            other.pop(k, None)
+        line["workloads"] = {"grid4096": other}
     print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="adaf4096", choices=sorted(WORKLOADS))
+    ap.add_argument("--ref-rays", type=int, default=4096, help="rays per step of the --impl reference arm")
+    ap.add_argument("--cpu-baseline-rays", type=int, default=16384)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--adaptive", type=int, default=0, metavar="LEVELS",
+                    help="adaptive ray tracing (PAPER.md:70) with this many lattice levels, rel_tol 0.02, abs_tol 1e-3 of the peak")
+    ap.add_argument("--unpolarized", action="store_true", help="I alone (PAPER.md:74 'nonpolarized images')")
+    ap.add_argument("--single-kernel", action="store_true",
+                    help="transfer in the single per-ray kernel k_transfer instead of k_stepop + k_apply (ipole_set_transfer_split 0)")
+    ap.add_argument("--no-second-workload", action="store_true",
+                    help="default run only: skip the grid4096 half of configs[4] that is otherwise timed after adaf4096")
+    ap.add_argument("--path-free", action="store_true",
+                    help="the paper's own GPU design (PAPER.md:43): no stored path, forward re-integration")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
     if world > 1:
-        dist.destroy_process_group()
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        import __graft_entry__ as ge
+        ge.build()
+    if world > 1:
+        dist.barrier()
+    from paper_2302_02733_b200 import ipole, replicas, workloads as W
+
+    wl = WORKLOADS[args.workload]
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def finish():
+        if world > 1:
+            dist.destroy_process_group()
+
+    if wl.get("cams"):
+        run_cams(args, ipole, replicas, W, wl, world, rank, local, barrier)
+        return finish()
+    if wl.get("sweep") or args.adaptive:
+        cam = W.camera(wl["kind"], wl["n"])
+        g = ipole.Ipole(**cam)
+        g.set_stream(torch.cuda.current_stream())
+        if args.unpolarized:
+            g.set_unpolarized(True)
+        grid = None
+        if wl["kind"] == "adaf":
+            g.load_adaf(**W.ADAF)
+        else:
+            grid = grid_inputs(tuple(wl["grid"]))
+            g.load_grid(*grid)
+        if wl.get("sweep"):
+            run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier, grid=grid)
+        else:
+            run_adaptive(args, g, replicas, wl, cam, world, rank, local, barrier)
+        return finish()
+
+    line = measure_image(args, args.workload, ipole, replicas, W, world, rank, local, barrier)
+    # The default run covers BOTH halves of BASELINE.json configs[4]: the analytic ADAF image is the top-level value,
+    # the GRMHD-like grid image of the same size is timed in the same process and reported under "workloads".
+    plain = not (args.path_free or args.unpolarized or args.single_kernel)
+    if args.workload == "adaf4096" and plain and not args.no_second_workload:
+        other = measure_image(args, "grid4096", ipole, replicas, W, world, rank, local, barrier)
+        if rank == 0:
+            for k in ("metric", "unit", "n_gpus", "steps", "warmup", "higher_is_better", "scaling", "vs_baseline", "dtype", "data", "paper_context"):
+                other.pop(k, None)
+            line["workloads"] = {"grid4096": other}
+            line["gpu_launches"] += other["gpu_launches"]
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    finish()
 
 
 if __name__ == "__main__":

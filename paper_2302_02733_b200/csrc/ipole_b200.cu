@@ -51,6 +51,8 @@ struct ipole_ctx {
   int last_pf = 0;               // the last image was made path-free
   int opt_unpol = 0;             // unpolarized transfer of I alone
   AdafParams adaf_host;          // host copy of the loaded analytic model (k_apply takes it by value)
+  int opt_group = 1;             // grid model: transfer with warp-level scheduling (k_transfer_group)
+  int occ_group = 0;
   int opt_tight = 1;             // sorted rays: path slots sized batch by batch from the predicted step counts
   int32_t* d_retry = nullptr;    // rays that outgrew their batch's slots (retried with the global S_cap)
   int opt_split = 1;             // stored path, analytic flow: transfer as k_stepop + k_apply (stepop.cuh)
@@ -60,7 +62,9 @@ struct ipole_ctx {
   int occ_unpol[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};
   double* d_endp = nullptr; int64_t endp_cap = 0;   // end points of the backward passes, [rays][8]
   long long* d_sum = nullptr;    // forward-step total of the path-free variant
-  void* d_sweep_models = nullptr; Units* d_sweep_units = nullptr;   // model sweep: SWEEP_MAX_MODELS entries each
+  void* d_sweep_models = nullptr; Units* d_sweep_units = nullptr;   // model sweep: SWEEP_MAX_MODELS entries each (main stream)
+  void* d_sweep_models_side = nullptr; Units* d_sweep_units_side = nullptr;   // the same for the long-ray passes on the side stream
+  GridParams grid_host; double grid_M_unit = 0.0;   // host copy of the loaded grid model (units are re-derived when the camera's mass changes)
   double* d_sweep_out = nullptr; size_t sweep_out_doubles = 0;            // staging for host outputs of a sweep
   int occ_sweep[4] = {0, 0, 0, 0};
   unsigned char* d_ada = nullptr; size_t ada_bytes = 0;   // adaptive ray tracing: staging planes, list, state, flags
@@ -195,6 +199,7 @@ int ensure_path_long(ipole_ctx* c, size_t bytes) {
 
 size_t path_budget(ipole_ctx* c) {
   if (c->opt_path_bytes) return (size_t)c->opt_path_bytes;
+  if (const char* e = std::getenv("IPOLE_PATH_GIB")) { const double gib = std::atof(e); if (gib > 0.0) return (size_t)(gib * 1073741824.0); }
   size_t fr = 0, tot = 0;
   cudaMemGetInfo(&fr, &tot);
   fr += c->path_bytes + c->path_long_bytes + c->ops_bytes;  // what we already hold counts as available
@@ -268,16 +273,19 @@ int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_
   }
   if (sw) {
     // chunks of SWEEP_MAX_MODELS parameter sets; the parameter tables are re-sent per chunk on the launching stream
-    // (stream order keeps a table alive until the kernel that reads it has finished)
+    // (stream order keeps a table alive until the kernel that reads it has finished).  The main stream and the side
+    // stream (long-ray passes) each have their own tables: they run concurrently.
+    void* tab_models = (st == c->side) ? c->d_sweep_models_side : c->d_sweep_models;
+    Units* tab_units = (st == c->side) ? c->d_sweep_units_side : c->d_sweep_units;
     RtArgs t = a;
     double* planes[6] = {a.I, a.Q, a.U, a.V, a.tau, a.tauF};
     for (int m0 = 0; m0 < sw->n_models; m0 += SWEEP_MAX_MODELS) {
       const int mc = std::min(SWEEP_MAX_MODELS, sw->n_models - m0);
       const int s = span_begin(c, kind, st);
-      CK(cudaMemcpyAsync(c->d_sweep_models, (const char*)sw->lane_tab + (size_t)m0 * sw->lane_bytes, mc * sw->lane_bytes,
+      CK(cudaMemcpyAsync(tab_models, (const char*)sw->lane_tab + (size_t)m0 * sw->lane_bytes, mc * sw->lane_bytes,
                          cudaMemcpyHostToDevice, st));
-      CK(cudaMemcpyAsync(c->d_sweep_units, sw->units + m0, mc * sizeof(Units), cudaMemcpyHostToDevice, st));
-      t.lane_tab = c->d_sweep_models; t.units_arr = c->d_sweep_units; t.n_models = mc; t.out_stride = sw->out_stride;
+      CK(cudaMemcpyAsync(tab_units, sw->units + m0, mc * sizeof(Units), cudaMemcpyHostToDevice, st));
+      t.lane_tab = tab_models; t.units_arr = tab_units; t.n_models = mc; t.out_stride = sw->out_stride;
       t.I = planes[0] + (size_t)m0 * sw->out_stride; t.Q = planes[1] + (size_t)m0 * sw->out_stride;
       t.U = planes[2] + (size_t)m0 * sw->out_stride; t.V = planes[3] + (size_t)m0 * sw->out_stride;
       t.tau = planes[4] ? planes[4] + (size_t)m0 * sw->out_stride : nullptr;
@@ -296,6 +304,15 @@ int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_
     return IPOLE_OK;
   }
   const int s = span_begin(c, kind, st);
+  if (pf == 0 && c->model == MODEL_GRID && c->opt_group && !a.slots) {
+    // warp-level scheduling: one warp per 32 consecutive rays (kernels.cuh, k_transfer_group)
+    const int gg = grid_for(c, c->occ_group, IPOLE_RT_THREADS / 32, (rays + 31) / 32, reserve);
+    k_transfer_group<MODEL_GRID><<<gg, IPOLE_RT_THREADS, 0, st>>>(a);
+    span_end(c, s, st);
+    c->stats.n_launches++;
+    CK(cudaGetLastError());
+    return IPOLE_OK;
+  }
   const int g = grid_for(c, pf ? c->occ_pf[c->model][pf] : c->occ_rt[c->model], IPOLE_RT_THREADS, rays, reserve);
   if (pf == 0) launch_transfer_model<0>(c->model, g, st, a);
   else if (pf == 1) launch_transfer_model<1>(c->model, g, st, a);
@@ -568,6 +585,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
       if (B >= 64) B &= ~(int64_t)31;           // whole groups of 32 slots (operator records, stepop.cuh)
       B = std::max<int64_t>(1, std::min(B, total_rays - base));
       plan.push_back({base, B, cb});
+      if (std::getenv("IPOLE_DEBUG_SPANS")) std::fprintf(stderr, "batch base %lld cnt %lld cap %d\n", (long long)base, (long long)B, cb);
       base += B;
     }
   };
@@ -707,6 +725,8 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   if (cudaMalloc(&c->d_sum, sizeof(long long)) != cudaSuccess) return fail(IPOLE_ENOMEM);
   if (cudaMalloc(&c->d_sweep_models, SWEEP_MAX_MODELS * std::max(sizeof(AdafParams), sizeof(GridScales))) != cudaSuccess) return fail(IPOLE_ENOMEM);
   if (cudaMalloc(&c->d_sweep_units, SWEEP_MAX_MODELS * sizeof(Units)) != cudaSuccess) return fail(IPOLE_ENOMEM);
+  if (cudaMalloc(&c->d_sweep_models_side, SWEEP_MAX_MODELS * std::max(sizeof(AdafParams), sizeof(GridScales))) != cudaSuccess) return fail(IPOLE_ENOMEM);
+  if (cudaMalloc(&c->d_sweep_units_side, SWEEP_MAX_MODELS * sizeof(Units)) != cudaSuccess) return fail(IPOLE_ENOMEM);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_sweep[MODEL_ADAF], k_transfer<MODEL_ADAF, 0, true>, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_unpol[MODEL_ADAF][0], k_transfer_unpol<MODEL_ADAF, false>, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_unpol[MODEL_SLAB][0], k_transfer_unpol<MODEL_SLAB, false>, IPOLE_RT_THREADS, 0);
@@ -718,6 +738,8 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap, k_apply, IPOLE_AP_THREADS, 0);
   { const char* e = std::getenv("IPOLE_NO_SPLIT"); if (e && e[0] == '1') c->opt_split = 0; }
   { const char* e = std::getenv("IPOLE_NO_TIGHT"); if (e && e[0] == '1') c->opt_tight = 0; }
+  { const char* e = std::getenv("IPOLE_NO_GROUP"); if (e && e[0] == '1') c->opt_group = 0; }
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_group, k_transfer_group<MODEL_GRID>, IPOLE_RT_THREADS, 0);
   rc = apply_camera(c, cam);
   if (rc != IPOLE_OK) return fail(rc);
   *out = c;
@@ -731,9 +753,18 @@ int ipole_set_camera(ipole_ctx* c, const ipole_camera* cam) {
   const double h_new = cam->hslope > 0.0 ? cam->hslope : 1.0;
   if (c->model == MODEL_GRID && h_new != c->cam.G.hslope) return IPOLE_EINVAL;
   if (c->model == MODEL_ADAF && cam->flat_metric) return IPOLE_EINVAL;
-  const double a_old = c->cam.G.a;
+  const double a_old = c->cam.G.a, L_old = c->units.L_unit;
   rc = apply_camera(c, cam);
   if (rc != IPOLE_OK) return rc;
+  if (c->model == MODEL_GRID && c->units.L_unit != L_old) {
+    // the density and field units of the grid model contain the length unit GM/c^2: keep them consistent with the
+    // path element dl_unit when the camera's mass changes
+    const double L = c->units.L_unit, rho_unit = c->grid_M_unit / (L * L * L);
+    c->grid_host.ne_unit = rho_unit / (IP_MP + IP_ME);
+    c->grid_host.B_unit = IP_CL * std::sqrt(4.0 * M_PI * rho_unit);
+    CK(cudaMemcpyAsync(c->d_model, &c->grid_host, sizeof(GridParams), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+  }
   if (c->model == MODEL_ADAF && a_old != cam->spin) {  // r_isco depends on the spin
     c->adaf_host.r_isco = isco_radius(cam->spin);
     CK(cudaMemcpyAsync(c->d_model, &c->adaf_host, sizeof(AdafParams), cudaMemcpyHostToDevice, c->stream));
@@ -850,7 +881,8 @@ int ipole_load_model_grid(ipole_ctx* c, const ipole_grid_desc* d, const double* 
   const double rho_unit = d->M_unit / (L * L * L);
   m.ne_unit = rho_unit / (IP_MP + IP_ME);
   m.B_unit = IP_CL * std::sqrt(4.0 * M_PI * rho_unit);
-  CK(cudaMemcpyAsync(c->d_model, &m, sizeof m, cudaMemcpyHostToDevice, c->stream));
+  c->grid_host = m; c->grid_M_unit = d->M_unit;
+  CK(cudaMemcpyAsync(c->d_model, &c->grid_host, sizeof m, cudaMemcpyHostToDevice, c->stream));
   CK(cudaStreamSynchronize(c->stream));
   c->model = MODEL_GRID;
   return IPOLE_OK;
@@ -1133,9 +1165,11 @@ int ipole_get_stats(ipole_ctx* c, ipole_stats* out) {
     s.total_steps_forward = f;
   }
   s.ms_probe = s.ms_geodesic = s.ms_transfer = s.ms_total = s.ms_long = s.ms_stepop = s.ms_apply = 0.f;
+  const bool dbg = std::getenv("IPOLE_DEBUG_SPANS") != nullptr;
   for (size_t i = 0; i < c->spans_used; ++i) {
     float ms = 0.f;
     if (cudaEventElapsedTime(&ms, c->spans[i].a, c->spans[i].b) != cudaSuccess) { cudaGetLastError(); continue; }
+    if (dbg) std::fprintf(stderr, "span %zu kind %d ms %.3f\n", i, c->spans[i].kind, ms);
     if (i == 0) s.ms_total = ms;
     else if (c->spans[i].kind == LK_PROBE) s.ms_probe += ms;
     else if (c->spans[i].kind == LK_GEO) s.ms_geodesic += ms;
@@ -1280,7 +1314,7 @@ void ipole_free(ipole_ctx* c) {
   cudaFree(c->d_cam); cudaFree(c->d_model); cudaFree(c->d_grid); cudaFree(c->d_path);
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long);
   cudaFree(c->d_out); cudaFree(c->d_pixels); cudaFree(c->d_probe); cudaFree(c->d_queues); cudaFree(c->d_hist);
-  cudaFree(c->d_small); cudaFree(c->d_part); cudaFree(c->d_red); cudaFree(c->d_endp); cudaFree(c->d_sum); cudaFree(c->d_sweep_models); cudaFree(c->d_sweep_units); cudaFree(c->d_sweep_out); cudaFree(c->d_ada);
+  cudaFree(c->d_small); cudaFree(c->d_part); cudaFree(c->d_red); cudaFree(c->d_endp); cudaFree(c->d_sum); cudaFree(c->d_sweep_models); cudaFree(c->d_sweep_units); cudaFree(c->d_sweep_models_side); cudaFree(c->d_sweep_units_side); cudaFree(c->d_sweep_out); cudaFree(c->d_ada);
   cudaFree(c->d_ops); cudaFree(c->d_irr); cudaFree(c->d_retry);
   if (c->ev_ada0) cudaEventDestroy(c->ev_ada0);
   if (c->ev_ada1) cudaEventDestroy(c->ev_ada1);

@@ -502,6 +502,110 @@ k_transfer(const __grid_constant__ RtArgs A) {
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// The same transfer on the stored path with WARP-level scheduling: one warp walks 32 consecutive rays of the batch in
+// lockstep, lane <-> ray, aligned on the step index s (distance from the camera in steps), from the largest first-contact
+// index of the group down to the camera; a lane joins when s reaches its own ray's start.
+//
+// Why (grid model): a walked step costs ~40 instructions where the stencil is empty and the ray still dark, ~400 in lit
+// vacuum (transport only) and ~1200 where it crosses plasma.  With lane-level refill (k_transfer) the lanes of a warp
+// drift to unrelated phases of unrelated rays and the warp pays for every kind of step present: 17 of 32 lanes active,
+// and the loss grows with the batch length (profiles/r2_notes.md: the same image is 30 % slower in 28 batches than in
+// 97).  Rays are ordered by predicted step count, so the 32 rays of a group lie on one ring of the image around the
+// spin axis: at equal s they are at nearly equal radius and in the same kind of step.  The arithmetic per ray is that
+// of k_transfer, operation for operation (bit-identical images).
+template <int MODEL>
+__global__ void __launch_bounds__(IPOLE_RT_THREADS, IPOLE_RT_MINB) k_transfer_group(const __grid_constant__ RtArgs A) {
+  const CamDev& C = A.cam;
+  const size_t slot_doubles = (size_t)(A.cap + 1) * REC_DOUBLES;
+  constexpr int MODEL_BYTES = MODEL == MODEL_ADAF ? sizeof(AdafParams) : (MODEL == MODEL_SLAB ? sizeof(SlabParams) : sizeof(GridParams));
+  __shared__ __align__(8) unsigned char model_smem[MODEL_BYTES];
+  for (int i = threadIdx.x; i < MODEL_BYTES; i += blockDim.x) model_smem[i] = ((const unsigned char*)A.model)[i];
+  __syncthreads();
+  const void* model = model_smem;
+  const int lane = threadIdx.x & 31;
+  const int64_t n_groups = (A.count + 31) >> 5;
+
+  for (;;) {
+    __syncwarp();
+    long long grp = 0;
+    if (lane == 0) grp = (long long)atomicAdd(A.queue, 1ULL);
+    grp = __shfl_sync(0xffffffffu, grp, 0);
+    if (grp >= n_groups) break;
+    const int64_t li = (grp << 5) + lane;
+    PolState st;
+    double Xhi[4] = {0, 0, 0, 0}, Khi[4] = {0, 0, 0, 0};
+    const double* rec = nullptr;
+    int32_t q = 0;
+    int s0 = -1, s_lo = 0;       // this lane walks steps s0 ... 0; -1: nothing to walk
+    bool lit = false;
+    if (li < A.count) {
+      q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
+      int n = A.nsteps[q];
+      if (n >= 0) {              // (n < 0: overflowed its slot, done by the long-ray pass)
+        if (MODEL == MODEL_GRID && A.srange) {
+          const int2 r = A.srange[q];
+          s_lo = r.y;
+          if (r.x < 0) {         // the ray meets no plasma: dark
+            A.I[q] = 0.0; A.Q[q] = 0.0; A.U[q] = 0.0; A.V[q] = 0.0;
+            if (A.tau) A.tau[q] = 0.0;
+            if (A.tauF) A.tauF[q] = 0.0;
+            n = 0;
+          } else n = r.x + 1;    // start at the first contact with plasma
+        }
+        if (n > 0) {
+          rec = A.path + (size_t)li * slot_doubles;
+          double dl;
+          load_record(rec + (size_t)n * REC_DOUBLES, Xhi, Khi, dl);
+          s0 = n - 1;
+        }
+      }
+    }
+#pragma unroll
+    for (int m = 0; m < 4; ++m) { st.f1[m] = 0.0; st.f2[m] = 0.0; st.S[m] = 0.0; }
+    st.tau = 0.0; st.tauF = 0.0;
+    int smax = s0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) smax = max(smax, __shfl_xor_sync(0xffffffffu, smax, o));
+
+    for (int s = smax; s >= 0; --s) {
+      if (s > s0) continue;
+      double Xlo[4], Klo[4], dl;
+      load_record(rec + (size_t)s * REC_DOUBLES, Xlo, Klo, dl);
+#if IPOLE_RT_PREFETCH
+      if (s > 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(rec + (size_t)(s - 1) * REC_DOUBLES));
+#endif
+      double Xm[4], Km[4];
+#pragma unroll
+      for (int m = 0; m < 4; ++m) { Xm[m] = 0.5 * (Xlo[m] + Xhi[m]); Km[m] = 0.5 * (Klo[m] + Khi[m]); }
+      bool maybe = true;
+      double prim[8];
+      if (MODEL == MODEL_GRID) maybe = (s >= s_lo) && grid_gather(*(const GridParams*)model, Xm, prim);
+      if (lit || maybe) {
+        Point p; Sym7 g; Inv6 gi; double Am[4][4];
+        transport_generator(C.G, Xm, Km, p, g, gi, Am);
+        const double h = 0.5 * dl;
+        if (lit) { transport_apply(Am, h, st.f1); transport_apply(Am, h, st.f2); }
+        PlasmaFrame F;
+        const bool applied = maybe && plasma_frame<MODEL>(C.G, model, nullptr, A.units, Xm, Km, p, g, gi, prim, st, F);
+        lit |= applied;
+        if (lit) { transport_apply(Am, h, st.f1); transport_apply(Am, h, st.f2); }
+        if (applied) plasma_apply<MODEL>(A.units, F, dl, st);
+      }
+#pragma unroll
+      for (int m = 0; m < 4; ++m) { Xhi[m] = Xlo[m]; Khi[m] = Klo[m]; }
+    }
+    if (s0 >= 0) {
+      stokes_congruence(dot4(C.ecov1, st.f1), dot4(C.ecov1, st.f2), dot4(C.ecov2, st.f1), dot4(C.ecov2, st.f2), st.S);
+      const double nu_o = A.units.nu_obs;
+      const double nu3 = nu_o * nu_o * nu_o;
+      A.I[q] = st.S[0] * nu3; A.Q[q] = st.S[1] * nu3; A.U[q] = st.S[2] * nu3; A.V[q] = st.S[3] * nu3;
+      if (A.tau) A.tau[q] = st.tau;
+      if (A.tauF) A.tauF[q] = st.tauF;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // Unpolarized transfer ("nonpolarized images" of the model-fitting loop; R-12): I alone on the
 // stored path.  Per step: midpoint, metric (no derivatives, no transport), plasma state, nu = -k.u nu_obs, pitch
 // angle, thermal synchrotron j_I and alpha_I, exact scalar step  I <- I e^{-x} + j ds (1 - e^{-x})/x,  x = alpha ds.

@@ -173,3 +173,51 @@ def test_independent_contexts_side_by_side(ipole):
             got = to_np(outs[k])
             for name in want[k]:
                 assert np.array_equal(got[name], want[k][name]), (k, name)
+
+
+def test_sweep_of_more_than_one_chunk_with_long_rays(ipole):
+    """70 parameter sets (two table chunks) AND a path budget so small that rays overflow their slots: the long-ray
+    passes walk the same chunks on the side stream while the main stream walks them for the bulk; each stream has its
+    own parameter tables (a shared one could hand a kernel the other chunk's parameters)."""
+    cam = W.camera("adaf", 24, max_steps=6000)
+    models = [dict(n0=1e6 * (1 + 0.03 * m), Th0=30.0 - 0.2 * (m % 64), B0=30.0 + 0.1 * m) for m in range(70)]
+    g = ipole.Ipole(**cam)
+    want = g.make_images_adaf(models)
+    assert g.stats()["n_long"] == 0
+    W_ = {k: want[k].cpu().numpy() for k in ("I", "Q", "U", "V")}
+    for rep in range(3):                       # a race would not show every time
+        g.set_options(6 << 20, 0)              # no probe, slots far shorter than the rays: every ray is a long ray
+        got = g.make_images_adaf(models)
+        assert g.stats()["n_long"] > 0
+        for k in W_:
+            assert np.array_equal(got[k].cpu().numpy(), W_[k]), (rep, k)
+
+
+def test_adaptive_sweep_adaptive_on_one_context(ipole):
+    """The sweep entry must leave the adaptive entry's buffers and events alone (it used to free them when its own
+    staging buffer grew): adaptive -> sweep with growing n_models -> adaptive gives the same image twice."""
+    cam = W.camera("adaf", 48)
+    g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
+    a1, i1 = g.make_image_adaptive(2, 0.05, 0.0, host=True)
+    for M in (2, 9, 33):                       # host outputs: the staging buffer grows with every call
+        g.make_images_adaf([dict(n0=1e6 * (1 + 0.1 * m)) for m in range(M)], host=True)
+    a2, i2 = g.make_image_adaptive(2, 0.05, 0.0, host=True)
+    for k in ("I", "Q", "U", "V", "state"):
+        assert np.array_equal(a1[k], a2[k]), k
+    assert i1["n_traced"] == i2["n_traced"]
+
+
+def test_set_camera_with_a_new_mass_rescales_the_grid_units(ipole):
+    """ipole_set_camera keeps the loaded grid model; its density and field units contain GM/c^2, so a new mass must give
+    the image a fresh context with that mass gives (they used to keep the old length unit)."""
+    desc, fields = W.fm_torus_grid(48, 24, 16)
+    cam1, cam2 = W.camera("grid", 24), W.camera("grid", 24, mbh_msun=6.5e9, dsource_pc=16.8e6)
+    g = ipole.Ipole(**cam1); g.load_grid(desc, fields)
+    g.make_image()
+    g.set_camera(**cam2)
+    a = to_np(g.make_image())
+    f = ipole.Ipole(**cam2); f.load_grid(desc, fields)
+    b = to_np(f.make_image())
+    assert (b["I"] > 0).any()
+    for k in ("I", "Q", "U", "V"):
+        assert np.array_equal(a[k], b[k]), k
