@@ -213,8 +213,64 @@ __device__ __forceinline__ void metric_derivs_at(const Geom& G, Point& p, Sym7& 
   D2.c33 = cs2 * (p.Sig + a2 * s2 * opf) + s2 * (St2 + a2 * e);
 }
 
-// dK^l / dlambda = - Gamma^l_{mn} K^m K^n
+#ifndef IPOLE_GEO_KS
+#define IPOLE_GEO_KS 1
+#endif
+
+// dK^l / dlambda = - Gamma^l_{mn} K^m K^n, written out for the Kerr-Schild form of the metric instead of through the
+// derivative matrices: in (t, r, theta, phi),  g = eta~ + f l l,  l_mu = (1, 1, 0, -a sin^2),  f = 2 m r / Sigma,
+//   eta~ = -dt^2 + dr^2 + Sigma dth^2 + (r^2+a^2) sin^2 dph^2 - 2 a sin^2 dr dph .
+// With u = dx/dlambda and P = l.u the Euler-Lagrange equations  d/dlambda (g_{kn} u^n) = 1/2 d_k g_{mn} u^m u^n  give
+//   g_{kn} du^n/dlambda = R_k = 1/2 d_k g(u,u) - (d eta~_{kn}/dlambda) u^n - W l_k - f P dl_k/dlambda ,
+//   W = f (dl/dlambda . u) + (df/dlambda) P ,   dl_phi/dlambda = -a sin(2 theta) dtheta/dlambda  (the only one),
+// and the closed-form inverse raises R.  The MKS components follow from r = e^{X1}, theta = theta(X2):
+//   dK1 = r''/r - K1^2,   dK2 = (theta'' - theta_XX K2^2) / theta_X .
+// The same equations as the contracted Christoffel symbols of geodesic_accel_gamma (identical up to rounding; the
+// traced paths are compared with the oracle's to 1e-11 in tests/test_gpu_stages.py), at ~100 instead of ~160 FP64
+// instructions per evaluation: k_geodesic is bound by the FP64 pipe, and this is four evaluations per step.
+__device__ __forceinline__ void geodesic_accel_ks(const Geom& G, Point& p, const double K[4], double dK[4]) {
+  const double a = G.a, a2 = a * a, m = G.mass;
+  const double r = p.r, s2 = p.s * p.s, S2 = 2.0 * p.s * p.c, r2 = r * r;
+  const double Sig = r2 + a2 * p.c * p.c;
+  // one reciprocal for 1/Sigma, 1/r, 1/sin^2, 1/theta_X
+  const double Sr = Sig * r, st = s2 * p.tp;
+  const double t = ip_rcp(Sr * st);
+  const double iS = t * r * st, ir = t * Sig * st, is2 = t * Sr * p.tp, itp = t * Sr * s2;
+  const double f = 2.0 * m * r * iS;
+  const double fr = 2.0 * m * (a2 * p.c * p.c - r2) * (iS * iS);   // df/dr
+  const double ft = f * a2 * S2 * iS;                               // df/dtheta
+  const double ut = K[0], ur = r * K[1], uh = p.tp * K[2], up = K[3];
+  const double P = ut + ur - a * s2 * up;
+  const double hp = uh * up;                       // theta' phi'
+  const double W = (fr * ur + ft * uh) * P - f * a * S2 * hp;
+  const double ra = r2 + a2;
+  const double Rt = -W;
+  const double Rr = r * (uh * uh + s2 * up * up) + 0.5 * fr * P * P + a * S2 * hp - W;
+  const double Rh = 0.5 * S2 * (ra * up * up - a2 * uh * uh - 2.0 * a * up * (ur + f * P)) + 0.5 * ft * P * P
+                    - (2.0 * r * ur - a2 * S2 * uh) * uh;
+  const double Rp = a * S2 * uh * (ur + f * P) + a * s2 * W - (2.0 * r * ur * s2 + ra * S2 * uh) * up;
+  const double Del = ra - 2.0 * m * r;
+  const double tdd = f * Rr - (1.0 + f) * Rt;
+  const double rdd = f * Rt + iS * (Del * Rr + a * Rp);
+  const double hdd = iS * Rh;
+  const double pdd = iS * (a * Rr + is2 * Rp);
+  dK[0] = tdd;
+  dK[1] = rdd * ir - K[1] * K[1];
+  dK[2] = (hdd - p.tpp * K[2] * K[2]) * itp;
+  dK[3] = pdd;
+}
+
+__device__ __forceinline__ void geodesic_accel_gamma(const Geom& G, Point& p, const double K[4], double dK[4]);
 __device__ __forceinline__ void geodesic_accel_at(const Geom& G, Point& p, const double K[4], double dK[4]) {
+#if IPOLE_GEO_KS
+  geodesic_accel_ks(G, p, K, dK);
+#else
+  geodesic_accel_gamma(G, p, K, dK);
+#endif
+}
+
+// the same through the derivative matrices D1, D2 (header of this file)
+__device__ __forceinline__ void geodesic_accel_gamma(const Geom& G, Point& p, const double K[4], double dK[4]) {
   Sym7 g, D1, D2; Inv6 gi;
   metric_derivs_at(G, p, g, gi, D1, D2);
   double v1[4], v2[4], F[4];
