@@ -12,8 +12,9 @@
  * this library.  It shares no source, header, table or constant generator with the CUDA path.
  *
  * Parity pins (tests/test_oracle_*.py, all -m "not gpu"): G1-G6 metric/connection/geodesic/shadow,
- * T1-T8 transport/operator/slab/absorption/Faraday/invariant/coefficients.  Parity unpinned: the
- * paper's Fig. 1 / Table 1 images (figures and data sets are not available).
+ * T1-T9 transport/operator/slab/absorption/Faraday/invariant/coefficients/frequency powers, E1-E5 numerically
+ * integrated eDF coefficients.  Parity unpinned: the paper's Fig. 1 / Table 1 images (figures and data sets are not
+ * available); the shape of the Faraday-conversion fit f(X) away from X -> 0; j_V, alpha_V of the kappa distribution.
  */
 #ifndef IPOLE_REF_H
 #define IPOLE_REF_H
@@ -73,6 +74,37 @@ int  ipole_ref_set_unpolarized(ipole_ref_ctx*, int on);
  * -(needed) if cap is too small. */
 int  ipole_ref_retrace(ipole_ref_ctx*, const double Xn[4], const double Kn[4], int cap,
                        double* X /*[cap+1][4]*/, double* K /*[cap+1][4]*/, double* dl /*[cap]*/);
+/* Second physics workload (eDFs whose synchrotron emissivity "requires numerical integration during ray
+ * tracing"; reading R-13 in ref_edf.hpp): kind 0 thermal fits (default), 1 Maxwell-Juettner, 2 kappa distribution with
+ * width w = Theta_e; j_{I,Q,V} and alpha_{I,Q,V} by the midpoint rule in ln(gamma) with n_nodes cells on [1, gamma_max];
+ * rho_Q, rho_V stay thermal.  Pins E1-E5 (tests/test_oracle_edf.py).  Returns -1 on bad arguments. */
+int  ipole_ref_set_edf(ipole_ref_ctx*, int kind, double kappa, double gamma_max, int n_nodes);
+/* the coefficient stage on its own: out = (jI,jQ,jV,aI,aQ,aV,rQ,rV), cgs, plasma frame */
+void ipole_ref_coefficients_edf(int kind, double kappa, double gamma_max, int n_nodes, double ne, double thetae, double B,
+                                double cosT, double nu, double out[8]);
+/* F(x) = x int_x^inf K_5/3, G(x) = x K_2/3(x), H(x) = x K_1/3(x) + int_x^inf K_1/3 */
+void ipole_ref_synchrotron_kernels(double x, double out[3]);
+/* ---- stage entries used by the pins (tests/test_oracle_*.py) ---- */
+void ipole_ref_gcov(double a, double hslope, int flat, const double X[4], double g[16]);
+void ipole_ref_gcon(double a, double hslope, int flat, const double X[4], double g[16]);
+void ipole_ref_dgcov(double a, double hslope, int flat, const double X[4], double dg[64]);
+void ipole_ref_conn(double a, double hslope, int flat, const double X[4], double Gamma[64]);
+void ipole_ref_coefficients(double ne, double thetae, double B, double cosT, double nu, double out[8]);
+void ipole_ref_bessel_kscaled(double z, double out[3]);
+void ipole_ref_stokes_operator(const double alpha[4], const double rho[3], double s, double O[16], double P[16]);
+int64_t ipole_ref_total_steps(ipole_ref_ctx*);                       /* geodesic steps of the last make_pixels */
+int  ipole_ref_camera_tetrad(ipole_ref_ctx*, double Xcam[4], double e[16]);
+int  ipole_ref_camera_ray(ipole_ref_ctx*, int i, int j, double X[4], double K[4]);
+int  ipole_ref_camera_ray_ab(ipole_ref_ctx*, double alpha, double beta, double X[4], double K[4]);
+/* backward geodesic from (X0, K0): points 0..n, step sizes, theta turning points, stop status (1 horizon, 2 escape,
+ * 3 step limit); returns n or -(needed) if cap is too small */
+int  ipole_ref_trace(ipole_ref_ctx*, const double X0[4], const double K0[4], int cap, double* X, double* K, double* dl,
+                     int32_t* nturn, int32_t* status);
+int  ipole_ref_plasma(ipole_ref_ctx*, const double X[4], double out[12]);   /* present, ne, thetae, B, u[4], b[4] */
+int  ipole_ref_plasma_tetrad(ipole_ref_ctx*, const double X[4], const double K[4], const double u[4], const double b[4],
+                             double econ[16], double ecov[16]);
+/* vacuum transport of a complex tensor N (32 doubles, re/im interleaved) along n stored steps, far end -> camera */
+int  ipole_ref_transport_vacuum(ipole_ref_ctx*, int n, const double* X, const double* K, const double* dl, double N[32]);
 /* camera-type tetrad e[a][mu] at an arbitrary point (static observer, e3 from d_X1, e2 from -d_X2, e1 from d_X3) */
 int  ipole_ref_observer_tetrad(ipole_ref_ctx*, const double X[4], double e[16]);
 

@@ -23,6 +23,7 @@
 #include "ref_geodesic.hpp"
 #include "ref_plasma.hpp"
 #include "ref_coeff.hpp"
+#include "ref_edf.hpp"
 #include "ref_stokes_op.hpp"
 
 namespace iref {
@@ -31,6 +32,7 @@ typedef std::complex<double> cplx;
 
 struct Model {
   int kind = MODEL_NONE;
+  EdfParams edf;       // kind 0: thermal fits; otherwise j, alpha integrated over the eDF (ref_edf.hpp)
   AdafParams adaf;
   SlabParams slab;
   GridParams grid;
@@ -188,7 +190,7 @@ inline bool plasma_operator(const Geom& G, const Model& M, const Units& U, const
     double cosT = bk / (om * p.B);
     if (cosT > 1.0) cosT = 1.0;
     if (cosT < -1.0) cosT = -1.0;
-    const CoeffCGS c = synchrotron_coefficients(p.ne, p.Th, p.B, cosT, nu);
+    const CoeffCGS c = synchrotron_coefficients_edf(M.edf, p.ne, p.Th, p.B, cosT, nu);
     jc[0] = c.jI; jc[1] = c.jQ; jc[2] = 0.0; jc[3] = c.jV;
     ac[0] = c.aI; ac[1] = c.aQ; ac[2] = 0.0; ac[3] = c.aV;
     rc[0] = c.rQ; rc[1] = 0.0; rc[2] = c.rV;

@@ -39,7 +39,7 @@ inline void unpolarized_step(const Geom& G, const Model& M, const Units& U, cons
     double cosT = bk / (om * p.B);
     if (cosT > 1.0) cosT = 1.0;
     if (cosT < -1.0) cosT = -1.0;
-    const CoeffCGS c = synchrotron_coefficients(p.ne, p.Th, p.B, cosT, nu);
+    const CoeffCGS c = synchrotron_coefficients_edf(M.edf, p.ne, p.Th, p.B, cosT, nu);
     jc = c.jI; ac = c.aI;
   }
   const double ji = jc / (nu * nu), ai = ac * nu;
