@@ -136,6 +136,20 @@ int  ipole_set_path_free(ipole_ctx*, int32_t on);
  * crosses no plasma).  The two give the same image up to rounding.  on == 2 is a test mode: as 1, but every seventh
  * ray of a batch is handed to the single kernel as if it had such a step.  Returns IPOLE_EINVAL for a NULL context. */
 int  ipole_set_transfer_split(ipole_ctx*, int32_t on);
+/* Second physics workload (outlook: electron distribution functions "for which accurate prescriptions ... do
+ * not exist and the integration of synchrotron emissivity over the electron energy distribution function requires
+ * numerical integration during ray tracing"; the paper gives no formulas: reading R-13 in DESIGN.md).
+ * kind 0 (default): the thermal fits.  kind 1: Maxwell-Juettner, n(gamma) = N gamma^2 beta exp(-gamma/Theta_e).  kind 2: kappa
+ * distribution, n(gamma) = N gamma^2 beta [1 + (gamma-1)/(kappa w)]^-(kappa+1) with w = Theta_e of the plasma model.  For
+ * kind != 0 every transfer step evaluates j_{I,Q,V} = C int n {F, G, (4 cot/3) H/gamma} dgamma and alpha_{I,Q,V} =
+ * -(C/(2 m nu^2)) int {..} gamma^2 d/dgamma[n/gamma^2] dgamma (single-electron synchrotron kernels F, G, H; x = nu / nu_cr(gamma))
+ * by the midpoint rule in ln(gamma) on n_nodes cells of [1, gamma_max]; N from int n dgamma = n_e with the same rule;
+ * rho_Q, rho_V stay thermal.  Supported for the analytic flow on the stored path (ipole_make_image, _pixels,
+ * _image_adaptive); those calls return IPOLE_EINVAL for another model, the sweeps, the path-free or the unpolarized
+ * variant while kind != 0.  Zero fields take the defaults kappa 3.5, gamma_max 3e4, n_nodes 128.
+ * IPOLE_EINVAL: NULL, kind outside 0..2, kappa <= 1, gamma_max <= 1, n_nodes > 65536. */
+typedef struct { int32_t kind; int32_t n_nodes; double kappa; double gamma_max; } ipole_edf;
+int  ipole_set_edf(ipole_ctx*, const ipole_edf*);
 /* Unpolarized transfer (the model-fitting loop makes "nonpolarized images"; polarized
  * transfer is "far more complex and computationally demanding"; reading R-12 in DESIGN.md).  on != 0: every image
  * entry (ipole_make_image, _pixels, _images_adaf, _images_grid, _image_adaptive) solves the scalar equation
@@ -223,6 +237,8 @@ int  ipole_trace_pixel(ipole_ctx*, int32_t i, int32_t j, int32_t cap, double* X,
  *   bessel: z[n] -> (e^z K0, e^z K1, e^z K2)[n][3] */
 int  ipole_eval_connection(ipole_ctx*, int64_t n, const double* X, double* Gamma);
 int  ipole_eval_coefficients(ipole_ctx*, int64_t n, const double* in5, double* out8);
+/* as coeff, with j and alpha of the context's electron distribution (ipole_set_edf) */
+int  ipole_eval_coefficients_edf(ipole_ctx*, int64_t n, const double* in5, double* out8);
 int  ipole_eval_stokes_step(ipole_ctx*, int64_t n, const double* in16, double* out4);
 int  ipole_eval_bessel(ipole_ctx*, int64_t n, const double* z, double* out3);
 /* The branch-free elementary functions of the hot loops (csrc/fpmath.cuh) at n points x (host):

@@ -58,7 +58,8 @@ struct ipole_ctx {
   int opt_split = 1;             // stored path, analytic flow: transfer as k_stepop + k_apply (stepop.cuh)
   double* d_ops = nullptr; size_t ops_bytes = 0;   // operator records of one batch
   int32_t* d_irr = nullptr;      // slots of the rays k_stepop leaves to k_transfer
-  int occ_op = 0, occ_ap = 0;
+  int occ_op = 0, occ_ap = 0, occ_ap_edf = 0;
+  EdfDev edf = {0, 128, 3.5, 0.0};   // electron distribution of the coefficient step (ipole_set_edf); kind 0: thermal fits
   int occ_unpol[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};
   double* d_endp = nullptr; int64_t endp_cap = 0;   // end points of the backward passes, [rays][8]
   long long* d_sum = nullptr;    // forward-step total of the path-free variant
@@ -351,7 +352,9 @@ int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStrea
   {
     const int s = span_begin(c, LK_APPLY, st);
     const int g = grid_for(c, c->occ_ap, IPOLE_AP_THREADS / 32, (rays + 31) / 32, reserve);   // one warp per 32 rays
-    k_apply<<<g, IPOLE_AP_THREADS, 0, st>>>(p);
+    p.edf = c->edf;
+    if (c->edf.kind != 0) k_apply<true><<<grid_for(c, c->occ_ap_edf, IPOLE_AP_THREADS / 32, (rays + 31) / 32, reserve), IPOLE_AP_THREADS, 0, st>>>(p);
+    else k_apply<false><<<g, IPOLE_AP_THREADS, 0, st>>>(p);
     span_end(c, s, st);
     c->stats.n_launches++;
     CK(cudaGetLastError());
@@ -479,6 +482,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     const int64_t per = (int64_t)(budget / rec_bytes / (size_t)n) - 1;
     cap = (int)std::max<int64_t>(64, std::min<int64_t>(max_steps, per));
   }
+  if (c->edf.kind != 0 && c->opt_path_free) return IPOLE_EINVAL;
   if (c->opt_path_free && !sw && !c->opt_unpol) {
     // ---- path-free bidirectional variant: one geodesic launch that keeps the end points, one
     // transfer launch that re-integrates forward.  Rays are ordered longest first, so the few very long rays start
@@ -567,7 +571,11 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   // the first batch or two; every later batch holds two to three times as many rays in the same memory, and the
   // persistent kernels have that many fewer tails.  A ray that outgrows its batch's slot is listed and retried at
   // the end with the global S_cap (second level); one that outgrows S_cap goes to the long-ray pass as before.
-  const bool split = c->opt_split && !sw && !c->opt_unpol && c->model == MODEL_ADAF;
+  // numerically integrated eDF coefficients (ipole_set_edf) live in k_apply only: that mode always runs split, and its
+  // long rays go through the same kernels (third level, slots of max_steps) instead of the single kernel on the side stream
+  const bool edf = c->edf.kind != 0;
+  if (edf && (sw || c->opt_unpol || c->model != MODEL_ADAF)) return IPOLE_EINVAL;
+  const bool split = edf || (c->opt_split && !sw && !c->opt_unpol && c->model == MODEL_ADAF);
   const size_t step_bytes = rec_bytes + (split ? OP_DOUBLES * sizeof(double) : 0);
   const bool tight = order != nullptr && !bin_prefix.empty() && c->opt_tight;
   struct Batch { int64_t base, cnt; int cap; };
@@ -618,7 +626,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     if (use_occ) { g.grid = (const GridParams*)c->d_model; g.srange = c->d_srange; }
     int rcb;
     if ((rcb = launch_geodesic(c, g, LK_GEO, b.cnt, c->stream, reserve)) != IPOLE_OK) return rcb;
-    if (top && cap < max_steps) {
+    if (top && cap < max_steps && !edf) {
       CK(cudaEventRecord(c->ev_geo, c->stream));
       CK(cudaStreamWaitEvent(c->side, c->ev_geo, 0));
     }
@@ -633,7 +641,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     else rcb = launch_transfer(c, t, LK_RT, b.cnt, c->stream, reserve, 0, sw);
     if (rcb != IPOLE_OK) return rcb;
     c->stats.n_batches++;
-    if (top && cap < max_steps) {   // the transfer kernel just queued keeps the GPU busy while the host waits here
+    if (top && cap < max_steps && !edf) {   // the transfer kernel just queued keeps the GPU busy while the host waits here
       if ((rcb = listed(c->ev_geo, n_long)) != IPOLE_OK) return rcb;
       if ((rcb = long_pass(n_long)) != IPOLE_OK) return rcb;
     }
@@ -661,7 +669,28 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
         if ((rc = run_batch(b, c->d_retry)) != IPOLE_OK) return rc;
     }
   }
-  c->stats.n_long = n_long;
+  if (edf && cap < max_steps) {
+    // third level: rays longer than S_cap, through the same split kernels with slots of max_steps
+    CK(cudaMemcpyAsync(&n_long, c->d_small, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    if (n_long > 0) {
+      const int cap_saved = cap;
+      cap = max_steps;
+      make_plan(n_long, false);
+      size_t np3 = 0, no3 = 0;
+      for (const Batch& b : plan) {
+        np3 = std::max(np3, (size_t)b.cnt * (size_t)(b.cap + 1) * rec_bytes);
+        no3 = std::max(no3, (size_t)((b.cnt + 31) / 32 * 32) * (size_t)(b.cap + 1) * OP_DOUBLES * sizeof(double));
+      }
+      if ((rc = ensure_path(c, np3)) != IPOLE_OK) return rc;
+      if ((rc = ensure_ops(c, no3)) != IPOLE_OK) return rc;
+      for (const Batch& b : plan)
+        if ((rc = run_batch(b, c->d_long)) != IPOLE_OK) return rc;
+      cap = cap_saved;
+    }
+    c->stats.n_long = n_long;
+    n_long = 0;   // nothing ran on the side stream
+  } else c->stats.n_long = n_long;
   if (n_long > 0) {
     // join the side stream, then publish the step counts of the long rays (the bulk transfer kernels read
     // nsteps[q] = -1 for them, so the long passes keep theirs apart until every bulk kernel is done)
@@ -735,7 +764,8 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_unpol[MODEL_GRID][1], k_transfer_unpol<MODEL_GRID, true>, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_sweep[MODEL_GRID], k_transfer<MODEL_GRID, 0, true>, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_op, k_stepop<MODEL_ADAF>, IPOLE_OP_THREADS, 0);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap, k_apply, IPOLE_AP_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap, k_apply<false>, IPOLE_AP_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_edf, k_apply<true>, IPOLE_AP_THREADS, 0);
   { const char* e = std::getenv("IPOLE_NO_SPLIT"); if (e && e[0] == '1') c->opt_split = 0; }
   { const char* e = std::getenv("IPOLE_NO_TIGHT"); if (e && e[0] == '1') c->opt_tight = 0; }
   { const char* e = std::getenv("IPOLE_NO_GROUP"); if (e && e[0] == '1') c->opt_group = 0; }
@@ -789,6 +819,17 @@ int ipole_set_options(ipole_ctx* c, uint64_t path_bytes, int32_t sort_rays) {
 int ipole_set_unpolarized(ipole_ctx* c, int32_t on) {
   if (!c) return IPOLE_EINVAL;
   c->opt_unpol = on ? 1 : 0;
+  return IPOLE_OK;
+}
+
+int ipole_set_edf(ipole_ctx* c, const ipole_edf* e) {
+  if (!c || !e) return IPOLE_EINVAL;
+  if (e->kind < 0 || e->kind > 2) return IPOLE_EINVAL;
+  const int nn = e->n_nodes > 0 ? e->n_nodes : 128;
+  const double gmax = e->gamma_max > 0.0 ? e->gamma_max : 3.0e4;
+  const double kappa = e->kappa > 0.0 ? e->kappa : 3.5;
+  if (e->kind != 0 && (!(gmax > 1.0) || nn > 65536 || (e->kind == 2 && !(kappa > 1.0)))) return IPOLE_EINVAL;
+  c->edf.kind = e->kind; c->edf.n_nodes = nn; c->edf.kappa = kappa; c->edf.du = std::log(gmax) / nn;
   return IPOLE_OK;
 }
 
@@ -1257,6 +1298,9 @@ int ipole_eval_connection(ipole_ctx* c, int64_t n, const double* X, double* Gamm
 }
 int ipole_eval_coefficients(ipole_ctx* c, int64_t n, const double* in5, double* out8) {
   return eval_host(c, n, in5, 5, out8, 8, [&](int g, int b, double* i, double* o) { k_eval_coefficients<<<g, b, 0, c->stream>>>(n, i, o); });
+}
+int ipole_eval_coefficients_edf(ipole_ctx* c, int64_t n, const double* in5, double* out8) {
+  return eval_host(c, n, in5, 5, out8, 8, [&](int g, int b, double* i, double* o) { k_eval_coefficients_edf<<<g, b, 0, c->stream>>>(c->edf, n, i, o); });
 }
 int ipole_eval_stokes_step(ipole_ctx* c, int64_t n, const double* in16, double* out4) {
   return eval_host(c, n, in16, 16, out4, 4, [&](int g, int b, double* i, double* o) { k_eval_stokes_step<<<g, b, 0, c->stream>>>(n, i, o); });

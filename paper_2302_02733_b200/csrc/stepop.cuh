@@ -21,6 +21,7 @@
 // buffer.  With the analytic ADAF flow every step crosses plasma, so the list is empty in practice.
 #pragma once
 #include "kernels.cuh"
+#include "edf.cuh"
 
 namespace ipole {
 
@@ -155,6 +156,7 @@ __global__ void __launch_bounds__(IPOLE_OP_THREADS, IPOLE_OP_MINB) k_stepop(cons
 
 struct ApArgs {
   AdafParams model;           // the three power laws (by value: 56 B)
+  EdfDev edf;                 // k_apply<true>: j, alpha by quadrature over the electron distribution (edf.cuh)
   double nu3;                 // nu_obs^3: invariant I/nu^3 -> specific intensity at the camera
   int cap;
   int64_t base, count;
@@ -187,7 +189,9 @@ __device__ __noinline__ Stokes4 stokes_step_qv_closed(double aI, double aQ, doub
 // to the camera; a lane joins when the walk reaches its own far end.  Rays are ordered by predicted step count, so
 // the 32 rays of a group have similar lengths.  The record of the next step is loaded (three coalesced 256-bit loads)
 // while the current one is applied.
-__global__ void __launch_bounds__(IPOLE_AP_THREADS, IPOLE_AP_MINB) k_apply(const __grid_constant__ ApArgs A) {
+// EDF: the coefficients of a step by numerical integration over the electron distribution function (edf.cuh)
+template <bool EDF>
+__global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? 3 : IPOLE_AP_MINB) k_apply(const __grid_constant__ ApArgs A) {
   const int lane = threadIdx.x & 31;
   const int64_t n_groups = (A.count + 31) >> 5;
   for (;;) {
@@ -222,7 +226,7 @@ __global__ void __launch_bounds__(IPOLE_AP_THREADS, IPOLE_AP_MINB) k_apply(const
       ld_global_v4(p, R[0], R[1], R[2], R[3]);
       ld_global_v4(p + 128, R[4], R[5], R[6], R[7]);
     };
-    if (smax - 1 < n) load(smax - 1);
+    if (smax > 0 && smax - 1 < n) load(smax - 1);   // (a group whose rays all went to another pass has smax = 0)
     for (int s = smax - 1; s >= 0; --s) {
       const bool on = s < n;
       const double m11 = R[0], m12 = R[1], m21 = R[2], m22 = R[3];
@@ -232,7 +236,7 @@ __global__ void __launch_bounds__(IPOLE_AP_THREADS, IPOLE_AP_MINB) k_apply(const
         stokes_congruence(m11, m12, m21, m22, S);
         double ne, Th, B;
         adaf_scalars(A.model, x1, ne, Th, B);
-        const Coeff c = synchrotron_invariant(ne, Th, B, cosT, nu);
+        const Coeff c = EDF ? synchrotron_edf_invariant(A.edf, ne, Th, B, cosT, nu) : synchrotron_invariant(ne, Th, B, cosT, nu);
         const double xI = c.aI * ds, xQ = c.aQ * ds, xV = c.aV * ds, yQ = c.rQ * ds, yV = c.rV * ds;
         const double eI = c.jI * ds, eQ = c.jQ * ds, eV = c.jV * ds;
         if (IP_UNLIKELY(!stokes_step_qv_series(xI, xQ, xV, yQ, yV, 1.0, eI, eQ, eV, S))) {

@@ -17,10 +17,10 @@ _LIB = None
 OK, EINVAL, ENOMODEL, ENOMEM, ECUDA, ENOIMAGE = 0, -1, -2, -3, -4, -5
 
 #: every symbol include/ipole.h declares (checked by tests/test_abi.py)
-SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_options", "ipole_set_path_free", "ipole_set_transfer_split", "ipole_set_unpolarized", "ipole_load_model_adaf",
+SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_options", "ipole_set_path_free", "ipole_set_edf", "ipole_set_transfer_split", "ipole_set_unpolarized", "ipole_load_model_adaf",
            "ipole_load_model_slab", "ipole_load_model_grid", "ipole_make_image", "ipole_make_pixels", "ipole_make_images_adaf", "ipole_make_images_grid", "ipole_make_image_adaptive",
            "ipole_get_ray_info", "ipole_get_stats", "ipole_get_camera_tetrad", "ipole_trace_pixel",
-           "ipole_eval_connection", "ipole_eval_coefficients", "ipole_eval_stokes_step", "ipole_eval_bessel",
+           "ipole_eval_connection", "ipole_eval_coefficients", "ipole_eval_coefficients_edf", "ipole_eval_stokes_step", "ipole_eval_bessel",
            "ipole_eval_plasma", "ipole_eval_math", "ipole_measure_fp64_peak", "ipole_last_cuda_error", "ipole_free", "ipole_strerror",
            "ipole_version"]
 
@@ -56,6 +56,10 @@ class Stats(C.Structure):
                 ("ms_long", C.c_float), ("total_steps_forward", C.c_int64), ("ms_stepop", C.c_float), ("ms_apply", C.c_float), ("n_retry", C.c_int64)]
 
 
+class Edf(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("n_nodes", C.c_int32), ("kappa", C.c_double), ("gamma_max", C.c_double)]
+
+
 class GridScales(C.Structure):
     _fields_ = [("M_unit", C.c_double), ("Rlow", C.c_double), ("Rhigh", C.c_double)]
 
@@ -87,6 +91,8 @@ def lib():
         L.ipole_set_path_free.argtypes = [vp, C.c_int32]
         L.ipole_set_unpolarized.argtypes = [vp, C.c_int32]
         L.ipole_set_transfer_split.argtypes = [vp, C.c_int32]
+        L.ipole_set_edf.argtypes = [vp, C.POINTER(Edf)]
+        L.ipole_eval_coefficients_edf.argtypes = [vp, C.c_int64, dp, dp]
         L.ipole_load_model_adaf.argtypes = [vp, C.POINTER(AdafParams)]
         L.ipole_load_model_slab.argtypes = [vp, C.POINTER(SlabParams)]
         L.ipole_load_model_grid.argtypes = [vp, C.POINTER(GridDesc), C.POINTER(vp)]
@@ -185,6 +191,12 @@ class Ipole:
     def set_transfer_split(self, on=True):
         """Transfer as a step-parallel operator pass + a per-ray apply pass (include/ipole.h ipole_set_transfer_split)."""
         _chk(lib().ipole_set_transfer_split(self._h, int(on)), "ipole_set_transfer_split")
+
+    def set_edf(self, kind, kappa=3.5, gamma_max=3.0e4, n_nodes=128):
+        """Electron distribution of the coefficient step (include/ipole.h ipole_set_edf): 0 thermal fits,
+        1 Maxwell-Juettner, 2 kappa; j and alpha by numerical integration over it."""
+        e = Edf(int(kind), int(n_nodes), float(kappa), float(gamma_max))
+        _chk(lib().ipole_set_edf(self._h, C.byref(e)), "ipole_set_edf")
 
     def set_unpolarized(self, on=True):
         """Unpolarized transfer of I alone (include/ipole.h ipole_set_unpolarized)."""
@@ -346,6 +358,10 @@ class Ipole:
     def eval_coefficients(self, ne, thetae, B, cosT, nu):
         x = np.stack(np.broadcast_arrays(ne, thetae, B, cosT, nu), axis=-1).astype(np.float64)
         return self._eval("coefficients", x, 5, 8)
+
+    def eval_coefficients_edf(self, ne, thetae, B, cosT, nu):
+        x = np.stack(np.broadcast_arrays(ne, thetae, B, cosT, nu), axis=-1).astype(np.float64)
+        return self._eval("coefficients_edf", x, 5, 8)
 
     def eval_stokes_step(self, alpha, rho, s, S0, J):
         x = np.concatenate([np.asarray(alpha, float).reshape(-1, 4), np.asarray(rho, float).reshape(-1, 3),

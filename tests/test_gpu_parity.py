@@ -195,6 +195,13 @@ def test_split_transfer_matches_the_single_kernel(ipole):
         assert np.max(np.abs(four[k] - two[k]) / scale) < 1e-11, k
         changed += int((four[k] != two[k]).sum())
     assert changed > 0   # the handed-over rays really went through the other kernel
+    # slots far too short for any ray: every ray goes to the long-ray pass and k_apply meets groups with nothing to do
+    g.set_transfer_split(True)
+    g.set_options(40 << 20, 0)
+    five = to_np(g.make_image(maps=True))
+    assert g.stats()["n_long"] == 64 * 64
+    for k in one:
+        assert np.array_equal(one[k], five[k]), k    # the long-ray pass is the single kernel
 
 
 def test_step_limit_flags_rays(ipole, ref):
