@@ -254,14 +254,14 @@ void ipole_ref_coefficients(double ne, double thetae, double B, double cosT, dou
 }
 void ipole_ref_bessel_kscaled(double z, double out[3]) { bessel_k_scaled(z, out); }
 
-int ipole_ref_set_edf(ipole_ref_ctx* x, int kind, double kappa, double gamma_max, int n_nodes) {
-  if (!x || kind < 0 || kind > 2 || (kind == 2 && !(kappa > 1.0)) || (kind != 0 && (!(gamma_max > 1.0) || n_nodes < 1))) return -1;
-  x->model.edf.kind = kind; x->model.edf.kappa = kappa; x->model.edf.gamma_max = gamma_max; x->model.edf.n_nodes = n_nodes;
+int ipole_ref_set_edf(ipole_ref_ctx* x, int kind, double kappa, int n_nodes) {
+  if (!x || kind < 0 || kind > 2 || (kind == 2 && !(kappa > 1.0)) || (kind != 0 && n_nodes < 1)) return -1;
+  x->model.edf.kind = kind; x->model.edf.kappa = kappa; x->model.edf.n_nodes = n_nodes;
   return 0;
 }
-void ipole_ref_coefficients_edf(int kind, double kappa, double gamma_max, int n_nodes, double ne, double thetae, double B,
+void ipole_ref_coefficients_edf(int kind, double kappa, int n_nodes, double ne, double thetae, double B,
                                 double cosT, double nu, double out[8]) {
-  EdfParams E; E.kind = kind; E.kappa = kappa; E.gamma_max = gamma_max; E.n_nodes = n_nodes;
+  EdfParams E; E.kind = kind; E.kappa = kappa; E.n_nodes = n_nodes;
   const CoeffCGS c = synchrotron_coefficients_edf(E, ne, thetae, B, cosT, nu);
   out[0] = c.jI; out[1] = c.jQ; out[2] = c.jV; out[3] = c.aI; out[4] = c.aQ; out[5] = c.aV; out[6] = c.rQ; out[7] = c.rV;
 }

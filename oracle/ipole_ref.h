@@ -76,11 +76,11 @@ int  ipole_ref_retrace(ipole_ref_ctx*, const double Xn[4], const double Kn[4], i
                        double* X /*[cap+1][4]*/, double* K /*[cap+1][4]*/, double* dl /*[cap]*/);
 /* Second physics workload (eDFs whose synchrotron emissivity "requires numerical integration during ray
  * tracing"; reading R-13 in ref_edf.hpp): kind 0 thermal fits (default), 1 Maxwell-Juettner, 2 kappa distribution with
- * width w = Theta_e; j_{I,Q,V} and alpha_{I,Q,V} by the midpoint rule in ln(gamma) with n_nodes cells on [1, gamma_max];
+ * width w = Theta_e; j_{I,Q,V} and alpha_{I,Q,V} by the midpoint rule on n_nodes cells in ln x, x = nu/nu_cr(gamma) (ref_edf.hpp);
  * rho_Q, rho_V stay thermal.  Pins E1-E5 (tests/test_oracle_edf.py).  Returns -1 on bad arguments. */
-int  ipole_ref_set_edf(ipole_ref_ctx*, int kind, double kappa, double gamma_max, int n_nodes);
+int  ipole_ref_set_edf(ipole_ref_ctx*, int kind, double kappa, int n_nodes);
 /* the coefficient stage on its own: out = (jI,jQ,jV,aI,aQ,aV,rQ,rV), cgs, plasma frame */
-void ipole_ref_coefficients_edf(int kind, double kappa, double gamma_max, int n_nodes, double ne, double thetae, double B,
+void ipole_ref_coefficients_edf(int kind, double kappa, int n_nodes, double ne, double thetae, double B,
                                 double cosT, double nu, double out[8]);
 /* F(x) = x int_x^inf K_5/3, G(x) = x K_2/3(x), H(x) = x K_1/3(x) + int_x^inf K_1/3 */
 void ipole_ref_synchrotron_kernels(double x, double out[3]);

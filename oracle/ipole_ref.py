@@ -82,8 +82,8 @@ def lib():
         L.ipole_ref_observer_tetrad.argtypes = [C.c_void_p, dp, dp]
         L.ipole_ref_total_steps.argtypes = [C.c_void_p]
         L.ipole_ref_total_steps.restype = C.c_int64
-        L.ipole_ref_set_edf.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_int]
-        L.ipole_ref_coefficients_edf.argtypes = [C.c_int, C.c_double, C.c_double, C.c_int] + [C.c_double] * 5 + [dp]
+        L.ipole_ref_set_edf.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_int]
+        L.ipole_ref_coefficients_edf.argtypes = [C.c_int, C.c_double, C.c_int] + [C.c_double] * 5 + [dp]
         L.ipole_ref_coefficients_edf.restype = None
         L.ipole_ref_synchrotron_kernels.argtypes = [C.c_double, dp]
         L.ipole_ref_synchrotron_kernels.restype = None
@@ -121,10 +121,10 @@ def coefficients(ne, thetae, B, cosT, nu):
     out = np.zeros(8); lib().ipole_ref_coefficients(ne, thetae, B, cosT, nu, _dp(out)); return out
 
 
-def coefficients_edf(kind, ne, thetae, B, cosT, nu, kappa=3.5, gamma_max=3.0e4, n_nodes=128):
+def coefficients_edf(kind, ne, thetae, B, cosT, nu, kappa=3.5, n_nodes=128):
     """(jI,jQ,jV,aI,aQ,aV,rQ,rV) with j, alpha integrated over the eDF (oracle/ref_edf.hpp): kind 1 Maxwell-Juettner, 2 kappa."""
     out = np.zeros(8)
-    lib().ipole_ref_coefficients_edf(int(kind), float(kappa), float(gamma_max), int(n_nodes), ne, thetae, B, cosT, nu, _dp(out))
+    lib().ipole_ref_coefficients_edf(int(kind), float(kappa), int(n_nodes), ne, thetae, B, cosT, nu, _dp(out))
     return out
 
 
@@ -245,9 +245,9 @@ class Ctx:
         if rc != 0:
             raise RuntimeError("set_path_free failed: %d" % rc)
 
-    def set_edf(self, kind, kappa=3.5, gamma_max=3.0e4, n_nodes=128):
+    def set_edf(self, kind, kappa=3.5, n_nodes=128):
         """j, alpha by numerical integration over the eDF (0 thermal fits, 1 Maxwell-Juettner, 2 kappa)."""
-        rc = lib().ipole_ref_set_edf(self._h, int(kind), float(kappa), float(gamma_max), int(n_nodes))
+        rc = lib().ipole_ref_set_edf(self._h, int(kind), float(kappa), int(n_nodes))
         if rc != 0:
             raise RuntimeError("set_edf failed: %d" % rc)
 
