@@ -33,8 +33,10 @@ FLOP_PER_STEP = {"transfer_adaf": 1576.0, "transfer_grid": 390.0, "geodesic_adaf
 # profiles/r2_k_stepop_adaf1024.txt, r2_k_apply_adaf1024.txt, r1_k_transfer_*.txt, r1_k_geodesic_*.txt
 FLOP_EXECUTED = {"k_stepop": 1018.0, "k_apply": 574.0, "k_transfer<adaf>": 1576.0, "k_transfer<grid>": 390.0,
                  "k_geodesic": 994.0, "k_geodesic<occ>": 1183.0}
+# second physics workload (--edf): k_apply<true> per step, 128 quadrature nodes (profiles/r2_k_apply_edf_adaf256.txt)
+FLOP_EXECUTED.update({"k_apply<edf 1>": 11383.0, "k_apply<edf 2>": 18268.0})
 FP64_PIPE_PCT = {"k_stepop": 72.7, "k_apply": 64.8, "k_transfer<adaf>": 58.5, "k_transfer<grid>": 48.0,
-                 "k_geodesic": 82.0, "k_geodesic<occ>": 79.0}
+                 "k_geodesic": 82.0, "k_geodesic<occ>": 79.0, "k_apply<edf 1>": 55.9, "k_apply<edf 2>": 55.2}
 # DRAM bytes per step of k_transfer (dram__bytes_read + write of one launch / its thread-steps, same captures)
 DRAM_BYTES_PER_STEP = {"transfer_adaf": 64.2, "transfer_grid": 33.8}
 DRAM_BYTES_PER_STEP_SPLIT = 192.0   # k_stepop reads 64.1 B and writes 64.0 B per step, k_apply reads 64.0 B (profiles/r2_k_*.txt)
@@ -248,7 +250,7 @@ def grid_inputs(shape):
     return _GRID_CACHE[shape]
 
 
-def oracle_sample(workload, n_rays, nthreads, path_free=False, unpolarized=False):
+def oracle_sample(workload, n_rays, nthreads, path_free=False, unpolarized=False, edf=0):
     """The CPU oracle, as it stands, on a strided sample of the workload's image.  Returns (rays, steps, seconds)."""
     import numpy as np
     from oracle import ipole_ref
@@ -265,6 +267,8 @@ def oracle_sample(workload, n_rays, nthreads, path_free=False, unpolarized=False
         r.set_path_free(True)
     if unpolarized:
         r.set_unpolarized(True)
+    if edf:
+        r.set_edf(edf)
     n = wl["n"]
     stride = max(1, int(round(n / max(1.0, n_rays ** 0.5))))
     ii, jj = np.meshgrid(np.arange(stride // 2, n, stride), np.arange(stride // 2, n, stride))
@@ -418,6 +422,8 @@ def measure_image(args, name, ipole, replicas, W, world, rank, local, barrier):
         g.set_unpolarized(True)
     if args.single_kernel:
         g.set_transfer_split(False)
+    if args.edf:
+        g.set_edf(args.edf)
     grid_bytes = 0
     if wl["kind"] == "adaf":
         g.load_adaf(**W.ADAF)
@@ -485,6 +491,8 @@ def measure_image(args, name, ipole, replicas, W, world, rank, local, barrier):
     pf = args.path_free
     split = st["ms_stepop"] > 0.0
     fl_rt = FLOP_PER_STEP_PF[key] if pf else FLOP_PER_STEP[key]
+    if args.edf:   # no round-1 count exists for this workload: its algorithmic count IS the executed one (k_stepop + k_apply<edf>)
+        fl_rt = FLOP_EXECUTED["k_stepop"] + FLOP_EXECUTED["k_apply<edf %d>" % args.edf]
     if args.unpolarized:
         fl_rt = FLOP_PER_STEP_UNPOL[key] or 0.0
     # steps the bulk transfer kernels walk: the long rays (>= path_cap steps each) run on the side stream, outside rt_ms
@@ -514,7 +522,9 @@ def measure_image(args, name, ipole, replicas, W, world, rank, local, barrier):
                           "CUDA-event time / peak; frac_executed uses what the shipped kernels execute (ncu); "
                           "fp64_pipe_pct is sm__inst_executed_pipe_fp64 of the ncu captures under profiles/, not live")
     if not (pf or args.unpolarized):
-        if split:
+        if args.edf:
+            parts = {"k_stepop": st["ms_stepop"], "k_apply<edf %d>" % args.edf: st["ms_apply"]}
+        elif split:
             parts = {"k_stepop": st["ms_stepop"], "k_apply": st["ms_apply"]}
         else:
             parts = {"k_transfer<%s>" % wl["kind"]: rt_ms}
@@ -545,6 +555,7 @@ def measure_image(args, name, ipole, replicas, W, world, rank, local, barrier):
                        "model": wl["kind"], "freq_ghz": 230, "eps": cam["eps"], "maps": maps,
                        "variant": "unpolarized, I alone (PAPER.md:74), stored path" if args.unpolarized else
                                   "path-free bidirectional (PAPER.md:43)" if pf else
+                                  "stored path, split transfer, j and alpha integrated over the eDF at every step (PAPER.md:78; kind %d)" % args.edf if args.edf else
                                   "stored path, split transfer (k_stepop + k_apply)" if split else "stored path, single transfer kernel",
                        "full_stokes": not args.unpolarized,
                        "l2": ("no flush needed: nothing is re-read; per image %.2f GB of end points and outputs stream once"
@@ -568,7 +579,8 @@ def measure_image(args, name, ipole, replicas, W, world, rank, local, barrier):
 
     if not args.no_cpu_baseline and world == 1:
         cores = os.cpu_count() or 1
-        n, steps, dt, stride = oracle_sample(name, args.cpu_baseline_rays, cores, path_free=pf, unpolarized=args.unpolarized)
+        n, steps, dt, stride = oracle_sample(name, args.cpu_baseline_rays if not args.edf else min(args.cpu_baseline_rays, 256), cores,
+                                             path_free=pf, unpolarized=args.unpolarized, edf=args.edf)
         line["cpu_baseline"] = {"value": n / dt, "unit": "rays/s", "cores": cores, "kind": "oracle",
                                 "sample": "%d rays: every %d-th pixel in x and y of the %dx%d image, %.1f s"
                                           % (n, stride, wl["n"], wl["n"], dt),
@@ -635,6 +647,9 @@ def main():
     ap.add_argument("--unpolarized", action="store_true", help="I alone (PAPER.md:74 'nonpolarized images')")
     ap.add_argument("--single-kernel", action="store_true",
                     help="transfer in the single per-ray kernel k_transfer instead of k_stepop + k_apply (ipole_set_transfer_split 0)")
+    ap.add_argument("--edf", type=int, default=0, choices=[0, 1, 2],
+                    help="second physics workload (PAPER.md:78): j, alpha integrated numerically over a Maxwell-Juettner (1) or "
+                         "kappa (2) electron distribution at every step (ipole_set_edf); analytic-flow workloads only")
     ap.add_argument("--no-second-workload", action="store_true",
                     help="default run only: skip the grid4096 half of configs[4] that is otherwise timed after adaf4096")
     ap.add_argument("--path-free", action="store_true",
@@ -696,7 +711,7 @@ def main():
     line = measure_image(args, args.workload, ipole, replicas, W, world, rank, local, barrier)
     # The default run covers BOTH halves of BASELINE.json configs[4]: the analytic ADAF image is the top-level value,
     # the GRMHD-like grid image of the same size is timed in the same process and reported under "workloads".
-    plain = not (args.path_free or args.unpolarized or args.single_kernel)
+    plain = not (args.path_free or args.unpolarized or args.single_kernel or args.edf)
     if args.workload == "adaf4096" and plain and not args.no_second_workload:
         other = measure_image(args, "grid4096", ipole, replicas, W, world, rank, local, barrier)
         if rank == 0:

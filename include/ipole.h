@@ -143,12 +143,14 @@ int  ipole_set_transfer_split(ipole_ctx*, int32_t on);
  * distribution, n(gamma) = N gamma^2 beta [1 + (gamma-1)/(kappa w)]^-(kappa+1) with w = Theta_e of the plasma model.  For
  * kind != 0 every transfer step evaluates j_{I,Q,V} = C int n {F, G, (4 cot/3) H/gamma} dgamma and alpha_{I,Q,V} =
  * -(C/(2 m nu^2)) int {..} gamma^2 d/dgamma[n/gamma^2] dgamma (single-electron synchrotron kernels F, G, H; x = nu / nu_cr(gamma))
- * by the midpoint rule in ln(gamma) on n_nodes cells of [1, gamma_max]; N from int n dgamma = n_e with the same rule;
- * rho_Q, rho_V stay thermal.  Supported for the analytic flow on the stored path (ipole_make_image, _pixels,
+ * by the midpoint rule on n_nodes equal cells of ln x in [-16, 4] (gamma = sqrt(xs/x), xs = nu / ((3/2) nu_B sin(theta)):
+ * the kernels are then constants of the nodes); N from int n dgamma = n_e by the midpoint rule on 512 cells of ln(gamma-1)
+ * in [-16, 16]; rho_Q, rho_V stay thermal.  Supported for the analytic flow on the stored path (ipole_make_image, _pixels,
  * _image_adaptive); those calls return IPOLE_EINVAL for another model, the sweeps, the path-free or the unpolarized
- * variant while kind != 0.  Zero fields take the defaults kappa 3.5, gamma_max 3e4, n_nodes 128.
- * IPOLE_EINVAL: NULL, kind outside 0..2, kappa <= 1, gamma_max <= 1, n_nodes > 65536. */
-typedef struct { int32_t kind; int32_t n_nodes; double kappa; double gamma_max; } ipole_edf;
+ * variant while kind != 0.  Zero fields take the defaults kappa 3.5, n_nodes 128.  The call enqueues two small set-up
+ * kernels (node constants, normalisation table) on the context's stream.
+ * IPOLE_EINVAL: NULL, kind outside 0..2, kappa <= 1, n_nodes > 1024. */
+typedef struct { int32_t kind; int32_t n_nodes; double kappa; } ipole_edf;
 int  ipole_set_edf(ipole_ctx*, const ipole_edf*);
 /* Unpolarized transfer (the model-fitting loop makes "nonpolarized images"; polarized
  * transfer is "far more complex and computationally demanding"; reading R-12 in DESIGN.md).  on != 0: every image

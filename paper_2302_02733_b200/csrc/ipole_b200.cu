@@ -59,7 +59,8 @@ struct ipole_ctx {
   double* d_ops = nullptr; size_t ops_bytes = 0;   // operator records of one batch
   int32_t* d_irr = nullptr;      // slots of the rays k_stepop leaves to k_transfer
   int occ_op = 0, occ_ap = 0, occ_ap_edf = 0;
-  EdfDev edf = {0, 128, 3.5, 0.0};   // electron distribution of the coefficient step (ipole_set_edf); kind 0: thermal fits
+  EdfDev edf = {0, 128, 3.5, 0.0, nullptr, nullptr};   // electron distribution of the coefficient step (ipole_set_edf); kind 0: thermal fits
+  double4* d_edf_nodes = nullptr; double* d_edf_lnnorm = nullptr;
   int occ_unpol[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};
   double* d_endp = nullptr; int64_t endp_cap = 0;   // end points of the backward passes, [rays][8]
   long long* d_sum = nullptr;    // forward-step total of the path-free variant
@@ -353,7 +354,7 @@ int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStrea
     const int s = span_begin(c, LK_APPLY, st);
     const int g = grid_for(c, c->occ_ap, IPOLE_AP_THREADS / 32, (rays + 31) / 32, reserve);   // one warp per 32 rays
     p.edf = c->edf;
-    if (c->edf.kind != 0) k_apply<true><<<grid_for(c, c->occ_ap_edf, IPOLE_AP_THREADS / 32, (rays + 31) / 32, reserve), IPOLE_AP_THREADS, 0, st>>>(p);
+    if (c->edf.kind != 0) k_apply<true><<<grid_for(c, c->occ_ap_edf, IPOLE_AP_THREADS / 32, (rays + 31) / 32, reserve), IPOLE_AP_THREADS, (size_t)c->edf.n_nodes * sizeof(double4), st>>>(p);
     else k_apply<false><<<g, IPOLE_AP_THREADS, 0, st>>>(p);
     span_end(c, s, st);
     c->stats.n_launches++;
@@ -765,7 +766,7 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_sweep[MODEL_GRID], k_transfer<MODEL_GRID, 0, true>, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_op, k_stepop<MODEL_ADAF>, IPOLE_OP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap, k_apply<false>, IPOLE_AP_THREADS, 0);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_edf, k_apply<true>, IPOLE_AP_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_edf, k_apply<true>, IPOLE_AP_THREADS, EDF_MAX_NODES * sizeof(double4));
   { const char* e = std::getenv("IPOLE_NO_SPLIT"); if (e && e[0] == '1') c->opt_split = 0; }
   { const char* e = std::getenv("IPOLE_NO_TIGHT"); if (e && e[0] == '1') c->opt_tight = 0; }
   { const char* e = std::getenv("IPOLE_NO_GROUP"); if (e && e[0] == '1') c->opt_group = 0; }
@@ -826,10 +827,17 @@ int ipole_set_edf(ipole_ctx* c, const ipole_edf* e) {
   if (!c || !e) return IPOLE_EINVAL;
   if (e->kind < 0 || e->kind > 2) return IPOLE_EINVAL;
   const int nn = e->n_nodes > 0 ? e->n_nodes : 128;
-  const double gmax = e->gamma_max > 0.0 ? e->gamma_max : 3.0e4;
-  const double kappa = e->kappa > 0.0 ? e->kappa : 3.5;
-  if (e->kind != 0 && (!(gmax > 1.0) || nn > 65536 || (e->kind == 2 && !(kappa > 1.0)))) return IPOLE_EINVAL;
-  c->edf.kind = e->kind; c->edf.n_nodes = nn; c->edf.kappa = kappa; c->edf.du = std::log(gmax) / nn;
+  const double kappa = e->kappa != 0.0 ? e->kappa : 3.5;
+  if (e->kind != 0 && (nn > EDF_MAX_NODES || (e->kind == 2 && !(kappa > 1.0)))) return IPOLE_EINVAL;
+  c->edf.kind = e->kind; c->edf.n_nodes = nn; c->edf.kappa = kappa; c->edf.dlx = (EDF_LNX_HI - EDF_LNX_LO) / nn;
+  if (e->kind == 0) return IPOLE_OK;
+  // per-node constants and the normalisation table of this distribution (once per call, not on the hot path)
+  if (!c->d_edf_nodes) CK(cudaMalloc(&c->d_edf_nodes, EDF_MAX_NODES * sizeof(double4)));
+  if (!c->d_edf_lnnorm) CK(cudaMalloc(&c->d_edf_lnnorm, EDF_TAB_N * sizeof(double)));
+  c->edf.nodes = c->d_edf_nodes; c->edf.lnnorm = c->d_edf_lnnorm;
+  k_edf_setup_nodes<<<(nn + 127) / 128, 128, 0, c->stream>>>(c->edf, c->d_edf_nodes);
+  k_edf_setup_norm<<<(EDF_TAB_N + 127) / 128, 128, 0, c->stream>>>(c->edf, c->d_edf_lnnorm);
+  CK(cudaGetLastError());
   return IPOLE_OK;
 }
 
@@ -1359,7 +1367,7 @@ void ipole_free(ipole_ctx* c) {
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long);
   cudaFree(c->d_out); cudaFree(c->d_pixels); cudaFree(c->d_probe); cudaFree(c->d_queues); cudaFree(c->d_hist);
   cudaFree(c->d_small); cudaFree(c->d_part); cudaFree(c->d_red); cudaFree(c->d_endp); cudaFree(c->d_sum); cudaFree(c->d_sweep_models); cudaFree(c->d_sweep_units); cudaFree(c->d_sweep_models_side); cudaFree(c->d_sweep_units_side); cudaFree(c->d_sweep_out); cudaFree(c->d_ada);
-  cudaFree(c->d_ops); cudaFree(c->d_irr); cudaFree(c->d_retry);
+  cudaFree(c->d_ops); cudaFree(c->d_irr); cudaFree(c->d_retry); cudaFree(c->d_edf_nodes); cudaFree(c->d_edf_lnnorm);
   if (c->ev_ada0) cudaEventDestroy(c->ev_ada0);
   if (c->ev_ada1) cudaEventDestroy(c->ev_ada1);
   for (auto& s : c->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }

@@ -190,8 +190,17 @@ __device__ __noinline__ Stokes4 stokes_step_qv_closed(double aI, double aQ, doub
 // the 32 rays of a group have similar lengths.  The record of the next step is loaded (three coalesced 256-bit loads)
 // while the current one is applied.
 // EDF: the coefficients of a step by numerical integration over the electron distribution function (edf.cuh)
+#ifndef IPOLE_AP_EDF_MINB
+#define IPOLE_AP_EDF_MINB 3
+#endif
 template <bool EDF>
-__global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? 3 : IPOLE_AP_MINB) k_apply(const __grid_constant__ ApArgs A) {
+__global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? IPOLE_AP_EDF_MINB : IPOLE_AP_MINB) k_apply(const __grid_constant__ ApArgs A) {
+  extern __shared__ double4 edf_nodes_smem[];          // EDF: the per-node constants {x^-1/2, F, G, H} (edf.cuh)
+  if (EDF) {
+    for (int k = threadIdx.x; k < A.edf.n_nodes; k += blockDim.x) edf_nodes_smem[k] = A.edf.nodes[k];
+    __syncthreads();
+  }
+  const double4* edf_nodes = edf_nodes_smem;
   const int lane = threadIdx.x & 31;
   const int64_t n_groups = (A.count + 31) >> 5;
   for (;;) {
@@ -236,7 +245,7 @@ __global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? 3 : IPOLE_AP_MINB) k_a
         stokes_congruence(m11, m12, m21, m22, S);
         double ne, Th, B;
         adaf_scalars(A.model, x1, ne, Th, B);
-        const Coeff c = EDF ? synchrotron_edf_invariant(A.edf, ne, Th, B, cosT, nu) : synchrotron_invariant(ne, Th, B, cosT, nu);
+        const Coeff c = EDF ? synchrotron_edf_invariant(A.edf, edf_nodes, ne, Th, B, cosT, nu) : synchrotron_invariant(ne, Th, B, cosT, nu);
         const double xI = c.aI * ds, xQ = c.aQ * ds, xV = c.aV * ds, yQ = c.rQ * ds, yV = c.rV * ds;
         const double eI = c.jI * ds, eQ = c.jQ * ds, eV = c.jV * ds;
         if (IP_UNLIKELY(!stokes_step_qv_series(xI, xQ, xV, yQ, yV, 1.0, eI, eQ, eV, S))) {

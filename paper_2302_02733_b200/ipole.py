@@ -57,7 +57,7 @@ class Stats(C.Structure):
 
 
 class Edf(C.Structure):
-    _fields_ = [("kind", C.c_int32), ("n_nodes", C.c_int32), ("kappa", C.c_double), ("gamma_max", C.c_double)]
+    _fields_ = [("kind", C.c_int32), ("n_nodes", C.c_int32), ("kappa", C.c_double)]
 
 
 class GridScales(C.Structure):
@@ -192,10 +192,10 @@ class Ipole:
         """Transfer as a step-parallel operator pass + a per-ray apply pass (include/ipole.h ipole_set_transfer_split)."""
         _chk(lib().ipole_set_transfer_split(self._h, int(on)), "ipole_set_transfer_split")
 
-    def set_edf(self, kind, kappa=3.5, gamma_max=3.0e4, n_nodes=128):
+    def set_edf(self, kind, kappa=3.5, n_nodes=128):
         """Electron distribution of the coefficient step (include/ipole.h ipole_set_edf): 0 thermal fits,
         1 Maxwell-Juettner, 2 kappa; j and alpha by numerical integration over it."""
-        e = Edf(int(kind), int(n_nodes), float(kappa), float(gamma_max))
+        e = Edf(int(kind), int(n_nodes), float(kappa))
         _chk(lib().ipole_set_edf(self._h, C.byref(e)), "ipole_set_edf")
 
     def set_unpolarized(self, on=True):
