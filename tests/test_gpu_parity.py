@@ -45,6 +45,13 @@ def check_parity(gpu, ref, label, min_lit=0.0):
         assert (gpu[k][dark] == 0.0).all(), (label, "dark pixels", k)
     lit = ~dark
     assert lit.mean() >= min_lit, (label, "lit fraction", lit.mean())
+    # Pixels more than ~250 decades below anything visible (I_nu < 1e-250 cgs; the peak of these images is ~1e-4): their
+    # invariant I/nu^3 ~ 1e-284 and the products that form it run through the subnormal range, where a double has a few
+    # bits.  "Relative to the pixel's own I" means nothing there; they must agree absolutely to 1e-250.
+    tiny = lit & (I0 < 1e-250)
+    for k in "IQUV":
+        assert (np.abs(gpu[k][tiny] - ref[k][tiny]) <= 1e-250).all(), (label, "underflowing pixels", k)
+    lit = lit & ~tiny
     err = np.zeros(n)
     for k in "IQUV":
         err[lit] = np.maximum(err[lit], np.abs(gpu[k][lit] - ref[k][lit]) / np.abs(I0[lit]))
@@ -65,7 +72,17 @@ def check_parity(gpu, ref, label, min_lit=0.0):
     for k in ("tau", "tauF"):
         if k in gpu and k in ref:
             assert np.allclose(gpu[k], ref[k], rtol=1e-7, atol=1e-300), (label, k)
-    return dict(max_err=float(err.max()), ring_frac=float(ring.mean()), lit=float(lit.mean()))
+    nt = ref["nturn"] & 0x7f
+    cls = {name: (float(err[m].max()) if m.any() else 0.0, int(m.sum())) for name, m in
+           (("n_turn<2", nt < 2), ("n_turn=2", nt == 2), ("n_turn>=3", nt >= 3))}
+    return dict(max_err=float(err.max()), ring_frac=float(ring.mean()), lit=float(lit.mean()), by_class=cls,
+                within_1e7=float(ok.mean()))
+
+
+def report(label, n, info):
+    """worst per-pixel error of each turning-point class (printed with pytest -s; the driver's log keeps it)"""
+    print("\n%s: %d sampled pixels, %.4f %% within 1e-7, worst |dS|/I by class: %s" % (
+        label, n, 100 * info["within_1e7"], ", ".join("%s %.2e (%d px)" % (k, v[0], v[1]) for k, v in info["by_class"].items())))
 
 
 def sample_pixels(nx, ny, stride, window=None):
@@ -349,10 +366,13 @@ def test_w5_adaf_4096_sampled(ipole, ref):
     cam = W.camera("adaf", 4096)
     g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
     r = ref.Ctx(**cam); r.load_adaf(**W.ADAF)
-    pix = sample_pixels(4096, 4096, 128, window=(2400, 2040, 256, 2))
+    # the sample DESIGN.md section 6 / BASELINE.md declare: every 16th pixel (65 536 rays) plus every pixel of a 512 x 128
+    # window across the photon ring on the +x side
+    pix = sample_pixels(4096, 4096, 16, window=(2300, 1984, 512, 128))
     want = r.make_pixels(pix, nthreads=NTHREADS)
     got, img = gpu_full_then_sample(g, pix, maps=False)
     info = check_parity(got, want, "W5 adaf", min_lit=0.99)
+    report("W5 adaf 4096^2", pix.size, info)
     st = g.stats()
     assert st["n_batches"] >= 1 and st["n_maxstep"] == 0
     # properties of the whole 4096^2 image
@@ -373,10 +393,11 @@ def test_w4_grid_1024_sampled_with_maps(ipole, ref, big_grid):
     cam = W.camera("grid", 1024)
     g = ipole.Ipole(**cam); g.load_grid(desc, fields)
     r = ref.Ctx(**cam); r.load_grid(desc, fields)
-    pix = sample_pixels(1024, 1024, 32, window=(560, 508, 128, 4))
+    pix = sample_pixels(1024, 1024, 4, window=(560, 496, 128, 32))      # every 4th pixel (65 536 rays) + a ring window
     want = r.make_pixels(pix, nthreads=NTHREADS)
     got, _ = gpu_full_then_sample(g, pix, maps=True)
-    check_parity(got, want, "W4", min_lit=0.3)
+    info = check_parity(got, want, "W4", min_lit=0.3)
+    report("W4 grid 1024^2", pix.size, info)
 
 
 def test_w5_grid_4096_sampled(ipole, ref, big_grid):
@@ -384,7 +405,8 @@ def test_w5_grid_4096_sampled(ipole, ref, big_grid):
     cam = W.camera("grid", 4096)
     g = ipole.Ipole(**cam); g.load_grid(desc, fields)
     r = ref.Ctx(**cam); r.load_grid(desc, fields)
-    pix = sample_pixels(4096, 4096, 128, window=(2240, 2040, 256, 2))
+    pix = sample_pixels(4096, 4096, 16, window=(2240, 1984, 512, 128))
     want = r.make_pixels(pix, nthreads=NTHREADS)
     got, _ = gpu_full_then_sample(g, pix, maps=False)
-    check_parity(got, want, "W5 grid", min_lit=0.3)
+    info = check_parity(got, want, "W5 grid", min_lit=0.3)
+    report("W5 grid 4096^2", pix.size, info)

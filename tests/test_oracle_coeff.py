@@ -70,6 +70,20 @@ def test_T8_faraday_cold_limits_and_parities(ref):
     # hot plasma suppresses rotation like K0/K2 ~ ln(Th)/(2 Th^2)
     c_hot = ref.coefficients(ne, 20.0, B, np.cos(th), nu)
     assert c_hot[7] / rV == pytest.approx(special.kve(0, 0.05) / special.kve(2, 0.05), rel=1e-12)
+    # hot plasma, high frequency (X -> 0, f(X) -> 1): the conversion coefficient of an isotropic distribution is the cold
+    # one times <gamma (1 + beta^2)> = <2 gamma - 1/gamma> (Melrose 1997; Shcherbakov 2008), which for Maxwell-Juettner
+    # electrons is K1/K2 + 6 Theta_e.  The average is taken here by quadrature over n(gamma) ~ gamma^2 beta e^(-gamma/Theta):
+    # a dropped 6 Theta_e, a wrong Bessel order or a wrong constant in the bracket fails this.
+    for Th_hot in (1.0, 10.0, 30.0):
+        nu_hi = 1e21                                   # X = Th [sqrt2 sin 1e3 nu_B/nu]^(1/2) ~ 4e-6 Th: f(X) = 1 - O(1e-5)
+        w = lambda g: g * np.sqrt(g * g - 1.0) * np.exp(-(g - 1.0) / Th_hot)
+        num = integrate.quad(lambda g: w(g) * (2.0 * g - 1.0 / g), 1.0, np.inf, limit=400)[0]
+        den = integrate.quad(w, 1.0, np.inf, limit=400)[0]
+        c_h = ref.coefficients(ne, Th_hot, B, np.cos(th), nu_hi)
+        rQ_cold = EE ** 4 * ne * B ** 2 * np.sin(th) ** 2 / (4 * np.pi ** 2 * ME ** 3 * CL ** 3 * nu_hi ** 3)
+        assert c_h[6] / rQ_cold == pytest.approx(num / den, rel=2e-4)
+    # f(X) itself (a published fit to a numerical integral, Shcherbakov 2008) is pinned only at X -> 0 (above): "parity
+    # unpinned" for its shape at X >~ 0.1
     # parities under theta_B -> pi - theta_B: j_V, alpha_V, rho_V odd; the rest even
     cp = ref.coefficients(ne, 5.0, B, np.cos(th), nu)
     cm = ref.coefficients(ne, 5.0, B, -np.cos(th), nu)
