@@ -59,8 +59,8 @@ WORKLOADS = {
     # many-small-images mode (128x128 images for model fitting): 64 parameter sets per call
     "sweep128": dict(kind="adaf", n=128, config=None, sweep=64),
     "gridsweep128": dict(kind="grid", n=128, config=None, sweep=64, grid=(288, 128, 128)),
-    # small images whose GEOMETRY differs (inclination): nothing to share, so independent contexts run side by side
-    "cams128": dict(kind="adaf", n=128, config=None, cams=8),
+    # small images whose GEOMETRY differs (inclination, spin): one ipole_make_images_cameras call over the union of their rays
+    "cams128": dict(kind="adaf", n=128, config=None, cams=64),
 }
 
 
@@ -280,65 +280,75 @@ def oracle_sample(workload, n_rays, nthreads, path_free=False, unpolarized=False
 
 
 def run_cams(args, ipole, replicas, W, wl, world, rank, local, barrier):
-    """One step = one 128x128 image for each of `cams` cameras (different inclinations).  Contexts are independent
-    (include/ipole.h), so each camera gets its own context, CUDA stream and host thread; compared with the same images
-    made one after the other on a single context."""
-    import threading as th
+    """One step = one ipole_make_images_cameras call: `cams` 128x128 images whose geometry differs (inclination and spin),
+    from ONE host thread and one context, in one pass of the pipeline over the union of their rays; compared with the same
+    images made one after the other by ipole_set_camera + ipole_make_image."""
     import torch
     n, nc = wl["n"], wl["cams"]
-    incl = [20.0 + 60.0 * k / max(1, nc - 1) for k in range(nc)]
-    cams = [W.camera("adaf", n, inclination_deg=a) for a in incl]
+    incl = [15.0 + 150.0 * k / max(1, nc - 1) for k in range(nc)]
+    spins = [0.0, 0.5, 0.9375, 0.99]
+    cams = [W.camera("adaf", n, inclination_deg=a, spin=spins[k % 4]) for k, a in enumerate(incl)]
     names = ["I", "Q", "U", "V"]
-    ctxs, streams, outs = [], [], []
-    for cam in cams:
-        g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
-        g.set_options(4 << 30, 1)                  # 4 GiB of path buffer per context instead of 40 % of the free memory
-        s = torch.cuda.Stream(); g.set_stream(s)
-        ctxs.append(g); streams.append(s)
-        outs.append({k: torch.empty((n, n), dtype=torch.float64, device="cuda") for k in names})
+    g = ipole.Ipole(**cams[0]); g.load_adaf(**W.ADAF)
+    g.set_stream(torch.cuda.current_stream())
+    out = {k: torch.empty((nc, n, n), dtype=torch.float64, device="cuda") for k in names}
+    single = {k: torch.empty((n, n), dtype=torch.float64, device="cuda") for k in names}
 
-    def side_by_side():
-        def work(k):
-            torch.cuda.set_device(local)
-            ctxs[k].make_image(out=outs[k])
-        ts = [th.Thread(target=work, args=(k,)) for k in range(nc)]
-        for t in ts: t.start()
-        for t in ts: t.join()
-        for s in streams: s.synchronize()
+    def batched():
+        g.make_images_cameras(cams, out=out)
 
     def one_by_one():
-        for k in range(nc):
-            ctxs[k].make_image(out=outs[k])
-            streams[k].synchronize()
+        for cam in cams:
+            g.set_camera(**cam)
+            g.make_image(out=single)
 
-    res = {}
-    for name, fn in (("side_by_side", side_by_side), ("one_by_one", one_by_one)):
+    res, st = {}, None
+    for name, fn in (("batched", batched), ("one_by_one", one_by_one)):
         for _ in range(args.warmup):
             fn()
         barrier()
-        t0 = time.perf_counter()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
         for _ in range(args.steps):
             fn()
-        torch.cuda.synchronize()
-        res[name] = replicas.max_over_ranks(time.perf_counter() - t0, "cuda") / args.steps
+        ev1.record()
+        barrier()
+        res[name] = replicas.max_over_ranks(ev0.elapsed_time(ev1), "cuda") * 1e-3 / args.steps
+        if name == "batched":
+            st = g.stats()
+    g.set_camera(**cams[0])
+    host = {k: torch.empty((nc, n, n), dtype=torch.float64).pin_memory().numpy() for k in names}
+    g.make_images_cameras(cams, out=host)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        g.make_images_cameras(cams, out=host)
+    torch.cuda.synchronize()
+    dt = replicas.max_over_ranks(time.perf_counter() - t0, "cuda") / args.steps
     if rank != 0:
         return
     rays = nc * n * n
-    line = {"metric": "rays_per_s", "value": world * rays / res["side_by_side"], "unit": "rays/s", "n_gpus": world,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": res["side_by_side"] * 1e3, "higher_is_better": True,
+    fl = FLOP_PER_STEP["transfer_adaf"]
+    line = {"metric": "rays_per_s", "value": world * rays / res["batched"], "unit": "rays/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": res["batched"] * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "image": "%dx%d" % (n, n), "cameras": nc, "inclinations_deg": incl,
-                       "model": "adaf", "freq_ghz": 230, "full_stokes": True, "timing": "host wall clock around %d threads, "
-                       "one context and stream each, all streams synchronised inside" % nc,
-                       "l2": "not flushed: 8 independent images per step, each streaming its own path buffer", "parallelism": "single GPU"},
-            "images_per_s": world * nc / res["side_by_side"],
+            "config": {"workload": args.workload, "image": "%dx%d" % (n, n), "cameras": nc, "inclinations_deg": [incl[0], incl[-1]],
+                       "spins": spins, "model": "adaf", "freq_ghz": 230, "full_stokes": True,
+                       "timing": "CUDA events around ipole_make_images_cameras from one host thread, one context",
+                       "l2": "no flush needed: each call streams %.1f GB of path and operator records" % (st["total_steps"] * 128 / 1e9),
+                       "parallelism": "single GPU"},
+            "images_per_s": world * nc / res["batched"],
             "one_by_one": {"images_per_s": world * nc / res["one_by_one"], "ms_per_%d_images" % nc: res["one_by_one"] * 1e3,
-                           "speedup_side_by_side": res["one_by_one"] / res["side_by_side"]},
-            "gpu_launches": sum(g.stats()["n_launches"] for g in ctxs) * args.steps,
-            "roofline": {"bound": "alu", "kernel": "k_transfer<adaf>", "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "achieved": None,
-                         "frac": None, "traffic": None, "note": "latency study of small images; see the default bench line for the kernels"},
-            "e2e": {"value": world * rays / res["side_by_side"], "unit": "rays/s", "h2d_bytes_per_step": 0,
-                    "d2h_bytes_per_step": 0, "note": "device outputs; the timing is host wall clock already"}}
+                           "speedup_of_the_batch_entry": res["one_by_one"] / res["batched"]},
+            "stage_ms": {"probe_sort": st["ms_probe"], "geodesic": st["ms_geodesic"], "transfer": st["ms_transfer"], "stepop": st["ms_stepop"],
+                         "apply": st["ms_apply"], "total": st["ms_total"], "batches": st["n_batches"]},
+            "gpu_launches": st["n_launches"] * args.steps,
+            "roofline": {"bound": "alu", "kernel": "k_stepop<adaf, cameras> + k_apply", "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                         "achieved": fl * st["total_steps"] / (st["ms_transfer"] * 1e-3) / 1e12,
+                         "frac": fl * st["total_steps"] / (st["ms_transfer"] * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+                         "flop_per_step_algorithmic": fl, "traffic": DRAM_BYTES_PER_STEP_SPLIT * st["total_steps"] / max(1, st["n_batches"])},
+            "e2e": {"value": world * rays / dt, "unit": "rays/s", "h2d_bytes_per_step": nc * ipole.C.sizeof(ipole.Camera),
+                    "d2h_bytes_per_step": 4 * rays * 8 + nc * 32}}
     print(json.dumps(line), flush=True)
 
 

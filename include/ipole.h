@@ -198,6 +198,20 @@ int  ipole_make_images_adaf(ipole_ctx*, int32_t n_models, const ipole_adaf_param
 typedef struct { double M_unit, Rlow, Rhigh; } ipole_grid_scales;
 int  ipole_make_images_grid(ipole_ctx*, int32_t n_models, const ipole_grid_scales* sets, const double* freq_hz,
                             double* I, double* Q, double* U, double* V, double* tau, double* tauF, double* flux_jy);
+/* Many small images whose GEOMETRY differs (the fitting loop also varies viewing angle and spin): n_cams
+ * cameras seen through the analytic flow loaded in the context, all in one pass of the pipeline -- one probe and sort over
+ * the union of their rays, geodesic / operator / apply launches over batches of that union -- so that 128 x 128 images
+ * fill the GPU although each has only 16 k rays.  Every image is what ipole_set_camera(cams[k]) + ipole_make_image
+ * would give.  The cameras may differ in spin, inclination, distance, field of view, frequency, mass, source distance,
+ * escape radius and stop factor; they must agree in nx, ny, eps, max_steps and hslope, and none may be a flat-metric
+ * camera.  The flow's ISCO follows each camera's spin.  Outputs I,Q,U,V (optional tau, tauF) are [n_cams][ny][nx], all
+ * host or all device; flux_jy (nullable, host or device) is [n_cams][4].  The context's own camera and model are left
+ * as they were; ipole_get_stats afterwards describes the union of the rays.  Works with ipole_set_edf; uses the split
+ * transfer whatever ipole_set_transfer_split says.
+ * IPOLE_ENOMODEL without a model, IPOLE_EINVAL for another model than the analytic flow, for cameras that disagree in
+ * the fields above, for the path-free or unpolarized variant, mixed host/device outputs, nx*ny*n_cams > 2^31-1. */
+int  ipole_make_images_cameras(ipole_ctx*, int32_t n_cams, const ipole_camera* cams, double* I, double* Q, double* U, double* V,
+                               double* tau, double* tauF, double* flux_jy);
 /* Adaptive ray tracing ("another factor of 10 with adaptive ray tracing which reduces the number of light
  * rays to follow"; the paper gives no algorithm: reading R-11 in DESIGN.md).  Dyadic lattice levels
  * l = 0..levels of stride 2^(levels-l) (plus the last row and column): level 0 and 1 are traced everywhere; from then

@@ -51,6 +51,10 @@ struct ipole_ctx {
   int last_pf = 0;               // the last image was made path-free
   int opt_unpol = 0;             // unpolarized transfer of I alone
   AdafParams adaf_host;          // host copy of the loaded analytic model (k_apply takes it by value)
+  // many cameras per call (ipole_make_images_cameras): device arrays of n_mc cameras, null outside such a call
+  CamDev* d_mc_cams = nullptr; Units* d_mc_units = nullptr; double* d_mc_nu3 = nullptr; double* d_mc_scale = nullptr;
+  int mc_cap = 0; int n_mc = 0; int64_t mc_rays_per_cam = 0;
+  int occ_geo_mc = 0, occ_op_mc = 0;
   int opt_group = 1;             // grid model: transfer with warp-level scheduling (k_transfer_group)
   int occ_group = 0;
   int opt_tight = 1;             // sorted rays: path slots sized batch by batch from the predicted step counts
@@ -121,8 +125,8 @@ int check_camera(const ipole_camera* k) {
   return IPOLE_OK;
 }
 
-int apply_camera(ipole_ctx* c, const ipole_camera* k) {
-  CamDev C;
+// host part of a camera: what k_camera_setup starts from, and the units that follow from mass, distance and frequency
+void fill_camera(const ipole_camera* k, CamDev& C, CameraSetupArgs& a, Units& u) {
   std::memset(&C, 0, sizeof C);
   C.G.a = k->spin;
   C.G.hslope = k->hslope > 0.0 ? k->hslope : 1.0;
@@ -133,22 +137,29 @@ int apply_camera(ipole_ctx* c, const ipole_camera* k) {
   C.pix = k->fov / k->nx;
   C.eps = k->eps > 0.0 ? k->eps : 0.01;
   C.max_steps = k->max_steps > 0 ? k->max_steps : 50000;
-  CameraSetupArgs a;
   a.inclination_deg = k->inclination_deg;
   a.r_esc = k->r_esc > 0.0 ? k->r_esc : k->r_cam;
   const double stop = k->stop_factor > 0.0 ? k->stop_factor : 1.05;
   a.r_in = k->flat_metric ? 1e-3 : stop * (1.0 + std::sqrt(1.0 - k->spin * k->spin));
+  const double M = (k->mbh_msun > 0.0 ? k->mbh_msun : 4.1e6) * IP_MSUN;
+  u.nu_obs = k->freq_hz;
+  u.L_unit = IP_GNEWT * M / (IP_CL * IP_CL);
+  u.D_cm = (k->dsource_pc > 0.0 ? k->dsource_pc : 8000.0) * IP_PC;
+  u.dl_unit = u.L_unit / u.nu_obs;
+}
+
+int apply_camera(ipole_ctx* c, const ipole_camera* k) {
+  CamDev C;
+  CameraSetupArgs a;
+  Units un;
+  fill_camera(k, C, a, un);
   CK(cudaMemcpyAsync(c->d_cam, &C, sizeof C, cudaMemcpyHostToDevice, c->stream));
   k_camera_setup<<<1, 32, 0, c->stream>>>(c->d_cam, a);
   CK(cudaGetLastError());
   CK(cudaMemcpyAsync(&c->cam, c->d_cam, sizeof C, cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
   c->cam_in = *k;
-  const double M = (k->mbh_msun > 0.0 ? k->mbh_msun : 4.1e6) * IP_MSUN;
-  c->units.nu_obs = k->freq_hz;
-  c->units.L_unit = IP_GNEWT * M / (IP_CL * IP_CL);
-  c->units.D_cm = (k->dsource_pc > 0.0 ? k->dsource_pc : 8000.0) * IP_PC;
-  c->units.dl_unit = c->units.L_unit / c->units.nu_obs;
+  c->units = un;
   c->have_image = false;
   return IPOLE_OK;
 }
@@ -235,7 +246,10 @@ int grid_for(ipole_ctx* c, int occ, int threads, int64_t rays, int reserve = 0) 
 
 int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays, cudaStream_t st, int reserve = 0) {
   const int s = span_begin(c, kind, st);
-  if (a.grid) k_geodesic<true><<<grid_for(c, c->occ_geo_occ, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
+  if (c->n_mc) {
+    a.cams = c->d_mc_cams; a.rays_per_cam = c->mc_rays_per_cam;
+    k_geodesic<false, true><<<grid_for(c, c->occ_geo_mc, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
+  } else if (a.grid) k_geodesic<true><<<grid_for(c, c->occ_geo_occ, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
   else k_geodesic<false><<<grid_for(c, c->occ_geo, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
   span_end(c, s, st);
   c->stats.n_launches++;
@@ -337,8 +351,13 @@ int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStrea
   {
     const int s = span_begin(c, LK_OPS, st);
     // one warp per ray at a time
-    const int g = grid_for(c, c->occ_op, IPOLE_OP_THREADS / 32, rays, reserve);
-    k_stepop<MODEL_ADAF><<<g, IPOLE_OP_THREADS, 0, st>>>(o);
+    if (c->n_mc) {
+      o.cams = c->d_mc_cams; o.units_arr = c->d_mc_units; o.rays_per_cam = c->mc_rays_per_cam;
+      k_stepop<MODEL_ADAF, true><<<grid_for(c, c->occ_op_mc, IPOLE_OP_THREADS / 32, rays, reserve), IPOLE_OP_THREADS, 0, st>>>(o);
+    } else {
+      const int g = grid_for(c, c->occ_op, IPOLE_OP_THREADS / 32, rays, reserve);
+      k_stepop<MODEL_ADAF><<<g, IPOLE_OP_THREADS, 0, st>>>(o);
+    }
     span_end(c, s, st);
     c->stats.n_launches++;
     CK(cudaGetLastError());
@@ -354,6 +373,7 @@ int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStrea
     const int s = span_begin(c, LK_APPLY, st);
     const int g = grid_for(c, c->occ_ap, IPOLE_AP_THREADS / 32, (rays + 31) / 32, reserve);   // one warp per 32 rays
     p.edf = c->edf;
+    if (c->n_mc) { p.nu3_arr = c->d_mc_nu3; p.rays_per_cam = c->mc_rays_per_cam; }
     if (c->edf.kind != 0) k_apply<true><<<grid_for(c, c->occ_ap_edf, IPOLE_AP_THREADS / 32, (rays + 31) / 32, reserve), IPOLE_AP_THREADS, (size_t)c->edf.n_nodes * sizeof(double4), st>>>(p);
     else k_apply<false><<<g, IPOLE_AP_THREADS, 0, st>>>(p);
     span_end(c, s, st);
@@ -433,11 +453,13 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     std::memset(&sa, 0, sizeof sa);
     int64_t np;
     if (!d_pixels) {
+      // one probe lattice per camera (c->n_mc cameras in a call of ipole_make_images_cameras, else one)
       const int stride = std::max(1, (int)std::ceil(std::sqrt((double)n / PROBE_TARGET)));
       const int lnx = std::max(1, c->cam.nx / stride), lny = std::max(1, c->cam.ny / stride);
-      np = (int64_t)lnx * lny;
-      g.lattice_stride = stride; g.lattice_nx = lnx;
+      np = (int64_t)lnx * lny * std::max(1, c->n_mc);
+      g.lattice_stride = stride; g.lattice_nx = lnx; g.lattice_ny = lny;
       sa.lattice_stride = stride; sa.lattice_nx = lnx; sa.lattice_ny = lny; sa.nx = c->cam.nx;
+      sa.rays_per_cam = c->n_mc ? c->mc_rays_per_cam : 0;
     } else {
       const int64_t ls = std::max<int64_t>(1, n / PROBE_TARGET);
       np = (n + ls - 1) / ls;
@@ -483,7 +505,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     const int64_t per = (int64_t)(budget / rec_bytes / (size_t)n) - 1;
     cap = (int)std::max<int64_t>(64, std::min<int64_t>(max_steps, per));
   }
-  if (c->edf.kind != 0 && c->opt_path_free) return IPOLE_EINVAL;
+  if ((c->edf.kind != 0 || c->n_mc) && c->opt_path_free) return IPOLE_EINVAL;
   if (c->opt_path_free && !sw && !c->opt_unpol) {
     // ---- path-free bidirectional variant: one geodesic launch that keeps the end points, one
     // transfer launch that re-integrates forward.  Rays are ordered longest first, so the few very long rays start
@@ -574,7 +596,8 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   // the end with the global S_cap (second level); one that outgrows S_cap goes to the long-ray pass as before.
   // numerically integrated eDF coefficients (ipole_set_edf) live in k_apply only: that mode always runs split, and its
   // long rays go through the same kernels (third level, slots of max_steps) instead of the single kernel on the side stream
-  const bool edf = c->edf.kind != 0;
+  // (many cameras per call, c->n_mc: the same -- only the split kernels know about per-ray cameras)
+  const bool edf = c->edf.kind != 0 || c->n_mc > 0;
   if (edf && (sw || c->opt_unpol || c->model != MODEL_ADAF)) return IPOLE_EINVAL;
   const bool split = edf || (c->opt_split && !sw && !c->opt_unpol && c->model == MODEL_ADAF);
   const size_t step_bytes = rec_bytes + (split ? OP_DOUBLES * sizeof(double) : 0);
@@ -765,6 +788,8 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_unpol[MODEL_GRID][1], k_transfer_unpol<MODEL_GRID, true>, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_sweep[MODEL_GRID], k_transfer<MODEL_GRID, 0, true>, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_op, k_stepop<MODEL_ADAF>, IPOLE_OP_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_op_mc, k_stepop<MODEL_ADAF, true>, IPOLE_OP_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo_mc, k_geodesic<false, true>, IPOLE_GEO_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap, k_apply<false>, IPOLE_AP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_edf, k_apply<true>, IPOLE_AP_THREADS, EDF_MAX_NODES * sizeof(double4));
   { const char* e = std::getenv("IPOLE_NO_SPLIT"); if (e && e[0] == '1') c->opt_split = 0; }
@@ -1058,6 +1083,80 @@ int ipole_make_images_adaf(ipole_ctx* c, int32_t n_models, const ipole_adaf_para
   }
   // the kernel reads the uniform model block too (unused by the analytic sweep): any valid device block will do
   return make_images(c, MODEL_ADAF, n_models, pm.data(), sizeof(AdafParams), um.data(), I, Q, U, V, tau, tauF, flux_jy);
+}
+
+int ipole_make_images_cameras(ipole_ctx* c, int32_t n_cams, const ipole_camera* cams, double* I, double* Q, double* U, double* V,
+                              double* tau, double* tauF, double* flux_jy) {
+  if (!c || !cams || n_cams < 1 || !I || !Q || !U || !V) return IPOLE_EINVAL;
+  if (c->model != MODEL_ADAF) return c->model == MODEL_NONE ? IPOLE_ENOMODEL : IPOLE_EINVAL;
+  for (int k = 0; k < n_cams; ++k) {
+    int rc = check_camera(&cams[k]);
+    if (rc != IPOLE_OK) return rc;
+    const ipole_camera &a = cams[k], &b = cams[0];
+    if (a.flat_metric || a.nx != b.nx || a.ny != b.ny || a.eps != b.eps || a.max_steps != b.max_steps || a.hslope != b.hslope) return IPOLE_EINVAL;
+  }
+  const int64_t npix = (int64_t)cams[0].nx * cams[0].ny, n = npix * n_cams;
+  if (n > 2147483647LL) return IPOLE_EINVAL;
+  const bool dev = is_device_ptr(I);
+  const void* outs[] = {Q, U, V, tau, tauF};
+  for (const void* p : outs) if (p && is_device_ptr(p) != dev) return IPOLE_EINVAL;
+  int rc;
+  if ((rc = ensure_rays(c, n)) != IPOLE_OK) return rc;
+  if (n_cams > c->mc_cap) {
+    cudaFree(c->d_mc_cams); cudaFree(c->d_mc_units); cudaFree(c->d_mc_nu3); cudaFree(c->d_mc_scale);
+    c->d_mc_cams = nullptr; c->d_mc_units = nullptr; c->d_mc_nu3 = nullptr; c->d_mc_scale = nullptr; c->mc_cap = 0;
+    CK(cudaMalloc(&c->d_mc_cams, n_cams * sizeof(CamDev)));
+    CK(cudaMalloc(&c->d_mc_units, n_cams * sizeof(Units)));
+    CK(cudaMalloc(&c->d_mc_nu3, n_cams * sizeof(double)));
+    CK(cudaMalloc(&c->d_mc_scale, n_cams * 5 * sizeof(double)));   // scale[n] then flux[4 n]
+    c->mc_cap = n_cams;
+  }
+  // camera tetrads on the device, one k_camera_setup each (a-1); units, nu_obs^3 and the Jy scale on the host
+  std::vector<CamDev> hc(n_cams);
+  std::vector<Units> hu(n_cams);
+  std::vector<double> hn(n_cams), hs(n_cams);
+  std::vector<CameraSetupArgs> ha(n_cams);
+  for (int k = 0; k < n_cams; ++k) {
+    fill_camera(&cams[k], hc[k], ha[k], hu[k]);
+    hn[k] = hu[k].nu_obs * hu[k].nu_obs * hu[k].nu_obs;
+    const double pix_rad = hc[k].pix * hu[k].L_unit / hu[k].D_cm;
+    hs[k] = pix_rad * pix_rad * 1e23;
+  }
+  CK(cudaMemcpyAsync(c->d_mc_cams, hc.data(), n_cams * sizeof(CamDev), cudaMemcpyHostToDevice, c->stream));
+  CK(cudaMemcpyAsync(c->d_mc_units, hu.data(), n_cams * sizeof(Units), cudaMemcpyHostToDevice, c->stream));
+  CK(cudaMemcpyAsync(c->d_mc_nu3, hn.data(), n_cams * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+  CK(cudaMemcpyAsync(c->d_mc_scale, hs.data(), n_cams * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+  for (int k = 0; k < n_cams; ++k) k_camera_setup<<<1, 32, 0, c->stream>>>(c->d_mc_cams + k, ha[k]);
+  CK(cudaGetLastError());
+  CK(cudaStreamSynchronize(c->stream));   // the host vectors above go out of scope
+  // the context's own camera lends eps, max_steps and the image shape to the shared parts of the pipeline
+  const CamDev cam_saved = c->cam;
+  c->cam.eps = hc[0].eps; c->cam.max_steps = hc[0].max_steps; c->cam.nx = hc[0].nx; c->cam.ny = hc[0].ny;
+  double* o[6] = {I, Q, U, V, tau, tauF};
+  if (!dev) {
+    for (int k = 0; k < 6; ++k) o[k] = c->d_out + (size_t)k * c->ray_cap;
+    if (!tau) o[4] = nullptr;
+    if (!tauF) o[5] = nullptr;
+  }
+  c->n_mc = n_cams; c->mc_rays_per_cam = npix;
+  rc = run_rays(c, n, nullptr, o[0], o[1], o[2], o[3], o[4], o[5]);
+  c->n_mc = 0; c->mc_rays_per_cam = 0;
+  c->cam = cam_saved;
+  if (rc != IPOLE_OK) return rc;
+  if (flux_jy) {
+    double* d_flux = c->d_mc_scale + n_cams;
+    k_reduce_cams<<<n_cams, 256, 0, c->stream>>>(npix, (size_t)npix, o[0], o[1], o[2], o[3], c->d_mc_scale, d_flux);
+    c->stats.n_launches++;
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(flux_jy, d_flux, (size_t)n_cams * 4 * sizeof(double), cudaMemcpyDefault, c->stream));
+  }
+  if (!dev) {
+    double* h[6] = {I, Q, U, V, tau, tauF};
+    for (int k = 0; k < 6; ++k)
+      if (h[k]) CK(cudaMemcpyAsync(h[k], o[k], (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  }
+  if (!dev || (flux_jy && !is_device_ptr(flux_jy))) CK(cudaStreamSynchronize(c->stream));
+  return IPOLE_OK;
 }
 
 int ipole_make_images_grid(ipole_ctx* c, int32_t n_models, const ipole_grid_scales* sets, const double* freq_hz,
@@ -1368,6 +1467,7 @@ void ipole_free(ipole_ctx* c) {
   cudaFree(c->d_out); cudaFree(c->d_pixels); cudaFree(c->d_probe); cudaFree(c->d_queues); cudaFree(c->d_hist);
   cudaFree(c->d_small); cudaFree(c->d_part); cudaFree(c->d_red); cudaFree(c->d_endp); cudaFree(c->d_sum); cudaFree(c->d_sweep_models); cudaFree(c->d_sweep_units); cudaFree(c->d_sweep_models_side); cudaFree(c->d_sweep_units_side); cudaFree(c->d_sweep_out); cudaFree(c->d_ada);
   cudaFree(c->d_ops); cudaFree(c->d_irr); cudaFree(c->d_retry); cudaFree(c->d_edf_nodes); cudaFree(c->d_edf_lnnorm);
+  cudaFree(c->d_mc_cams); cudaFree(c->d_mc_units); cudaFree(c->d_mc_nu3); cudaFree(c->d_mc_scale);
   if (c->ev_ada0) cudaEventDestroy(c->ev_ada0);
   if (c->ev_ada1) cudaEventDestroy(c->ev_ada1);
   for (auto& s : c->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }

@@ -98,7 +98,7 @@ struct GeoArgs {
   const int32_t* order;       // permutation of ray indices q (nullable: identity)
   const int64_t* pixels;      // flat pixel index of ray q (nullable: q itself); with lattice_stride > 0 ignored
   int64_t list_stride;        // probe over a pixel list: ray q stands for list entry q * list_stride (else 1)
-  int lattice_stride, lattice_nx;  // probe: ray q is pixel (ix*stride + stride/2, iy*stride + stride/2)
+  int lattice_stride, lattice_nx, lattice_ny;  // probe: ray q is pixel (ix*stride + stride/2, iy*stride + stride/2) [of camera q / (lattice_nx lattice_ny)]
   double* path;               // [count][cap+1][8] or nullptr (count-only)
   int32_t* nsteps;            // [total rays], indexed by q; -1 = overflowed the slot
   int32_t* nturn;             // [total rays]
@@ -109,6 +109,10 @@ struct GeoArgs {
   // grid model (k_geodesic<true>): the steps of the ray whose midpoint stencil holds plasma
   const GridParams* grid;     // device
   int2* srange;               // [total rays], indexed by q: (largest, smallest) such step index; (-1, 0) if none
+  // many cameras in one launch (k_geodesic<OCC, true>; ipole_make_images_cameras): ray q belongs to camera
+  // q / rays_per_cam and is its pixel q % rays_per_cam; eps and max_steps are those of `cam` for all of them
+  const CamDev* cams;         // device
+  int64_t rays_per_cam;
 };
 
 __device__ __forceinline__ void pixel_ray(const CamDev& C, int64_t pix, double X[4], double K[4]) {
@@ -206,9 +210,15 @@ __device__ __forceinline__ void load_record(const double* rec, double X[4], doub
 // grid's stencil-occupancy bitmap, and the first and last step that may cross plasma are kept per ray.  k_transfer
 // then starts a ray at its first contact with plasma instead of its far end (everything before is dark vacuum and
 // changes nothing), skips the bitmap test after the last contact, and a ray that meets no plasma is not walked at all.
-template <bool OCC>
-__global__ void __launch_bounds__(IPOLE_GEO_THREADS, IPOLE_GEO_MINB) k_geodesic(const __grid_constant__ GeoArgs A) {
+//
+// MC (many cameras per launch: a fit that varies inclination or spin): the geometry and the stop radii are
+// per-lane values taken from the ray's own camera at refill; the single-camera instantiation keeps them in the
+// constant bank.
+template <bool OCC, bool MC = false>
+__global__ void __launch_bounds__(IPOLE_GEO_THREADS, MC ? 3 : IPOLE_GEO_MINB) k_geodesic(const __grid_constant__ GeoArgs A) {
   const CamDev& C = A.cam;
+  Geom Gl = C.G;                      // MC: the lane's own
+  double lx_in_l = C.lx_in, lx_esc_l = C.lx_esc;
   __shared__ __align__(8) unsigned char grid_smem[OCC ? sizeof(GridParams) : 8];
   if (OCC) {
     for (int i = threadIdx.x; i < (int)sizeof(GridParams); i += blockDim.x) grid_smem[i] = ((const unsigned char*)A.grid)[i];
@@ -232,12 +242,18 @@ __global__ void __launch_bounds__(IPOLE_GEO_THREADS, IPOLE_GEO_MINB) k_geodesic(
     q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
     int64_t pix;
     if (A.lattice_stride > 0) {
-      const int ix = q % A.lattice_nx, iy = q / A.lattice_nx;
+      const int per = A.lattice_nx * A.lattice_ny, cam = MC ? q / per : 0, ql = MC ? q % per : q;
+      const int ix = ql % A.lattice_nx, iy = ql / A.lattice_nx;
       pix = (int64_t)(iy * A.lattice_stride + A.lattice_stride / 2) * C.nx + (ix * A.lattice_stride + A.lattice_stride / 2);
+      if (MC) pix += (int64_t)cam * A.rays_per_cam;
     } else {
       pix = A.pixels ? A.pixels[(int64_t)q * A.list_stride] : (int64_t)q * A.list_stride;
     }
-    pixel_ray(C, pix, X, K);
+    if (MC) {
+      const CamDev& Cc = A.cams[pix / A.rays_per_cam];
+      pixel_ray(Cc, pix % A.rays_per_cam, X, K);
+      Gl = Cc.G; lx_in_l = Cc.lx_in; lx_esc_l = Cc.lx_esc;
+    } else pixel_ray(C, pix, X, K);
     rec = A.path ? A.path + (size_t)li * slot_doubles : nullptr;
     n = 0; nt = 0;
     s_hi = -1; s_lo = 0;
@@ -253,8 +269,8 @@ __global__ void __launch_bounds__(IPOLE_GEO_THREADS, IPOLE_GEO_MINB) k_geodesic(
     const bool k2neg = K[2] < 0.0;
     double Xa[4];
     if (OCC) { Xa[0] = X[0]; Xa[1] = X[1]; Xa[2] = X[2]; Xa[3] = X[3]; }
-    if (small_steps) rk4_push<true>(C.G, X, K, -dl);
-    else rk4_push<false>(C.G, X, K, -dl);
+    if (small_steps) rk4_push<true>(MC ? Gl : C.G, X, K, -dl);
+    else rk4_push<false>(MC ? Gl : C.G, X, K, -dl);
     if (OCC) {
       // the midpoint exactly as k_transfer forms it: 0.5 * (X_lo + X_hi) with lo = point n, hi = point n + 1
       double Xm[4];
@@ -265,8 +281,8 @@ __global__ void __launch_bounds__(IPOLE_GEO_THREADS, IPOLE_GEO_MINB) k_geodesic(
     ++n;
     if ((K[2] < 0.0) != k2neg) ++nt;
     int status = 0;
-    if (X[1] <= C.lx_in) status = 1;
-    else if (X[1] > C.lx_esc && X[1] > x1_before) status = 2;
+    if (X[1] <= (MC ? lx_in_l : C.lx_in)) status = 1;
+    else if (X[1] > (MC ? lx_esc_l : C.lx_esc) && X[1] > x1_before) status = 2;
     else if (n >= A.max_steps) status = 3;
     const bool overflow = (status == 0) && rec && (n >= A.cap);
     if (status != 0 || overflow) {
@@ -742,6 +758,7 @@ struct SortArgs {
   int64_t n;                  // rays
   const int32_t* probe;       // step counts of the probe lattice / probe list
   int scale;                  // predicted = probe * scale
+  int64_t rays_per_cam;       // many cameras per call: pixel p belongs to camera p / rays_per_cam, one lattice per camera (0: one camera)
   int lattice_stride, lattice_nx, lattice_ny, nx;  // full-image mode: pixel -> nearest lattice point
   const int64_t* pixels;      // list mode with lattice: pixel of ray q (nullable)
   int list_stride;            // list mode without lattice_stride: probe index = q / list_stride
@@ -758,12 +775,15 @@ __global__ void k_predict_hist(SortArgs A) {
       // the longest of the four probe rays around the pixel (lattice point (ix, iy) is pixel (ix + 1/2) * stride):
       // next to the photon ring the step count jumps by a factor of two to three within one lattice cell, and the
       // per-batch path slots (run_rays) are sized from this prediction
-      const int64_t pix = A.pixels ? A.pixels[q] : q;
+      int64_t pix = A.pixels ? A.pixels[q] : q;
+      const int64_t cam = A.rays_per_cam ? pix / A.rays_per_cam : 0;
+      pix -= cam * A.rays_per_cam;
+      const int32_t* probe = A.probe + cam * (A.lattice_nx * A.lattice_ny);
       const int px = (int)(pix % A.nx) - A.lattice_stride / 2, py = (int)(pix / A.nx) - A.lattice_stride / 2;
       const int ix0 = min(max(px, 0) / A.lattice_stride, A.lattice_nx - 1), iy0 = min(max(py, 0) / A.lattice_stride, A.lattice_ny - 1);
       const int ix1 = min(ix0 + 1, A.lattice_nx - 1), iy1 = min(iy0 + 1, A.lattice_ny - 1);
-      pr = max(max(A.probe[iy0 * A.lattice_nx + ix0], A.probe[iy0 * A.lattice_nx + ix1]),
-               max(A.probe[iy1 * A.lattice_nx + ix0], A.probe[iy1 * A.lattice_nx + ix1]));
+      pr = max(max(probe[iy0 * A.lattice_nx + ix0], probe[iy0 * A.lattice_nx + ix1]),
+               max(probe[iy1 * A.lattice_nx + ix0], probe[iy1 * A.lattice_nx + ix1]));
     } else {
       pr = A.probe[(int)(q / A.list_stride)];
     }
@@ -888,6 +908,24 @@ __global__ void __launch_bounds__(256) k_reduce_models(int64_t n, size_t stride,
     double t = sh[0][threadIdx.x];
     for (int w = 1; w < 8; ++w) t += sh[w][threadIdx.x];
     flux[4 * blockIdx.x + threadIdx.x] = t * scale;
+  }
+}
+
+// the same with one scale per image (many cameras per call: the pixel solid angle is the camera's)
+__global__ void __launch_bounds__(256) k_reduce_cams(int64_t n, size_t stride, const double* I, const double* Q, const double* U,
+                                                     const double* V, const double* scale, double* flux) {
+  const size_t o = (size_t)blockIdx.x * stride;
+  double s[4] = {0, 0, 0, 0};
+  for (int64_t q = threadIdx.x; q < n; q += blockDim.x) { s[0] += I[o + q]; s[1] += Q[o + q]; s[2] += U[o + q]; s[3] += V[o + q]; }
+  __shared__ double sh[8][4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) s[k] = warp_sum(s[k]);
+  if ((threadIdx.x & 31) == 0) for (int k = 0; k < 4; ++k) sh[threadIdx.x >> 5][k] = s[k];
+  __syncthreads();
+  if (threadIdx.x < 4) {
+    double t = sh[0][threadIdx.x];
+    for (int w = 1; w < 8; ++w) t += sh[w][threadIdx.x];
+    flux[4 * blockIdx.x + threadIdx.x] = t * scale[blockIdx.x];
   }
 }
 

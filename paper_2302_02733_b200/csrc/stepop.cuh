@@ -50,6 +50,8 @@ struct OpArgs {
   double* ops;                // operator records of the batch, layout op_addr(); record n of a ray: camera projection (4), irregular flag (1)
   int32_t* irr_slots; int* irr_count;   // slots (positions in the batch) of the rays left to k_transfer
   int test_irregular;         // tests: declare every 7th slot irregular, so that the hand-over to k_transfer is exercised
+  // many cameras per launch (k_stepop<MODEL, true>): ray q belongs to camera q / rays_per_cam
+  const CamDev* cams; const Units* units_arr; int64_t rays_per_cam;
 };
 
 #ifndef IPOLE_OP_THREADS
@@ -64,16 +66,21 @@ __device__ __forceinline__ void shfl_down4(const double v[4], double o[4]) {
   for (int m = 0; m < 4; ++m) o[m] = __shfl_down_sync(0xffffffffu, v[m], 1);
 }
 
-template <int MODEL>
+template <int MODEL, bool MC = false>
 __global__ void __launch_bounds__(IPOLE_OP_THREADS, IPOLE_OP_MINB) k_stepop(const __grid_constant__ OpArgs A) {
   static_assert(MODEL == MODEL_ADAF, "the step-parallel pass is built for the analytic flow");
-  const CamDev& C = A.cam;
+  const CamDev& C0 = A.cam;
   __shared__ __align__(8) unsigned char model_smem[sizeof(AdafParams)];
   for (int i = threadIdx.x; i < (int)sizeof(AdafParams); i += blockDim.x) model_smem[i] = ((const unsigned char*)A.model)[i];
   __syncthreads();
-  const void* model = model_smem;
   const int lane = threadIdx.x & 31;
   const size_t slot_rec = (size_t)(A.cap + 1) * REC_DOUBLES;
+  // MC: the ray's own camera (geometry, transverse legs) and units, and the flow's ISCO for that spin, in registers
+  AdafParams model_l = *(const AdafParams*)model_smem;
+  Geom Gl = C0.G;
+  double ec1[4], ec2[4], nu_obs_l = A.units.nu_obs, dl_unit_l = A.units.dl_unit;
+#pragma unroll
+  for (int m = 0; m < 4; ++m) { ec1[m] = C0.ecov1[m]; ec2[m] = C0.ecov2[m]; }
 
   for (;;) {
     // lane 0 leaves the previous iteration later than the others (it writes the ray's last record): without this
@@ -86,6 +93,19 @@ __global__ void __launch_bounds__(IPOLE_OP_THREADS, IPOLE_OP_MINB) k_stepop(cons
     const int32_t q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
     const int n = A.nsteps[q];
     if (n < 0) continue;                     // overflowed its slot: done by the long-ray pass
+    if (MC) {
+      const int ci = (int)(q / A.rays_per_cam);
+      const CamDev& Cc = A.cams[ci];
+      Gl = Cc.G;
+#pragma unroll
+      for (int m = 0; m < 4; ++m) { ec1[m] = Cc.ecov1[m]; ec2[m] = Cc.ecov2[m]; }
+      nu_obs_l = A.units_arr[ci].nu_obs; dl_unit_l = A.units_arr[ci].dl_unit;
+      model_l.r_isco = isco_radius(Gl.a);
+    }
+    const Geom& G = MC ? Gl : C0.G;
+    Units Ul = A.units;
+    if (MC) { Ul.nu_obs = nu_obs_l; Ul.dl_unit = dl_unit_l; }
+    const void* model = MC ? (const void*)&model_l : (const void*)model_smem;
     const double* rec = A.path + (size_t)li * slot_rec;
     bool regular = true;
     double mc[4] = {0.0, 0.0, 0.0, 0.0};     // lane 0, first chunk: projection of step 0's legs on the camera tetrad
@@ -113,10 +133,10 @@ __global__ void __launch_bounds__(IPOLE_OP_THREADS, IPOLE_OP_MINB) k_stepop(cons
         }
         x1m = Xm[1];
         Point p; Sym7 g; Inv6 gi;
-        transport_generator(C.G, Xm, Km, p, g, gi, Am);
+        transport_generator(G, Xm, Km, p, g, gi, Am);
         h = 0.5 * dl;
         double e1[4], e2[4];
-        applied = plasma_tetrad<MODEL, false>(C.G, model, nullptr, A.units, Xm, Km, p, g, gi, nullptr, e1, e2, e1c, e2c, F);
+        applied = plasma_tetrad<MODEL, false>(G, model, nullptr, Ul, Xm, Km, p, g, gi, nullptr, e1, e2, e1c, e2c, F);
         if (applied) {
 #pragma unroll
           for (int m = 0; m < 4; ++m) { fo1[m] = e1[m]; fo2[m] = e2[m]; }
@@ -138,9 +158,10 @@ __global__ void __launch_bounds__(IPOLE_OP_THREADS, IPOLE_OP_MINB) k_stepop(cons
         }
         double* o = A.ops + op_addr(li, A.cap, s, 0);   // part 1 at o + 128
         st_global_v4(o, m11, m12, m21, m22);
-        st_global_v4(o + 128, x1m, applied ? F.cosT : 0.0, applied ? F.nu : 0.0, dl * A.units.dl_unit);
+        st_global_v4(o + 128, x1m, applied ? F.cosT : 0.0, applied ? F.nu : 0.0, dl * Ul.dl_unit);
         if (s == 0) {
-          mc[0] = dot4(C.ecov1, fo1); mc[1] = dot4(C.ecov1, fo2); mc[2] = dot4(C.ecov2, fo1); mc[3] = dot4(C.ecov2, fo2);
+          mc[0] = dot4(MC ? ec1 : C0.ecov1, fo1); mc[1] = dot4(MC ? ec1 : C0.ecov1, fo2);
+          mc[2] = dot4(MC ? ec2 : C0.ecov2, fo1); mc[3] = dot4(MC ? ec2 : C0.ecov2, fo2);
         }
       }
     }
@@ -155,6 +176,7 @@ __global__ void __launch_bounds__(IPOLE_OP_THREADS, IPOLE_OP_MINB) k_stepop(cons
 }
 
 struct ApArgs {
+  const double* nu3_arr; int64_t rays_per_cam;   // many cameras per launch: nu_obs^3 of camera q / rays_per_cam (nullable)
   AdafParams model;           // the three power laws (by value: 56 B)
   EdfDev edf;                 // k_apply<true>: j, alpha by quadrature over the electron distribution (edf.cuh)
   double nu3;                 // nu_obs^3: invariant I/nu^3 -> specific intensity at the camera
@@ -259,7 +281,8 @@ __global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? IPOLE_AP_EDF_MINB : IP
     }
     if (n > 0) {
       stokes_congruence(mc[0], mc[1], mc[2], mc[3], S);
-      A.I[q] = S[0] * A.nu3; A.Q[q] = S[1] * A.nu3; A.U[q] = S[2] * A.nu3; A.V[q] = S[3] * A.nu3;
+      const double nu3 = A.nu3_arr ? A.nu3_arr[q / A.rays_per_cam] : A.nu3;
+      A.I[q] = S[0] * nu3; A.Q[q] = S[1] * nu3; A.U[q] = S[2] * nu3; A.V[q] = S[3] * nu3;
       if (A.tau) A.tau[q] = tau;
       if (A.tauF) A.tauF[q] = tauF;
     }

@@ -18,7 +18,7 @@ OK, EINVAL, ENOMODEL, ENOMEM, ECUDA, ENOIMAGE = 0, -1, -2, -3, -4, -5
 
 #: every symbol include/ipole.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_options", "ipole_set_path_free", "ipole_set_edf", "ipole_set_transfer_split", "ipole_set_unpolarized", "ipole_load_model_adaf",
-           "ipole_load_model_slab", "ipole_load_model_grid", "ipole_make_image", "ipole_make_pixels", "ipole_make_images_adaf", "ipole_make_images_grid", "ipole_make_image_adaptive",
+           "ipole_load_model_slab", "ipole_load_model_grid", "ipole_make_image", "ipole_make_pixels", "ipole_make_images_adaf", "ipole_make_images_grid", "ipole_make_images_cameras", "ipole_make_image_adaptive",
            "ipole_get_ray_info", "ipole_get_stats", "ipole_get_camera_tetrad", "ipole_trace_pixel",
            "ipole_eval_connection", "ipole_eval_coefficients", "ipole_eval_coefficients_edf", "ipole_eval_stokes_step", "ipole_eval_bessel",
            "ipole_eval_plasma", "ipole_eval_math", "ipole_measure_fp64_peak", "ipole_last_cuda_error", "ipole_free", "ipole_strerror",
@@ -101,6 +101,7 @@ def lib():
         L.ipole_make_images_adaf.argtypes = [vp, C.c_int32, C.POINTER(AdafParams), vp] + [vp] * 7
         L.ipole_make_image_adaptive.argtypes = [vp, C.c_int32, C.c_double, C.c_double, vp, vp, vp, vp, vp, C.POINTER(AdaptiveInfo)]
         L.ipole_make_images_grid.argtypes = [vp, C.c_int32, C.POINTER(GridScales), vp] + [vp] * 7
+        L.ipole_make_images_cameras.argtypes = [vp, C.c_int32, C.POINTER(Camera)] + [vp] * 7
         L.ipole_get_ray_info.argtypes = [vp, vp, vp]
         L.ipole_get_stats.argtypes = [vp, C.POINTER(Stats)]
         L.ipole_get_camera_tetrad.argtypes = [vp, dp, dp]
@@ -270,6 +271,30 @@ class Ipole:
         for m, kw in enumerate(sets):
             arr[m] = GridScales(kw["M_unit"], kw["Rlow"], kw["Rhigh"])
         return self._make_images(lib().ipole_make_images_grid, "ipole_make_images_grid", M, arr, freqs, maps, out, host)
+
+    def make_images_cameras(self, cams, maps=False, out=None, host=False):
+        """Many small images whose geometry differs (include/ipole.h ipole_make_images_cameras): `cams` is a
+        list of camera dicts (the keys of the constructor); one pass of the pipeline over the union of their rays.
+        Returns dict of [n_cams, ny, nx] arrays plus "flux_jy" [n_cams, 4]."""
+        M = len(cams)
+        arr = (Camera * M)()
+        for m, kw in enumerate(cams):
+            for k, v in kw.items():
+                setattr(arr[m], k, v)
+        ny, nx = arr[0].ny, arr[0].nx
+        names = ["I", "Q", "U", "V"] + (["tau", "tauF"] if maps else [])
+        if out is None:
+            if host:
+                out = {k: np.empty((M, ny, nx), dtype=np.float64) for k in names}
+            else:
+                import torch
+                out = {k: torch.empty((M, ny, nx), dtype=torch.float64, device="cuda") for k in names}
+        flux = np.zeros((M, 4))
+        args = [_ptr(out.get(k)) for k in ("I", "Q", "U", "V", "tau", "tauF")]
+        _chk(lib().ipole_make_images_cameras(self._h, M, arr, *args, _ptr(flux)), "ipole_make_images_cameras")
+        out = dict(out)
+        out["flux_jy"] = flux
+        return out
 
     def _make_images(self, fn, what, M, arr, freqs, maps, out, host):
         fr = None if freqs is None else np.ascontiguousarray(freqs, dtype=np.float64)
