@@ -352,6 +352,46 @@ def run_cams(args, ipole, replicas, W, wl, world, rank, local, barrier):
     print(json.dumps(line), flush=True)
 
 
+def run_fp32_study(args, ipole, W, wl):
+    """--fp32-geodesic: the same image with the geodesics integrated in single precision
+    (ipole_set_geodesic_fp32; transfer still FP64) beside the FP64 image: stage times and per-pixel differences.  A study
+    line, not a bench value: `value` is the FP32-geodesic image's rays/s."""
+    import torch
+    n = wl["n"]
+    cam = W.camera("adaf", n)
+    g = ipole.Ipole(**cam); g.set_stream(torch.cuda.current_stream()); g.load_adaf(**W.ADAF)
+    ref = {k: torch.empty((n, n), dtype=torch.float64, device="cuda") for k in "IQUV"}
+    out = {k: torch.empty((n, n), dtype=torch.float64, device="cuda") for k in "IQUV"}
+    for _ in range(args.warmup + args.steps):
+        g.make_image(out=ref)
+    torch.cuda.synchronize(); s64 = g.stats(); ns64, nt64 = g.ray_info()
+    g.set_geodesic_fp32(True)
+    for _ in range(args.warmup + args.steps):
+        g.make_image(out=out)
+    torch.cuda.synchronize(); s32 = g.stats(); ns32, nt32 = g.ray_info()
+    I = ref["I"]; peak = float(I.max())
+    rel = ((out["I"] - I).abs() / (I.abs() + 1e-300)).flatten()
+    lit = (I > 1e-6 * peak).flatten()
+    pol = torch.maximum(torch.maximum((out["Q"] - ref["Q"]).abs(), (out["U"] - ref["U"]).abs()), (out["V"] - ref["V"]).abs()).flatten() / peak
+    sub = rel[lit][:: max(1, int(lit.sum()) // 2000000)]
+    line = {"metric": "rays_per_s", "value": n * n / (s32["ms_total"] * 1e-3), "unit": "rays/s", "n_gpus": 1, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": s32["ms_total"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32 geodesics + f64 transfer (study)", "data": "synthetic",
+            "config": {"workload": args.workload, "image": "%dx%d" % (n, n), "model": "adaf", "variant": "FP32 study, not a product path"},
+            "fp32_study": {"ms_geodesic_f64": s64["ms_geodesic"], "ms_geodesic_f32": s32["ms_geodesic"],
+                           "ms_image_f64": s64["ms_total"], "ms_image_f32": s32["ms_total"],
+                           "geodesic_speedup": s64["ms_geodesic"] / s32["ms_geodesic"], "image_speedup": s64["ms_total"] / s32["ms_total"],
+                           "rel_dI_median": float(sub.median()), "rel_dI_p99": float(torch.quantile(sub, 0.99)),
+                           "rel_dI_max": float(rel[lit].max()), "dI_over_peak_max": float(((out["I"] - I).abs() / peak).max()),
+                           "dQUV_over_peak_max": float(pol.max()),
+                           "flux_rel": [abs(a / b - 1) if b else 0.0 for a, b in zip(s32["flux_jy"], s64["flux_jy"])],
+                           "rays_with_other_step_count": float((ns64 != ns32).mean()), "rays_with_other_turn_count": float((nt64 != nt32).mean()),
+                           "note": "differences are FP32-geodesic image minus the FP64 image of this library (which matches the oracle "
+                                   "to <= 1e-9 per pixel, tests/test_gpu_parity.py); pixels brighter than 1e-6 of the peak"},
+            "gpu_launches": s32["n_launches"], "roofline": None, "e2e": None}
+    print(json.dumps(line), flush=True)
+
+
 def run_adaptive(args, g, replicas, wl, cam, world, rank, local, barrier):
     """One step = one ipole_make_image_adaptive call; the full image of the same workload is made once for the error."""
     import torch
@@ -660,6 +700,8 @@ def main():
     ap.add_argument("--edf", type=int, default=0, choices=[0, 1, 2],
                     help="second physics workload (PAPER.md:78): j, alpha integrated numerically over a Maxwell-Juettner (1) or "
                          "kappa (2) electron distribution at every step (ipole_set_edf); analytic-flow workloads only")
+    ap.add_argument("--fp32-geodesic", action="store_true",
+                    help="FP32 study (PAPER.md:70): geodesics in single precision, compared with the FP64 image; analytic-flow workloads")
     ap.add_argument("--no-second-workload", action="store_true",
                     help="default run only: skip the grid4096 half of configs[4] that is otherwise timed after adaf4096")
     ap.add_argument("--path-free", action="store_true",
@@ -699,6 +741,10 @@ def main():
 
     if wl.get("cams"):
         run_cams(args, ipole, replicas, W, wl, world, rank, local, barrier)
+        return finish()
+    if args.fp32_geodesic:
+        if rank == 0:
+            run_fp32_study(args, ipole, W, wl)
         return finish()
     if wl.get("sweep") or args.adaptive:
         cam = W.camera(wl["kind"], wl["n"])

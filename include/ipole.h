@@ -152,6 +152,13 @@ int  ipole_set_transfer_split(ipole_ctx*, int32_t on);
  * IPOLE_EINVAL: NULL, kind outside 0..2, kappa <= 1, n_nodes > 1024. */
 typedef struct { int32_t kind; int32_t n_nodes; double kappa; } ipole_edf;
 int  ipole_set_edf(ipole_ctx*, const ipole_edf*);
+/* FP32 STUDY switch, not a product path ("further code acceleration may be also obtained by switching to single
+ * precision calculations").  on != 0: the geodesics of the analytic-flow and slab models on the stored
+ * path are integrated in single precision (k_geodesic_f32: same step rule and stop rules), their path records widened to
+ * FP64, and the transfer runs on them in FP64 as usual -- a mixed-precision image whose error and speed
+ * profiles/r2_fp32_study.md reports (bench.py --fp32-geodesic).  Ignored for the grid model, the path-free variant and
+ * ipole_make_images_cameras.  Returns IPOLE_EINVAL for a NULL context. */
+int  ipole_set_geodesic_fp32(ipole_ctx*, int32_t on);
 /* Unpolarized transfer (the model-fitting loop makes "nonpolarized images"; polarized
  * transfer is "far more complex and computationally demanding"; reading R-12 in DESIGN.md).  on != 0: every image
  * entry (ipole_make_image, _pixels, _images_adaf, _images_grid, _image_adaptive) solves the scalar equation

@@ -12,6 +12,7 @@
 #include <vector>
 #include "kernels.cuh"
 #include "stepop.cuh"
+#include "geo_f32.cuh"
 #include "adaptive.cuh"
 
 using namespace ipole;
@@ -55,6 +56,8 @@ struct ipole_ctx {
   CamDev* d_mc_cams = nullptr; Units* d_mc_units = nullptr; double* d_mc_nu3 = nullptr; double* d_mc_scale = nullptr;
   int mc_cap = 0; int n_mc = 0; int64_t mc_rays_per_cam = 0;
   int occ_geo_mc = 0, occ_op_mc = 0;
+  int opt_geo_fp32 = 0;          // FP32 study (geo_f32.cuh): geodesics in single precision, transfer in FP64
+  int occ_geo_f32 = 0;
   int opt_group = 1;             // grid model: transfer with warp-level scheduling (k_transfer_group)
   int occ_group = 0;
   int opt_tight = 1;             // sorted rays: path slots sized batch by batch from the predicted step counts
@@ -246,7 +249,9 @@ int grid_for(ipole_ctx* c, int occ, int threads, int64_t rays, int reserve = 0) 
 
 int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays, cudaStream_t st, int reserve = 0) {
   const int s = span_begin(c, kind, st);
-  if (c->n_mc) {
+  if (c->opt_geo_fp32 && kind != LK_PROBE && !c->n_mc && !a.grid && !a.endp) {
+    k_geodesic_f32<<<grid_for(c, c->occ_geo_f32, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
+  } else if (c->n_mc) {
     a.cams = c->d_mc_cams; a.rays_per_cam = c->mc_rays_per_cam;
     k_geodesic<false, true><<<grid_for(c, c->occ_geo_mc, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
   } else if (a.grid) k_geodesic<true><<<grid_for(c, c->occ_geo_occ, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
@@ -790,6 +795,7 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_op, k_stepop<MODEL_ADAF>, IPOLE_OP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_op_mc, k_stepop<MODEL_ADAF, true>, IPOLE_OP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo_mc, k_geodesic<false, true>, IPOLE_GEO_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo_f32, k_geodesic_f32, IPOLE_GEO_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap, k_apply<false>, IPOLE_AP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_edf, k_apply<true>, IPOLE_AP_THREADS, EDF_MAX_NODES * sizeof(double4));
   { const char* e = std::getenv("IPOLE_NO_SPLIT"); if (e && e[0] == '1') c->opt_split = 0; }
@@ -863,6 +869,12 @@ int ipole_set_edf(ipole_ctx* c, const ipole_edf* e) {
   k_edf_setup_nodes<<<(nn + 127) / 128, 128, 0, c->stream>>>(c->edf, c->d_edf_nodes);
   k_edf_setup_norm<<<(EDF_TAB_N + 127) / 128, 128, 0, c->stream>>>(c->edf, c->d_edf_lnnorm);
   CK(cudaGetLastError());
+  return IPOLE_OK;
+}
+
+int ipole_set_geodesic_fp32(ipole_ctx* c, int32_t on) {
+  if (!c) return IPOLE_EINVAL;
+  c->opt_geo_fp32 = on ? 1 : 0;
   return IPOLE_OK;
 }
 
