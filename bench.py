@@ -681,6 +681,64 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+NCU_KEYS = ["gpu__time_duration.sum", "launch__grid_size", "launch__block_size", "launch__registers_per_thread",
+            "sm__warps_active.avg.pct_of_peak_sustained_active", "smsp__thread_inst_executed_per_inst_executed.ratio",
+            "smsp__sass_average_branch_targets_threads_uniform.pct", "sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active",
+            "smsp__issue_active.avg.pct_of_peak_sustained_active", "sm__inst_executed_pipe_alu.avg.pct_of_peak_sustained_active",
+            "sm__inst_executed_pipe_lsu.avg.pct_of_peak_sustained_active", "l1tex__data_pipe_lsu_wavefronts.avg.pct_of_peak_sustained_elapsed",
+            "smsp__inst_executed.sum", "dram__bytes_read.sum", "dram__bytes_write.sum",
+            "gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed", "l1tex__t_sector_hit_rate.pct", "lts__t_sector_hit_rate.pct",
+            "sass__inst_executed_local_loads", "sass__inst_executed_local_stores", "sm__cycles_elapsed.avg"]
+
+
+def summarize_ncu(args):
+    """--summarize-ncu REPORT: the text summaries under profiles/ (no GPU needed: reads an .ncu-rep with the ncu CLI).
+    Quoted counters come straight from `ncu -i REPORT --page raw --csv`; the lines after the blank line are DERIVED here:
+    FP64 thread instructions = per_cycle_elapsed counters x sm__cycles_elapsed, flop = 2 DFMA + DADD + DMUL, and, with
+    --ncu-steps-from read|write, per-step figures with steps = DRAM bytes read|written / --ncu-bytes-per-step."""
+    import csv
+    import io
+    import re
+    raw = subprocess.run(["ncu", "-i", args.summarize_ncu, "--page", "raw", "--csv"], capture_output=True, text=True, check=True).stdout
+    rows = list(csv.reader(io.StringIO(raw)))
+    hdr, units = rows[0], rows[1]
+    mult = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}
+    tmul = {"s": 1e3, "ms": 1.0, "us": 1e-3, "ns": 1e-6}   # -> ms (ncu picks the unit per report)
+    for r in rows[2:]:
+        d = dict(zip(hdr, r))
+        if args.ncu_kernel and not re.search(args.ncu_kernel, d["Kernel Name"]):
+            continue
+        num = lambda k: float(d[k].replace(",", ""))
+        un = lambda k: units[hdr.index(k)]
+        print("%-78s %s" % ("Kernel Name", d["Kernel Name"]))
+        for k in NCU_KEYS:
+            if k in d:
+                print("%-78s %s %s" % (k, d[k], un(k)))
+        cyc = num("sm__cycles_elapsed.avg")
+        ops = {k: num("smsp__sass_thread_inst_executed_op_%s_pred_on.sum.per_cycle_elapsed" % k) * cyc for k in ("dfma", "dadd", "dmul")}
+        flop = 2 * ops["dfma"] + ops["dadd"] + ops["dmul"]
+        ms = num("gpu__time_duration.sum") * tmul.get(un("gpu__time_duration.sum"), 1.0)
+        print()
+        print("FP64 thread instructions: DFMA %.4e  DADD %.4e  DMUL %.4e   flop (DFMA=2) %.4e" % (ops["dfma"], ops["dadd"], ops["dmul"], flop))
+        tf = flop / (ms * 1e-3) / 1e12
+        print("achieved %.2f TFLOP/s = %.3f of %.2f TFLOP/s (148 SM x 64 lanes x 2 x 1.965 GHz); FMA share of FP64 instructions %.2f"
+              % (tf, tf / FP64_PEAK_TFLOPS, FP64_PEAK_TFLOPS, ops["dfma"] / sum(ops.values())))
+        st = {k: float(v.replace(",", "")) for k, v in d.items()
+              if k.startswith("smsp__average_warps_issue_stalled") and k.endswith("_per_issue_active.ratio") and v}
+        print("warp stall cycles per issued instruction: " + "  ".join(
+            "%s %.2f" % (k.replace("smsp__average_warps_issue_stalled_", "").replace("_per_issue_active.ratio", ""), v)
+            for k, v in sorted(st.items(), key=lambda x: -x[1])[:9]))
+        if args.ncu_steps_from:
+            key = "dram__bytes_read.sum" if args.ncu_steps_from == "read" else "dram__bytes_write.sum"
+            steps = num(key) * mult[un(key)] / args.ncu_bytes_per_step
+            traffic = (num("dram__bytes_read.sum") * mult[un("dram__bytes_read.sum")] + num("dram__bytes_write.sum") * mult[un("dram__bytes_write.sum")])
+            print("steps of this launch (DRAM bytes %s / %g): %.4e" % ("read" if args.ncu_steps_from == "read" else "written", args.ncu_bytes_per_step, steps))
+            print("=> %.0f flop per step, %.0f FP64 instructions per step, %.0f warp instructions x threads per step, %.1f B of DRAM traffic per step"
+                  % (flop / steps, sum(ops.values()) / steps, num("smsp__inst_executed.sum") * num("smsp__thread_inst_executed_per_inst_executed.ratio") / steps,
+                     traffic / steps))
+        print()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -706,7 +764,13 @@ def main():
                     help="default run only: skip the grid4096 half of configs[4] that is otherwise timed after adaf4096")
     ap.add_argument("--path-free", action="store_true",
                     help="the paper's own GPU design (PAPER.md:43): no stored path, forward re-integration")
+    ap.add_argument("--summarize-ncu", metavar="REPORT", help="print the text summary of an .ncu-rep (profiles/*.txt); no GPU needed")
+    ap.add_argument("--ncu-kernel", default=None, help="--summarize-ncu: only kernels whose name matches this regex")
+    ap.add_argument("--ncu-steps-from", choices=["read", "write"], default=None)
+    ap.add_argument("--ncu-bytes-per-step", type=float, default=64.0)
     args = ap.parse_args()
+    if args.summarize_ncu:
+        return summarize_ncu(args)
     if args.impl == "reference":
         return run_reference(args)
 

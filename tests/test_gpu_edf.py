@@ -75,3 +75,20 @@ def test_edf_long_rays_batches_and_unsupported_combinations(ipole):
         g.set_edf(2, kappa=0.5)
     g.set_edf(0)
     g.make_images_adaf([dict(n0=1e6)])
+
+
+def test_fp32_geodesic_study_switch(ipole):
+    """ipole_set_geodesic_fp32 (PAPER.md:70 study, profiles/r2_fp32_study.md): single-precision geodesics give the image to
+    ~1e-5..1e-3 per pixel, not to 1e-7; switching back restores the FP64 image bit for bit."""
+    cam = W.camera("adaf", 48)
+    g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
+    a = to_np(g.make_image())
+    g.set_geodesic_fp32(True)
+    b = to_np(g.make_image())
+    g.set_geodesic_fp32(False)
+    c = to_np(g.make_image())
+    for k in a:
+        assert np.array_equal(a[k], c[k]), k
+    lit = a["I"] > 1e-6 * a["I"].max()
+    rel = np.abs(b["I"] - a["I"])[lit] / a["I"][lit]
+    assert 1e-7 < np.median(rel) < 1e-3 and abs(b["I"].sum() / a["I"].sum() - 1) < 1e-3
