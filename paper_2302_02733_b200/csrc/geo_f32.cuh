@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(IPOLE_GEO_THREADS, 6) k_geodesic_f32(const __g
   const CamDev& C = A.cam;
   const int64_t count = A.count_dev ? (int64_t)*A.count_dev : A.count;
   const size_t slot_doubles = (size_t)(A.cap + 1) * REC_DOUBLES;
-  float X[4], K[4];
+  float X[4] = {0.f, 0.f, 0.f, 0.f}, K[4] = {0.f, 0.f, 0.f, 0.f};
   double* rec = nullptr;
   int64_t li;
   int32_t q = 0;
