@@ -103,6 +103,10 @@ typedef struct {
                               the per-ray apply pass; both are part of ms_transfer                      */
   int64_t n_retry;         /* rays that outgrew the path slots of their batch (sized from the predicted step count of the
                               batch's longest ray) and were traced again with S_cap slots                  */
+  int32_t n_lanes;         /* 2: the batches alternated between two streams (ipole_set_batch_overlap) -- kernels of
+                              consecutive batches then run side by side, their event times overlap, and ms_geodesic +
+                              ms_transfer exceeds ms_total; 1: one batch after the other                   */
+  int32_t reserved_;
 } ipole_stats;
 
 /* Create a context. Computes the camera tetrad on the device. IPOLE_EINVAL on bad parameters. */
@@ -127,15 +131,24 @@ int  ipole_set_options(ipole_ctx*, uint64_t path_bytes, int32_t sort_rays);
  * on == 0 (default): stored path.  Returns IPOLE_EINVAL for a NULL context. */
 int  ipole_set_path_free(ipole_ctx*, int32_t on);
 /* Transfer as two kernels (default on; "at every single step ... evaluate emission, self-absorption and
- * Faraday coefficients at a given point": everything of a step except the update of the four Stokes numbers depends
- * on the stored path alone).  on != 0: on the stored path, for the analytic flow, a step-parallel kernel turns every
- * path step into a 96-byte operator record (projection of the carried polarization basis on the step's plasma tetrad,
- * and the eight coefficients times the step length), and a per-ray kernel applies the records from the far end to
- * the camera.  on == 0: the single per-ray transfer kernel does both (also used, whatever this switch says, for the
+ * Faraday coefficients at a given point": everything of a step except the coefficients' action on the four Stokes
+ * numbers depends on the stored path alone).  on != 0: on the stored path, for the analytic flow, a step-parallel kernel
+ * turns every path step into a 64-byte operator record (the projection of the carried polarization basis on the step's
+ * plasma tetrad; ln r, the angle to the field, the frequency in the plasma frame, the step length), and a per-ray
+ * kernel evaluates the coefficients from it and applies them, from the far end to the camera.  on == 0: the single
+ * per-ray transfer kernel does both (also used, whatever this switch says, for the
  * slab and grid models, the sweeps, the path-free and unpolarized variants, long rays, and rays with a step that
  * crosses no plasma).  The two give the same image up to rounding.  on == 2 is a test mode: as 1, but every seventh
  * ray of a batch is handed to the single kernel as if it had such a step.  Returns IPOLE_EINVAL for a NULL context. */
 int  ipole_set_transfer_split(ipole_ctx*, int32_t on);
+/* Batches side by side (default on).  A 4096 x 4096 image is 25-31 G steps of 64 (+ 64) bytes and goes through HBM in
+ * tens of batches (PAPER.md:43 is the paper's answer to the same memory limit).  Every kernel of
+ * a batch is persistent and ends in a tail of milliseconds while its last rays finish.  on != 0: consecutive batches
+ * alternate between two streams, each with half of the path memory, so that the next batch's kernels fill those tails.
+ * on == 0: one batch after the other on the context's stream (then the per-stage times of ipole_get_stats add up to
+ * ms_total; bench.py measures its per-kernel figures this way).  Same image either way, bit for bit (a ray's arithmetic
+ * does not depend on its batch).  Single-batch images and the sweeps always run on one stream.  IPOLE_EINVAL for NULL. */
+int  ipole_set_batch_overlap(ipole_ctx*, int32_t on);
 /* Second physics workload (outlook: electron distribution functions "for which accurate prescriptions ... do
  * not exist and the integration of synchrotron emissivity over the electron energy distribution function requires
  * numerical integration during ray tracing"; the paper gives no formulas: reading R-13 in DESIGN.md).

@@ -85,6 +85,11 @@ struct ipole_ctx {
   cudaStream_t side = nullptr;                                  // long-ray passes overlap the bulk batches here
   cudaStream_t qstream = nullptr;                               // 4-byte read-backs that must not wait for `side`
   cudaEvent_t ev_geo = nullptr, ev_side = nullptr;
+  // bulk batches alternate between `stream` and `lane2`, each with its own half of the path and operator buffers: the
+  // persistent kernels of one batch drain while those of the next fill the GPU
+  cudaStream_t lane2 = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+  int opt_overlap = 1;
   int64_t ray_cap = 0;           // capacity of the per-ray buffers below
   int32_t *d_nsteps = nullptr, *d_nturn = nullptr, *d_order = nullptr, *d_key = nullptr, *d_long = nullptr;
   int2* d_srange = nullptr;      // grid model: per ray, the steps that may cross plasma (k_geodesic<true>)
@@ -93,7 +98,7 @@ struct ipole_ctx {
   int32_t* d_probe = nullptr; int64_t probe_cap = 0;
   unsigned long long* d_queues = nullptr;
   unsigned int* d_hist = nullptr;
-  int* d_small = nullptr;        // [0] long_count, [1] probe max, [2] adaptive list length, [4] irregular rays of a batch
+  int* d_small = nullptr;        // [0] long_count, [1] probe max, [2] adaptive list length, [4] / [6] irregular rays of a batch (lane 0 / 1), [5] retries
   ReducePartial* d_part = nullptr;
   ReduceOut* d_red = nullptr;
 
@@ -179,7 +184,7 @@ int ensure_rays(ipole_ctx* c, int64_t n) {
   CK(cudaMalloc(&c->d_long, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_nsteps_long, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_srange, n * sizeof(int2)));
-  CK(cudaMalloc(&c->d_irr, n * sizeof(int32_t)));
+  CK(cudaMalloc(&c->d_irr, 2 * n * sizeof(int32_t)));   // one list per lane
   CK(cudaMalloc(&c->d_retry, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_out, 6 * n * sizeof(double)));
   c->ray_cap = n;
@@ -346,13 +351,14 @@ int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_
 
 // split transfer of one batch (stepop.cuh): k_stepop over the steps, k_apply over the rays, then k_transfer for the
 // rays k_stepop could not express (listed on the device; usually none)
-int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStream_t st, int reserve) {
-  int* irr_count = c->d_small + 4;
+int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStream_t st, int reserve, double* ops, int lane) {
+  int* irr_count = c->d_small + (lane ? 6 : 4);
+  int32_t* irr = c->d_irr + (lane ? c->ray_cap : 0);
   CK(cudaMemsetAsync(irr_count, 0, sizeof(int), st));
   OpArgs o;
   std::memset(&o, 0, sizeof o);
   o.cam = a.cam; o.units = a.units; o.model = a.model; o.cap = a.cap; o.base = a.base; o.count = a.count; o.order = a.order;
-  o.path = a.path; o.nsteps = a.nsteps; o.queue = a.queue; o.ops = c->d_ops; o.irr_slots = c->d_irr; o.irr_count = irr_count; o.test_irregular = (c->opt_split == 2);
+  o.path = a.path; o.nsteps = a.nsteps; o.queue = a.queue; o.ops = ops; o.irr_slots = irr; o.irr_count = irr_count; o.test_irregular = (c->opt_split == 2);
   {
     const int s = span_begin(c, LK_OPS, st);
     // one warp per ray at a time
@@ -371,7 +377,7 @@ int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStrea
   std::memset(&p, 0, sizeof p);
   p.nu3 = a.units.nu_obs * a.units.nu_obs * a.units.nu_obs;
   p.model = c->adaf_host;
-  p.cap = a.cap; p.base = a.base; p.count = a.count; p.order = a.order; p.ops = c->d_ops; p.nsteps = a.nsteps;
+  p.cap = a.cap; p.base = a.base; p.count = a.count; p.order = a.order; p.ops = ops; p.nsteps = a.nsteps;
   p.queue = a.queue + 1;
   p.I = a.I; p.Q = a.Q; p.U = a.U; p.V = a.V; p.tau = a.tau; p.tauF = a.tauF;
   {
@@ -386,7 +392,7 @@ int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStrea
     CK(cudaGetLastError());
   }
   RtArgs t = a;
-  t.queue = a.queue + 2; t.count_dev = irr_count; t.slots = c->d_irr;
+  t.queue = a.queue + 2; t.count_dev = irr_count; t.slots = irr;
   {
     const int s = span_begin(c, LK_RT, st);
     k_transfer<MODEL_ADAF, 0><<<std::max(1, c->n_sm / 8), IPOLE_RT_THREADS, 0, st>>>(t);
@@ -609,6 +615,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   const bool tight = order != nullptr && !bin_prefix.empty() && c->opt_tight;
   struct Batch { int64_t base, cnt; int cap; };
   std::vector<Batch> plan;
+  size_t lane_budget = budget;            // path (+ operator) memory of one lane
   auto make_plan = [&](int64_t total_rays, bool use_bins) {
     plan.clear();
     for (int64_t base = 0; base < total_rays;) {
@@ -618,7 +625,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
         const int64_t pred_hi = (int64_t)(SORT_BINS - std::max(bin, 0)) * bin_width;
         cb = (int)std::min<int64_t>(cap, (int64_t)(pred_hi * 1.15) + 64);
       }
-      int64_t B = (int64_t)(budget / ((size_t)(cb + 1) * step_bytes));
+      int64_t B = (int64_t)(lane_budget / ((size_t)(cb + 1) * step_bytes));
       if (B >= 64) B &= ~(int64_t)31;           // whole groups of 32 slots (operator records, stepop.cuh)
       B = std::max<int64_t>(1, std::min(B, total_rays - base));
       plan.push_back({base, B, cb});
@@ -626,48 +633,70 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
       base += B;
     }
   };
+  // Two lanes: consecutive batches alternate between two streams, each with its own half of the path (and operator)
+  // memory.  Every kernel of a batch is persistent and ends in a tail during which the GPU drains (the last rays of a
+  // geodesic launch are milliseconds long); the other lane's kernels fill those tails.  One lane when a single batch
+  // holds everything, and for the sweeps (their parameter tables are per stream).
+  int n_lanes = 1;
   make_plan(n, tight);
-  size_t need_path = 0, need_ops = 0;
-  for (const Batch& b : plan) {
-    need_path = std::max(need_path, (size_t)b.cnt * (size_t)(b.cap + 1) * rec_bytes);
-    need_ops = std::max(need_ops, (size_t)((b.cnt + 31) / 32 * 32) * (size_t)(b.cap + 1) * OP_DOUBLES * sizeof(double));
+  if (c->opt_overlap && c->lane2 && !sw && plan.size() >= 2) {
+    n_lanes = 2;
+    lane_budget = budget / 2;
+    make_plan(n, tight);
   }
-  if (tight) {   // the retry level runs with the global S_cap
-    const int64_t Br = std::max<int64_t>(1, (int64_t)(budget / ((size_t)(cap + 1) * step_bytes)));
-    const int64_t rr = std::min<int64_t>(Br, std::max<int64_t>(n / 8, 1));   // more than n/8 retries never happen; the buffer grows if they do
-    need_path = std::max(need_path, (size_t)rr * (size_t)(cap + 1) * rec_bytes);
-    need_ops = std::max(need_ops, (size_t)((rr + 31) / 32 * 32) * (size_t)(cap + 1) * OP_DOUBLES * sizeof(double));
-  }
-  if ((rc = ensure_path(c, need_path)) != IPOLE_OK) return rc;
-  if (split && (rc = ensure_ops(c, need_ops)) != IPOLE_OK) return rc;
+  c->stats.n_lanes = n_lanes;
+  size_t lane_path = 0, lane_ops = 0;     // bytes per lane
+  auto prepare = [&](bool with_retry_level) -> int {
+    size_t np = 0, no = 0;
+    for (const Batch& b : plan) {
+      np = std::max(np, (size_t)b.cnt * (size_t)(b.cap + 1) * rec_bytes);
+      no = std::max(no, (size_t)((b.cnt + 31) / 32 * 32) * (size_t)(b.cap + 1) * OP_DOUBLES * sizeof(double));
+    }
+    if (with_retry_level) {   // the retry level runs with the global S_cap
+      const int64_t Br = std::max<int64_t>(1, (int64_t)(lane_budget / ((size_t)(cap + 1) * step_bytes)));
+      const int64_t rr = std::min<int64_t>(Br, std::max<int64_t>(n / 8, 1));   // more than n/8 retries never happen; the buffer grows if they do
+      np = std::max(np, (size_t)rr * (size_t)(cap + 1) * rec_bytes);
+      no = std::max(no, (size_t)((rr + 31) / 32 * 32) * (size_t)(cap + 1) * OP_DOUBLES * sizeof(double));
+    }
+    lane_path = std::max(lane_path, (np + 255) & ~(size_t)255);
+    lane_ops = std::max(lane_ops, (no + 255) & ~(size_t)255);
+    int rcp;
+    if ((rcp = ensure_path(c, lane_path * n_lanes)) != IPOLE_OK) return rcp;
+    if (split && (rcp = ensure_ops(c, lane_ops * n_lanes)) != IPOLE_OK) return rcp;
+    return IPOLE_OK;
+  };
+  if ((rc = prepare(tight)) != IPOLE_OK) return rc;
   int n_long = 0;
   int* retry_count = c->d_small + 5;
   // with few batches the long-ray passes cannot wait for kernel boundaries: keep 8 block slots free for them
   const int reserve = (cap < max_steps && plan.size() <= 16) ? 8 : 0;
-  auto run_batch = [&](const Batch& b, const int32_t* ord) -> int {
+  auto run_batch = [&](const Batch& b, const int32_t* ord, int lane) -> int {
     if (qi + 4 > N_QUEUES) return IPOLE_EINVAL;
+    cudaStream_t st = lane ? c->lane2 : c->stream;
+    double* path = c->d_path + (size_t)lane * (lane_path / sizeof(double));
+    double* ops = split ? c->d_ops + (size_t)lane * (lane_ops / sizeof(double)) : nullptr;
     const bool top = b.cap >= cap;             // overflow means "longer than S_cap": the long-ray pass
     GeoArgs g = geo_args(c);
     g.cap = b.cap; g.base = b.base; g.count = b.cnt; g.order = ord; g.pixels = d_pixels;
-    g.path = c->d_path; g.nsteps = c->d_nsteps; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
+    g.path = path; g.nsteps = c->d_nsteps; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
     if (top) { g.long_list = c->d_long; g.long_count = c->d_small; }
     else { g.long_list = c->d_retry; g.long_count = retry_count; }
     if (use_occ) { g.grid = (const GridParams*)c->d_model; g.srange = c->d_srange; }
     int rcb;
-    if ((rcb = launch_geodesic(c, g, LK_GEO, b.cnt, c->stream, reserve)) != IPOLE_OK) return rcb;
+    if ((rcb = launch_geodesic(c, g, LK_GEO, b.cnt, st, reserve)) != IPOLE_OK) return rcb;
     if (top && cap < max_steps && !edf) {
-      CK(cudaEventRecord(c->ev_geo, c->stream));
+      CK(cudaEventRecord(c->ev_geo, st));
       CK(cudaStreamWaitEvent(c->side, c->ev_geo, 0));
     }
     RtArgs t;
     std::memset(&t, 0, sizeof t);
     t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = b.cap; t.base = b.base; t.count = b.cnt; t.order = ord;
-    t.path = c->d_path; t.nsteps = c->d_nsteps; t.queue = c->d_queues + qi;
+    t.path = path; t.nsteps = c->d_nsteps; t.queue = c->d_queues + qi;
     qi += split ? 3 : 1;
     if (use_occ) t.srange = c->d_srange;
     t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
-    if (split) rcb = launch_transfer_split(c, t, b.cnt, c->stream, reserve);
-    else rcb = launch_transfer(c, t, LK_RT, b.cnt, c->stream, reserve, 0, sw);
+    if (split) rcb = launch_transfer_split(c, t, b.cnt, st, reserve, ops, lane);
+    else rcb = launch_transfer(c, t, LK_RT, b.cnt, st, reserve, 0, sw);
     if (rcb != IPOLE_OK) return rcb;
     c->stats.n_batches++;
     if (top && cap < max_steps && !edf) {   // the transfer kernel just queued keeps the GPU busy while the host waits here
@@ -676,9 +705,24 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     }
     return IPOLE_OK;
   };
+  // the batches of `plan`, alternating between the lanes; the main stream continues when both are done
+  auto run_plan = [&](const int32_t* ord) -> int {
+    const bool two = n_lanes == 2 && plan.size() >= 2;
+    if (two) {
+      CK(cudaEventRecord(c->ev_fork, c->stream));
+      CK(cudaStreamWaitEvent(c->lane2, c->ev_fork, 0));
+    }
+    int k = 0, rcp;
+    for (const Batch& b : plan)
+      if ((rcp = run_batch(b, ord, two ? (k++ & 1) : 0)) != IPOLE_OK) return rcp;
+    if (two) {
+      CK(cudaEventRecord(c->ev_join, c->lane2));
+      CK(cudaStreamWaitEvent(c->stream, c->ev_join, 0));
+    }
+    return IPOLE_OK;
+  };
   CK(cudaMemsetAsync(retry_count, 0, sizeof(int), c->stream));
-  for (const Batch& b : plan)
-    if ((rc = run_batch(b, order)) != IPOLE_OK) return rc;
+  if ((rc = run_plan(order)) != IPOLE_OK) return rc;
   if (tight) {
     // second level: the rays that outgrew their batch's slots, with the global S_cap
     int n_retry = 0;
@@ -687,15 +731,8 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     c->stats.n_retry = n_retry;
     if (n_retry > 0) {
       make_plan(n_retry, false);
-      size_t np2 = 0, no2 = 0;
-      for (const Batch& b : plan) {
-        np2 = std::max(np2, (size_t)b.cnt * (size_t)(b.cap + 1) * rec_bytes);
-        no2 = std::max(no2, (size_t)((b.cnt + 31) / 32 * 32) * (size_t)(b.cap + 1) * OP_DOUBLES * sizeof(double));
-      }
-      if ((rc = ensure_path(c, np2)) != IPOLE_OK) return rc;
-      if (split && (rc = ensure_ops(c, no2)) != IPOLE_OK) return rc;
-      for (const Batch& b : plan)
-        if ((rc = run_batch(b, c->d_retry)) != IPOLE_OK) return rc;
+      if ((rc = prepare(false)) != IPOLE_OK) return rc;
+      if ((rc = run_plan(c->d_retry)) != IPOLE_OK) return rc;
     }
   }
   if (edf && cap < max_steps) {
@@ -706,15 +743,8 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
       const int cap_saved = cap;
       cap = max_steps;
       make_plan(n_long, false);
-      size_t np3 = 0, no3 = 0;
-      for (const Batch& b : plan) {
-        np3 = std::max(np3, (size_t)b.cnt * (size_t)(b.cap + 1) * rec_bytes);
-        no3 = std::max(no3, (size_t)((b.cnt + 31) / 32 * 32) * (size_t)(b.cap + 1) * OP_DOUBLES * sizeof(double));
-      }
-      if ((rc = ensure_path(c, np3)) != IPOLE_OK) return rc;
-      if ((rc = ensure_ops(c, no3)) != IPOLE_OK) return rc;
-      for (const Batch& b : plan)
-        if ((rc = run_batch(b, c->d_long)) != IPOLE_OK) return rc;
+      if ((rc = prepare(false)) != IPOLE_OK) return rc;
+      if ((rc = run_plan(c->d_long)) != IPOLE_OK) return rc;
       cap = cap_saved;
     }
     c->stats.n_long = n_long;
@@ -767,6 +797,9 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
     if (cudaStreamCreateWithFlags(&c->qstream, cudaStreamNonBlocking) != cudaSuccess) return fail(IPOLE_ECUDA);
     if (cudaEventCreateWithFlags(&c->ev_geo, cudaEventDisableTiming) != cudaSuccess) return fail(IPOLE_ECUDA);
     if (cudaEventCreateWithFlags(&c->ev_side, cudaEventDisableTiming) != cudaSuccess) return fail(IPOLE_ECUDA);
+    if (cudaStreamCreateWithFlags(&c->lane2, cudaStreamNonBlocking) != cudaSuccess) return fail(IPOLE_ECUDA);
+    if (cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess) return fail(IPOLE_ECUDA);
+    if (cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) return fail(IPOLE_ECUDA);
   }
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo, k_geodesic<false>, IPOLE_GEO_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo_occ, k_geodesic<true>, IPOLE_GEO_THREADS, 0);
@@ -801,6 +834,7 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   { const char* e = std::getenv("IPOLE_NO_SPLIT"); if (e && e[0] == '1') c->opt_split = 0; }
   { const char* e = std::getenv("IPOLE_NO_TIGHT"); if (e && e[0] == '1') c->opt_tight = 0; }
   { const char* e = std::getenv("IPOLE_NO_GROUP"); if (e && e[0] == '1') c->opt_group = 0; }
+  { const char* e = std::getenv("IPOLE_NO_OVERLAP"); if (e && e[0] == '1') c->opt_overlap = 0; }
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_group, k_transfer_group<MODEL_GRID>, IPOLE_RT_THREADS, 0);
   rc = apply_camera(c, cam);
   if (rc != IPOLE_OK) return fail(rc);
@@ -881,6 +915,12 @@ int ipole_set_geodesic_fp32(ipole_ctx* c, int32_t on) {
 int ipole_set_transfer_split(ipole_ctx* c, int32_t on) {
   if (!c) return IPOLE_EINVAL;
   c->opt_split = (on == 2) ? 2 : (on ? 1 : 0);
+  return IPOLE_OK;
+}
+
+int ipole_set_batch_overlap(ipole_ctx* c, int32_t on) {
+  if (!c) return IPOLE_EINVAL;
+  c->opt_overlap = on ? 1 : 0;
   return IPOLE_OK;
 }
 
@@ -1473,6 +1513,9 @@ void ipole_free(ipole_ctx* c) {
   if (c->qstream) cudaStreamDestroy(c->qstream);
   if (c->ev_geo) cudaEventDestroy(c->ev_geo);
   if (c->ev_side) cudaEventDestroy(c->ev_side);
+  if (c->lane2) cudaStreamDestroy(c->lane2);
+  if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+  if (c->ev_join) cudaEventDestroy(c->ev_join);
   cudaFree(c->d_path_long); cudaFree(c->d_nsteps_long); cudaFree(c->d_occ);
   cudaFree(c->d_cam); cudaFree(c->d_model); cudaFree(c->d_grid); cudaFree(c->d_path);
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long);

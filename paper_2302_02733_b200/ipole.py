@@ -17,7 +17,7 @@ _LIB = None
 OK, EINVAL, ENOMODEL, ENOMEM, ECUDA, ENOIMAGE = 0, -1, -2, -3, -4, -5
 
 #: every symbol include/ipole.h declares (checked by tests/test_abi.py)
-SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_options", "ipole_set_path_free", "ipole_set_edf", "ipole_set_geodesic_fp32", "ipole_set_transfer_split", "ipole_set_unpolarized", "ipole_load_model_adaf",
+SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_options", "ipole_set_path_free", "ipole_set_edf", "ipole_set_geodesic_fp32", "ipole_set_transfer_split", "ipole_set_batch_overlap", "ipole_set_unpolarized", "ipole_load_model_adaf",
            "ipole_load_model_slab", "ipole_load_model_grid", "ipole_make_image", "ipole_make_pixels", "ipole_make_images_adaf", "ipole_make_images_grid", "ipole_make_images_cameras", "ipole_make_image_adaptive",
            "ipole_get_ray_info", "ipole_get_stats", "ipole_get_camera_tetrad", "ipole_trace_pixel",
            "ipole_eval_connection", "ipole_eval_coefficients", "ipole_eval_coefficients_edf", "ipole_eval_stokes_step", "ipole_eval_bessel",
@@ -53,7 +53,8 @@ class Stats(C.Structure):
                 ("max_steps_seen", C.c_int32), ("path_cap", C.c_int32), ("n_ring", C.c_int64),
                 ("n_maxstep", C.c_int64), ("n_long", C.c_int64), ("n_batches", C.c_int32), ("n_launches", C.c_int32),
                 ("ms_probe", C.c_float), ("ms_geodesic", C.c_float), ("ms_transfer", C.c_float), ("ms_total", C.c_float),
-                ("ms_long", C.c_float), ("total_steps_forward", C.c_int64), ("ms_stepop", C.c_float), ("ms_apply", C.c_float), ("n_retry", C.c_int64)]
+                ("ms_long", C.c_float), ("total_steps_forward", C.c_int64), ("ms_stepop", C.c_float), ("ms_apply", C.c_float), ("n_retry", C.c_int64),
+                ("n_lanes", C.c_int32), ("reserved_", C.c_int32)]
 
 
 class Edf(C.Structure):
@@ -91,6 +92,7 @@ def lib():
         L.ipole_set_path_free.argtypes = [vp, C.c_int32]
         L.ipole_set_unpolarized.argtypes = [vp, C.c_int32]
         L.ipole_set_transfer_split.argtypes = [vp, C.c_int32]
+        L.ipole_set_batch_overlap.argtypes = [vp, C.c_int32]
         L.ipole_set_geodesic_fp32.argtypes = [vp, C.c_int32]
         L.ipole_set_edf.argtypes = [vp, C.POINTER(Edf)]
         L.ipole_eval_coefficients_edf.argtypes = [vp, C.c_int64, dp, dp]
@@ -193,6 +195,10 @@ class Ipole:
     def set_geodesic_fp32(self, on=True):
         """FP32 study switch (include/ipole.h ipole_set_geodesic_fp32): geodesics in single precision."""
         _chk(lib().ipole_set_geodesic_fp32(self._h, 1 if on else 0), "ipole_set_geodesic_fp32")
+
+    def set_batch_overlap(self, on=True):
+        """Consecutive batches side by side on two streams (include/ipole.h ipole_set_batch_overlap)."""
+        _chk(lib().ipole_set_batch_overlap(self._h, int(on)), "ipole_set_batch_overlap")
 
     def set_transfer_split(self, on=True):
         """Transfer as a step-parallel operator pass + a per-ray apply pass (include/ipole.h ipole_set_transfer_split)."""
