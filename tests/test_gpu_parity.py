@@ -172,7 +172,13 @@ def test_batching_sorting_and_long_ray_pass_are_bit_neutral(ipole):
     # tiny path buffer: many batches; S_cap from the probe
     g.set_options(24 << 20, 2)
     b = to_np(g.make_image(maps=True)); st2 = g.stats()
-    assert st2["n_batches"] > 3
+    assert st2["n_batches"] > 3 and st2["n_lanes"] == 2      # batches alternate between two streams by default
+    g.set_batch_overlap(False)
+    b1 = to_np(g.make_image(maps=True)); st2b = g.stats()
+    assert st2b["n_batches"] > 1 and st2b["n_lanes"] == 1
+    g.set_batch_overlap(True)
+    for k in b:
+        assert np.array_equal(b[k], b1[k]), k
     # no probe and a slot far too small for any ray: every ray goes through the long-ray pass
     g.set_options(40 << 20, 0)
     c = to_np(g.make_image(maps=True)); st3 = g.stats()
@@ -201,9 +207,15 @@ def test_split_transfer_matches_the_single_kernel(ipole):
     # many batches with slots sized from the predicted step counts; some rays outgrow them and are retried
     g.set_options(48 << 20, 2)
     three = to_np(g.make_image(maps=True)); st3 = g.stats()
-    assert st3["n_batches"] > 3
+    assert st3["n_batches"] > 3 and st3["n_lanes"] == 2
     for k in two:
         assert np.array_equal(two[k], three[k]), k
+    g.set_batch_overlap(False)          # the same batches one after the other on one stream
+    three1 = to_np(g.make_image(maps=True))
+    assert g.stats()["n_lanes"] == 1
+    g.set_batch_overlap(True)
+    for k in two:
+        assert np.array_equal(two[k], three1[k]), k
     g.set_options(0, 1)
     g.set_transfer_split(2)
     four = to_np(g.make_image(maps=True))
