@@ -759,6 +759,54 @@ def summarize_ncu(args):
         print()
 
 
+LAUNCH_METRICS = ("gpu__time_duration.sum,dram__bytes_read.sum,dram__bytes_write.sum,"
+                  "smsp__sass_thread_inst_executed_op_dfma_pred_on.sum,smsp__sass_thread_inst_executed_op_dadd_pred_on.sum,"
+                  "smsp__sass_thread_inst_executed_op_dmul_pred_on.sum,sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active,"
+                  "smsp__thread_inst_executed_per_inst_executed.ratio")
+
+
+def summarize_launches(args):
+    """--summarize-launches CSV: totals per kernel over EVERY launch of a run, from the log of
+    `ncu --metrics LAUNCH_METRICS --clock-control none --csv --log-file CSV python bench.py ...` (no GPU needed).
+    Steps of the run = DRAM bytes written by the k_geodesic launches / 64 (one path record per step; the probe launches
+    write none), so "per step" is an average over all steps of all images of the run, whatever a kernel does with them."""
+    import csv
+    import collections
+    import re
+    rows = [r for r in csv.reader(l for l in open(args.summarize_launches) if l.startswith('"'))]
+    hdr = rows[0]
+    ix = {h: i for i, h in enumerate(hdr)}
+    mult = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0, "s": 1e3, "ms": 1.0, "us": 1e-3, "ns": 1e-6, "msecond": 1.0,
+            "usecond": 1e-3, "nsecond": 1e-6, "second": 1e3}
+    launches = collections.OrderedDict()
+    for r in rows[1:]:
+        key = r[ix["ID"]]
+        d = launches.setdefault(key, {"name": re.sub(r"\(.*", "", r[ix["Kernel Name"]])})
+        v = float(r[ix["Metric Value"]].replace(",", ""))
+        d[r[ix["Metric Name"]]] = v * mult.get(r[ix["Metric Unit"]], 1.0)
+    tot = collections.OrderedDict()
+    for d in launches.values():
+        t = tot.setdefault(d["name"], collections.Counter())
+        ms = d.get("gpu__time_duration.sum", 0.0)
+        t["launches"] += 1
+        t["ms"] += ms
+        t["read"] += d.get("dram__bytes_read.sum", 0.0)
+        t["write"] += d.get("dram__bytes_write.sum", 0.0)
+        for k in ("dfma", "dadd", "dmul"):
+            t[k] += d.get("smsp__sass_thread_inst_executed_op_%s_pred_on.sum" % k, 0.0)
+        t["pipe_ms"] += d.get("sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active", 0.0) * ms
+        t["lanes_ms"] += d.get("smsp__thread_inst_executed_per_inst_executed.ratio", 0.0) * ms
+    steps = max(1.0, sum(t["write"] for n, t in tot.items() if "k_geodesic" in n) / 64.0)   # (1: a log without the byte counters)
+    all_ms = sum(t["ms"] for t in tot.values())
+    print("steps of the run (bytes written by k_geodesic / 64): %.4e; kernel time under ncu %.1f ms" % (steps, all_ms))
+    print("%-34s %8s %10s %7s %10s %10s %8s %7s %9s %9s" % ("kernel", "launches", "ms (ncu)", "share", "flop/step", "FP64/step", "pipe %", "lanes", "B rd/step", "B wr/step"))
+    for n, t in tot.items():
+        flop = 2 * t["dfma"] + t["dadd"] + t["dmul"]
+        print("%-34s %8d %10.2f %6.1f%% %10.1f %10.1f %8.1f %7.2f %9.1f %9.1f"
+              % (n[-34:], t["launches"], t["ms"], 100 * t["ms"] / all_ms, flop / steps, (t["dfma"] + t["dadd"] + t["dmul"]) / steps,
+                 t["pipe_ms"] / max(t["ms"], 1e-9), t["lanes_ms"] / max(t["ms"], 1e-9), t["read"] / steps, t["write"] / steps))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -785,12 +833,15 @@ def main():
     ap.add_argument("--path-free", action="store_true",
                     help="the paper's own GPU design (PAPER.md:43): no stored path, forward re-integration")
     ap.add_argument("--summarize-ncu", metavar="REPORT", help="print the text summary of an .ncu-rep (profiles/*.txt); no GPU needed")
+    ap.add_argument("--summarize-launches", metavar="CSV", help="per-kernel totals of an ncu --metrics launch log (see summarize_launches); no GPU needed")
     ap.add_argument("--ncu-kernel", default=None, help="--summarize-ncu: only kernels whose name matches this regex")
     ap.add_argument("--ncu-steps-from", choices=["read", "write"], default=None)
     ap.add_argument("--ncu-bytes-per-step", type=float, default=64.0)
     args = ap.parse_args()
     if args.summarize_ncu:
         return summarize_ncu(args)
+    if args.summarize_launches:
+        return summarize_launches(args)
     if args.impl == "reference":
         return run_reference(args)
 

@@ -90,6 +90,11 @@ struct ipole_ctx {
   cudaStream_t lane2 = nullptr;
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   int opt_overlap = 1;
+  // retry level on the side stream: its own slots, so that it starts as soon as the last geodesic kernel of the bulk has
+  // listed the rays, beside the last transfer kernels, instead of after them (one ray of S_cap steps is ~30 ms of latency)
+  cudaEvent_t ev_lastgeo[2] = {nullptr, nullptr};
+  double* d_retry_buf = nullptr; size_t retry_buf_bytes = 0;
+  int opt_side_retry = 1;
   int64_t ray_cap = 0;           // capacity of the per-ray buffers below
   int32_t *d_nsteps = nullptr, *d_nturn = nullptr, *d_order = nullptr, *d_key = nullptr, *d_long = nullptr;
   int2* d_srange = nullptr;      // grid model: per ray, the steps that may cross plasma (k_geodesic<true>)
@@ -184,7 +189,7 @@ int ensure_rays(ipole_ctx* c, int64_t n) {
   CK(cudaMalloc(&c->d_long, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_nsteps_long, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_srange, n * sizeof(int2)));
-  CK(cudaMalloc(&c->d_irr, 2 * n * sizeof(int32_t)));   // one list per lane
+  CK(cudaMalloc(&c->d_irr, 3 * n * sizeof(int32_t)));   // one list per lane, one for the retry level on the side stream
   CK(cudaMalloc(&c->d_retry, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_out, 6 * n * sizeof(double)));
   c->ray_cap = n;
@@ -209,6 +214,15 @@ int ensure_ops(ipole_ctx* c, size_t bytes) {
   return IPOLE_OK;
 }
 
+int ensure_retry_buf(ipole_ctx* c, size_t bytes) {
+  if (bytes <= c->retry_buf_bytes) return IPOLE_OK;
+  cudaFree(c->d_retry_buf); c->d_retry_buf = nullptr; c->retry_buf_bytes = 0;
+  cudaError_t e = cudaMalloc(&c->d_retry_buf, bytes);
+  if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
+  c->retry_buf_bytes = bytes;
+  return IPOLE_OK;
+}
+
 int ensure_path_long(ipole_ctx* c, size_t bytes) {
   if (bytes <= c->path_long_bytes) return IPOLE_OK;
   cudaFree(c->d_path_long); c->d_path_long = nullptr; c->path_long_bytes = 0;
@@ -223,7 +237,7 @@ size_t path_budget(ipole_ctx* c) {
   if (const char* e = std::getenv("IPOLE_PATH_GIB")) { const double gib = std::atof(e); if (gib > 0.0) return (size_t)(gib * 1073741824.0); }
   size_t fr = 0, tot = 0;
   cudaMemGetInfo(&fr, &tot);
-  fr += c->path_bytes + c->path_long_bytes + c->ops_bytes;  // what we already hold counts as available
+  fr += c->path_bytes + c->path_long_bytes + c->ops_bytes + c->retry_buf_bytes;  // what we already hold counts as available
   size_t b = (size_t)(0.5 * (double)fr);
   const size_t cap = (size_t)96 << 30;
   return std::min(b, cap);
@@ -352,15 +366,18 @@ int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_
 // split transfer of one batch (stepop.cuh): k_stepop over the steps, k_apply over the rays, then k_transfer for the
 // rays k_stepop could not express (listed on the device; usually none)
 int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStream_t st, int reserve, double* ops, int lane) {
-  int* irr_count = c->d_small + (lane ? 6 : 4);
-  int32_t* irr = c->d_irr + (lane ? c->ray_cap : 0);
+  // lane 0 / 1: the bulk lanes; 2: the retry level on the side stream (its times count as ms_long)
+  static const int irr_slot[3] = {4, 6, 3};
+  int* irr_count = c->d_small + irr_slot[lane];
+  int32_t* irr = c->d_irr + (size_t)lane * c->ray_cap;
+  const bool on_side = lane == 2;
   CK(cudaMemsetAsync(irr_count, 0, sizeof(int), st));
   OpArgs o;
   std::memset(&o, 0, sizeof o);
   o.cam = a.cam; o.units = a.units; o.model = a.model; o.cap = a.cap; o.base = a.base; o.count = a.count; o.order = a.order;
-  o.path = a.path; o.nsteps = a.nsteps; o.queue = a.queue; o.ops = ops; o.irr_slots = irr; o.irr_count = irr_count; o.test_irregular = (c->opt_split == 2);
+  o.count_dev = a.count_dev; o.path = a.path; o.nsteps = a.nsteps; o.queue = a.queue; o.ops = ops; o.irr_slots = irr; o.irr_count = irr_count; o.test_irregular = (c->opt_split == 2);
   {
-    const int s = span_begin(c, LK_OPS, st);
+    const int s = span_begin(c, on_side ? LK_LONG : LK_OPS, st);
     // one warp per ray at a time
     if (c->n_mc) {
       o.cams = c->d_mc_cams; o.units_arr = c->d_mc_units; o.rays_per_cam = c->mc_rays_per_cam;
@@ -377,11 +394,11 @@ int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStrea
   std::memset(&p, 0, sizeof p);
   p.nu3 = a.units.nu_obs * a.units.nu_obs * a.units.nu_obs;
   p.model = c->adaf_host;
-  p.cap = a.cap; p.base = a.base; p.count = a.count; p.order = a.order; p.ops = ops; p.nsteps = a.nsteps;
+  p.cap = a.cap; p.base = a.base; p.count = a.count; p.count_dev = a.count_dev; p.order = a.order; p.ops = ops; p.nsteps = a.nsteps;
   p.queue = a.queue + 1;
   p.I = a.I; p.Q = a.Q; p.U = a.U; p.V = a.V; p.tau = a.tau; p.tauF = a.tauF;
   {
-    const int s = span_begin(c, LK_APPLY, st);
+    const int s = span_begin(c, on_side ? LK_LONG : LK_APPLY, st);
     const int g = grid_for(c, c->occ_ap, IPOLE_AP_THREADS / 32, (rays + 31) / 32, reserve);   // one warp per 32 rays
     p.edf = c->edf;
     if (c->n_mc) { p.nu3_arr = c->d_mc_nu3; p.rays_per_cam = c->mc_rays_per_cam; }
@@ -394,7 +411,7 @@ int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStrea
   RtArgs t = a;
   t.queue = a.queue + 2; t.count_dev = irr_count; t.slots = irr;
   {
-    const int s = span_begin(c, LK_RT, st);
+    const int s = span_begin(c, on_side ? LK_LONG : LK_RT, st);
     k_transfer<MODEL_ADAF, 0><<<std::max(1, c->n_sm / 8), IPOLE_RT_THREADS, 0, st>>>(t);
     span_end(c, s, st);
     c->stats.n_launches++;
@@ -684,6 +701,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     if (use_occ) { g.grid = (const GridParams*)c->d_model; g.srange = c->d_srange; }
     int rcb;
     if ((rcb = launch_geodesic(c, g, LK_GEO, b.cnt, st, reserve)) != IPOLE_OK) return rcb;
+    CK(cudaEventRecord(c->ev_lastgeo[lane], st));
     if (top && cap < max_steps && !edf) {
       CK(cudaEventRecord(c->ev_geo, st));
       CK(cudaStreamWaitEvent(c->side, c->ev_geo, 0));
@@ -722,21 +740,72 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     return IPOLE_OK;
   };
   CK(cudaMemsetAsync(retry_count, 0, sizeof(int), c->stream));
+  // ---- second level on the side stream: slots of its own for up to R_max retried rays, sized before their number is
+  // known (the kernels read the count on the device), so that the pass starts when the LAST geodesic kernel of the bulk
+  // has finished and runs beside the last transfer kernels.  What does not fit (never seen) takes the lanes afterwards.
+  int64_t R_max = 0;
+  if (tight && !sw && c->opt_side_retry && plan.size() >= 2) {
+    const size_t slot = (size_t)(cap + 1) * step_bytes;
+    R_max = std::max<int64_t>(256, n / 512);
+    R_max = std::min<int64_t>(R_max, (int64_t)(std::min<size_t>(budget / 8, (size_t)8 << 30) / slot)) & ~(int64_t)31;
+    if (R_max >= 32 && ensure_retry_buf(c, (size_t)R_max * slot) != IPOLE_OK) R_max = 0;
+    if (R_max < 32) R_max = 0;
+  }
+  const int n_lanes_bulk = (n_lanes == 2 && plan.size() >= 2) ? 2 : 1;
   if ((rc = run_plan(order)) != IPOLE_OK) return rc;
+  bool side_used = false;
+  if (R_max > 0) {
+    if (qi + 4 > N_QUEUES) return IPOLE_EINVAL;
+    for (int l = 0; l < n_lanes_bulk; ++l) CK(cudaStreamWaitEvent(c->side, c->ev_lastgeo[l], 0));
+    int* rcount = c->d_small + 7;
+    k_clamp_count<<<1, 1, 0, c->side>>>(retry_count, (int)R_max, rcount);
+    c->stats.n_launches++;
+    double* rpath = c->d_retry_buf;
+    double* rops = split ? c->d_retry_buf + (size_t)R_max * (size_t)(cap + 1) * REC_DOUBLES : nullptr;
+    GeoArgs g = geo_args(c);
+    g.cap = cap; g.base = 0; g.count = R_max; g.count_dev = rcount; g.order = c->d_retry; g.pixels = d_pixels;
+    g.path = rpath; g.nsteps = c->d_nsteps_long; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
+    g.long_list = c->d_long; g.long_count = c->d_small;
+    if (use_occ) { g.grid = (const GridParams*)c->d_model; g.srange = c->d_srange; }
+    if ((rc = launch_geodesic(c, g, LK_LONG, R_max, c->side)) != IPOLE_OK) return rc;
+    CK(cudaEventRecord(c->ev_geo, c->side));
+    RtArgs t;
+    std::memset(&t, 0, sizeof t);
+    t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = cap; t.base = 0; t.count = R_max; t.count_dev = rcount;
+    t.order = c->d_retry; t.path = rpath; t.nsteps = c->d_nsteps_long; t.queue = c->d_queues + qi;
+    qi += split ? 3 : 1;
+    if (use_occ) t.srange = c->d_srange;
+    t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
+    if (split) rc = launch_transfer_split(c, t, R_max, c->side, 0, rops, 2);
+    else rc = launch_transfer(c, t, LK_LONG, R_max, c->side, 0, 0, nullptr);
+    if (rc != IPOLE_OK) return rc;
+    side_used = true;
+  }
+  int n_retry_side = 0;
   if (tight) {
-    // second level: the rays that outgrew their batch's slots, with the global S_cap
     int n_retry = 0;
     CK(cudaMemcpyAsync(&n_retry, retry_count, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     c->stats.n_retry = n_retry;
-    if (n_retry > 0) {
-      make_plan(n_retry, false);
+    n_retry_side = (int)std::min<int64_t>(n_retry, R_max);
+    if (n_retry_side > 0 && cap < max_steps && !edf) {
+      // retried rays that outgrow S_cap as well: listed by the geodesic kernel above, long-ray pass
+      if ((rc = listed(c->ev_geo, n_long)) != IPOLE_OK) return rc;
+      if ((rc = long_pass(n_long)) != IPOLE_OK) return rc;
+    }
+    if (n_retry > n_retry_side) {
+      // the rest of the second level on the lanes, with the global S_cap
+      make_plan(n_retry - n_retry_side, false);
       if ((rc = prepare(false)) != IPOLE_OK) return rc;
-      if ((rc = run_plan(c->d_retry)) != IPOLE_OK) return rc;
+      if ((rc = run_plan(c->d_retry + n_retry_side)) != IPOLE_OK) return rc;
     }
   }
   if (edf && cap < max_steps) {
     // third level: rays longer than S_cap, through the same split kernels with slots of max_steps
+    if (side_used) {   // the list is complete once the geodesic kernel of the side-stream retry has run
+      CK(cudaEventRecord(c->ev_side, c->side));
+      CK(cudaStreamWaitEvent(c->stream, c->ev_side, 0));
+    }
     CK(cudaMemcpyAsync(&n_long, c->d_small, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     if (n_long > 0) {
@@ -750,13 +819,19 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     c->stats.n_long = n_long;
     n_long = 0;   // nothing ran on the side stream
   } else c->stats.n_long = n_long;
-  if (n_long > 0) {
-    // join the side stream, then publish the step counts of the long rays (the bulk transfer kernels read
-    // nsteps[q] = -1 for them, so the long passes keep theirs apart until every bulk kernel is done)
+  if (n_long > 0 || side_used) {
+    // join the side stream, then publish the step counts of the long and the retried rays (the bulk transfer kernels
+    // read nsteps[q] = -1 for them, so the side-stream passes keep theirs apart until every bulk kernel is done)
     CK(cudaEventRecord(c->ev_side, c->side));
     CK(cudaStreamWaitEvent(c->stream, c->ev_side, 0));
-    k_merge_long<<<(n_long + 255) / 256, 256, 0, c->stream>>>(n_long, c->d_long, c->d_nsteps_long, c->d_nsteps);
-    c->stats.n_launches++;
+    if (n_long > 0) {
+      k_merge_long<<<(n_long + 255) / 256, 256, 0, c->stream>>>(n_long, c->d_long, c->d_nsteps_long, c->d_nsteps);
+      c->stats.n_launches++;
+    }
+    if (n_retry_side > 0) {
+      k_merge_long<<<(n_retry_side + 255) / 256, 256, 0, c->stream>>>(n_retry_side, c->d_retry, c->d_nsteps_long, c->d_nsteps);
+      c->stats.n_launches++;
+    }
     CK(cudaGetLastError());
   }
 
@@ -800,6 +875,8 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
     if (cudaStreamCreateWithFlags(&c->lane2, cudaStreamNonBlocking) != cudaSuccess) return fail(IPOLE_ECUDA);
     if (cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess) return fail(IPOLE_ECUDA);
     if (cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) return fail(IPOLE_ECUDA);
+    for (int l = 0; l < 2; ++l)
+      if (cudaEventCreateWithFlags(&c->ev_lastgeo[l], cudaEventDisableTiming) != cudaSuccess) return fail(IPOLE_ECUDA);
   }
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo, k_geodesic<false>, IPOLE_GEO_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo_occ, k_geodesic<true>, IPOLE_GEO_THREADS, 0);
@@ -835,6 +912,7 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   { const char* e = std::getenv("IPOLE_NO_TIGHT"); if (e && e[0] == '1') c->opt_tight = 0; }
   { const char* e = std::getenv("IPOLE_NO_GROUP"); if (e && e[0] == '1') c->opt_group = 0; }
   { const char* e = std::getenv("IPOLE_NO_OVERLAP"); if (e && e[0] == '1') c->opt_overlap = 0; }
+  { const char* e = std::getenv("IPOLE_NO_SIDE_RETRY"); if (e && e[0] == '1') c->opt_side_retry = 0; }
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_group, k_transfer_group<MODEL_GRID>, IPOLE_RT_THREADS, 0);
   rc = apply_camera(c, cam);
   if (rc != IPOLE_OK) return fail(rc);
@@ -1516,6 +1594,8 @@ void ipole_free(ipole_ctx* c) {
   if (c->lane2) cudaStreamDestroy(c->lane2);
   if (c->ev_fork) cudaEventDestroy(c->ev_fork);
   if (c->ev_join) cudaEventDestroy(c->ev_join);
+  for (int l = 0; l < 2; ++l) if (c->ev_lastgeo[l]) cudaEventDestroy(c->ev_lastgeo[l]);
+  cudaFree(c->d_retry_buf);
   cudaFree(c->d_path_long); cudaFree(c->d_nsteps_long); cudaFree(c->d_occ);
   cudaFree(c->d_cam); cudaFree(c->d_model); cudaFree(c->d_grid); cudaFree(c->d_path);
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long);

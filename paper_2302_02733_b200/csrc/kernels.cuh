@@ -539,7 +539,8 @@ __global__ void __launch_bounds__(IPOLE_RT_THREADS, IPOLE_RT_MINB) k_transfer_gr
   __syncthreads();
   const void* model = model_smem;
   const int lane = threadIdx.x & 31;
-  const int64_t n_groups = (A.count + 31) >> 5;
+  const int64_t count = A.count_dev ? (int64_t)*A.count_dev : A.count;
+  const int64_t n_groups = (count + 31) >> 5;
 
   for (;;) {
     __syncwarp();
@@ -554,7 +555,7 @@ __global__ void __launch_bounds__(IPOLE_RT_THREADS, IPOLE_RT_MINB) k_transfer_gr
     int32_t q = 0;
     int s0 = -1, s_lo = 0;       // this lane walks steps s0 ... 0; -1: nothing to walk
     bool lit = false;
-    if (li < A.count) {
+    if (li < count) {
       q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
       int n = A.nsteps[q];
       if (n >= 0) {              // (n < 0: overflowed its slot, done by the long-ray pass)
@@ -929,10 +930,13 @@ __global__ void __launch_bounds__(256) k_reduce_cams(int64_t n, size_t stride, c
   }
 }
 
+// out = min(*in, limit): the ray count of a pass sized before the count is known (retry level on the side stream)
+__global__ void k_clamp_count(const int* in, int limit, int* out) { *out = min(*in, limit); }
+
 // step counts of the long-ray passes -> nsteps (after every bulk kernel has finished)
 __global__ void k_merge_long(int n_long, const int32_t* long_list, const int32_t* nsteps_long, int32_t* nsteps) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n_long) { const int32_t q = long_list[i]; nsteps[q] = nsteps_long[q]; }
+  if (i < n_long) { const int32_t q = long_list[i]; const int32_t v = nsteps_long[q]; if (v >= 0) nsteps[q] = v; }
 }
 
 // sum of the forward-step counts of the path-free variant (integer: order-independent)

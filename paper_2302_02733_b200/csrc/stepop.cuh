@@ -43,6 +43,7 @@ struct OpArgs {
   const void* model;          // device pointer to AdafParams
   int cap;                    // steps per slot (records = cap + 1) of both the path and the operator buffer
   int64_t base, count;        // rays [base, base+count) of the order
+  const int* count_dev;       // if non-null, count = *count_dev (retry level on the side stream)
   const int32_t* order;
   const double* path;         // [count][cap+1][8]
   const int32_t* nsteps;      // indexed by q; -1 = overflowed its slot (long-ray pass)
@@ -74,6 +75,7 @@ __global__ void __launch_bounds__(IPOLE_OP_THREADS, IPOLE_OP_MINB) k_stepop(cons
   for (int i = threadIdx.x; i < (int)sizeof(AdafParams); i += blockDim.x) model_smem[i] = ((const unsigned char*)A.model)[i];
   __syncthreads();
   const int lane = threadIdx.x & 31;
+  const int64_t count = A.count_dev ? (int64_t)*A.count_dev : A.count;
   const size_t slot_rec = (size_t)(A.cap + 1) * REC_DOUBLES;
   // MC: the ray's own camera (geometry, transverse legs) and units, and the flow's ISCO for that spin, in registers
   AdafParams model_l = *(const AdafParams*)model_smem;
@@ -89,7 +91,7 @@ __global__ void __launch_bounds__(IPOLE_OP_THREADS, IPOLE_OP_MINB) k_stepop(cons
     long long li = 0;
     if (lane == 0) li = (long long)atomicAdd(A.queue, 1ULL);
     li = __shfl_sync(0xffffffffu, li, 0);
-    if (li >= A.count) break;
+    if (li >= count) break;
     const int32_t q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
     const int n = A.nsteps[q];
     if (n < 0) continue;                     // overflowed its slot: done by the long-ray pass
@@ -182,6 +184,7 @@ struct ApArgs {
   double nu3;                 // nu_obs^3: invariant I/nu^3 -> specific intensity at the camera
   int cap;
   int64_t base, count;
+  const int* count_dev;       // if non-null, count = *count_dev
   const int32_t* order;
   const double* ops;
   const int32_t* nsteps;
@@ -224,7 +227,8 @@ __global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? IPOLE_AP_EDF_MINB : IP
   }
   const double4* edf_nodes = edf_nodes_smem;
   const int lane = threadIdx.x & 31;
-  const int64_t n_groups = (A.count + 31) >> 5;
+  const int64_t count = A.count_dev ? (int64_t)*A.count_dev : A.count;
+  const int64_t n_groups = (count + 31) >> 5;
   for (;;) {
     __syncwarp();
     long long g = 0;
@@ -235,7 +239,7 @@ __global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? IPOLE_AP_EDF_MINB : IP
     int32_t q = 0;
     int n = 0;                                   // steps of this lane's ray; 0: nothing to do
     double mc[4] = {0, 0, 0, 0};
-    if (li < A.count) {
+    if (li < count) {
       q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
       n = A.nsteps[q];
       if (n < 0) n = 0;                          // overflowed its slot: long-ray pass
