@@ -28,17 +28,18 @@ if ROOT not in sys.path:
 # the live CUDA-event time, so a faster kernel can only raise it; what the shipped kernels actually execute is reported
 # beside it (FLOP_EXECUTED, frac_executed).  Grid transfer: 786 per WALKED step = 390 averaged over all steps of a ray.
 FLOP_PER_STEP = {"transfer_adaf": 1576.0, "transfer_grid": 390.0, "geodesic_adaf": 994.0, "geodesic_grid": 1183.0}
-# executed by the kernels as shipped, per step, and their FP64-pipe utilisation, both from ncu --set full captures
-# (smsp__sass_thread_inst_executed_op_d{fma,add,mul}_pred_on / steps of the launch; sm__inst_executed_pipe_fp64):
-# profiles/r2_k_stepop_adaf1024.txt, r2_k_apply_adaf1024.txt, r1_k_transfer_*.txt, r1_k_geodesic_*.txt
-FLOP_EXECUTED = {"k_stepop": 1018.0, "k_apply": 574.0, "k_transfer<adaf>": 1576.0, "k_transfer<grid>": 390.0,
-                 "k_geodesic": 994.0, "k_geodesic<occ>": 1183.0}
-# second physics workload (--edf): k_apply<true> per step, 128 quadrature nodes (profiles/r2_k_apply_edf_adaf256.txt)
+# executed by the kernels as shipped, per step: smsp__sass_thread_inst_executed_op_d{fma,add,mul}_pred_on summed over EVERY
+# launch of a run / the steps of the run (profiles/r2_image_flops.md, made by --summarize-launches); and their FP64-pipe
+# utilisation (sm__inst_executed_pipe_fp64) in a bulk launch of the ncu --set full captures profiles/r2_k_*.txt.
+# k_transfer<adaf> (single kernel, --single-kernel) and the path-free / unpolarized variants: profiles/r1_k_*.txt.
+FLOP_EXECUTED = {"k_stepop": 1019.0, "k_apply": 578.0, "k_transfer<adaf>": 1576.0, "k_transfer_group<grid>": 397.0,
+                 "k_geodesic": 839.0, "k_geodesic<occ>": 1020.0}
+# second physics workload (--edf): k_apply<true> per step, 128 quadrature nodes (profiles/r2_k_apply_edf{1,2}_adaf256.txt)
 FLOP_EXECUTED.update({"k_apply<edf 1>": 11383.0, "k_apply<edf 2>": 18268.0})
-FP64_PIPE_PCT = {"k_stepop": 72.7, "k_apply": 64.8, "k_transfer<adaf>": 58.5, "k_transfer<grid>": 48.0,
-                 "k_geodesic": 82.0, "k_geodesic<occ>": 79.0, "k_apply<edf 1>": 55.9, "k_apply<edf 2>": 55.2}
+FP64_PIPE_PCT = {"k_stepop": 72.6, "k_apply": 61.7, "k_transfer<adaf>": 58.5, "k_transfer_group<grid>": 50.9,
+                 "k_geodesic": 82.5, "k_geodesic<occ>": 79.5, "k_apply<edf 1>": 55.9, "k_apply<edf 2>": 55.2}
 # DRAM bytes per step of k_transfer (dram__bytes_read + write of one launch / its thread-steps, same captures)
-DRAM_BYTES_PER_STEP = {"transfer_adaf": 64.2, "transfer_grid": 33.8}
+DRAM_BYTES_PER_STEP = {"transfer_adaf": 64.2, "transfer_grid": 37.2}
 DRAM_BYTES_PER_STEP_SPLIT = 192.0   # k_stepop reads 64.1 B and writes 64.0 B per step, k_apply reads 64.0 B (profiles/r2_k_*.txt)
 # --unpolarized: per step of k_transfer_unpol<model> (ncu, profiles/r1_unpolarized.md)
 FLOP_PER_STEP_UNPOL = {"transfer_adaf": 652.0, "transfer_grid": 76.4}   # grid: 601 per walked step, 12.7 % of the steps walked
@@ -572,7 +573,7 @@ def measure_image(args, name, ipole, replicas, W, world, rank, local, barrier):
     elif split:
         kname = "k_stepop<%s> + k_apply (split transfer)" % wl["kind"]
     else:
-        kname = "k_transfer<%s%s>" % (wl["kind"], ", path-free" if pf else "")
+        kname = "k_transfer_group<grid>" if (wl["kind"] == "grid" and not pf) else "k_transfer<%s%s>" % (wl["kind"], ", path-free" if pf else "")
     roof = {"bound": "alu", "kernel": kname, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
             "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz; DFMA micro-benchmark on this GPU: %.1f" % dfma_tf,
             "launches": n_rt * (2 if split else 1), "avg_launch_ms": rt_ms / n_rt, "kernel_share_of_step": rt_ms / st["ms_total"],
@@ -593,7 +594,7 @@ def measure_image(args, name, ipole, replicas, W, world, rank, local, barrier):
         elif split:
             parts = {"k_stepop": st["ms_stepop"], "k_apply": st["ms_apply"]}
         else:
-            parts = {"k_transfer<%s>" % wl["kind"]: rt_ms}
+            parts = {("k_transfer_group<grid>" if wl["kind"] == "grid" else "k_transfer<%s>" % wl["kind"]): rt_ms}
         roof["kernels"] = {k: {"ms": v, "flop_per_step_executed": FLOP_EXECUTED[k], "fp64_pipe_pct": FP64_PIPE_PCT[k],
                                "tflops_executed": FLOP_EXECUTED[k] * rt_steps / (v * 1e-3) / 1e12,
                                "frac_executed": FLOP_EXECUTED[k] * rt_steps / (v * 1e-3) / 1e12 / FP64_PEAK_TFLOPS}

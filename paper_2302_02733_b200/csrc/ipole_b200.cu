@@ -65,6 +65,8 @@ struct ipole_ctx {
   int opt_split = 1;             // stored path, analytic flow: transfer as k_stepop + k_apply (stepop.cuh)
   double* d_ops = nullptr; size_t ops_bytes = 0;   // operator records of one batch
   int32_t* d_irr = nullptr;      // slots of the rays k_stepop leaves to k_transfer
+  int32_t *d_rank_pos = nullptr, *d_rank_slot = nullptr;   // k_rank_window: operator-record places of a batch's slots, by position in the order
+  int opt_rank = 1;
   int occ_op = 0, occ_ap = 0, occ_ap_edf = 0;
   EdfDev edf = {0, 128, 3.5, 0.0, nullptr, nullptr};   // electron distribution of the coefficient step (ipole_set_edf); kind 0: thermal fits
   double4* d_edf_nodes = nullptr; double* d_edf_lnnorm = nullptr;
@@ -180,7 +182,7 @@ int apply_camera(ipole_ctx* c, const ipole_camera* k) {
 int ensure_rays(ipole_ctx* c, int64_t n) {
   if (n <= c->ray_cap) return IPOLE_OK;
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long); cudaFree(c->d_out);
-  cudaFree(c->d_nsteps_long); cudaFree(c->d_srange); c->d_srange = nullptr; cudaFree(c->d_irr); cudaFree(c->d_retry); c->d_retry = nullptr;
+  cudaFree(c->d_nsteps_long); cudaFree(c->d_srange); c->d_srange = nullptr; cudaFree(c->d_irr); cudaFree(c->d_retry); c->d_retry = nullptr; cudaFree(c->d_rank_pos); cudaFree(c->d_rank_slot); c->d_rank_pos = c->d_rank_slot = nullptr;
   c->d_nsteps = c->d_nturn = c->d_order = c->d_key = c->d_long = c->d_nsteps_long = c->d_irr = nullptr; c->d_out = nullptr; c->ray_cap = 0;
   CK(cudaMalloc(&c->d_nsteps, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_nturn, n * sizeof(int32_t)));
@@ -189,6 +191,8 @@ int ensure_rays(ipole_ctx* c, int64_t n) {
   CK(cudaMalloc(&c->d_long, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_nsteps_long, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_srange, n * sizeof(int2)));
+  CK(cudaMalloc(&c->d_rank_pos, 2 * n * sizeof(int32_t)));    // second half: the retry level on the side stream
+  CK(cudaMalloc(&c->d_rank_slot, 2 * n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_irr, 3 * n * sizeof(int32_t)));   // one list per lane, one for the retry level on the side stream
   CK(cudaMalloc(&c->d_retry, n * sizeof(int32_t)));
   CK(cudaMalloc(&c->d_out, 6 * n * sizeof(double)));
@@ -376,6 +380,18 @@ int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStrea
   std::memset(&o, 0, sizeof o);
   o.cam = a.cam; o.units = a.units; o.model = a.model; o.cap = a.cap; o.base = a.base; o.count = a.count; o.order = a.order;
   o.count_dev = a.count_dev; o.path = a.path; o.nsteps = a.nsteps; o.queue = a.queue; o.ops = ops; o.irr_slots = irr; o.irr_count = irr_count; o.test_irregular = (c->opt_split == 2);
+  const bool rank = c->opt_rank && rays > 32;
+  int32_t* rank_pos = c->d_rank_pos + (on_side ? c->ray_cap : 0);     // (the side-stream retry indexes from 0 like a bulk batch)
+  int32_t* rank_slot = c->d_rank_slot + (on_side ? c->ray_cap : 0);
+  if (rank) {
+    RankArgs r = {a.base, a.count, a.count_dev, a.order, a.nsteps, rank_pos, rank_slot};
+    const int s = span_begin(c, on_side ? LK_LONG : LK_OPS, st);
+    k_rank_window<<<(unsigned)((rays + RANK_WINDOW - 1) / RANK_WINDOW), RANK_WINDOW, 0, st>>>(r);
+    span_end(c, s, st);
+    c->stats.n_launches++;
+    CK(cudaGetLastError());
+    o.pos = rank_pos;
+  }
   {
     const int s = span_begin(c, on_side ? LK_LONG : LK_OPS, st);
     // one warp per ray at a time
@@ -396,6 +412,7 @@ int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStrea
   p.model = c->adaf_host;
   p.cap = a.cap; p.base = a.base; p.count = a.count; p.count_dev = a.count_dev; p.order = a.order; p.ops = ops; p.nsteps = a.nsteps;
   p.queue = a.queue + 1;
+  if (rank) p.slot = rank_slot;
   p.I = a.I; p.Q = a.Q; p.U = a.U; p.V = a.V; p.tau = a.tau; p.tauF = a.tauF;
   {
     const int s = span_begin(c, on_side ? LK_LONG : LK_APPLY, st);
@@ -912,6 +929,7 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   { const char* e = std::getenv("IPOLE_NO_TIGHT"); if (e && e[0] == '1') c->opt_tight = 0; }
   { const char* e = std::getenv("IPOLE_NO_GROUP"); if (e && e[0] == '1') c->opt_group = 0; }
   { const char* e = std::getenv("IPOLE_NO_OVERLAP"); if (e && e[0] == '1') c->opt_overlap = 0; }
+  { const char* e = std::getenv("IPOLE_NO_RANK"); if (e && e[0] == '1') c->opt_rank = 0; }
   { const char* e = std::getenv("IPOLE_NO_SIDE_RETRY"); if (e && e[0] == '1') c->opt_side_retry = 0; }
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_group, k_transfer_group<MODEL_GRID>, IPOLE_RT_THREADS, 0);
   rc = apply_camera(c, cam);
@@ -1601,7 +1619,7 @@ void ipole_free(ipole_ctx* c) {
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long);
   cudaFree(c->d_out); cudaFree(c->d_pixels); cudaFree(c->d_probe); cudaFree(c->d_queues); cudaFree(c->d_hist);
   cudaFree(c->d_small); cudaFree(c->d_part); cudaFree(c->d_red); cudaFree(c->d_endp); cudaFree(c->d_sum); cudaFree(c->d_sweep_models); cudaFree(c->d_sweep_units); cudaFree(c->d_sweep_models_side); cudaFree(c->d_sweep_units_side); cudaFree(c->d_sweep_out); cudaFree(c->d_ada);
-  cudaFree(c->d_ops); cudaFree(c->d_irr); cudaFree(c->d_retry); cudaFree(c->d_edf_nodes); cudaFree(c->d_edf_lnnorm);
+  cudaFree(c->d_ops); cudaFree(c->d_irr); cudaFree(c->d_rank_pos); cudaFree(c->d_rank_slot); cudaFree(c->d_retry); cudaFree(c->d_edf_nodes); cudaFree(c->d_edf_lnnorm);
   cudaFree(c->d_mc_cams); cudaFree(c->d_mc_units); cudaFree(c->d_mc_nu3); cudaFree(c->d_mc_scale);
   if (c->ev_ada0) cudaEventDestroy(c->ev_ada0);
   if (c->ev_ada1) cudaEventDestroy(c->ev_ada1);

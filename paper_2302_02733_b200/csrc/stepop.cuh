@@ -53,7 +53,45 @@ struct OpArgs {
   int test_irregular;         // tests: declare every 7th slot irregular, so that the hand-over to k_transfer is exercised
   // many cameras per launch (k_stepop<MODEL, true>): ray q belongs to camera q / rays_per_cam
   const CamDev* cams; const Units* units_arr; int64_t rays_per_cam;
+  const int32_t* pos;         // [base + li]: where k_apply finds slot li (k_rank_window); null: at li
 };
+
+// k_apply walks 32 rays in lockstep, so the rays of a group should be equally long.  The batch is in order of PREDICTED
+// length (probe pass); once k_geodesic has run the true step counts are known, and every window of RANK_WINDOW consecutive
+// slots is re-ranked by them: pos[base + li] = the place of slot li's operator records, slot[base + a] = the slot at place a.
+constexpr int RANK_WINDOW = 1024;
+struct RankArgs { int64_t base, count; const int* count_dev; const int32_t* order; const int32_t* nsteps; int32_t* pos; int32_t* slot; };
+__global__ void __launch_bounds__(RANK_WINDOW) k_rank_window(RankArgs A) {
+  __shared__ unsigned long long key[RANK_WINDOW];
+  const int64_t count = A.count_dev ? (int64_t)*A.count_dev : A.count;
+  const int64_t w0 = (int64_t)blockIdx.x * RANK_WINDOW;
+  if (w0 >= count) return;
+  const int t = threadIdx.x;
+  unsigned long long k = ~0ULL;                  // padding sorts last
+  if (w0 + t < count) {
+    const int32_t q = A.order ? A.order[A.base + w0 + t] : (int32_t)(A.base + w0 + t);
+    int n = A.nsteps[q];
+    if (n < 0) n = 0;
+    k = ((unsigned long long)(0x7fffffff - n) << 32) | (unsigned)t;   // longest first, then by slot: a fixed order
+  }
+  key[t] = k;
+  __syncthreads();
+  for (int size = 2; size <= RANK_WINDOW; size <<= 1)
+    for (int stride = size >> 1; stride > 0; stride >>= 1) {
+      const int partner = t ^ stride;
+      if (partner > t) {
+        const bool up = (t & size) == 0;
+        const unsigned long long a = key[t], b = key[partner];
+        if ((a > b) == up) { key[t] = b; key[partner] = a; }
+      }
+      __syncthreads();
+    }
+  if (w0 + t < count) {
+    const int src = (int)(key[t] & 0xffffffffULL);
+    A.slot[A.base + w0 + t] = (int32_t)(w0 + src);
+    A.pos[A.base + w0 + src] = (int32_t)(w0 + t);
+  }
+}
 
 #ifndef IPOLE_OP_THREADS
 #define IPOLE_OP_THREADS 128
@@ -109,6 +147,7 @@ __global__ void __launch_bounds__(IPOLE_OP_THREADS, IPOLE_OP_MINB) k_stepop(cons
     if (MC) { Ul.nu_obs = nu_obs_l; Ul.dl_unit = dl_unit_l; }
     const void* model = MC ? (const void*)&model_l : (const void*)model_smem;
     const double* rec = A.path + (size_t)li * slot_rec;
+    const int64_t la = A.pos ? (int64_t)A.pos[A.base + li] : li;   // place of this ray's operator records
     bool regular = true;
     double mc[4] = {0.0, 0.0, 0.0, 0.0};     // lane 0, first chunk: projection of step 0's legs on the camera tetrad
 
@@ -158,7 +197,7 @@ __global__ void __launch_bounds__(IPOLE_OP_THREADS, IPOLE_OP_MINB) k_stepop(cons
           transport_apply(Am, h, fi2);
           m11 = dot4(e1c, fi1); m12 = dot4(e1c, fi2); m21 = dot4(e2c, fi1); m22 = dot4(e2c, fi2);
         }
-        double* o = A.ops + op_addr(li, A.cap, s, 0);   // part 1 at o + 128
+        double* o = A.ops + op_addr(la, A.cap, s, 0);   // part 1 at o + 128
         st_global_v4(o, m11, m12, m21, m22);
         st_global_v4(o + 128, x1m, applied ? F.cosT : 0.0, applied ? F.nu : 0.0, dl * Ul.dl_unit);
         if (s == 0) {
@@ -169,7 +208,7 @@ __global__ void __launch_bounds__(IPOLE_OP_THREADS, IPOLE_OP_MINB) k_stepop(cons
     }
     regular = __all_sync(0xffffffffu, regular) && !(A.test_irregular && (li % 7) == 3);
     if (lane == 0) {
-      double* o = A.ops + op_addr(li, A.cap, n, 0);
+      double* o = A.ops + op_addr(la, A.cap, n, 0);
       st_global_v4(o, mc[0], mc[1], mc[2], mc[3]);
       st_global_v4(o + 128, regular ? 0.0 : 1.0, 0.0, 0.0, 0.0);
       if (!regular) { const int w = atomicAdd(A.irr_count, 1); A.irr_slots[w] = (int32_t)li; }
@@ -178,6 +217,7 @@ __global__ void __launch_bounds__(IPOLE_OP_THREADS, IPOLE_OP_MINB) k_stepop(cons
 }
 
 struct ApArgs {
+  const int32_t* slot;        // [base + a]: the slot whose operator records sit at place a (k_rank_window); null: a
   const double* nu3_arr; int64_t rays_per_cam;   // many cameras per launch: nu_obs^3 of camera q / rays_per_cam (nullable)
   AdafParams model;           // the three power laws (by value: 56 B)
   EdfDev edf;                 // k_apply<true>: j, alpha by quadrature over the electron distribution (edf.cuh)
@@ -235,12 +275,13 @@ __global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? IPOLE_AP_EDF_MINB : IP
     if (lane == 0) g = (long long)atomicAdd(A.queue, 1ULL);
     g = __shfl_sync(0xffffffffu, g, 0);
     if (g >= n_groups) break;
-    const int64_t li = (g << 5) + lane;
+    const int64_t li = (g << 5) + lane;          // place in the batch's operator buffer
     int32_t q = 0;
     int n = 0;                                   // steps of this lane's ray; 0: nothing to do
     double mc[4] = {0, 0, 0, 0};
     if (li < count) {
-      q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
+      const int64_t ls = A.slot ? (int64_t)A.slot[A.base + li] : li;
+      q = A.order ? A.order[A.base + ls] : (int32_t)(A.base + ls);
       n = A.nsteps[q];
       if (n < 0) n = 0;                          // overflowed its slot: long-ray pass
       else {
