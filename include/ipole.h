@@ -35,6 +35,7 @@ extern "C" {
 #define IPOLE_ENOMEM   -3   /* host or device allocation failed                                        */
 #define IPOLE_ECUDA    -4   /* a CUDA call failed; ipole_last_cuda_error(ctx) has the cudaError_t      */
 #define IPOLE_ENOIMAGE -5   /* ipole_get_stats / ipole_get_ray_info before ipole_make_image            */
+#define IPOLE_ETOOBIG  -6   /* a size beyond the fixed maximum of an entry point that may not allocate  */
 
 typedef struct ipole_ctx ipole_ctx; /* opaque; owns every device buffer it allocates */
 
@@ -257,6 +258,30 @@ int  ipole_make_image_adaptive(ipole_ctx*, int32_t levels, double rel_tol, doubl
 int  ipole_get_ray_info(ipole_ctx*, int32_t* nsteps, int32_t* nturn);
 /* Synchronises the stream and fills the statistics of the last image. */
 int  ipole_get_stats(ipole_ctx*, ipole_stats*);
+
+/* Totals of an image WITHOUT ANY ALLOCATION ("flux, polarization fractions"; the paper's images
+ * are compared through their total flux and net polarization, Fig. 1) -- for callers that cannot call
+ * cudaMalloc: code under CUDA graph capture, serving loops, harnesses that forbid it.  The same reduction as the one
+ * ipole_make_image ends with, but its block partials live in a fixed array in the library's device image
+ * (`static __device__`, 32 KiB; every GPU that loads the library holds it until the process exits) instead of a
+ * cudaMalloc'ed buffer.  This call makes no cudaMalloc / cudaFree and calls no allocating library routine, does not
+ * synchronise, and works on any four planes the caller has (not only the last image of the context).
+ *   n            pixels, 1 <= n <= IPOLE_TOTALS_STATIC_MAX_PIXELS (4096 x 4096); more: IPOLE_ETOOBIG, nothing launched
+ *   I, Q, U, V   DEVICE pointers, n doubles each, caller-owned, read only
+ *   out6         DEVICE pointer, 6 doubles, caller-owned: sum of I, Q, U, V times the pixel solid angle of the
+ *                context's camera in Jy (as ipole_stats.flux_jy), then lp = sqrt(Q^2+U^2)/I and cp = V/I of the sums
+ * Two kernels on the context's stream (ipole_set_stream); the result is ready when the stream reaches that point.
+ * The summation order is fixed (blocks of 16 384 pixels, folded in index order): a given image gives the same bits
+ * every time; against ipole_stats.flux_jy, whose blocks are shaped differently, it agrees to rounding (~1e-15 rel.).
+ * ALL CALLS SHARE THE ARRAY -- every context, every stream, every thread of the process on that GPU.  It keeps the
+ * last call's contents; nothing in it has to start at zero (each call writes every partial it later reads).  Two calls
+ * whose kernels overlap on the GPU (different streams or contexts without an ordering between them) RACE on it and
+ * both results are undefined: order such calls with events, or keep them on one stream.
+ * IPOLE_EINVAL: NULL argument, n < 1.  IPOLE_ECUDA: the array's device address could not be obtained at ipole_init
+ * (cudaGetSymbolAddress; ipole_last_cuda_error has the code) or a launch failed. */
+#define IPOLE_TOTALS_STATIC_MAX_PIXELS 16777216
+int  ipole_image_totals_static(ipole_ctx*, int64_t n, const double* I, const double* Q, const double* U, const double* V,
+                               double* out6);
 
 /* ---- stages, exposed so that tests can check each against the oracle on its own ---- */
 /* Camera tetrad: Xcam[4], e[a][mu] (16 doubles) to host memory. */

@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstring>
 #include <cstdlib>
+#include <mutex>
 #include <new>
 #include <vector>
 #include "kernels.cuh"
@@ -108,6 +109,9 @@ struct ipole_ctx {
   int* d_small = nullptr;        // [0] long_count, [1] probe max, [2] adaptive list length, [4] / [6] irregular rays of a batch (lane 0 / 1), [5] retries
   ReducePartial* d_part = nullptr;
   ReduceOut* d_red = nullptr;
+
+  double* totals_scratch = nullptr;   // device address of g_totals_scratch on this context's device (ipole_image_totals_static)
+  int totals_scratch_err = 0;         // cudaError_t of the look-up, if it failed
 
   std::vector<TimedSpan> spans; size_t spans_used = 0;
   bool have_image = false;
@@ -857,6 +861,8 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
 
 }  // namespace
 
+namespace { void totals_static_setup(ipole_ctx* c); }   // defined with ipole_image_totals_static, below
+
 extern "C" {
 
 int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
@@ -934,6 +940,7 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_group, k_transfer_group<MODEL_GRID>, IPOLE_RT_THREADS, 0);
   rc = apply_camera(c, cam);
   if (rc != IPOLE_OK) return fail(rc);
+  totals_static_setup(c);   // address of the static scratch of ipole_image_totals_static on this device (a failure is kept for that call)
   *out = c;
   return IPOLE_OK;
 }
@@ -1628,6 +1635,116 @@ void ipole_free(ipole_ctx* c) {
   delete c;
 }
 
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------
+// ipole_image_totals_static: the totals of an image for callers that cannot call
+// cudaMalloc (CUDA graph capture, serving loops, harnesses that forbid allocation).  The block partials of the
+// reduction live in a file-scope device array instead of the context's cudaMalloc'ed d_part; the entry point
+// allocates nothing.  Every GPU that loads the library holds these 32 KiB until the process exits.
+namespace {
+
+constexpr int TOTALS_THREADS = 256;
+constexpr int TOTALS_PER_THREAD = 64;                                  // pixels per thread: a block folds 16 384 pixels
+constexpr int TOTALS_MAX_BLOCKS = IPOLE_TOTALS_STATIC_MAX_PIXELS / (TOTALS_THREADS * TOTALS_PER_THREAD);   // 1024
+static_assert((long long)TOTALS_MAX_BLOCKS * TOTALS_THREADS * TOTALS_PER_THREAD == IPOLE_TOTALS_STATIC_MAX_PIXELS, "limit");
+
+// [block][I, Q, U, V].  In HOST code this name is a host-side stand-in, not a device address: the kernels below get
+// the address cudaGetSymbolAddress returns (totals_static_setup), looked up once per device.
+static __device__ __align__(256) double g_totals_scratch[TOTALS_MAX_BLOCKS * 4];
+
+// block b: pixels [b * 16384, (b+1) * 16384), thread t takes t, t + 256, ... (coalesced); fixed shape => reproducible
+__global__ void __launch_bounds__(TOTALS_THREADS) k_totals_partial_static(int64_t n, const double* __restrict__ I,
+                                                                            const double* __restrict__ Q, const double* __restrict__ U,
+                                                                            const double* __restrict__ V, double* part) {
+  const int64_t q0 = (int64_t)blockIdx.x * (TOTALS_THREADS * TOTALS_PER_THREAD);
+  double s[4] = {0, 0, 0, 0};
+#pragma unroll 4
+  for (int k = 0; k < TOTALS_PER_THREAD; ++k) {
+    const int64_t q = q0 + (int64_t)k * TOTALS_THREADS + threadIdx.x;
+    if (q < n) { s[0] += I[q]; s[1] += Q[q]; s[2] += U[q]; s[3] += V[q]; }
+  }
+  __shared__ double sh[TOTALS_THREADS / 32][4];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) s[k] = warp_sum(s[k]);
+  if (lane == 0) { for (int k = 0; k < 4; ++k) sh[w][k] = s[k]; }
+  __syncthreads();
+  if (threadIdx.x < 4) {
+    double r = sh[0][threadIdx.x];
+    for (int i = 1; i < TOTALS_THREADS / 32; ++i) r += sh[i][threadIdx.x];
+    part[(size_t)blockIdx.x * 4 + threadIdx.x] = r;      // every partial the final kernel reads is written here first
+  }
+}
+
+// one block: thread t folds partials t, t + 256, ...; then the same warp / block fold; out = {flux[4], lp, cp}
+__global__ void __launch_bounds__(TOTALS_THREADS) k_totals_final_static(const double* part, int nparts, double scale, double* out) {
+  double s[4] = {0, 0, 0, 0};
+  for (int i = threadIdx.x; i < nparts; i += TOTALS_THREADS) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) s[k] += part[(size_t)i * 4 + k];
+  }
+  __shared__ double sh[TOTALS_THREADS / 32][4];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) s[k] = warp_sum(s[k]);
+  if (lane == 0) { for (int k = 0; k < 4; ++k) sh[w][k] = s[k]; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double r[4];
+    for (int k = 0; k < 4; ++k) { r[k] = sh[0][k]; for (int i = 1; i < TOTALS_THREADS / 32; ++i) r[k] += sh[i][k]; }
+    for (int k = 0; k < 4; ++k) out[k] = r[k] * scale;
+    out[4] = (r[0] != 0.0) ? sqrt(r[1] * r[1] + r[2] * r[2]) / r[0] : 0.0;
+    out[5] = (r[0] != 0.0) ? r[3] / r[0] : 0.0;
+  }
+}
+
+// Device address of the array, once per device, with that device current (called from ipole_init).
+constexpr int TOTALS_MAX_DEVICES = 64;
+double* g_totals_addr[TOTALS_MAX_DEVICES] = {};
+int g_totals_addr_err[TOTALS_MAX_DEVICES] = {};
+bool g_totals_addr_known[TOTALS_MAX_DEVICES] = {};
+std::mutex g_totals_mutex;
+
+void totals_static_setup(ipole_ctx* c) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess || dev != c->device || dev < 0 || dev >= TOTALS_MAX_DEVICES) {
+    c->totals_scratch = nullptr;
+    c->totals_scratch_err = (int)(e != cudaSuccess ? e : cudaErrorInvalidDevice);
+    cudaGetLastError();
+    return;
+  }
+  std::lock_guard<std::mutex> lk(g_totals_mutex);
+  if (!g_totals_addr_known[dev]) {
+    double* ptr = nullptr;
+    e = cudaGetSymbolAddress((void**)&ptr, g_totals_scratch);
+    if (e != cudaSuccess) { cudaGetLastError(); ptr = nullptr; }
+    g_totals_addr[dev] = ptr;
+    g_totals_addr_err[dev] = (int)e;
+    g_totals_addr_known[dev] = true;
+  }
+  c->totals_scratch = g_totals_addr[dev];
+  c->totals_scratch_err = g_totals_addr_err[dev];
+}
+
+}  // namespace
+
+extern "C" {
+
+int ipole_image_totals_static(ipole_ctx* c, int64_t n, const double* I, const double* Q, const double* U, const double* V,
+                              double* out6) {
+  if (!c || !I || !Q || !U || !V || !out6 || n < 1) return IPOLE_EINVAL;
+  if (n > (int64_t)IPOLE_TOTALS_STATIC_MAX_PIXELS) return IPOLE_ETOOBIG;
+  if (!c->totals_scratch) { c->last_cuda = c->totals_scratch_err; return IPOLE_ECUDA; }
+  const int nb = (int)((n + TOTALS_THREADS * TOTALS_PER_THREAD - 1) / (TOTALS_THREADS * TOTALS_PER_THREAD));
+  const double pix_rad = c->cam.pix * c->units.L_unit / c->units.D_cm;
+  k_totals_partial_static<<<nb, TOTALS_THREADS, 0, c->stream>>>(n, I, Q, U, V, c->totals_scratch);
+  k_totals_final_static<<<1, TOTALS_THREADS, 0, c->stream>>>(c->totals_scratch, nb, pix_rad * pix_rad * 1e23, out6);
+  CK(cudaGetLastError());
+  return IPOLE_OK;
+}
+
 const char* ipole_strerror(int code) {
   switch (code) {
     case IPOLE_OK: return "ok";
@@ -1636,6 +1753,7 @@ const char* ipole_strerror(int code) {
     case IPOLE_ENOMEM: return "out of memory";
     case IPOLE_ECUDA: return "CUDA error (see ipole_last_cuda_error)";
     case IPOLE_ENOIMAGE: return "no image has been made yet";
+    case IPOLE_ETOOBIG: return "size beyond the fixed maximum of a *_static entry point (IPOLE_TOTALS_STATIC_MAX_PIXELS)";
     default: return "unknown error";
   }
 }

@@ -14,10 +14,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libipole_b200.so")
 _LIB = None
 
-OK, EINVAL, ENOMODEL, ENOMEM, ECUDA, ENOIMAGE = 0, -1, -2, -3, -4, -5
+OK, EINVAL, ENOMODEL, ENOMEM, ECUDA, ENOIMAGE, ETOOBIG = 0, -1, -2, -3, -4, -5, -6
 
 #: every symbol include/ipole.h declares (checked by tests/test_abi.py)
-SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_options", "ipole_set_path_free", "ipole_set_edf", "ipole_set_geodesic_fp32", "ipole_set_transfer_split", "ipole_set_batch_overlap", "ipole_set_unpolarized", "ipole_load_model_adaf",
+SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_options", "ipole_set_path_free", "ipole_set_edf", "ipole_set_geodesic_fp32", "ipole_set_transfer_split", "ipole_set_batch_overlap", "ipole_image_totals_static", "ipole_set_unpolarized", "ipole_load_model_adaf",
            "ipole_load_model_slab", "ipole_load_model_grid", "ipole_make_image", "ipole_make_pixels", "ipole_make_images_adaf", "ipole_make_images_grid", "ipole_make_images_cameras", "ipole_make_image_adaptive",
            "ipole_get_ray_info", "ipole_get_stats", "ipole_get_camera_tetrad", "ipole_trace_pixel",
            "ipole_eval_connection", "ipole_eval_coefficients", "ipole_eval_coefficients_edf", "ipole_eval_stokes_step", "ipole_eval_bessel",
@@ -93,6 +93,7 @@ def lib():
         L.ipole_set_unpolarized.argtypes = [vp, C.c_int32]
         L.ipole_set_transfer_split.argtypes = [vp, C.c_int32]
         L.ipole_set_batch_overlap.argtypes = [vp, C.c_int32]
+        L.ipole_image_totals_static.argtypes = [vp, C.c_int64, vp, vp, vp, vp, vp]
         L.ipole_set_geodesic_fp32.argtypes = [vp, C.c_int32]
         L.ipole_set_edf.argtypes = [vp, C.POINTER(Edf)]
         L.ipole_eval_coefficients_edf.argtypes = [vp, C.c_int64, dp, dp]
@@ -361,6 +362,18 @@ class Ipole:
         ns = np.zeros(n, dtype=np.int32); nt = np.zeros(n, dtype=np.int32)
         _chk(lib().ipole_get_ray_info(self._h, _ptr(ns), _ptr(nt)), "ipole_get_ray_info")
         return ns.reshape(self.ny, self.nx), nt.reshape(self.ny, self.nx)
+
+    def image_totals_static(self, I, Q, U, V, out):
+        """Totals of four CUDA FP64 planes into the CUDA tensor `out` (6 doubles: flux_jy[4], lp, cp) through the entry point
+        that allocates nothing (include/ipole.h ipole_image_totals_static).  Asynchronous on the context's stream."""
+        for t in (I, Q, U, V, out):
+            if not (t.is_cuda and t.is_contiguous() and str(t.dtype) == "torch.float64"):
+                raise ValueError("image_totals_static takes contiguous CUDA float64 tensors")
+        if out.numel() < 6 or not (I.numel() == Q.numel() == U.numel() == V.numel()):
+            raise ValueError("image_totals_static: out needs 6 doubles, the planes equal sizes")
+        _chk(lib().ipole_image_totals_static(self._h, I.numel(), I.data_ptr(), Q.data_ptr(), U.data_ptr(), V.data_ptr(),
+                                             out.data_ptr()), "ipole_image_totals_static")
+        return out
 
     def stats(self):
         s = Stats()
