@@ -503,22 +503,41 @@ def measure_image(args, name, ipole, replicas, W, world, rank, local, barrier):
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     ev0.record()
+    host_s = 0.0
     for _ in range(args.steps):
+        th = time.perf_counter()
         g.make_image(maps=maps, out=out)
+        host_s += time.perf_counter() - th      # the call alone: with a reused plan it only enqueues (ipole_set_plan_reuse)
     ev1.record()
     barrier()
     ms = ev0.elapsed_time(ev1)
     st = g.stats()  # of the last timed image (event times are per image)
     st_live = st
-    if st.get("n_lanes", 1) == 2:
-        # the timed images ran with consecutive batches side by side on two streams (ipole_set_batch_overlap): the event
-        # spans of concurrent kernels overlap, so the per-kernel times come from one more image with the lanes off
+    st_plan = st
+    if st.get("n_lanes", 1) == 2 or st.get("plan_reused", 0):
+        # The timed images ran with consecutive batches side by side on two streams (ipole_set_batch_overlap): the event
+        # spans of concurrent kernels overlap, so the per-kernel times come from one more image with the lanes off.  The
+        # first image after the switch plans afresh (probe pass: its time is the probe_sort entry), the second reuses
+        # that plan like the timed ones.
         g.set_batch_overlap(False)
-        for _ in range(2):
-            g.make_image(maps=maps, out=out)
+        g.make_image(maps=maps, out=out)
+        torch.cuda.synchronize()
+        st_plan = g.stats()
+        g.make_image(maps=maps, out=out)
         torch.cuda.synchronize()
         st = g.stats()
         g.set_batch_overlap(True)
+    # one image planned afresh with everything else as timed: what the first call for a camera costs
+    planning = None
+    if st_live.get("plan_reused", 0) and not (args.path_free or args.edf):
+        g.set_plan_reuse(False)
+        tp = time.perf_counter()
+        g.make_image(maps=maps, out=out)
+        host_plan = time.perf_counter() - tp
+        torch.cuda.synchronize()
+        sp = g.stats()
+        planning = {"ms_total": sp["ms_total"], "ms_probe": sp["ms_probe"], "host_call_ms": host_plan * 1e3, "gpu_launches": sp["n_launches"]}
+        g.set_plan_reuse(True)
     clocks = sampler.stop() if rank == 0 else None
     ms = replicas.max_over_ranks(ms, "cuda")
     value = replicas.job_throughput(rays * args.steps, ms * 1e-3, world)
@@ -632,7 +651,7 @@ def measure_image(args, name, ipole, replicas, W, world, rank, local, barrier):
                        "parallelism": "rays sharded: one replica per GPU" if world > 1 else "single GPU"},
             "images_per_s": value / rays, "steps_per_s": world * st["total_steps"] * args.steps / (ms * 1e-3),
             "mean_steps_per_ray": st["total_steps"] / rays, "forward_steps": st["total_steps_forward"],
-            "stage_ms": {"probe_sort": st["ms_probe"], "geodesic": st["ms_geodesic"], "transfer": st["ms_transfer"],
+            "stage_ms": {"probe_sort": st_plan["ms_probe"], "geodesic": st["ms_geodesic"], "transfer": st["ms_transfer"],
                          "stepop": st["ms_stepop"], "apply": st["ms_apply"],
                          "long_rays_side_stream": st["ms_long"], "total": st["ms_total"], "batches": st["n_batches"], "path_cap": st["path_cap"],
                          "long_rays": st["n_long"], "retried_rays": st["n_retry"],
@@ -642,6 +661,12 @@ def measure_image(args, name, ipole, replicas, W, world, rank, local, barrier):
                                  if st_live.get("n_lanes", 1) == 2 else "one stream"},
             "flux_jy": st["flux_jy"], "lp": st["lp"], "cp": st["cp"], "ring_rays": st["n_ring"],
             "gpu_launches": st_live["n_launches"] * args.steps, "roofline": roof, "e2e": e2e, "clocks": clocks,
+            "plan": {"reused": bool(st_live.get("plan_reused", 0)), "host_ms_per_call": host_s * 1e3 / args.steps,
+                     "planning_call": planning,
+                     "note": "the timed images are scheduled from the plan of the call before them (ipole_set_plan_reuse: same camera, no "
+                             "probe pass, no host-device synchronisation; the call returns after host_ms_per_call while the GPU works for "
+                             "ms_per_step); planning_call = one image planned afresh (probe pass, read-backs, blocking), as the first "
+                             "call for a camera is; stage_ms.probe_sort is that call's probe time and is not part of a reused image"},
             "paper_context": {"note": "paper Table 1, other model/hardware (A100): context only",
                               "a100_semianalytic_4096_rays_per_s": 127583, "a100_grmhd_4096_rays_per_s": 188720}}
     g.close()

@@ -107,7 +107,8 @@ typedef struct {
   int32_t n_lanes;         /* 2: the batches alternated between two streams (ipole_set_batch_overlap) -- kernels of
                               consecutive batches then run side by side, their event times overlap, and ms_geodesic +
                               ms_transfer exceeds ms_total; 1: one batch after the other                   */
-  int32_t reserved_;
+  int32_t plan_reused;     /* 1: the image was scheduled from the plan of the previous call (ipole_set_plan_reuse): no
+                              probe pass (ms_probe = 0), no read-back, the call returned without waiting for the GPU */
 } ipole_stats;
 
 /* Create a context. Computes the camera tetrad on the device. IPOLE_EINVAL on bad parameters. */
@@ -150,6 +151,22 @@ int  ipole_set_transfer_split(ipole_ctx*, int32_t on);
  * ms_total; bench.py measures its per-kernel figures this way).  Same image either way, bit for bit (a ray's arithmetic
  * does not depend on its batch).  Single-batch images and the sweeps always run on one stream.  IPOLE_EINVAL for NULL. */
 int  ipole_set_batch_overlap(ipole_ctx*, int32_t on);
+/* Asynchronous images by plan reuse (default on).  To schedule an image the host needs four facts from the device: the
+ * longest probe ray (S_cap), the populations of the step-count bins (slots per batch), which rays outgrew their slots and
+ * which are longer than S_cap.  Reading them back costs a probe pass and several host-device synchronisations, during
+ * which ipole_make_image blocks.  All four depend on the geodesics alone -- camera, spin, eps, image size, scheduling
+ * options -- not on the plasma model or its parameters (the geodesic is integrated first, "saved", and the
+ * transfer then runs along it).  on != 0: the context keeps them from the last full-image call (and the ray order and
+ * the two ray lists on the device); the next ipole_make_image with the SAME camera, image size, options and (to 1.5 %)
+ * memory budget is scheduled from them: no probe pass, no read-back, the retried and the long rays start at once on
+ * the side stream.  With device outputs such a call only enqueues work and RETURNS WHILE THE GPU IS STILL RUNNING
+ * (ipole_stats.plan_reused = 1); outputs are valid once the context's stream reaches that point (stream order, an
+ * event, or ipole_get_stats, which synchronises).  The model may be reloaded or its parameters changed in between (a
+ * time series of GRMHD slices, a parameter fit at fixed geometry).  Any other call in between, a changed camera or
+ * option, or a different amount of free memory falls back to the planning call, which blocks as before and records a
+ * new plan.  The image is the same, bit for bit, either way.  Not used for pixel lists, sweeps, many-camera calls, the
+ * path-free variant and eDF coefficients.  on == 0: every call plans afresh.  IPOLE_EINVAL for a NULL context. */
+int  ipole_set_plan_reuse(ipole_ctx*, int32_t on);
 /* Second physics workload (outlook: electron distribution functions "for which accurate prescriptions ... do
  * not exist and the integration of synchrotron emissivity over the electron energy distribution function requires
  * numerical integration during ray tracing"; the paper gives no formulas: reading R-13 in DESIGN.md).
@@ -190,7 +207,11 @@ int  ipole_load_model_grid(ipole_ctx*, const ipole_grid_desc*, const double* con
 
 /* One full-Stokes image: I,Q,U,V [ny][nx] row-major, specific intensity in erg s^-1 cm^-2 Hz^-1 sr^-1.
  * tau (absorption optical depth) and tauF (Faraday depth, int |rho_V| dl) are optional [ny][nx] maps.
- * All non-NULL outputs must be of one kind (all host or all device). */
+ * All non-NULL outputs must be of one kind (all host or all device).
+ * Blocking: the FIRST image of a camera plans its batches from a probe pass and reads a few counters back, so the call
+ * blocks for most of the image; with device outputs it returns with the last kernels still in flight.  Further images
+ * of the same camera are scheduled from that plan and the call returns at once (ipole_set_plan_reuse, default on).
+ * Either way the outputs are valid in stream order on the context's stream. */
 int  ipole_make_image(ipole_ctx*, double* I, double* Q, double* U, double* V, double* tau, double* tauF);
 /* Same for a list of n flat pixel indices j*nx+i (device or host int64); outputs have n entries. Used for
  * sampled parity checks at resolutions whose full image the CPU oracle cannot afford. pixels == NULL means

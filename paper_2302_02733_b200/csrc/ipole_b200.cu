@@ -110,6 +110,19 @@ struct ipole_ctx {
   ReducePartial* d_part = nullptr;
   ReduceOut* d_red = nullptr;
 
+  // Plan of the last full-image call (ipole_set_plan_reuse): what the host had to READ BACK from the device to schedule
+  // it -- S_cap and the bin populations of the sort (the ray order itself stays in d_order), the rays that outgrew their
+  // slots and the rays longer than S_cap.  All of it depends on the camera and the scheduling options alone, not on the
+  // plasma, so a call with the same key replays it without a single host-device synchronisation.
+  struct PlanCache {
+    bool valid = false;
+    ipole_camera cam; int64_t n = 0; size_t budget = 0; unsigned flags = 0;
+    int cap = 0, bin_width = 1; std::vector<unsigned int> bin_prefix;
+    int n_long = 0, n_retry = 0;
+    int32_t* d_long = nullptr; int32_t* d_retry = nullptr; int long_cap = 0, retry_cap = 0;   // the two lists as that call left them
+  } plan_cache;
+  int opt_plan_reuse = 1;
+
   double* totals_scratch = nullptr;   // device address of g_totals_scratch on this context's device (ipole_image_totals_static)
   int totals_scratch_err = 0;         // cudaError_t of the look-up, if it failed
 
@@ -185,6 +198,7 @@ int apply_camera(ipole_ctx* c, const ipole_camera* k) {
 
 int ensure_rays(ipole_ctx* c, int64_t n) {
   if (n <= c->ray_cap) return IPOLE_OK;
+  c->plan_cache.valid = false;
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long); cudaFree(c->d_out);
   cudaFree(c->d_nsteps_long); cudaFree(c->d_srange); c->d_srange = nullptr; cudaFree(c->d_irr); cudaFree(c->d_retry); c->d_retry = nullptr; cudaFree(c->d_rank_pos); cudaFree(c->d_rank_slot); c->d_rank_pos = c->d_rank_slot = nullptr;
   c->d_nsteps = c->d_nturn = c->d_order = c->d_key = c->d_long = c->d_nsteps_long = c->d_irr = nullptr; c->d_out = nullptr; c->ray_cap = 0;
@@ -224,7 +238,7 @@ int ensure_ops(ipole_ctx* c, size_t bytes) {
 
 int ensure_retry_buf(ipole_ctx* c, size_t bytes) {
   if (bytes <= c->retry_buf_bytes) return IPOLE_OK;
-  cudaFree(c->d_retry_buf); c->d_retry_buf = nullptr; c->retry_buf_bytes = 0;
+  cudaFree(c->d_retry_buf); cudaFree(c->plan_cache.d_long); cudaFree(c->plan_cache.d_retry); c->d_retry_buf = nullptr; c->retry_buf_bytes = 0;
   cudaError_t e = cudaMalloc(&c->d_retry_buf, bytes);
   if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
   c->retry_buf_bytes = bytes;
@@ -484,15 +498,28 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   int qi = 0;
   const int total = span_begin(c, LK_OTHER, c->stream);
 
-  const size_t budget = path_budget(c);
+  size_t budget = path_budget(c);
   const size_t rec_bytes = REC_DOUBLES * sizeof(double);
   const int max_steps = c->cam.max_steps;
   int cap = max_steps;
   const int32_t* order = nullptr;
   std::vector<unsigned int> bin_prefix;   // sorted rays: number of rays in the bins before each bin (longer rays)
   int bin_width = 1;
+  // ---- plan of the previous call (ctx.plan_cache): a full image with the same camera and scheduling options is
+  // scheduled from it, with no probe pass and no read-back, so the call returns while the GPU is still working ----
+  ipole_ctx::PlanCache& pc = c->plan_cache;
+  const unsigned plan_flags = (unsigned)c->opt_sort | (unsigned)c->opt_tight << 2 | (unsigned)(c->opt_split != 0) << 3 | (unsigned)c->opt_overlap << 4 |
+                              (unsigned)c->opt_unpol << 5 | (unsigned)c->opt_geo_fp32 << 6 | (unsigned)c->opt_side_retry << 7 |
+                              (unsigned)c->opt_occ << 8 | (unsigned)c->opt_rank << 9 | (unsigned)c->model << 12;
+  const bool cacheable = c->opt_plan_reuse && !d_pixels && !sw && c->n_mc == 0 && !c->opt_path_free && c->edf.kind == 0 && c->opt_sort != 0;
+  const bool replay = cacheable && pc.valid && pc.n == n && pc.flags == plan_flags && std::memcmp(&pc.cam, &c->cam_in, sizeof(ipole_camera)) == 0 &&
+                      (budget > pc.budget ? budget - pc.budget : pc.budget - budget) <= pc.budget / 64;
+  if (!replay) pc.valid = false;          // (this call may overwrite d_order)
+  if (replay) budget = pc.budget;         // the same plan needs the memory that is already there
+  c->stats.plan_reused = replay ? 1 : 0;
   const bool fits_all = (double)n * (double)(max_steps + 1) * (double)rec_bytes <= (double)budget;
-  const bool probe = (n >= 32768 || c->opt_sort == 2) && (c->opt_sort || !fits_all);
+  const bool probe = !replay && (n >= 32768 || c->opt_sort == 2) && (c->opt_sort || !fits_all);
+  if (replay) { cap = pc.cap; bin_width = pc.bin_width; bin_prefix = pc.bin_prefix; order = c->d_order; }
 
   if (probe) {
     // ---- probe pass: coarse lattice (or strided list), 4 eps, no path storage ----
@@ -549,7 +576,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     }
     span_end(c, sp, c->stream);
   }
-  if (!probe) {
+  if (!probe && !replay) {
     // everything in flight at once: give each ray what the budget allows
     const int64_t per = (int64_t)(budget / rec_bytes / (size_t)n) - 1;
     cap = (int)std::max<int64_t>(64, std::min<int64_t>(max_steps, per));
@@ -596,6 +623,8 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   const size_t lslot = (size_t)(max_steps + 1) * rec_bytes;
   int long_done = 0;          // entries of d_long already handed to the side stream
   int64_t LBcap = 0;          // rays that fit the long path buffer
+  const int32_t* long_src = replay ? pc.d_long : c->d_long;       // replay: the list the recorded call ended with
+  const int32_t* retry_src = replay ? pc.d_retry : c->d_retry;
   auto long_pass = [&](int upto) -> int {
     if (upto <= long_done) return IPOLE_OK;
     if (LBcap == 0) {
@@ -609,7 +638,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
       const int64_t cnt = std::min<int64_t>(LBcap, upto - base);
       if (qi + 2 > N_QUEUES) return IPOLE_EINVAL;
       GeoArgs g = geo_args(c);
-      g.cap = max_steps; g.base = base; g.count = cnt; g.order = c->d_long; g.pixels = d_pixels;
+      g.cap = max_steps; g.base = base; g.count = cnt; g.order = long_src; g.pixels = d_pixels;
       g.path = c->d_path_long; g.nsteps = c->d_nsteps_long; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
       if (use_occ) { g.grid = (const GridParams*)c->d_model; g.srange = c->d_srange; }
       int rcl = launch_geodesic(c, g, LK_LONG, cnt, c->side);
@@ -617,7 +646,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
       RtArgs t;
       std::memset(&t, 0, sizeof t);
       t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = max_steps; t.base = base; t.count = cnt;
-      t.order = c->d_long; t.path = c->d_path_long; t.nsteps = c->d_nsteps_long; t.queue = c->d_queues + (qi++);
+      t.order = long_src; t.path = c->d_path_long; t.nsteps = c->d_nsteps_long; t.queue = c->d_queues + (qi++);
       if (use_occ) t.srange = c->d_srange;
       t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
       if ((rcl = launch_transfer(c, t, LK_LONG, cnt, c->side, 0, 0, sw)) != IPOLE_OK) return rcl;
@@ -723,7 +752,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     int rcb;
     if ((rcb = launch_geodesic(c, g, LK_GEO, b.cnt, st, reserve)) != IPOLE_OK) return rcb;
     CK(cudaEventRecord(c->ev_lastgeo[lane], st));
-    if (top && cap < max_steps && !edf) {
+    if (top && cap < max_steps && !edf && !replay) {
       CK(cudaEventRecord(c->ev_geo, st));
       CK(cudaStreamWaitEvent(c->side, c->ev_geo, 0));
     }
@@ -738,7 +767,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     else rcb = launch_transfer(c, t, LK_RT, b.cnt, st, reserve, 0, sw);
     if (rcb != IPOLE_OK) return rcb;
     c->stats.n_batches++;
-    if (top && cap < max_steps && !edf) {   // the transfer kernel just queued keeps the GPU busy while the host waits here
+    if (top && cap < max_steps && !edf && !replay) {   // the transfer kernel just queued keeps the GPU busy while the host waits here
       if ((rcb = listed(c->ev_geo, n_long)) != IPOLE_OK) return rcb;
       if ((rcb = long_pass(n_long)) != IPOLE_OK) return rcb;
     }
@@ -773,52 +802,72 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     if (R_max < 32) R_max = 0;
   }
   const int n_lanes_bulk = (n_lanes == 2 && plan.size() >= 2) ? 2 : 1;
-  if ((rc = run_plan(order)) != IPOLE_OK) return rc;
-  bool side_used = false;
-  if (R_max > 0) {
+  // the retry level on the side stream for the first `count` (or *count_dev) entries of `list`
+  auto side_retry = [&](const int32_t* list, int64_t count, const int* count_dev) -> int {
     if (qi + 4 > N_QUEUES) return IPOLE_EINVAL;
+    double* rpath = c->d_retry_buf;
+    double* rops = split ? c->d_retry_buf + (size_t)R_max * (size_t)(cap + 1) * REC_DOUBLES : nullptr;
+    GeoArgs g = geo_args(c);
+    g.cap = cap; g.base = 0; g.count = count; g.count_dev = count_dev; g.order = list; g.pixels = d_pixels;
+    g.path = rpath; g.nsteps = c->d_nsteps_long; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
+    g.long_list = c->d_long; g.long_count = c->d_small;
+    if (use_occ) { g.grid = (const GridParams*)c->d_model; g.srange = c->d_srange; }
+    int rcs;
+    if ((rcs = launch_geodesic(c, g, LK_LONG, count, c->side)) != IPOLE_OK) return rcs;
+    CK(cudaEventRecord(c->ev_geo, c->side));
+    RtArgs t;
+    std::memset(&t, 0, sizeof t);
+    t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = cap; t.base = 0; t.count = count; t.count_dev = count_dev;
+    t.order = list; t.path = rpath; t.nsteps = c->d_nsteps_long; t.queue = c->d_queues + qi;
+    qi += split ? 3 : 1;
+    if (use_occ) t.srange = c->d_srange;
+    t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
+    if (split) rcs = launch_transfer_split(c, t, count, c->side, 0, rops, 2);
+    else rcs = launch_transfer(c, t, LK_LONG, count, c->side, 0, 0, nullptr);
+    return rcs;
+  };
+  bool side_used = false;
+  int n_retry_side = 0;
+  if (replay) {
+    // Everything the side stream does is known: the retried rays, then the long rays, from the recorded lists, started
+    // now, beside the first bulk batches (the retry level first: a retried ray that is also long is marked by it and
+    // traced by the long pass, in that order, as in the recorded call).
+    CK(cudaEventRecord(c->ev_fork, c->stream));
+    CK(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+    n_retry_side = (int)std::min<int64_t>(pc.n_retry, R_max);
+    if (n_retry_side > 0 && (rc = side_retry(retry_src, n_retry_side, nullptr)) != IPOLE_OK) return rc;
+    n_long = pc.n_long;
+    if (n_long > 0 && (rc = long_pass(n_long)) != IPOLE_OK) return rc;
+    side_used = n_retry_side > 0;
+  }
+  if ((rc = run_plan(order)) != IPOLE_OK) return rc;
+  if (R_max > 0 && !replay) {
     for (int l = 0; l < n_lanes_bulk; ++l) CK(cudaStreamWaitEvent(c->side, c->ev_lastgeo[l], 0));
     int* rcount = c->d_small + 7;
     k_clamp_count<<<1, 1, 0, c->side>>>(retry_count, (int)R_max, rcount);
     c->stats.n_launches++;
-    double* rpath = c->d_retry_buf;
-    double* rops = split ? c->d_retry_buf + (size_t)R_max * (size_t)(cap + 1) * REC_DOUBLES : nullptr;
-    GeoArgs g = geo_args(c);
-    g.cap = cap; g.base = 0; g.count = R_max; g.count_dev = rcount; g.order = c->d_retry; g.pixels = d_pixels;
-    g.path = rpath; g.nsteps = c->d_nsteps_long; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
-    g.long_list = c->d_long; g.long_count = c->d_small;
-    if (use_occ) { g.grid = (const GridParams*)c->d_model; g.srange = c->d_srange; }
-    if ((rc = launch_geodesic(c, g, LK_LONG, R_max, c->side)) != IPOLE_OK) return rc;
-    CK(cudaEventRecord(c->ev_geo, c->side));
-    RtArgs t;
-    std::memset(&t, 0, sizeof t);
-    t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = cap; t.base = 0; t.count = R_max; t.count_dev = rcount;
-    t.order = c->d_retry; t.path = rpath; t.nsteps = c->d_nsteps_long; t.queue = c->d_queues + qi;
-    qi += split ? 3 : 1;
-    if (use_occ) t.srange = c->d_srange;
-    t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
-    if (split) rc = launch_transfer_split(c, t, R_max, c->side, 0, rops, 2);
-    else rc = launch_transfer(c, t, LK_LONG, R_max, c->side, 0, 0, nullptr);
-    if (rc != IPOLE_OK) return rc;
+    if ((rc = side_retry(retry_src, R_max, rcount)) != IPOLE_OK) return rc;
     side_used = true;
   }
-  int n_retry_side = 0;
+  int n_retry = 0;
   if (tight) {
-    int n_retry = 0;
-    CK(cudaMemcpyAsync(&n_retry, retry_count, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-    CK(cudaStreamSynchronize(c->stream));
-    c->stats.n_retry = n_retry;
-    n_retry_side = (int)std::min<int64_t>(n_retry, R_max);
-    if (n_retry_side > 0 && cap < max_steps && !edf) {
-      // retried rays that outgrow S_cap as well: listed by the geodesic kernel above, long-ray pass
-      if ((rc = listed(c->ev_geo, n_long)) != IPOLE_OK) return rc;
-      if ((rc = long_pass(n_long)) != IPOLE_OK) return rc;
+    if (replay) n_retry = pc.n_retry;
+    else {
+      CK(cudaMemcpyAsync(&n_retry, retry_count, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+      CK(cudaStreamSynchronize(c->stream));
+      n_retry_side = (int)std::min<int64_t>(n_retry, R_max);
+      if (n_retry_side > 0 && cap < max_steps && !edf) {
+        // retried rays that outgrow S_cap as well: listed by the geodesic kernel above, long-ray pass
+        if ((rc = listed(c->ev_geo, n_long)) != IPOLE_OK) return rc;
+        if ((rc = long_pass(n_long)) != IPOLE_OK) return rc;
+      }
     }
+    c->stats.n_retry = n_retry;
     if (n_retry > n_retry_side) {
       // the rest of the second level on the lanes, with the global S_cap
       make_plan(n_retry - n_retry_side, false);
       if ((rc = prepare(false)) != IPOLE_OK) return rc;
-      if ((rc = run_plan(c->d_retry + n_retry_side)) != IPOLE_OK) return rc;
+      if ((rc = run_plan(retry_src + n_retry_side)) != IPOLE_OK) return rc;
     }
   }
   if (edf && cap < max_steps) {
@@ -846,14 +895,33 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     CK(cudaEventRecord(c->ev_side, c->side));
     CK(cudaStreamWaitEvent(c->stream, c->ev_side, 0));
     if (n_long > 0) {
-      k_merge_long<<<(n_long + 255) / 256, 256, 0, c->stream>>>(n_long, c->d_long, c->d_nsteps_long, c->d_nsteps);
+      k_merge_long<<<(n_long + 255) / 256, 256, 0, c->stream>>>(n_long, long_src, c->d_nsteps_long, c->d_nsteps);
       c->stats.n_launches++;
     }
     if (n_retry_side > 0) {
-      k_merge_long<<<(n_retry_side + 255) / 256, 256, 0, c->stream>>>(n_retry_side, c->d_retry, c->d_nsteps_long, c->d_nsteps);
+      k_merge_long<<<(n_retry_side + 255) / 256, 256, 0, c->stream>>>(n_retry_side, retry_src, c->d_nsteps_long, c->d_nsteps);
       c->stats.n_launches++;
     }
     CK(cudaGetLastError());
+  }
+  if (cacheable && !replay && order != nullptr && !bin_prefix.empty()) {
+    // keep what this call had to read back, and the two lists as they stand now (every kernel that appends has been
+    // joined into the stream)
+    pc.cam = c->cam_in; pc.n = n; pc.budget = budget; pc.flags = plan_flags;
+    pc.cap = cap; pc.bin_width = bin_width; pc.bin_prefix = bin_prefix;
+    pc.n_long = c->stats.n_long > 0 ? (int)c->stats.n_long : 0; pc.n_retry = n_retry;
+    bool ok = true;
+    if (pc.n_long > pc.long_cap) {
+      cudaFree(pc.d_long); pc.d_long = nullptr; pc.long_cap = 0;
+      if (cudaMalloc(&pc.d_long, (size_t)pc.n_long * sizeof(int32_t)) == cudaSuccess) pc.long_cap = pc.n_long; else { cudaGetLastError(); ok = false; }
+    }
+    if (pc.n_retry > pc.retry_cap) {
+      cudaFree(pc.d_retry); pc.d_retry = nullptr; pc.retry_cap = 0;
+      if (cudaMalloc(&pc.d_retry, (size_t)pc.n_retry * sizeof(int32_t)) == cudaSuccess) pc.retry_cap = pc.n_retry; else { cudaGetLastError(); ok = false; }
+    }
+    if (ok && pc.n_long > 0) CK(cudaMemcpyAsync(pc.d_long, c->d_long, (size_t)pc.n_long * sizeof(int32_t), cudaMemcpyDeviceToDevice, c->stream));
+    if (ok && pc.n_retry > 0) CK(cudaMemcpyAsync(pc.d_retry, c->d_retry, (size_t)pc.n_retry * sizeof(int32_t), cudaMemcpyDeviceToDevice, c->stream));
+    pc.valid = ok;
   }
 
   return finish_image(c, n, I, Q, U, V, total);
@@ -935,6 +1003,7 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   { const char* e = std::getenv("IPOLE_NO_TIGHT"); if (e && e[0] == '1') c->opt_tight = 0; }
   { const char* e = std::getenv("IPOLE_NO_GROUP"); if (e && e[0] == '1') c->opt_group = 0; }
   { const char* e = std::getenv("IPOLE_NO_OVERLAP"); if (e && e[0] == '1') c->opt_overlap = 0; }
+  { const char* e = std::getenv("IPOLE_NO_PLAN_REUSE"); if (e && e[0] == '1') c->opt_plan_reuse = 0; }
   { const char* e = std::getenv("IPOLE_NO_RANK"); if (e && e[0] == '1') c->opt_rank = 0; }
   { const char* e = std::getenv("IPOLE_NO_SIDE_RETRY"); if (e && e[0] == '1') c->opt_side_retry = 0; }
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_group, k_transfer_group<MODEL_GRID>, IPOLE_RT_THREADS, 0);
@@ -1018,6 +1087,13 @@ int ipole_set_geodesic_fp32(ipole_ctx* c, int32_t on) {
 int ipole_set_transfer_split(ipole_ctx* c, int32_t on) {
   if (!c) return IPOLE_EINVAL;
   c->opt_split = (on == 2) ? 2 : (on ? 1 : 0);
+  return IPOLE_OK;
+}
+
+int ipole_set_plan_reuse(ipole_ctx* c, int32_t on) {
+  if (!c) return IPOLE_EINVAL;
+  c->opt_plan_reuse = on ? 1 : 0;
+  c->plan_cache.valid = false;
   return IPOLE_OK;
 }
 

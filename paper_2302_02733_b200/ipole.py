@@ -17,7 +17,7 @@ _LIB = None
 OK, EINVAL, ENOMODEL, ENOMEM, ECUDA, ENOIMAGE, ETOOBIG = 0, -1, -2, -3, -4, -5, -6
 
 #: every symbol include/ipole.h declares (checked by tests/test_abi.py)
-SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_options", "ipole_set_path_free", "ipole_set_edf", "ipole_set_geodesic_fp32", "ipole_set_transfer_split", "ipole_set_batch_overlap", "ipole_image_totals_static", "ipole_set_unpolarized", "ipole_load_model_adaf",
+SYMBOLS = ["ipole_init", "ipole_set_camera", "ipole_set_stream", "ipole_set_options", "ipole_set_path_free", "ipole_set_edf", "ipole_set_geodesic_fp32", "ipole_set_transfer_split", "ipole_set_batch_overlap", "ipole_set_plan_reuse", "ipole_image_totals_static", "ipole_set_unpolarized", "ipole_load_model_adaf",
            "ipole_load_model_slab", "ipole_load_model_grid", "ipole_make_image", "ipole_make_pixels", "ipole_make_images_adaf", "ipole_make_images_grid", "ipole_make_images_cameras", "ipole_make_image_adaptive",
            "ipole_get_ray_info", "ipole_get_stats", "ipole_get_camera_tetrad", "ipole_trace_pixel",
            "ipole_eval_connection", "ipole_eval_coefficients", "ipole_eval_coefficients_edf", "ipole_eval_stokes_step", "ipole_eval_bessel",
@@ -54,7 +54,7 @@ class Stats(C.Structure):
                 ("n_maxstep", C.c_int64), ("n_long", C.c_int64), ("n_batches", C.c_int32), ("n_launches", C.c_int32),
                 ("ms_probe", C.c_float), ("ms_geodesic", C.c_float), ("ms_transfer", C.c_float), ("ms_total", C.c_float),
                 ("ms_long", C.c_float), ("total_steps_forward", C.c_int64), ("ms_stepop", C.c_float), ("ms_apply", C.c_float), ("n_retry", C.c_int64),
-                ("n_lanes", C.c_int32), ("reserved_", C.c_int32)]
+                ("n_lanes", C.c_int32), ("plan_reused", C.c_int32)]
 
 
 class Edf(C.Structure):
@@ -93,6 +93,7 @@ def lib():
         L.ipole_set_unpolarized.argtypes = [vp, C.c_int32]
         L.ipole_set_transfer_split.argtypes = [vp, C.c_int32]
         L.ipole_set_batch_overlap.argtypes = [vp, C.c_int32]
+        L.ipole_set_plan_reuse.argtypes = [vp, C.c_int32]
         L.ipole_image_totals_static.argtypes = [vp, C.c_int64, vp, vp, vp, vp, vp]
         L.ipole_set_geodesic_fp32.argtypes = [vp, C.c_int32]
         L.ipole_set_edf.argtypes = [vp, C.POINTER(Edf)]
@@ -196,6 +197,11 @@ class Ipole:
     def set_geodesic_fp32(self, on=True):
         """FP32 study switch (include/ipole.h ipole_set_geodesic_fp32): geodesics in single precision."""
         _chk(lib().ipole_set_geodesic_fp32(self._h, 1 if on else 0), "ipole_set_geodesic_fp32")
+
+    def set_plan_reuse(self, on=True):
+        """Schedule an image from the previous call's plan when camera and options are unchanged: the call then does not
+        block (include/ipole.h ipole_set_plan_reuse)."""
+        _chk(lib().ipole_set_plan_reuse(self._h, int(on)), "ipole_set_plan_reuse")
 
     def set_batch_overlap(self, on=True):
         """Consecutive batches side by side on two streams (include/ipole.h ipole_set_batch_overlap)."""

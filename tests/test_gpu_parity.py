@@ -233,6 +233,59 @@ def test_split_transfer_matches_the_single_kernel(ipole):
         assert np.array_equal(one[k], five[k]), k    # the long-ray pass is the single kernel
 
 
+def test_plan_reuse_is_bit_neutral_and_follows_camera_model_and_calls(ipole):
+    """ipole_set_plan_reuse: a full image scheduled from the previous call's plan (no probe, no read-back, retried and long
+    rays from the recorded lists) is the image the planning call makes, bit for bit; the plan follows the camera and is
+    dropped by any other call in between; the model may change under it."""
+    def fresh(cam, adaf, budget):
+        f = ipole.Ipole(**cam); f.load_adaf(**adaf); f.set_plan_reuse(False); f.set_options(budget, 2)
+        img = to_np(f.make_image(maps=True)); ns, nt = f.ray_info(); st = f.stats()
+        assert st["plan_reused"] == 0
+        f.close()
+        return img, ns, nt, st
+
+    def same(a, b):
+        for k in a:
+            assert np.array_equal(a[k], b[k]), k
+
+    for n, budget in ((256, 1 << 30), (96, 0)):       # many batches on two lanes + retries + long rays; one batch
+        cam = W.camera("adaf", n)
+        g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF); g.set_options(budget, 2)
+        a = to_np(g.make_image(maps=True)); nsa, nta = g.ray_info(); sta = g.stats()
+        assert sta["plan_reused"] == 0 and sta["ms_probe"] > 0
+        b = to_np(g.make_image(maps=True)); nsb, ntb = g.ray_info(); stb = g.stats()
+        assert stb["plan_reused"] == 1 and stb["ms_probe"] == 0
+        same(a, b)
+        assert np.array_equal(nsa, nsb) and np.array_equal(nta, ntb)
+        for k in ("total_steps", "n_long", "n_retry", "n_batches", "n_ring", "flux_jy", "path_cap"):
+            assert sta[k] == stb[k], k
+        if budget:
+            assert sta["n_batches"] > 3 and sta["n_lanes"] == 2 and sta["n_long"] + sta["n_retry"] > 0
+        # another model under the same plan
+        other = dict(W.ADAF); other["n0"] = 0.4 * W.ADAF["n0"]; other["Th0"] = 1.5 * W.ADAF["Th0"]
+        g.load_adaf(**other)
+        c1 = to_np(g.make_image(maps=True)); st = g.stats()
+        assert st["plan_reused"] == 1
+        want, ns, nt, _ = fresh(cam, other, budget)
+        same(c1, want)
+        assert np.array_equal(g.ray_info()[0], ns)
+        # another camera: planned afresh, then reused again
+        cam2 = W.camera("adaf", n, inclination_deg=35.0)
+        g.set_camera(**cam2)
+        d1 = to_np(g.make_image(maps=True)); assert g.stats()["plan_reused"] == 0
+        d2 = to_np(g.make_image(maps=True)); assert g.stats()["plan_reused"] == 1
+        want, ns, nt, _ = fresh(cam2, other, budget)
+        same(d1, want); same(d2, want)
+        # a pixel-list call in between drops the plan; so does the switch
+        g.make_pixels(np.arange(0, n * n, 7, dtype=np.int64))
+        e1 = to_np(g.make_image(maps=True)); assert g.stats()["plan_reused"] == 0
+        same(e1, want)
+        g.set_plan_reuse(False)
+        e2 = to_np(g.make_image(maps=True)); assert g.stats()["plan_reused"] == 0
+        same(e2, want)
+        g.close()
+
+
 def test_step_limit_flags_rays(ipole, ref):
     cam = W.camera("adaf", 16, max_steps=900)
     g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
@@ -386,6 +439,12 @@ def test_w5_adaf_4096_sampled(ipole, ref):
     info = check_parity(got, want, "W5 adaf", min_lit=0.99)
     report("W5 adaf 4096^2", pix.size, info)
     st = g.stats()
+    # the images bench.py times are scheduled from the plan of the call before them (ipole_set_plan_reuse): same bits
+    again = g.make_image(maps=False)
+    assert g.stats()["plan_reused"] == 1 and st["plan_reused"] == 0
+    for k in img:
+        assert bool((again[k] == img[k]).all()), k
+    del again
     assert st["n_batches"] >= 1 and st["n_maxstep"] == 0
     # properties of the whole 4096^2 image
     import torch
@@ -419,6 +478,10 @@ def test_w5_grid_4096_sampled(ipole, ref, big_grid):
     r = ref.Ctx(**cam); r.load_grid(desc, fields)
     pix = sample_pixels(4096, 4096, 16, window=(2240, 1984, 512, 128))
     want = r.make_pixels(pix, nthreads=NTHREADS)
-    got, _ = gpu_full_then_sample(g, pix, maps=False)
+    got, img = gpu_full_then_sample(g, pix, maps=False)
     info = check_parity(got, want, "W5 grid", min_lit=0.3)
     report("W5 grid 4096^2", pix.size, info)
+    again = g.make_image(maps=False)          # scheduled from the recorded plan, as the images bench.py times
+    assert g.stats()["plan_reused"] == 1
+    for k in img:
+        assert bool((again[k] == img[k]).all()), k
