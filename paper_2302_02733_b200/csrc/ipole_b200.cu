@@ -369,6 +369,15 @@ int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_
   if (pf == 0 && c->model == MODEL_GRID && c->opt_group && !a.slots) {
     // warp-level scheduling: one warp per 32 consecutive rays (kernels.cuh, k_transfer_group)
     const int gg = grid_for(c, c->occ_group, IPOLE_RT_THREADS / 32, (rays + 31) / 32, reserve);
+    if (c->opt_rank && a.srange && rays > 32) {
+      // the 32 rays of a group walk in lockstep from the group's first plasma contact: windows of 1024 slots are ranked by
+      // each ray's contact range, known since k_geodesic<true> (the side stream has its own half of the two arrays)
+      const size_t off = (st == c->side) ? (size_t)c->ray_cap : 0;
+      RankArgs r = {a.base, a.count, a.count_dev, a.order, a.nsteps, c->d_rank_pos + off, c->d_rank_slot + off, a.srange};
+      k_rank_window<<<(unsigned)((rays + RANK_WINDOW - 1) / RANK_WINDOW), RANK_WINDOW, 0, st>>>(r);
+      c->stats.n_launches++;
+      a.rank_slot = c->d_rank_slot + off;
+    }
     k_transfer_group<MODEL_GRID><<<gg, IPOLE_RT_THREADS, 0, st>>>(a);
     span_end(c, s, st);
     c->stats.n_launches++;
@@ -402,7 +411,7 @@ int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStrea
   int32_t* rank_pos = c->d_rank_pos + (on_side ? c->ray_cap : 0);     // (the side-stream retry indexes from 0 like a bulk batch)
   int32_t* rank_slot = c->d_rank_slot + (on_side ? c->ray_cap : 0);
   if (rank) {
-    RankArgs r = {a.base, a.count, a.count_dev, a.order, a.nsteps, rank_pos, rank_slot};
+    RankArgs r = {a.base, a.count, a.count_dev, a.order, a.nsteps, rank_pos, rank_slot, nullptr};
     const int s = span_begin(c, on_side ? LK_LONG : LK_OPS, st);
     k_rank_window<<<(unsigned)((rays + RANK_WINDOW - 1) / RANK_WINDOW), RANK_WINDOW, 0, st>>>(r);
     span_end(c, s, st);

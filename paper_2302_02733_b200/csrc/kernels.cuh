@@ -315,6 +315,7 @@ struct RtArgs {
   unsigned long long* queue;
   double *I, *Q, *U, *V, *tau, *tauF;   // indexed by q
   const int2* srange;         // grid model, stored path: steps that may cross plasma (from k_geodesic<true>; nullable)
+  const int32_t* rank_slot;   // k_transfer_group: [base + a] = the slot of the batch that takes place a of its groups (k_rank_window; nullable)
   // path-free variant (PF != 0): no path; the ray restarts from the end point of its backward pass
   const double* endp;         // [total rays][8], indexed by q
   int32_t* nfwd;              // [total rays] steps of the forward pass (nullable)
@@ -556,7 +557,8 @@ __global__ void __launch_bounds__(IPOLE_RT_THREADS, IPOLE_RT_MINB) k_transfer_gr
     int s0 = -1, s_lo = 0;       // this lane walks steps s0 ... 0; -1: nothing to walk
     bool lit = false;
     if (li < count) {
-      q = A.order ? A.order[A.base + li] : (int32_t)(A.base + li);
+      const int64_t ls = A.rank_slot ? (int64_t)A.rank_slot[A.base + li] : li;    // this lane's slot in the batch
+      q = A.order ? A.order[A.base + ls] : (int32_t)(A.base + ls);
       int n = A.nsteps[q];
       if (n >= 0) {              // (n < 0: overflowed its slot, done by the long-ray pass)
         if (MODEL == MODEL_GRID && A.srange) {
@@ -570,7 +572,7 @@ __global__ void __launch_bounds__(IPOLE_RT_THREADS, IPOLE_RT_MINB) k_transfer_gr
           } else n = r.x + 1;    // start at the first contact with plasma
         }
         if (n > 0) {
-          rec = A.path + (size_t)li * slot_doubles;
+          rec = A.path + (size_t)ls * slot_doubles;
           double dl;
           load_record(rec + (size_t)n * REC_DOUBLES, Xhi, Khi, dl);
           s0 = n - 1;

@@ -59,8 +59,12 @@ struct OpArgs {
 // k_apply walks 32 rays in lockstep, so the rays of a group should be equally long.  The batch is in order of PREDICTED
 // length (probe pass); once k_geodesic has run the true step counts are known, and every window of RANK_WINDOW consecutive
 // slots is re-ranked by them: pos[base + li] = the place of slot li's operator records, slot[base + a] = the slot at place a.
+// The grid model's lockstep kernel (k_transfer_group) uses the same ranking on each ray's plasma-contact range.
 constexpr int RANK_WINDOW = 1024;
-struct RankArgs { int64_t base, count; const int* count_dev; const int32_t* order; const int32_t* nsteps; int32_t* pos; int32_t* slot; };
+struct RankArgs {
+  int64_t base, count; const int* count_dev; const int32_t* order; const int32_t* nsteps; int32_t* pos; int32_t* slot;
+  const int2* srange;         // grid model (k_transfer_group): rank by the plasma-contact range instead (first contact, then last)
+};
 __global__ void __launch_bounds__(RANK_WINDOW) k_rank_window(RankArgs A) {
   __shared__ unsigned long long key[RANK_WINDOW];
   const int64_t count = A.count_dev ? (int64_t)*A.count_dev : A.count;
@@ -70,9 +74,12 @@ __global__ void __launch_bounds__(RANK_WINDOW) k_rank_window(RankArgs A) {
   unsigned long long k = ~0ULL;                  // padding sorts last
   if (w0 + t < count) {
     const int32_t q = A.order ? A.order[A.base + w0 + t] : (int32_t)(A.base + w0 + t);
-    int n = A.nsteps[q];
+    int n = A.nsteps[q], lo = 0;
     if (n < 0) n = 0;
-    k = ((unsigned long long)(0x7fffffff - n) << 32) | (unsigned)t;   // longest first, then by slot: a fixed order
+    else if (A.srange) { const int2 r = A.srange[q]; n = r.x + 1; lo = r.y; }   // steps the walk takes; where the plasma ends
+    n = min(n, 0x1fffff); lo = min(max(lo, 0), 0x1fffff);
+    // longest first, then by the second key, then by slot: a fixed order
+    k = ((unsigned long long)(0x1fffff - n) << 31) | ((unsigned long long)lo << 10) | (unsigned)t;
   }
   key[t] = k;
   __syncthreads();
@@ -87,7 +94,7 @@ __global__ void __launch_bounds__(RANK_WINDOW) k_rank_window(RankArgs A) {
       __syncthreads();
     }
   if (w0 + t < count) {
-    const int src = (int)(key[t] & 0xffffffffULL);
+    const int src = (int)(key[t] & 1023ULL);
     A.slot[A.base + w0 + t] = (int32_t)(w0 + src);
     A.pos[A.base + w0 + src] = (int32_t)(w0 + t);
   }
