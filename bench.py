@@ -514,6 +514,7 @@ def measure_image(args, name, ipole, replicas, W, world, rank, local, barrier):
     st = g.stats()  # of the last timed image (event times are per image)
     st_live = st
     st_plan = st
+    host_idle = None
     if st.get("n_lanes", 1) == 2 or st.get("plan_reused", 0):
         # The timed images ran with consecutive batches side by side on two streams (ipole_set_batch_overlap): the event
         # spans of concurrent kernels overlap, so the per-kernel times come from one more image with the lanes off.  The
@@ -523,7 +524,9 @@ def measure_image(args, name, ipole, replicas, W, world, rank, local, barrier):
         g.make_image(maps=maps, out=out)
         torch.cuda.synchronize()
         st_plan = g.stats()
+        th = time.perf_counter()
         g.make_image(maps=maps, out=out)
+        host_idle = time.perf_counter() - th      # a reused-plan call into an empty launch queue
         torch.cuda.synchronize()
         st = g.stats()
         g.set_batch_overlap(True)
@@ -633,6 +636,28 @@ def measure_image(args, name, ipole, replicas, W, world, rank, local, barrier):
                           "geodesic_fp64_pipe_pct": FP64_PIPE_PCT[gk]}
     path_bytes = 0.0 if pf else (256.0 if split else 128.0)
     roof["hbm_path_gbs"] = path_bytes * st["total_steps"] / ((st["ms_geodesic"] + st["ms_transfer"]) * 1e-3) / 1e9
+    # The roofline object describes the DOMINANT kernel.  Stored path: the geodesic kernel is one launch per batch like the
+    # transfer stage; where it takes the larger share of the image (the grid model: k_geodesic<occ>) it becomes the
+    # top-level entry and the transfer stage moves to roofline.other_stage, else the other way round.
+    if not (pf or args.unpolarized or args.edf):
+        gms = st["ms_geodesic"]
+        gach = FLOP_PER_STEP[gkey] * st["total_steps"] / (gms * 1e-3) / 1e12
+        geo = {"bound": "alu", "kernel": "k_geodesic<true> (h != 1, stencil-occupancy test)" if wl["kind"] == "grid" else "k_geodesic<false>",
+               "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "launches": n_rt, "avg_launch_ms": gms / n_rt,
+               "kernel_share_of_step": gms / st["ms_total"], "steps_per_launch": st["total_steps"] / n_rt,
+               "traffic": 64.0 * st["total_steps"] / n_rt,
+               "traffic_note": "ncu dram__bytes_write per step (64.0-64.1 B: one path record, profiles/r2_k_geodesic_*.txt) x steps of a batch; algorithmic: the same 64 B",
+               "achieved": gach, "frac": gach / FP64_PEAK_TFLOPS, "flop_per_step_algorithmic": FLOP_PER_STEP[gkey],
+               "flop_per_step_executed": FLOP_EXECUTED[gk],
+               "frac_executed": FLOP_EXECUTED[gk] * st["total_steps"] / (gms * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+               "fp64_pipe_pct": FP64_PIPE_PCT[gk]}
+        if gms > rt_ms:
+            for k in ("peak_source", "flop_note", "whole_step", "hbm_path_gbs"):
+                geo[k] = roof.pop(k)
+            geo["other_stage"] = roof
+            roof = geo
+        else:
+            roof["other_stage"] = geo
 
     line = {"metric": "rays_per_s", "value": value, "unit": "rays/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -662,10 +687,13 @@ def measure_image(args, name, ipole, replicas, W, world, rank, local, barrier):
             "flux_jy": st["flux_jy"], "lp": st["lp"], "cp": st["cp"], "ring_rays": st["n_ring"],
             "gpu_launches": st_live["n_launches"] * args.steps, "roofline": roof, "e2e": e2e, "clocks": clocks,
             "plan": {"reused": bool(st_live.get("plan_reused", 0)), "host_ms_per_call": host_s * 1e3 / args.steps,
+                     "host_ms_per_call_idle_queue": None if host_idle is None else host_idle * 1e3,
                      "planning_call": planning,
                      "note": "the timed images are scheduled from the plan of the call before them (ipole_set_plan_reuse: same camera, no "
                              "probe pass, no host-device synchronisation; the call returns after host_ms_per_call while the GPU works for "
-                             "ms_per_step); planning_call = one image planned afresh (probe pass, read-backs, blocking), as the first "
+                             "ms_per_step -- in this back-to-back loop that includes waiting for room in the driver's launch queue when "
+                             "several images of some 400 launches each are pending; host_ms_per_call_idle_queue is one such call after a "
+                             "synchronise); planning_call = one image planned afresh (probe pass, read-backs, blocking), as the first "
                              "call for a camera is; stage_ms.probe_sort is that call's probe time and is not part of a reused image"},
             "paper_context": {"note": "paper Table 1, other model/hardware (A100): context only",
                               "a100_semianalytic_4096_rays_per_s": 127583, "a100_grmhd_4096_rays_per_s": 188720}}
