@@ -26,7 +26,7 @@
 namespace ipole {
 
 #ifndef IPOLE_EDF_UNROLL
-#define IPOLE_EDF_UNROLL 4
+#define IPOLE_EDF_UNROLL 8
 #endif
 constexpr int EDF_UNROLL = IPOLE_EDF_UNROLL;
 constexpr double EDF_LNX_LO = -16.0, EDF_LNX_HI = 4.0;
@@ -69,8 +69,9 @@ __device__ __forceinline__ void synch_kernels_scaled(const double* __restrict__ 
 }
 
 // g(gamma) and L = -dln g/dgamma at gamma - 1 = gm1
+template <int KIND>
 __device__ __forceinline__ void edf_shape(const EdfDev& E, double iTh, double ikw, double gm1, double& g, double& L) {
-  if (E.kind == 1) { g = ip_exp(-gm1 * iTh); L = iTh; }
+  if (KIND == 1) { g = ip_exp(-gm1 * iTh); L = iTh; }
   else {
     const double q = fma(gm1, ikw, 1.0);
     const double kp1 = E.kappa + 1.0;
@@ -122,6 +123,34 @@ __device__ __forceinline__ double edf_lnnorm(const EdfDev& E, double Th) {
   return w0 * f0 + w1 * f1 + w2 * f2 + w3 * f3;
 }
 
+// The node sums.  KIND is a template parameter so that the loop body holds no branch at all: the unrolled iterations then
+// sit in one basic block and their reciprocal -> reciprocal square root -> exponential chains interleave.
+template <int KIND>
+__device__ __forceinline__ void edf_node_sums(const EdfDev& E, const double4* __restrict__ nodes, double sx, double iTh, double ikw,
+                                              double& sI, double& sQ, double& sV, double& aI, double& aQ, double& aV) {
+#pragma unroll EDF_UNROLL
+  for (int k = 0; k < E.n_nodes; ++k) {
+    const double4 nd = nodes[k];
+    const double gam0 = sx * nd.x;
+    const bool on = gam0 > 1.0;                        // cells below gamma = 1 carry no electrons (branch-free: the
+    const double gam = on ? gam0 : 2.0;                // iterations of the unrolled loop interleave)
+    const double ig = ip_rcp(gam), ig2 = ig * ig;
+    const double b2 = 1.0 - ig2;
+    const double ibeta = ip_rsqrt(b2), beta = b2 * ibeta;
+    const double dbeta = ig2 * ig * ibeta;
+    double g, L;
+    edf_shape<KIND>(E, iTh, ikw, gam - 1.0, g, L);
+    const double g3 = on ? gam * gam * gam * g : 0.0;             // gamma^3 g: n/N times the varying part of the cell width, over beta
+    const double A1 = g3 * beta, A2 = g3 * (dbeta - beta * L);
+    sI = fma(A1, nd.y, sI);
+    sQ = fma(A1, nd.z, sQ);
+    sV = fma(A1 * ig, nd.w, sV);
+    aI = fma(A2, nd.y, aI);
+    aQ = fma(A2, nd.z, aQ);
+    aV = fma(A2 * ig, nd.w, aV);
+  }
+}
+
 // plasma-frame cgs j_{I,Q,V}, alpha_{I,Q,V} into c (rho_Q, rho_V untouched).  `nodes`: E.nodes or a copy in shared memory.
 __device__ __forceinline__ void synchrotron_edf_cgs(const EdfDev& E, const double4* __restrict__ nodes,
                                                     double ne, double Th, double B, double cosT, double nu, Coeff& c) {
@@ -134,27 +163,8 @@ __device__ __forceinline__ void synchrotron_edf_cgs(const EdfDev& E, const doubl
   const double iTh = ip_rcp(Th);
   const double ikw = ip_rcp(E.kappa * Th);
   double sI = 0.0, sQ = 0.0, sV = 0.0, aI = 0.0, aQ = 0.0, aV = 0.0;
-#pragma unroll EDF_UNROLL
-  for (int k = 0; k < E.n_nodes; ++k) {
-    const double4 nd = nodes[k];
-    const double gam0 = sx * nd.x;
-    const bool on = gam0 > 1.0;                        // cells below gamma = 1 carry no electrons (branch-free: the
-    const double gam = on ? gam0 : 2.0;                // iterations of the unrolled loop interleave)
-    const double ig = ip_rcp(gam), ig2 = ig * ig;
-    const double b2 = 1.0 - ig2;
-    const double ibeta = ip_rsqrt(b2), beta = b2 * ibeta;
-    const double dbeta = ig2 * ig * ibeta;
-    double g, L;
-    edf_shape(E, iTh, ikw, gam - 1.0, g, L);
-    const double g3 = on ? gam * gam * gam * g : 0.0;             // gamma^3 g: n/N times the varying part of the cell width, over beta
-    const double A1 = g3 * beta, A2 = g3 * (dbeta - beta * L);
-    sI = fma(A1, nd.y, sI);
-    sQ = fma(A1, nd.z, sQ);
-    sV = fma(A1 * ig, nd.w, sV);
-    aI = fma(A2, nd.y, aI);
-    aQ = fma(A2, nd.z, aQ);
-    aV = fma(A2 * ig, nd.w, aV);
-  }
+  if (E.kind == 1) edf_node_sums<1>(E, nodes, sx, iTh, ikw, sI, sQ, sV, aI, aQ, aV);
+  else edf_node_sums<2>(E, nodes, sx, iTh, ikw, sI, sQ, sV, aI, aQ, aV);
   const double C = (IP_SQRT3 * IP_EE * IP_EE * IP_EE / (4.0 * M_PI * IP_ME * IP_CL * IP_CL)) * B * sinT;
   const double Nn = ne * ip_exp(-edf_lnnorm(E, Th)) * (0.5 * E.dlx);   // N times the constant part of the cell width
   const double cot43 = (4.0 / 3.0) * cosT * isinT;

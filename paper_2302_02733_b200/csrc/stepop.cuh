@@ -262,8 +262,10 @@ __device__ __noinline__ Stokes4 stokes_step_qv_closed(double aI, double aQ, doub
 // the 32 rays of a group have similar lengths.  The record of the next step is loaded (three coalesced 256-bit loads)
 // while the current one is applied.
 // EDF: the coefficients of a step by numerical integration over the electron distribution function (edf.cuh)
+// (2 blocks per SM: the node loop, unrolled 8 times with no branch in its body, wants ~220 registers to keep eight
+// reciprocal -> rsqrt -> exp chains in flight; measured faster than 3 blocks at 164, profiles/r2_notes.md)
 #ifndef IPOLE_AP_EDF_MINB
-#define IPOLE_AP_EDF_MINB 3
+#define IPOLE_AP_EDF_MINB 2
 #endif
 template <bool EDF>
 __global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? IPOLE_AP_EDF_MINB : IPOLE_AP_MINB) k_apply(const __grid_constant__ ApArgs A) {
