@@ -35,9 +35,9 @@ FLOP_PER_STEP = {"transfer_adaf": 1576.0, "transfer_grid": 390.0, "geodesic_adaf
 FLOP_EXECUTED = {"k_stepop": 1019.0, "k_apply": 578.0, "k_transfer<adaf>": 1576.0, "k_transfer_group<grid>": 397.0,
                  "k_geodesic": 839.0, "k_geodesic<occ>": 1020.0}
 # second physics workload (--edf): k_apply<true> per step, 128 quadrature nodes (profiles/r2_k_apply_edf{1,2}_adaf256.txt)
-FLOP_EXECUTED.update({"k_apply<edf 1>": 11383.0, "k_apply<edf 2>": 18268.0})
+FLOP_EXECUTED.update({"k_apply<edf 1>": 11558.0, "k_apply<edf 2>": 18290.0})
 FP64_PIPE_PCT = {"k_stepop": 72.6, "k_apply": 61.7, "k_transfer<adaf>": 58.5, "k_transfer_group<grid>": 50.6,
-                 "k_geodesic": 82.5, "k_geodesic<occ>": 79.5, "k_apply<edf 1>": 55.9, "k_apply<edf 2>": 55.2}
+                 "k_geodesic": 82.5, "k_geodesic<occ>": 79.5, "k_apply<edf 1>": 75.4, "k_apply<edf 2>": 70.1}
 # DRAM bytes per step of k_transfer (dram__bytes_read + write of one launch / its thread-steps, same captures)
 DRAM_BYTES_PER_STEP = {"transfer_adaf": 64.2, "transfer_grid": 37.2}
 DRAM_BYTES_PER_STEP_SPLIT = 192.0   # k_stepop reads 64.1 B and writes 64.0 B per step, k_apply reads 64.0 B (profiles/r2_k_*.txt)
