@@ -122,6 +122,7 @@ struct ipole_ctx {
     int32_t* d_long = nullptr; int32_t* d_retry = nullptr; int long_cap = 0, retry_cap = 0;   // the two lists as that call left them
   } plan_cache;
   int opt_plan_reuse = 1;
+  int opt_lowlat = 1;            // under-filled launches: kernels built for single-ray latency (IPOLE_NO_LOWLAT=1 turns it off)
 
   double* totals_scratch = nullptr;   // device address of g_totals_scratch on this context's device (ipole_image_totals_static)
   int totals_scratch_err = 0;         // cudaError_t of the look-up, if it failed
@@ -295,8 +296,17 @@ int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays, cudaStream
   } else if (c->n_mc) {
     a.cams = c->d_mc_cams; a.rays_per_cam = c->mc_rays_per_cam;
     k_geodesic<false, true><<<grid_for(c, c->occ_geo_mc, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
-  } else if (a.grid) k_geodesic<true><<<grid_for(c, c->occ_geo_occ, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
-  else k_geodesic<false><<<grid_for(c, c->occ_geo, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
+  } else {
+    // a launch that leaves the GPU part empty whatever the kernel: the build that is fastest for a lone ray (kernels.cuh, LOWLAT)
+    const bool lowlat = c->opt_lowlat && rays <= (int64_t)c->n_sm * IPOLE_GEO_THREADS * 2;
+    if (a.grid) {
+      if (lowlat) k_geodesic<true, false, true><<<grid_for(c, 2, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
+      else k_geodesic<true><<<grid_for(c, c->occ_geo_occ, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
+    } else {
+      if (lowlat) k_geodesic<false, false, true><<<grid_for(c, 2, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
+      else k_geodesic<false><<<grid_for(c, c->occ_geo, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
+    }
+  }
   span_end(c, s, st);
   c->stats.n_launches++;
   CK(cudaGetLastError());
@@ -1013,6 +1023,7 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   { const char* e = std::getenv("IPOLE_NO_GROUP"); if (e && e[0] == '1') c->opt_group = 0; }
   { const char* e = std::getenv("IPOLE_NO_OVERLAP"); if (e && e[0] == '1') c->opt_overlap = 0; }
   { const char* e = std::getenv("IPOLE_NO_PLAN_REUSE"); if (e && e[0] == '1') c->opt_plan_reuse = 0; }
+  { const char* e = std::getenv("IPOLE_NO_LOWLAT"); if (e && e[0] == '1') c->opt_lowlat = 0; }
   { const char* e = std::getenv("IPOLE_NO_RANK"); if (e && e[0] == '1') c->opt_rank = 0; }
   { const char* e = std::getenv("IPOLE_NO_SIDE_RETRY"); if (e && e[0] == '1') c->opt_side_retry = 0; }
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_group, k_transfer_group<MODEL_GRID>, IPOLE_RT_THREADS, 0);

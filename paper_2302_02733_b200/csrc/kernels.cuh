@@ -214,8 +214,13 @@ __device__ __forceinline__ void load_record(const double* rec, double X[4], doub
 // MC (many cameras per launch: a fit that varies inclination or spin): the geometry and the stop radii are
 // per-lane values taken from the ray's own camera at refill; the single-camera instantiation keeps them in the
 // constant bank.
-template <bool OCC, bool MC = false>
-__global__ void __launch_bounds__(IPOLE_GEO_THREADS, MC ? 3 : IPOLE_GEO_MINB) k_geodesic(const __grid_constant__ GeoArgs A) {
+//
+// LOWLAT: the same code compiled for 2 blocks per SM (180 registers instead of 128).  ptxas then keeps more independent
+// operations in flight per thread, which is worth nothing when the SM is full (the 4-block build wins a 4096^2 image by
+// 3-10 %) but shortens the dependent chain of a LONE ray: launches that cannot fill the GPU anyway -- long-ray and retry
+// passes, probe passes, the levels of an adaptive image, small images -- take it (profiles/r2_notes.md).  Same arithmetic.
+template <bool OCC, bool MC = false, bool LOWLAT = false>
+__global__ void __launch_bounds__(IPOLE_GEO_THREADS, LOWLAT ? 2 : (MC ? 3 : IPOLE_GEO_MINB)) k_geodesic(const __grid_constant__ GeoArgs A) {
   const CamDev& C = A.cam;
   Geom Gl = C.G;                      // MC: the lane's own
   double lx_in_l = C.lx_in, lx_esc_l = C.lx_esc;

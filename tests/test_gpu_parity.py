@@ -415,6 +415,30 @@ def test_grid_plasma_contact_range_is_bit_neutral(ipole, small_grid, monkeypatch
     assert (base["I"] == 0).any() and (base["I"] > 0).any()   # dark rays (never walked) and lit ones
 
 
+def test_low_latency_geodesic_build_is_bit_neutral(ipole, small_grid, monkeypatch):
+    """Launches that cannot fill the GPU use k_geodesic compiled for 2 blocks per SM (kernels.cuh, LOWLAT): the same path
+    records, step counts and images as the 4-block build (IPOLE_NO_LOWLAT=1), for both flows."""
+    desc, fields = small_grid
+    for kind in ("adaf", "grid"):
+        cam = W.camera(kind, 96)                       # 9216 rays: every launch is under-filled
+        outs = []
+        for off in (True, False):
+            if off:
+                monkeypatch.setenv("IPOLE_NO_LOWLAT", "1")
+            g = ipole.Ipole(**cam)
+            if off:
+                monkeypatch.delenv("IPOLE_NO_LOWLAT")
+            g.load_adaf(**W.ADAF) if kind == "adaf" else g.load_grid(desc, fields)
+            img = to_np(g.make_image(maps=True)); ns, nt = g.ray_info()
+            outs.append((img, ns.copy(), nt.copy(), g.stats()))
+            g.close()
+        (a, nsa, nta, sa), (b, nsb, ntb, sb) = outs
+        for k in a:
+            assert np.array_equal(a[k], b[k]), (kind, k)
+        assert np.array_equal(nsa, nsb) and np.array_equal(nta, ntb)
+        assert sa["total_steps"] == sb["total_steps"] and sa["flux_jy"] == sb["flux_jy"]
+
+
 def test_w3_grid_256_sampled(ipole, ref):
     desc, fields = W.fm_torus_grid(288, 128, 128)
     cam = W.camera("grid", 256)
