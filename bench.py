@@ -62,6 +62,8 @@ WORKLOADS = {
     "gridsweep128": dict(kind="grid", n=128, config=None, sweep=64, grid=(288, 128, 128)),
     # small images whose GEOMETRY differs (inclination, spin): one ipole_make_images_cameras call over the union of their rays
     "cams128": dict(kind="adaf", n=128, config=None, cams=64),
+    # the same for the grid model: one snapshot seen from 64 directions at three frequencies (spin and mass are the grid's)
+    "gridcams128": dict(kind="grid", n=128, config=None, cams=64, grid=(288, 128, 128)),
 }
 
 
@@ -287,10 +289,22 @@ def run_cams(args, ipole, replicas, W, wl, world, rank, local, barrier):
     import torch
     n, nc = wl["n"], wl["cams"]
     incl = [15.0 + 150.0 * k / max(1, nc - 1) for k in range(nc)]
-    spins = [0.0, 0.5, 0.9375, 0.99]
-    cams = [W.camera("adaf", n, inclination_deg=a, spin=spins[k % 4]) for k, a in enumerate(incl)]
+    grid = wl["kind"] == "grid"
+    if grid:   # a grid belongs to one spacetime: its cameras vary direction and frequency
+        spins = [W.camera("grid", n)["spin"]]
+        freqs = [230e9, 345e9, 86e9]
+        cams = [W.camera("grid", n, inclination_deg=a, freq_hz=freqs[k % 3]) for k, a in enumerate(incl)]
+    else:
+        spins = [0.0, 0.5, 0.9375, 0.99]
+        freqs = [230e9]
+        cams = [W.camera("adaf", n, inclination_deg=a, spin=spins[k % 4]) for k, a in enumerate(incl)]
     names = ["I", "Q", "U", "V"]
-    g = ipole.Ipole(**cams[0]); g.load_adaf(**W.ADAF)
+    g = ipole.Ipole(**cams[0])
+    if grid:
+        desc, fields = grid_inputs(tuple(wl["grid"]))
+        g.load_grid(desc, fields)
+    else:
+        g.load_adaf(**W.ADAF)
     g.set_stream(torch.cuda.current_stream())
     out = {k: torch.empty((nc, n, n), dtype=torch.float64, device="cuda") for k in names}
     single = {k: torch.empty((n, n), dtype=torch.float64, device="cuda") for k in names}
@@ -335,12 +349,12 @@ def run_cams(args, ipole, replicas, W, wl, world, rank, local, barrier):
     if rank != 0:
         return
     rays = nc * n * n
-    fl = FLOP_PER_STEP["transfer_adaf"]
+    fl = FLOP_PER_STEP["transfer_grid" if grid else "transfer_adaf"]
     line = {"metric": "rays_per_s", "value": world * rays / res["batched"], "unit": "rays/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": res["batched"] * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.workload, "image": "%dx%d" % (n, n), "cameras": nc, "inclinations_deg": [incl[0], incl[-1]],
-                       "spins": spins, "model": "adaf", "freq_ghz": 230, "full_stokes": True,
+                       "spins": spins, "model": wl["kind"], "freq_ghz": [f / 1e9 for f in freqs], "full_stokes": True,
                        "timing": "CUDA events around ipole_make_images_cameras from one host thread, one context",
                        "l2": "no flush needed: each call streams %.1f GB of path and operator records" % (st["total_steps"] * 128 / 1e9),
                        "parallelism": "single GPU"},
@@ -350,10 +364,11 @@ def run_cams(args, ipole, replicas, W, wl, world, rank, local, barrier):
             "stage_ms": {"probe_sort": st["ms_probe"], "geodesic": st["ms_geodesic"], "transfer": st["ms_transfer"], "stepop": st["ms_stepop"],
                          "apply": st["ms_apply"], "total": st["ms_total"], "batches": st["n_batches"]},
             "gpu_launches": st["n_launches"] * args.steps,
-            "roofline": {"bound": "alu", "kernel": "k_stepop<adaf, cameras> + k_apply", "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+            "roofline": {"bound": "alu", "kernel": "k_transfer_group<grid, cameras>" if grid else "k_stepop<adaf, cameras> + k_apply", "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                          "achieved": fl * st["total_steps"] / (st["ms_transfer"] * 1e-3) / 1e12,
                          "frac": fl * st["total_steps"] / (st["ms_transfer"] * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
-                         "flop_per_step_algorithmic": fl, "traffic": DRAM_BYTES_PER_STEP_SPLIT * st["total_steps"] / max(1, st["n_batches"])},
+                         "flop_per_step_algorithmic": fl,
+                         "traffic": (DRAM_BYTES_PER_STEP["transfer_grid"] if grid else DRAM_BYTES_PER_STEP_SPLIT) * st["total_steps"] / max(1, st["n_batches"])},
             "e2e": {"value": world * rays / dt, "unit": "rays/s", "h2d_bytes_per_step": nc * ipole.C.sizeof(ipole.Camera),
                     "d2h_bytes_per_step": 4 * rays * 8 + nc * 32}}
     print(json.dumps(line), flush=True)

@@ -241,7 +241,7 @@ typedef struct { double M_unit, Rlow, Rhigh; } ipole_grid_scales;
 int  ipole_make_images_grid(ipole_ctx*, int32_t n_models, const ipole_grid_scales* sets, const double* freq_hz,
                             double* I, double* Q, double* U, double* V, double* tau, double* tauF, double* flux_jy);
 /* Many small images whose GEOMETRY differs (the fitting loop also varies viewing angle and spin): n_cams
- * cameras seen through the analytic flow loaded in the context, all in one pass of the pipeline -- one probe and sort over
+ * cameras seen through the model loaded in the context (analytic flow or grid), all in one pass of the pipeline -- one probe and sort over
  * the union of their rays, geodesic / operator / apply launches over batches of that union -- so that 128 x 128 images
  * fill the GPU although each has only 16 k rays.  Every image is what ipole_set_camera(cams[k]) + ipole_make_image
  * would give.  The cameras may differ in spin, inclination, distance, field of view, frequency, mass, source distance,
@@ -250,8 +250,13 @@ int  ipole_make_images_grid(ipole_ctx*, int32_t n_models, const ipole_grid_scale
  * host or all device; flux_jy (nullable, host or device) is [n_cams][4].  The context's own camera and model are left
  * as they were; ipole_get_stats afterwards describes the union of the rays.  Works with ipole_set_edf; uses the split
  * transfer whatever ipole_set_transfer_split says.
- * IPOLE_ENOMODEL without a model, IPOLE_EINVAL for another model than the analytic flow, for cameras that disagree in
- * the fields above, for the path-free or unpolarized variant, mixed host/device outputs, nx*ny*n_cams > 2^31-1. */
+ * Grid model: a grid was computed in one spacetime and scaled with one mass, so its cameras must ALSO share spin, mass
+ * and hslope with the context's camera (the one the grid was loaded under); they differ in inclination, azimuth, field
+ * of view, frequency, distance and source distance.  The geodesic kernel marks plasma-contact ranges per ray as for a
+ * single camera; the lockstep transfer kernel takes frequency, length unit and the camera's transverse legs from each
+ * ray's own camera.
+ * IPOLE_ENOMODEL without a model, IPOLE_EINVAL for the slab model, for cameras that disagree in the fields above, for
+ * the path-free or unpolarized variant, mixed host/device outputs, nx*ny*n_cams > 2^31-1. */
 int  ipole_make_images_cameras(ipole_ctx*, int32_t n_cams, const ipole_camera* cams, double* I, double* Q, double* U, double* V,
                                double* tau, double* tauF, double* flux_jy);
 /* Adaptive ray tracing ("another factor of 10 with adaptive ray tracing which reduces the number of light

@@ -56,7 +56,7 @@ struct ipole_ctx {
   // many cameras per call (ipole_make_images_cameras): device arrays of n_mc cameras, null outside such a call
   CamDev* d_mc_cams = nullptr; Units* d_mc_units = nullptr; double* d_mc_nu3 = nullptr; double* d_mc_scale = nullptr;
   int mc_cap = 0; int n_mc = 0; int64_t mc_rays_per_cam = 0;
-  int occ_geo_mc = 0, occ_op_mc = 0;
+  int occ_geo_mc = 0, occ_op_mc = 0, occ_geo_occ_mc = 0, occ_group_mc = 0;
   int opt_geo_fp32 = 0;          // FP32 study (geo_f32.cuh): geodesics in single precision, transfer in FP64
   int occ_geo_f32 = 0;
   int opt_group = 1;             // grid model: transfer with warp-level scheduling (k_transfer_group)
@@ -295,7 +295,8 @@ int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays, cudaStream
     k_geodesic_f32<<<grid_for(c, c->occ_geo_f32, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
   } else if (c->n_mc) {
     a.cams = c->d_mc_cams; a.rays_per_cam = c->mc_rays_per_cam;
-    k_geodesic<false, true><<<grid_for(c, c->occ_geo_mc, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
+    if (a.grid) k_geodesic<true, true><<<grid_for(c, c->occ_geo_occ_mc, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
+    else k_geodesic<false, true><<<grid_for(c, c->occ_geo_mc, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
   } else {
     // a launch that leaves the GPU part empty whatever the kernel: the build that is fastest for a lone ray (kernels.cuh, LOWLAT)
     const bool lowlat = c->opt_lowlat && rays <= (int64_t)c->n_sm * IPOLE_GEO_THREADS * 2;
@@ -376,7 +377,7 @@ int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_
     return IPOLE_OK;
   }
   const int s = span_begin(c, kind, st);
-  if (pf == 0 && c->model == MODEL_GRID && c->opt_group && !a.slots) {
+  if (pf == 0 && c->model == MODEL_GRID && (c->opt_group || c->n_mc) && !a.slots) {
     // warp-level scheduling: one warp per 32 consecutive rays (kernels.cuh, k_transfer_group)
     const int gg = grid_for(c, c->occ_group, IPOLE_RT_THREADS / 32, (rays + 31) / 32, reserve);
     if (c->opt_rank && a.srange && rays > 32) {
@@ -388,7 +389,10 @@ int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_
       c->stats.n_launches++;
       a.rank_slot = c->d_rank_slot + off;
     }
-    k_transfer_group<MODEL_GRID><<<gg, IPOLE_RT_THREADS, 0, st>>>(a);
+    if (c->n_mc) {   // many cameras per call: the lanes take frequency, units and camera legs from their ray's camera
+      a.cams = c->d_mc_cams; a.units_arr = c->d_mc_units; a.rays_per_cam = c->mc_rays_per_cam;
+      k_transfer_group<MODEL_GRID, true><<<grid_for(c, c->occ_group_mc, IPOLE_RT_THREADS / 32, (rays + 31) / 32, reserve), IPOLE_RT_THREADS, 0, st>>>(a);
+    } else k_transfer_group<MODEL_GRID><<<gg, IPOLE_RT_THREADS, 0, st>>>(a);
     span_end(c, s, st);
     c->stats.n_launches++;
     CK(cudaGetLastError());
@@ -694,7 +698,9 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   // numerically integrated eDF coefficients (ipole_set_edf) live in k_apply only: that mode always runs split, and its
   // long rays go through the same kernels (third level, slots of max_steps) instead of the single kernel on the side stream
   // (many cameras per call, c->n_mc: the same -- only the split kernels know about per-ray cameras)
-  const bool edf = c->edf.kind != 0 || c->n_mc > 0;
+  // (the grid model's k_transfer_group knows per-ray cameras itself and keeps the ordinary flow)
+  if (c->n_mc > 0 && c->model != MODEL_ADAF && (c->model != MODEL_GRID || sw || c->opt_unpol)) return IPOLE_EINVAL;
+  const bool edf = c->edf.kind != 0 || (c->n_mc > 0 && c->model == MODEL_ADAF);
   if (edf && (sw || c->opt_unpol || c->model != MODEL_ADAF)) return IPOLE_EINVAL;
   const bool split = edf || (c->opt_split && !sw && !c->opt_unpol && c->model == MODEL_ADAF);
   const size_t step_bytes = rec_bytes + (split ? OP_DOUBLES * sizeof(double) : 0);
@@ -1015,6 +1021,8 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_op, k_stepop<MODEL_ADAF>, IPOLE_OP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_op_mc, k_stepop<MODEL_ADAF, true>, IPOLE_OP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo_mc, k_geodesic<false, true>, IPOLE_GEO_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo_occ_mc, k_geodesic<true, true>, IPOLE_GEO_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_group_mc, k_transfer_group<MODEL_GRID, true>, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo_f32, k_geodesic_f32, IPOLE_GEO_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap, k_apply<false>, IPOLE_AP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_edf, k_apply<true>, IPOLE_AP_THREADS, EDF_MAX_NODES * sizeof(double4));
@@ -1339,12 +1347,18 @@ int ipole_make_images_adaf(ipole_ctx* c, int32_t n_models, const ipole_adaf_para
 int ipole_make_images_cameras(ipole_ctx* c, int32_t n_cams, const ipole_camera* cams, double* I, double* Q, double* U, double* V,
                               double* tau, double* tauF, double* flux_jy) {
   if (!c || !cams || n_cams < 1 || !I || !Q || !U || !V) return IPOLE_EINVAL;
-  if (c->model != MODEL_ADAF) return c->model == MODEL_NONE ? IPOLE_ENOMODEL : IPOLE_EINVAL;
+  if (c->model != MODEL_ADAF && c->model != MODEL_GRID) return c->model == MODEL_NONE ? IPOLE_ENOMODEL : IPOLE_EINVAL;
+  if (c->model == MODEL_GRID && (c->opt_unpol || c->opt_path_free)) return IPOLE_EINVAL;
   for (int k = 0; k < n_cams; ++k) {
     int rc = check_camera(&cams[k]);
     if (rc != IPOLE_OK) return rc;
     const ipole_camera &a = cams[k], &b = cams[0];
     if (a.flat_metric || a.nx != b.nx || a.ny != b.ny || a.eps != b.eps || a.max_steps != b.max_steps || a.hslope != b.hslope) return IPOLE_EINVAL;
+    // a grid was computed in one spacetime and scaled with one mass: its cameras share spin, mass and coordinates with the
+    // context's camera and differ in direction, field of view, frequency and distance
+    const ipole_camera& g0 = c->cam_in;
+    auto eff = [](double v, double dflt) { return v == 0.0 ? dflt : v; };   // (0 stands for the default, include/ipole.h)
+    if (c->model == MODEL_GRID && (a.spin != g0.spin || eff(a.mbh_msun, 4.1e6) != eff(g0.mbh_msun, 4.1e6) || eff(a.hslope, 1.0) != eff(g0.hslope, 1.0))) return IPOLE_EINVAL;
   }
   const int64_t npix = (int64_t)cams[0].nx * cams[0].ny, n = npix * n_cams;
   if (n > 2147483647LL) return IPOLE_EINVAL;

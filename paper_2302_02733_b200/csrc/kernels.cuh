@@ -331,6 +331,9 @@ struct RtArgs {
   int n_models; const void* lane_tab; const Units* units_arr; size_t out_stride;
   // work item -> slot of the batch (nullable: identity): the rays k_stepop left to this kernel (stepop.cuh)
   const int32_t* slots;
+  // many cameras per launch (k_transfer_group<MODEL, true>): ray q belongs to camera q / rays_per_cam; the cameras share
+  // spin, mass and hslope with `cam` (its geometry serves all) and differ in direction, field of view, frequency, distance
+  const CamDev* cams; int64_t rays_per_cam;   // units of camera k: units_arr[k]
 };
 
 constexpr int SWEEP_MAX_MODELS = 64;   // parameter sets per transfer launch (shared memory: <= 88 B each)
@@ -535,7 +538,9 @@ k_transfer(const __grid_constant__ RtArgs A) {
 // 97).  Rays are ordered by predicted step count, so the 32 rays of a group lie on one ring of the image around the
 // spin axis: at equal s they are at nearly equal radius and in the same kind of step.  The arithmetic per ray is that
 // of k_transfer, operation for operation (bit-identical images).
-template <int MODEL>
+// MC (many cameras per launch, grid model: ipole_make_images_cameras): frequency, length unit and the camera's transverse
+// legs are the ray's own camera's; the single-camera instantiation is unchanged.
+template <int MODEL, bool MC = false>
 __global__ void __launch_bounds__(IPOLE_RT_THREADS, IPOLE_RT_MINB) k_transfer_group(const __grid_constant__ RtArgs A) {
   const CamDev& C = A.cam;
   const size_t slot_doubles = (size_t)(A.cap + 1) * REC_DOUBLES;
@@ -561,9 +566,12 @@ __global__ void __launch_bounds__(IPOLE_RT_THREADS, IPOLE_RT_MINB) k_transfer_gr
     int32_t q = 0;
     int s0 = -1, s_lo = 0;       // this lane walks steps s0 ... 0; -1: nothing to walk
     bool lit = false;
+    Units Ul = A.units;          // MC: the units of the lane's camera
+    int cam_i = 0;
     if (li < count) {
       const int64_t ls = A.rank_slot ? (int64_t)A.rank_slot[A.base + li] : li;    // this lane's slot in the batch
       q = A.order ? A.order[A.base + ls] : (int32_t)(A.base + ls);
+      if (MC) { cam_i = (int)(q / A.rays_per_cam); Ul = A.units_arr[cam_i]; }
       int n = A.nsteps[q];
       if (n >= 0) {              // (n < 0: overflowed its slot, done by the long-ray pass)
         if (MODEL == MODEL_GRID && A.srange) {
@@ -610,17 +618,19 @@ __global__ void __launch_bounds__(IPOLE_RT_THREADS, IPOLE_RT_MINB) k_transfer_gr
         const double h = 0.5 * dl;
         if (lit) { transport_apply(Am, h, st.f1); transport_apply(Am, h, st.f2); }
         PlasmaFrame F;
-        const bool applied = maybe && plasma_frame<MODEL>(C.G, model, nullptr, A.units, Xm, Km, p, g, gi, prim, st, F);
+        const bool applied = maybe && plasma_frame<MODEL>(C.G, model, nullptr, MC ? Ul : A.units, Xm, Km, p, g, gi, prim, st, F);
         lit |= applied;
         if (lit) { transport_apply(Am, h, st.f1); transport_apply(Am, h, st.f2); }
-        if (applied) plasma_apply<MODEL>(A.units, F, dl, st);
+        if (applied) plasma_apply<MODEL>(MC ? Ul : A.units, F, dl, st);
       }
 #pragma unroll
       for (int m = 0; m < 4; ++m) { Xhi[m] = Xlo[m]; Khi[m] = Klo[m]; }
     }
     if (s0 >= 0) {
-      stokes_congruence(dot4(C.ecov1, st.f1), dot4(C.ecov1, st.f2), dot4(C.ecov2, st.f1), dot4(C.ecov2, st.f2), st.S);
-      const double nu_o = A.units.nu_obs;
+      const double* ec1 = MC ? A.cams[cam_i].ecov1 : C.ecov1;
+      const double* ec2 = MC ? A.cams[cam_i].ecov2 : C.ecov2;
+      stokes_congruence(dot4(ec1, st.f1), dot4(ec1, st.f2), dot4(ec2, st.f1), dot4(ec2, st.f2), st.S);
+      const double nu_o = MC ? Ul.nu_obs : A.units.nu_obs;
       const double nu3 = nu_o * nu_o * nu_o;
       A.I[q] = st.S[0] * nu3; A.Q[q] = st.S[1] * nu3; A.U[q] = st.S[2] * nu3; A.V[q] = st.S[3] * nu3;
       if (A.tau) A.tau[q] = st.tau;

@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 
 from paper_2302_02733_b200 import workloads as W
-from test_gpu_parity import check_parity, to_np, ipole, NTHREADS  # noqa: F401
+from test_gpu_parity import check_parity, to_np, ipole, small_grid, NTHREADS  # noqa: F401
 
 pytestmark = pytest.mark.gpu
 
@@ -84,3 +84,50 @@ def test_cameras_errors(ipole):
         g.make_images_cameras(cams)
     g.set_path_free(False)
     g.make_images_cameras(cams)
+
+
+def test_grid_cameras_equal_single_calls_and_oracle(ipole, ref, small_grid):
+    """The grid model through ipole_make_images_cameras: cameras that share spin, mass and hslope with the context's and
+    differ in inclination, frequency, field of view and distance; k_geodesic<true, MC> + k_transfer_group<grid, MC>."""
+    desc, fields = small_grid
+    base = W.camera("grid", 40)
+    cams = []
+    for k, (inc, fr, fov, dist) in enumerate(((20.0, 230e9, 40.0, 8000.0), (60.0, 345e9, 40.0, 8000.0), (85.0, 86e9, 60.0, 8000.0),
+                                              (140.0, 230e9, 30.0, 16000.0), (20.0, 690e9, 40.0, 8000.0))):
+        cam = dict(base); cam.update(inclination_deg=inc, freq_hz=fr, fov=fov, dsource_pc=dist)
+        cams.append(cam)
+    g = ipole.Ipole(**base); g.load_grid(desc, fields)
+    out = g.make_images_cameras(cams, maps=True)
+    for m, cam in enumerate(cams):
+        f = ipole.Ipole(**cam); f.load_grid(desc, fields)
+        one = to_np(f.make_image(maps=True)); st = f.stats()
+        f.close()
+        sc = np.abs(one["I"]).max()
+        assert sc > 0
+        for k in ("I", "Q", "U", "V"):
+            # (another instantiation of the same kernels: rounding-level differences, amplified where the Faraday depth is large)
+            assert np.abs(out[k][m].cpu().numpy().ravel() - one[k]).max() <= 1e-9 * sc, (m, k)
+        for k in ("tau", "tauF"):
+            assert np.allclose(out[k][m].cpu().numpy().ravel(), one[k], rtol=1e-9, atol=1e-12 * np.abs(one[k]).max()), (m, k)
+        assert np.allclose(out["flux_jy"][m], st["flux_jy"], rtol=1e-9, atol=1e-11 * abs(st["flux_jy"][0]))
+        if m == 2:
+            r = ref.Ctx(**cam); r.load_grid(desc, fields)
+            want = r.make_pixels(nthreads=NTHREADS)
+            got = {k: out[k][m].cpu().numpy().ravel() for k in ("I", "Q", "U", "V", "tau", "tauF")}
+            check_parity(got, want, "grid camera %d" % m, min_lit=0.2)
+    # many batches, per-batch slots, retry level and long rays with cameras
+    g.set_options(24 << 20, 2)
+    out2 = g.make_images_cameras(cams, maps=True)
+    assert g.stats()["n_batches"] > 3
+    for k in ("I", "Q", "U", "V", "tau", "tauF"):
+        assert np.array_equal(out2[k].cpu().numpy(), out[k].cpu().numpy()), k
+    # the context's own camera is untouched, and a camera of another spin or mass is refused
+    again = to_np(g.make_image(maps=True))
+    f = ipole.Ipole(**base); f.load_grid(desc, fields); f.set_options(24 << 20, 2)
+    want = to_np(f.make_image(maps=True))
+    for k in want:
+        assert np.array_equal(again[k], want[k]), k
+    bad = dict(cams[1]); bad["spin"] = 0.5
+    with pytest.raises(ipole.IpoleError) as ei:
+        g.make_images_cameras([cams[0], bad])
+    assert ei.value.code == ipole.EINVAL
