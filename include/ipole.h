@@ -162,7 +162,7 @@ int  ipole_set_batch_overlap(ipole_ctx*, int32_t on);
  * the side stream.  With device outputs such a call only enqueues work and RETURNS WHILE THE GPU IS STILL RUNNING
  * (ipole_stats.plan_reused = 1); outputs are valid once the context's stream reaches that point (stream order, an
  * event, or ipole_get_stats, which synchronises).  The model may be reloaded or its parameters changed in between (a
- * time series of GRMHD slices, a parameter fit at fixed geometry).  Any other call in between, a changed camera or
+ * time series of GRMHD slices, a parameter fit at fixed geometry).  Any other call in between, a changed camera, stream or
  * option, or a different amount of free memory falls back to the planning call, which blocks as before and records a
  * new plan.  The image is the same, bit for bit, either way.  Not used for pixel lists, sweeps, many-camera calls, the
  * path-free variant and eDF coefficients.  on == 0: every call plans afresh.  IPOLE_EINVAL for a NULL context. */

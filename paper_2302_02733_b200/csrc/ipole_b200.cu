@@ -1071,6 +1071,7 @@ int ipole_set_camera(ipole_ctx* c, const ipole_camera* cam) {
 
 int ipole_set_stream(ipole_ctx* c, void* s) {
   if (!c) return IPOLE_EINVAL;
+  if ((cudaStream_t)s != c->stream) c->plan_cache.valid = false;   // the recorded lists were written in the old stream's order
   c->stream = (cudaStream_t)s;
   return IPOLE_OK;
 }
