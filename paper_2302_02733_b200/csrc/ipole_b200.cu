@@ -601,7 +601,12 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   }
   if (!probe && !replay) {
     // everything in flight at once: give each ray what the budget allows
-    const int64_t per = (int64_t)(budget / rec_bytes / (size_t)n) - 1;
+    // (per step: the path record and, where the split transfer will run, the operator record -- so that the slots the
+    // plan below can afford hold every ray in ONE batch: a pixel list of an adaptive level is a few thousand rays whose
+    // time is the latency of the longest, and two batches are twice that)
+    const bool will_split = c->edf.kind != 0 || c->n_mc > 0 || (c->opt_split && !sw && !c->opt_unpol && c->model == MODEL_ADAF);
+    const size_t per_step = rec_bytes + ((will_split && !c->opt_path_free) ? OP_DOUBLES * sizeof(double) : 0);
+    const int64_t per = (int64_t)(budget / per_step / (size_t)(((n + 31) / 32) * 32)) - 1;
     cap = (int)std::max<int64_t>(64, std::min<int64_t>(max_steps, per));
   }
   if ((c->edf.kind != 0 || c->n_mc) && c->opt_path_free) return IPOLE_EINVAL;
@@ -1532,9 +1537,16 @@ int ipole_make_image_adaptive(ipole_ctx* c, int32_t levels, double rel_tol, doub
     }
   }
   const double pix_rad = c->cam.pix * c->units.L_unit / c->units.D_cm;
-  k_reduce_models<<<1, 256, 0, c->stream>>>(n, (size_t)n, A.img[0], A.img[1], A.img[2], A.img[3], pix_rad * pix_rad * 1e23,
-                                            (double*)c->d_part);
-  ++launches;
+  {
+    // d_part holds REDUCE_BLOCKS ReducePartial (64 B each): room for the 4 results and REDUCE_BLOCKS x 4 partial sums
+    static_assert(sizeof(ReducePartial) >= 8 * sizeof(double), "d_part is reused for the plane partials");
+    double* flux4 = (double*)c->d_part;
+    double* parts = flux4 + 4;
+    const int nb = (int)std::min<int64_t>(REDUCE_BLOCKS - 1, (n + 255) / 256);
+    k_reduce_planes_partial<<<nb, 256, 0, c->stream>>>(n, A.img[0], A.img[1], A.img[2], A.img[3], parts);
+    k_reduce_planes_final<<<1, 32, 0, c->stream>>>(parts, nb, pix_rad * pix_rad * 1e23, flux4);
+    launches += 2;
+  }
   CK(cudaGetLastError());
   CK(cudaMemcpyAsync(inf.flux_jy, c->d_part, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
   CK(cudaEventRecord(c->ev_ada1, c->stream));

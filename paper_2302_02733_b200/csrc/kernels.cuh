@@ -911,6 +911,33 @@ __global__ void k_reduce_final(const ReducePartial* part, int nparts, double sca
   *out = o;
 }
 
+// Flux of ONE large image in two stages (ipole_make_image_adaptive: 16.7 M pixels are too many for the single block per
+// image of k_reduce_models below): REDUCE_BLOCKS partial sums, then one block folds them in index order => reproducible.
+__global__ void __launch_bounds__(256) k_reduce_planes_partial(int64_t n, const double* I, const double* Q, const double* U,
+                                                               const double* V, double* part /* [gridDim.x][4] */) {
+  double s[4] = {0, 0, 0, 0};
+  for (int64_t q = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; q < n; q += (int64_t)gridDim.x * blockDim.x) {
+    s[0] += I[q]; s[1] += Q[q]; s[2] += U[q]; s[3] += V[q];
+  }
+  __shared__ double sh[8][4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) s[k] = warp_sum(s[k]);
+  if ((threadIdx.x & 31) == 0) for (int k = 0; k < 4; ++k) sh[threadIdx.x >> 5][k] = s[k];
+  __syncthreads();
+  if (threadIdx.x < 4) {
+    double t = sh[0][threadIdx.x];
+    for (int w = 1; w < 8; ++w) t += sh[w][threadIdx.x];
+    part[4 * blockIdx.x + threadIdx.x] = t;
+  }
+}
+__global__ void k_reduce_planes_final(const double* part, int nparts, double scale, double* flux /* [4] */) {
+  if (threadIdx.x < 4 && blockIdx.x == 0) {
+    double t = 0.0;
+    for (int i = 0; i < nparts; ++i) t += part[4 * i + threadIdx.x];
+    flux[threadIdx.x] = t * scale;
+  }
+}
+
 // model sweep: flux of every image of the batch, one block per model (fixed shape => reproducible)
 __global__ void __launch_bounds__(256) k_reduce_models(int64_t n, size_t stride, const double* I, const double* Q,
                                                        const double* U, const double* V, double scale, double* flux) {
