@@ -97,6 +97,7 @@ struct ipole_ctx {
   // listed the rays, beside the last transfer kernels, instead of after them (one ray of S_cap steps is ~30 ms of latency)
   cudaEvent_t ev_lastgeo[2] = {nullptr, nullptr};
   double* d_retry_buf = nullptr; size_t retry_buf_bytes = 0;
+  double* d_ops_long = nullptr; size_t ops_long_bytes = 0;   // operator records of a long-ray pass through the split kernels (eDF, cameras)
   int opt_side_retry = 1;
   int64_t ray_cap = 0;           // capacity of the per-ray buffers below
   int32_t *d_nsteps = nullptr, *d_nturn = nullptr, *d_order = nullptr, *d_key = nullptr, *d_long = nullptr;
@@ -239,10 +240,19 @@ int ensure_ops(ipole_ctx* c, size_t bytes) {
 
 int ensure_retry_buf(ipole_ctx* c, size_t bytes) {
   if (bytes <= c->retry_buf_bytes) return IPOLE_OK;
-  cudaFree(c->d_retry_buf); cudaFree(c->plan_cache.d_long); cudaFree(c->plan_cache.d_retry); c->d_retry_buf = nullptr; c->retry_buf_bytes = 0;
+  cudaFree(c->d_retry_buf); cudaFree(c->d_ops_long); cudaFree(c->plan_cache.d_long); cudaFree(c->plan_cache.d_retry); c->d_retry_buf = nullptr; c->retry_buf_bytes = 0;
   cudaError_t e = cudaMalloc(&c->d_retry_buf, bytes);
   if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
   c->retry_buf_bytes = bytes;
+  return IPOLE_OK;
+}
+
+int ensure_ops_long(ipole_ctx* c, size_t bytes) {
+  if (bytes <= c->ops_long_bytes) return IPOLE_OK;
+  cudaFree(c->d_ops_long); c->d_ops_long = nullptr; c->ops_long_bytes = 0;
+  cudaError_t e = cudaMalloc(&c->d_ops_long, bytes);
+  if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
+  c->ops_long_bytes = bytes;
   return IPOLE_OK;
 }
 
@@ -260,7 +270,7 @@ size_t path_budget(ipole_ctx* c) {
   if (const char* e = std::getenv("IPOLE_PATH_GIB")) { const double gib = std::atof(e); if (gib > 0.0) return (size_t)(gib * 1073741824.0); }
   size_t fr = 0, tot = 0;
   cudaMemGetInfo(&fr, &tot);
-  fr += c->path_bytes + c->path_long_bytes + c->ops_bytes + c->retry_buf_bytes;  // what we already hold counts as available
+  fr += c->path_bytes + c->path_long_bytes + c->ops_bytes + c->retry_buf_bytes + c->ops_long_bytes;  // what we already hold counts as available
   size_t b = (size_t)(0.5 * (double)fr);
   const size_t cap = (size_t)96 << 30;
   return std::min(b, cap);
@@ -649,6 +659,9 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   // grid model: k_geodesic marks the steps that may cross plasma, k_transfer walks only from the first of them
   const bool use_occ = (c->model == MODEL_GRID) && c->opt_occ;
   const size_t lslot = (size_t)(max_steps + 1) * rec_bytes;
+  // eDF coefficients and many ADAF cameras live in the split kernels only: their long rays take k_stepop + k_apply here
+  // (operator records in d_ops_long) instead of the single kernel
+  const bool long_split = c->edf.kind != 0 || (c->n_mc > 0 && c->model == MODEL_ADAF);
   int long_done = 0;          // entries of d_long already handed to the side stream
   int64_t LBcap = 0;          // rays that fit the long path buffer
   const int32_t* long_src = replay ? pc.d_long : c->d_long;       // replay: the list the recorded call ended with
@@ -657,14 +670,17 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     if (upto <= long_done) return IPOLE_OK;
     if (LBcap == 0) {
       const size_t lbudget = std::max(lslot, std::min<size_t>(budget / 4, (size_t)16 << 30));
-      LBcap = std::max<int64_t>(1, std::min<int64_t>(std::max(upto - long_done, 256), (int64_t)(lbudget / lslot)));
-      if (c->path_long_bytes >= lslot) LBcap = std::max<int64_t>(LBcap, (int64_t)(c->path_long_bytes / lslot));
+      const size_t lboth = long_split ? 2 * lslot : lslot;      // (an operator record is as large as a path record)
+      LBcap = std::max<int64_t>(1, std::min<int64_t>(std::max(upto - long_done, 256), (int64_t)(lbudget / lboth)));
+      if (!long_split && c->path_long_bytes >= lslot) LBcap = std::max<int64_t>(LBcap, (int64_t)(c->path_long_bytes / lslot));
+      if (long_split && LBcap >= 64) LBcap &= ~(int64_t)31;     // whole groups of 32 slots (operator records)
       int rcl = ensure_path_long(c, (size_t)LBcap * lslot);
       if (rcl != IPOLE_OK) return rcl;
+      if (long_split && (rcl = ensure_ops_long(c, (size_t)((LBcap + 31) / 32 * 32) * (size_t)(max_steps + 1) * OP_DOUBLES * sizeof(double))) != IPOLE_OK) return rcl;
     }
     for (int64_t base = long_done; base < upto; base += LBcap) {
       const int64_t cnt = std::min<int64_t>(LBcap, upto - base);
-      if (qi + 2 > N_QUEUES) return IPOLE_EINVAL;
+      if (qi + 4 > N_QUEUES) return IPOLE_EINVAL;
       GeoArgs g = geo_args(c);
       g.cap = max_steps; g.base = base; g.count = cnt; g.order = long_src; g.pixels = d_pixels;
       g.path = c->d_path_long; g.nsteps = c->d_nsteps_long; g.nturn = c->d_nturn; g.queue = c->d_queues + (qi++);
@@ -674,10 +690,13 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
       RtArgs t;
       std::memset(&t, 0, sizeof t);
       t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = max_steps; t.base = base; t.count = cnt;
-      t.order = long_src; t.path = c->d_path_long; t.nsteps = c->d_nsteps_long; t.queue = c->d_queues + (qi++);
+      t.order = long_src; t.path = c->d_path_long; t.nsteps = c->d_nsteps_long; t.queue = c->d_queues + qi;
+      qi += long_split ? 3 : 1;
       if (use_occ) t.srange = c->d_srange;
       t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
-      if ((rcl = launch_transfer(c, t, LK_LONG, cnt, c->side, 0, 0, sw)) != IPOLE_OK) return rcl;
+      if (long_split) rcl = launch_transfer_split(c, t, cnt, c->side, 0, c->d_ops_long, 2);
+      else rcl = launch_transfer(c, t, LK_LONG, cnt, c->side, 0, 0, sw);
+      if (rcl != IPOLE_OK) return rcl;
     }
     long_done = upto;
     return IPOLE_OK;
@@ -701,8 +720,8 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   // persistent kernels have that many fewer tails.  A ray that outgrows its batch's slot is listed and retried at
   // the end with the global S_cap (second level); one that outgrows S_cap goes to the long-ray pass as before.
   // numerically integrated eDF coefficients (ipole_set_edf) live in k_apply only: that mode always runs split, and its
-  // long rays go through the same kernels (third level, slots of max_steps) instead of the single kernel on the side stream
-  // (many cameras per call, c->n_mc: the same -- only the split kernels know about per-ray cameras)
+  // long rays go through the same kernels on the side stream (long_pass above) instead of the single kernel
+  // (many cameras per call, c->n_mc, analytic flow: the same -- only the split kernels know about per-ray cameras)
   // (the grid model's k_transfer_group knows per-ray cameras itself and keeps the ordinary flow)
   if (c->n_mc > 0 && c->model != MODEL_ADAF && (c->model != MODEL_GRID || sw || c->opt_unpol)) return IPOLE_EINVAL;
   const bool edf = c->edf.kind != 0 || (c->n_mc > 0 && c->model == MODEL_ADAF);
@@ -782,7 +801,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     int rcb;
     if ((rcb = launch_geodesic(c, g, LK_GEO, b.cnt, st, reserve)) != IPOLE_OK) return rcb;
     CK(cudaEventRecord(c->ev_lastgeo[lane], st));
-    if (top && cap < max_steps && !edf && !replay) {
+    if (top && cap < max_steps && !replay) {
       CK(cudaEventRecord(c->ev_geo, st));
       CK(cudaStreamWaitEvent(c->side, c->ev_geo, 0));
     }
@@ -797,7 +816,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     else rcb = launch_transfer(c, t, LK_RT, b.cnt, st, reserve, 0, sw);
     if (rcb != IPOLE_OK) return rcb;
     c->stats.n_batches++;
-    if (top && cap < max_steps && !edf && !replay) {   // the transfer kernel just queued keeps the GPU busy while the host waits here
+    if (top && cap < max_steps && !replay) {   // the transfer kernel just queued keeps the GPU busy while the host waits here
       if ((rcb = listed(c->ev_geo, n_long)) != IPOLE_OK) return rcb;
       if ((rcb = long_pass(n_long)) != IPOLE_OK) return rcb;
     }
@@ -826,7 +845,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   int64_t R_max = 0;
   if (tight && !sw && c->opt_side_retry && plan.size() >= 2) {
     const size_t slot = (size_t)(cap + 1) * step_bytes;
-    R_max = std::max<int64_t>(256, n / 512);
+    R_max = std::max<int64_t>(256, n / 64);     // (what limits it is the memory below: 8 GiB of slots)
     R_max = std::min<int64_t>(R_max, (int64_t)(std::min<size_t>(budget / 8, (size_t)8 << 30) / slot)) & ~(int64_t)31;
     if (R_max >= 32 && ensure_retry_buf(c, (size_t)R_max * slot) != IPOLE_OK) R_max = 0;
     if (R_max < 32) R_max = 0;
@@ -886,7 +905,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
       CK(cudaMemcpyAsync(&n_retry, retry_count, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
       CK(cudaStreamSynchronize(c->stream));
       n_retry_side = (int)std::min<int64_t>(n_retry, R_max);
-      if (n_retry_side > 0 && cap < max_steps && !edf) {
+      if (n_retry_side > 0 && cap < max_steps) {
         // retried rays that outgrow S_cap as well: listed by the geodesic kernel above, long-ray pass
         if ((rc = listed(c->ev_geo, n_long)) != IPOLE_OK) return rc;
         if ((rc = long_pass(n_long)) != IPOLE_OK) return rc;
@@ -900,25 +919,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
       if ((rc = run_plan(retry_src + n_retry_side)) != IPOLE_OK) return rc;
     }
   }
-  if (edf && cap < max_steps) {
-    // third level: rays longer than S_cap, through the same split kernels with slots of max_steps
-    if (side_used) {   // the list is complete once the geodesic kernel of the side-stream retry has run
-      CK(cudaEventRecord(c->ev_side, c->side));
-      CK(cudaStreamWaitEvent(c->stream, c->ev_side, 0));
-    }
-    CK(cudaMemcpyAsync(&n_long, c->d_small, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-    CK(cudaStreamSynchronize(c->stream));
-    if (n_long > 0) {
-      const int cap_saved = cap;
-      cap = max_steps;
-      make_plan(n_long, false);
-      if ((rc = prepare(false)) != IPOLE_OK) return rc;
-      if ((rc = run_plan(c->d_long)) != IPOLE_OK) return rc;
-      cap = cap_saved;
-    }
-    c->stats.n_long = n_long;
-    n_long = 0;   // nothing ran on the side stream
-  } else c->stats.n_long = n_long;
+  c->stats.n_long = n_long;
   if (n_long > 0 || side_used) {
     // join the side stream, then publish the step counts of the long and the retried rays (the bulk transfer kernels
     // read nsteps[q] = -1 for them, so the side-stream passes keep theirs apart until every bulk kernel is done)
