@@ -755,7 +755,9 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   // holds everything, and for the sweeps (their parameter tables are per stream).
   int n_lanes = 1;
   make_plan(n, tight);
-  if (c->opt_overlap && c->lane2 && !sw && plan.size() >= 2) {
+  // (from three batches on: with two, halving them adds more kernel tails and retried rays than the overlap hides --
+  // 64 grid cameras of 128^2: 205 ms on one lane, 220 ms on two)
+  if (c->opt_overlap && c->lane2 && !sw && plan.size() >= 3) {
     n_lanes = 2;
     lane_budget = budget / 2;
     make_plan(n, tight);
