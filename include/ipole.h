@@ -149,7 +149,7 @@ int  ipole_set_transfer_split(ipole_ctx*, int32_t on);
  * alternate between two streams, each with half of the path memory, so that the next batch's kernels fill those tails.
  * on == 0: one batch after the other on the context's stream (then the per-stage times of ipole_get_stats add up to
  * ms_total; bench.py measures its per-kernel figures this way).  Same image either way, bit for bit (a ray's arithmetic
- * does not depend on its batch).  Single-batch images and the sweeps always run on one stream.  IPOLE_EINVAL for NULL. */
+ * does not depend on its batch).  Images of one or two batches and the sweeps always run on one stream.  IPOLE_EINVAL for NULL. */
 int  ipole_set_batch_overlap(ipole_ctx*, int32_t on);
 /* Asynchronous images by plan reuse (default on).  To schedule an image the host needs four facts from the device: the
  * longest probe ray (S_cap), the populations of the step-count bins (slots per batch), which rays outgrew their slots and
