@@ -145,6 +145,18 @@ def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier,
     fkey = "transfer_" + wl["kind"]
     fl_step = (FLOP_PER_STEP_UNPOL[fkey] or 0.0) if args.unpolarized else FLOP_PER_STEP[fkey]
     ach = fl_step * steps_rt / (rt_ms * 1e-3) / 1e12
+    kname = "k_transfer<%s, sweep>" % wl["kind"]
+    flop_note = "flop per step of the single-image kernel (the sweep runs the same arithmetic per pair)"
+    if st.get("ms_stepop", 0.0) > 0.0 and not args.unpolarized:
+        # analytic flow through the split kernels: k_stepop ONCE per call, k_apply once per parameter set.  The work the sets
+        # share is counted once: executed flop (profiles/r2_image_flops.md) of k_stepop x steps + of k_apply x steps x M
+        flop = st["total_steps"] * (FLOP_EXECUTED["k_stepop"] + M * FLOP_EXECUTED["k_apply"])
+        ach = flop / (rt_ms * 1e-3) / 1e12
+        fl_step = flop / steps_rt
+        kname = "k_stepop<adaf> (once) + k_apply<sweep> (per parameter set)"
+        flop_note = ("executed flop per (step, parameter set): k_apply's %.0f plus k_stepop's %.0f shared by the %d sets of a call; "
+                     "against the single kernel's frozen 1576 per pair the call does %.2fx the images per FP64 operation"
+                     % (FLOP_EXECUTED["k_apply"], FLOP_EXECUTED["k_stepop"], M, FLOP_PER_STEP[fkey] / fl_step))
     line = {"metric": "rays_per_s", "value": value, "unit": "rays/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -157,12 +169,13 @@ def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier,
             "images_per_s": world * M * args.steps / (ms * 1e-3),
             "separate_calls": {"images_per_s": world * M * args.steps / (ms_sep * 1e-3), "ms_per_%d_images" % M: ms_sep / args.steps,
                                "speedup_of_the_batch_entry": ms_sep / ms},
-            "stage_ms": {"probe_sort": st["ms_probe"], "geodesic": st["ms_geodesic"], "transfer": rt_ms, "total": st["ms_total"]},
+            "stage_ms": {"probe_sort": st["ms_probe"], "geodesic": st["ms_geodesic"], "transfer": rt_ms, "stepop": st.get("ms_stepop", 0.0),
+                         "apply": st.get("ms_apply", 0.0), "total": st["ms_total"]},
             "gpu_launches": st["n_launches"] * args.steps,
-            "roofline": {"bound": "alu", "kernel": "k_transfer<%s, sweep>" % wl["kind"], "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+            "roofline": {"bound": "alu", "kernel": kname, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                          "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz; DFMA micro-benchmark on this GPU: %.1f" % dfma_tf,
                          "achieved": ach, "frac": ach / FP64_PEAK_TFLOPS, "flop_per_step": fl_step,
-                         "flop_note": "flop per step of the single-image kernel (the sweep runs the same arithmetic per pair)",
+                         "flop_note": flop_note,
                          "avg_launch_ms": rt_ms, "kernel_share_of_step": rt_ms / st["ms_total"], "traffic": None},
             "e2e": {"value": replicas.job_throughput(rays * args.steps, dt, world), "unit": "rays/s",
                     "h2d_bytes_per_step": ipole.C.sizeof(ipole.Camera) + M * (ipole.C.sizeof(ipole.AdafParams) + 32),

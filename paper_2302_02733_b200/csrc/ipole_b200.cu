@@ -340,6 +340,8 @@ void launch_transfer_model(int model, int g, cudaStream_t st, const RtArgs& a) {
   else k_transfer<MODEL_GRID, PF><<<g, IPOLE_RT_THREADS, 0, st>>>(a);
 }
 
+int launch_transfer_sweep_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStream_t st, const Sweep* sw);
+
 // pf: 0 stored path, 1 path-free with eps <= 0.04, 2 path-free with any eps
 int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_t st, int reserve = 0, int pf = 0,
                     const Sweep* sw = nullptr) {
@@ -358,6 +360,12 @@ int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_
     // chunks of SWEEP_MAX_MODELS parameter sets; the parameter tables are re-sent per chunk on the launching stream
     // (stream order keeps a table alive until the kernel that reads it has finished).  The main stream and the side
     // stream (long-ray passes) each have their own tables: they run concurrently.
+    // analytic flow, bulk batches: the operator records are the same for every parameter set -- k_stepop once, k_apply
+    // per set (1: a ray with a step outside the split's reach is in the batch; the single kernel below takes it all)
+    if (c->model == MODEL_ADAF && c->opt_split && !c->opt_unpol && st != c->side && a.path == c->d_path && c->d_ops) {
+      const int r = launch_transfer_sweep_split(c, a, rays, st, sw);
+      if (r != 1) return r;
+    }
     void* tab_models = (st == c->side) ? c->d_sweep_models_side : c->d_sweep_models;
     Units* tab_units = (st == c->side) ? c->d_sweep_units_side : c->d_sweep_units;
     RtArgs t = a;
@@ -481,6 +489,75 @@ int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStrea
   {
     const int s = span_begin(c, on_side ? LK_LONG : LK_RT, st);
     k_transfer<MODEL_ADAF, 0><<<std::max(1, c->n_sm / 8), IPOLE_RT_THREADS, 0, st>>>(t);
+    span_end(c, s, st);
+    c->stats.n_launches++;
+    CK(cudaGetLastError());
+  }
+  return IPOLE_OK;
+}
+
+// Model sweep of the analytic flow through the split kernels (ipole_make_images_adaf): everything k_stepop computes --
+// metric, generator, flow, field direction, tetrad, leg projections -- is the same for every parameter set, so it runs ONCE
+// per batch; k_apply then walks the records once per set (work item = ray group x set, the sets of a group back to back so
+// that its records come from L2), in chunks of SWEEP_MAX_MODELS sets whose tables are re-sent on the stream.
+// Returns 1 (nothing written that matters) when k_stepop met an irregular ray: the caller runs the single sweep kernel.
+int launch_transfer_sweep_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStream_t st, const Sweep* sw) {
+  int* irr_count = c->d_small + 4;
+  CK(cudaMemsetAsync(irr_count, 0, sizeof(int), st));
+  void* tab_models = c->d_sweep_models;
+  Units* tab_units = c->d_sweep_units;
+  auto send_tables = [&](int m0, int mc) -> int {
+    CK(cudaMemcpyAsync(tab_models, (const char*)sw->lane_tab + (size_t)m0 * sw->lane_bytes, mc * sw->lane_bytes, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(tab_units, sw->units + m0, mc * sizeof(Units), cudaMemcpyHostToDevice, st));
+    return IPOLE_OK;
+  };
+  int rc;
+  const int mc0 = std::min(SWEEP_MAX_MODELS, sw->n_models);
+  if ((rc = send_tables(0, mc0)) != IPOLE_OK) return rc;
+  OpArgs o;
+  std::memset(&o, 0, sizeof o);
+  o.cam = a.cam; o.units = a.units; o.model = tab_models;   // (any set: the flow's geometry needs the ISCO radius only)
+  o.cap = a.cap; o.base = a.base; o.count = a.count; o.order = a.order;
+  o.path = a.path; o.nsteps = a.nsteps; o.queue = a.queue; o.ops = c->d_ops; o.irr_slots = c->d_irr; o.irr_count = irr_count;
+  o.test_irregular = (c->opt_split == 2);
+  const bool rank = c->opt_rank && rays > 32;
+  if (rank) {
+    RankArgs r = {a.base, a.count, nullptr, a.order, a.nsteps, c->d_rank_pos, c->d_rank_slot, nullptr};
+    const int s = span_begin(c, LK_OPS, st);
+    k_rank_window<<<(unsigned)((rays + RANK_WINDOW - 1) / RANK_WINDOW), RANK_WINDOW, 0, st>>>(r);
+    span_end(c, s, st);
+    c->stats.n_launches++;
+    o.pos = c->d_rank_pos;
+  }
+  {
+    const int s = span_begin(c, LK_OPS, st);
+    k_stepop<MODEL_ADAF><<<grid_for(c, c->occ_op, IPOLE_OP_THREADS / 32, rays), IPOLE_OP_THREADS, 0, st>>>(o);
+    span_end(c, s, st);
+    c->stats.n_launches++;
+    CK(cudaGetLastError());
+  }
+  int n_irr = 0;
+  CK(cudaMemcpyAsync(&n_irr, irr_count, sizeof(int), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  if (n_irr > 0) return 1;
+  ApArgs p;
+  std::memset(&p, 0, sizeof p);
+  p.cap = a.cap; p.base = a.base; p.count = a.count; p.order = a.order; p.ops = c->d_ops; p.nsteps = a.nsteps;
+  p.queue = a.queue + 1;
+  if (rank) p.slot = c->d_rank_slot;
+  p.lane_tab = (const AdafParams*)tab_models; p.units_arr = tab_units; p.units_ref = a.units; p.out_stride = sw->out_stride;
+  double* planes[6] = {a.I, a.Q, a.U, a.V, a.tau, a.tauF};
+  for (int m0 = 0; m0 < sw->n_models; m0 += SWEEP_MAX_MODELS) {
+    const int mc = std::min(SWEEP_MAX_MODELS, sw->n_models - m0);
+    if (m0 > 0 && (rc = send_tables(m0, mc)) != IPOLE_OK) return rc;
+    p.n_models = mc;
+    p.I = planes[0] + (size_t)m0 * sw->out_stride; p.Q = planes[1] + (size_t)m0 * sw->out_stride;
+    p.U = planes[2] + (size_t)m0 * sw->out_stride; p.V = planes[3] + (size_t)m0 * sw->out_stride;
+    p.tau = planes[4] ? planes[4] + (size_t)m0 * sw->out_stride : nullptr;
+    p.tauF = planes[5] ? planes[5] + (size_t)m0 * sw->out_stride : nullptr;
+    CK(cudaMemsetAsync(p.queue, 0, sizeof(unsigned long long), st));
+    const int s = span_begin(c, LK_APPLY, st);
+    k_apply<false, true><<<grid_for(c, c->occ_ap, IPOLE_AP_THREADS / 32, ((rays + 31) / 32) * mc), IPOLE_AP_THREADS, 0, st>>>(p);
     span_end(c, s, st);
     c->stats.n_launches++;
     CK(cudaGetLastError());
@@ -614,7 +691,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     // (per step: the path record and, where the split transfer will run, the operator record -- so that the slots the
     // plan below can afford hold every ray in ONE batch: a pixel list of an adaptive level is a few thousand rays whose
     // time is the latency of the longest, and two batches are twice that)
-    const bool will_split = c->edf.kind != 0 || c->n_mc > 0 || (c->opt_split && !sw && !c->opt_unpol && c->model == MODEL_ADAF);
+    const bool will_split = c->edf.kind != 0 || c->n_mc > 0 || (c->opt_split && !c->opt_unpol && c->model == MODEL_ADAF);
     const size_t per_step = rec_bytes + ((will_split && !c->opt_path_free) ? OP_DOUBLES * sizeof(double) : 0);
     const int64_t per = (int64_t)(budget / per_step / (size_t)(((n + 31) / 32) * 32)) - 1;
     cap = (int)std::max<int64_t>(64, std::min<int64_t>(max_steps, per));
@@ -727,7 +804,10 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   const bool edf = c->edf.kind != 0 || (c->n_mc > 0 && c->model == MODEL_ADAF);
   if (edf && (sw || c->opt_unpol || c->model != MODEL_ADAF)) return IPOLE_EINVAL;
   const bool split = edf || (c->opt_split && !sw && !c->opt_unpol && c->model == MODEL_ADAF);
-  const size_t step_bytes = rec_bytes + (split ? OP_DOUBLES * sizeof(double) : 0);
+  // the sweep of the analytic flow keeps operator records too (launch_transfer_sweep_split); its batches run through
+  // launch_transfer as before
+  const bool sweep_split = sw && c->opt_split && !c->opt_unpol && c->model == MODEL_ADAF;
+  const size_t step_bytes = rec_bytes + ((split || sweep_split) ? OP_DOUBLES * sizeof(double) : 0);
   const bool tight = order != nullptr && !bin_prefix.empty() && c->opt_tight;
   struct Batch { int64_t base, cnt; int cap; };
   std::vector<Batch> plan;
@@ -780,7 +860,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     lane_ops = std::max(lane_ops, (no + 255) & ~(size_t)255);
     int rcp;
     if ((rcp = ensure_path(c, lane_path * n_lanes)) != IPOLE_OK) return rcp;
-    if (split && (rcp = ensure_ops(c, lane_ops * n_lanes)) != IPOLE_OK) return rcp;
+    if ((split || sweep_split) && (rcp = ensure_ops(c, lane_ops * n_lanes)) != IPOLE_OK) return rcp;
     return IPOLE_OK;
   };
   if ((rc = prepare(tight)) != IPOLE_OK) return rc;
@@ -811,7 +891,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     std::memset(&t, 0, sizeof t);
     t.cam = c->cam; t.units = c->units; t.model = c->d_model; t.cap = b.cap; t.base = b.base; t.count = b.cnt; t.order = ord;
     t.path = path; t.nsteps = c->d_nsteps; t.queue = c->d_queues + qi;
-    qi += split ? 3 : 1;
+    qi += (split || sweep_split) ? 3 : 1;
     if (use_occ) t.srange = c->d_srange;
     t.I = I; t.Q = Q; t.U = U; t.V = V; t.tau = tau; t.tauF = tauF;
     if (split) rcb = launch_transfer_split(c, t, b.cnt, st, reserve, ops, lane);

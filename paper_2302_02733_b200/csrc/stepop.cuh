@@ -237,6 +237,11 @@ struct ApArgs {
   const int32_t* nsteps;
   unsigned long long* queue;
   double *I, *Q, *U, *V, *tau, *tauF;   // indexed by q
+  // model sweep (k_apply<false, true>; ipole_make_images_adaf): work item = (group of 32 rays, parameter set m).  The operator
+  // records do not depend on the parameter set (flow and field DIRECTION are the model's geometry); its three power laws
+  // come from lane_tab[m], its frequency from units_arr[m] relative to units_ref (the units k_stepop wrote the records with);
+  // outputs of set m start at plane + m * out_stride
+  int n_models; const AdafParams* lane_tab; const Units* units_arr; Units units_ref; size_t out_stride;
 };
 
 #ifndef IPOLE_AP_THREADS
@@ -267,8 +272,9 @@ __device__ __noinline__ Stokes4 stokes_step_qv_closed(double aI, double aQ, doub
 #ifndef IPOLE_AP_EDF_MINB
 #define IPOLE_AP_EDF_MINB 2
 #endif
-template <bool EDF>
+template <bool EDF, bool SWEEP = false>
 __global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? IPOLE_AP_EDF_MINB : IPOLE_AP_MINB) k_apply(const __grid_constant__ ApArgs A) {
+  static_assert(!(EDF && SWEEP), "the sweep is built for the thermal coefficients");
   extern __shared__ double4 edf_nodes_smem[];          // EDF: the per-node constants {x^-1/2, F, G, H} (edf.cuh)
   if (EDF) {
     for (int k = threadIdx.x; k < A.edf.n_nodes; k += blockDim.x) edf_nodes_smem[k] = A.edf.nodes[k];
@@ -278,12 +284,29 @@ __global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? IPOLE_AP_EDF_MINB : IP
   const int lane = threadIdx.x & 31;
   const int64_t count = A.count_dev ? (int64_t)*A.count_dev : A.count;
   const int64_t n_groups = (count + 31) >> 5;
+  const int64_t n_items = SWEEP ? n_groups * A.n_models : n_groups;
   for (;;) {
     __syncwarp();
     long long g = 0;
     if (lane == 0) g = (long long)atomicAdd(A.queue, 1ULL);
     g = __shfl_sync(0xffffffffu, g, 0);
-    if (g >= n_groups) break;
+    if (g >= n_items) break;
+    // SWEEP: consecutive work items are the parameter sets of one ray group, so its records are re-read from L2
+    int mi = 0;
+    AdafParams Mm = A.model;
+    double nu_r = 1.0, ds_r = 1.0, nu3_m = A.nu3;
+    size_t oo = 0;
+    if (SWEEP) {
+      const long long grp = g / A.n_models;
+      mi = (int)(g - grp * A.n_models);
+      g = grp;
+      Mm = A.lane_tab[mi];
+      const Units Um = A.units_arr[mi];
+      nu_r = Um.nu_obs / A.units_ref.nu_obs;       // exactly 1 where the set keeps the camera's frequency
+      ds_r = Um.dl_unit / A.units_ref.dl_unit;
+      nu3_m = Um.nu_obs * Um.nu_obs * Um.nu_obs;
+      oo = (size_t)mi * A.out_stride;
+    }
     const int64_t li = (g << 5) + lane;          // place in the batch's operator buffer
     int32_t q = 0;
     int n = 0;                                   // steps of this lane's ray; 0: nothing to do
@@ -315,12 +338,12 @@ __global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? IPOLE_AP_EDF_MINB : IP
     for (int s = smax - 1; s >= 0; --s) {
       const bool on = s < n;
       const double m11 = R[0], m12 = R[1], m21 = R[2], m22 = R[3];
-      const double x1 = R[4], cosT = R[5], nu = R[6], ds = R[7];
+      const double x1 = R[4], cosT = R[5], nu = SWEEP ? R[6] * nu_r : R[6], ds = SWEEP ? R[7] * ds_r : R[7];
       if (s > 0 && s - 1 < n) load(s - 1);
       if (on) {
         stokes_congruence(m11, m12, m21, m22, S);
         double ne, Th, B;
-        adaf_scalars(A.model, x1, ne, Th, B);
+        adaf_scalars(SWEEP ? Mm : A.model, x1, ne, Th, B);
         const Coeff c = EDF ? synchrotron_edf_invariant(A.edf, edf_nodes, ne, Th, B, cosT, nu) : synchrotron_invariant(ne, Th, B, cosT, nu);
         const double xI = c.aI * ds, xQ = c.aQ * ds, xV = c.aV * ds, yQ = c.rQ * ds, yV = c.rV * ds;
         const double eI = c.jI * ds, eQ = c.jQ * ds, eV = c.jV * ds;
@@ -335,10 +358,10 @@ __global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? IPOLE_AP_EDF_MINB : IP
     }
     if (n > 0) {
       stokes_congruence(mc[0], mc[1], mc[2], mc[3], S);
-      const double nu3 = A.nu3_arr ? A.nu3_arr[q / A.rays_per_cam] : A.nu3;
-      A.I[q] = S[0] * nu3; A.Q[q] = S[1] * nu3; A.U[q] = S[2] * nu3; A.V[q] = S[3] * nu3;
-      if (A.tau) A.tau[q] = tau;
-      if (A.tauF) A.tauF[q] = tauF;
+      const double nu3 = SWEEP ? nu3_m : (A.nu3_arr ? A.nu3_arr[q / A.rays_per_cam] : A.nu3);
+      A.I[oo + q] = S[0] * nu3; A.Q[oo + q] = S[1] * nu3; A.U[oo + q] = S[2] * nu3; A.V[oo + q] = S[3] * nu3;
+      if (A.tau) A.tau[oo + q] = tau;
+      if (A.tauF) A.tauF[oo + q] = tauF;
     }
   }
 }

@@ -71,14 +71,30 @@ def test_sweep_chunks_batches_long_rays_and_host_buffers(ipole):
     for k in A:
         assert np.array_equal(h[k], A[k]), k
     assert np.array_equal(h["flux_jy"], a["flux_jy"])
-    # tiny path buffer: several ray batches, S_cap from the probe; then a slot too small for any ray (long-ray pass)
+    # tiny path buffer: several ray batches, S_cap from the probe; then a slot too small for any ray (long-ray pass).
+    # The bulk of a sweep runs k_stepop once + k_apply per parameter set, its long rays the single sweep kernel: the two
+    # agree to rounding (as for single images), and each is bit-neutral to batching on its own.
+    peak = A["I"][:9].max()
     for opts in ((8 << 20, 2), (12 << 20, 0)):
         g.set_options(*opts)
         b = g.make_images_adaf(models[:9], maps=True)
         st = g.stats()
         assert st["n_batches"] > 1 or st["n_long"] > 0
+        for k in ("I", "Q", "U", "V"):
+            assert np.abs(b[k].cpu().numpy() - A[k][:9]).max() <= 1e-11 * peak, (opts, k)
+        for k in ("tau", "tauF"):
+            assert np.allclose(b[k].cpu().numpy(), A[k][:9], rtol=1e-11, atol=0), (opts, k)
+    g.set_options(0, 1); g.set_transfer_split(False)          # the single sweep kernel everywhere: same bits whatever the batching
+    a0 = g.make_images_adaf(models[:9], maps=True)
+    A0 = {k: a0[k].cpu().numpy() for k in A}
+    for k in ("I", "Q", "U", "V"):
+        assert np.abs(A0[k] - A[k][:9]).max() <= 1e-11 * peak, k
+    for opts in ((8 << 20, 2), (12 << 20, 0)):
+        g.set_options(*opts)
+        b = g.make_images_adaf(models[:9], maps=True)
         for k in A:
-            assert np.array_equal(b[k].cpu().numpy(), A[k][:9]), (opts, k)
+            assert np.array_equal(b[k].cpu().numpy(), A0[k]), (opts, k)
+    g.set_transfer_split(True)
     # the path-free switch does not apply to the sweep (the shared stored path is its point)
     g.set_options(0, 1); g.set_path_free(True)
     c = g.make_images_adaf(models[:3])
@@ -182,9 +198,20 @@ def test_sweep_of_more_than_one_chunk_with_long_rays(ipole):
     cam = W.camera("adaf", 24, max_steps=6000)
     models = [dict(n0=1e6 * (1 + 0.03 * m), Th0=30.0 - 0.2 * (m % 64), B0=30.0 + 0.1 * m) for m in range(70)]
     g = ipole.Ipole(**cam)
+    split = g.make_images_adaf(models)         # bulk through k_stepop + k_apply<sweep>
+    g.set_transfer_split(False)                # long rays take the single sweep kernel: compare like with like
     want = g.make_images_adaf(models)
     assert g.stats()["n_long"] == 0
     W_ = {k: want[k].cpu().numpy() for k in ("I", "Q", "U", "V")}
+    for k in W_:
+        assert np.abs(split[k].cpu().numpy() - W_[k]).max() <= 1e-11 * W_["I"].max(), k
+    # a batch in which k_stepop meets a ray it cannot express falls back to the single sweep kernel as a whole (test mode 2
+    # of the switch declares every seventh ray such a ray)
+    g.set_transfer_split(2)
+    fb = g.make_images_adaf(models)
+    for k in W_:
+        assert np.array_equal(fb[k].cpu().numpy(), W_[k]), k
+    g.set_transfer_split(False)
     for rep in range(3):                       # a race would not show every time
         g.set_options(6 << 20, 0)              # no probe, slots far shorter than the rays: every ray is a long ray
         got = g.make_images_adaf(models)
