@@ -139,7 +139,7 @@ int  ipole_set_path_free(ipole_ctx*, int32_t on);
  * plasma tetrad; ln r, the angle to the field, the frequency in the plasma frame, the step length), and a per-ray
  * kernel evaluates the coefficients from it and applies them, from the far end to the camera.  on == 0: the single
  * per-ray transfer kernel does both (also used, whatever this switch says, for the
- * slab and grid models, the sweeps, the path-free and unpolarized variants, long rays, and rays with a step that
+ * slab and grid models, the grid and unpolarized sweeps, the path-free and unpolarized variants, long rays, and rays with a step that
  * crosses no plasma).  The two give the same image up to rounding.  on == 2 is a test mode: as 1, but every seventh
  * ray of a batch is handed to the single kernel as if it had such a step.  Returns IPOLE_EINVAL for a NULL context. */
 int  ipole_set_transfer_split(ipole_ctx*, int32_t on);
