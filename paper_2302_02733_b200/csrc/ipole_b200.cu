@@ -68,7 +68,7 @@ struct ipole_ctx {
   int32_t* d_irr = nullptr;      // slots of the rays k_stepop leaves to k_transfer
   int32_t *d_rank_pos = nullptr, *d_rank_slot = nullptr;   // k_rank_window: operator-record places of a batch's slots, by position in the order
   int opt_rank = 1;
-  int occ_op = 0, occ_ap = 0, occ_ap_edf = 0;
+  int occ_op = 0, occ_ap = 0, occ_ap_edf = 0, occ_ap_unpol = 0;
   EdfDev edf = {0, 128, 3.5, 0.0, nullptr, nullptr};   // electron distribution of the coefficient step (ipole_set_edf); kind 0: thermal fits
   double4* d_edf_nodes = nullptr; double* d_edf_lnnorm = nullptr;
   int occ_unpol[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};
@@ -362,7 +362,8 @@ int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_
     // stream (long-ray passes) each have their own tables: they run concurrently.
     // analytic flow, bulk batches: the operator records are the same for every parameter set -- k_stepop once, k_apply
     // per set (1: a ray with a step outside the split's reach is in the batch; the single kernel below takes it all)
-    if (c->model == MODEL_ADAF && c->opt_split && !c->opt_unpol && st != c->side && a.path == c->d_path && c->d_ops) {
+    // (unpolarized: the same records serve I alone; worth k_stepop's full geometry from a few parameter sets on)
+    if (c->model == MODEL_ADAF && c->opt_split && (!c->opt_unpol || sw->n_models >= 4) && st != c->side && a.path == c->d_path && c->d_ops) {
       const int r = launch_transfer_sweep_split(c, a, rays, st, sw);
       if (r != 1) return r;
     }
@@ -557,7 +558,9 @@ int launch_transfer_sweep_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cud
     p.tauF = planes[5] ? planes[5] + (size_t)m0 * sw->out_stride : nullptr;
     CK(cudaMemsetAsync(p.queue, 0, sizeof(unsigned long long), st));
     const int s = span_begin(c, LK_APPLY, st);
-    k_apply<false, true><<<grid_for(c, c->occ_ap, IPOLE_AP_THREADS / 32, ((rays + 31) / 32) * mc), IPOLE_AP_THREADS, 0, st>>>(p);
+    const int ga = grid_for(c, c->opt_unpol ? c->occ_ap_unpol : c->occ_ap, IPOLE_AP_THREADS / 32, ((rays + 31) / 32) * mc);
+    if (c->opt_unpol) k_apply_unpol_sweep<<<ga, IPOLE_AP_THREADS, 0, st>>>(p);
+    else k_apply<false, true><<<ga, IPOLE_AP_THREADS, 0, st>>>(p);
     span_end(c, s, st);
     c->stats.n_launches++;
     CK(cudaGetLastError());
@@ -691,7 +694,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     // (per step: the path record and, where the split transfer will run, the operator record -- so that the slots the
     // plan below can afford hold every ray in ONE batch: a pixel list of an adaptive level is a few thousand rays whose
     // time is the latency of the longest, and two batches are twice that)
-    const bool will_split = c->edf.kind != 0 || c->n_mc > 0 || (c->opt_split && !c->opt_unpol && c->model == MODEL_ADAF);
+    const bool will_split = c->edf.kind != 0 || c->n_mc > 0 || (c->opt_split && (!c->opt_unpol || (sw && sw->n_models >= 4)) && c->model == MODEL_ADAF);
     const size_t per_step = rec_bytes + ((will_split && !c->opt_path_free) ? OP_DOUBLES * sizeof(double) : 0);
     const int64_t per = (int64_t)(budget / per_step / (size_t)(((n + 31) / 32) * 32)) - 1;
     cap = (int)std::max<int64_t>(64, std::min<int64_t>(max_steps, per));
@@ -806,7 +809,7 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   const bool split = edf || (c->opt_split && !sw && !c->opt_unpol && c->model == MODEL_ADAF);
   // the sweep of the analytic flow keeps operator records too (launch_transfer_sweep_split); its batches run through
   // launch_transfer as before
-  const bool sweep_split = sw && c->opt_split && !c->opt_unpol && c->model == MODEL_ADAF;
+  const bool sweep_split = sw && c->opt_split && (!c->opt_unpol || sw->n_models >= 4) && c->model == MODEL_ADAF;
   const size_t step_bytes = rec_bytes + ((split || sweep_split) ? OP_DOUBLES * sizeof(double) : 0);
   const bool tight = order != nullptr && !bin_prefix.empty() && c->opt_tight;
   struct Batch { int64_t base, cnt; int cap; };
@@ -1113,6 +1116,7 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_group_mc, k_transfer_group<MODEL_GRID, true>, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo_f32, k_geodesic_f32, IPOLE_GEO_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap, k_apply<false>, IPOLE_AP_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_unpol, k_apply_unpol_sweep, IPOLE_AP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_edf, k_apply<true>, IPOLE_AP_THREADS, EDF_MAX_NODES * sizeof(double4));
   { const char* e = std::getenv("IPOLE_NO_SPLIT"); if (e && e[0] == '1') c->opt_split = 0; }
   { const char* e = std::getenv("IPOLE_NO_TIGHT"); if (e && e[0] == '1') c->opt_tight = 0; }

@@ -366,4 +366,70 @@ __global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? IPOLE_AP_EDF_MINB : IP
   }
 }
 
+// Unpolarized sweep ("nonpolarized images" of the fitting loop; R-12) on the same operator records:
+// I alone needs their second half only -- ln r, the angle to the field, the frequency, the step length -- and per
+// parameter set the three power laws, j_I, alpha_I and the exact scalar step of k_transfer_unpol:
+//   I <- I e^{-x} + j ds (1 - e^{-x})/x,  x = alpha ds.
+// Work items and lockstep walk as in k_apply<false, true>.
+#ifndef IPOLE_APU_MINB
+#define IPOLE_APU_MINB 4
+#endif
+__global__ void __launch_bounds__(IPOLE_AP_THREADS, IPOLE_APU_MINB) k_apply_unpol_sweep(const __grid_constant__ ApArgs A) {
+  const int lane = threadIdx.x & 31;
+  const int64_t count = A.count;
+  const int64_t n_groups = (count + 31) >> 5;
+  const int64_t n_items = n_groups * A.n_models;
+  for (;;) {
+    __syncwarp();
+    long long g = 0;
+    if (lane == 0) g = (long long)atomicAdd(A.queue, 1ULL);
+    g = __shfl_sync(0xffffffffu, g, 0);
+    if (g >= n_items) break;
+    const long long grp = g / A.n_models;
+    const int mi = (int)(g - grp * A.n_models);
+    const AdafParams Mm = A.lane_tab[mi];
+    const Units Um = A.units_arr[mi];
+    const double nu_r = Um.nu_obs / A.units_ref.nu_obs, ds_r = Um.dl_unit / A.units_ref.dl_unit;
+    const size_t oo = (size_t)mi * A.out_stride;
+    const int64_t li = (grp << 5) + lane;
+    int32_t q = 0;
+    int n = 0;
+    if (li < count) {
+      const int64_t ls = A.slot ? (int64_t)A.slot[A.base + li] : li;
+      q = A.order ? A.order[A.base + ls] : (int32_t)(A.base + ls);
+      n = A.nsteps[q];
+      if (n < 0) n = 0;                          // overflowed its slot: long-ray pass
+    }
+    int smax = n;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) smax = max(smax, __shfl_xor_sync(0xffffffffu, smax, o));
+    double I = 0.0, tau = 0.0;
+    double R[4] = {0, 0, 0, 0};
+    const double* base = A.ops + op_addr(li, A.cap, 0, 1);   // part 1 of step s at base + s * OP_PARTS * 128
+    auto load = [&](int s) { ld_global_v4(base + (size_t)s * (OP_PARTS * 128), R[0], R[1], R[2], R[3]); };
+    if (smax > 0 && smax - 1 < n) load(smax - 1);
+    for (int s = smax - 1; s >= 0; --s) {
+      const bool on = s < n;
+      const double x1 = R[0], cosT = R[1], nu = R[2] * nu_r, ds = R[3] * ds_r;
+      if (s > 0 && s - 1 < n) load(s - 1);
+      if (on) {
+        double ne, Th, B;
+        adaf_scalars(Mm, x1, ne, Th, B);
+        const Coeff c = synchrotron_invariant(ne, Th, B, cosT, nu);
+        const double x = c.aI * ds;
+        const double em = ip_expm1(-x);
+        const double E = (x > 0.0) ? -em * ip_rcp(x) : 1.0;
+        I = I + I * em + c.jI * ds * E;
+        tau += x;
+      }
+    }
+    if (n > 0) {
+      const double nu3 = Um.nu_obs * Um.nu_obs * Um.nu_obs;
+      A.I[oo + q] = I * nu3; A.Q[oo + q] = 0.0; A.U[oo + q] = 0.0; A.V[oo + q] = 0.0;
+      if (A.tau) A.tau[oo + q] = tau;
+      if (A.tauF) A.tauF[oo + q] = 0.0;
+    }
+  }
+}
+
 }  // namespace ipole
