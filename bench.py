@@ -36,6 +36,9 @@ FLOP_EXECUTED = {"k_stepop": 1019.0, "k_apply": 578.0, "k_transfer<adaf>": 1576.
                  "k_geodesic": 839.0, "k_geodesic<occ>": 1020.0}
 # second physics workload (--edf): k_apply<true> per step, 128 quadrature nodes (profiles/r2_k_apply_edf{1,2}_adaf256.txt)
 FLOP_EXECUTED.update({"k_apply<edf 1>": 11558.0, "k_apply<edf 2>": 18290.0})
+# unpolarized sweep on the operator records, per (step, parameter set): ncu per-launch counters of two launches of a sweep128 call
+# (1.047e12 flop over 2.981e9 pairs; 216 FP64 instructions per pair, FP64 pipe 68.9 %)
+FLOP_EXECUTED["k_apply_unpol_sweep"] = 351.0
 FP64_PIPE_PCT = {"k_stepop": 72.6, "k_apply": 61.7, "k_transfer<adaf>": 58.5, "k_transfer_group<grid>": 50.6,
                  "k_geodesic": 82.5, "k_geodesic<occ>": 79.5, "k_apply<edf 1>": 75.4, "k_apply<edf 2>": 70.1}
 # DRAM bytes per step of k_transfer (dram__bytes_read + write of one launch / its thread-steps, same captures)
@@ -147,6 +150,13 @@ def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier,
     ach = fl_step * steps_rt / (rt_ms * 1e-3) / 1e12
     kname = "k_transfer<%s, sweep>" % wl["kind"]
     flop_note = "flop per step of the single-image kernel (the sweep runs the same arithmetic per pair)"
+    if st.get("ms_stepop", 0.0) > 0.0 and args.unpolarized:
+        flop = st["total_steps"] * (FLOP_EXECUTED["k_stepop"] + M * FLOP_EXECUTED["k_apply_unpol_sweep"])
+        ach = flop / (rt_ms * 1e-3) / 1e12
+        fl_step = flop / steps_rt
+        kname = "k_stepop<adaf> (once) + k_apply_unpol_sweep (per parameter set)"
+        flop_note = ("executed flop per (step, parameter set): k_apply_unpol_sweep's %.0f plus k_stepop's %.0f shared by the %d sets of a "
+                     "call (the single unpolarized kernel: 652 per pair)" % (FLOP_EXECUTED["k_apply_unpol_sweep"], FLOP_EXECUTED["k_stepop"], M))
     if st.get("ms_stepop", 0.0) > 0.0 and not args.unpolarized:
         # analytic flow through the split kernels: k_stepop ONCE per call, k_apply once per parameter set.  The work the sets
         # share is counted once: executed flop (profiles/r2_image_flops.md) of k_stepop x steps + of k_apply x steps x M
