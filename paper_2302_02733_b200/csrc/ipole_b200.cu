@@ -13,6 +13,7 @@
 #include <vector>
 #include "kernels.cuh"
 #include "stepop.cuh"
+#include "gridsweep.cuh"
 #include "geo_f32.cuh"
 #include "adaptive.cuh"
 
@@ -68,7 +69,7 @@ struct ipole_ctx {
   int32_t* d_irr = nullptr;      // slots of the rays k_stepop leaves to k_transfer
   int32_t *d_rank_pos = nullptr, *d_rank_slot = nullptr;   // k_rank_window: operator-record places of a batch's slots, by position in the order
   int opt_rank = 1;
-  int occ_op = 0, occ_ap = 0, occ_ap_edf = 0, occ_ap_unpol = 0;
+  int occ_op = 0, occ_ap = 0, occ_ap_edf = 0, occ_ap_unpol = 0, occ_gridop = 0, occ_gridapply = 0;
   EdfDev edf = {0, 128, 3.5, 0.0, nullptr, nullptr};   // electron distribution of the coefficient step (ipole_set_edf); kind 0: thermal fits
   double4* d_edf_nodes = nullptr; double* d_edf_lnnorm = nullptr;
   int occ_unpol[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};
@@ -341,6 +342,7 @@ void launch_transfer_model(int model, int g, cudaStream_t st, const RtArgs& a) {
 }
 
 int launch_transfer_sweep_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStream_t st, const Sweep* sw);
+int launch_transfer_gridsweep_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStream_t st, const Sweep* sw);
 
 // pf: 0 stored path, 1 path-free with eps <= 0.04, 2 path-free with any eps
 int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_t st, int reserve = 0, int pf = 0,
@@ -367,6 +369,9 @@ int launch_transfer(ipole_ctx* c, RtArgs& a, int kind, int64_t rays, cudaStream_
       const int r = launch_transfer_sweep_split(c, a, rays, st, sw);
       if (r != 1) return r;
     }
+    // grid model, bulk batches: gather, flow, tetrad and leg transport once per call, coefficients and Stokes update per set
+    if (c->model == MODEL_GRID && c->opt_split && !c->opt_unpol && st != c->side && a.path == c->d_path && c->d_ops && a.srange)
+      return launch_transfer_gridsweep_split(c, a, rays, st, sw);
     void* tab_models = (st == c->side) ? c->d_sweep_models_side : c->d_sweep_models;
     Units* tab_units = (st == c->side) ? c->d_sweep_units_side : c->d_sweep_units;
     RtArgs t = a;
@@ -568,6 +573,55 @@ int launch_transfer_sweep_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cud
   return IPOLE_OK;
 }
 
+// Model sweep of the grid model with the geometry done once (gridsweep.cuh): k_gridop walks every ray of the batch once and
+// leaves a compact record per plasma step, k_gridapply_sweep walks the compact records once per parameter set.
+int launch_transfer_gridsweep_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStream_t st, const Sweep* sw) {
+  int32_t* npl = c->d_irr;                   // (the irregular-ray lists of the analytic split are not in use here)
+  const bool rank = c->opt_rank && rays > 32;
+  if (rank) {
+    RankArgs r = {a.base, a.count, nullptr, a.order, a.nsteps, c->d_rank_pos, c->d_rank_slot, a.srange};
+    const int s = span_begin(c, LK_OPS, st);
+    k_rank_window<<<(unsigned)((rays + RANK_WINDOW - 1) / RANK_WINDOW), RANK_WINDOW, 0, st>>>(r);
+    span_end(c, s, st);
+    c->stats.n_launches++;
+  }
+  {
+    GopArgs o;
+    std::memset(&o, 0, sizeof o);
+    o.cam = a.cam; o.units = a.units; o.model = a.model; o.cap = a.cap; o.base = a.base; o.count = a.count; o.order = a.order;
+    o.path = a.path; o.nsteps = a.nsteps; o.srange = a.srange; o.rank_slot = rank ? c->d_rank_slot : nullptr;
+    o.queue = a.queue; o.ops = c->d_ops; o.npl = npl;
+    const int s = span_begin(c, LK_OPS, st);
+    k_gridop<<<grid_for(c, c->occ_gridop, IPOLE_RT_THREADS / 32, (rays + 31) / 32), IPOLE_RT_THREADS, 0, st>>>(o);
+    span_end(c, s, st);
+    c->stats.n_launches++;
+    CK(cudaGetLastError());
+  }
+  GapArgs p;
+  std::memset(&p, 0, sizeof p);
+  p.cap = a.cap; p.base = a.base; p.count = a.count; p.order = a.order; p.rank_slot = rank ? c->d_rank_slot : nullptr;
+  p.ops = c->d_ops; p.npl = npl; p.queue = a.queue + 1;
+  p.lane_tab = (const GridScales*)c->d_sweep_models; p.units_arr = c->d_sweep_units; p.units_ref = a.units; p.out_stride = sw->out_stride;
+  double* planes[6] = {a.I, a.Q, a.U, a.V, a.tau, a.tauF};
+  for (int m0 = 0; m0 < sw->n_models; m0 += SWEEP_MAX_MODELS) {
+    const int mc = std::min(SWEEP_MAX_MODELS, sw->n_models - m0);
+    CK(cudaMemcpyAsync(c->d_sweep_models, (const char*)sw->lane_tab + (size_t)m0 * sw->lane_bytes, mc * sw->lane_bytes, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(c->d_sweep_units, sw->units + m0, mc * sizeof(Units), cudaMemcpyHostToDevice, st));
+    p.n_models = mc;
+    p.I = planes[0] + (size_t)m0 * sw->out_stride; p.Q = planes[1] + (size_t)m0 * sw->out_stride;
+    p.U = planes[2] + (size_t)m0 * sw->out_stride; p.V = planes[3] + (size_t)m0 * sw->out_stride;
+    p.tau = planes[4] ? planes[4] + (size_t)m0 * sw->out_stride : nullptr;
+    p.tauF = planes[5] ? planes[5] + (size_t)m0 * sw->out_stride : nullptr;
+    CK(cudaMemsetAsync(p.queue, 0, sizeof(unsigned long long), st));
+    const int s = span_begin(c, LK_APPLY, st);
+    k_gridapply_sweep<<<grid_for(c, c->occ_gridapply, IPOLE_AP_THREADS / 32, ((rays + 31) / 32) * mc), IPOLE_AP_THREADS, 0, st>>>(p);
+    span_end(c, s, st);
+    c->stats.n_launches++;
+    CK(cudaGetLastError());
+  }
+  return IPOLE_OK;
+}
+
 GeoArgs geo_args(ipole_ctx* c) {
   GeoArgs g;
   std::memset(&g, 0, sizeof g);
@@ -695,7 +749,8 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     // plan below can afford hold every ray in ONE batch: a pixel list of an adaptive level is a few thousand rays whose
     // time is the latency of the longest, and two batches are twice that)
     const bool will_split = c->edf.kind != 0 || c->n_mc > 0 || (c->opt_split && (!c->opt_unpol || (sw && sw->n_models >= 4)) && c->model == MODEL_ADAF);
-    const size_t per_step = rec_bytes + ((will_split && !c->opt_path_free) ? OP_DOUBLES * sizeof(double) : 0);
+    const bool will_grid = sw && c->opt_split && !c->opt_unpol && c->model == MODEL_GRID && c->opt_occ;
+    const size_t per_step = rec_bytes + (will_grid ? GOP_DOUBLES * sizeof(double) : (will_split && !c->opt_path_free) ? OP_DOUBLES * sizeof(double) : 0);
     const int64_t per = (int64_t)(budget / per_step / (size_t)(((n + 31) / 32) * 32)) - 1;
     cap = (int)std::max<int64_t>(64, std::min<int64_t>(max_steps, per));
   }
@@ -809,8 +864,10 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   const bool split = edf || (c->opt_split && !sw && !c->opt_unpol && c->model == MODEL_ADAF);
   // the sweep of the analytic flow keeps operator records too (launch_transfer_sweep_split); its batches run through
   // launch_transfer as before
-  const bool sweep_split = sw && c->opt_split && (!c->opt_unpol || sw->n_models >= 4) && c->model == MODEL_ADAF;
-  const size_t step_bytes = rec_bytes + ((split || sweep_split) ? OP_DOUBLES * sizeof(double) : 0);
+  const bool grid_sweep_split = sw && c->opt_split && !c->opt_unpol && c->model == MODEL_GRID && use_occ;   // gridsweep.cuh
+  const bool sweep_split = grid_sweep_split || (sw && c->opt_split && (!c->opt_unpol || sw->n_models >= 4) && c->model == MODEL_ADAF);
+  const size_t op_doubles = grid_sweep_split ? GOP_DOUBLES : OP_DOUBLES;
+  const size_t step_bytes = rec_bytes + ((split || sweep_split) ? op_doubles * sizeof(double) : 0);
   const bool tight = order != nullptr && !bin_prefix.empty() && c->opt_tight;
   struct Batch { int64_t base, cnt; int cap; };
   std::vector<Batch> plan;
@@ -851,13 +908,13 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
     size_t np = 0, no = 0;
     for (const Batch& b : plan) {
       np = std::max(np, (size_t)b.cnt * (size_t)(b.cap + 1) * rec_bytes);
-      no = std::max(no, (size_t)((b.cnt + 31) / 32 * 32) * (size_t)(b.cap + 1) * OP_DOUBLES * sizeof(double));
+      no = std::max(no, (size_t)((b.cnt + 31) / 32 * 32) * (size_t)(b.cap + 1) * op_doubles * sizeof(double));
     }
     if (with_retry_level) {   // the retry level runs with the global S_cap
       const int64_t Br = std::max<int64_t>(1, (int64_t)(lane_budget / ((size_t)(cap + 1) * step_bytes)));
       const int64_t rr = std::min<int64_t>(Br, std::max<int64_t>(n / 8, 1));   // more than n/8 retries never happen; the buffer grows if they do
       np = std::max(np, (size_t)rr * (size_t)(cap + 1) * rec_bytes);
-      no = std::max(no, (size_t)((rr + 31) / 32 * 32) * (size_t)(cap + 1) * OP_DOUBLES * sizeof(double));
+      no = std::max(no, (size_t)((rr + 31) / 32 * 32) * (size_t)(cap + 1) * op_doubles * sizeof(double));
     }
     lane_path = std::max(lane_path, (np + 255) & ~(size_t)255);
     lane_ops = std::max(lane_ops, (no + 255) & ~(size_t)255);
@@ -1117,6 +1174,8 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo_f32, k_geodesic_f32, IPOLE_GEO_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap, k_apply<false>, IPOLE_AP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_unpol, k_apply_unpol_sweep, IPOLE_AP_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_gridop, k_gridop, IPOLE_RT_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_gridapply, k_gridapply_sweep, IPOLE_AP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_edf, k_apply<true>, IPOLE_AP_THREADS, EDF_MAX_NODES * sizeof(double4));
   { const char* e = std::getenv("IPOLE_NO_SPLIT"); if (e && e[0] == '1') c->opt_split = 0; }
   { const char* e = std::getenv("IPOLE_NO_TIGHT"); if (e && e[0] == '1') c->opt_tight = 0; }

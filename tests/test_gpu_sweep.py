@@ -152,6 +152,23 @@ def test_grid_sweep_equals_single_images_and_oracle(ipole, ref):
     for k in ("I", "Q", "U", "V"):
         A = a[k].cpu().numpy()
         assert np.array_equal(A[0:6], A[64:70]) and np.array_equal(h[k], A), k
+    # The bulk of a grid sweep runs k_gridop once + k_gridapply_sweep per set (gridsweep.cuh), long rays the single sweep
+    # kernel.  Several ray batches, then slots too short for any ray (every ray a long ray), then the single kernel
+    # everywhere (ipole_set_transfer_split(0)): the same images to rounding, amplified where the Faraday depth is large.
+    A = {k: a[k].cpu().numpy()[:9] for k in ("I", "Q", "U", "V")}
+    peak = A["I"].max()
+    for opts, split in (((8 << 20, 2), True), ((12 << 20, 0), True), ((0, 1), False)):
+        g.set_options(*opts); g.set_transfer_split(split)
+        b = g.make_images_grid(many[:9])
+        st = g.stats()
+        if split:
+            assert st["n_batches"] > 1 or st["n_long"] > 0
+        else:
+            assert st["ms_stepop"] == 0
+        for k in A:
+            assert np.abs(b[k].cpu().numpy() - A[k]).max() <= 1e-9 * peak, (opts, split, k)
+    g.set_options(0, 1); g.set_transfer_split(True)
+    assert g.make_images_grid(many[:2]) is not None and g.stats()["ms_stepop"] > 0
     # errors
     with pytest.raises(ipole.IpoleError):
         g.make_images_grid([dict(M_unit=0.0, Rlow=1.0, Rhigh=1.0)])
