@@ -39,6 +39,9 @@ FLOP_EXECUTED.update({"k_apply<edf 1>": 11558.0, "k_apply<edf 2>": 18290.0})
 # unpolarized sweep on the operator records, per (step, parameter set): ncu per-launch counters of two launches of a sweep128 call
 # (1.047e12 flop over 2.981e9 pairs; 216 FP64 instructions per pair, FP64 pipe 68.9 %)
 FLOP_EXECUTED["k_apply_unpol_sweep"] = 351.0
+# grid sweep (gridsweep.cuh), per step of a RAY (all its steps): k_gridop once per call, k_gridapply_sweep per parameter set
+# (ncu per-launch counters of a gridsweep128 call: 359.0, and 3647.6 for 64 sets)
+FLOP_EXECUTED.update({"k_gridop": 359.0, "k_gridapply_sweep": 57.0})
 FP64_PIPE_PCT = {"k_stepop": 72.6, "k_apply": 61.7, "k_transfer<adaf>": 58.5, "k_transfer_group<grid>": 50.6,
                  "k_geodesic": 82.5, "k_geodesic<occ>": 79.5, "k_apply<edf 1>": 75.4, "k_apply<edf 2>": 70.1}
 # DRAM bytes per step of k_transfer (dram__bytes_read + write of one launch / its thread-steps, same captures)
@@ -150,14 +153,23 @@ def run_sweep(args, g, ipole, replicas, W, wl, cam, world, rank, local, barrier,
     ach = fl_step * steps_rt / (rt_ms * 1e-3) / 1e12
     kname = "k_transfer<%s, sweep>" % wl["kind"]
     flop_note = "flop per step of the single-image kernel (the sweep runs the same arithmetic per pair)"
-    if st.get("ms_stepop", 0.0) > 0.0 and args.unpolarized:
+    if st.get("ms_stepop", 0.0) > 0.0 and wl["kind"] == "grid" and not args.unpolarized:
+        flop = st["total_steps"] * (FLOP_EXECUTED["k_gridop"] + M * FLOP_EXECUTED["k_gridapply_sweep"])
+        ach = flop / (rt_ms * 1e-3) / 1e12
+        fl_step = flop / steps_rt
+        kname = "k_gridop (once) + k_gridapply_sweep (per parameter set)"
+        flop_note = ("executed flop per (step of a ray, parameter set): k_gridapply_sweep's %.0f plus k_gridop's %.0f shared by the %d sets "
+                     "of a call; the single sweep kernel's frozen count is 390 per pair, so the call does %.1fx the images per FP64 operation "
+                     "-- and the launches are short and latency-bound, which is what the low fraction says"
+                     % (FLOP_EXECUTED["k_gridapply_sweep"], FLOP_EXECUTED["k_gridop"], M, FLOP_PER_STEP[fkey] / fl_step))
+    elif st.get("ms_stepop", 0.0) > 0.0 and args.unpolarized:
         flop = st["total_steps"] * (FLOP_EXECUTED["k_stepop"] + M * FLOP_EXECUTED["k_apply_unpol_sweep"])
         ach = flop / (rt_ms * 1e-3) / 1e12
         fl_step = flop / steps_rt
         kname = "k_stepop<adaf> (once) + k_apply_unpol_sweep (per parameter set)"
         flop_note = ("executed flop per (step, parameter set): k_apply_unpol_sweep's %.0f plus k_stepop's %.0f shared by the %d sets of a "
                      "call (the single unpolarized kernel: 652 per pair)" % (FLOP_EXECUTED["k_apply_unpol_sweep"], FLOP_EXECUTED["k_stepop"], M))
-    if st.get("ms_stepop", 0.0) > 0.0 and not args.unpolarized:
+    elif st.get("ms_stepop", 0.0) > 0.0:
         # analytic flow through the split kernels: k_stepop ONCE per call, k_apply once per parameter set.  The work the sets
         # share is counted once: executed flop (profiles/r2_image_flops.md) of k_stepop x steps + of k_apply x steps x M
         flop = st["total_steps"] * (FLOP_EXECUTED["k_stepop"] + M * FLOP_EXECUTED["k_apply"])
