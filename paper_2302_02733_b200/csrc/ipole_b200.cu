@@ -69,7 +69,7 @@ struct ipole_ctx {
   int32_t* d_irr = nullptr;      // slots of the rays k_stepop leaves to k_transfer
   int32_t *d_rank_pos = nullptr, *d_rank_slot = nullptr;   // k_rank_window: operator-record places of a batch's slots, by position in the order
   int opt_rank = 1;
-  int occ_op = 0, occ_ap = 0, occ_ap_edf = 0, occ_ap_unpol = 0, occ_gridop = 0, occ_gridapply = 0;
+  int occ_op = 0, occ_ap = 0, occ_ap_edf = 0, occ_ap_unpol = 0, occ_gridop = 0, occ_gridapply = 0, occ_ap_wide = 0;
   EdfDev edf = {0, 128, 3.5, 0.0, nullptr, nullptr};   // electron distribution of the coefficient step (ipole_set_edf); kind 0: thermal fits
   double4* d_edf_nodes = nullptr; double* d_edf_lnnorm = nullptr;
   int occ_unpol[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};
@@ -485,6 +485,8 @@ int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStrea
     p.edf = c->edf;
     if (c->n_mc) { p.nu3_arr = c->d_mc_nu3; p.rays_per_cam = c->mc_rays_per_cam; }
     if (c->edf.kind != 0) k_apply<true><<<grid_for(c, c->occ_ap_edf, IPOLE_AP_THREADS / 32, (rays + 31) / 32, reserve), IPOLE_AP_THREADS, (size_t)c->edf.n_nodes * sizeof(double4), st>>>(p);
+    else if (c->opt_lowlat && rays <= (int64_t)c->n_sm * IPOLE_AP_THREADS * 2)   // the launch cannot fill the GPU: a warp per ray (stepop.cuh)
+      k_apply_wide<<<grid_for(c, c->occ_ap_wide, IPOLE_AP_THREADS / 32, rays, reserve), IPOLE_AP_THREADS, 0, st>>>(p);
     else k_apply<false><<<g, IPOLE_AP_THREADS, 0, st>>>(p);
     span_end(c, s, st);
     c->stats.n_launches++;
@@ -1174,6 +1176,7 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo_f32, k_geodesic_f32, IPOLE_GEO_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap, k_apply<false>, IPOLE_AP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_unpol, k_apply_unpol_sweep, IPOLE_AP_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_wide, k_apply_wide, IPOLE_AP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_gridop, k_gridop, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_gridapply, k_gridapply_sweep, IPOLE_AP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_edf, k_apply<true>, IPOLE_AP_THREADS, EDF_MAX_NODES * sizeof(double4));

@@ -240,14 +240,20 @@ __device__ __forceinline__ void levi4(const double p[4], const double q[4], cons
 // Stokes vector under the real 2x2 congruence n <- M n M^T
 __device__ __forceinline__ void stokes_congruence(const double m11, const double m12, const double m21, const double m22,
                                                   double S[4]) {
+  // Every rounding is spelt out (no contraction left to the compiler): kernels that walk the same ray in different ways
+  // (k_apply, k_apply_wide) must reach the same bits.
   const double R11 = 0.5 * (S[0] + S[1]), R22 = 0.5 * (S[0] - S[1]), R12 = 0.5 * S[2];
-  const double T11 = m11 * m11 * R11 + 2.0 * m11 * m12 * R12 + m12 * m12 * R22;
-  const double T22 = m21 * m21 * R11 + 2.0 * m21 * m22 * R12 + m22 * m22 * R22;
-  const double T12 = m11 * m21 * R11 + (m11 * m22 + m12 * m21) * R12 + m12 * m22 * R22;
-  S[0] = T11 + T22;
-  S[1] = T11 - T22;
+  const double a11 = __dmul_rn(m11, m11), a12 = __dmul_rn(m11, m12), a22 = __dmul_rn(m12, m12);
+  const double b11 = __dmul_rn(m21, m21), b12 = __dmul_rn(m21, m22), b22 = __dmul_rn(m22, m22);
+  const double c11 = __dmul_rn(m11, m21), c22 = __dmul_rn(m12, m22);
+  const double c12 = fma(m12, m21, __dmul_rn(m11, m22)), det = fma(-m12, m21, __dmul_rn(m11, m22));
+  const double T11 = fma(a22, R22, fma(2.0 * a12, R12, __dmul_rn(a11, R11)));
+  const double T22 = fma(b22, R22, fma(2.0 * b12, R12, __dmul_rn(b11, R11)));
+  const double T12 = fma(c22, R22, fma(c12, R12, __dmul_rn(c11, R11)));
+  S[0] = __dadd_rn(T11, T22);
+  S[1] = __dadd_rn(T11, -T22);
   S[2] = 2.0 * T12;
-  S[3] = (m11 * m22 - m12 * m21) * S[3];
+  S[3] = __dmul_rn(det, S[3]);
 }
 
 struct PolState {

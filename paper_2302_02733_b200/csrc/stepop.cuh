@@ -345,15 +345,17 @@ __global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? IPOLE_AP_EDF_MINB : IP
         double ne, Th, B;
         adaf_scalars(SWEEP ? Mm : A.model, x1, ne, Th, B);
         const Coeff c = EDF ? synchrotron_edf_invariant(A.edf, edf_nodes, ne, Th, B, cosT, nu) : synchrotron_invariant(ne, Th, B, cosT, nu);
-        const double xI = c.aI * ds, xQ = c.aQ * ds, xV = c.aV * ds, yQ = c.rQ * ds, yV = c.rV * ds;
-        const double eI = c.jI * ds, eQ = c.jQ * ds, eV = c.jV * ds;
+        // (products rounded on their own, not contracted into the sums of the step: k_apply_wide hands the same eight
+        // numbers from lane to lane and must get the same bits)
+        const double xI = __dmul_rn(c.aI, ds), xQ = __dmul_rn(c.aQ, ds), xV = __dmul_rn(c.aV, ds), yQ = __dmul_rn(c.rQ, ds), yV = __dmul_rn(c.rV, ds);
+        const double eI = __dmul_rn(c.jI, ds), eQ = __dmul_rn(c.jQ, ds), eV = __dmul_rn(c.jV, ds);
         if (IP_UNLIKELY(!stokes_step_qv_series(xI, xQ, xV, yQ, yV, 1.0, eI, eQ, eV, S))) {
           const Stokes4 in = {S[0], S[1], S[2], S[3]};
           const Stokes4 o = stokes_step_qv_closed(xI, xQ, xV, yQ, yV, eI, eQ, eV, in);
           S[0] = o.I; S[1] = o.Q; S[2] = o.U; S[3] = o.V;
         }
-        tau += xI;
-        tauF += fabs(yV);
+        tau = __dadd_rn(tau, xI);                // (no contraction with the product above: k_apply_wide adds the same numbers)
+        tauF = __dadd_rn(tauF, fabs(yV));
       }
     }
     if (n > 0) {
@@ -362,6 +364,70 @@ __global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? IPOLE_AP_EDF_MINB : IP
       A.I[oo + q] = S[0] * nu3; A.Q[oo + q] = S[1] * nu3; A.U[oo + q] = S[2] * nu3; A.V[oo + q] = S[3] * nu3;
       if (A.tau) A.tau[oo + q] = tau;
       if (A.tauF) A.tauF[oo + q] = tauF;
+    }
+  }
+}
+
+// k_apply for launches that cannot fill the GPU (adaptive levels, retry and long-ray passes, pixel lists, small images):
+// ONE WARP PER RAY.  The lockstep kernel above gives every ray one lane, and a lone photon-ring ray of 4 500 steps is then
+// 4 500 x ~700 dependent instructions = 9 ms however empty the GPU is.  Here the 32 lanes take 32 consecutive steps of the
+// ray and evaluate their scalars and coefficients side by side (they do not depend on the Stokes numbers); only the
+// congruence and the 4x4 step run in sequence, every lane doing the same update on values broadcast from the lane that
+// owns the step.  Per ray the arithmetic and its order are k_apply's (same functions, same operands).
+__global__ void __launch_bounds__(IPOLE_AP_THREADS, IPOLE_AP_MINB) k_apply_wide(const __grid_constant__ ApArgs A) {
+  const int lane = threadIdx.x & 31;
+  const int64_t count = A.count_dev ? (int64_t)*A.count_dev : A.count;
+  for (;;) {
+    __syncwarp();
+    long long li = 0;                            // place in the batch's operator buffer
+    if (lane == 0) li = (long long)atomicAdd(A.queue, 1ULL);
+    li = __shfl_sync(0xffffffffu, li, 0);
+    if (li >= count) break;
+    const int64_t ls = A.slot ? (int64_t)A.slot[A.base + li] : li;
+    const int32_t q = A.order ? A.order[A.base + ls] : (int32_t)(A.base + ls);
+    int n = A.nsteps[q];
+    if (n < 0) continue;                         // overflowed its slot: long-ray pass
+    double mc[4], flag, z0, z1, z2;
+    ld_global_v4(A.ops + op_addr(li, A.cap, n, 0), mc[0], mc[1], mc[2], mc[3]);
+    ld_global_v4(A.ops + op_addr(li, A.cap, n, 1), flag, z0, z1, z2);
+    if (flag != 0.0) continue;                   // irregular: rendered by k_transfer
+    double S[4] = {0, 0, 0, 0}, tau = 0.0, tauF = 0.0;
+    const double* base = A.ops + op_addr(li, A.cap, 0, 0);
+    for (int s_top = n - 1; s_top >= 0; s_top -= 32) {
+      const int s = s_top - lane;                // this lane's step of the chunk (the chunk is walked from lane 0 on)
+      double v[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+      if (s >= 0) {
+        const double* p = base + (size_t)s * (OP_PARTS * 128);
+        double x1, cosT, nu, ds;
+        ld_global_v4(p, v[0], v[1], v[2], v[3]);
+        ld_global_v4(p + 128, x1, cosT, nu, ds);
+        double ne, Th, B;
+        adaf_scalars(A.model, x1, ne, Th, B);
+        const Coeff c = synchrotron_invariant(ne, Th, B, cosT, nu);
+        v[4] = __dmul_rn(c.aI, ds); v[5] = __dmul_rn(c.aQ, ds); v[6] = __dmul_rn(c.aV, ds); v[7] = __dmul_rn(c.rQ, ds); v[8] = __dmul_rn(c.rV, ds);
+        v[9] = __dmul_rn(c.jI, ds); v[10] = __dmul_rn(c.jQ, ds); v[11] = __dmul_rn(c.jV, ds);
+      }
+      const int m = min(32, s_top + 1);
+      for (int j = 0; j < m; ++j) {
+        double w[12];
+#pragma unroll
+        for (int i = 0; i < 12; ++i) w[i] = __shfl_sync(0xffffffffu, v[i], j);
+        stokes_congruence(w[0], w[1], w[2], w[3], S);
+        if (IP_UNLIKELY(!stokes_step_qv_series(w[4], w[5], w[6], w[7], w[8], 1.0, w[9], w[10], w[11], S))) {
+          const Stokes4 in = {S[0], S[1], S[2], S[3]};
+          const Stokes4 o = stokes_step_qv_closed(w[4], w[5], w[6], w[7], w[8], w[9], w[10], w[11], in);
+          S[0] = o.I; S[1] = o.Q; S[2] = o.U; S[3] = o.V;
+        }
+        tau = __dadd_rn(tau, w[4]);
+        tauF = __dadd_rn(tauF, fabs(w[8]));
+      }
+    }
+    if (lane == 0) {
+      stokes_congruence(mc[0], mc[1], mc[2], mc[3], S);
+      const double nu3 = A.nu3_arr ? A.nu3_arr[q / A.rays_per_cam] : A.nu3;
+      A.I[q] = S[0] * nu3; A.Q[q] = S[1] * nu3; A.U[q] = S[2] * nu3; A.V[q] = S[3] * nu3;
+      if (A.tau) A.tau[q] = tau;
+      if (A.tauF) A.tauF[q] = tauF;
     }
   }
 }

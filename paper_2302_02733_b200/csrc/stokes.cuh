@@ -138,29 +138,30 @@ __device__ __forceinline__ bool stokes_step_qv_series(double aI, double aQ, doub
                                                       double jI, double jQ, double jV, double S[4]) {
   const double nb = fabs(s) * (fabs(aI) + fabs(aQ) + fabs(aV) + fabs(rQ) + fabs(rV));
   if (IP_UNLIKELY(!(nb < 0.0078125))) return false;
-  double w0 = s * (jI - (aI * S[0] + aQ * S[1] + aV * S[3]));
-  double w1 = s * (jQ - (aQ * S[0] + aI * S[1] + rV * S[2]));
-  double w2 = s * (rV * S[1] - aI * S[2] - rQ * S[3]);
-  double w3 = s * (jV - (aV * S[0] - rQ * S[2] + aI * S[3]));
+  // (every rounding spelt out, as in stokes_congruence: the same bits in every kernel that calls this)
+  double w0 = __dmul_rn(s, __dadd_rn(jI, -fma(aV, S[3], fma(aQ, S[1], __dmul_rn(aI, S[0])))));
+  double w1 = __dmul_rn(s, __dadd_rn(jQ, -fma(rV, S[2], fma(aI, S[1], __dmul_rn(aQ, S[0])))));
+  double w2 = __dmul_rn(s, fma(-rQ, S[3], fma(-aI, S[2], __dmul_rn(rV, S[1]))));
+  double w3 = __dmul_rn(s, __dadd_rn(jV, -fma(aI, S[3], fma(-rQ, S[2], __dmul_rn(aV, S[0])))));
   double o0 = w0, o1 = w1, o2 = w2, o3 = w3;
   // The chain is cut where the first dropped term is below 2e-17 of w_1: three terms for nb < 2^-17, five for
   // nb < 2^-10, seven otherwise.  Most steps of the ADAF workloads are in the lowest tier, and a warp whose lanes
   // all are skips the rest of the chain.
   auto term = [&](int n) {
-    const double c = -s * (1.0 / (double)n);
-    const double t0 = aI * w0 + aQ * w1 + aV * w3;
-    const double t1 = aQ * w0 + aI * w1 + rV * w2;
-    const double t2 = aI * w2 - rV * w1 + rQ * w3;
-    const double t3 = aV * w0 - rQ * w2 + aI * w3;
-    w0 = c * t0; w1 = c * t1; w2 = c * t2; w3 = c * t3;
-    o0 += w0; o1 += w1; o2 += w2; o3 += w3;
+    const double c = __dmul_rn(-s, 1.0 / (double)n);
+    const double t0 = fma(aV, w3, fma(aQ, w1, __dmul_rn(aI, w0)));
+    const double t1 = fma(rV, w2, fma(aI, w1, __dmul_rn(aQ, w0)));
+    const double t2 = fma(rQ, w3, fma(-rV, w1, __dmul_rn(aI, w2)));
+    const double t3 = fma(aI, w3, fma(-rQ, w2, __dmul_rn(aV, w0)));
+    w0 = __dmul_rn(c, t0); w1 = __dmul_rn(c, t1); w2 = __dmul_rn(c, t2); w3 = __dmul_rn(c, t3);
+    o0 = __dadd_rn(o0, w0); o1 = __dadd_rn(o1, w1); o2 = __dadd_rn(o2, w2); o3 = __dadd_rn(o3, w3);
   };
   term(2); term(3);
   if (nb >= 7.62939453125e-06) {          // 2^-17: (2^-17)^3 / 4! = 1.8e-17
     term(4); term(5);
     if (nb >= 9.765625e-4) { term(6); term(7); }   // 2^-10: (2^-10)^5 / 6! = 1.2e-18
   }
-  S[0] += o0; S[1] += o1; S[2] += o2; S[3] += o3;
+  S[0] = __dadd_rn(S[0], o0); S[1] = __dadd_rn(S[1], o1); S[2] = __dadd_rn(S[2], o2); S[3] = __dadd_rn(S[3], o3);
   return true;
 }
 

@@ -417,7 +417,9 @@ def test_grid_plasma_contact_range_is_bit_neutral(ipole, small_grid, monkeypatch
 
 def test_low_latency_geodesic_build_is_bit_neutral(ipole, small_grid, monkeypatch):
     """Launches that cannot fill the GPU use k_geodesic compiled for 2 blocks per SM (kernels.cuh, LOWLAT): the same path
-    records, step counts and images as the 4-block build (IPOLE_NO_LOWLAT=1), for both flows."""
+    records, step counts and images as the 4-block build (IPOLE_NO_LOWLAT=1), for both flows.  The same switch picks the
+    operator walk of the analytic flow: one warp per RAY (k_apply_wide, stepop.cuh) against one warp per 32 rays (k_apply);
+    the two must agree to the bit (every rounding of the Stokes update is spelt out in stokes.cuh / plasma.cuh)."""
     desc, fields = small_grid
     for kind in ("adaf", "grid"):
         cam = W.camera(kind, 96)                       # 9216 rays: every launch is under-filled
