@@ -485,8 +485,10 @@ int launch_transfer_split(ipole_ctx* c, const RtArgs& a, int64_t rays, cudaStrea
     p.edf = c->edf;
     if (c->n_mc) { p.nu3_arr = c->d_mc_nu3; p.rays_per_cam = c->mc_rays_per_cam; }
     if (c->edf.kind != 0) k_apply<true><<<grid_for(c, c->occ_ap_edf, IPOLE_AP_THREADS / 32, (rays + 31) / 32, reserve), IPOLE_AP_THREADS, (size_t)c->edf.n_nodes * sizeof(double4), st>>>(p);
-    else if (c->opt_lowlat && rays <= (int64_t)c->n_sm * IPOLE_AP_THREADS * 2)   // the launch cannot fill the GPU: a warp per ray (stepop.cuh)
-      k_apply_wide<<<grid_for(c, c->occ_ap_wide, IPOLE_AP_THREADS / 32, rays, reserve), IPOLE_AP_THREADS, 0, st>>>(p);
+    else if (c->opt_lowlat && rays <= 1024)      // a handful of rays (long-ray and retry passes): a warp per ray (stepop.cuh)
+      k_apply_wide<32><<<grid_for(c, c->occ_ap_wide, IPOLE_AP_THREADS / 32, rays, reserve), IPOLE_AP_THREADS, 0, st>>>(p);
+    else if (c->opt_lowlat && rays <= (int64_t)c->n_sm * IPOLE_AP_THREADS * 2)   // the launch cannot fill the GPU: 8 lanes per ray
+      k_apply_wide<8><<<grid_for(c, c->occ_ap_wide, IPOLE_AP_THREADS / 32, (rays + 3) / 4, reserve), IPOLE_AP_THREADS, 0, st>>>(p);
     else k_apply<false><<<g, IPOLE_AP_THREADS, 0, st>>>(p);
     span_end(c, s, st);
     c->stats.n_launches++;
@@ -798,7 +800,11 @@ int run_rays(ipole_ctx* c, int64_t n, const int64_t* d_pixels, double* I, double
   const size_t lslot = (size_t)(max_steps + 1) * rec_bytes;
   // eDF coefficients and many ADAF cameras live in the split kernels only: their long rays take k_stepop + k_apply here
   // (operator records in d_ops_long) instead of the single kernel
-  const bool long_split = c->edf.kind != 0 || (c->n_mc > 0 && c->model == MODEL_ADAF);
+  // (and the long rays of a small call -- an adaptive level, a pixel list, a small image -- of the analytic flow: nothing
+  // hides the single kernel's one-lane walk of 50 000 steps there, k_apply_wide is 6x quicker on it)
+  const bool long_split = c->edf.kind != 0 || (c->n_mc > 0 && c->model == MODEL_ADAF) ||
+                          (c->opt_lowlat && c->opt_split == 1 && !sw && !c->opt_unpol && c->model == MODEL_ADAF && n <= (int64_t)c->n_sm * IPOLE_AP_THREADS * 4 &&
+                           budget / 4 >= 128 * lslot);      // (room for 64 long rays with both records per pass)
   int long_done = 0;          // entries of d_long already handed to the side stream
   int64_t LBcap = 0;          // rays that fit the long path buffer
   const int32_t* long_src = replay ? pc.d_long : c->d_long;       // replay: the list the recorded call ended with
@@ -1176,7 +1182,7 @@ int ipole_init(const ipole_camera* cam, ipole_ctx** out) {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_geo_f32, k_geodesic_f32, IPOLE_GEO_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap, k_apply<false>, IPOLE_AP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_unpol, k_apply_unpol_sweep, IPOLE_AP_THREADS, 0);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_wide, k_apply_wide, IPOLE_AP_THREADS, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_wide, k_apply_wide<8>, IPOLE_AP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_gridop, k_gridop, IPOLE_RT_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_gridapply, k_gridapply_sweep, IPOLE_AP_THREADS, 0);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_ap_edf, k_apply<true>, IPOLE_AP_THREADS, EDF_MAX_NODES * sizeof(double4));

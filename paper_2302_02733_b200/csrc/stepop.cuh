@@ -369,32 +369,53 @@ __global__ void __launch_bounds__(IPOLE_AP_THREADS, EDF ? IPOLE_AP_EDF_MINB : IP
 }
 
 // k_apply for launches that cannot fill the GPU (adaptive levels, retry and long-ray passes, pixel lists, small images):
-// ONE WARP PER RAY.  The lockstep kernel above gives every ray one lane, and a lone photon-ring ray of 4 500 steps is then
-// 4 500 x ~700 dependent instructions = 9 ms however empty the GPU is.  Here the 32 lanes take 32 consecutive steps of the
-// ray and evaluate their scalars and coefficients side by side (they do not depend on the Stokes numbers); only the
-// congruence and the 4x4 step run in sequence, every lane doing the same update on values broadcast from the lane that
-// owns the step.  Per ray the arithmetic and its order are k_apply's (same functions, same operands).
+// LANES LANES PER RAY instead of one.  The lockstep kernel above gives every ray one lane, and a lone photon-ring ray of
+// 4 500 steps is then 4 500 x ~560 dependent instructions = 9 ms however empty the GPU is.  Here the LANES lanes of a ray
+// take LANES consecutive steps and evaluate their scalars and coefficients side by side (they do not depend on the Stokes
+// numbers); only the congruence and the 4x4 step run in sequence, every lane of the ray doing the same update on values
+// broadcast from the lane that owns the step.  Per ray the arithmetic and its order are k_apply's (same functions, same
+// operands, every rounding spelt out): the same bits.  Dependent instructions per step: (480 + 80 LANES) / LANES -- 95 at
+// 32 lanes, 140 at 8; warp instructions per ray step: 15 + 80 LANES / 32 -- 95 at 32 lanes, 35 at 8 (k_apply: 17.5).  So
+// 32 lanes for a handful of rays, 8 for a few thousand.
+template <int LANES>
 __global__ void __launch_bounds__(IPOLE_AP_THREADS, IPOLE_AP_MINB) k_apply_wide(const __grid_constant__ ApArgs A) {
+  constexpr int RPW = 32 / LANES;                // rays per warp
   const int lane = threadIdx.x & 31;
+  const int sub = lane / LANES, sl = lane % LANES;
   const int64_t count = A.count_dev ? (int64_t)*A.count_dev : A.count;
+  const int64_t n_items = (count + RPW - 1) / RPW;
   for (;;) {
     __syncwarp();
-    long long li = 0;                            // place in the batch's operator buffer
-    if (lane == 0) li = (long long)atomicAdd(A.queue, 1ULL);
-    li = __shfl_sync(0xffffffffu, li, 0);
-    if (li >= count) break;
-    const int64_t ls = A.slot ? (int64_t)A.slot[A.base + li] : li;
-    const int32_t q = A.order ? A.order[A.base + ls] : (int32_t)(A.base + ls);
-    int n = A.nsteps[q];
-    if (n < 0) continue;                         // overflowed its slot: long-ray pass
-    double mc[4], flag, z0, z1, z2;
-    ld_global_v4(A.ops + op_addr(li, A.cap, n, 0), mc[0], mc[1], mc[2], mc[3]);
-    ld_global_v4(A.ops + op_addr(li, A.cap, n, 1), flag, z0, z1, z2);
-    if (flag != 0.0) continue;                   // irregular: rendered by k_transfer
+    long long g = 0;
+    if (lane == 0) g = (long long)atomicAdd(A.queue, 1ULL);
+    g = __shfl_sync(0xffffffffu, g, 0);
+    if (g >= n_items) break;
+    const int64_t li = g * RPW + sub;            // place in the batch's operator buffer
+    int32_t q = 0;
+    int n = 0;                                   // steps of this ray; 0: nothing to do
+    double mc[4] = {0, 0, 0, 0};
+    if (li < count) {
+      const int64_t ls = A.slot ? (int64_t)A.slot[A.base + li] : li;
+      q = A.order ? A.order[A.base + ls] : (int32_t)(A.base + ls);
+      n = A.nsteps[q];
+      if (n < 0) n = 0;                          // overflowed its slot: long-ray pass
+      else {
+        double flag, z0, z1, z2;
+        ld_global_v4(A.ops + op_addr(li, A.cap, n, 0), mc[0], mc[1], mc[2], mc[3]);
+        ld_global_v4(A.ops + op_addr(li, A.cap, n, 1), flag, z0, z1, z2);
+        if (flag != 0.0) n = 0;                  // irregular: rendered by k_transfer
+      }
+    }
+    int nmax = n;
+    if (RPW > 1) {
+#pragma unroll
+      for (int o = 16; o >= LANES; o >>= 1) nmax = max(nmax, __shfl_xor_sync(0xffffffffu, nmax, o));
+    }
     double S[4] = {0, 0, 0, 0}, tau = 0.0, tauF = 0.0;
-    const double* base = A.ops + op_addr(li, A.cap, 0, 0);
-    for (int s_top = n - 1; s_top >= 0; s_top -= 32) {
-      const int s = s_top - lane;                // this lane's step of the chunk (the chunk is walked from lane 0 on)
+    const double* base = A.ops + op_addr(li < count ? li : 0, A.cap, 0, 0);
+    for (int done = 0; done < nmax; done += LANES) {
+      const int s_top = n - 1 - done;            // the ray's chunk is walked from its lane 0 on; < 0: the ray is through
+      const int s = s_top - sl;
       double v[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
       if (s >= 0) {
         const double* p = base + (size_t)s * (OP_PARTS * 128);
@@ -407,22 +428,29 @@ __global__ void __launch_bounds__(IPOLE_AP_THREADS, IPOLE_AP_MINB) k_apply_wide(
         v[4] = __dmul_rn(c.aI, ds); v[5] = __dmul_rn(c.aQ, ds); v[6] = __dmul_rn(c.aV, ds); v[7] = __dmul_rn(c.rQ, ds); v[8] = __dmul_rn(c.rV, ds);
         v[9] = __dmul_rn(c.jI, ds); v[10] = __dmul_rn(c.jQ, ds); v[11] = __dmul_rn(c.jV, ds);
       }
-      const int m = min(32, s_top + 1);
-      for (int j = 0; j < m; ++j) {
+      const int m = min(LANES, s_top + 1);
+      int mmax = m;
+      if (RPW > 1) {
+#pragma unroll
+        for (int o = 16; o >= LANES; o >>= 1) mmax = max(mmax, __shfl_xor_sync(0xffffffffu, mmax, o));
+      }
+      for (int j = 0; j < mmax; ++j) {
         double w[12];
 #pragma unroll
-        for (int i = 0; i < 12; ++i) w[i] = __shfl_sync(0xffffffffu, v[i], j);
-        stokes_congruence(w[0], w[1], w[2], w[3], S);
-        if (IP_UNLIKELY(!stokes_step_qv_series(w[4], w[5], w[6], w[7], w[8], 1.0, w[9], w[10], w[11], S))) {
-          const Stokes4 in = {S[0], S[1], S[2], S[3]};
-          const Stokes4 o = stokes_step_qv_closed(w[4], w[5], w[6], w[7], w[8], w[9], w[10], w[11], in);
-          S[0] = o.I; S[1] = o.Q; S[2] = o.U; S[3] = o.V;
+        for (int i = 0; i < 12; ++i) w[i] = __shfl_sync(0xffffffffu, v[i], j, LANES);
+        if (j < m) {
+          stokes_congruence(w[0], w[1], w[2], w[3], S);
+          if (IP_UNLIKELY(!stokes_step_qv_series(w[4], w[5], w[6], w[7], w[8], 1.0, w[9], w[10], w[11], S))) {
+            const Stokes4 in = {S[0], S[1], S[2], S[3]};
+            const Stokes4 o = stokes_step_qv_closed(w[4], w[5], w[6], w[7], w[8], w[9], w[10], w[11], in);
+            S[0] = o.I; S[1] = o.Q; S[2] = o.U; S[3] = o.V;
+          }
+          tau = __dadd_rn(tau, w[4]);
+          tauF = __dadd_rn(tauF, fabs(w[8]));
         }
-        tau = __dadd_rn(tau, w[4]);
-        tauF = __dadd_rn(tauF, fabs(w[8]));
       }
     }
-    if (lane == 0) {
+    if (n > 0 && sl == 0) {
       stokes_congruence(mc[0], mc[1], mc[2], mc[3], S);
       const double nu3 = A.nu3_arr ? A.nu3_arr[q / A.rays_per_cam] : A.nu3;
       A.I[q] = S[0] * nu3; A.Q[q] = S[1] * nu3; A.U[q] = S[2] * nu3; A.V[q] = S[3] * nu3;
