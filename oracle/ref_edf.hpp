@@ -34,8 +34,7 @@
 //   K_nu(x) = int_0^inf exp(-x cosh t) cosh(nu t) dt,   int_x^inf K_nu = int_0^inf exp(-x cosh t) cosh(nu t) / cosh t dt .
 // Pins (tests/test_oracle_edf.py): F, G, H against mpmath/scipy; kind 1 against the thermal fits and Kirchhoff's law;
 // kind 2 -> kind 1 for kappa -> infinity and the Rybicki & Lightman power-law closed forms (6.36, 6.53) in the tail;
-// distance of the rule from adaptive quadrature.  Parity unpinned: j_V, alpha_V of the kappa distribution (no independent
-// closed form at hand).
+// distance of the rule from adaptive quadrature; j_V, alpha_V of the kappa tail against the Mellin transform of H (E6).
 #pragma once
 #include <cmath>
 #include "ref_coeff.hpp"

@@ -1,9 +1,10 @@
-"""Pins E1-E5 of the oracle's numerically integrated eDF coefficients (oracle/ref_edf.hpp; reading R-13).
+"""Pins E1-E6 of the oracle's numerically integrated eDF coefficients (oracle/ref_edf.hpp; reading R-13).
 
 References outside the oracle: scipy's K_nu and adaptive quadrature for the kernels F, G, H; the published thermal fits
 and Kirchhoff's law (Rayleigh-Jeans) for the Maxwell-Juettner case; the Rybicki & Lightman power-law closed forms
 (6.36 emission, 6.53 absorption) for the tail of the kappa distribution; scipy quadrature of the same integrands with an
-independent rule for the convergence of the midpoint rule."""
+independent rule for the convergence of the midpoint rule; Mellin transforms of the kernel H (Gamma functions) for j_V and
+alpha_V of the power-law tail."""
 import numpy as np
 import pytest
 from scipy import integrate, special
@@ -99,6 +100,55 @@ def test_E4_kappa_tail_matches_the_power_law_closed_forms(ref):
         # linear-polarization fraction of a power law: (p + 1) / (p + 7/3)
         assert c[1] / c[0] == pytest.approx((p + 1) / (p + 7.0 / 3.0), rel=0.03)
     assert abs(prev[0]) < 0.025 and abs(prev[1]) < 0.03
+
+
+def _mellin_H(s):
+    """int_0^inf x^(s-1) H(x) dx for H(x) = x K_1/3(x) + int_x^inf K_1/3, from int_0^inf x^(mu-1) K_nu = 2^(mu-2) Gamma((mu-nu)/2)
+    Gamma((mu+nu)/2) (Gradshteyn & Ryzhik 6.561.16) and one integration by parts for the tail term."""
+    from scipy.special import gamma as Gm
+    return 2.0 ** (s - 1.0) * (1.0 + 1.0 / s) * Gm(0.5 * s + 1.0 / 3.0) * Gm(0.5 * s + 2.0 / 3.0)
+
+
+def test_E6_kappa_tail_circular_coefficients_match_the_power_law_closed_forms(ref):
+    """j_V and alpha_V of the kappa distribution where the tail n -> K gamma^-p emits: with x = nu/nu_c(gamma) the gamma
+    integrals become Mellin transforms of H,
+      j_V     = C (4 cot th / 3) K (1/2) xs^(-p/2)     M_H(p/2),
+      alpha_V = C/(2 m_e nu^2) (4 cot th / 3) K (p+2) (1/2) xs^(-(p+1)/2) M_H((p+1)/2),      xs = nu / (1.5 nu_B sin th),
+    products of Gamma functions -- no quadrature of the oracle's enters (the Mellin transform itself is checked here against
+    scipy quadrature of the mpmath kernel)."""
+    K13 = lambda t: special.kv(1.0 / 3.0, t)
+    def Hq(x):      # (the tail in u = ln t below 1: K_1/3 ~ t^-1/3 there)
+        lo = integrate.quad(lambda u: K13(np.exp(u)) * np.exp(u), np.log(x), 0.0, epsabs=0, epsrel=1e-10)[0] if x < 1.0 else 0.0
+        return x * K13(x) + lo + integrate.quad(K13, max(x, 1.0), np.inf, epsabs=0, epsrel=1e-10)[0]
+    assert Hq(0.29) == pytest.approx(_H(0.29), rel=1e-8)
+    for s in (1.25, 1.75):
+        num = integrate.quad(lambda u: np.exp(u * s) * Hq(np.exp(u)), np.log(1e-9), np.log(80.0), limit=200, epsabs=0, epsrel=1e-8)[0]
+        assert num == pytest.approx(_mellin_H(s), rel=1e-6)
+    kappa, w, ne, B, th = 3.5, 3.0, 1.0e4, 0.5, 1.2
+    p = kappa - 1.0
+    nuB = EE * B / (2 * np.pi * ME * CL)
+    nrm = integrate.quad(lambda g: g * np.sqrt(g * g - 1) * (1 + (g - 1) / (kappa * w)) ** -(kappa + 1), 1, np.inf, limit=400)[0]
+    Kpl = ne / nrm * (kappa * w) ** (kappa + 1)
+    C = np.sqrt(3) * EE ** 3 * B * np.sin(th) / (4 * np.pi * ME * CL ** 2)
+    cot43 = 4.0 / (3.0 * np.tan(th))
+    prev = None
+    for gstar in (1e3, 3e3):
+        nu = 1.5 * gstar ** 2 * nuB * np.sin(th)
+        xs = nu / (1.5 * nuB * np.sin(th))
+        c = ref.coefficients_edf(2, ne, w, B, np.cos(th), nu, kappa=kappa, n_nodes=400)
+        jV = C * cot43 * Kpl * 0.5 * xs ** (-p / 2) * _mellin_H(p / 2)
+        aV = C / (2 * ME * nu * nu) * cot43 * Kpl * (p + 2) * 0.5 * xs ** (-(p + 1) / 2) * _mellin_H((p + 1) / 2)
+        dj, da = c[2] / jV - 1, c[5] / aV - 1
+        assert abs(dj) < 0.08 and abs(da) < 0.08, (dj, da)
+        if prev is not None:
+            assert abs(dj) < 0.45 * abs(prev[0]) and abs(da) < 0.45 * abs(prev[1])
+        prev = (dj, da)
+        # circular over total emission of a power law falls like 1/gamma*: j_V / j_I ~ cot th / gamma*
+        assert 0.3 < (c[2] / c[0]) * gstar * np.tan(th) < 3.0
+    assert abs(prev[0]) < 0.03 and abs(prev[1]) < 0.03
+    # the sign follows cos th (the handedness of the gyration seen from the two sides of the field)
+    cm = ref.coefficients_edf(2, ne, w, B, -np.cos(th), nu, kappa=kappa, n_nodes=400)
+    assert cm[2] == pytest.approx(-c[2], rel=1e-12) and cm[5] == pytest.approx(-c[5], rel=1e-12)
 
 
 def test_E5_midpoint_rule_converges_to_adaptive_quadrature(ref):
