@@ -32,7 +32,7 @@ FLOP_PER_STEP = {"transfer_adaf": 1576.0, "transfer_grid": 390.0, "geodesic_adaf
 # launch of a run / the steps of the run (profiles/r2_image_flops.md, made by --summarize-launches); and their FP64-pipe
 # utilisation (sm__inst_executed_pipe_fp64) in a bulk launch of the ncu --set full captures profiles/r2_k_*.txt.
 # k_transfer<adaf> (single kernel, --single-kernel) and the path-free / unpolarized variants: profiles/r1_k_*.txt.
-FLOP_EXECUTED = {"k_stepop": 1019.0, "k_apply": 578.0, "k_transfer<adaf>": 1576.0, "k_transfer_group<grid>": 397.0,
+FLOP_EXECUTED = {"k_stepop": 1019.0, "k_apply": 585.0, "k_transfer<adaf>": 1576.0, "k_transfer_group<grid>": 397.0,
                  "k_geodesic": 839.0, "k_geodesic<occ>": 1020.0}
 # second physics workload (--edf): k_apply<true> per step, 128 quadrature nodes (profiles/r2_k_apply_edf{1,2}_adaf256.txt)
 FLOP_EXECUTED.update({"k_apply<edf 1>": 11558.0, "k_apply<edf 2>": 18290.0})
