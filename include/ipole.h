@@ -338,7 +338,8 @@ int  ipole_eval_plasma(ipole_ctx*, int64_t n, const double* X, double* out12);
  * denominator: returns achieved TFLOP/s in *tflops and the kernel time in *ms. */
 int  ipole_measure_fp64_peak(ipole_ctx*, double* tflops, float* ms);
 
-int  ipole_last_cuda_error(const ipole_ctx*);  /* cudaError_t of the last failed CUDA call, 0 if none */
+int  ipole_last_cuda_error(const ipole_ctx*);  /* cudaError_t of the last failed CUDA call, 0 if none;
+                                                * IPOLE_DEBUG=1 in the environment: its source line and text go to stderr */
 void ipole_free(ipole_ctx*);
 const char* ipole_strerror(int code);
 const char* ipole_version(void);

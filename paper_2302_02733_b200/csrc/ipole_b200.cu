@@ -138,10 +138,16 @@ struct ipole_ctx {
 
 namespace {
 
+// IPOLE_DEBUG=1 in the environment: the failing call's line and CUDA's text for the error go to stderr
+static void report_cuda_failure(int e, int line) {
+  static const bool on = [] { const char* v = std::getenv("IPOLE_DEBUG"); return v && v[0] == '1'; }();
+  if (on) std::fprintf(stderr, "ipole: CUDA error %d (%s) at ipole_b200.cu:%d\n", e, cudaGetErrorString((cudaError_t)e), line);
+}
+
 #define CK(call)                                                        \
   do {                                                                  \
     cudaError_t e_ = (call);                                            \
-    if (e_ != cudaSuccess) { c->last_cuda = (int)e_; return IPOLE_ECUDA; } \
+    if (e_ != cudaSuccess) { c->last_cuda = (int)e_; report_cuda_failure((int)e_, __LINE__); return IPOLE_ECUDA; } \
   } while (0)
 
 bool is_device_ptr(const void* p) {
@@ -241,7 +247,7 @@ int ensure_ops(ipole_ctx* c, size_t bytes) {
 
 int ensure_retry_buf(ipole_ctx* c, size_t bytes) {
   if (bytes <= c->retry_buf_bytes) return IPOLE_OK;
-  cudaFree(c->d_retry_buf); cudaFree(c->d_ops_long); cudaFree(c->plan_cache.d_long); cudaFree(c->plan_cache.d_retry); c->d_retry_buf = nullptr; c->retry_buf_bytes = 0;
+  cudaFree(c->d_retry_buf); c->d_retry_buf = nullptr; c->retry_buf_bytes = 0;
   cudaError_t e = cudaMalloc(&c->d_retry_buf, bytes);
   if (e != cudaSuccess) { c->last_cuda = (int)e; cudaGetLastError(); return IPOLE_ENOMEM; }
   c->retry_buf_bytes = bytes;
@@ -301,6 +307,7 @@ int grid_for(ipole_ctx* c, int occ, int threads, int64_t rays, int reserve = 0) 
 }
 
 int launch_geodesic(ipole_ctx* c, GeoArgs& a, int kind, int64_t rays, cudaStream_t st, int reserve = 0) {
+  CK(cudaGetLastError());     // (an error left behind by an unchecked call is reported here, not as this launch's)
   const int s = span_begin(c, kind, st);
   if (c->opt_geo_fp32 && kind != LK_PROBE && !c->n_mc && !a.grid && !a.endp) {
     k_geodesic_f32<<<grid_for(c, c->occ_geo_f32, IPOLE_GEO_THREADS, rays, reserve), IPOLE_GEO_THREADS, 0, st>>>(a);
@@ -1898,7 +1905,7 @@ void ipole_free(ipole_ctx* c) {
   if (c->ev_fork) cudaEventDestroy(c->ev_fork);
   if (c->ev_join) cudaEventDestroy(c->ev_join);
   for (int l = 0; l < 2; ++l) if (c->ev_lastgeo[l]) cudaEventDestroy(c->ev_lastgeo[l]);
-  cudaFree(c->d_retry_buf);
+  cudaFree(c->d_retry_buf); cudaFree(c->d_ops_long); cudaFree(c->plan_cache.d_long); cudaFree(c->plan_cache.d_retry);
   cudaFree(c->d_path_long); cudaFree(c->d_nsteps_long); cudaFree(c->d_occ);
   cudaFree(c->d_cam); cudaFree(c->d_model); cudaFree(c->d_grid); cudaFree(c->d_path);
   cudaFree(c->d_nsteps); cudaFree(c->d_nturn); cudaFree(c->d_order); cudaFree(c->d_key); cudaFree(c->d_long);

@@ -415,6 +415,42 @@ def test_grid_plasma_contact_range_is_bit_neutral(ipole, small_grid, monkeypatch
     assert (base["I"] == 0).any() and (base["I"] > 0).any()   # dark rays (never walked) and lit ones
 
 
+def test_growing_retry_buffer_leaves_the_plan_lists_and_long_operator_records_alone(ipole):
+    """Regression: ensure_retry_buf (the slots of the side-stream retry level) once freed the recorded plan's ray lists and
+    the long-ray operator records when it grew, without forgetting the pointers -- a later call used freed memory and
+    reported cudaErrorInvalidValue (seen as an intermittent failure of 4096^2 adaptive grid images).  Here the buffer is
+    made to grow between images of one context (larger memory budget), with a recorded plan and long rays in play."""
+    cam = W.camera("adaf", 128)
+    g = ipole.Ipole(**cam); g.load_adaf(**W.ADAF)
+    g.set_options(768 << 20, 2)
+    a = to_np(g.make_image(maps=True)); sta = g.stats()
+    b = to_np(g.make_image(maps=True)); stb = g.stats()
+    assert stb["plan_reused"] == 1 and sta["n_batches"] >= 3 and sta["n_long"] + sta["n_retry"] > 0
+    pix = sample_pixels(128, 128, 8)
+    lst0 = g.make_pixels(pix)                            # a small call: its long rays keep operator records (d_ops_long)
+    for budget in (3 << 30, 12 << 30):                   # the retry level's slots grow with the budget
+        g.set_options(budget, 2)
+        c1 = to_np(g.make_image(maps=True)); assert g.stats()["plan_reused"] == 0
+        c2 = to_np(g.make_image(maps=True)); assert g.stats()["plan_reused"] == 1
+        lst = g.make_pixels(pix)
+        for k in a:
+            assert np.array_equal(a[k], c1[k]) and np.array_equal(a[k], c2[k]) and np.array_equal(a[k], b[k]), k
+        for k in ("I", "Q", "U", "V", "tau", "tauF"):
+            assert np.array_equal(lst[k], lst0[k]), k
+    # a larger image on the same context: the recorded lists have to grow (freeing the old ones -- a second time, before the fix)
+    cam2 = W.camera("adaf", 256)
+    g.set_camera(**cam2); g.set_options(1 << 30, 2)
+    d1 = to_np(g.make_image(maps=True)); assert g.stats()["plan_reused"] == 0
+    d2 = to_np(g.make_image(maps=True)); st = g.stats()
+    assert st["plan_reused"] == 1 and st["n_long"] + st["n_retry"] > sta["n_long"] + sta["n_retry"]
+    f = ipole.Ipole(**cam2); f.load_adaf(**W.ADAF); f.set_options(1 << 30, 2)
+    want = to_np(f.make_image(maps=True)); f.close()
+    for k in want:
+        assert np.array_equal(d1[k], want[k]) and np.array_equal(d2[k], want[k]), k
+    assert ipole.lib().ipole_last_cuda_error(g._h) == 0
+    g.close()
+
+
 def test_low_latency_geodesic_build_is_bit_neutral(ipole, small_grid, monkeypatch):
     """Launches that cannot fill the GPU use k_geodesic compiled for 2 blocks per SM (kernels.cuh, LOWLAT): the same path
     records, step counts and images as the 4-block build (IPOLE_NO_LOWLAT=1), for both flows.  The same switch picks the
