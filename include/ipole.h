@@ -117,9 +117,13 @@ int  ipole_init(const ipole_camera* cam, ipole_ctx** out);
 int  ipole_set_camera(ipole_ctx*, const ipole_camera* cam);
 /* cuda_stream is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = legacy stream. */
 int  ipole_set_stream(ipole_ctx*, void* cuda_stream);
-/* Tunables: path_bytes = size of the geodesic path buffer in HBM (0 => 40% of free memory, at most
- * 64 GiB); sort_rays: 0 = pixel order, 1 = order rays by predicted step count, longest first, when the image
- * has >= 32768 rays (default), 2 = always run the probe pass and sort (tests). */
+/* Tunables: path_bytes = memory for the stored paths (and operator records) of a batch in HBM (0 => 50% of free
+ * memory, at most 96 GiB); sort_rays: 0 = pixel order, 1 = order rays by predicted step count, longest first, when the
+ * image has >= 32768 rays (default), 2 = always run the probe pass and sort (tests).
+ * A budget far too small for the call makes the slots shorter than most rays, every ray then takes the long-ray pass a
+ * few at a time, and a call that would need more than 8192 kernel work queues that way (e.g. a 128^2 eDF image with
+ * 128 MiB) returns IPOLE_EINVAL without rendering: give it room for at least a few hundred full-length slots
+ * ((max_steps + 1) x 128 B each). */
 int  ipole_set_options(ipole_ctx*, uint64_t path_bytes, int32_t sort_rays);
 /* Path-free bidirectional variant, the paper's own GPU design (section 2.2: "The GPU code does this
  * integration in both directions, away from the observer ... and toward the observer ..., without saving the path in
